@@ -1,0 +1,115 @@
+/* pm.h — C ABI of libpm: construction of the sparse particle-permutation matrix P0 of the Faddeev
+ * equation in the three-body lattice (free wave-packet) basis on one NVIDIA B200 (sm_100a).
+ *
+ * What is computed (arXiv:1508.07441; line numbers refer to PAPER.md):
+ *   [P0]_{ij alpha, i'j' alpha'} = <X_ij^alpha | P | X_i'j'^alpha'>,  P = P12 P23 + P13 P23   (eq. 18;
+ *   eq. 20-21), an integral of the partial-wave kernel  sum g * I  (eq. 22) over the
+ *   lattice cells D_ij = D_i x Dbar_j (L154), stored in CSR (arrays B, C, W of L339).
+ *   Evaluation scheme (BASELINE.json north_star; written out in DESIGN.md sec. 3): a tensor Gauss-Legendre rule
+ *   in (p, q, x = cos(p^,q^)) inside every source cell; each node is mapped by
+ *       p'^2 = p^2/4 + 9 q^2/16 + (3/4) p q x ,   q'^2 = p^2 + q^2/4 - p q x ,
+ *   located in its target cell (half-open cells [e_k, e_k+1)), and contributes
+ *       w * p q/(p' q') * G_{alpha alpha'}(p,q,x) / sqrt(d_i dbar_j d_i' dbar_j').
+ *
+ * Index convention (part of the contract — the pattern is compared bit-exactly with the oracle):
+ *   source cell  cell = i*Nq + j ; row  r = cell*n_ch + alpha ; column c = cell'*n_ch + alpha' ; 0-based ;
+ *   columns ascending within a row ; rowptr is standard CSR (int64), colidx int32, values double.
+ *   A row (cell, alpha) holds, for every hit cell in ascending order, every alpha' coupled to alpha in ascending
+ *   order: the pattern is structural (hit cells x integer channel mask), never thresholded by value.
+ *
+ * Memory: pointers named d_* are DEVICE pointers on the current CUDA device, h_* / unprefixed are HOST pointers.
+ * The library owns only the handle and its small device tables; every output buffer belongs to the caller and is
+ * never freed or reallocated here.  All entry points return a status code; none throws or aborts.  There is no
+ * CPU fallback: without a usable sm_100 device the compute calls return PM_ERR_DEVICE.
+ * Kernels are launched on the caller's stream (`cuda_stream` is a cudaStream_t cast to void*; NULL = default
+ * stream) and are asynchronous, except that a call which returns a host scalar (nnz) synchronises that stream.
+ */
+#ifndef PM_H_
+#define PM_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pm_lattice pm_lattice;                        /* opaque, owned by the library */
+
+/* A spin-angular channel alpha = {(l s) j t ; (lam 1/2) I} ('Gamma alpha beta').
+ * I2 = 2*I.  Spinless bosons: s = t = 0, j = l, I2 = 2*lam. */
+typedef struct { int32_t l, s, j, t, lam, I2; } pm_channel;
+
+enum {
+    PM_OK = 0, PM_ERR_ARG = -1, PM_ERR_GRID = -2, PM_ERR_CHANNEL = -3, PM_ERR_ORDER = -4, PM_ERR_CUDA = -5,
+    PM_ERR_NOMEM = -6, PM_ERR_STATE = -7, PM_ERR_OVERFLOW = -8, PM_ERR_DEVICE = -9
+};
+enum { PM_FERMION_ISOSPIN = 0, PM_SPINLESS_BOSON = 1 };      /* `statistics` */
+enum { PM_MAX_CHANNELS = 64, PM_MAX_ORDER = 64, PM_MAX_L = 8 };
+
+/* Create a lattice (host work only: validation, Gauss-Legendre rules, recoupling tables — PAPER.md:L247-256
+ * step 1, 'calculation of algebraic coefficients g').
+ *   p_edges[Np+1], q_edges[Nq+1] : host, finite, strictly increasing, first edge >= 0   (cells D_i, Dbar_j, L146)
+ *   ch[n_ch]                     : host, 1 <= n_ch <= PM_MAX_CHANNELS, distinct, each consistent with
+ *                                  (J2 = 2J, parity = +-1, T2 = 2T) and, for fermions, (-1)^(l+s+t) = -1
+ *   n_p, n_q, n_x                : Gauss-Legendre orders in p, q, x, each 1..PM_MAX_ORDER; n_p*n_q*n_x <= 16384; Np*Nq <= 262144
+ * Errors: PM_ERR_ARG (null pointers), PM_ERR_GRID, PM_ERR_CHANNEL, PM_ERR_ORDER, PM_ERR_OVERFLOW (M >= 2^31). */
+int32_t pm_lattice_create(const double* p_edges, int32_t Np, const double* q_edges, int32_t Nq,
+                          const pm_channel* ch, int32_t n_ch,
+                          int32_t J2, int32_t parity, int32_t T2, int32_t statistics,
+                          int32_t n_p, int32_t n_q, int32_t n_x, pm_lattice** out);
+int32_t pm_lattice_destroy(pm_lattice* lat);
+
+/* M = n_ch*Np*Nq (matrix dimension) and the number of lattice cells. */
+int32_t pm_lattice_dims(const pm_lattice* lat, int64_t* M, int32_t* n_cells);
+
+/* Read / replace the quadrature rule of one axis (0 = p, 1 = q, 2 = x) on [-1,1].  `nodes`, `weights`: host,
+ * length = that axis' order.  set_rule lets a caller feed the very arrays it gives to another implementation
+ * (reading R12); nodes must be strictly increasing inside (-1,1); the x-rule must be symmetric. */
+int32_t pm_lattice_rule(const pm_lattice* lat, int32_t axis, double* nodes, double* weights);
+int32_t pm_lattice_set_rule(pm_lattice* lat, int32_t axis, const double* nodes, const double* weights);
+
+/* Channel tables (host out): coupled[n_ch*n_ch] (1 iff the integer selection rules couple alpha, alpha');
+ * *n_functions = number of distinct orbital functions A^L_{l lam, l' lam'} the fill evaluates per node. */
+int32_t pm_lattice_coupling(const pm_lattice* lat, uint8_t* coupled, int32_t* n_functions);
+
+/* Pattern pass (the paper's step 2a 'pre-selection') for the rows of source cells
+ * [cell_begin, cell_end):
+ *   d_rowptr : device, (cell_end-cell_begin)*n_ch + 1 int64, block-local (d_rowptr[0] = 0)
+ *   d_colidx : device, nnz int32 GLOBAL column indices — or NULL to count only (d_rowptr is still written)
+ *   colidx_capacity : number of int32 d_colidx can hold (ignored when d_colidx is NULL); if nnz exceeds it
+ *                     nothing is written to d_colidx and PM_ERR_OVERFLOW is returned (*nnz_host is valid)
+ *   nnz_host : host, receives the block's nnz (the stream is synchronised for this)                     */
+int32_t pm_pattern(pm_lattice* lat, int32_t cell_begin, int32_t cell_end,
+                   int64_t* d_rowptr, int32_t* d_colidx, int64_t colidx_capacity,
+                   int64_t* nnz_host, void* cuda_stream);
+
+/* Fill pass (step 2b 'calculation of nonzero elements'): values of the block
+ * whose d_rowptr was produced by pm_pattern for the same [cell_begin, cell_end).  d_vals: device, nnz doubles,
+ * every entry is written exactly once; sums are formed in a fixed order (bitwise reproducible run to run). */
+int32_t pm_fill(pm_lattice* lat, int32_t cell_begin, int32_t cell_end,
+                const int64_t* d_rowptr, double* d_vals, void* cuda_stream);
+
+/* y = A x for a CSR block (convenience check only): n_rows rows, GLOBAL columns. */
+int32_t pm_spmv(pm_lattice* lat, int64_t n_rows, const int64_t* d_rowptr, const int32_t* d_colidx,
+                const double* d_vals, const double* d_x, double* d_y, void* cuda_stream);
+
+/* Whole build with HOST output buffers and row-block streaming: source-cell ranges are
+ * chosen so that one block's CSR (12 B per nonzero) fits `device_budget_bytes` (0 = 3/4 of free device memory);
+ * each block is built on the device and copied to the host arrays.
+ *   pm_build_host_count : *nnz_total and *n_blocks for that budget (pattern counting only)
+ *   pm_build_host       : h_rowptr[M+1] (global CSR), h_colidx[nnz_total], h_vals[nnz_total]  (host; pinned or not) */
+int32_t pm_build_host_count(pm_lattice* lat, int64_t device_budget_bytes, int64_t* nnz_total, int32_t* n_blocks);
+int32_t pm_build_host(pm_lattice* lat, int64_t device_budget_bytes,
+                      int64_t* h_rowptr, int32_t* h_colidx, double* h_vals, int64_t capacity,
+                      int64_t* nnz_total, int32_t* n_blocks);
+
+/* Number of kernels this library has launched so far in the calling process (bench.py `gpu_launches`). */
+int64_t pm_launch_count(void);
+
+/* Thread-local message of the last failing call on this thread; library-owned, never NULL. */
+const char* pm_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PM_H_ */

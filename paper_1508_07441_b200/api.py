@@ -1,0 +1,229 @@
+"""Thin Python binding of libpm (include/pm.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of libpm.so; this module turns numpy arrays and
+torch CUDA tensors into raw pointers and back.  torch is used for device memory, pinned host memory
+and streams only.  There is no CPU fallback: a missing libpm.so or a failing call raises.
+
+Function names mirror the C ABI: pm_lattice_create, pm_pattern, pm_fill, pm_spmv, pm_build_host.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libpm.so")
+_lib = None
+
+PM_OK = 0
+ERRORS = {-1: "PM_ERR_ARG", -2: "PM_ERR_GRID", -3: "PM_ERR_CHANNEL", -4: "PM_ERR_ORDER", -5: "PM_ERR_CUDA",
+          -6: "PM_ERR_NOMEM", -7: "PM_ERR_STATE", -8: "PM_ERR_OVERFLOW", -9: "PM_ERR_DEVICE"}
+
+EXPORTS = ["pm_lattice_create", "pm_lattice_destroy", "pm_lattice_dims", "pm_lattice_rule", "pm_lattice_set_rule",
+           "pm_lattice_coupling", "pm_pattern", "pm_fill", "pm_spmv", "pm_build_host_count", "pm_build_host",
+           "pm_launch_count", "pm_last_error"]
+
+
+class PmError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"{ERRORS.get(code, code)}: {msg}")
+        self.code = code
+
+
+class _Channel(C.Structure):
+    _fields_ = [(k, C.c_int32) for k in ("l", "s", "j", "t", "lam", "I2")]
+
+
+_vp, _dp, _i32p, _i64p = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_int64)
+
+
+def lib():
+    """Load libpm.so (built in-tree by csrc/build.py).  Raises if it is missing: no fallback exists."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(f"{_LIB_PATH} is missing: run `python -m paper_1508_07441_b200.csrc.build` "
+                          "(or __graft_entry__.build()); libpm has no CPU fallback")
+    L = C.CDLL(_LIB_PATH)
+    L.pm_last_error.restype = C.c_char_p
+    L.pm_launch_count.restype = C.c_int64
+    L.pm_lattice_create.argtypes = [_dp, C.c_int32, _dp, C.c_int32, C.POINTER(_Channel), C.c_int32,
+                                    C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
+                                    C.POINTER(_vp)]
+    L.pm_lattice_destroy.argtypes = [_vp]
+    L.pm_lattice_dims.argtypes = [_vp, _i64p, _i32p]
+    L.pm_lattice_rule.argtypes = [_vp, C.c_int32, _dp, _dp]
+    L.pm_lattice_set_rule.argtypes = [_vp, C.c_int32, _dp, _dp]
+    L.pm_lattice_coupling.argtypes = [_vp, C.POINTER(C.c_uint8), _i32p]
+    L.pm_pattern.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, C.c_int64, _i64p, _vp]
+    L.pm_fill.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, _vp]
+    L.pm_spmv.argtypes = [_vp, C.c_int64, _vp, _vp, _vp, _vp, _vp, _vp]
+    L.pm_build_host_count.argtypes = [_vp, C.c_int64, _i64p, _i32p]
+    L.pm_build_host.argtypes = [_vp, C.c_int64, _vp, _vp, _vp, C.c_int64, _i64p, _i32p]
+    for name in EXPORTS:
+        if name not in ("pm_last_error", "pm_launch_count"):
+            getattr(L, name).restype = C.c_int32
+    _lib = L
+    return L
+
+
+def _check(rc):
+    if rc != PM_OK:
+        raise PmError(rc, lib().pm_last_error().decode())
+
+
+def _d(a):
+    return a.ctypes.data_as(_dp)
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+# ------------------------------------------------------------------ C-ABI mirrors
+def pm_lattice_create(p_edges, q_edges, channels, J2, parity, T2, statistics, n_p, n_q, n_x):
+    pe = np.ascontiguousarray(p_edges, dtype=np.float64)
+    qe = np.ascontiguousarray(q_edges, dtype=np.float64)
+    ch = (_Channel * len(channels))(*[_Channel(*(int(c[k]) for k in ("l", "s", "j", "t", "lam", "I2"))) for c in channels])
+    h = _vp()
+    _check(lib().pm_lattice_create(_d(pe), len(pe) - 1, _d(qe), len(qe) - 1, ch, len(channels),
+                                   int(J2), int(parity), int(T2), int(statistics), int(n_p), int(n_q), int(n_x),
+                                   C.byref(h)))
+    return h
+
+
+def pm_lattice_destroy(h):
+    _check(lib().pm_lattice_destroy(h))
+
+
+def pm_lattice_dims(h):
+    M, nc = C.c_int64(), C.c_int32()
+    _check(lib().pm_lattice_dims(h, C.byref(M), C.byref(nc)))
+    return M.value, nc.value
+
+
+def pm_lattice_rule(h, axis, n):
+    t, w = np.empty(n), np.empty(n)
+    _check(lib().pm_lattice_rule(h, axis, _d(t), _d(w)))
+    return t, w
+
+
+def pm_lattice_set_rule(h, axis, nodes, weights):
+    t = np.ascontiguousarray(nodes, dtype=np.float64)
+    w = np.ascontiguousarray(weights, dtype=np.float64)
+    _check(lib().pm_lattice_set_rule(h, axis, _d(t), _d(w)))
+
+
+def pm_lattice_coupling(h, n_ch):
+    m = np.zeros(n_ch * n_ch, dtype=np.uint8)
+    nf = C.c_int32()
+    _check(lib().pm_lattice_coupling(h, m.ctypes.data_as(C.POINTER(C.c_uint8)), C.byref(nf)))
+    return m.reshape(n_ch, n_ch).astype(bool), nf.value
+
+
+def pm_pattern(h, cell_begin, cell_end, d_rowptr, d_colidx=None, stream=None):
+    """d_rowptr: int64 CUDA tensor; d_colidx: int32 CUDA tensor or None (count only).  Returns nnz."""
+    nnz = C.c_int64()
+    _check(lib().pm_pattern(h, cell_begin, cell_end, d_rowptr.data_ptr(),
+                            d_colidx.data_ptr() if d_colidx is not None else None,
+                            d_colidx.numel() if d_colidx is not None else 0, C.byref(nnz), _stream_ptr(stream)))
+    return nnz.value
+
+
+def pm_fill(h, cell_begin, cell_end, d_rowptr, d_vals, stream=None):
+    _check(lib().pm_fill(h, cell_begin, cell_end, d_rowptr.data_ptr(), d_vals.data_ptr(), _stream_ptr(stream)))
+
+
+def pm_spmv(h, d_rowptr, d_colidx, d_vals, d_x, d_y, stream=None):
+    _check(lib().pm_spmv(h, d_rowptr.numel() - 1, d_rowptr.data_ptr(), d_colidx.data_ptr(), d_vals.data_ptr(),
+                         d_x.data_ptr(), d_y.data_ptr(), _stream_ptr(stream)))
+
+
+def pm_build_host_count(h, budget_bytes=0):
+    nnz, nb = C.c_int64(), C.c_int32()
+    _check(lib().pm_build_host_count(h, int(budget_bytes), C.byref(nnz), C.byref(nb)))
+    return nnz.value, nb.value
+
+
+def pm_build_host(h, budget_bytes, h_rowptr, h_colidx, h_vals):
+    """Host outputs: torch CPU tensors (pinned or not) or numpy arrays.  Returns (nnz, n_blocks)."""
+    def ptr(a):
+        return a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
+    cap = h_colidx.numel() if hasattr(h_colidx, "numel") else h_colidx.size
+    nnz, nb = C.c_int64(), C.c_int32()
+    _check(lib().pm_build_host(h, int(budget_bytes), ptr(h_rowptr), ptr(h_colidx), ptr(h_vals), cap,
+                               C.byref(nnz), C.byref(nb)))
+    return nnz.value, nb.value
+
+
+def pm_launch_count():
+    return lib().pm_launch_count()
+
+
+# ------------------------------------------------------------------ convenience wrapper
+class Lattice:
+    """Owns a pm_lattice handle created from a `inputs.Workload`; allocates outputs with torch."""
+
+    def __init__(self, wl, use_workload_rules: bool = True):
+        self.wl = wl
+        self.h = pm_lattice_create(wl.p_edges, wl.q_edges, wl.channels, wl.J2, wl.parity, wl.T2, wl.statistics,
+                                   wl.n_p, wl.n_q, wl.n_x)
+        if use_workload_rules:                      # feed the very arrays the oracle gets (reading R12)
+            for axis, key in enumerate(("p", "q", "x")):
+                pm_lattice_set_rule(self.h, axis, *wl.rules[key])
+        self.M, self.n_cells = pm_lattice_dims(self.h)
+        self.n_ch = wl.n_ch
+
+    def close(self):
+        if self.h is not None:
+            pm_lattice_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def pattern(self, cell_begin=0, cell_end=None, count_only=False, stream=None):
+        import torch
+        cell_end = self.n_cells if cell_end is None else cell_end
+        rowptr = torch.empty((cell_end - cell_begin) * self.n_ch + 1, dtype=torch.int64, device="cuda")
+        nnz = pm_pattern(self.h, cell_begin, cell_end, rowptr, None, stream)
+        if count_only:
+            return rowptr, None, nnz
+        colidx = torch.empty(max(nnz, 1), dtype=torch.int32, device="cuda")[:nnz]
+        pm_pattern(self.h, cell_begin, cell_end, rowptr, colidx, stream)
+        return rowptr, colidx, nnz
+
+    def fill(self, rowptr, nnz, cell_begin=0, cell_end=None, out=None, stream=None):
+        import torch
+        cell_end = self.n_cells if cell_end is None else cell_end
+        vals = out if out is not None else torch.empty(max(nnz, 1), dtype=torch.float64, device="cuda")[:nnz]
+        pm_fill(self.h, cell_begin, cell_end, rowptr, vals, stream)
+        return vals
+
+    def build(self, cell_begin=0, cell_end=None):
+        rowptr, colidx, nnz = self.pattern(cell_begin, cell_end)
+        return rowptr, colidx, self.fill(rowptr, nnz, cell_begin, cell_end)
+
+    def spmv(self, rowptr, colidx, vals, x):
+        import torch
+        y = torch.empty(rowptr.numel() - 1, dtype=torch.float64, device="cuda")
+        pm_spmv(self.h, rowptr, colidx, vals, x, y)
+        return y
+
+    def build_host(self, budget_bytes=0, pinned=True):
+        import torch
+        nnz, _ = pm_build_host_count(self.h, budget_bytes)
+        rowptr = torch.empty(self.M + 1, dtype=torch.int64, pin_memory=pinned)
+        colidx = torch.empty(max(nnz, 1), dtype=torch.int32, pin_memory=pinned)
+        vals = torch.empty(max(nnz, 1), dtype=torch.float64, pin_memory=pinned)
+        nnz, nb = pm_build_host(self.h, budget_bytes, rowptr, colidx, vals)
+        return rowptr, colidx[:nnz], vals[:nnz], nnz, nb

@@ -1,0 +1,31 @@
+// pm_kernels.cuh — launcher declarations of libpm's kernels (definitions in pm_kernels.cu).
+#pragma once
+#include <algorithm>
+#include <atomic>
+#include <cstddef>
+#include <cstdint>
+
+#include "pm_device.cuh"
+
+namespace pm {
+
+constexpr int kThreads = 256;
+constexpr int kMaxFun = 256;        // generic fill: per-lane private accumulators
+constexpr int kMaxSlot = 160;
+constexpr int kMaxY = 45;           // (PM_MAX_L+1)(PM_MAX_L+2)/2
+
+size_t stage_bytes(const DevLattice& L, int threads);
+size_t fill_generic_smem(const DevLattice& L, int hmax);
+int64_t launch_count();
+
+cudaError_t launch_count_hits(const DevLattice& L, int cell_begin, int n_blk, int* hits, cudaStream_t st);
+cudaError_t launch_scan_rows(const DevLattice& L, int n_blk, const int* hits, int64_t* cellbase, int64_t* rowptr,
+                             int64_t* summary, cudaStream_t st);
+cudaError_t launch_emit_cols(const DevLattice& L, int cell_begin, int n_blk, const int64_t* rowptr, int32_t* colidx,
+                             cudaStream_t st);
+cudaError_t launch_fill_generic(const DevLattice& L, int cell_begin, int n_blk, int hmax, const int64_t* rowptr,
+                                double* vals, cudaStream_t st);
+cudaError_t launch_spmv(int64_t n_rows, const int64_t* rowptr, const int32_t* colidx, const double* vals,
+                        const double* x, double* y, cudaStream_t st);
+
+}  // namespace pm

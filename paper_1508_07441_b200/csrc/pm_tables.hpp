@@ -1,0 +1,60 @@
+// pm_tables.hpp — host-side channel / coefficient precompute of libpm (hot-path step a1).
+// PAPER.md:L256 "calculation of algebraic coefficients g ... for recoupling between different spin-angular
+// channels" (step 1), L341 "algebraic coefficients g, values of Legendre polynomials at the nodal points".
+// The formulas are derived in DESIGN.md sec. 3.2.  No code is shared with oracle/.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/pm.h"
+
+namespace pm {
+
+// index of Y_{l m}, m >= 0, in the packed per-direction table
+inline int ylm_index(int l, int m) { return l * (l + 1) / 2 + m; }
+
+// One bipolar harmonic family (l, lam, L).  Only M >= 0 is stored: for coplanar arguments
+// Y^{L,-M} = (-1)^{l+lam-L+M} Y^{L,M}; families with l+lam+L odd have no M = 0 member.
+struct Triple { int l, lam, L, M0, nM, slot0; };
+
+// One distinct orbital function A^L_{l lam, l' lam'}: sum over nM slots of bra[sa0+i]*ket[sb0+i].
+struct OrbFun { int ta, tb, L, sa0, sb0, nM; };
+
+struct Tables {
+    int n_ch = 0, lmax = 0, n_slot = 0, totcoup = 0;
+    std::vector<uint8_t> coupled;          // [n_ch*n_ch]
+    std::vector<int32_t> cl_off, cl;       // coupled lists: cl[cl_off[a] .. cl_off[a+1]) = alpha' ascending
+    std::vector<Triple> tri;
+    std::vector<OrbFun> fun;
+    // ket side: slot s = sum over terms t in [kt_off[s], kt_off[s+1]) of kt_c[t]*Yp[kt_ip[t]]*Yq[kt_iq[t]]
+    std::vector<int32_t> kt_off, kt_ip, kt_iq;
+    std::vector<double> kt_c;
+    // per output o = cl_off[a] + m: P = norm * sum_{t in [ot_off[o], ot_off[o+1])} ot_c[t]*acc[ot_f[t]]
+    std::vector<int32_t> ot_off, ot_f;
+    std::vector<double> ot_c;
+    // bra weights per slot: wM/(2L+1) * <l M lam 0|L M> * sqrt((2 lam+1)/4pi); bra[c][s] = slot_w[s]*Y_{l M}(x_c)
+    std::vector<double> slot_w;
+    std::vector<int32_t> slot_l, slot_M;
+    // normalised Legendre recurrence constants (see pm_ylm.h)
+    std::vector<double> ya, yb, ydiag;
+};
+
+// Algebra (doubled arguments), exposed for host tests through the C ABI indirectly (pm_lattice_coupling).
+double clebsch(int j1, int m1, int j2, int m2, int j3, int m3);
+double sixj(int a, int b, int c, int d, int e, int f);
+double ninej(int a, int b, int c, int d, int e, int f, int g, int h, int i);
+
+// Validates the channel list against (J2, parity, T2, statistics); returns "" or a message.
+std::string validate_channels(const pm_channel* ch, int n_ch, int J2, int parity, int T2, int stat);
+
+// Builds every channel-dependent table.  Returns "" or a message.
+std::string build_tables(const pm_channel* ch, int n_ch, int J2, int T2, int stat, Tables& T);
+
+// Gauss-Legendre rule on [-1,1] by Newton iteration, ascending, exactly symmetric.
+void gauss_legendre(int n, std::vector<double>& t, std::vector<double>& w);
+
+// bra[c*n_slot + s] for the x-rule nodes
+void build_bra(const Tables& T, const std::vector<double>& tx, std::vector<double>& bra);
+
+}  // namespace pm

@@ -1,0 +1,154 @@
+"""GPU parity: libpm (through the C ABI) against the CPU oracle on the same inputs.
+
+Bar (BASELINE.json north_star): rowptr and colidx bit-exact; |dP| <= max(1e-11*|P_ref|, 1e-14*max|P|).
+"""
+import numpy as np
+import pytest
+
+from paper_1508_07441_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+REL, FLOOR = 1e-11, 1e-14
+
+
+@pytest.fixture(scope="module")
+def api():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1508_07441_b200 import api as a
+    a.lib()                                    # fails loudly if libpm.so is missing
+    return a
+
+
+def _assert_values(v_gpu, v_ref, scale=None):
+    scale = np.max(np.abs(v_ref)) if scale is None else scale
+    tol = np.maximum(REL * np.abs(v_ref), FLOOR * scale)
+    bad = np.abs(v_gpu - v_ref) > tol
+    assert not bad.any(), (int(bad.sum()), float(np.max(np.abs(v_gpu - v_ref) / tol)))
+
+
+def _gpu_csr(api, wl, cb=0, ce=None):
+    lat = api.Lattice(wl)
+    rp, ci, v = lat.build(cb, ce)
+    out = rp.cpu().numpy(), ci.cpu().numpy(), v.cpu().numpy()
+    lat.close()
+    return out
+
+
+def _small_cases():
+    g7 = I.tan_grid(7, 1.0)
+    return [
+        I.config(0),
+        I.config(1),
+        I.small_coupled(N=6, jmax=2, orders=(3, 3, 6)),
+        I.small_coupled(N=7, jmax=3, orders=(4, 5, 7)),                   # ragged: odd orders, n_p != n_q
+        I.Workload("boson_dwave", g7, g7, np.concatenate([I.boson_channel(0, 0), I.boson_channel(2, 2)]),
+                   0, +1, 0, I.PM_SPINLESS_BOSON, 5, 5, 9),
+        I.Workload("3N_J3half-", g7, 0.9 * g7, I.enumerate_3n_channels(3, -1, 1, 1), 3, -1, 1, 0, 3, 4, 8),
+        I.Workload("offset_grid", 0.3 + g7, 0.2 + g7, I.swave_3n_channels(), 1, 1, 1, 0, 4, 4, 8),   # p_edges[0] > 0
+    ]
+
+
+@pytest.mark.parametrize("wl", _small_cases(), ids=lambda w: w.name)
+def test_full_parity_small(api, oracle, wl):
+    rp, ci, v = _gpu_csr(api, wl)
+    rpo, cio, vo = oracle.build_csr(wl)
+    assert np.array_equal(rp, rpo)
+    assert np.array_equal(ci, cio)
+    _assert_values(v, vo)
+
+
+def test_block_ranges_and_empty(api, oracle):
+    wl = I.config(1)
+    lat = api.Lattice(wl)
+    rp, ci, nnz = lat.pattern(7, 7)
+    assert nnz == 0 and rp.cpu().tolist() == [0]
+    for cb, ce in ((0, 1), (17, 130), (2499, 2500)):
+        rp, ci, v = lat.build(cb, ce)
+        rpo, cio, vo = oracle.build_csr(wl, cb, ce)
+        assert np.array_equal(rp.cpu().numpy(), rpo) and np.array_equal(ci.cpu().numpy(), cio)
+        _assert_values(v.cpu().numpy(), vo)
+    lat.close()
+
+
+def test_bitwise_reproducible(api):
+    wl = I.small_coupled(N=8, jmax=3, orders=(4, 4, 8))
+    a = _gpu_csr(api, wl)
+    b = _gpu_csr(api, wl)
+    assert all(np.array_equal(x, y) for x, y in zip(a, b))
+
+
+def test_fill_requires_pattern(api):
+    import torch
+    wl = I.config(0)
+    lat = api.Lattice(wl)
+    rp = torch.zeros(wl.M + 1, dtype=torch.int64, device="cuda")
+    v = torch.zeros(10, dtype=torch.float64, device="cuda")
+    with pytest.raises(api.PmError) as e:
+        api.pm_fill(lat.h, 0, wl.n_cells, rp, v)
+    assert e.value.code == -7
+    lat.close()
+
+
+@pytest.mark.parametrize("k", [2, 3, 4])
+def test_full_size_sampled_rows(api, oracle, k):
+    """BASELINE configs[2..4] in the launch configuration bench.py times (whole lattice, one block):
+    the complete pattern of sampled source cells is bit-exact and their values meet the tolerance;
+    global invariants hold for the rest (row lengths, sorted columns, nnz)."""
+    import torch
+    wl = I.config(k)
+    lat = api.Lattice(wl)
+    rp, ci, v = lat.build()
+    rp_h = rp.cpu().numpy()
+    rng = np.random.default_rng(100 + k)
+    cells = sorted(set(rng.integers(0, wl.n_cells, size=5).tolist()) | {0, wl.n_cells - 1, wl.Nq * (wl.Np // 2) + 3})
+    scale = float(v.abs().max())
+    for c in cells:
+        rpo, cio, vo = oracle.build_csr(wl, c, c + 1)
+        r0, r1 = c * wl.n_ch, (c + 1) * wl.n_ch
+        assert np.array_equal(rp_h[r0:r1 + 1] - rp_h[r0], rpo)
+        sl = slice(int(rp_h[r0]), int(rp_h[r1]))
+        assert np.array_equal(ci[sl].cpu().numpy(), cio)
+        _assert_values(v[sl].cpu().numpy(), vo, scale)
+    # pattern counted by the oracle for the whole lattice (cheap: no values)
+    rpo_all, _, _ = oracle.build_csr(wl, values=False)
+    assert np.array_equal(rp_h, rpo_all)
+    # columns strictly ascending within every row, all finite
+    d = ci[1:].to(torch.int64) - ci[:-1].to(torch.int64)
+    row_starts = rp[1:-1]
+    row_starts = row_starts[(row_starts > 0) & (row_starts < ci.numel())]
+    mask = torch.ones_like(d, dtype=torch.bool)
+    mask[row_starts - 1] = False
+    assert bool((d[mask] > 0).all())
+    assert bool(torch.isfinite(v).all())
+    assert int(ci.max()) < wl.M and int(ci.min()) >= 0
+    lat.close()
+
+
+def test_spmv_matches_scipy(api):
+    import scipy.sparse as sp
+    import torch
+    wl = I.config(1)
+    lat = api.Lattice(wl)
+    rp, ci, v = lat.build()
+    x = np.random.default_rng(2024).uniform(-1, 1, wl.M)
+    y = lat.spmv(rp, ci, v, torch.from_numpy(x).cuda()).cpu().numpy()
+    A = sp.csr_matrix((v.cpu().numpy(), ci.cpu().numpy(), rp.cpu().numpy()), shape=(wl.M, wl.M))
+    assert np.max(np.abs(y - A @ x)) < 1e-12 * np.max(np.abs(y))
+    lat.close()
+
+
+@pytest.mark.parametrize("budget_blocks", [1, 3, 17])
+def test_streaming_build_identical(api, oracle, budget_blocks):
+    """Row-block streaming: identical CSR whatever the number of blocks."""
+    wl = I.config(1)
+    lat = api.Lattice(wl)
+    nnz, _ = api.pm_build_host_count(lat.h, 1 << 40)
+    budget = (1 << 40) if budget_blocks == 1 else int(12 * nnz / budget_blocks) + 1
+    rp, ci, v, nnz2, nb = lat.build_host(budget, pinned=(budget_blocks != 3))
+    assert nnz2 == nnz and (nb == 1 if budget_blocks == 1 else budget_blocks <= nb <= budget_blocks + 2)
+    rpo, cio, vo = oracle.build_csr(wl)
+    assert np.array_equal(rp.numpy(), rpo) and np.array_equal(ci.numpy(), cio)
+    _assert_values(v.numpy(), vo)
+    lat.close()

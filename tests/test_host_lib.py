@@ -1,0 +1,133 @@
+"""CPU-only checks of libpm: the C ABI loads, exports every symbol include/pm.h declares, validates its
+inputs, and its host precompute (coupling mask, Gauss-Legendre rules) agrees with the oracle / numpy.
+No compute entry point is exercised here (there is no GPU); they must fail loudly with PM_ERR_DEVICE."""
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_1508_07441_b200 import api, inputs as I
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    from paper_1508_07441_b200.csrc import build
+    build.build()
+
+
+def _create(wl, **over):
+    kw = dict(p_edges=wl.p_edges, q_edges=wl.q_edges, channels=wl.channels, J2=wl.J2, parity=wl.parity, T2=wl.T2,
+              statistics=wl.statistics, n_p=wl.n_p, n_q=wl.n_q, n_x=wl.n_x)
+    kw.update(over)
+    return api.pm_lattice_create(**kw)
+
+
+def test_every_declared_symbol_is_exported():
+    hdr = open(os.path.join(ROOT, "include", "pm.h")).read()
+    declared = set(re.findall(r"\b(pm_[a-z_]+)\s*\(", hdr))
+    assert declared == set(api.EXPORTS)
+    L = api.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+
+
+def test_dims_and_coupling_match_oracle(oracle):
+    for k in range(5):
+        wl = I.config(k)
+        h = _create(wl)
+        assert api.pm_lattice_dims(h) == (wl.M, wl.n_cells)
+        mask, nfun = api.pm_lattice_coupling(h, wl.n_ch)
+        ref = np.array([[oracle.coupled(a, b, wl.J2, wl.statistics) for b in wl.channels] for a in wl.channels])
+        assert np.array_equal(mask, ref)
+        assert nfun == [1, 1, 73, 140, 140][k]       # 74 / 141 of SURVEY.md minus one whose c^L cancels exactly
+        api.pm_lattice_destroy(h)
+
+
+def test_library_gauss_legendre_vs_numpy():
+    wl = I.config(0)
+    for n in (1, 2, 5, 10, 32, 64):
+        h = _create(wl, n_p=1, n_q=2, n_x=n)
+        t, w = api.pm_lattice_rule(h, 2, n)
+        tr, wr = np.polynomial.legendre.leggauss(n)
+        assert np.max(np.abs(t - tr)) < 2e-15 and np.max(np.abs(w - wr)) < 1e-14
+        assert np.all(t == -t[::-1])
+        api.pm_lattice_destroy(h)
+
+
+def test_set_rule_validation():
+    wl = I.config(0)
+    h = _create(wl)
+    t, w = wl.rules["x"]
+    api.pm_lattice_set_rule(h, 2, t, w)
+    with pytest.raises(api.PmError) as e:
+        api.pm_lattice_set_rule(h, 2, t + 0.01, w)          # asymmetric x-rule
+    assert e.value.code == -4
+    with pytest.raises(api.PmError):
+        api.pm_lattice_set_rule(h, 0, t[::-1].copy()[: wl.n_p], w[: wl.n_p])   # decreasing nodes
+    api.pm_lattice_destroy(h)
+
+
+@pytest.mark.parametrize("over,code", [
+    (dict(p_edges=np.array([0.0, 1.0, 1.0, 2.0])), -2),
+    (dict(p_edges=np.array([-0.1, 1.0, 2.0])), -2),
+    (dict(q_edges=np.array([0.0, np.nan, 2.0])), -2),
+    (dict(n_x=0), -4),
+    (dict(n_p=65), -4),
+    (dict(n_p=64, n_q=64, n_x=64), -4),
+    (dict(parity=-1), -3),
+    (dict(channels=np.array([(0, 0, 0, 0, 0, 1)], dtype=I.CH_DTYPE)), -3),       # Pauli-forbidden
+    (dict(channels=np.array([(0, 1, 1, 0, 0, 1), (0, 1, 1, 0, 0, 1)], dtype=I.CH_DTYPE)), -3),   # duplicate
+    (dict(channels=np.array([(0, 1, 1, 0, 2, 3)], dtype=I.CH_DTYPE), J2=7), -3),  # triangle (j I J)
+    (dict(statistics=7), -3),
+])
+def test_create_rejects_bad_input(over, code):
+    wl = I.config(1)
+    with pytest.raises(api.PmError) as e:
+        _create(wl, **over)
+    assert e.value.code == code
+    assert str(e.value)
+
+
+def test_lattice_size_limit():
+    g, g2 = I.tan_grid(512, 1.0), I.tan_grid(513, 1.0)
+    with pytest.raises(api.PmError) as e:
+        api.pm_lattice_create(g2, g, I.boson_channel(), 0, 1, 0, I.PM_SPINLESS_BOSON, 2, 2, 2)
+    assert e.value.code == -2
+    h = api.pm_lattice_create(g, g, I.boson_channel(), 0, 1, 0, I.PM_SPINLESS_BOSON, 2, 2, 2)
+    assert api.pm_lattice_dims(h) == (262144, 262144)
+    api.pm_lattice_destroy(h)
+
+
+def test_compute_calls_fail_loudly_without_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    wl = I.config(0)
+    h = _create(wl)
+
+    class Fake:
+        def data_ptr(self):
+            return 256
+
+        def numel(self):
+            return 1
+    with pytest.raises(api.PmError) as e:
+        api.pm_pattern(h, 0, 1, Fake(), None, stream=0)
+    assert e.value.code == -9
+    with pytest.raises(api.PmError) as e:
+        api.pm_build_host_count(h, 0)
+    assert e.value.code in (-9, -6, -5)
+    api.pm_lattice_destroy(h)
+
+
+def test_product_does_not_import_oracle():
+    """The product path must never route through the oracle (or any CPU fallback)."""
+    pkg = os.path.join(ROOT, "paper_1508_07441_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".cpp", ".hpp", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "pm_oracle" not in src and "from oracle" not in src and "import oracle" not in src, f
