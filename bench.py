@@ -1,0 +1,269 @@
+#!/usr/bin/env python
+"""bench.py — P-matrix build throughput on B200 (BASELINE.json metric: nonzeros/s, build time, % FP64 peak).
+
+A "step" is one pass of the whole hot path — pm_pattern (count, scan, emit columns) + pm_fill — over one
+lattice; the default workload is BASELINE.json configs[4] (the largest lattice; its CSR fits HBM, one block).
+`value` times the device-resident path with CUDA events; `e2e` times pm_build_host (host buffers, D2H copies
+inside the timed region); `roofline` is for the dominant kernel (the fill); `cpu_baseline` times the oracle on
+a bounded sample of source cells on the host cores.  `--impl reference` times the oracle alone.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_1508_07441_b200 import inputs  # noqa: E402
+
+METRIC = "P-matrix nonzeros/sec (pattern + fill, FP64)"
+UNIT = "nnz/s"
+# FP64 ALU peak used for the roofline: SMs x 64 DFMA lanes x 2 flop x max SM clock
+FP64_LANES_PER_SM = 64
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return {"hbm_gbs": d.get("hbm_gbs", 6650.0), "sm_max_mhz": d.get("sm_max_mhz", 1965.0), "src": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "src": "fallback"}
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([c.strip() for c in out.split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=6)
+
+    def summary(self):
+        sm, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = max(mx, float(r[1]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                continue
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def build_flops(lat_api, h, wl, nnz):
+    """Algorithmic FP64 flops of one build from pm_lattice_work."""
+    per_node, per_hit, n_pairs = lat_api.pm_lattice_work(h)
+    return per_node * wl.n_cells * wl.nodes_per_cell + per_hit * (nnz / n_pairs), per_node, per_hit
+
+
+def oracle_sample(wl, seconds_target=15.0, max_cells=64):
+    """Times the oracle as it stands on evenly spaced source cells of `wl` (bounded CPU work)."""
+    from oracle.pm_oracle import Oracle
+    o = Oracle()
+    cells = np.unique(np.linspace(0, wl.n_cells - 1, max_cells).astype(int))
+    t0 = time.perf_counter()
+    nnz, done = 0, 0
+    for c in cells:
+        rp, _, _ = o.build_csr(wl, int(c), int(c) + 1)
+        nnz += int(rp[-1]); done += 1
+        if time.perf_counter() - t0 > seconds_target:
+            break
+    dt = time.perf_counter() - t0
+    return {"value": nnz / dt, "unit": UNIT, "cores": o.threads(), "kind": "oracle",
+            "sample": f"{done} evenly spaced source cells of {wl.name} ({nnz} nnz in {dt:.1f} s), one cell per call"}, nnz, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    wl = inputs.config(args.config)
+    per_step = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_sample(wl, per_step, 16)
+    tot_nnz, tot_t, info = 0, 0.0, None
+    for _ in range(args.steps):
+        info, nnz, dt = oracle_sample(wl, per_step, 16)
+        tot_nnz += nnz; tot_t += dt
+    v = tot_nnz / tot_t
+    info["value"] = v
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+                      "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                      "data": "synthetic", "config": {"workload": wl.name, "M": wl.M, "sampled": True},
+                      "cpu_baseline": info,
+                      "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="pm")
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (default 4, the metric's workload)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1508_07441_b200 import api
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    api.lib()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    wl = inputs.config(args.config)
+    lat = api.Lattice(wl)
+    st = torch.cuda.current_stream()
+    # outputs allocated once (caller-owned buffers); every step rewrites them completely
+    rowptr = torch.empty(wl.M + 1, dtype=torch.int64, device="cuda")
+    nnz = api.pm_pattern(lat.h, 0, wl.n_cells, rowptr, None)
+    colidx = torch.empty(nnz, dtype=torch.int32, device="cuda")
+    vals = torch.empty(nnz, dtype=torch.float64, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+
+    def step(ev=None):
+        api.pm_pattern(lat.h, 0, wl.n_cells, rowptr, colidx)
+        if ev:
+            ev[0].record(st)
+        api.pm_fill(lat.h, 0, wl.n_cells, rowptr, vals)
+        if ev:
+            ev[1].record(st)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    l0 = api.pm_launch_count()
+    step_ms, fill_ms = [], []
+    with ClockSampler(local) as clocks:
+        for _ in range(args.steps):
+            flush.zero_()                                     # L2 flush between timed iterations (untimed)
+            e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            barrier()
+            e0.record(st)
+            step((e1, e2))
+            torch.cuda.synchronize()
+            step_ms.append(e0.elapsed_time(e2)); fill_ms.append(e1.elapsed_time(e2))
+        barrier()
+    launches = api.pm_launch_count() - l0
+    tot = torch.tensor([sum(step_ms)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tot, op=dist.ReduceOp.MAX)
+    total_ms = float(tot.item())
+    value = world * nnz * args.steps / (total_ms * 1e-3)
+
+    # ---- roofline of the dominant kernel (fill): FP64 ALU bound
+    pk = _peaks()
+    n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+    peak_tf = n_sm * FP64_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 * 1e-12
+    flops, per_node, per_hit = build_flops(api, lat.h, wl, nnz)
+    fill_avg = float(np.mean(fill_ms)) * 1e-3
+    achieved_tf = flops / fill_avg * 1e-12
+    dfma = api.pm_diag_dfma_tflops()
+    roof = {"bound": "alu", "kernel": "pm_fill", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
+            "frac": achieved_tf / peak_tf, "traffic": None,
+            "peak_source": f"{n_sm} SM x {FP64_LANES_PER_SM} DFMA lanes x 2 x {pk['sm_max_mhz']:.0f} MHz ({pk['src']} clock); "
+                           f"DFMA microbenchmark on this box: {dfma:.1f} TFLOP/s",
+            "flop_per_node": per_node, "flop_per_hit_cell": per_hit, "fill_ms": fill_avg * 1e3,
+            "csr_write_gbs": 8.0 * nnz / fill_avg * 1e-9, "hbm_peak_gbs": pk["hbm_gbs"]}
+
+    # ---- end to end through the C ABI with HOST buffers (D2H copies inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        h_rp = torch.empty(wl.M + 1, dtype=torch.int64, pin_memory=True)
+        h_ci = torch.empty(nnz, dtype=torch.int32, pin_memory=True)
+        h_v = torch.empty(nnz, dtype=torch.float64, pin_memory=True)
+        del colidx, vals
+        torch.cuda.empty_cache()
+        def e2e_step():
+            # the call a user makes: create the lattice from host arrays (host precompute + table upload),
+            # build with host outputs (pattern, fill and device->host copies), destroy
+            l2 = api.Lattice(wl)
+            r = api.pm_build_host(l2.h, 0, h_rp, h_ci, h_v)
+            l2.close()
+            return r
+
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        nb = 1
+        for _ in range(args.e2e_steps):
+            _, nb = e2e_step()
+        barrier()
+        dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+        h2d = wl.p_edges.nbytes + wl.q_edges.nbytes + wl.channels.nbytes + sum(a.nbytes + b.nbytes for a, b in wl.rules.values())
+        e2e = {"value": world * nnz * args.e2e_steps / float(dt.item()), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(12 * nnz + 8 * (wl.M + 1)), "blocks": nb, "steps": args.e2e_steps,
+               "api": "pm_lattice_create + pm_lattice_set_rule + pm_build_host (pinned host buffers) + pm_lattice_destroy"}
+
+    if rank == 0:
+        cpu = None
+        if not args.no_cpu and world == 1:
+            cpu, _, _ = oracle_sample(wl)
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+               "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+               "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+               "config": {"workload": wl.name, "M": wl.M, "n_channels": wl.n_ch, "cells": wl.n_cells,
+                          "nodes_per_cell": wl.nodes_per_cell, "nnz": nnz, "csr_bytes": 12 * nnz, "blocks": 1,
+                          "l2": "256 MiB buffer written between timed steps (L2 flush); outputs (12 B/nnz) exceed L2",
+                          "replicas": "each rank builds the whole lattice (rows are independent; no data-path collective)"},
+               "build_ms": {"best": float(np.min(step_ms)), "median": float(np.median(step_ms)),
+                            "pattern_median": float(np.median(np.array(step_ms) - np.array(fill_ms))),
+                            "fill_median": float(np.median(fill_ms))},
+               "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
+               "clocks": clocks.summary()}
+        print(json.dumps(out))
+    lat.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

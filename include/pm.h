@@ -103,6 +103,15 @@ int32_t pm_build_host(pm_lattice* lat, int64_t device_budget_bytes,
                       int64_t* h_rowptr, int32_t* h_colidx, double* h_vals, int64_t capacity,
                       int64_t* nnz_total, int32_t* n_blocks);
 
+/* Algorithmic work of this lattice's formulation (add = mul = div = sqrt = 1 flop, FMA = 2;
+ * comparisons and integer work not counted): FP64 flops per quadrature node and per hit (source, target) cell
+ * pair.  One build = flop_per_node * n_cells*n_p*n_q*n_x + flop_per_hit_cell * nnz/n_coupled_pairs.  Host only. */
+int32_t pm_lattice_work(const pm_lattice* lat, double* flop_per_node, double* flop_per_hit_cell, int32_t* n_coupled_pairs);
+
+/* Diagnostic: measured FP64 FMA throughput of the current device in TFLOP/s (a dependent-free DFMA loop on every
+ * SM, timed with CUDA events on `cuda_stream`); the roofline denominator is stated beside it in DESIGN.md sec. 7. */
+int32_t pm_diag_dfma_tflops(double* tflops, void* cuda_stream);
+
 /* Number of kernels this library has launched so far in the calling process (bench.py `gpu_launches`). */
 int64_t pm_launch_count(void);
 

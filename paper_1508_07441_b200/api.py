@@ -22,7 +22,7 @@ ERRORS = {-1: "PM_ERR_ARG", -2: "PM_ERR_GRID", -3: "PM_ERR_CHANNEL", -4: "PM_ERR
           -6: "PM_ERR_NOMEM", -7: "PM_ERR_STATE", -8: "PM_ERR_OVERFLOW", -9: "PM_ERR_DEVICE"}
 
 EXPORTS = ["pm_lattice_create", "pm_lattice_destroy", "pm_lattice_dims", "pm_lattice_rule", "pm_lattice_set_rule",
-           "pm_lattice_coupling", "pm_pattern", "pm_fill", "pm_spmv", "pm_build_host_count", "pm_build_host",
+           "pm_lattice_coupling", "pm_lattice_work", "pm_diag_dfma_tflops", "pm_pattern", "pm_fill", "pm_spmv", "pm_build_host_count", "pm_build_host",
            "pm_launch_count", "pm_last_error"]
 
 
@@ -58,6 +58,8 @@ def lib():
     L.pm_lattice_rule.argtypes = [_vp, C.c_int32, _dp, _dp]
     L.pm_lattice_set_rule.argtypes = [_vp, C.c_int32, _dp, _dp]
     L.pm_lattice_coupling.argtypes = [_vp, C.POINTER(C.c_uint8), _i32p]
+    L.pm_lattice_work.argtypes = [_vp, _dp, _dp, _i32p]
+    L.pm_diag_dfma_tflops.argtypes = [_dp, _vp]
     L.pm_pattern.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, C.c_int64, _i64p, _vp]
     L.pm_fill.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, _vp]
     L.pm_spmv.argtypes = [_vp, C.c_int64, _vp, _vp, _vp, _vp, _vp, _vp]
@@ -125,6 +127,19 @@ def pm_lattice_coupling(h, n_ch):
     nf = C.c_int32()
     _check(lib().pm_lattice_coupling(h, m.ctypes.data_as(C.POINTER(C.c_uint8)), C.byref(nf)))
     return m.reshape(n_ch, n_ch).astype(bool), nf.value
+
+
+def pm_lattice_work(h):
+    """(flop per node, flop per hit cell pair, number of coupled channel pairs) of the formulation."""
+    a, b, n = C.c_double(), C.c_double(), C.c_int32()
+    _check(lib().pm_lattice_work(h, C.byref(a), C.byref(b), C.byref(n)))
+    return a.value, b.value, n.value
+
+
+def pm_diag_dfma_tflops(stream=None):
+    t = C.c_double()
+    _check(lib().pm_diag_dfma_tflops(C.byref(t), _stream_ptr(stream)))
+    return t.value
 
 
 def pm_pattern(h, cell_begin, cell_end, d_rowptr, d_colidx=None, stream=None):

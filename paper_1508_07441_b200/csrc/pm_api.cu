@@ -254,6 +254,45 @@ int32_t pm_lattice_coupling(const pm_lattice* lat, uint8_t* coupled, int32_t* n_
     return PM_OK;
 }
 
+int32_t pm_lattice_work(const pm_lattice* lat, double* flop_per_node, double* flop_per_hit_cell, int32_t* n_coupled_pairs)
+{
+    if (!lat) return fail(PM_ERR_ARG, "lat is NULL");
+    const pm::Tables& T = lat->T;
+    // node generation + map (p, q, pq, p^2, q^2, pqx, P2, Q2, 2 sqrt) = 18, weight 4, omega 3
+    double node = 25.0;
+    // rotated directions from components: 4 components (8), two norms (2*(3+1)), 4 scalings
+    node += 20.0;
+    // two sets of Y_lm, m >= 0, l <= lmax: diagonal terms 2 flop, the others 4 flop
+    const int lmax = T.lmax;
+    node += 2.0 * (2.0 * lmax + 4.0 * (lmax * (lmax + 1) / 2));
+    // ket bipolar harmonics: c*Yp*Yq accumulated (mul + FMA = 3) per term, one scaling by omega per slot
+    node += 3.0 * (double)T.kt_c.size() + (double)T.n_slot;
+    // orbital functions: one FMA per (function, M) whose bra weight is not structurally zero
+    double fma = 0.0;
+    for (const pm::OrbFun& f : T.fun) for (int i = 0; i < f.nM; ++i) if (T.slot_w[(size_t)f.sa0 + i] != 0.0) fma += 1.0;
+    node += 2.0 * fma;
+    if (flop_per_node) *flop_per_node = node;
+    // per hit cell: normalisation (~8), one FMA per (channel pair, L) term, one scaling per output
+    if (flop_per_hit_cell) *flop_per_hit_cell = 8.0 + 2.0 * (double)T.ot_c.size() + (double)T.totcoup;
+    if (n_coupled_pairs) *n_coupled_pairs = T.totcoup;
+    return PM_OK;
+}
+
+int32_t pm_diag_dfma_tflops(double* tflops, void* cuda_stream)
+{
+    if (!tflops) return fail(PM_ERR_ARG, "NULL argument");
+    int dev = -1;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(PM_ERR_DEVICE, "no CUDA device");
+    }
+    if (prop.major < 10) return fail(PM_ERR_DEVICE, "libpm is built for sm_100a (B200); this device is older");
+    cudaError_t e = pm::measure_dfma(prop.multiProcessorCount, tflops, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e, "k_dfma_peak");
+    return PM_OK;
+}
+
 int32_t pm_pattern(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int64_t* d_rowptr, int32_t* d_colidx,
                    int64_t colidx_capacity, int64_t* nnz_host, void* cuda_stream)
 {

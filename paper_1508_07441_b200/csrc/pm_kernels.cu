@@ -379,4 +379,48 @@ cudaError_t launch_spmv(int64_t n_rows, const int64_t* rowptr, const int32_t* co
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------------
+// FP64 peak diagnostic: 16 independent FMA chains per thread, 1024 threads per CTA, 2 CTAs per SM.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024) k_dfma_peak(int iters, double seed, double* __restrict__ sink)
+{
+    double a[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) a[k] = seed + k + threadIdx.x;
+    const double m = 1.0000001, c = 1e-9;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) a[k] = fma(a[k], m, c);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) s += a[k];
+    if (s == 12345.678) sink[0] = s;           // never true; keeps the chains alive
+}
+
+cudaError_t measure_dfma(int n_sm, double* tflops, cudaStream_t st)
+{
+    double* sink = nullptr;
+    cudaError_t e = cudaMalloc(&sink, 8);
+    if (e != cudaSuccess) return e;
+    cudaEvent_t t0, t1;
+    cudaEventCreate(&t0); cudaEventCreate(&t1);
+    const int iters = 4096, blocks = 2 * n_sm;
+    float best = 1e30f;
+    for (int rep = 0; rep < 6; ++rep) {
+        cudaEventRecord(t0, st);
+        k_dfma_peak<<<blocks, 1024, 0, st>>>(iters, 1.0, sink);
+        ++g_launches;
+        cudaEventRecord(t1, st);
+        if ((e = cudaEventSynchronize(t1)) != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, t0, t1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(t0); cudaEventDestroy(t1); cudaFree(sink);
+    if (e != cudaSuccess) return e;
+    *tflops = 2.0 * 16.0 * iters * 1024.0 * blocks / (best * 1e-3) * 1e-12;
+    return cudaGetLastError();
+}
+
 }  // namespace pm

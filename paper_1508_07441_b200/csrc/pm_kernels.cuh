@@ -28,4 +28,7 @@ cudaError_t launch_fill_generic(const DevLattice& L, int cell_begin, int n_blk, 
 cudaError_t launch_spmv(int64_t n_rows, const int64_t* rowptr, const int32_t* colidx, const double* vals,
                         const double* x, double* y, cudaStream_t st);
 
+// dependent-free DFMA loop on every SM: measured FP64 FMA throughput in TFLOP/s (diagnostic)
+cudaError_t measure_dfma(int n_sm, double* tflops, cudaStream_t st);
+
 }  // namespace pm
