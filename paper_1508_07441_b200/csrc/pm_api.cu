@@ -2,6 +2,7 @@
 // entry points pm_pattern / pm_fill / pm_spmv / pm_build_host.  No torch types, no CPU fallback.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <new>
@@ -45,6 +46,10 @@ struct pm_lattice {
     int64_t* h_summary = nullptr;      // pinned
     int hits_cap = 0;
     int hmax = -1, hmax_begin = -1, hmax_end = -1;   // from the last pattern call and its cell range
+    double* d_acc = nullptr;           // fill scratch: per persistent CTA, hmax rows of n_fun sums
+    size_t acc_bytes = 0;
+    unsigned long long hash = 0;       // pm::tables_hash of T (selects a generated fill kernel)
+    int n_sm = 0;
     pm::DevLattice dev{};
 };
 
@@ -57,6 +62,8 @@ void free_device(pm_lattice* L)
     if (L->d_cellbase) cudaFree(L->d_cellbase);
     if (L->d_summary) cudaFree(L->d_summary);
     if (L->h_summary) cudaFreeHost(L->h_summary);
+    if (L->d_acc) cudaFree(L->d_acc);
+    L->d_acc = nullptr; L->acc_bytes = 0;
     L->d_blob = nullptr; L->d_hits = nullptr; L->d_cellbase = nullptr; L->d_summary = nullptr; L->h_summary = nullptr;
     L->hits_cap = 0;
 }
@@ -74,6 +81,7 @@ int32_t ensure_device(pm_lattice* L)
     if (!L->dirty && L->device == dev) return PM_OK;
     free_device(L);
     L->device = dev;
+    L->n_sm = prop.multiProcessorCount;
 
     const pm::Tables& T = L->T;
     pm::DevLattice D{};
@@ -94,6 +102,9 @@ int32_t ensure_device(pm_lattice* L)
     std::vector<double> pe(D.pe_pad, inf), qe(D.qe_pad, inf);
     std::copy(L->pe.begin(), L->pe.end(), pe.begin());
     std::copy(L->qe.begin(), L->qe.end(), qe.begin());
+    std::vector<double> thp(D.pe_pad, inf), thq(D.qe_pad, inf);          // +inf has the largest bit pattern of all
+    for (int k = 0; k <= L->Np; ++k) thp[(size_t)k] = pm::sqrt_threshold(L->pe[(size_t)k]);
+    for (int k = 0; k <= L->Nq; ++k) thq[(size_t)k] = pm::sqrt_threshold(L->qe[(size_t)k]);
     std::vector<double> sx(L->n_x), bra;
     for (int c = 0; c < L->n_x; ++c) { const double x = L->rule_t[2][c]; sx[c] = std::sqrt((1.0 - x) * (1.0 + x)); }
     pm::build_bra(T, L->rule_t[2], bra);
@@ -103,6 +114,7 @@ int32_t ensure_device(pm_lattice* L)
     for (size_t f = 0; f < T.fun.size(); ++f) fun[f] = make_int4(T.fun[f].sa0, T.fun[f].sb0, T.fun[f].nM, T.fun[f].L);
 
     const size_t o_pe = put(pe.data(), 8 * pe.size()), o_qe = put(qe.data(), 8 * qe.size());
+    const size_t o_thp = put(thp.data(), 8 * thp.size()), o_thq = put(thq.data(), 8 * thq.size());
     size_t o_t[3], o_w[3];
     for (int k = 0; k < 3; ++k) { o_t[k] = put(L->rule_t[k].data(), 8 * L->rule_t[k].size()); o_w[k] = put(L->rule_w[k].data(), 8 * L->rule_w[k].size()); }
     const size_t o_sx = put(sx.data(), 8 * sx.size());
@@ -123,6 +135,7 @@ int32_t ensure_device(pm_lattice* L)
     if ((e = cudaMallocHost(&L->h_summary, 2 * sizeof(int64_t))) != cudaSuccess) return cuda_fail(e, "cudaMallocHost(summary)");
     char* b = L->d_blob;
     D.pe = (const double*)(b + o_pe); D.qe = (const double*)(b + o_qe);
+    D.thr_p = (const long long*)(b + o_thp); D.thr_q = (const long long*)(b + o_thq);
     D.tp = (const double*)(b + o_t[0]); D.wp = (const double*)(b + o_w[0]);
     D.tq = (const double*)(b + o_t[1]); D.wq = (const double*)(b + o_w[1]);
     D.tx = (const double*)(b + o_t[2]); D.wx = (const double*)(b + o_w[2]);
@@ -194,6 +207,7 @@ int32_t pm_lattice_create(const double* p_edges, int32_t Np, const double* q_edg
     L->ch.assign(ch, ch + n_ch);
     msg = pm::build_tables(ch, n_ch, J2, T2, statistics, L->T);
     if (!msg.empty()) { delete L; return fail(PM_ERR_CHANNEL, msg); }
+    L->hash = pm::tables_hash(L->T);
     if ((int)L->T.fun.size() > pm::kMaxFun || L->T.n_slot > pm::kMaxSlot) {
         delete L; return fail(PM_ERR_CHANNEL, "channel set needs more orbital functions than this build supports");
     }
@@ -337,8 +351,26 @@ int32_t pm_fill(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const int
     if (cell_begin == cell_end) return PM_OK;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int hmax = std::max(lat->hmax, 1);
-    if (pm::fill_generic_smem(lat->dev, hmax) > 227 * 1024) return fail(PM_ERR_NOMEM, "source cell needs more shared memory than one SM has");
-    cudaError_t e = pm::launch_fill_generic(lat->dev, cell_begin, cell_end - cell_begin, hmax, d_rowptr, d_vals, st);
+    const int n_blk = cell_end - cell_begin;
+    cudaError_t e;
+    static const bool use_v1 = std::getenv("PM_FILL_V1") != nullptr;        // first-round table-driven kernel (debug aid)
+    if (use_v1) {
+        if (pm::fill_generic_smem(lat->dev, hmax) > 227 * 1024) return fail(PM_ERR_NOMEM, "source cell needs more shared memory than one SM has");
+        e = pm::launch_fill_generic(lat->dev, cell_begin, n_blk, hmax, d_rowptr, d_vals, st);
+    } else {
+        pm::FillLaunch F;
+        e = pm::fill_plan(lat->dev, lat->hash, hmax, lat->n_sm, &F);
+        if (e == cudaErrorInvalidConfiguration) { cudaGetLastError(); return fail(PM_ERR_NOMEM, "source cell needs more shared memory than one SM has"); }
+        if (e != cudaSuccess) return cuda_fail(e, "fill_plan");
+        const size_t need = sizeof(double) * (size_t)F.grid * (size_t)hmax * (size_t)lat->dev.n_fun;
+        if (need > lat->acc_bytes) {
+            if (lat->d_acc) { if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e, "sync"); cudaFree(lat->d_acc); }
+            lat->d_acc = nullptr; lat->acc_bytes = 0;
+            if ((e = cudaMalloc(&lat->d_acc, need)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(fill scratch)");
+            lat->acc_bytes = need;
+        }
+        e = pm::launch_fill(lat->dev, F, cell_begin, n_blk, hmax, d_rowptr, d_vals, lat->d_acc, st);
+    }
     if (e != cudaSuccess) return cuda_fail(e, "k_fill");
     return PM_OK;
 }

@@ -14,6 +14,7 @@ struct DevLattice {
     int Np, Nq, n_ch, n_p, n_q, n_x, nnode, n_cells, n_words, pe_pad, qe_pad;
     int totcoup, n_slot, n_fun, lmax, ny;
     const double *pe, *qe;                      // edges padded with +inf to pe_pad / qe_pad (powers of two)
+    const long long *thr_p, *thr_q;             // bit patterns of sqrt_threshold(edge), same padding (+inf)
     const double *tp, *wp, *tq, *wq, *tx, *wx;  // Gauss-Legendre rules on [-1,1]
     const double *sx;                           // sqrt(1-x^2) per x-node
     const int *cl_off, *cl, *o_alpha;           // coupled lists; o_alpha[o] = alpha of output o

@@ -1,0 +1,82 @@
+// pm_fill.cu — instantiations and launcher of the fill kernel (pm_fill.cuh): one instantiation per generated
+// channel-set specialisation (gen/pm_spec_gen.cuh, written by pm_codegen at build time) plus the table-driven one.
+#include "pm_fill.cuh"
+
+#include <cstdlib>
+
+#include "gen/pm_spec_gen.cuh"
+#include "pm_kernels.cuh"
+
+namespace pm {
+
+namespace {
+
+constexpr int kSmemLimit = 227 * 1024;
+
+using FillKernel = void (*)(DevLattice, FillSmem, int, int, int, const int64_t*, double*, double*);
+
+struct FillVariant { unsigned long long hash; int nw; FillKernel fn; const char* name; };
+
+#define PM_SPEC(S) {gen::S::kHash, 4, k_fill_seg<gen::S, 4>, #S}, {gen::S::kHash, 8, k_fill_seg<gen::S, 8>, #S}, \
+                   {gen::S::kHash, 12, k_fill_seg<gen::S, 12>, #S},
+const FillVariant kVariants[] = {
+    PM_SPEC_LIST
+    {0ull, 4, k_fill_seg<SpecGeneric, 4>, "generic"}, {0ull, 8, k_fill_seg<SpecGeneric, 8>, "generic"},
+};
+#undef PM_SPEC
+
+int preferred_warps()
+{
+    static const int v = [] { const char* e = std::getenv("PM_FILL_WARPS"); return e ? std::atoi(e) : 8; }();
+    return v;
+}
+
+}  // namespace
+
+bool fill_has_spec(unsigned long long hash)
+{
+    for (const FillVariant& v : kVariants) if (v.hash == hash && hash != 0ull) return true;
+    return false;
+}
+
+// Picks the variant (specialised when `hash` matches a generated kernel, else table-driven; the preferred warp count
+// if its shared memory fits, else a smaller one) and the persistent grid.  Returns cudaErrorInvalidConfiguration
+// when no variant fits in shared memory.
+cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int hmax, int n_sm, FillLaunch* out)
+{
+    const unsigned long long key = fill_has_spec(hash) ? hash : 0ull;
+    const int want = preferred_warps();
+    const FillVariant* best = nullptr;          // largest warp count <= want whose shared memory fits, else the smallest that fits
+    for (const FillVariant& v : kVariants) {
+        if (v.hash != key || fill_smem_plan(L, hmax, v.nw).total > kSmemLimit) continue;
+        if (!best) { best = &v; continue; }
+        const bool v_ok = v.nw <= want, b_ok = best->nw <= want;
+        if ((v_ok && (!b_ok || v.nw > best->nw)) || (!v_ok && !b_ok && v.nw < best->nw)) best = &v;
+    }
+    if (!best) return cudaErrorInvalidConfiguration;
+    out->fn = (const void*)best->fn;
+    out->nw = best->nw;
+    out->name = best->name;
+    out->smem = fill_smem_plan(L, hmax, best->nw);
+    cudaError_t e = cudaFuncSetAttribute(out->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, out->smem.total);
+    if (e != cudaSuccess) return e;
+    int per_sm = 1;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, out->fn, best->nw * 32, (size_t)out->smem.total);
+    if (e != cudaSuccess) return e;
+    out->grid = n_sm * (per_sm > 0 ? per_sm : 1);
+    return cudaSuccess;
+}
+
+cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, int hmax, const int64_t* rowptr,
+                        double* vals, double* accG, cudaStream_t st)
+{
+    const int grid = n_blk < F.grid ? n_blk : F.grid;
+    DevLattice Lc = L;
+    FillSmem S = F.smem;
+    void* args[] = {&Lc, &S, &cell_begin, &n_blk, &hmax, (void*)&rowptr, &vals, &accG};
+    cudaError_t e = cudaLaunchKernel(F.fn, dim3((unsigned)grid), dim3((unsigned)(F.nw * 32)), args, (size_t)S.total, st);
+    count_launch();
+    return e != cudaSuccess ? e : cudaGetLastError();
+}
+
+}  // namespace pm

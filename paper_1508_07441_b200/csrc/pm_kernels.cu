@@ -320,6 +320,7 @@ __global__ void __launch_bounds__(256) k_spmv(int64_t n_rows, const int64_t* __r
 // ------------------------------------------------------------------------------------------------
 static std::atomic<int64_t> g_launches{0};
 int64_t launch_count() { return g_launches.load(); }
+void count_launch() { ++g_launches; }
 
 size_t fill_generic_smem(const DevLattice& L, int hmax)
 {

@@ -6,6 +6,7 @@
 #include <cstdint>
 
 #include "pm_device.cuh"
+#include "pm_fill.cuh"
 
 namespace pm {
 
@@ -27,6 +28,14 @@ cudaError_t launch_fill_generic(const DevLattice& L, int cell_begin, int n_blk, 
                                 double* vals, cudaStream_t st);
 cudaError_t launch_spmv(int64_t n_rows, const int64_t* rowptr, const int32_t* colidx, const double* vals,
                         const double* x, double* y, cudaStream_t st);
+
+// fill pass (pm_fill.cuh): variant selection and launch
+struct FillLaunch { const void* fn; int nw, grid; FillSmem smem; const char* name; };
+bool fill_has_spec(unsigned long long tables_hash);
+cudaError_t fill_plan(const DevLattice& L, unsigned long long tables_hash, int hmax, int n_sm, FillLaunch* out);
+cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, int hmax, const int64_t* rowptr,
+                        double* vals, double* accG, cudaStream_t st);
+void count_launch();
 
 // dependent-free DFMA loop on every SM: measured FP64 FMA throughput in TFLOP/s (diagnostic)
 cudaError_t measure_dfma(int n_sm, double* tflops, cudaStream_t st);

@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdlib>
+#include <limits>
 #include <map>
 #include <tuple>
 
@@ -289,6 +290,49 @@ void build_bra(const Tables& T, const std::vector<double>& tx, std::vector<doubl
             if (T.slot_w[(size_t)s] != 0.0)
                 bra[c * (size_t)T.n_slot + (size_t)s] = T.slot_w[(size_t)s] * Y[(size_t)ylm_index(T.slot_l[(size_t)s], T.slot_M[(size_t)s])];
     }
+}
+
+uint64_t tables_hash(const Tables& T)
+{
+    uint64_t h = 1469598103934665603ull;
+    auto mix = [&](const void* p, size_t n) {
+        const unsigned char* b = (const unsigned char*)p;
+        for (size_t i = 0; i < n; ++i) { h ^= b[i]; h *= 1099511628211ull; }
+    };
+    auto mixi = [&](int64_t v) { mix(&v, sizeof v); };
+    mixi(T.lmax); mixi(T.n_slot); mixi((int64_t)T.tri.size()); mixi((int64_t)T.fun.size());
+    for (const Triple& t : T.tri) { mixi(t.l); mixi(t.lam); mixi(t.L); mixi(t.M0); mixi(t.nM); mixi(t.slot0); }
+    for (const OrbFun& f : T.fun) { mixi(f.sa0); mixi(f.sb0); mixi(f.nM); mixi(f.L); }
+    mix(T.kt_off.data(), 4 * T.kt_off.size()); mix(T.kt_ip.data(), 4 * T.kt_ip.size());
+    mix(T.kt_iq.data(), 4 * T.kt_iq.size()); mix(T.kt_c.data(), 8 * T.kt_c.size());
+    return h;
+}
+
+void scaled_harmonics(int lmax, std::vector<double>& ynorm, std::vector<double>& ybeta)
+{
+    const int ny = ylm_index(lmax, lmax) + 1;
+    std::vector<long double> N((size_t)ny, 0.0L);
+    ynorm.assign((size_t)ny, 0.0); ybeta.assign((size_t)ny, 0.0);
+    auto ya = [](int l, int m) { return sqrtl((4.0L * l * l - 1.0L) / ((long double)l * l - (long double)m * m)); };
+    auto yb = [](int l, int m) { return sqrtl((((long double)l - 1) * (l - 1) - (long double)m * m) / (4.0L * (l - 1) * (l - 1) - 1.0L)); };
+    N[0] = 0.5L / sqrtl(3.14159265358979323846264338327950288L);
+    for (int m = 0; m <= lmax; ++m) {
+        if (m > 0) N[(size_t)ylm_index(m, m)] = -sqrtl((2.0L * m + 1.0L) / (2.0L * m)) * N[(size_t)ylm_index(m - 1, m - 1)];
+        for (int l = m + 1; l <= lmax; ++l) {
+            N[(size_t)ylm_index(l, m)] = ya(l, m) * N[(size_t)ylm_index(l - 1, m)];
+            if (l - 2 >= m) ybeta[(size_t)ylm_index(l, m)] = (double)(yb(l, m) / ya(l - 1, m));
+        }
+    }
+    for (int k = 0; k < ny; ++k) ynorm[(size_t)k] = (double)N[(size_t)k];
+}
+
+double sqrt_threshold(double e)
+{
+    if (!(e > 0.0)) return 0.0;                         // every y >= 0 has sqrt(y) >= 0
+    double y = e * e;
+    while (std::sqrt(y) >= e && y > 0.0) y = std::nextafter(y, 0.0);
+    while (std::sqrt(y) < e) y = std::nextafter(y, std::numeric_limits<double>::infinity());
+    return y;
 }
 
 }  // namespace pm

@@ -57,4 +57,17 @@ void gauss_legendre(int n, std::vector<double>& t, std::vector<double>& w);
 // bra[c*n_slot + s] for the x-rule nodes
 void build_bra(const Tables& T, const std::vector<double>& tx, std::vector<double>& bra);
 
+// FNV-1a hash of everything the ket-side code of a fill kernel depends on (slot layout, ket term lists with
+// the coefficient bit patterns, function list).  A kernel specialised at build time by pm_codegen carries the
+// hash of the tables it was generated from; pm_fill uses it only when the lattice's tables hash equal.
+uint64_t tables_hash(const Tables& T);
+
+// Scaled harmonics used by generated code: Y_lm = ynorm[lm] * Q_lm with the constant-free recurrence
+//   Q_00 = 1, Q_mm = ux*Q_{m-1,m-1}, Q_{m+1,m} = uz*Q_mm, Q_lm = uz*Q_{l-1,m} - ybeta[lm]*Q_{l-2,m}.
+void scaled_harmonics(int lmax, std::vector<double>& ynorm, std::vector<double>& ybeta);
+
+// Smallest double y with sqrt(y) >= e (IEEE, correctly rounded): "e <= sqrt(y)" <=> "y >= sqrt_threshold(e)",
+// so a node is located from p'^2 with the very decisions the oracle takes on p' = sqrt(p'^2) (reading R6).
+double sqrt_threshold(double e);
+
 }  // namespace pm
