@@ -256,7 +256,8 @@ def main():
                           "replicas": "each rank builds the whole lattice (rows are independent; no data-path collective)"},
                "build_ms": {"best": float(np.min(step_ms)), "median": float(np.median(step_ms)),
                             "pattern_median": float(np.median(np.array(step_ms) - np.array(fill_ms))),
-                            "fill_median": float(np.median(fill_ms))},
+                            "fill_median": float(np.median(fill_ms)), "fill_best": float(np.min(fill_ms)),
+                            "fill_all": [round(float(x), 3) for x in fill_ms]},
                "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
                "clocks": clocks.summary()}
         print(json.dumps(out))

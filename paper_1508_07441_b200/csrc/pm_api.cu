@@ -40,12 +40,12 @@ struct pm_lattice {
     bool dirty = true;                 // tables need (re)upload
     int device = -1;
     char* d_blob = nullptr;            // all small tables
-    int* d_hits = nullptr;             // per-source-cell hit counts of the last pattern call
+    pm::NodeLists nl{};                // sorted node lists of the last pattern call (cells [pat_begin, pat_end))
     int64_t* d_cellbase = nullptr;
     int64_t* d_summary = nullptr;      // {nnz, hmax}
     int64_t* h_summary = nullptr;      // pinned
     int hits_cap = 0;
-    int hmax = -1, hmax_begin = -1, hmax_end = -1;   // from the last pattern call and its cell range
+    int hmax = -1, pat_begin = -1, pat_end = -1;     // max hit cells, and the cell range, of the last pattern call
     double* d_acc = nullptr;           // fill scratch: per persistent CTA, hmax rows of n_fun sums
     size_t acc_bytes = 0;
     unsigned long long hash = 0;       // pm::tables_hash of T (selects a generated fill kernel)
@@ -58,13 +58,16 @@ namespace {
 void free_device(pm_lattice* L)
 {
     if (L->d_blob) cudaFree(L->d_blob);
-    if (L->d_hits) cudaFree(L->d_hits);
+    if (L->nl.sorted) cudaFree(L->nl.sorted);
+    if (L->nl.rkpos) cudaFree(L->nl.rkpos);
+    if (L->nl.ntot) cudaFree(L->nl.ntot);
+    if (L->nl.hits) cudaFree(L->nl.hits);
     if (L->d_cellbase) cudaFree(L->d_cellbase);
     if (L->d_summary) cudaFree(L->d_summary);
     if (L->h_summary) cudaFreeHost(L->h_summary);
     if (L->d_acc) cudaFree(L->d_acc);
     L->d_acc = nullptr; L->acc_bytes = 0;
-    L->d_blob = nullptr; L->d_hits = nullptr; L->d_cellbase = nullptr; L->d_summary = nullptr; L->h_summary = nullptr;
+    L->d_blob = nullptr; L->nl = pm::NodeLists{}; L->d_cellbase = nullptr; L->d_summary = nullptr; L->h_summary = nullptr;
     L->hits_cap = 0;
 }
 
@@ -90,6 +93,8 @@ int32_t ensure_device(pm_lattice* L)
     D.pe_pad = next_pow2(L->Np + 1); D.qe_pad = next_pow2(L->Nq + 1);
     D.totcoup = T.totcoup; D.n_slot = T.n_slot; D.n_fun = (int)T.fun.size(); D.lmax = T.lmax;
     D.ny = pm::ylm_index(T.lmax, T.lmax) + 1;
+    auto magic = [](int d) { return d <= 1 ? 0u : (unsigned)(((1ull << 32) + (unsigned)d - 1) / (unsigned)d); };
+    D.mg_npq = magic(L->n_p * L->n_q); D.mg_nq = magic(L->n_q);
 
     std::vector<char> blob;
     auto put = [&](const void* src, size_t bytes) {
@@ -135,7 +140,7 @@ int32_t ensure_device(pm_lattice* L)
     if ((e = cudaMallocHost(&L->h_summary, 2 * sizeof(int64_t))) != cudaSuccess) return cuda_fail(e, "cudaMallocHost(summary)");
     char* b = L->d_blob;
     D.pe = (const double*)(b + o_pe); D.qe = (const double*)(b + o_qe);
-    D.thr_p = (const long long*)(b + o_thp); D.thr_q = (const long long*)(b + o_thq);
+    D.thr_p = (const double*)(b + o_thp); D.thr_q = (const double*)(b + o_thq);
     D.tp = (const double*)(b + o_t[0]); D.wp = (const double*)(b + o_w[0]);
     D.tq = (const double*)(b + o_t[1]); D.wq = (const double*)(b + o_w[1]);
     D.tx = (const double*)(b + o_t[2]); D.wx = (const double*)(b + o_w[2]);
@@ -156,11 +161,18 @@ int32_t ensure_device(pm_lattice* L)
 int32_t ensure_cell_scratch(pm_lattice* L, int n_blk)
 {
     if (n_blk <= L->hits_cap) return PM_OK;
-    if (L->d_hits) cudaFree(L->d_hits);
+    if (L->nl.sorted) cudaFree(L->nl.sorted);
+    if (L->nl.rkpos) cudaFree(L->nl.rkpos);
+    if (L->nl.ntot) cudaFree(L->nl.ntot);
+    if (L->nl.hits) cudaFree(L->nl.hits);
     if (L->d_cellbase) cudaFree(L->d_cellbase);
-    L->d_hits = nullptr; L->d_cellbase = nullptr; L->hits_cap = 0;
+    L->nl = pm::NodeLists{}; L->d_cellbase = nullptr; L->hits_cap = 0;
+    const size_t nn = (size_t)n_blk * (size_t)L->dev.nnode;
     cudaError_t e;
-    if ((e = cudaMalloc(&L->d_hits, sizeof(int) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(hits)");
+    if ((e = cudaMalloc(&L->nl.sorted, sizeof(unsigned short) * nn)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(node lists)");
+    if ((e = cudaMalloc(&L->nl.rkpos, sizeof(unsigned short) * nn)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(node lists)");
+    if ((e = cudaMalloc(&L->nl.ntot, sizeof(int) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(ntot)");
+    if ((e = cudaMalloc(&L->nl.hits, sizeof(int) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(hits)");
     if ((e = cudaMalloc(&L->d_cellbase, sizeof(int64_t) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(cellbase)");
     L->hits_cap = n_blk;
     return PM_OK;
@@ -208,7 +220,7 @@ int32_t pm_lattice_create(const double* p_edges, int32_t Np, const double* q_edg
     msg = pm::build_tables(ch, n_ch, J2, T2, statistics, L->T);
     if (!msg.empty()) { delete L; return fail(PM_ERR_CHANNEL, msg); }
     L->hash = pm::tables_hash(L->T);
-    if ((int)L->T.fun.size() > pm::kMaxFun || L->T.n_slot > pm::kMaxSlot) {
+    if ((int)L->T.fun.size() > pm::kFillMaxFun || L->T.n_slot > pm::kFillMaxSlot) {
         delete L; return fail(PM_ERR_CHANNEL, "channel set needs more orbital functions than this build supports");
     }
     const int orders[3] = {n_p, n_q, n_x};
@@ -321,21 +333,27 @@ int32_t pm_pattern(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int64_
     if (n_blk == 0) {
         if ((e = cudaMemsetAsync(d_rowptr, 0, sizeof(int64_t), st)) != cudaSuccess) return cuda_fail(e, "memset");
         if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e, "sync");
-        *nnz_host = 0; lat->hmax = 0; lat->hmax_begin = cell_begin; lat->hmax_end = cell_end;
+        *nnz_host = 0; lat->hmax = 0; lat->pat_begin = cell_begin; lat->pat_end = cell_end;
         return PM_OK;
     }
-    if ((rc = ensure_cell_scratch(lat, n_blk))) return rc;
-    if ((e = pm::launch_count_hits(lat->dev, cell_begin, n_blk, lat->d_hits, st)) != cudaSuccess) return cuda_fail(e, "k_count_hits");
-    if ((e = pm::launch_scan_rows(lat->dev, n_blk, lat->d_hits, lat->d_cellbase, d_rowptr, lat->d_summary, st)) != cudaSuccess)
+    // The node lists of the last call are reused when the range is the same (count first, then emit: one map pass).
+    const bool reuse = lat->hmax >= 0 && lat->pat_begin == cell_begin && lat->pat_end == cell_end && lat->hits_cap >= n_blk;
+    if (!reuse) {
+        lat->hmax = -1;
+        if ((rc = ensure_cell_scratch(lat, n_blk))) return rc;
+        if ((e = pm::launch_map_sort(lat->dev, cell_begin, n_blk, lat->nl, st)) != cudaSuccess) return cuda_fail(e, "k_map_sort");
+    }
+    if ((e = pm::launch_scan_rows(lat->dev, n_blk, lat->nl.hits, lat->d_cellbase, d_rowptr, lat->d_summary, st)) != cudaSuccess)
         return cuda_fail(e, "k_scan_rows");
     if ((e = cudaMemcpyAsync(lat->h_summary, lat->d_summary, 2 * sizeof(int64_t), cudaMemcpyDeviceToHost, st)) != cudaSuccess)
         return cuda_fail(e, "cudaMemcpyAsync(summary)");
-    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e, "pattern: count/scan");
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e, "pattern: map/scan");
     *nnz_host = lat->h_summary[0];
-    lat->hmax = (int)lat->h_summary[1]; lat->hmax_begin = cell_begin; lat->hmax_end = cell_end;
+    lat->hmax = (int)lat->h_summary[1]; lat->pat_begin = cell_begin; lat->pat_end = cell_end;
     if (!d_colidx) return PM_OK;
     if (*nnz_host > colidx_capacity) return fail(PM_ERR_OVERFLOW, "d_colidx too small for this block's nnz");
-    if ((e = pm::launch_emit_cols(lat->dev, cell_begin, n_blk, d_rowptr, d_colidx, st)) != cudaSuccess) return cuda_fail(e, "k_emit_cols");
+    if ((e = pm::launch_emit_cols(lat->dev, cell_begin, n_blk, lat->nl, lat->hmax, d_rowptr, d_colidx, st)) != cudaSuccess)
+        return cuda_fail(e, "k_emit_cols");
     return PM_OK;
 }
 
@@ -346,18 +364,14 @@ int32_t pm_fill(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const int
     if (cell_begin < 0 || cell_end > n_cells || cell_begin > cell_end) return fail(PM_ERR_ARG, "bad cell range");
     int32_t rc = ensure_device(lat);
     if (rc) return rc;
-    if (lat->hmax < 0 || cell_begin < lat->hmax_begin || cell_end > lat->hmax_end)
-        return fail(PM_ERR_STATE, "pm_fill needs a preceding pm_pattern covering the same cell range");
+    if (lat->hmax < 0 || cell_begin != lat->pat_begin || cell_end != lat->pat_end)
+        return fail(PM_ERR_STATE, "pm_fill needs a preceding pm_pattern of the same cell range on this lattice");
     if (cell_begin == cell_end) return PM_OK;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int hmax = std::max(lat->hmax, 1);
     const int n_blk = cell_end - cell_begin;
     cudaError_t e;
-    static const bool use_v1 = std::getenv("PM_FILL_V1") != nullptr;        // first-round table-driven kernel (debug aid)
-    if (use_v1) {
-        if (pm::fill_generic_smem(lat->dev, hmax) > 227 * 1024) return fail(PM_ERR_NOMEM, "source cell needs more shared memory than one SM has");
-        e = pm::launch_fill_generic(lat->dev, cell_begin, n_blk, hmax, d_rowptr, d_vals, st);
-    } else {
+    {
         pm::FillLaunch F;
         e = pm::fill_plan(lat->dev, lat->hash, hmax, lat->n_sm, &F);
         if (e == cudaErrorInvalidConfiguration) { cudaGetLastError(); return fail(PM_ERR_NOMEM, "source cell needs more shared memory than one SM has"); }
@@ -369,7 +383,7 @@ int32_t pm_fill(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const int
             if ((e = cudaMalloc(&lat->d_acc, need)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(fill scratch)");
             lat->acc_bytes = need;
         }
-        e = pm::launch_fill(lat->dev, F, cell_begin, n_blk, hmax, d_rowptr, d_vals, lat->d_acc, st);
+        e = pm::launch_fill(lat->dev, F, cell_begin, n_blk, lat->nl, hmax, d_rowptr, d_vals, lat->d_acc, st);
     }
     if (e != cudaSuccess) return cuda_fail(e, "k_fill");
     return PM_OK;

@@ -2,8 +2,10 @@
 // node generation (step a3), kinematic map (a4), branch-free cell location (a5), per-source-cell hit
 // bitset and ranks (a6).  SURVEY.md sec. 8(a); DESIGN.md sec. 3.1 gives the operation order that
 // makes a node land in the same cell as in the CPU oracle: every operation from the Gauss node to
-// p', q' is a single IEEE-754 double operation issued through __dadd_rn/__dmul_rn/__dsqrt_rn, which
-// the compiler never contracts into FMAs (north_star: "FMA contraction off").
+// p'^2, q'^2 is a single IEEE-754 double operation issued through __dadd_rn/__dmul_rn, which the compiler
+// never contracts into FMAs (north_star: "FMA contraction off").  The oracle then takes p' = sqrt(p'^2) and
+// compares it with the edges; here p'^2 is compared with sqrt_threshold(edge) (pm_tables.hpp), the smallest
+// double whose correctly rounded square root reaches the edge — the same decision without the square root.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -13,8 +15,9 @@ namespace pm {
 struct DevLattice {
     int Np, Nq, n_ch, n_p, n_q, n_x, nnode, n_cells, n_words, pe_pad, qe_pad;
     int totcoup, n_slot, n_fun, lmax, ny;
-    const double *pe, *qe;                      // edges padded with +inf to pe_pad / qe_pad (powers of two)
-    const long long *thr_p, *thr_q;             // bit patterns of sqrt_threshold(edge), same padding (+inf)
+    unsigned mg_npq, mg_nq;                     // ceil(2^32 / (n_p*n_q)), ceil(2^32 / n_q): exact division of node ids
+    const double *pe, *qe;                      // edges, Np+1 / Nq+1 entries (padded with +inf to pe_pad / qe_pad)
+    const double *thr_p, *thr_q;                // sqrt_threshold(edge), padded with +inf to a power of two
     const double *tp, *wp, *tq, *wq, *tx, *wx;  // Gauss-Legendre rules on [-1,1]
     const double *sx;                           // sqrt(1-x^2) per x-node
     const int *cl_off, *cl, *o_alpha;           // coupled lists; o_alpha[o] = alpha of output o
@@ -25,15 +28,15 @@ struct DevLattice {
     const double *ya, *yb, *ydiag;
 };
 
-// number of edges <= v, minus one; e has `pad` (power of two) entries, the tail filled with +inf
-__device__ __forceinline__ int locate(const double* __restrict__ e, int pad, double v)
-{
-    int lo = 0;
-#pragma unroll 1
-    for (int s = pad >> 1; s > 0; s >>= 1) lo += (e[lo + s - 1] <= v) ? s : 0;
-    lo += (e[lo] <= v) ? 1 : 0;          // entries beyond N+1 are +inf, so lo <= N+1
-    return lo - 1;
-}
+// Per-source-cell node lists written by the pattern pass and read by the fill pass (library-owned scratch):
+// the node ids m = c*(n_p*n_q) + a*n_q + b of the nodes that hit the grid, sorted by (rank of target cell, m),
+// and the rank of the target at every sorted position.  Stride nnode per source cell.
+struct NodeLists {
+    unsigned short* sorted;     // [n_blk][nnode]
+    unsigned short* rkpos;      // [n_blk][nnode]
+    int* ntot;                  // [n_blk] nodes on the grid
+    int* hits;                  // [n_blk] hit cells H
+};
 
 struct CellGeom { double cp, hp, cq, hq; };
 
@@ -45,28 +48,46 @@ __device__ __forceinline__ CellGeom cell_geom(const double* pe, const double* qe
     return g;
 }
 
+// node id m -> (c, a, b), m = c*npq + a*n_q + b, by multiply-high with precomputed magic numbers (m*d < 2^32)
+__device__ __forceinline__ void split_node(const DevLattice& L, int m, int& c, int& a, int& b)
+{
+    const int npq = L.n_p * L.n_q;
+    c = L.mg_npq ? (int)__umulhi((unsigned)m, L.mg_npq) : m;        // magic 0 encodes divisor 1
+    const int ab = m - c * npq;
+    a = L.mg_nq ? (int)__umulhi((unsigned)ab, L.mg_nq) : ab;
+    b = ab - a * L.n_q;
+}
+
 // DESIGN.md sec. 3.1, exactly:  p = cp + hp*t_a ; q = cq + hq*t_b ; x = t_c ; pq = p*q
-//   P2 = (0.25*(p*p) + 0.5625*(q*q)) + 0.75*(pq*x) ;  Q2 = ((p*p) + 0.25*(q*q)) - pq*x ; clamp at 0 ; sqrt
-__device__ __forceinline__ void map_node(const CellGeom& g, double ta, double tb, double tc,
-                                         double& p, double& q, double& pp, double& qq)
+//   P2 = (0.25*(p*p) + 0.5625*(q*q)) + 0.75*(pq*x) ;  Q2 = ((p*p) + 0.25*(q*q)) - pq*x ; clamp at 0
+__device__ __forceinline__ void map_node_sq(const CellGeom& g, double ta, double tb, double tc,
+                                            double& p, double& q, double& P2, double& Q2)
 {
     p = __dadd_rn(g.cp, __dmul_rn(g.hp, ta));
     q = __dadd_rn(g.cq, __dmul_rn(g.hq, tb));
     const double pq = __dmul_rn(p, q), p2 = __dmul_rn(p, p), q2 = __dmul_rn(q, q), pqx = __dmul_rn(pq, tc);
-    double P2 = __dadd_rn(__dadd_rn(__dmul_rn(0.25, p2), __dmul_rn(0.5625, q2)), __dmul_rn(0.75, pqx));
-    double Q2 = __dsub_rn(__dadd_rn(p2, __dmul_rn(0.25, q2)), pqx);
+    P2 = __dadd_rn(__dadd_rn(__dmul_rn(0.25, p2), __dmul_rn(0.5625, q2)), __dmul_rn(0.75, pqx));
+    Q2 = __dsub_rn(__dadd_rn(p2, __dmul_rn(0.25, q2)), pqx);
     P2 = P2 < 0.0 ? 0.0 : P2;
     Q2 = Q2 < 0.0 ? 0.0 : Q2;
-    pp = __dsqrt_rn(P2);
-    qq = __dsqrt_rn(Q2);
 }
 
-// target cell of a mapped node, or -1 (outside the grid, or p' = 0 / q' = 0): readings R5, R6
-__device__ __forceinline__ int target_cell(const double* s_pe, int pe_pad, int Np, const double* s_qe, int qe_pad, int Nq,
-                                           double pp, double qq)
+// number of thresholds <= v, minus one; thr has `pad` (power of two) entries, the tail filled with +inf
+__device__ __forceinline__ int locate(const double* __restrict__ thr, int pad, double v)
 {
-    const int ic = locate(s_pe, pe_pad, pp), jc = locate(s_qe, qe_pad, qq);
-    const bool ok = (ic >= 0) & (ic < Np) & (jc >= 0) & (jc < Nq) & (pp != 0.0) & (qq != 0.0);
+    int lo = 0;
+#pragma unroll 1
+    for (int s = pad >> 1; s > 0; s >>= 1) lo += (thr[lo + s - 1] <= v) ? s : 0;
+    lo += (thr[lo] <= v) ? 1 : 0;          // entries beyond N+1 are +inf, so lo <= N+1
+    return lo - 1;
+}
+
+// target cell of a mapped node, or -1 (outside the grid, or p' = 0 / q' = 0): readings R5, R6.  sqrt(y) = 0 <=> y = 0.
+__device__ __forceinline__ int target_cell_sq(const double* thr_p, int pe_pad, int Np, const double* thr_q, int qe_pad, int Nq,
+                                              double P2, double Q2)
+{
+    const int ic = locate(thr_p, pe_pad, P2), jc = locate(thr_q, qe_pad, Q2);
+    const bool ok = (ic >= 0) & (ic < Np) & (jc >= 0) & (jc < Nq) & (P2 != 0.0) & (Q2 != 0.0);
     return ok ? ic * Nq + jc : -1;
 }
 
@@ -98,6 +119,21 @@ __device__ inline int block_exclusive_scan(int* data, int n, int* scratch)
     const int total = scratch[T];
     __syncthreads();
     return total;
+}
+
+// hit bitset of one source cell with word-prefix popcounts (ranks of the hit cells)
+struct HitSet { unsigned* bits; int* wpre; int* scratch; };
+
+__device__ inline int rank_bits_n(int n_words, const HitSet& s)
+{
+    for (int k = threadIdx.x; k < n_words; k += blockDim.x) s.wpre[k] = __popc(s.bits[k]);
+    __syncthreads();
+    return block_exclusive_scan(s.wpre, n_words, s.scratch);
+}
+
+__device__ __forceinline__ int rank_of(const HitSet& s, int t)
+{
+    return s.wpre[t >> 5] + __popc(s.bits[t >> 5] & ((1u << (t & 31)) - 1u));
 }
 
 }  // namespace pm

@@ -13,12 +13,12 @@ namespace {
 
 constexpr int kSmemLimit = 227 * 1024;
 
-using FillKernel = void (*)(DevLattice, FillSmem, int, int, int, const int64_t*, double*, double*);
+using FillKernel = void (*)(DevLattice, FillSmem, NodeLists, int, int, int, const int64_t*, double*, double*);
 
 struct FillVariant { unsigned long long hash; int nw; FillKernel fn; const char* name; };
 
-#define PM_SPEC(S) {gen::S::kHash, 4, k_fill_seg<gen::S, 4>, #S}, {gen::S::kHash, 8, k_fill_seg<gen::S, 8>, #S}, \
-                   {gen::S::kHash, 12, k_fill_seg<gen::S, 12>, #S},
+#define PM_SPEC(S) {gen::S::kHash, 4, k_fill_seg<gen::S, 4>, #S}, {gen::S::kHash, 6, k_fill_seg<gen::S, 6>, #S}, \
+                   {gen::S::kHash, 8, k_fill_seg<gen::S, 8>, #S}, {gen::S::kHash, 12, k_fill_seg<gen::S, 12>, #S},
 const FillVariant kVariants[] = {
     PM_SPEC_LIST
     {0ull, 4, k_fill_seg<SpecGeneric, 4>, "generic"}, {0ull, 8, k_fill_seg<SpecGeneric, 8>, "generic"},
@@ -67,13 +67,14 @@ cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int hmax, in
     return cudaSuccess;
 }
 
-cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, int hmax, const int64_t* rowptr,
-                        double* vals, double* accG, cudaStream_t st)
+cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl, int hmax,
+                        const int64_t* rowptr, double* vals, double* accG, cudaStream_t st)
 {
     const int grid = n_blk < F.grid ? n_blk : F.grid;
     DevLattice Lc = L;
     FillSmem S = F.smem;
-    void* args[] = {&Lc, &S, &cell_begin, &n_blk, &hmax, (void*)&rowptr, &vals, &accG};
+    NodeLists N = nl;
+    void* args[] = {&Lc, &S, &N, &cell_begin, &n_blk, &hmax, (void*)&rowptr, &vals, &accG};
     cudaError_t e = cudaLaunchKernel(F.fn, dim3((unsigned)grid), dim3((unsigned)(F.nw * 32)), args, (size_t)S.total, st);
     count_launch();
     return e != cudaSuccess ? e : cudaGetLastError();

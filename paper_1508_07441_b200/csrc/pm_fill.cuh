@@ -1,10 +1,8 @@
 // pm_fill.cuh — the fill pass (hot-path step a7; the paper's step 2b).
 //
 // One persistent CTA per SM slot walks source cells D_ij.  Per source cell:
-//   A  map    every node (c-major node ids) -> target cell from p'^2, q'^2 against sqrt-thresholds of the edges
-//             (bit-identical decisions to "sqrt, then compare with the edges"), hit bitset
-//   B  sort   ranks of the hit cells, stable counting sort of the node ids by rank: the sorted list is ordered by
-//             (target t, x-node c, a, b), so the nodes of one (t, c) pair are consecutive
+//   (the pattern pass has left the cell's node ids sorted by (target t, x-node c, a, b) in NodeLists, so the nodes
+//    of one (t, c) pair are consecutive; nothing is mapped or sorted again here)
 //   C  nodes  lane = node, 32 consecutive sorted nodes per warp step: omega, directions, the ket harmonics K[slot]
 //             (Spec::ket — generated straight-line code, registers only), K tile -> shared memory (XOR swizzle)
 //   D  sums   lane = slot: walks the 32 nodes of the tile, summing K over each (t, c) segment; at a segment end
@@ -31,7 +29,7 @@ constexpr int kFillMaxY = 45;
 // Table-driven ket code for channel sets without a generated kernel (slow: local arrays, table loads).
 struct SpecGeneric {
     static constexpr bool kStatic = false;
-    static constexpr int NS = kFillMaxSlot, NF = kFillMaxFun, NCH = kFillMaxFun / 32;
+    static constexpr int NS = kFillMaxSlot, NF = kFillMaxFun, NCH = kFillMaxFun / 32, MAXM = 99;
     static constexpr unsigned long long kHash = 0ull;
     static __device__ __noinline__ void ket(const DevLattice& L, double om, double uxa, double uza, double uxb, double uzb,
                                             double (&K)[NS])
@@ -48,13 +46,14 @@ struct SpecGeneric {
 };
 
 struct FillSmem {           // byte offsets into dynamic shared memory, computed on the host
-    int thr_p, thr_q, tp, tq, tx, sx, wx, wpa, wqb, bra, bits, wpre, rk, sorted, hitcell, start, hist, scratch,
-        tile, sseg, head, normk, k0, total;
+    int thr_p, thr_q, tp, tq, tx, sx, wx, wpa, wqb, bra, tile, tile_bytes, sseg, head, normk, k0, total;
 };
+
+constexpr int kTileStride = 33;        // double2 per K-tile row: 32 nodes + 1 pad (conflict-free rows and columns)
 
 inline int fill_align16(int b) { return (b + 15) & ~15; }
 
-// shared-memory plan for NW warps; ns = slots, nf = functions
+// shared-memory plan for nw warps
 inline FillSmem fill_smem_plan(const DevLattice& L, int hmax, int nw)
 {
     FillSmem s{};
@@ -63,14 +62,12 @@ inline FillSmem fill_smem_plan(const DevLattice& L, int hmax, int nw)
     s.thr_p = take(8 * L.pe_pad); s.thr_q = take(8 * L.qe_pad);
     s.tp = take(8 * L.n_p); s.tq = take(8 * L.n_q); s.tx = take(8 * L.n_x); s.sx = take(8 * L.n_x); s.wx = take(8 * L.n_x);
     s.wpa = take(8 * L.n_p); s.wqb = take(8 * L.n_q);
-    s.bra = take(8 * L.n_x * L.n_slot);
-    s.bits = take(4 * L.n_words); s.wpre = take(4 * L.n_words);
-    s.rk = take(2 * L.nnode); s.sorted = take(2 * (L.nnode + 1));
-    s.hitcell = take(4 * hmax); s.start = take(4 * (hmax + 1)); s.hist = take(4 * nw * hmax);
-    s.scratch = take(4 * (nw * 32 + 1));
-    const int tile_tgt = 4 * L.nnode, tile_k = 8 * 32 * L.n_slot * nw;       // union: tgt[nnode] (A, B) / K tiles (C, D)
-    s.tile = take(tile_tgt > tile_k ? tile_tgt : tile_k);
-    s.sseg = take(8 * L.n_slot * nw);
+    s.bra = take(8 * L.n_x * (L.n_slot + 1));       // rows padded with one zero slot
+    const int np = (L.n_slot + 1) / 2;              // slot pairs
+    s.tile_bytes = 16 * kTileStride * np * nw;      // K tiles (phases C, D); staging of target sums (phase E)
+    if (s.tile_bytes < 8 * L.n_fun) s.tile_bytes = 8 * L.n_fun;
+    s.tile = take(s.tile_bytes);
+    s.sseg = take(16 * np * nw);
     s.head = take(8 * L.n_fun * nw);
     s.normk = take(8 * hmax);
     s.k0 = take(4 * (2 * nw + 2));
@@ -78,92 +75,28 @@ inline FillSmem fill_smem_plan(const DevLattice& L, int hmax, int nw)
     return s;
 }
 
-// number of thresholds <= v, minus one, by integer comparison of the bit patterns (valid for v >= +0; a negative
-// pattern, i.e. -0.0, sorts below every threshold).  thr has `pad` (power of two) entries, tail = +inf.
-__device__ __forceinline__ int locate_bits(const long long* __restrict__ thr, int pad, long long v)
-{
-    int lo = 0;
-#pragma unroll 1
-    for (int s = pad >> 1; s > 0; s >>= 1) lo += (thr[lo + s - 1] <= v) ? s : 0;
-    lo += (thr[lo] <= v) ? 1 : 0;
-    return lo - 1;
-}
-
-// exact node map up to p'^2, q'^2 (every operation a single IEEE double operation)
-__device__ __forceinline__ void map_node_sq(const CellGeom& g, double ta, double tb, double tc,
-                                            double& p, double& q, double& P2, double& Q2)
-{
-    p = __dadd_rn(g.cp, __dmul_rn(g.hp, ta));
-    q = __dadd_rn(g.cq, __dmul_rn(g.hq, tb));
-    const double pq = __dmul_rn(p, q), p2 = __dmul_rn(p, p), q2 = __dmul_rn(q, q), pqx = __dmul_rn(pq, tc);
-    P2 = __dadd_rn(__dadd_rn(__dmul_rn(0.25, p2), __dmul_rn(0.5625, q2)), __dmul_rn(0.75, pqx));
-    Q2 = __dsub_rn(__dadd_rn(p2, __dmul_rn(0.25, q2)), pqx);
-    P2 = P2 < 0.0 ? 0.0 : P2;
-    Q2 = Q2 < 0.0 ? 0.0 : Q2;
-}
-
-__device__ __forceinline__ int target_cell_sq(const long long* thr_p, int pe_pad, int Np, const long long* thr_q, int qe_pad,
-                                              int Nq, double P2, double Q2)
-{
-    const int ic = locate_bits(thr_p, pe_pad, __double_as_longlong(P2)), jc = locate_bits(thr_q, qe_pad, __double_as_longlong(Q2));
-    const bool ok = (ic >= 0) & (ic < Np) & (jc >= 0) & (jc < Nq) & (P2 != 0.0) & (Q2 != 0.0);   // sqrt(y) = 0 <=> y = 0
-    return ok ? ic * Nq + jc : -1;
-}
-
-// hit bitset of one source cell with word-prefix popcounts (ranks of the hit cells)
-struct HitSet { unsigned* bits; int* wpre; int* scratch; };
-
-__device__ inline int rank_bits_n(int n_words, const HitSet& s)
-{
-    for (int k = threadIdx.x; k < n_words; k += blockDim.x) s.wpre[k] = __popc(s.bits[k]);
-    __syncthreads();
-    return block_exclusive_scan(s.wpre, n_words, s.scratch);
-}
-
-__device__ __forceinline__ int rank_of(const HitSet& s, int t)
-{
-    return s.wpre[t >> 5] + __popc(s.bits[t >> 5] & ((1u << (t & 31)) - 1u));
-}
-
-__device__ inline void list_hits_n(int n_words, const HitSet& s, int* hitcell)
-{
-    for (int k = threadIdx.x; k < n_words; k += blockDim.x) {
-        unsigned w = s.bits[k];
-        int r = s.wpre[k];
-        while (w) { const int b = __ffs(w) - 1; hitcell[r++] = (k << 5) + b; w &= w - 1; }
-    }
-}
-
 template <class Spec, int NW>
 __global__ void __launch_bounds__(NW * 32, 1)
-k_fill_seg(DevLattice L, FillSmem S, int cell_begin, int n_blk, int hmax, const int64_t* __restrict__ rowptr,
+k_fill_seg(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, int hmax, const int64_t* __restrict__ rowptr,
            double* __restrict__ vals, double* __restrict__ accG)
 {
     constexpr int T = NW * 32;
-    constexpr int NSC = (Spec::NS + 31) / 32;           // slot chunks of the lane = slot walk
+    constexpr int NP = (Spec::NS + 1) / 2;              // slot pairs (one double2 per pair and node in the K tile)
+    constexpr int NPC = (NP + 31) / 32;                 // pair chunks of the lane = slot-pair walk
     constexpr int NCH = Spec::NCH;                      // function chunks of the lane = function stage
     extern __shared__ __align__(16) char smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int ns = Spec::kStatic ? Spec::NS : L.n_slot, nf = L.n_fun;
-    const int npq = L.n_p * L.n_q;
+    const int ns = Spec::kStatic ? Spec::NS : L.n_slot, nf = L.n_fun, np = (ns + 1) >> 1;
 
-    long long* s_thr_p = (long long*)(smem + S.thr_p);
-    long long* s_thr_q = (long long*)(smem + S.thr_q);
+    double* s_thr_p = (double*)(smem + S.thr_p);
+    double* s_thr_q = (double*)(smem + S.thr_q);
     double* s_tp = (double*)(smem + S.tp);   double* s_tq = (double*)(smem + S.tq);   double* s_tx = (double*)(smem + S.tx);
     double* s_sx = (double*)(smem + S.sx);   double* s_wx = (double*)(smem + S.wx);
     double* s_wpa = (double*)(smem + S.wpa); double* s_wqb = (double*)(smem + S.wqb);
     double* s_bra = (double*)(smem + S.bra);
-    unsigned* s_bits = (unsigned*)(smem + S.bits);
-    int* s_wpre = (int*)(smem + S.wpre);
-    unsigned short* s_rk = (unsigned short*)(smem + S.rk);
-    unsigned short* s_sorted = (unsigned short*)(smem + S.sorted);
-    int* s_hitcell = (int*)(smem + S.hitcell);
-    int* s_start = (int*)(smem + S.start);
-    int* s_hist = (int*)(smem + S.hist);
-    int* s_scratch = (int*)(smem + S.scratch);
-    int* s_tgt = (int*)(smem + S.tile);
-    double* s_tile = (double*)(smem + S.tile) + (size_t)warp * 32 * ns;
-    double* s_sseg = (double*)(smem + S.sseg) + warp * ns;
+    double2* s_tile = (double2*)(smem + S.tile) + (size_t)warp * kTileStride * np;
+    double2* s_sseg2 = (double2*)(smem + S.sseg) + warp * np;
+    const double* s_sseg = (const double*)s_sseg2;
     double* s_head = (double*)(smem + S.head);
     double* s_normk = (double*)(smem + S.normk);
     int* s_k0 = (int*)(smem + S.k0);                   // [NW] first target of each warp range, then [NW+1] range starts
@@ -175,107 +108,86 @@ k_fill_seg(DevLattice L, FillSmem S, int cell_begin, int n_blk, int hmax, const 
     for (int k = tid; k < L.n_p; k += T) s_tp[k] = L.tp[k];
     for (int k = tid; k < L.n_q; k += T) s_tq[k] = L.tq[k];
     for (int k = tid; k < L.n_x; k += T) { s_tx[k] = L.tx[k]; s_sx[k] = L.sx[k]; s_wx[k] = L.wx[k]; }
-    for (int k = tid; k < L.n_x * ns; k += T) s_bra[k] = L.bra[k];
-    int fd[NCH];                                        // sa | sb << 8 | nM << 16 of function f = ch*32 + lane
+    const int nsb = ns + 1;                             // bra rows carry one trailing zero slot (index ns)
+    for (int k = tid; k < L.n_x * nsb; k += T) { const int c = k / nsb, sl = k - c * nsb; s_bra[k] = sl < ns ? L.bra[c * ns + sl] : 0.0; }
+    // per-lane descriptors of function f = ch*32 + lane.  kPacked (at most 3 M-terms per function): byte i of fa / fb =
+    // bra / ket slot of term i, unused terms point at the zero bra slot; else fa = sa | sb << 8 | nM << 16.
+    constexpr bool kPacked = Spec::MAXM <= 3;
+    int fa[NCH], fb[NCH];
 #pragma unroll
     for (int ch = 0; ch < NCH; ++ch) {
         const int f = ch * 32 + lane;
-        fd[ch] = 0;
-        if (f < nf) { const int4 fn = L.fun[f]; fd[ch] = fn.x | (fn.y << 8) | (fn.z << 16); }
+        fa[ch] = kPacked ? (ns | (ns << 8) | (ns << 16)) : 0;
+        fb[ch] = 0;
+        if (f < nf) {
+            const int4 fn = L.fun[f];
+            if (kPacked) {
+                fa[ch] = 0;
+                for (int i = 0; i < 3; ++i) {
+                    fa[ch] |= (i < fn.z ? fn.x + i : ns) << (8 * i);
+                    fb[ch] |= (i < fn.z ? fn.y + i : 0) << (8 * i);
+                }
+            } else fa[ch] = fn.x | (fn.y << 8) | (fn.z << 16);
+        }
     }
     double* accS = accG + (size_t)blockIdx.x * hmax * nf;
-    HitSet st;
-    st.bits = s_bits; st.wpre = s_wpre; st.scratch = s_scratch;
 
     for (int cb = blockIdx.x; cb < n_blk; cb += gridDim.x) {
         const int cell = cell_begin + cb;
         const int ci = cell / L.Nq, cj = cell - ci * L.Nq;
         const CellGeom g = cell_geom(L.pe, L.qe, ci, cj);
+        const int H = nl.hits[cb], ntot = nl.ntot[cb];
+        const unsigned short* __restrict__ g_sorted = nl.sorted + (size_t)cb * L.nnode;
+        const unsigned short* __restrict__ g_rkpos = nl.rkpos + (size_t)cb * L.nnode;
         __syncthreads();                                // previous cell's phase E is done with shared memory
-        for (int k = tid; k < L.n_words; k += T) s_bits[k] = 0u;
         for (int k = tid; k < L.n_p; k += T) s_wpa[k] = __dmul_rn(g.hp, L.wp[k]);
         for (int k = tid; k < L.n_q; k += T) s_wqb[k] = __dmul_rn(g.hq, L.wq[k]);
-        for (int k = tid; k < NW * hmax; k += T) s_hist[k] = 0;
-        __syncthreads();
-
-        // ---- A: map (node id m = c*npq + a*n_q + b)
-        for (int m = tid; m < L.nnode; m += T) {
-            const int c = m / npq, ab = m - c * npq, a = ab / L.n_q, b = ab - a * L.n_q;
-            double p, q, P2, Q2;
-            map_node_sq(g, s_tp[a], s_tq[b], s_tx[c], p, q, P2, Q2);
-            const int t = target_cell_sq(s_thr_p, L.pe_pad, L.Np, s_thr_q, L.qe_pad, L.Nq, P2, Q2);
-            if (t >= 0) atomicOr(&s_bits[t >> 5], 1u << (t & 31));
-            s_tgt[m] = t;
-        }
-        __syncthreads();
-        const int H = rank_bits_n(L.n_words, st);
-        if (H > hmax) continue;                         // cannot happen: hmax comes from pm_pattern of this block
-        list_hits_n(L.n_words, st, s_hitcell);
-
-        // ---- B: stable counting sort of node ids by rank; each warp owns a contiguous slice of ids
-        const int slice = (((L.nnode + NW - 1) / NW) + 31) & ~31;
-        const int nb = warp * slice, ne = min(nb + slice, L.nnode);
-        for (int m = nb + lane; m < ne; m += 32) {
-            const int t = s_tgt[m];
-            const int r = (t >= 0) ? rank_of(st, t) : 0xffff;
-            s_rk[m] = (unsigned short)r;
-            if (t >= 0) atomicAdd(&s_hist[warp * hmax + r], 1);
-        }
-        __syncthreads();
-        for (int k = tid; k < H; k += T) {
-            int tot = 0;
-            for (int w = 0; w < NW; ++w) tot += s_hist[w * hmax + k];
-            s_start[k] = tot;
-        }
-        if (tid == 0) s_start[H] = 0;
-        __syncthreads();
-        block_exclusive_scan(s_start, H + 1, s_scratch);
-        for (int k = tid; k < H; k += T) {
-            int run = s_start[k];
-            for (int w = 0; w < NW; ++w) { const int v = s_hist[w * hmax + k]; s_hist[w * hmax + k] = run; run += v; }
-        }
-        __syncthreads();
-        for (int m0 = nb; m0 < ne; m0 += 32) {
-            const int m = m0 + lane;
-            const int key = (m < ne) ? (int)s_rk[m] : 0xffff;
-            const unsigned same = __match_any_sync(0xffffffffu, key);
-            if (key != 0xffff) {
-                const int pos = s_hist[warp * hmax + key] + __popc(same & ((1u << lane) - 1u));
-                s_sorted[pos] = (unsigned short)m;
-            }
-            __syncwarp();
-            if (key != 0xffff && lane == (__ffs(same) - 1)) s_hist[warp * hmax + key] += __popc(same);
-            __syncwarp();
-        }
-        const int ntot = s_start[H];
-        // warp ranges over the sorted list, in whole 32-node steps
+        // warp ranges over the sorted list, in whole 32-node steps; first target of each range
         if (tid <= NW) { const int G = (ntot + 31) >> 5; s_wbeg[tid] = min(ntot, ((int)(((long long)tid * G) / NW)) << 5); }
-        __syncthreads();                                // sorted[], rk[] complete; tgt[] dead from here (tile reuse)
+        // normalisation of every target: its first node is mapped again (exact arithmetic: the same cell)
+        {
+            const double dsrc = (L.pe[ci + 1] - L.pe[ci]) * (L.qe[cj + 1] - L.qe[cj]);
+            for (int pos = tid; pos < ntot; pos += T) {
+                const int r = g_rkpos[pos];
+                if (pos > 0 && g_rkpos[pos - 1] == r) continue;
+                int c, a, b;
+                split_node(L, g_sorted[pos], c, a, b);
+                double p, q, P2, Q2;
+                map_node_sq(g, s_tp[a], s_tq[b], s_tx[c], p, q, P2, Q2);
+                const int hc = target_cell_sq(s_thr_p, L.pe_pad, L.Np, s_thr_q, L.qe_pad, L.Nq, P2, Q2);
+                const int ic = hc / L.Nq, jc = hc - ic * L.Nq;
+                s_normk[r] = 1.0 / sqrt(dsrc * ((L.pe[ic + 1] - L.pe[ic]) * (L.qe[jc + 1] - L.qe[jc])));
+            }
+        }
+        __syncthreads();
         const int wb = s_wbeg[warp], we = s_wbeg[warp + 1];
-        const int k0 = (wb < we) ? (int)s_rk[s_sorted[wb]] : -1;
+        const int k0 = (wb < we) ? (int)g_rkpos[wb] : -1;
         if (lane == 0) s_k0[warp] = k0;
 
-        // ---- C + D: 32 sorted nodes per step
+        // ---- C + D: 32 sorted nodes per step; the node ids of the next two steps are already in flight
         double runT[NCH];
 #pragma unroll
         for (int ch = 0; ch < NCH; ++ch) runT[ch] = 0.0;
-        double runS[NSC];
+        double2 runS[NPC];
 #pragma unroll
-        for (int i = 0; i < NSC; ++i) runS[i] = 0.0;
+        for (int i = 0; i < NPC; ++i) runS[i] = make_double2(0.0, 0.0);
+        int mC = 0, rC = -1, mN = 0, rN = -1;           // this step's and the next step's node id / target rank (-1: none)
+        if (wb + lane < we) { mC = g_sorted[wb + lane]; rC = g_rkpos[wb + lane]; }
+        if (wb + 32 + lane < we) { mN = g_sorted[wb + 32 + lane]; rN = g_rkpos[wb + 32 + lane]; }
         for (int base = wb; base < we; base += 32) {
-            const int pos = base + lane;
-            const bool active = pos < we;
-            const int m = s_sorted[active ? pos : wb];
-            const int c = m / npq, ab = m - c * npq, a = ab / L.n_q, b = ab - a * L.n_q;
-            const int rkv = s_rk[m];
-            // segment ends: (t, c) changes after this node, or the tile ends; target ends: t changes / range ends
-            bool tend = false, send = false;
-            if (active) {
-                const bool last = (pos + 1 >= we);
-                const int m1 = s_sorted[last ? pos : pos + 1];
-                tend = last || ((int)s_rk[m1] != rkv);
-                send = tend || (m1 / npq != c) || lane == 31;
-            }
+            int mF = 0, rF = -1;
+            if (base + 64 + lane < we) { mF = g_sorted[base + 64 + lane]; rF = g_rkpos[base + 64 + lane]; }
+            const bool active = rC >= 0;
+            int c, a, b;
+            split_node(L, mC, c, a, b);
+            // the node after this one (next lane, or lane 0 of the next step); rank -1 past the end of the range
+            int m1 = __shfl_down_sync(0xffffffffu, mC, 1), r1 = __shfl_down_sync(0xffffffffu, rC, 1);
+            const int m1n = __shfl_sync(0xffffffffu, mN, 0), r1n = __shfl_sync(0xffffffffu, rN, 0);
+            if (lane == 31) { m1 = m1n; r1 = r1n; }
+            const int c1 = L.mg_npq ? (int)__umulhi((unsigned)m1, L.mg_npq) : m1;
+            // target ends: t changes after this node (or the range ends); segment ends: (t, c) changes
+            const bool tend = active && (r1 != rC);
+            const bool send = active && (tend || c1 != c);
             const unsigned tmask = __ballot_sync(0xffffffffu, tend), smask = __ballot_sync(0xffffffffu, send);
             const int cnt = min(32, we - base);
             {
@@ -295,38 +207,67 @@ k_fill_seg(DevLattice L, FillSmem S, int cell_begin, int n_blk, int hmax, const 
                 Spec::ket(L, om, ax * ra, az * ra, bx * rb, bz * rb, K);
                 if (Spec::kStatic) {
 #pragma unroll
-                    for (int s = 0; s < Spec::NS; ++s) s_tile[s * 32 + (lane ^ (s & 31))] = K[s];
+                    for (int i = 0; i < NP; ++i)
+                        s_tile[i * kTileStride + lane] = make_double2(K[2 * i], (2 * i + 1 < Spec::NS) ? K[(2 * i + 1) % Spec::NS] : 0.0);
                 } else {
-                    for (int s = 0; s < ns; ++s) s_tile[s * 32 + (lane ^ (s & 31))] = K[s];
+                    for (int i = 0; i < np; ++i)
+                        s_tile[i * kTileStride + lane] = make_double2(K[2 * i], (2 * i + 1 < ns) ? K[2 * i + 1] : 0.0);
                 }
             }
             __syncwarp();
-            // lane = slot walk over the tile's nodes
-            for (int j = 0; j < cnt; ++j) {
+            // lane = slot pair: walks the tile's nodes, up to 4 per step, never across a segment end
+            for (int j = 0; j < cnt;) {
+                const int nbnd = __ffs((smask >> j) & 0xfu);             // 1-based offset of the next segment end, 0 = none in 4
+                const int step = nbnd ? nbnd : min(4, cnt - j);
+                if (step == 4) {
 #pragma unroll
-                for (int i = 0; i < NSC; ++i) {
-                    const int s = i * 32 + lane;
-                    if (s < ns) runS[i] += s_tile[s * 32 + (j ^ lane)];
+                    for (int i = 0; i < NPC; ++i) {
+                        const int sp = i * 32 + lane;
+                        if (sp < np) {
+                            const double2* row = s_tile + sp * kTileStride + j;
+                            const double2 d0 = row[0], d1 = row[1], d2 = row[2], d3 = row[3];
+                            runS[i].x += (d0.x + d1.x) + (d2.x + d3.x);
+                            runS[i].y += (d0.y + d1.y) + (d2.y + d3.y);
+                        }
+                    }
+                } else {
+                    for (int r = 0; r < step; ++r) {
+#pragma unroll
+                        for (int i = 0; i < NPC; ++i) {
+                            const int sp = i * 32 + lane;
+                            if (sp < np) { const double2 d = s_tile[sp * kTileStride + j + r]; runS[i].x += d.x; runS[i].y += d.y; }
+                        }
+                    }
                 }
-                if ((smask >> j) & 1u) {
+                j += step;
+                if (nbnd) {                                              // node jb ends a (t, c) segment
+                    const int jb = j - 1;
 #pragma unroll
-                    for (int i = 0; i < NSC; ++i) {
-                        const int s = i * 32 + lane;
-                        if (s < ns) s_sseg[s] = runS[i];
-                        runS[i] = 0.0;
+                    for (int i = 0; i < NPC; ++i) {
+                        const int sp = i * 32 + lane;
+                        if (sp < np) s_sseg2[sp] = runS[i];
+                        runS[i] = make_double2(0.0, 0.0);
                     }
                     __syncwarp();
-                    const int cseg = __shfl_sync(0xffffffffu, c, j);
-                    const double* bra = s_bra + cseg * ns;
+                    const int cseg = __shfl_sync(0xffffffffu, c, jb);
+                    const double* bra = s_bra + cseg * nsb;
 #pragma unroll
                     for (int ch = 0; ch < NCH; ++ch) {
-                        const int sa = fd[ch] & 255, sb = (fd[ch] >> 8) & 255, nM = fd[ch] >> 16;
-                        double v = 0.0;
-                        for (int i = 0; i < nM; ++i) v = fma(bra[sa + i], s_sseg[sb + i], v);
-                        runT[ch] += v;
+                        if (kPacked) {
+                            const int ia = fa[ch], ib = fb[ch];
+                            double v = bra[ia & 255] * s_sseg[ib & 255];
+                            v = fma(bra[(ia >> 8) & 255], s_sseg[(ib >> 8) & 255], v);
+                            v = fma(bra[ia >> 16], s_sseg[ib >> 16], v);
+                            runT[ch] += v;
+                        } else {
+                            const int sa = fa[ch] & 255, sb = (fa[ch] >> 8) & 255, nM = fa[ch] >> 16;
+                            double v = 0.0;
+                            for (int i = 0; i < nM; ++i) v = fma(bra[sa + i], s_sseg[sb + i], v);
+                            runT[ch] += v;
+                        }
                     }
-                    if ((tmask >> j) & 1u) {
-                        const int kseg = __shfl_sync(0xffffffffu, rkv, j);
+                    if ((tmask >> jb) & 1u) {                            // ... and ends target t: its sums are complete
+                        const int kseg = __shfl_sync(0xffffffffu, rC, jb);
                         double* dst = (kseg == k0) ? (s_head + warp * nf) : (accS + (size_t)kseg * nf);
 #pragma unroll
                         for (int ch = 0; ch < NCH; ++ch) {
@@ -339,49 +280,60 @@ k_fill_seg(DevLattice L, FillSmem S, int cell_begin, int n_blk, int hmax, const 
                 }
             }
             __syncwarp();
+            mC = mN; rC = rN; mN = mF; rN = rF;
         }
         __syncthreads();
 
-        // ---- targets shared by several warp ranges: add the range heads in warp order; per-target norms
+        // ---- targets shared by several warp ranges: add the range heads in warp order
+        for (int w = 0; w < NW; ++w) {
+            const int k = s_k0[w];
+            if (k < 0 || (w > 0 && s_k0[w - 1] == k)) continue;              // empty range, or not the first head of k
+            // k began in an earlier range (then accS[k] already holds that part) iff the node before this range is in k
+            const bool own = s_wbeg[w] > 0 && (int)g_rkpos[s_wbeg[w] - 1] == k;
+            for (int f = tid; f < nf; f += T) {
+                double sum = own ? accS[(size_t)k * nf + f] : 0.0;
+                for (int w2 = w; w2 < NW && s_k0[w2] == k; ++w2) sum += s_head[w2 * nf + f];
+                accS[(size_t)k * nf + f] = sum;
+            }
+        }
+        __syncthreads();
+
+        // ---- E: thread = output o = (alpha, m-th coupled alpha'); P = norm_k * sum_t c_t * acc_k[f_t].
+        // The sums of a chunk of targets are staged in shared memory (the K-tile area is free here).
         {
-            const double dsrc = (L.pe[ci + 1] - L.pe[ci]) * (L.qe[cj + 1] - L.qe[cj]);
-            for (int k = tid; k < H; k += T) {
-                const int hc = s_hitcell[k], ic = hc / L.Nq, jc = hc - ic * L.Nq;
-                s_normk[k] = 1.0 / sqrt(dsrc * ((L.pe[ic + 1] - L.pe[ic]) * (L.qe[jc + 1] - L.qe[jc])));
-            }
-            for (int w = 0; w < NW; ++w) {
-                const int k = s_k0[w];
-                if (k < 0 || (w > 0 && s_k0[w - 1] == k)) continue;          // empty range, or not the first head of k
-                const bool own = s_start[k] < s_wbeg[w];                     // k began in an earlier range: accS[k] was written
-                // (k began before range w but is w's first target only if the earlier warp wrote it as a non-head)
-                for (int f = tid; f < nf; f += T) {
-                    double sum = own ? accS[(size_t)k * nf + f] : 0.0;
-                    for (int w2 = w; w2 < NW && s_k0[w2] == k; ++w2) sum += s_head[w2 * nf + f];
-                    accS[(size_t)k * nf + f] = sum;
+            double* s_acc = (double*)(smem + S.tile);
+            const int kc = max(1, S.tile_bytes / (8 * nf));
+            for (int kb = 0; kb < H; kb += kc) {
+                const int ke = min(H, kb + kc), n = (ke - kb) * nf;
+                const double* src = accS + (size_t)kb * nf;
+                for (int idx = tid; idx < n; idx += T) s_acc[idx] = src[idx];
+                __syncthreads();
+                for (int o = tid; o < L.totcoup; o += T) {
+                    const int al = L.o_alpha[o], off = L.cl_off[al], nc = L.cl_off[al + 1] - off;
+                    const int t0 = L.ot_off[o], nt = L.ot_off[o + 1] - t0;
+                    double* out = vals + rowptr[(int64_t)cb * L.n_ch + al] + (o - off) + (size_t)kb * nc;
+                    double c0 = 0.0, c1 = 0.0, c2 = 0.0;
+                    int f0 = 0, f1 = 0, f2 = 0;
+                    if (nt > 0) { c0 = L.ot_c[t0]; f0 = L.ot_f[t0]; }
+                    if (nt > 1) { c1 = L.ot_c[t0 + 1]; f1 = L.ot_f[t0 + 1]; }
+                    if (nt > 2) { c2 = L.ot_c[t0 + 2]; f2 = L.ot_f[t0 + 2]; }
+                    if (nt <= 3) {
+#pragma unroll 4
+                        for (int k = 0; k < ke - kb; ++k) {
+                            const double* acc = s_acc + k * nf;
+                            const double v = fma(c2, acc[f2], fma(c1, acc[f1], c0 * acc[f0]));
+                            out[(size_t)k * nc] = v * s_normk[kb + k];
+                        }
+                    } else {
+                        for (int k = 0; k < ke - kb; ++k) {
+                            const double* acc = s_acc + k * nf;
+                            double v = fma(c2, acc[f2], fma(c1, acc[f1], c0 * acc[f0]));
+                            for (int t = 3; t < nt; ++t) v = fma(L.ot_c[t0 + t], acc[L.ot_f[t0 + t]], v);
+                            out[(size_t)k * nc] = v * s_normk[kb + k];
+                        }
+                    }
                 }
-            }
-        }
-        __syncthreads();
-
-        // ---- E: thread = output o = (alpha, m-th coupled alpha'); P = norm_k * sum_t c_t * acc_k[f_t]
-        for (int o = tid; o < L.totcoup; o += T) {
-            const int al = L.o_alpha[o], off = L.cl_off[al], nc = L.cl_off[al + 1] - off;
-            const int t0 = L.ot_off[o], nt = L.ot_off[o + 1] - t0;
-            double* out = vals + rowptr[(int64_t)cb * L.n_ch + al] + (o - off);
-            double c0 = 0.0, c1 = 0.0, c2 = 0.0, c3 = 0.0;
-            int f0 = 0, f1 = 0, f2 = 0, f3 = 0;
-            if (nt > 0) { c0 = L.ot_c[t0]; f0 = L.ot_f[t0]; }
-            if (nt > 1) { c1 = L.ot_c[t0 + 1]; f1 = L.ot_f[t0 + 1]; }
-            if (nt > 2) { c2 = L.ot_c[t0 + 2]; f2 = L.ot_f[t0 + 2]; }
-            if (nt > 3) { c3 = L.ot_c[t0 + 3]; f3 = L.ot_f[t0 + 3]; }
-            for (int k = 0; k < H; ++k) {
-                const double* acc = accS + (size_t)k * nf;
-                double v = c0 * acc[f0];
-                v = fma(c1, acc[f1], v);
-                v = fma(c2, acc[f2], v);
-                v = fma(c3, acc[f3], v);
-                for (int t = 4; t < nt; ++t) v = fma(L.ot_c[t0 + t], acc[L.ot_f[t0 + t]], v);
-                out[(size_t)k * nc] = v * s_normk[k];
+                __syncthreads();
             }
         }
     }

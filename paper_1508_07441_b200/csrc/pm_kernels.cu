@@ -1,24 +1,13 @@
-// pm_kernels.cu — CUDA kernels of libpm for sm_100a: pattern pass (a6), generic fill pass (a7), SpMV (a9).
+// pm_kernels.cu — CUDA kernels of libpm for sm_100a: pattern pass (a6), SpMV (a9), FP64 peak diagnostic.
 // One CTA per source cell D_ij; the node map and location live in pm_device.cuh.
-// Paper's prior art: one thread per pre-selected element or per cell pair (L376) with
-// constants in global memory (L341) and a CPU repack into CSR (L376).  Here all constants sit in shared
-// memory, a source cell's nodes are binned once and serve every channel pair, and the cell-major row order
-// makes every row segment contiguous, so no repack exists.
+// Paper's prior art: pre-selection of the nonzero elements by a separate GPU pass,
+// one thread per element, constants in global memory (L341), CPU repack into CSR for coupled channels (L376).
+// Here the pattern pass bins every quadrature node ONCE: k_map_sort leaves, per source cell, the node ids sorted
+// by target cell (NodeLists); the column indices and the whole fill pass are driven by those lists, and the
+// cell-major row order makes every row segment contiguous, so no repack exists.
 #include "pm_kernels.cuh"
 
-#include "pm_ylm.h"
-
 namespace pm {
-
-// ------------------------------------------------------------------------------------------------
-// Shared-memory staging common to pattern and fill: edges, rules, hit bitset.
-// ------------------------------------------------------------------------------------------------
-struct Stage {
-    double *pe, *qe, *tp, *tq, *tx;
-    unsigned* bits;      // n_words hit bitset of this source cell
-    int* wpre;           // n_words exclusive prefix popcounts
-    int* scratch;        // blockDim+1
-};
 
 __device__ __forceinline__ char* carve(char*& p, size_t bytes)
 {
@@ -27,86 +16,111 @@ __device__ __forceinline__ char* carve(char*& p, size_t bytes)
     return r;
 }
 
-__device__ inline Stage stage_common(const DevLattice& L, char*& sp)
-{
-    Stage s;
-    s.pe = (double*)carve(sp, sizeof(double) * L.pe_pad);
-    s.qe = (double*)carve(sp, sizeof(double) * L.qe_pad);
-    s.tp = (double*)carve(sp, sizeof(double) * L.n_p);
-    s.tq = (double*)carve(sp, sizeof(double) * L.n_q);
-    s.tx = (double*)carve(sp, sizeof(double) * L.n_x);
-    s.bits = (unsigned*)carve(sp, sizeof(unsigned) * L.n_words);
-    s.wpre = (int*)carve(sp, sizeof(int) * L.n_words);
-    s.scratch = (int*)carve(sp, sizeof(int) * (blockDim.x + 1));
-    for (int k = threadIdx.x; k < L.pe_pad; k += blockDim.x) s.pe[k] = L.pe[k];
-    for (int k = threadIdx.x; k < L.qe_pad; k += blockDim.x) s.qe[k] = L.qe[k];
-    for (int k = threadIdx.x; k < L.n_p; k += blockDim.x) s.tp[k] = L.tp[k];
-    for (int k = threadIdx.x; k < L.n_q; k += blockDim.x) s.tq[k] = L.tq[k];
-    for (int k = threadIdx.x; k < L.n_x; k += blockDim.x) s.tx[k] = L.tx[k];
-    for (int k = threadIdx.x; k < L.n_words; k += blockDim.x) s.bits[k] = 0u;
-    return s;
-}
-
-// size in bytes of what stage_common carves (host mirror)
-size_t stage_bytes(const DevLattice& L, int threads)
-{
-    auto al = [](size_t b) { return (b + 15) & ~size_t(15); };
-    return al(8 * (size_t)L.pe_pad) + al(8 * (size_t)L.qe_pad) + al(8 * (size_t)L.n_p) + al(8 * (size_t)L.n_q)
-         + al(8 * (size_t)L.n_x) + 2 * al(4 * (size_t)L.n_words) + al(4 * (size_t)(threads + 1));
-}
-
-// Map every node of source cell `cell`, mark its target in the bitset and (optionally) record it.
-template <bool kRecord>
-__device__ inline void map_cell(const DevLattice& L, const Stage& s, int cell, int* tgt)
-{
-    const int i = cell / L.Nq, j = cell - i * L.Nq;
-    const CellGeom g = cell_geom(s.pe, s.qe, i, j);
-    const int nqx = L.n_q * L.n_x;
-    for (int n = threadIdx.x; n < L.nnode; n += blockDim.x) {
-        const int a = n / nqx, r = n - a * nqx, b = r / L.n_x, c = r - b * L.n_x;
-        double p, q, pp, qq;
-        map_node(g, s.tp[a], s.tq[b], s.tx[c], p, q, pp, qq);
-        const int t = target_cell(s.pe, L.pe_pad, L.Np, s.qe, L.qe_pad, L.Nq, pp, qq);
-        if (t >= 0) atomicOr(&s.bits[t >> 5], 1u << (t & 31));
-        if (kRecord) tgt[n] = t;
-    }
-}
-
-// popcount prefix over the bitset words; returns the number of hit cells H
-__device__ inline int rank_bits(const DevLattice& L, const Stage& s)
-{
-    for (int k = threadIdx.x; k < L.n_words; k += blockDim.x) s.wpre[k] = __popc(s.bits[k]);
-    __syncthreads();
-    return block_exclusive_scan(s.wpre, L.n_words, s.scratch);
-}
-
-__device__ __forceinline__ int rank_of(const Stage& s, int t)
-{
-    return s.wpre[t >> 5] + __popc(s.bits[t >> 5] & ((1u << (t & 31)) - 1u));
-}
-
-__device__ inline void list_hits(const DevLattice& L, const Stage& s, int* hitcell)
-{
-    for (int k = threadIdx.x; k < L.n_words; k += blockDim.x) {
-        unsigned w = s.bits[k];
-        int r = s.wpre[k];
-        while (w) { const int b = __ffs(w) - 1; hitcell[r++] = (k << 5) + b; w &= w - 1; }
-    }
-}
+static size_t al16(size_t b) { return (b + 15) & ~size_t(15); }
 
 // ------------------------------------------------------------------------------------------------
-// Pattern pass, kernel A: number of hit cells per source cell.
+// Pattern pass, kernel A: map every node of a source cell, rank the hit cells, stable counting sort of the
+// node ids by rank.  Node id m = c*(n_p*n_q) + a*n_q + b, so the sorted list is ordered by (target, x-node, a, b).
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kThreads) k_count_hits(DevLattice L, int cell_begin, int n_blk, int* __restrict__ hits)
+size_t map_sort_smem(const DevLattice& L)
+{
+    const int nw = kThreads / 32;
+    const int hcap = std::min(L.nnode, L.n_cells);
+    return al16(8 * (size_t)L.pe_pad) + al16(8 * (size_t)L.qe_pad) + al16(8 * (size_t)L.n_p) + al16(8 * (size_t)L.n_q)
+         + al16(8 * (size_t)L.n_x) + 2 * al16(4 * (size_t)L.n_words) + al16(4 * (size_t)(kThreads + 1))
+         + al16(4 * (size_t)L.nnode) + 2 * al16(2 * (size_t)L.nnode) + al16(4 * (size_t)(hcap + 1))
+         + al16(4 * (size_t)std::max(nw * std::min(hcap, kHitsFast), hcap));
+}
+
+__global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_begin, NodeLists nl)
 {
     extern __shared__ __align__(16) char smem[];
+    constexpr int T = kThreads, NW = kThreads / 32;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int hcap = min(L.nnode, L.n_cells);
     char* sp = smem;
-    Stage s = stage_common(L, sp);
+    double* s_thr_p = (double*)carve(sp, 8 * (size_t)L.pe_pad);
+    double* s_thr_q = (double*)carve(sp, 8 * (size_t)L.qe_pad);
+    double* s_tp = (double*)carve(sp, 8 * (size_t)L.n_p);
+    double* s_tq = (double*)carve(sp, 8 * (size_t)L.n_q);
+    double* s_tx = (double*)carve(sp, 8 * (size_t)L.n_x);
+    HitSet hs;
+    hs.bits = (unsigned*)carve(sp, 4 * (size_t)L.n_words);
+    hs.wpre = (int*)carve(sp, 4 * (size_t)L.n_words);
+    hs.scratch = (int*)carve(sp, 4 * (size_t)(T + 1));
+    int* s_tgt = (int*)carve(sp, 4 * (size_t)L.nnode);
+    unsigned short* s_sorted = (unsigned short*)carve(sp, 2 * (size_t)L.nnode);
+    unsigned short* s_rkpos = (unsigned short*)carve(sp, 2 * (size_t)L.nnode);
+    int* s_start = (int*)carve(sp, 4 * (size_t)(hcap + 1));
+    int* s_hist = (int*)carve(sp, 4 * (size_t)max(NW * min(hcap, kHitsFast), hcap));
+
+    for (int k = tid; k < L.pe_pad; k += T) s_thr_p[k] = L.thr_p[k];
+    for (int k = tid; k < L.qe_pad; k += T) s_thr_q[k] = L.thr_q[k];
+    for (int k = tid; k < L.n_p; k += T) s_tp[k] = L.tp[k];
+    for (int k = tid; k < L.n_q; k += T) s_tq[k] = L.tq[k];
+    for (int k = tid; k < L.n_x; k += T) s_tx[k] = L.tx[k];
+    for (int k = tid; k < L.n_words; k += T) hs.bits[k] = 0u;
+    const int cell = cell_begin + blockIdx.x;
+    const int ci = cell / L.Nq, cj = cell - ci * L.Nq;
+    const CellGeom g = cell_geom(L.pe, L.qe, ci, cj);
     __syncthreads();
-    map_cell<false>(L, s, cell_begin + blockIdx.x, nullptr);
+
+    for (int m = tid; m < L.nnode; m += T) {
+        int c, a, b;
+        split_node(L, m, c, a, b);
+        double p, q, P2, Q2;
+        map_node_sq(g, s_tp[a], s_tq[b], s_tx[c], p, q, P2, Q2);
+        const int t = target_cell_sq(s_thr_p, L.pe_pad, L.Np, s_thr_q, L.qe_pad, L.Nq, P2, Q2);
+        if (t >= 0) atomicOr(&hs.bits[t >> 5], 1u << (t & 31));
+        s_tgt[m] = t;
+    }
     __syncthreads();
-    const int H = rank_bits(L, s);
-    if (threadIdx.x == 0) hits[blockIdx.x] = H;
+    const int H = rank_bits_n(L.n_words, hs);
+    // stable counting sort: each of `nwe` warps owns a contiguous slice of node ids and a histogram of H counters
+    // (all warps when H <= kHitsFast, else warp 0 alone: rare, slow, same result); ranks replace the cell ids in s_tgt
+    const int nwe = (H <= kHitsFast) ? NW : 1;
+    for (int k = tid; k < nwe * H; k += T) s_hist[k] = 0;
+    __syncthreads();
+    const int slice = (((L.nnode + nwe - 1) / nwe) + 31) & ~31;
+    const int nb = min(warp * slice, L.nnode), ne = (warp < nwe) ? min(nb + slice, L.nnode) : nb;
+    for (int m = nb + lane; m < ne; m += 32) {
+        const int t = s_tgt[m];
+        const int r = (t >= 0) ? rank_of(hs, t) : -1;
+        s_tgt[m] = r;
+        if (r >= 0) atomicAdd(&s_hist[warp * H + r], 1);
+    }
+    __syncthreads();
+    for (int k = tid; k < H; k += T) {
+        int tot = 0;
+        for (int w = 0; w < nwe; ++w) tot += s_hist[w * H + k];
+        s_start[k] = tot;
+    }
+    if (tid == 0) s_start[H] = 0;
+    __syncthreads();
+    const int ntot = block_exclusive_scan(s_start, H + 1, hs.scratch);
+    for (int k = tid; k < H; k += T) {
+        int run = s_start[k];
+        for (int w = 0; w < nwe; ++w) { const int v = s_hist[w * H + k]; s_hist[w * H + k] = run; run += v; }
+    }
+    __syncthreads();
+    for (int m0 = nb; m0 < ne; m0 += 32) {
+        const int m = m0 + lane;
+        const int key = (m < ne) ? s_tgt[m] : -1;
+        const unsigned same = __match_any_sync(0xffffffffu, key);
+        if (key >= 0) {
+            const int pos = s_hist[warp * H + key] + __popc(same & ((1u << lane) - 1u));
+            s_sorted[pos] = (unsigned short)m;
+            s_rkpos[pos] = (unsigned short)key;
+        }
+        __syncwarp();
+        if (key >= 0 && lane == (__ffs(same) - 1)) s_hist[warp * H + key] += __popc(same);
+        __syncwarp();
+    }
+    __syncthreads();
+    unsigned short* g_sorted = nl.sorted + (size_t)blockIdx.x * L.nnode;
+    unsigned short* g_rkpos = nl.rkpos + (size_t)blockIdx.x * L.nnode;
+    for (int k = tid; k < ntot; k += T) { g_sorted[k] = s_sorted[k]; g_rkpos[k] = s_rkpos[k]; }
+    if (tid == 0) { nl.hits[blockIdx.x] = H; nl.ntot[blockIdx.x] = ntot; }
 }
 
 // Pattern pass, kernel S: exclusive scan of hits -> rowptr (block-local), nnz and max hits.  One CTA.
@@ -139,161 +153,45 @@ __global__ void __launch_bounds__(1024) k_scan_rows(DevLattice L, int n_blk, con
     }
 }
 
-// Pattern pass, kernel B: column indices, ascending within each row.
-__global__ void __launch_bounds__(kThreads) k_emit_cols(DevLattice L, int cell_begin, const int64_t* __restrict__ rowptr,
-                                                       int32_t* __restrict__ colidx)
+// Pattern pass, kernel B: column indices, ascending within each row.  The hit cells of a source cell are
+// recovered from its node lists: the first node of every target is mapped again (exact arithmetic, same cell).
+__global__ void __launch_bounds__(kThreads) k_emit_cols(DevLattice L, int cell_begin, NodeLists nl, int hmax,
+                                                       const int64_t* __restrict__ rowptr, int32_t* __restrict__ colidx)
 {
     extern __shared__ __align__(16) char smem[];
+    constexpr int T = kThreads;
+    const int tid = threadIdx.x;
     char* sp = smem;
-    Stage s = stage_common(L, sp);
-    int* hitcell = (int*)carve(sp, sizeof(int) * min(L.n_cells, L.nnode));
+    double* s_thr_p = (double*)carve(sp, 8 * (size_t)L.pe_pad);
+    double* s_thr_q = (double*)carve(sp, 8 * (size_t)L.qe_pad);
+    int* hitcell = (int*)carve(sp, 4 * (size_t)hmax);
+    for (int k = tid; k < L.pe_pad; k += T) s_thr_p[k] = L.thr_p[k];
+    for (int k = tid; k < L.qe_pad; k += T) s_thr_q[k] = L.thr_q[k];
+    const int cell = cell_begin + blockIdx.x;
+    const int ci = cell / L.Nq, cj = cell - ci * L.Nq;
+    const CellGeom g = cell_geom(L.pe, L.qe, ci, cj);
+    const int H = nl.hits[blockIdx.x], ntot = nl.ntot[blockIdx.x];
+    const unsigned short* g_sorted = nl.sorted + (size_t)blockIdx.x * L.nnode;
+    const unsigned short* g_rkpos = nl.rkpos + (size_t)blockIdx.x * L.nnode;
     __syncthreads();
-    map_cell<false>(L, s, cell_begin + blockIdx.x, nullptr);
-    __syncthreads();
-    const int H = rank_bits(L, s);
-    list_hits(L, s, hitcell);
+    for (int pos = tid; pos < ntot; pos += T) {
+        const int r = g_rkpos[pos];
+        if (pos > 0 && g_rkpos[pos - 1] == r) continue;
+        int c, a, b;
+        split_node(L, g_sorted[pos], c, a, b);
+        double p, q, P2, Q2;
+        map_node_sq(g, L.tp[a], L.tq[b], L.tx[c], p, q, P2, Q2);
+        hitcell[r] = target_cell_sq(s_thr_p, L.pe_pad, L.Np, s_thr_q, L.qe_pad, L.Nq, P2, Q2);
+    }
     __syncthreads();
     for (int a = 0; a < L.n_ch; ++a) {
         const int off = L.cl_off[a], nc = L.cl_off[a + 1] - off;
         int32_t* out = colidx + rowptr[(int64_t)blockIdx.x * L.n_ch + a];
         const int len = H * nc;
-        for (int idx = threadIdx.x; idx < len; idx += blockDim.x) {
+        for (int idx = tid; idx < len; idx += T) {
             const int k = idx / nc, m = idx - k * nc;
             out[idx] = hitcell[k] * L.n_ch + L.cl[off + m];
         }
-    }
-}
-
-// ------------------------------------------------------------------------------------------------
-// Fill pass, generic (table-driven) kernel: any channel list.  One CTA per source cell.
-//   phase 1  map nodes -> target cells, bitset, ranks, hit list
-//   phase 2  deterministic counting sort of the node ids by hit rank (stable in node order)
-//   phase 3  one warp per hit cell: lanes take that cell's nodes, evaluate the ket harmonics and the
-//            n_fun orbital functions, accumulate privately, then a fixed-shape butterfly reduces the lanes
-//   phase 4  per hit cell: contract with the channel coefficients c^L and write the row segments
-// Node sums are formed in an order fixed by (node id, lane, butterfly): bitwise reproducible.
-// ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kThreads) k_fill_generic(DevLattice L, int cell_begin, int hmax,
-                                                          const int64_t* __restrict__ rowptr, double* __restrict__ vals)
-{
-    extern __shared__ __align__(16) char smem[];
-    char* sp = smem;
-    Stage s = stage_common(L, sp);
-    const int nw = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    double* s_wp = (double*)carve(sp, sizeof(double) * L.n_p);
-    double* s_wq = (double*)carve(sp, sizeof(double) * L.n_q);
-    double* s_wx = (double*)carve(sp, sizeof(double) * L.n_x);
-    double* s_sx = (double*)carve(sp, sizeof(double) * L.n_x);
-    double* s_acc = (double*)carve(sp, sizeof(double) * nw * L.n_fun);
-    int* tgt = (int*)carve(sp, sizeof(int) * L.nnode);
-    int* sorted = (int*)carve(sp, sizeof(int) * L.nnode);
-    int* hitcell = (int*)carve(sp, sizeof(int) * hmax);
-    int* start = (int*)carve(sp, sizeof(int) * (hmax + 1));
-    int* hist = (int*)carve(sp, sizeof(int) * nw * hmax);
-    for (int k = threadIdx.x; k < L.n_p; k += blockDim.x) s_wp[k] = L.wp[k];
-    for (int k = threadIdx.x; k < L.n_q; k += blockDim.x) s_wq[k] = L.wq[k];
-    for (int k = threadIdx.x; k < L.n_x; k += blockDim.x) { s_wx[k] = L.wx[k]; s_sx[k] = L.sx[k]; }
-    for (int k = threadIdx.x; k < nw * hmax; k += blockDim.x) hist[k] = 0;
-    __syncthreads();
-
-    // ---- phase 1
-    const int cell = cell_begin + blockIdx.x;
-    map_cell<true>(L, s, cell, tgt);
-    __syncthreads();
-    const int H = rank_bits(L, s);
-    if (H > hmax) return;                       // cannot happen when hmax comes from pm_pattern of this block
-    list_hits(L, s, hitcell);
-
-    // ---- phase 2: each warp owns a contiguous slice of node ids
-    const int slice = (((L.nnode + nw - 1) / nw) + 31) & ~31;
-    const int nb = warp * slice, ne = min(nb + slice, L.nnode);
-    for (int n = nb + lane; n < ne; n += 32) {
-        const int t = tgt[n];
-        if (t >= 0) atomicAdd(&hist[warp * hmax + rank_of(s, t)], 1);
-    }
-    __syncthreads();
-    for (int k = threadIdx.x; k < H; k += blockDim.x) {
-        int tot = 0;
-        for (int w = 0; w < nw; ++w) tot += hist[w * hmax + k];
-        start[k] = tot;
-    }
-    if (threadIdx.x == 0) start[H] = 0;
-    __syncthreads();
-    block_exclusive_scan(start, H + 1, s.scratch);
-    for (int k = threadIdx.x; k < H; k += blockDim.x) {
-        int run = start[k];
-        for (int w = 0; w < nw; ++w) { const int v = hist[w * hmax + k]; hist[w * hmax + k] = run; run += v; }
-    }
-    __syncthreads();
-    for (int n0 = nb; n0 < ne; n0 += 32) {
-        const int n = n0 + lane;
-        const int t = (n < ne) ? tgt[n] : -1;
-        const int key = (t >= 0) ? rank_of(s, t) : -1;
-        const unsigned same = __match_any_sync(0xffffffffu, key);
-        if (key >= 0) {
-            const int pos = hist[warp * hmax + key] + __popc(same & ((1u << lane) - 1u));
-            sorted[pos] = n;
-        }
-        __syncwarp();
-        if (key >= 0 && lane == (__ffs(same) - 1)) hist[warp * hmax + key] += __popc(same);
-        __syncwarp();
-    }
-    __syncthreads();
-
-    // ---- phase 3 + 4
-    const int i = cell / L.Nq, j = cell - i * L.Nq;
-    const CellGeom g = cell_geom(s.pe, s.qe, i, j);
-    const double dsrc = (s.pe[i + 1] - s.pe[i]) * (s.qe[j + 1] - s.qe[j]);
-    const int nqx = L.n_q * L.n_x;
-    double* wacc = s_acc + warp * L.n_fun;
-    for (int k = warp; k < H; k += nw) {
-        double acc[kMaxFun];
-        for (int f = 0; f < L.n_fun; ++f) acc[f] = 0.0;
-        for (int sidx = start[k] + lane; sidx < start[k + 1]; sidx += 32) {
-            const int n = sorted[sidx];
-            const int a = n / nqx, r = n - a * nqx, b = r / L.n_x, c = r - b * L.n_x;
-            double p, q, pp, qq;
-            const double x = s.tx[c];
-            map_node(g, s.tp[a], s.tq[b], x, p, q, pp, qq);
-            const double w = __dmul_rn(__dmul_rn(__dmul_rn(g.hp, s_wp[a]), __dmul_rn(g.hq, s_wq[b])), s_wx[c]);
-            const double omega = w * ((p * q) / (pp * qq));
-            // rotated directions from vector components (frame: q^ = z, p^ = (sx, 0, x))
-            const double sx = s_sx[c];
-            const double ax = -0.5 * p * sx, az = -0.5 * p * x - 0.75 * q;
-            const double bx = p * sx, bz = p * x - 0.5 * q;
-            const double ra = rsqrt(ax * ax + az * az), rb = rsqrt(bx * bx + bz * bz);
-            double Yp[kMaxY], Yq[kMaxY], K[kMaxSlot];
-            ylm_fill(L.lmax, ax * ra, az * ra, L.ya, L.yb, L.ydiag, Yp);
-            ylm_fill(L.lmax, bx * rb, bz * rb, L.ya, L.yb, L.ydiag, Yq);
-            for (int sl = 0; sl < L.n_slot; ++sl) {
-                double v = 0.0;
-                for (int t = L.kt_off[sl]; t < L.kt_off[sl + 1]; ++t) v += L.kt_c[t] * Yp[L.kt_ip[t]] * Yq[L.kt_iq[t]];
-                K[sl] = v * omega;
-            }
-            const double* bra = L.bra + (size_t)c * L.n_slot;
-            for (int f = 0; f < L.n_fun; ++f) {
-                const int4 fn = L.fun[f];
-                double v = 0.0;
-                for (int m = 0; m < fn.z; ++m) v += bra[fn.x + m] * K[fn.y + m];
-                acc[f] += v;
-            }
-        }
-        for (int f = 0; f < L.n_fun; ++f) {
-            double v = acc[f];
-#pragma unroll
-            for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
-            if (lane == 0) wacc[f] = v;
-        }
-        __syncwarp();
-        const int hc = hitcell[k], ic = hc / L.Nq, jc = hc - ic * L.Nq;
-        const double norm = 1.0 / sqrt(dsrc * ((s.pe[ic + 1] - s.pe[ic]) * (s.qe[jc + 1] - s.qe[jc])));
-        for (int o = lane; o < L.totcoup; o += 32) {
-            const int a = L.o_alpha[o], off = L.cl_off[a], nc = L.cl_off[a + 1] - off;
-            double v = 0.0;
-            for (int t = L.ot_off[o]; t < L.ot_off[o + 1]; ++t) v += L.ot_c[t] * wacc[L.ot_f[t]];
-            vals[rowptr[(int64_t)blockIdx.x * L.n_ch + a] + (int64_t)k * nc + (o - off)] = v * norm;
-        }
-        __syncwarp();
     }
 }
 
@@ -322,21 +220,12 @@ static std::atomic<int64_t> g_launches{0};
 int64_t launch_count() { return g_launches.load(); }
 void count_launch() { ++g_launches; }
 
-size_t fill_generic_smem(const DevLattice& L, int hmax)
+cudaError_t launch_map_sort(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, cudaStream_t st)
 {
-    auto al = [](size_t b) { return (b + 15) & ~size_t(15); };
-    const int nw = kThreads / 32;
-    return stage_bytes(L, kThreads) + al(8 * (size_t)L.n_p) + al(8 * (size_t)L.n_q) + 2 * al(8 * (size_t)L.n_x)
-         + al(8 * (size_t)nw * L.n_fun) + 2 * al(4 * (size_t)L.nnode) + al(4 * (size_t)hmax) + al(4 * (size_t)(hmax + 1))
-         + al(4 * (size_t)nw * hmax);
-}
-
-cudaError_t launch_count_hits(const DevLattice& L, int cell_begin, int n_blk, int* hits, cudaStream_t st)
-{
-    const size_t sm = stage_bytes(L, kThreads);
-    cudaError_t e = cudaFuncSetAttribute(k_count_hits, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    const size_t sm = map_sort_smem(L);
+    cudaError_t e = cudaFuncSetAttribute(k_map_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
-    k_count_hits<<<n_blk, kThreads, sm, st>>>(L, cell_begin, n_blk, hits);
+    k_map_sort<<<n_blk, kThreads, sm, st>>>(L, cell_begin, nl);
     ++g_launches;
     return cudaGetLastError();
 }
@@ -349,24 +238,13 @@ cudaError_t launch_scan_rows(const DevLattice& L, int n_blk, const int* hits, in
     return cudaGetLastError();
 }
 
-cudaError_t launch_emit_cols(const DevLattice& L, int cell_begin, int n_blk, const int64_t* rowptr, int32_t* colidx,
-                             cudaStream_t st)
+cudaError_t launch_emit_cols(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, int hmax,
+                             const int64_t* rowptr, int32_t* colidx, cudaStream_t st)
 {
-    const size_t sm = stage_bytes(L, kThreads) + 16 + 4 * (size_t)std::min(L.n_cells, L.nnode);
+    const size_t sm = al16(8 * (size_t)L.pe_pad) + al16(8 * (size_t)L.qe_pad) + al16(4 * (size_t)std::max(hmax, 1));
     cudaError_t e = cudaFuncSetAttribute(k_emit_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
-    k_emit_cols<<<n_blk, kThreads, sm, st>>>(L, cell_begin, rowptr, colidx);
-    ++g_launches;
-    return cudaGetLastError();
-}
-
-cudaError_t launch_fill_generic(const DevLattice& L, int cell_begin, int n_blk, int hmax, const int64_t* rowptr,
-                                double* vals, cudaStream_t st)
-{
-    const size_t sm = fill_generic_smem(L, hmax);
-    cudaError_t e = cudaFuncSetAttribute(k_fill_generic, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    if (e != cudaSuccess) return e;
-    k_fill_generic<<<n_blk, kThreads, sm, st>>>(L, cell_begin, hmax, rowptr, vals);
+    k_emit_cols<<<n_blk, kThreads, sm, st>>>(L, cell_begin, nl, hmax, rowptr, colidx);
     ++g_launches;
     return cudaGetLastError();
 }

@@ -1,4 +1,4 @@
-// pm_kernels.cuh — launcher declarations of libpm's kernels (definitions in pm_kernels.cu).
+// pm_kernels.cuh — launcher declarations of libpm's kernels (definitions in pm_kernels.cu, pm_fill.cu).
 #pragma once
 #include <algorithm>
 #include <atomic>
@@ -11,31 +11,28 @@
 namespace pm {
 
 constexpr int kThreads = 256;
-constexpr int kMaxFun = 256;        // generic fill: per-lane private accumulators
-constexpr int kMaxSlot = 160;
-constexpr int kMaxY = 45;           // (PM_MAX_L+1)(PM_MAX_L+2)/2
+constexpr int kHitsFast = 512;      // k_map_sort: per-warp histograms up to this many hit cells, one warp beyond
 
-size_t stage_bytes(const DevLattice& L, int threads);
-size_t fill_generic_smem(const DevLattice& L, int hmax);
+size_t map_sort_smem(const DevLattice& L);
 int64_t launch_count();
+void count_launch();
 
-cudaError_t launch_count_hits(const DevLattice& L, int cell_begin, int n_blk, int* hits, cudaStream_t st);
+// pattern pass
+cudaError_t launch_map_sort(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, cudaStream_t st);
 cudaError_t launch_scan_rows(const DevLattice& L, int n_blk, const int* hits, int64_t* cellbase, int64_t* rowptr,
                              int64_t* summary, cudaStream_t st);
-cudaError_t launch_emit_cols(const DevLattice& L, int cell_begin, int n_blk, const int64_t* rowptr, int32_t* colidx,
-                             cudaStream_t st);
-cudaError_t launch_fill_generic(const DevLattice& L, int cell_begin, int n_blk, int hmax, const int64_t* rowptr,
-                                double* vals, cudaStream_t st);
-cudaError_t launch_spmv(int64_t n_rows, const int64_t* rowptr, const int32_t* colidx, const double* vals,
-                        const double* x, double* y, cudaStream_t st);
+cudaError_t launch_emit_cols(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, int hmax,
+                             const int64_t* rowptr, int32_t* colidx, cudaStream_t st);
 
 // fill pass (pm_fill.cuh): variant selection and launch
 struct FillLaunch { const void* fn; int nw, grid; FillSmem smem; const char* name; };
 bool fill_has_spec(unsigned long long tables_hash);
 cudaError_t fill_plan(const DevLattice& L, unsigned long long tables_hash, int hmax, int n_sm, FillLaunch* out);
-cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, int hmax, const int64_t* rowptr,
-                        double* vals, double* accG, cudaStream_t st);
-void count_launch();
+cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl, int hmax,
+                        const int64_t* rowptr, double* vals, double* accG, cudaStream_t st);
+
+cudaError_t launch_spmv(int64_t n_rows, const int64_t* rowptr, const int32_t* colidx, const double* vals,
+                        const double* x, double* y, cudaStream_t st);
 
 // dependent-free DFMA loop on every SM: measured FP64 FMA throughput in TFLOP/s (diagnostic)
 cudaError_t measure_dfma(int n_sm, double* tflops, cudaStream_t st);
