@@ -46,8 +46,7 @@ struct pm_lattice {
     int64_t* h_summary = nullptr;      // pinned
     int hits_cap = 0;
     int hmax = -1, pat_begin = -1, pat_end = -1;     // max hit cells, and the cell range, of the last pattern call
-    double* d_acc = nullptr;           // fill scratch: per persistent CTA, hmax rows of n_fun sums
-    size_t acc_bytes = 0;
+    int* d_counter = nullptr;          // work counter of the fill kernel
     unsigned long long hash = 0;       // pm::tables_hash of T (selects a generated fill kernel)
     int n_sm = 0;
     pm::DevLattice dev{};
@@ -60,13 +59,14 @@ void free_device(pm_lattice* L)
     if (L->d_blob) cudaFree(L->d_blob);
     if (L->nl.sorted) cudaFree(L->nl.sorted);
     if (L->nl.rkpos) cudaFree(L->nl.rkpos);
+    if (L->nl.tcell) cudaFree(L->nl.tcell);
     if (L->nl.ntot) cudaFree(L->nl.ntot);
     if (L->nl.hits) cudaFree(L->nl.hits);
     if (L->d_cellbase) cudaFree(L->d_cellbase);
     if (L->d_summary) cudaFree(L->d_summary);
     if (L->h_summary) cudaFreeHost(L->h_summary);
-    if (L->d_acc) cudaFree(L->d_acc);
-    L->d_acc = nullptr; L->acc_bytes = 0;
+    if (L->d_counter) cudaFree(L->d_counter);
+    L->d_counter = nullptr;
     L->d_blob = nullptr; L->nl = pm::NodeLists{}; L->d_cellbase = nullptr; L->d_summary = nullptr; L->h_summary = nullptr;
     L->hits_cap = 0;
 }
@@ -137,6 +137,7 @@ int32_t ensure_device(pm_lattice* L)
     if ((e = cudaMalloc(&L->d_blob, blob.size())) != cudaSuccess) return cuda_fail(e, "cudaMalloc(tables)");
     if ((e = cudaMemcpy(L->d_blob, blob.data(), blob.size(), cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_fail(e, "cudaMemcpy(tables)");
     if ((e = cudaMalloc(&L->d_summary, 2 * sizeof(int64_t))) != cudaSuccess) return cuda_fail(e, "cudaMalloc(summary)");
+    if ((e = cudaMalloc(&L->d_counter, sizeof(int))) != cudaSuccess) return cuda_fail(e, "cudaMalloc(counter)");
     if ((e = cudaMallocHost(&L->h_summary, 2 * sizeof(int64_t))) != cudaSuccess) return cuda_fail(e, "cudaMallocHost(summary)");
     char* b = L->d_blob;
     D.pe = (const double*)(b + o_pe); D.qe = (const double*)(b + o_qe);
@@ -163,6 +164,7 @@ int32_t ensure_cell_scratch(pm_lattice* L, int n_blk)
     if (n_blk <= L->hits_cap) return PM_OK;
     if (L->nl.sorted) cudaFree(L->nl.sorted);
     if (L->nl.rkpos) cudaFree(L->nl.rkpos);
+    if (L->nl.tcell) cudaFree(L->nl.tcell);
     if (L->nl.ntot) cudaFree(L->nl.ntot);
     if (L->nl.hits) cudaFree(L->nl.hits);
     if (L->d_cellbase) cudaFree(L->d_cellbase);
@@ -171,6 +173,7 @@ int32_t ensure_cell_scratch(pm_lattice* L, int n_blk)
     cudaError_t e;
     if ((e = cudaMalloc(&L->nl.sorted, sizeof(unsigned short) * nn)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(node lists)");
     if ((e = cudaMalloc(&L->nl.rkpos, sizeof(unsigned short) * nn)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(node lists)");
+    if ((e = cudaMalloc(&L->nl.tcell, sizeof(int) * nn)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(node lists)");
     if ((e = cudaMalloc(&L->nl.ntot, sizeof(int) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(ntot)");
     if ((e = cudaMalloc(&L->nl.hits, sizeof(int) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(hits)");
     if ((e = cudaMalloc(&L->d_cellbase, sizeof(int64_t) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(cellbase)");
@@ -352,7 +355,7 @@ int32_t pm_pattern(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int64_
     lat->hmax = (int)lat->h_summary[1]; lat->pat_begin = cell_begin; lat->pat_end = cell_end;
     if (!d_colidx) return PM_OK;
     if (*nnz_host > colidx_capacity) return fail(PM_ERR_OVERFLOW, "d_colidx too small for this block's nnz");
-    if ((e = pm::launch_emit_cols(lat->dev, cell_begin, n_blk, lat->nl, lat->hmax, d_rowptr, d_colidx, st)) != cudaSuccess)
+    if ((e = pm::launch_emit_cols(lat->dev, n_blk, lat->nl, lat->hmax, d_rowptr, d_colidx, st)) != cudaSuccess)
         return cuda_fail(e, "k_emit_cols");
     return PM_OK;
 }
@@ -368,23 +371,12 @@ int32_t pm_fill(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const int
         return fail(PM_ERR_STATE, "pm_fill needs a preceding pm_pattern of the same cell range on this lattice");
     if (cell_begin == cell_end) return PM_OK;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const int hmax = std::max(lat->hmax, 1);
     const int n_blk = cell_end - cell_begin;
-    cudaError_t e;
-    {
-        pm::FillLaunch F;
-        e = pm::fill_plan(lat->dev, lat->hash, hmax, lat->n_sm, &F);
-        if (e == cudaErrorInvalidConfiguration) { cudaGetLastError(); return fail(PM_ERR_NOMEM, "source cell needs more shared memory than one SM has"); }
-        if (e != cudaSuccess) return cuda_fail(e, "fill_plan");
-        const size_t need = sizeof(double) * (size_t)F.grid * (size_t)hmax * (size_t)lat->dev.n_fun;
-        if (need > lat->acc_bytes) {
-            if (lat->d_acc) { if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e, "sync"); cudaFree(lat->d_acc); }
-            lat->d_acc = nullptr; lat->acc_bytes = 0;
-            if ((e = cudaMalloc(&lat->d_acc, need)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(fill scratch)");
-            lat->acc_bytes = need;
-        }
-        e = pm::launch_fill(lat->dev, F, cell_begin, n_blk, lat->nl, hmax, d_rowptr, d_vals, lat->d_acc, st);
-    }
+    pm::FillLaunch F;
+    cudaError_t e = pm::fill_plan(lat->dev, lat->hash, lat->n_sm, &F);
+    if (e == cudaErrorInvalidConfiguration) { cudaGetLastError(); return fail(PM_ERR_NOMEM, "channel set needs more shared memory than one SM has"); }
+    if (e != cudaSuccess) return cuda_fail(e, "fill_plan");
+    e = pm::launch_fill(lat->dev, F, cell_begin, n_blk, lat->nl, d_rowptr, d_vals, lat->d_counter, st);
     if (e != cudaSuccess) return cuda_fail(e, "k_fill");
     return PM_OK;
 }

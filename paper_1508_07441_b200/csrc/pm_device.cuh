@@ -30,10 +30,11 @@ struct DevLattice {
 
 // Per-source-cell node lists written by the pattern pass and read by the fill pass (library-owned scratch):
 // the node ids m = c*(n_p*n_q) + a*n_q + b of the nodes that hit the grid, sorted by (rank of target cell, m),
-// and the rank of the target at every sorted position.  Stride nnode per source cell.
+// and the rank and the cell id of the target at every sorted position.  Stride nnode per source cell.
 struct NodeLists {
     unsigned short* sorted;     // [n_blk][nnode]
     unsigned short* rkpos;      // [n_blk][nnode]
+    int* tcell;                 // [n_blk][nnode]
     int* ntot;                  // [n_blk] nodes on the grid
     int* hits;                  // [n_blk] hit cells H
 };

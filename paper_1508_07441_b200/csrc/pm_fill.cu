@@ -13,15 +13,15 @@ namespace {
 
 constexpr int kSmemLimit = 227 * 1024;
 
-using FillKernel = void (*)(DevLattice, FillSmem, NodeLists, int, int, int, const int64_t*, double*, double*);
+using FillKernel = void (*)(DevLattice, FillSmem, NodeLists, int, int, const int64_t*, double*, int*);
 
 struct FillVariant { unsigned long long hash; int nw; FillKernel fn; const char* name; };
 
-#define PM_SPEC(S) {gen::S::kHash, 4, k_fill_seg<gen::S, 4>, #S}, {gen::S::kHash, 6, k_fill_seg<gen::S, 6>, #S}, \
-                   {gen::S::kHash, 8, k_fill_seg<gen::S, 8>, #S}, {gen::S::kHash, 12, k_fill_seg<gen::S, 12>, #S},
+#define PM_SPEC(S) {gen::S::kHash, 4, k_fill_warp<gen::S, 4>, #S}, {gen::S::kHash, 6, k_fill_warp<gen::S, 6>, #S}, \
+                   {gen::S::kHash, 8, k_fill_warp<gen::S, 8>, #S}, {gen::S::kHash, 12, k_fill_warp<gen::S, 12>, #S},
 const FillVariant kVariants[] = {
     PM_SPEC_LIST
-    {0ull, 4, k_fill_seg<SpecGeneric, 4>, "generic"}, {0ull, 8, k_fill_seg<SpecGeneric, 8>, "generic"},
+    {0ull, 4, k_fill_warp<SpecGeneric, 4>, "generic"}, {0ull, 8, k_fill_warp<SpecGeneric, 8>, "generic"},
 };
 #undef PM_SPEC
 
@@ -42,13 +42,13 @@ bool fill_has_spec(unsigned long long hash)
 // Picks the variant (specialised when `hash` matches a generated kernel, else table-driven; the preferred warp count
 // if its shared memory fits, else a smaller one) and the persistent grid.  Returns cudaErrorInvalidConfiguration
 // when no variant fits in shared memory.
-cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int hmax, int n_sm, FillLaunch* out)
+cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int n_sm, FillLaunch* out)
 {
     const unsigned long long key = fill_has_spec(hash) ? hash : 0ull;
     const int want = preferred_warps();
     const FillVariant* best = nullptr;          // largest warp count <= want whose shared memory fits, else the smallest that fits
     for (const FillVariant& v : kVariants) {
-        if (v.hash != key || fill_smem_plan(L, hmax, v.nw).total > kSmemLimit) continue;
+        if (v.hash != key || fill_smem_plan(L, v.nw).total > kSmemLimit) continue;
         if (!best) { best = &v; continue; }
         const bool v_ok = v.nw <= want, b_ok = best->nw <= want;
         if ((v_ok && (!b_ok || v.nw > best->nw)) || (!v_ok && !b_ok && v.nw < best->nw)) best = &v;
@@ -57,7 +57,7 @@ cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int hmax, in
     out->fn = (const void*)best->fn;
     out->nw = best->nw;
     out->name = best->name;
-    out->smem = fill_smem_plan(L, hmax, best->nw);
+    out->smem = fill_smem_plan(L, best->nw);
     cudaError_t e = cudaFuncSetAttribute(out->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, out->smem.total);
     if (e != cudaSuccess) return e;
     int per_sm = 1;
@@ -67,15 +67,18 @@ cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int hmax, in
     return cudaSuccess;
 }
 
-cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl, int hmax,
-                        const int64_t* rowptr, double* vals, double* accG, cudaStream_t st)
+cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl,
+                        const int64_t* rowptr, double* vals, int* counter, cudaStream_t st)
 {
-    const int grid = n_blk < F.grid ? n_blk : F.grid;
+    const int need = (n_blk + F.nw - 1) / F.nw;                        // one cell per warp at a time
+    const int grid = need < F.grid ? need : F.grid;
     DevLattice Lc = L;
     FillSmem S = F.smem;
     NodeLists N = nl;
-    void* args[] = {&Lc, &S, &N, &cell_begin, &n_blk, &hmax, (void*)&rowptr, &vals, &accG};
-    cudaError_t e = cudaLaunchKernel(F.fn, dim3((unsigned)grid), dim3((unsigned)(F.nw * 32)), args, (size_t)S.total, st);
+    cudaError_t e = cudaMemsetAsync(counter, 0, sizeof(int), st);      // the work counter the warps draw cells from
+    if (e != cudaSuccess) return e;
+    void* args[] = {&Lc, &S, &N, &cell_begin, &n_blk, (void*)&rowptr, &vals, &counter};
+    e = cudaLaunchKernel(F.fn, dim3((unsigned)grid), dim3((unsigned)(F.nw * 32)), args, (size_t)S.total, st);
     count_launch();
     return e != cudaSuccess ? e : cudaGetLastError();
 }

@@ -28,7 +28,7 @@ size_t map_sort_smem(const DevLattice& L)
     const int hcap = std::min(L.nnode, L.n_cells);
     return al16(8 * (size_t)L.pe_pad) + al16(8 * (size_t)L.qe_pad) + al16(8 * (size_t)L.n_p) + al16(8 * (size_t)L.n_q)
          + al16(8 * (size_t)L.n_x) + 2 * al16(4 * (size_t)L.n_words) + al16(4 * (size_t)(kThreads + 1))
-         + al16(4 * (size_t)L.nnode) + 2 * al16(2 * (size_t)L.nnode) + al16(4 * (size_t)(hcap + 1))
+         + 2 * al16(4 * (size_t)L.nnode) + 3 * al16(2 * (size_t)L.nnode) + al16(4 * (size_t)(hcap + 1))
          + al16(4 * (size_t)std::max(nw * std::min(hcap, kHitsFast), hcap));
 }
 
@@ -51,6 +51,8 @@ __global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_be
     int* s_tgt = (int*)carve(sp, 4 * (size_t)L.nnode);
     unsigned short* s_sorted = (unsigned short*)carve(sp, 2 * (size_t)L.nnode);
     unsigned short* s_rkpos = (unsigned short*)carve(sp, 2 * (size_t)L.nnode);
+    unsigned short* s_rk = (unsigned short*)carve(sp, 2 * (size_t)L.nnode);     // rank of each node's target (0xffff: off the grid)
+    int* s_tcpos = (int*)carve(sp, 4 * (size_t)L.nnode);                         // target cell at each sorted position
     int* s_start = (int*)carve(sp, 4 * (size_t)(hcap + 1));
     int* s_hist = (int*)carve(sp, 4 * (size_t)max(NW * min(hcap, kHitsFast), hcap));
 
@@ -77,7 +79,7 @@ __global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_be
     __syncthreads();
     const int H = rank_bits_n(L.n_words, hs);
     // stable counting sort: each of `nwe` warps owns a contiguous slice of node ids and a histogram of H counters
-    // (all warps when H <= kHitsFast, else warp 0 alone: rare, slow, same result); ranks replace the cell ids in s_tgt
+    // (all warps when H <= kHitsFast, else warp 0 alone: rare, slow, same result)
     const int nwe = (H <= kHitsFast) ? NW : 1;
     for (int k = tid; k < nwe * H; k += T) s_hist[k] = 0;
     __syncthreads();
@@ -85,9 +87,9 @@ __global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_be
     const int nb = min(warp * slice, L.nnode), ne = (warp < nwe) ? min(nb + slice, L.nnode) : nb;
     for (int m = nb + lane; m < ne; m += 32) {
         const int t = s_tgt[m];
-        const int r = (t >= 0) ? rank_of(hs, t) : -1;
-        s_tgt[m] = r;
-        if (r >= 0) atomicAdd(&s_hist[warp * H + r], 1);
+        const int r = (t >= 0) ? rank_of(hs, t) : 0xffff;
+        s_rk[m] = (unsigned short)r;
+        if (t >= 0) atomicAdd(&s_hist[warp * H + r], 1);
     }
     __syncthreads();
     for (int k = tid; k < H; k += T) {
@@ -105,21 +107,23 @@ __global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_be
     __syncthreads();
     for (int m0 = nb; m0 < ne; m0 += 32) {
         const int m = m0 + lane;
-        const int key = (m < ne) ? s_tgt[m] : -1;
+        const int key = (m < ne) ? (int)s_rk[m] : 0xffff;
         const unsigned same = __match_any_sync(0xffffffffu, key);
-        if (key >= 0) {
+        if (key != 0xffff) {
             const int pos = s_hist[warp * H + key] + __popc(same & ((1u << lane) - 1u));
             s_sorted[pos] = (unsigned short)m;
             s_rkpos[pos] = (unsigned short)key;
+            s_tcpos[pos] = s_tgt[m];
         }
         __syncwarp();
-        if (key >= 0 && lane == (__ffs(same) - 1)) s_hist[warp * H + key] += __popc(same);
+        if (key != 0xffff && lane == (__ffs(same) - 1)) s_hist[warp * H + key] += __popc(same);
         __syncwarp();
     }
     __syncthreads();
     unsigned short* g_sorted = nl.sorted + (size_t)blockIdx.x * L.nnode;
     unsigned short* g_rkpos = nl.rkpos + (size_t)blockIdx.x * L.nnode;
-    for (int k = tid; k < ntot; k += T) { g_sorted[k] = s_sorted[k]; g_rkpos[k] = s_rkpos[k]; }
+    int* g_tcell = nl.tcell + (size_t)blockIdx.x * L.nnode;
+    for (int k = tid; k < ntot; k += T) { g_sorted[k] = s_sorted[k]; g_rkpos[k] = s_rkpos[k]; g_tcell[k] = s_tcpos[k]; }
     if (tid == 0) { nl.hits[blockIdx.x] = H; nl.ntot[blockIdx.x] = ntot; }
 }
 
@@ -153,35 +157,21 @@ __global__ void __launch_bounds__(1024) k_scan_rows(DevLattice L, int n_blk, con
     }
 }
 
-// Pattern pass, kernel B: column indices, ascending within each row.  The hit cells of a source cell are
-// recovered from its node lists: the first node of every target is mapped again (exact arithmetic, same cell).
-__global__ void __launch_bounds__(kThreads) k_emit_cols(DevLattice L, int cell_begin, NodeLists nl, int hmax,
+// Pattern pass, kernel B: column indices, ascending within each row.  The hit cells of a source cell are read
+// off its node lists (the target cell at the first sorted position of every rank).
+__global__ void __launch_bounds__(kThreads) k_emit_cols(DevLattice L, NodeLists nl, int hmax,
                                                        const int64_t* __restrict__ rowptr, int32_t* __restrict__ colidx)
 {
     extern __shared__ __align__(16) char smem[];
     constexpr int T = kThreads;
     const int tid = threadIdx.x;
-    char* sp = smem;
-    double* s_thr_p = (double*)carve(sp, 8 * (size_t)L.pe_pad);
-    double* s_thr_q = (double*)carve(sp, 8 * (size_t)L.qe_pad);
-    int* hitcell = (int*)carve(sp, 4 * (size_t)hmax);
-    for (int k = tid; k < L.pe_pad; k += T) s_thr_p[k] = L.thr_p[k];
-    for (int k = tid; k < L.qe_pad; k += T) s_thr_q[k] = L.thr_q[k];
-    const int cell = cell_begin + blockIdx.x;
-    const int ci = cell / L.Nq, cj = cell - ci * L.Nq;
-    const CellGeom g = cell_geom(L.pe, L.qe, ci, cj);
+    int* hitcell = (int*)smem;
     const int H = nl.hits[blockIdx.x], ntot = nl.ntot[blockIdx.x];
-    const unsigned short* g_sorted = nl.sorted + (size_t)blockIdx.x * L.nnode;
     const unsigned short* g_rkpos = nl.rkpos + (size_t)blockIdx.x * L.nnode;
-    __syncthreads();
+    const int* g_tcell = nl.tcell + (size_t)blockIdx.x * L.nnode;
     for (int pos = tid; pos < ntot; pos += T) {
         const int r = g_rkpos[pos];
-        if (pos > 0 && g_rkpos[pos - 1] == r) continue;
-        int c, a, b;
-        split_node(L, g_sorted[pos], c, a, b);
-        double p, q, P2, Q2;
-        map_node_sq(g, L.tp[a], L.tq[b], L.tx[c], p, q, P2, Q2);
-        hitcell[r] = target_cell_sq(s_thr_p, L.pe_pad, L.Np, s_thr_q, L.qe_pad, L.Nq, P2, Q2);
+        if (pos == 0 || g_rkpos[pos - 1] != r) hitcell[r] = g_tcell[pos];
     }
     __syncthreads();
     for (int a = 0; a < L.n_ch; ++a) {
@@ -238,13 +228,13 @@ cudaError_t launch_scan_rows(const DevLattice& L, int n_blk, const int* hits, in
     return cudaGetLastError();
 }
 
-cudaError_t launch_emit_cols(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, int hmax,
-                             const int64_t* rowptr, int32_t* colidx, cudaStream_t st)
+cudaError_t launch_emit_cols(const DevLattice& L, int n_blk, const NodeLists& nl, int hmax, const int64_t* rowptr,
+                             int32_t* colidx, cudaStream_t st)
 {
-    const size_t sm = al16(8 * (size_t)L.pe_pad) + al16(8 * (size_t)L.qe_pad) + al16(4 * (size_t)std::max(hmax, 1));
+    const size_t sm = al16(4 * (size_t)std::max(hmax, 1));
     cudaError_t e = cudaFuncSetAttribute(k_emit_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
-    k_emit_cols<<<n_blk, kThreads, sm, st>>>(L, cell_begin, nl, hmax, rowptr, colidx);
+    k_emit_cols<<<n_blk, kThreads, sm, st>>>(L, nl, hmax, rowptr, colidx);
     ++g_launches;
     return cudaGetLastError();
 }

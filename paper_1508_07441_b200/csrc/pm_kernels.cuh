@@ -21,15 +21,15 @@ void count_launch();
 cudaError_t launch_map_sort(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, cudaStream_t st);
 cudaError_t launch_scan_rows(const DevLattice& L, int n_blk, const int* hits, int64_t* cellbase, int64_t* rowptr,
                              int64_t* summary, cudaStream_t st);
-cudaError_t launch_emit_cols(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, int hmax,
-                             const int64_t* rowptr, int32_t* colidx, cudaStream_t st);
+cudaError_t launch_emit_cols(const DevLattice& L, int n_blk, const NodeLists& nl, int hmax, const int64_t* rowptr,
+                             int32_t* colidx, cudaStream_t st);
 
 // fill pass (pm_fill.cuh): variant selection and launch
 struct FillLaunch { const void* fn; int nw, grid; FillSmem smem; const char* name; };
 bool fill_has_spec(unsigned long long tables_hash);
-cudaError_t fill_plan(const DevLattice& L, unsigned long long tables_hash, int hmax, int n_sm, FillLaunch* out);
-cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl, int hmax,
-                        const int64_t* rowptr, double* vals, double* accG, cudaStream_t st);
+cudaError_t fill_plan(const DevLattice& L, unsigned long long tables_hash, int n_sm, FillLaunch* out);
+cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl,
+                        const int64_t* rowptr, double* vals, int* counter, cudaStream_t st);
 
 cudaError_t launch_spmv(int64_t n_rows, const int64_t* rowptr, const int32_t* colidx, const double* vals,
                         const double* x, double* y, cudaStream_t st);

@@ -93,8 +93,13 @@ int32_t pm_build_host(pm_lattice* lat, int64_t device_budget_bytes, int64_t* h_r
             return PM_ERR_NOMEM;
         }
     }
+    // The lattice's node lists and work counter serve one block at a time: block b+1's kernels wait for block b's
+    // fill (event), so only the device->host copies of block b overlap the kernels of block b+1.
+    cudaEvent_t filled = nullptr;
+    if (cudaEventCreateWithFlags(&filled, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return PM_ERR_CUDA; }
     for (int b = 0; b < nb && rc == PM_OK; ++b) {
         DevBuf& B = buf[b % nset];
+        if (b > 0 && cudaStreamWaitEvent(B.st, filled, 0) != cudaSuccess) { rc = PM_ERR_CUDA; break; }
         const int cb = P.cuts[(size_t)b], ce = P.cuts[(size_t)b + 1];
         const int64_t off = P.rowptr[(size_t)cb * P.n_ch];
         int64_t nnz = 0;
@@ -104,10 +109,12 @@ int32_t pm_build_host(pm_lattice* lat, int64_t device_budget_bytes, int64_t* h_r
         if (nnz != P.rowptr[(size_t)ce * P.n_ch] - off) { rc = PM_ERR_STATE; break; }
         rc = pm_fill(lat, cb, ce, B.rowptr, B.val, B.st);
         if (rc) break;
+        if (cudaEventRecord(filled, B.st) != cudaSuccess) { rc = PM_ERR_CUDA; break; }
         if (cudaMemcpyAsync(h_colidx + off, B.col, sizeof(int32_t) * (size_t)nnz, cudaMemcpyDeviceToHost, B.st) != cudaSuccess ||
             cudaMemcpyAsync(h_vals + off, B.val, sizeof(double) * (size_t)nnz, cudaMemcpyDeviceToHost, B.st) != cudaSuccess)
             rc = PM_ERR_CUDA;
     }
+    cudaEventDestroy(filled);
     for (int s = 0; s < nset; ++s)
         if (buf[s].st && cudaStreamSynchronize(buf[s].st) != cudaSuccess && rc == PM_OK) rc = PM_ERR_CUDA;
     return rc;
