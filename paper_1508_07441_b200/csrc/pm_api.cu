@@ -46,6 +46,9 @@ struct pm_lattice {
     int64_t* h_summary = nullptr;      // pinned
     int hits_cap = 0;
     int hmax = -1, pat_begin = -1, pat_end = -1;     // max hit cells, and the cell range, of the last pattern call
+    bool pat_count_only = false;       // the last pattern call only counted: an emit call for the same range reuses its lists
+    bool have_plan = false;
+    pm::FillLaunch plan{};
     int* d_counter = nullptr;          // work counter of the fill kernel
     unsigned long long hash = 0;       // pm::tables_hash of T (selects a generated fill kernel)
     int n_sm = 0;
@@ -156,6 +159,7 @@ int32_t ensure_device(pm_lattice* L)
     L->dev = D;
     L->dirty = false;
     L->hmax = -1;
+    L->have_plan = false;
     return PM_OK;
 }
 
@@ -339,8 +343,11 @@ int32_t pm_pattern(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int64_
         *nnz_host = 0; lat->hmax = 0; lat->pat_begin = cell_begin; lat->pat_end = cell_end;
         return PM_OK;
     }
-    // The node lists of the last call are reused when the range is the same (count first, then emit: one map pass).
-    const bool reuse = lat->hmax >= 0 && lat->pat_begin == cell_begin && lat->pat_end == cell_end && lat->hits_cap >= n_blk;
+    // Two-phase use (count, allocate, emit): the emit call reuses the node lists of the count call of the same range,
+    // so the nodes are mapped once.  Any other call maps afresh.
+    const bool reuse = lat->hmax >= 0 && lat->pat_count_only && d_colidx && lat->pat_begin == cell_begin && lat->pat_end == cell_end
+                    && lat->hits_cap >= n_blk;
+    lat->pat_count_only = (d_colidx == nullptr);
     if (!reuse) {
         lat->hmax = -1;
         if ((rc = ensure_cell_scratch(lat, n_blk))) return rc;
@@ -372,11 +379,14 @@ int32_t pm_fill(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const int
     if (cell_begin == cell_end) return PM_OK;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int n_blk = cell_end - cell_begin;
-    pm::FillLaunch F;
-    cudaError_t e = pm::fill_plan(lat->dev, lat->hash, lat->n_sm, &F);
-    if (e == cudaErrorInvalidConfiguration) { cudaGetLastError(); return fail(PM_ERR_NOMEM, "channel set needs more shared memory than one SM has"); }
-    if (e != cudaSuccess) return cuda_fail(e, "fill_plan");
-    e = pm::launch_fill(lat->dev, F, cell_begin, n_blk, lat->nl, d_rowptr, d_vals, lat->d_counter, st);
+    cudaError_t e;
+    if (!lat->have_plan) {
+        e = pm::fill_plan(lat->dev, lat->hash, lat->n_sm, &lat->plan);
+        if (e == cudaErrorInvalidConfiguration) { cudaGetLastError(); return fail(PM_ERR_NOMEM, "channel set needs more shared memory than one SM has"); }
+        if (e != cudaSuccess) return cuda_fail(e, "fill_plan");
+        lat->have_plan = true;
+    }
+    e = pm::launch_fill(lat->dev, lat->plan, cell_begin, n_blk, lat->nl, d_rowptr, d_vals, lat->d_counter, st);
     if (e != cudaSuccess) return cuda_fail(e, "k_fill");
     return PM_OK;
 }

@@ -47,9 +47,10 @@ struct SpecGeneric {
 };
 
 struct FillSmem {           // byte offsets into dynamic shared memory, computed on the host
-    int dp, dq, tp, tq, tx, sx, wx, bra, odesc, ofi, oc, warp0, warp_bytes, w_tile, w_sseg, w_acc, w_wpa, w_wqb, total;
+    int dp, dq, tp, tq, tx, sx, wx, bra, odesc, ofi, oc, warp0, warp_bytes, w_tile, w_sseg, w_acc, w_norm, w_wpa, w_wqb, total;
 };
 
+constexpr int kRowBatch = 4;           // finished targets held per warp before their row entries are written
 constexpr int kTileStride = 33;        // double2 per K-tile row: 32 nodes + 1 pad (conflict-free rows and columns)
 
 inline int fill_align16(int b) { return (b + 15) & ~15; }
@@ -69,7 +70,8 @@ inline FillSmem fill_smem_plan(const DevLattice& L, int nw)
     auto wtake = [&](int bytes) { int r = w; w += fill_align16(bytes); return r; };
     s.w_tile = wtake(16 * kTileStride * np);
     s.w_sseg = wtake(16 * np);
-    s.w_acc = wtake(8 * L.n_fun);
+    s.w_acc = wtake(8 * L.n_fun * kRowBatch);
+    s.w_norm = wtake(8 * kRowBatch);
     s.w_wpa = wtake(8 * L.n_p); s.w_wqb = wtake(8 * L.n_q);
     s.warp_bytes = w;
     s.warp0 = take(w * nw);
@@ -101,7 +103,8 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
     double2* s_tile = (double2*)(wsm + S.w_tile);
     double2* s_sseg2 = (double2*)(wsm + S.w_sseg);
     const double* s_sseg = (const double*)s_sseg2;
-    double* s_acc = (double*)(wsm + S.w_acc);
+    double* s_acc = (double*)(wsm + S.w_acc);         // [kRowBatch][nf] sums of finished targets
+    double* s_norm = (double*)(wsm + S.w_norm);
     double* s_wpa = (double*)(wsm + S.w_wpa);
     double* s_wqb = (double*)(wsm + S.w_wqb);
 
@@ -162,7 +165,30 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         for (int k = lane; k < L.n_p; k += 32) s_wpa[k] = __dmul_rn(g.hp, L.wp[k]);
         for (int k = lane; k < L.n_q; k += 32) s_wqb[k] = __dmul_rn(g.hq, L.wq[k]);
         __syncwarp();
-        int kcur = 0;                                   // rank of the current target = its position in every row
+        int kcur = 0, kdone = 0;                        // targets finished / written; a target's rank is its position in every row
+        // ---- E: lane = output (alpha, m-th coupled alpha'): P = norm_t * sum_L c^L acc_t[f] for targets k0 .. k0+nb-1
+        auto write_rows = [&](int k0, int nb) {
+            for (int o = lane; o < L.totcoup; o += 32) {
+                const int od = s_odesc[o], fi = s_ofi[o];
+                const int clo = od & 4095, nc = (od >> 12) & 127, mm = od >> 19;
+                const double c0 = s_oc[3 * o], c1 = s_oc[3 * o + 1], c2 = s_oc[3 * o + 2];
+                const int f0 = fi & 255, f1 = (fi >> 8) & 255, f2 = (fi >> 16) & 255, nt = fi >> 24;
+                double* out = row0 + ((size_t)H * clo + (size_t)k0 * nc + mm);
+#pragma unroll
+                for (int bb = 0; bb < kRowBatch; ++bb) {
+                    if (bb < nb) {
+                        const double* acc = s_acc + bb * nf;
+                        double v = fma(c2, acc[f2], fma(c1, acc[f1], c0 * acc[f0]));
+                        if (nt > 3) {
+                            const int t0 = L.ot_off[o];
+                            for (int t = 3; t < nt; ++t) v = fma(L.ot_c[t0 + t], acc[L.ot_f[t0 + t]], v);
+                        }
+                        out[(size_t)bb * nc] = v * s_norm[bb];
+                    }
+                }
+            }
+            __syncwarp();
+        };
 
         // ---- C + D: 32 sorted nodes per step; the node ids of the next two steps are already in flight
         double runT[NCH];
@@ -215,32 +241,31 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 }
             }
             __syncwarp();
-            // lane = slot pair: walks the tile's nodes, up to 4 per step, never across a segment end
+            // lane = slot pair: walks the tile's nodes in steps of 8, 4 or 1; a segment may end only at a step's last node
             for (int j = 0; j < cnt;) {
-                const int nbnd = __ffs((smask >> j) & 0xfu);             // 1-based offset of the next segment end, 0 = none in 4
-                const int step = nbnd ? nbnd : min(4, cnt - j);
-                if (step == 4) {
+                const unsigned rest = smask >> j;
+                const int step = ((rest & 0x7fu) == 0 && j + 8 <= cnt) ? 8 : ((rest & 0x7u) == 0 && j + 4 <= cnt) ? 4 : 1;
 #pragma unroll
-                    for (int i = 0; i < NPC; ++i) {
-                        const int sp = i * 32 + lane;
-                        if (sp < np) {
-                            const double2* row = s_tile + sp * kTileStride + j;
+                for (int i = 0; i < NPC; ++i) {
+                    const int sp = i * 32 + lane;
+                    if (sp < np) {
+                        const double2* row = s_tile + sp * kTileStride + j;
+                        if (step == 8) {
+                            const double2 d0 = row[0], d1 = row[1], d2 = row[2], d3 = row[3], d4 = row[4], d5 = row[5], d6 = row[6], d7 = row[7];
+                            runS[i].x += ((d0.x + d1.x) + (d2.x + d3.x)) + ((d4.x + d5.x) + (d6.x + d7.x));
+                            runS[i].y += ((d0.y + d1.y) + (d2.y + d3.y)) + ((d4.y + d5.y) + (d6.y + d7.y));
+                        } else if (step == 4) {
                             const double2 d0 = row[0], d1 = row[1], d2 = row[2], d3 = row[3];
                             runS[i].x += (d0.x + d1.x) + (d2.x + d3.x);
                             runS[i].y += (d0.y + d1.y) + (d2.y + d3.y);
-                        }
-                    }
-                } else {
-                    for (int r = 0; r < step; ++r) {
-#pragma unroll
-                        for (int i = 0; i < NPC; ++i) {
-                            const int sp = i * 32 + lane;
-                            if (sp < np) { const double2 d = s_tile[sp * kTileStride + j + r]; runS[i].x += d.x; runS[i].y += d.y; }
+                        } else {
+                            const double2 d = row[0];
+                            runS[i].x += d.x; runS[i].y += d.y;
                         }
                     }
                 }
                 j += step;
-                if (!nbnd) continue;
+                if (!((smask >> (j - 1)) & 1u)) continue;
                 const int jb = j - 1;                                    // node jb ends a (t, c) segment
 #pragma unroll
                 for (int i = 0; i < NPC; ++i) {
@@ -268,36 +293,27 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 }
                 __syncwarp();
                 if (!((tmask >> jb) & 1u)) continue;
-                // ---- E: node jb also ends target t: its sums are complete, write its entry of every row
+                // node jb also ends target t: its sums are complete; kRowBatch finished targets are written together
+                {
+                    const int slot = kcur - kdone;
 #pragma unroll
-                for (int ch = 0; ch < NCH; ++ch) {
-                    const int f = ch * 32 + lane;
-                    if (f < nf) s_acc[f] = runT[ch];
-                    runT[ch] = 0.0;
-                }
-                __syncwarp();
-                const int tcell = __shfl_sync(0xffffffffu, tC, jb);
-                const int ic = tcell / L.Nq, jc = tcell - ic * L.Nq;
-                const double norm = 1.0 / sqrt(dsrc * (s_dp[ic] * s_dq[jc]));
-                for (int o = lane; o < L.totcoup; o += 32) {
-                    const int od = s_odesc[o], fi = s_ofi[o];
-                    const int clo = od & 4095, nc = (od >> 12) & 127, mm = od >> 19;
-                    double v = s_oc[3 * o] * s_acc[fi & 255];
-                    v = fma(s_oc[3 * o + 1], s_acc[(fi >> 8) & 255], v);
-                    v = fma(s_oc[3 * o + 2], s_acc[(fi >> 16) & 255], v);
-                    const int nt = fi >> 24;
-                    if (nt > 3) {
-                        const int t0 = L.ot_off[o];
-                        for (int t = 3; t < nt; ++t) v = fma(L.ot_c[t0 + t], s_acc[L.ot_f[t0 + t]], v);
+                    for (int ch = 0; ch < NCH; ++ch) {
+                        const int f = ch * 32 + lane;
+                        if (f < nf) s_acc[slot * nf + f] = runT[ch];
+                        runT[ch] = 0.0;
                     }
-                    row0[(size_t)H * clo + (size_t)kcur * nc + mm] = v * norm;
+                    const int tcell = __shfl_sync(0xffffffffu, tC, jb);
+                    const int ic = tcell / L.Nq, jc = tcell - ic * L.Nq;
+                    if (lane == 0) s_norm[slot] = 1.0 / sqrt(dsrc * (s_dp[ic] * s_dq[jc]));
+                    ++kcur;
+                    __syncwarp();
+                    if (kcur - kdone == kRowBatch) { write_rows(kdone, kRowBatch); kdone = kcur; }
                 }
-                ++kcur;
-                __syncwarp();
             }
             __syncwarp();
             mC = mN; tC = tN; mN = mF; tN = tF;
         }
+        if (kcur > kdone) write_rows(kdone, kcur - kdone);
     }
 }
 
