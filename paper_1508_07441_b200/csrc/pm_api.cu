@@ -80,11 +80,11 @@ int32_t ensure_device(pm_lattice* L)
     int dev = -1;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(PM_ERR_DEVICE, std::string("no CUDA device: ") + cudaGetErrorString(e)); }
+    if (!L->dirty && L->device == dev) return PM_OK;     // (cudaGetDeviceProperties costs milliseconds: first use only)
     cudaDeviceProp prop;
     e = cudaGetDeviceProperties(&prop, dev);
     if (e != cudaSuccess) return fail(PM_ERR_DEVICE, std::string("cudaGetDeviceProperties: ") + cudaGetErrorString(e));
     if (prop.major < 10) return fail(PM_ERR_DEVICE, "libpm is built for sm_100a (B200); this device is older");
-    if (!L->dirty && L->device == dev) return PM_OK;
     free_device(L);
     L->device = dev;
     L->n_sm = prop.multiProcessorCount;
