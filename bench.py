@@ -82,10 +82,13 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def build_flops(lat_api, h, wl, nnz):
-    """Algorithmic FP64 flops of one build from pm_lattice_work."""
-    per_node, per_hit, n_pairs = lat_api.pm_lattice_work(h)
-    return per_node * wl.n_cells * wl.nodes_per_cell + per_hit * (nnz / n_pairs), per_node, per_hit
+def build_flops(lat_api, h):
+    """Algorithmic FP64 flops of one build: pm_lattice_work x pm_pattern_counts."""
+    per_node, per_seg, per_hit, _ = lat_api.pm_lattice_work(h)
+    nodes, segs, hits = lat_api.pm_pattern_counts(h)
+    return per_node * nodes + per_seg * segs + per_hit * hits, {"flop_per_node": per_node, "flop_per_segment": per_seg,
+                                                                 "flop_per_hit_cell": per_hit, "nodes_on_grid": nodes,
+                                                                 "segments": segs, "hit_cells": hits}
 
 
 def oracle_sample(wl, seconds_target=15.0, max_cells=64):
@@ -201,7 +204,7 @@ def main():
     pk = _peaks()
     n_sm = torch.cuda.get_device_properties(local).multi_processor_count
     peak_tf = n_sm * FP64_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 * 1e-12
-    flops, per_node, per_hit = build_flops(api, lat.h, wl, nnz)
+    flops, work = build_flops(api, lat.h)
     fill_avg = float(np.mean(fill_ms)) * 1e-3
     achieved_tf = flops / fill_avg * 1e-12
     dfma = api.pm_diag_dfma_tflops()
@@ -209,7 +212,7 @@ def main():
             "frac": achieved_tf / peak_tf, "traffic": None,
             "peak_source": f"{n_sm} SM x {FP64_LANES_PER_SM} DFMA lanes x 2 x {pk['sm_max_mhz']:.0f} MHz ({pk['src']} clock); "
                            f"DFMA microbenchmark on this box: {dfma:.1f} TFLOP/s",
-            "flop_per_node": per_node, "flop_per_hit_cell": per_hit, "fill_ms": fill_avg * 1e3,
+            "flops_per_launch": flops, "work": work, "fill_ms": fill_avg * 1e3,
             "csr_write_gbs": 8.0 * nnz / fill_avg * 1e-9, "hbm_peak_gbs": pk["hbm_gbs"]}
 
     # ---- end to end through the C ABI with HOST buffers (D2H copies inside the timed region)

@@ -74,6 +74,9 @@ int32_t pm_lattice_coupling(const pm_lattice* lat, uint8_t* coupled, int32_t* n_
 
 /* Pattern pass (the paper's step 2a 'pre-selection') for the rows of source cells
  * [cell_begin, cell_end):
+ * The pass bins every quadrature node of the range once and keeps, in library-owned device memory, the node lists
+ * sorted by target cell (about 8 bytes per node); pm_fill of the same range reads them.  Calling with d_colidx = NULL
+ * (count) and then with d_colidx for the same range maps the nodes only once.
  *   d_rowptr : device, (cell_end-cell_begin)*n_ch + 1 int64, block-local (d_rowptr[0] = 0)
  *   d_colidx : device, nnz int32 GLOBAL column indices — or NULL to count only (d_rowptr is still written)
  *   colidx_capacity : number of int32 d_colidx can hold (ignored when d_colidx is NULL); if nnz exceeds it
@@ -84,7 +87,8 @@ int32_t pm_pattern(pm_lattice* lat, int32_t cell_begin, int32_t cell_end,
                    int64_t* nnz_host, void* cuda_stream);
 
 /* Fill pass (step 2b 'calculation of nonzero elements'): values of the block
- * whose d_rowptr was produced by pm_pattern for the same [cell_begin, cell_end).  d_vals: device, nnz doubles,
+ * whose d_rowptr was produced by the LAST pm_pattern call on this lattice, for the same [cell_begin, cell_end)
+ * (PM_ERR_STATE otherwise: the fill reads that call's node lists).  d_vals: device, nnz doubles,
  * every entry is written exactly once; sums are formed in a fixed order (bitwise reproducible run to run). */
 int32_t pm_fill(pm_lattice* lat, int32_t cell_begin, int32_t cell_end,
                 const int64_t* d_rowptr, double* d_vals, void* cuda_stream);
@@ -103,10 +107,19 @@ int32_t pm_build_host(pm_lattice* lat, int64_t device_budget_bytes,
                       int64_t* h_rowptr, int32_t* h_colidx, double* h_vals, int64_t capacity,
                       int64_t* nnz_total, int32_t* n_blocks);
 
-/* Algorithmic work of this lattice's formulation (add = mul = div = sqrt = 1 flop, FMA = 2;
- * comparisons and integer work not counted): FP64 flops per quadrature node and per hit (source, target) cell
- * pair.  One build = flop_per_node * n_cells*n_p*n_q*n_x + flop_per_hit_cell * nnz/n_coupled_pairs.  Host only. */
-int32_t pm_lattice_work(const pm_lattice* lat, double* flop_per_node, double* flop_per_hit_cell, int32_t* n_coupled_pairs);
+/* Algorithmic work of this lattice's formulation (add = mul = div = sqrt = rsqrt = 1 flop, FMA = 2;
+ * comparisons and integer work not counted): FP64 flops per quadrature node that lands on the grid, per
+ * (target cell, x-node) segment of a source cell's sorted node list (the bra harmonics are applied once per
+ * segment), and per hit (source, target) cell pair.  One build =
+ *   flop_per_node * nodes_on_grid + flop_per_segment * segments + flop_per_hit_cell * hit_cells,
+ * the three counts coming from pm_pattern_counts.  Host only. */
+int32_t pm_lattice_work(const pm_lattice* lat, double* flop_per_node, double* flop_per_segment, double* flop_per_hit_cell,
+                        int32_t* n_coupled_pairs);
+
+/* Counts of the last pm_pattern call on this lattice (host out): quadrature nodes that landed on the grid,
+ * (target cell, x-node) segments, hit (source, target) cell pairs (= nnz / number of coupled channel pairs).
+ * PM_ERR_STATE before the first pm_pattern. */
+int32_t pm_pattern_counts(const pm_lattice* lat, int64_t* nodes_on_grid, int64_t* segments, int64_t* hit_cells);
 
 /* Diagnostic: measured FP64 FMA throughput of the current device in TFLOP/s (a dependent-free DFMA loop on every
  * SM, timed with CUDA events on `cuda_stream`); the roofline denominator is stated beside it in DESIGN.md sec. 7. */

@@ -22,7 +22,7 @@ ERRORS = {-1: "PM_ERR_ARG", -2: "PM_ERR_GRID", -3: "PM_ERR_CHANNEL", -4: "PM_ERR
           -6: "PM_ERR_NOMEM", -7: "PM_ERR_STATE", -8: "PM_ERR_OVERFLOW", -9: "PM_ERR_DEVICE"}
 
 EXPORTS = ["pm_lattice_create", "pm_lattice_destroy", "pm_lattice_dims", "pm_lattice_rule", "pm_lattice_set_rule",
-           "pm_lattice_coupling", "pm_lattice_work", "pm_diag_dfma_tflops", "pm_pattern", "pm_fill", "pm_spmv", "pm_build_host_count", "pm_build_host",
+           "pm_lattice_coupling", "pm_lattice_work", "pm_pattern_counts", "pm_diag_dfma_tflops", "pm_pattern", "pm_fill", "pm_spmv", "pm_build_host_count", "pm_build_host",
            "pm_launch_count", "pm_last_error"]
 
 
@@ -58,7 +58,8 @@ def lib():
     L.pm_lattice_rule.argtypes = [_vp, C.c_int32, _dp, _dp]
     L.pm_lattice_set_rule.argtypes = [_vp, C.c_int32, _dp, _dp]
     L.pm_lattice_coupling.argtypes = [_vp, C.POINTER(C.c_uint8), _i32p]
-    L.pm_lattice_work.argtypes = [_vp, _dp, _dp, _i32p]
+    L.pm_lattice_work.argtypes = [_vp, _dp, _dp, _dp, _i32p]
+    L.pm_pattern_counts.argtypes = [_vp, _i64p, _i64p, _i64p]
     L.pm_diag_dfma_tflops.argtypes = [_dp, _vp]
     L.pm_pattern.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, C.c_int64, _i64p, _vp]
     L.pm_fill.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, _vp]
@@ -130,10 +131,17 @@ def pm_lattice_coupling(h, n_ch):
 
 
 def pm_lattice_work(h):
-    """(flop per node, flop per hit cell pair, number of coupled channel pairs) of the formulation."""
-    a, b, n = C.c_double(), C.c_double(), C.c_int32()
-    _check(lib().pm_lattice_work(h, C.byref(a), C.byref(b), C.byref(n)))
-    return a.value, b.value, n.value
+    """(flop per node on the grid, flop per (target, x-node) segment, flop per hit cell pair, coupled channel pairs)."""
+    a, s_, b, n = C.c_double(), C.c_double(), C.c_double(), C.c_int32()
+    _check(lib().pm_lattice_work(h, C.byref(a), C.byref(s_), C.byref(b), C.byref(n)))
+    return a.value, s_.value, b.value, n.value
+
+
+def pm_pattern_counts(h):
+    """(nodes on the grid, (target, x-node) segments, hit cell pairs) of the last pm_pattern call."""
+    a, s_, b = C.c_int64(), C.c_int64(), C.c_int64()
+    _check(lib().pm_pattern_counts(h, C.byref(a), C.byref(s_), C.byref(b)))
+    return a.value, s_.value, b.value
 
 
 def pm_diag_dfma_tflops(stream=None):

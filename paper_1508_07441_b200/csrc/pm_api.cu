@@ -47,6 +47,7 @@ struct pm_lattice {
     int hits_cap = 0;
     int hmax = -1, pat_begin = -1, pat_end = -1;     // max hit cells, and the cell range, of the last pattern call
     bool pat_count_only = false;       // the last pattern call only counted: an emit call for the same range reuses its lists
+    int64_t counts[3] = {0, 0, 0};     // nodes on the grid, (target, x-node) segments, hit cells of the last pattern call
     bool have_plan = false;
     pm::FillLaunch plan{};
     int* d_counter = nullptr;          // work counter of the fill kernel
@@ -65,6 +66,7 @@ void free_device(pm_lattice* L)
     if (L->nl.tcell) cudaFree(L->nl.tcell);
     if (L->nl.ntot) cudaFree(L->nl.ntot);
     if (L->nl.hits) cudaFree(L->nl.hits);
+    if (L->nl.nseg) cudaFree(L->nl.nseg);
     if (L->d_cellbase) cudaFree(L->d_cellbase);
     if (L->d_summary) cudaFree(L->d_summary);
     if (L->h_summary) cudaFreeHost(L->h_summary);
@@ -139,9 +141,9 @@ int32_t ensure_device(pm_lattice* L)
 
     if ((e = cudaMalloc(&L->d_blob, blob.size())) != cudaSuccess) return cuda_fail(e, "cudaMalloc(tables)");
     if ((e = cudaMemcpy(L->d_blob, blob.data(), blob.size(), cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_fail(e, "cudaMemcpy(tables)");
-    if ((e = cudaMalloc(&L->d_summary, 2 * sizeof(int64_t))) != cudaSuccess) return cuda_fail(e, "cudaMalloc(summary)");
+    if ((e = cudaMalloc(&L->d_summary, 4 * sizeof(int64_t))) != cudaSuccess) return cuda_fail(e, "cudaMalloc(summary)");
     if ((e = cudaMalloc(&L->d_counter, sizeof(int))) != cudaSuccess) return cuda_fail(e, "cudaMalloc(counter)");
-    if ((e = cudaMallocHost(&L->h_summary, 2 * sizeof(int64_t))) != cudaSuccess) return cuda_fail(e, "cudaMallocHost(summary)");
+    if ((e = cudaMallocHost(&L->h_summary, 4 * sizeof(int64_t))) != cudaSuccess) return cuda_fail(e, "cudaMallocHost(summary)");
     char* b = L->d_blob;
     D.pe = (const double*)(b + o_pe); D.qe = (const double*)(b + o_qe);
     D.thr_p = (const double*)(b + o_thp); D.thr_q = (const double*)(b + o_thq);
@@ -171,6 +173,7 @@ int32_t ensure_cell_scratch(pm_lattice* L, int n_blk)
     if (L->nl.tcell) cudaFree(L->nl.tcell);
     if (L->nl.ntot) cudaFree(L->nl.ntot);
     if (L->nl.hits) cudaFree(L->nl.hits);
+    if (L->nl.nseg) cudaFree(L->nl.nseg);
     if (L->d_cellbase) cudaFree(L->d_cellbase);
     L->nl = pm::NodeLists{}; L->d_cellbase = nullptr; L->hits_cap = 0;
     const size_t nn = (size_t)n_blk * (size_t)L->dev.nnode;
@@ -180,7 +183,8 @@ int32_t ensure_cell_scratch(pm_lattice* L, int n_blk)
     if ((e = cudaMalloc(&L->nl.tcell, sizeof(int) * nn)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(node lists)");
     if ((e = cudaMalloc(&L->nl.ntot, sizeof(int) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(ntot)");
     if ((e = cudaMalloc(&L->nl.hits, sizeof(int) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(hits)");
-    if ((e = cudaMalloc(&L->d_cellbase, sizeof(int64_t) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(cellbase)");
+    if ((e = cudaMalloc(&L->nl.nseg, sizeof(int) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(nseg)");
+    if ((e = cudaMalloc(&L->d_cellbase, sizeof(int64_t) * ((size_t)n_blk + 1))) != cudaSuccess) return cuda_fail(e, "cudaMalloc(cellbase)");
     L->hits_cap = n_blk;
     return PM_OK;
 }
@@ -287,27 +291,31 @@ int32_t pm_lattice_coupling(const pm_lattice* lat, uint8_t* coupled, int32_t* n_
     return PM_OK;
 }
 
-int32_t pm_lattice_work(const pm_lattice* lat, double* flop_per_node, double* flop_per_hit_cell, int32_t* n_coupled_pairs)
+int32_t pm_lattice_work(const pm_lattice* lat, double* flop_per_node, double* flop_per_segment, double* flop_per_hit_cell,
+                        int32_t* n_coupled_pairs)
 {
     if (!lat) return fail(PM_ERR_ARG, "lat is NULL");
     const pm::Tables& T = lat->T;
-    // node generation + map (p, q, pq, p^2, q^2, pqx, P2, Q2, 2 sqrt) = 18, weight 4, omega 3
-    double node = 25.0;
-    // rotated directions from components: 4 components (8), two norms (2*(3+1)), 4 scalings
-    node += 20.0;
-    // two sets of Y_lm, m >= 0, l <= lmax: diagonal terms 2 flop, the others 4 flop
-    const int lmax = T.lmax;
-    node += 2.0 * (2.0 * lmax + 4.0 * (lmax * (lmax + 1) / 2));
-    // ket bipolar harmonics: c*Yp*Yq accumulated (mul + FMA = 3) per term, one scaling by omega per slot
-    node += 3.0 * (double)T.kt_c.size() + (double)T.n_slot;
-    // orbital functions: one FMA per (function, M) whose bra weight is not structurally zero
-    double fma = 0.0;
-    for (const pm::OrbFun& f : T.fun) for (int i = 0; i < f.nM; ++i) if (T.slot_w[(size_t)f.sa0 + i] != 0.0) fma += 1.0;
-    node += 2.0 * fma;
-    if (flop_per_node) *flop_per_node = node;
-    // per hit cell: normalisation (~8), one FMA per (channel pair, L) term, one scaling per output
-    if (flop_per_hit_cell) *flop_per_hit_cell = 8.0 + 2.0 * (double)T.ot_c.size() + (double)T.totcoup;
+    // per node on the grid (pm_fill.cuh, phase C): node map 16, weight and omega 7 (one rsqrt), rotated directions 20
+    // (two rsqrt), the generated ket code, and one add per slot in the segment sum (phase D)
+    if (flop_per_node) *flop_per_node = 16.0 + 7.0 + 20.0 + pm::ket_flops(T) + (double)T.n_slot;
+    // per (target, x-node) segment: sum_M bra*S per orbital function (nM multiply-adds) and one add into the target sum
+    double seg = 0.0;
+    for (const pm::OrbFun& f : T.fun) seg += 2.0 * f.nM;
+    if (flop_per_segment) *flop_per_segment = seg;
+    // per hit cell: normalisation 5, per output one multiply-add per (channel pair, L) term and the scaling by the norm
+    if (flop_per_hit_cell) *flop_per_hit_cell = 5.0 + 2.0 * (double)T.ot_c.size();
     if (n_coupled_pairs) *n_coupled_pairs = T.totcoup;
+    return PM_OK;
+}
+
+int32_t pm_pattern_counts(const pm_lattice* lat, int64_t* nodes_on_grid, int64_t* segments, int64_t* hit_cells)
+{
+    if (!lat) return fail(PM_ERR_ARG, "lat is NULL");
+    if (lat->hmax < 0) return fail(PM_ERR_STATE, "pm_pattern_counts needs a preceding pm_pattern");
+    if (nodes_on_grid) *nodes_on_grid = lat->counts[0];
+    if (segments) *segments = lat->counts[1];
+    if (hit_cells) *hit_cells = lat->counts[2];
     return PM_OK;
 }
 
@@ -341,6 +349,7 @@ int32_t pm_pattern(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int64_
         if ((e = cudaMemsetAsync(d_rowptr, 0, sizeof(int64_t), st)) != cudaSuccess) return cuda_fail(e, "memset");
         if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e, "sync");
         *nnz_host = 0; lat->hmax = 0; lat->pat_begin = cell_begin; lat->pat_end = cell_end;
+        lat->counts[0] = lat->counts[1] = lat->counts[2] = 0;
         return PM_OK;
     }
     // Two-phase use (count, allocate, emit): the emit call reuses the node lists of the count call of the same range,
@@ -353,13 +362,14 @@ int32_t pm_pattern(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int64_
         if ((rc = ensure_cell_scratch(lat, n_blk))) return rc;
         if ((e = pm::launch_map_sort(lat->dev, cell_begin, n_blk, lat->nl, st)) != cudaSuccess) return cuda_fail(e, "k_map_sort");
     }
-    if ((e = pm::launch_scan_rows(lat->dev, n_blk, lat->nl.hits, lat->d_cellbase, d_rowptr, lat->d_summary, st)) != cudaSuccess)
+    if ((e = pm::launch_scan_rows(lat->dev, n_blk, lat->nl, lat->d_cellbase, d_rowptr, lat->d_summary, st)) != cudaSuccess)
         return cuda_fail(e, "k_scan_rows");
-    if ((e = cudaMemcpyAsync(lat->h_summary, lat->d_summary, 2 * sizeof(int64_t), cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+    if ((e = cudaMemcpyAsync(lat->h_summary, lat->d_summary, 4 * sizeof(int64_t), cudaMemcpyDeviceToHost, st)) != cudaSuccess)
         return cuda_fail(e, "cudaMemcpyAsync(summary)");
     if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return cuda_fail(e, "pattern: map/scan");
     *nnz_host = lat->h_summary[0];
     lat->hmax = (int)lat->h_summary[1]; lat->pat_begin = cell_begin; lat->pat_end = cell_end;
+    lat->counts[0] = lat->h_summary[2]; lat->counts[1] = lat->h_summary[3]; lat->counts[2] = *nnz_host / lat->T.totcoup;
     if (!d_colidx) return PM_OK;
     if (*nnz_host > colidx_capacity) return fail(PM_ERR_OVERFLOW, "d_colidx too small for this block's nnz");
     if ((e = pm::launch_emit_cols(lat->dev, n_blk, lat->nl, lat->hmax, d_rowptr, d_colidx, st)) != cudaSuccess)

@@ -37,6 +37,7 @@ struct NodeLists {
     int* tcell;                 // [n_blk][nnode]
     int* ntot;                  // [n_blk] nodes on the grid
     int* hits;                  // [n_blk] hit cells H
+    int* nseg;                  // [n_blk] (target, x-node) segments of the sorted list
 };
 
 struct CellGeom { double cp, hp, cq, hq; };

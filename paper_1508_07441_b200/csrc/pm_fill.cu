@@ -27,7 +27,7 @@ const FillVariant kVariants[] = {
 
 int preferred_warps()
 {
-    static const int v = [] { const char* e = std::getenv("PM_FILL_WARPS"); return e ? std::atoi(e) : 8; }();
+    static const int v = [] { const char* e = std::getenv("PM_FILL_WARPS"); return e ? std::atoi(e) : 12; }();
     return v;
 }
 

@@ -124,36 +124,74 @@ __global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_be
     unsigned short* g_rkpos = nl.rkpos + (size_t)blockIdx.x * L.nnode;
     int* g_tcell = nl.tcell + (size_t)blockIdx.x * L.nnode;
     for (int k = tid; k < ntot; k += T) { g_sorted[k] = s_sorted[k]; g_rkpos[k] = s_rkpos[k]; g_tcell[k] = s_tcpos[k]; }
-    if (tid == 0) { nl.hits[blockIdx.x] = H; nl.ntot[blockIdx.x] = ntot; }
+    // (target, x-node) segments of the sorted list: the fill pass applies the bra harmonics once per segment
+    int seg = 0;
+    for (int k = tid; k < ntot; k += T) {
+        const int ck = L.mg_npq ? (int)__umulhi((unsigned)s_sorted[k], L.mg_npq) : (int)s_sorted[k];
+        const int cp = k ? (L.mg_npq ? (int)__umulhi((unsigned)s_sorted[k - 1], L.mg_npq) : (int)s_sorted[k - 1]) : -1;
+        seg += (k == 0 || s_rkpos[k] != s_rkpos[k - 1] || ck != cp) ? 1 : 0;
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) seg += __shfl_xor_sync(0xffffffffu, seg, d);
+    if (lane == 0) hs.scratch[warp] = seg;
+    __syncthreads();
+    if (tid == 0) {
+        int tot = 0;
+        for (int w = 0; w < NW; ++w) tot += hs.scratch[w];
+        nl.hits[blockIdx.x] = H; nl.ntot[blockIdx.x] = ntot; nl.nseg[blockIdx.x] = tot;
+    }
 }
 
-// Pattern pass, kernel S: exclusive scan of hits -> rowptr (block-local), nnz and max hits.  One CTA.
-__global__ void __launch_bounds__(1024) k_scan_rows(DevLattice L, int n_blk, const int* __restrict__ hits,
-                                                   int64_t* __restrict__ cellbase, int64_t* __restrict__ rowptr,
-                                                   int64_t* __restrict__ summary)
+// Pattern pass, kernel S: exclusive scan of the hit counts -> cellbase, nnz and max hits.  One CTA.
+__global__ void __launch_bounds__(1024) k_scan_cells(DevLattice L, int n_blk, const int* __restrict__ hits,
+                                                    const int* __restrict__ ntot, const int* __restrict__ nseg,
+                                                    int64_t* __restrict__ cellbase, int64_t* __restrict__ summary)
 {
     __shared__ long long part[1024];
     __shared__ int pmax[1024];
+    if (blockDim.x == 1024 && threadIdx.x >= 992) {  // last warp: totals of nodes on the grid and of segments (statistics)
+        long long a = 0, s2 = 0;
+        for (int k = threadIdx.x - 992; k < n_blk; k += 32) { a += ntot[k]; s2 += nseg[k]; }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, d); s2 += __shfl_xor_sync(0xffffffffu, s2, d); }
+        if (threadIdx.x == 992) { summary[2] = a; summary[3] = s2; }
+    }
     const int T = blockDim.x, t = threadIdx.x;
     const int chunk = (n_blk + T - 1) / T, b = min(t * chunk, n_blk), e = min(b + chunk, n_blk);
     long long sum = 0; int mx = 0;
     for (int k = b; k < e; ++k) { sum += hits[k]; mx = max(mx, hits[k]); }
     part[t] = sum; pmax[t] = mx;
     __syncthreads();
-    if (t == 0) {
+    if (t < 32) {                                   // warp 0 scans the 1024 partial sums, 32 per lane
         long long run = 0; int m = 0;
-        for (int k = 0; k < T; ++k) { long long v = part[k]; part[k] = run; run += v; m = max(m, pmax[k]); }
-        summary[0] = run * L.totcoup;      // nnz of the block
-        summary[1] = m;                    // max hit cells of any source cell
-        rowptr[(int64_t)n_blk * L.n_ch] = run * L.totcoup;
+        for (int k = t * 32; k < t * 32 + 32; ++k) { run += part[k]; m = max(m, pmax[k]); }
+        long long inc = run;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const long long y = __shfl_up_sync(0xffffffffu, inc, d);
+            const int my = __shfl_xor_sync(0xffffffffu, m, d);
+            if (t >= d) inc += y;
+            m = max(m, my);
+        }
+        long long ex = inc - run;
+        for (int k = t * 32; k < t * 32 + 32; ++k) { const long long v = part[k]; part[k] = ex; ex += v; }
+        if (t == 31) { summary[0] = inc * L.totcoup; summary[1] = m; cellbase[n_blk] = inc; }
     }
     __syncthreads();
     long long run = part[t];
-    for (int k = b; k < e; ++k) {
-        cellbase[k] = run;
-        const int H = hits[k];
-        for (int a = 0; a < L.n_ch; ++a) rowptr[(int64_t)k * L.n_ch + a] = run * L.totcoup + (long long)H * L.cl_off[a];
-        run += H;
+    for (int k = b; k < e; ++k) { cellbase[k] = run; run += hits[k]; }
+}
+
+// Pattern pass, kernel R: rowptr (block-local) from cellbase: row (cell k, alpha) starts at
+// cellbase[k]*totcoup + H_k*cl_off[alpha] (PAPER.md:L339 keeps the row END addresses W; same information).
+__global__ void __launch_bounds__(256) k_write_rowptr(DevLattice L, int n_blk, const int* __restrict__ hits,
+                                                     const int64_t* __restrict__ cellbase, int64_t* __restrict__ rowptr)
+{
+    const int64_t n = (int64_t)n_blk * L.n_ch;
+    for (int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; r <= n; r += (int64_t)gridDim.x * blockDim.x) {
+        if (r == n) { rowptr[r] = cellbase[n_blk] * L.totcoup; continue; }
+        const int k = (int)(r / L.n_ch), a = (int)(r - (int64_t)k * L.n_ch);
+        rowptr[r] = cellbase[k] * L.totcoup + (int64_t)hits[k] * L.cl_off[a];
     }
 }
 
@@ -178,9 +216,11 @@ __global__ void __launch_bounds__(kThreads) k_emit_cols(DevLattice L, NodeLists 
         const int off = L.cl_off[a], nc = L.cl_off[a + 1] - off;
         int32_t* out = colidx + rowptr[(int64_t)blockIdx.x * L.n_ch + a];
         const int len = H * nc;
+        const unsigned mg = nc > 1 ? (unsigned)(((1ull << 32) + (unsigned)nc - 1) / (unsigned)nc) : 0u;   // idx*nc < 2^32
+        const int* cl = L.cl + off;
         for (int idx = tid; idx < len; idx += T) {
-            const int k = idx / nc, m = idx - k * nc;
-            out[idx] = hitcell[k] * L.n_ch + L.cl[off + m];
+            const int k = mg ? (int)__umulhi((unsigned)idx, mg) : idx, m = idx - k * nc;
+            out[idx] = hitcell[k] * L.n_ch + cl[m];
         }
     }
 }
@@ -220,10 +260,13 @@ cudaError_t launch_map_sort(const DevLattice& L, int cell_begin, int n_blk, cons
     return cudaGetLastError();
 }
 
-cudaError_t launch_scan_rows(const DevLattice& L, int n_blk, const int* hits, int64_t* cellbase, int64_t* rowptr,
+cudaError_t launch_scan_rows(const DevLattice& L, int n_blk, const NodeLists& nl, int64_t* cellbase, int64_t* rowptr,
                              int64_t* summary, cudaStream_t st)
 {
-    k_scan_rows<<<1, 1024, 0, st>>>(L, n_blk, hits, cellbase, rowptr, summary);
+    k_scan_cells<<<1, 1024, 0, st>>>(L, n_blk, nl.hits, nl.ntot, nl.nseg, cellbase, summary);
+    ++g_launches;
+    const int64_t n = (int64_t)n_blk * L.n_ch + 1;
+    k_write_rowptr<<<(unsigned)std::min<int64_t>((n + 255) / 256, 148 * 8), 256, 0, st>>>(L, n_blk, nl.hits, cellbase, rowptr);
     ++g_launches;
     return cudaGetLastError();
 }

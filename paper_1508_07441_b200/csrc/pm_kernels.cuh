@@ -19,7 +19,7 @@ void count_launch();
 
 // pattern pass
 cudaError_t launch_map_sort(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, cudaStream_t st);
-cudaError_t launch_scan_rows(const DevLattice& L, int n_blk, const int* hits, int64_t* cellbase, int64_t* rowptr,
+cudaError_t launch_scan_rows(const DevLattice& L, int n_blk, const NodeLists& nl, int64_t* cellbase, int64_t* rowptr,
                              int64_t* summary, cudaStream_t st);
 cudaError_t launch_emit_cols(const DevLattice& L, int n_blk, const NodeLists& nl, int hmax, const int64_t* rowptr,
                              int32_t* colidx, cudaStream_t st);

@@ -326,6 +326,29 @@ void scaled_harmonics(int lmax, std::vector<double>& ynorm, std::vector<double>&
     for (int k = 0; k < ny; ++k) ynorm[(size_t)k] = (double)N[(size_t)k];
 }
 
+double ket_flops(const Tables& T)
+{
+    int la = 0, lb = 0;
+    for (const Triple& t : T.tri) { la = std::max(la, t.l); lb = std::max(lb, t.lam); }
+    auto rec = [](int lmax, bool unit_seed) {       // Q_mm: 1 mul; Q_{m+1,m}: 1 mul; Q_lm (l >= m+2): mul + FMA = 3
+        double f = 0.0;
+        for (int m = 0; m <= lmax; ++m) {
+            if (m > 0) f += 1.0;
+            for (int l = m + 1; l <= lmax; ++l) f += (l == m + 1) ? 1.0 : 3.0;
+        }
+        if (unit_seed && lmax >= 1) f -= 2.0;       // ux*1 and uz*1 are not operations
+        return f;
+    };
+    std::map<std::pair<int, int>, int> prod;
+    for (size_t t = 0; t < T.kt_c.size(); ++t) prod[{T.kt_ip[t], T.kt_iq[t]}]++;
+    double f = rec(la, false) + rec(lb, true) + (double)prod.size();
+    for (int s = 0; s < T.n_slot; ++s) {
+        const int n = T.kt_off[(size_t)s + 1] - T.kt_off[(size_t)s];
+        if (n > 0) f += 1.0 + 2.0 * (n - 1);
+    }
+    return f;
+}
+
 double sqrt_threshold(double e)
 {
     if (!(e > 0.0)) return 0.0;                         // every y >= 0 has sqrt(y) >= 0

@@ -66,6 +66,10 @@ uint64_t tables_hash(const Tables& T);
 //   Q_00 = 1, Q_mm = ux*Q_{m-1,m-1}, Q_{m+1,m} = uz*Q_mm, Q_lm = uz*Q_{l-1,m} - ybeta[lm]*Q_{l-2,m}.
 void scaled_harmonics(int lmax, std::vector<double>& ynorm, std::vector<double>& ybeta);
 
+// FP64 flops (add = mul = 1, FMA = 2) of the ket code pm_codegen emits for these tables: the two scaled-harmonic
+// recurrences, one product per distinct (Y_l'm, Y_lam'mu) pair, one multiply or FMA per ket term.
+double ket_flops(const Tables& T);
+
 // Smallest double y with sqrt(y) >= e (IEEE, correctly rounded): "e <= sqrt(y)" <=> "y >= sqrt_threshold(e)",
 // so a node is located from p'^2 with the very decisions the oracle takes on p' = sqrt(p'^2) (reading R6).
 double sqrt_threshold(double e);
