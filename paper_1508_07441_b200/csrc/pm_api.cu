@@ -61,9 +61,8 @@ namespace {
 void free_device(pm_lattice* L)
 {
     if (L->d_blob) cudaFree(L->d_blob);
-    if (L->nl.sorted) cudaFree(L->nl.sorted);
+    if (L->nl.key) cudaFree(L->nl.key);
     if (L->nl.rkpos) cudaFree(L->nl.rkpos);
-    if (L->nl.tcell) cudaFree(L->nl.tcell);
     if (L->nl.ntot) cudaFree(L->nl.ntot);
     if (L->nl.hits) cudaFree(L->nl.hits);
     if (L->nl.nseg) cudaFree(L->nl.nseg);
@@ -168,9 +167,8 @@ int32_t ensure_device(pm_lattice* L)
 int32_t ensure_cell_scratch(pm_lattice* L, int n_blk)
 {
     if (n_blk <= L->hits_cap) return PM_OK;
-    if (L->nl.sorted) cudaFree(L->nl.sorted);
+    if (L->nl.key) cudaFree(L->nl.key);
     if (L->nl.rkpos) cudaFree(L->nl.rkpos);
-    if (L->nl.tcell) cudaFree(L->nl.tcell);
     if (L->nl.ntot) cudaFree(L->nl.ntot);
     if (L->nl.hits) cudaFree(L->nl.hits);
     if (L->nl.nseg) cudaFree(L->nl.nseg);
@@ -178,9 +176,8 @@ int32_t ensure_cell_scratch(pm_lattice* L, int n_blk)
     L->nl = pm::NodeLists{}; L->d_cellbase = nullptr; L->hits_cap = 0;
     const size_t nn = (size_t)n_blk * (size_t)L->dev.nnode;
     cudaError_t e;
-    if ((e = cudaMalloc(&L->nl.sorted, sizeof(unsigned short) * nn)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(node lists)");
+    if ((e = cudaMalloc(&L->nl.key, sizeof(unsigned) * nn)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(node lists)");
     if ((e = cudaMalloc(&L->nl.rkpos, sizeof(unsigned short) * nn)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(node lists)");
-    if ((e = cudaMalloc(&L->nl.tcell, sizeof(int) * nn)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(node lists)");
     if ((e = cudaMalloc(&L->nl.ntot, sizeof(int) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(ntot)");
     if ((e = cudaMalloc(&L->nl.hits, sizeof(int) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(hits)");
     if ((e = cudaMalloc(&L->nl.nseg, sizeof(int) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(nseg)");

@@ -28,13 +28,13 @@ struct DevLattice {
     const double *ya, *yb, *ydiag;
 };
 
-// Per-source-cell node lists written by the pattern pass and read by the fill pass (library-owned scratch):
-// the node ids m = c*(n_p*n_q) + a*n_q + b of the nodes that hit the grid, sorted by (rank of target cell, m),
-// and the rank and the cell id of the target at every sorted position.  Stride nnode per source cell.
+// Per-source-cell node lists written by the pattern pass and read by the fill pass (library-owned scratch), stride
+// nnode per source cell: for every node that hit the grid, in the order (rank of target cell, node id),
+//   key   = target cell << 14 | node id     (node id m = c*(n_p*n_q) + a*n_q + b < 2^14, cell < 2^18)
+//   rkpos = rank of the target cell among the source cell's hit cells.
 struct NodeLists {
-    unsigned short* sorted;     // [n_blk][nnode]
+    unsigned* key;              // [n_blk][nnode]
     unsigned short* rkpos;      // [n_blk][nnode]
-    int* tcell;                 // [n_blk][nnode]
     int* ntot;                  // [n_blk] nodes on the grid
     int* hits;                  // [n_blk] hit cells H
     int* nseg;                  // [n_blk] (target, x-node) segments of the sorted list

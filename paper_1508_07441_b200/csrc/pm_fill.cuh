@@ -158,8 +158,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         const int ci = cell / L.Nq, cj = cell - ci * L.Nq;
         const CellGeom g = cell_geom(L.pe, L.qe, ci, cj);
         const int H = nl.hits[cb], we = nl.ntot[cb];
-        const unsigned short* __restrict__ g_sorted = nl.sorted + (size_t)cb * L.nnode;
-        const int* __restrict__ g_tcell = nl.tcell + (size_t)cb * L.nnode;
+        const unsigned* __restrict__ g_key = nl.key + (size_t)cb * L.nnode;       // target cell << 14 | node id
         double* __restrict__ row0 = vals + rowptr[(int64_t)cb * L.n_ch];
         const double dsrc = s_dp[ci] * s_dq[cj];
         for (int k = lane; k < L.n_p; k += 32) s_wpa[k] = __dmul_rn(g.hp, L.wp[k]);
@@ -197,22 +196,24 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         double2 runS[NPC];
 #pragma unroll
         for (int i = 0; i < NPC; ++i) runS[i] = make_double2(0.0, 0.0);
-        int mC = 0, tC = -1, mN = 0, tN = -1;           // this step's and the next step's node id / target cell (-1: none)
-        if (lane < we) { mC = g_sorted[lane]; tC = g_tcell[lane]; }
-        if (32 + lane < we) { mN = g_sorted[32 + lane]; tN = g_tcell[32 + lane]; }
+        unsigned kC = 0, kN = 0;                        // this step's and the next step's keys
+        if (lane < we) kC = g_key[lane];
+        if (32 + lane < we) kN = g_key[32 + lane];
         for (int base = 0; base < we; base += 32) {
-            int mF = 0, tF = -1;
-            if (base + 64 + lane < we) { mF = g_sorted[base + 64 + lane]; tF = g_tcell[base + 64 + lane]; }
-            const bool active = tC >= 0;
+            unsigned kF = 0;
+            if (base + 64 + lane < we) kF = g_key[base + 64 + lane];
+            const bool active = base + lane < we;
+            const int tC = (int)(kC >> 14);
             int c, a, b;
-            split_node(L, mC, c, a, b);
-            // the node after this one (next lane, or lane 0 of the next step); target -1 past the end of the list
-            int m1 = __shfl_down_sync(0xffffffffu, mC, 1), t1 = __shfl_down_sync(0xffffffffu, tC, 1);
-            const int m1n = __shfl_sync(0xffffffffu, mN, 0), t1n = __shfl_sync(0xffffffffu, tN, 0);
-            if (lane == 31) { m1 = m1n; t1 = t1n; }
+            split_node(L, (int)(kC & 16383u), c, a, b);
+            // the node after this one (next lane, or lane 0 of the next step)
+            unsigned k1 = __shfl_down_sync(0xffffffffu, kC, 1);
+            const unsigned k1n = __shfl_sync(0xffffffffu, kN, 0);
+            if (lane == 31) k1 = k1n;
+            const int m1 = (int)(k1 & 16383u);
             const int c1 = L.mg_npq ? (int)__umulhi((unsigned)m1, L.mg_npq) : m1;
             // target ends: t changes after this node (or the list ends); segment ends: (t, c) changes
-            const bool tend = active && (t1 != tC);
+            const bool tend = active && (base + lane + 1 >= we || (int)(k1 >> 14) != tC);
             const bool send = active && (tend || c1 != c);
             const unsigned tmask = __ballot_sync(0xffffffffu, tend), smask = __ballot_sync(0xffffffffu, send);
             const int cnt = min(32, we - base);
@@ -241,30 +242,37 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 }
             }
             __syncwarp();
-            // lane = slot pair: walks the tile's nodes in steps of 8, 4 or 1; a segment may end only at a step's last node
+            // lane = slot pair: walks the tile's nodes, up to 8 per step, stopping at every segment end (and at the tile end)
+            const unsigned stops = smask | (1u << (cnt - 1));
             for (int j = 0; j < cnt;) {
-                const unsigned rest = smask >> j;
-                const int step = ((rest & 0x7fu) == 0 && j + 8 <= cnt) ? 8 : ((rest & 0x7u) == 0 && j + 4 <= cnt) ? 4 : 1;
+                const int n = min(__ffs(stops >> j), 8);                 // nodes up to and including the next stop, at most 8
 #pragma unroll
                 for (int i = 0; i < NPC; ++i) {
                     const int sp = i * 32 + lane;
                     if (sp < np) {
                         const double2* row = s_tile + sp * kTileStride + j;
-                        if (step == 8) {
+                        if (n == 8) {
                             const double2 d0 = row[0], d1 = row[1], d2 = row[2], d3 = row[3], d4 = row[4], d5 = row[5], d6 = row[6], d7 = row[7];
                             runS[i].x += ((d0.x + d1.x) + (d2.x + d3.x)) + ((d4.x + d5.x) + (d6.x + d7.x));
                             runS[i].y += ((d0.y + d1.y) + (d2.y + d3.y)) + ((d4.y + d5.y) + (d6.y + d7.y));
-                        } else if (step == 4) {
-                            const double2 d0 = row[0], d1 = row[1], d2 = row[2], d3 = row[3];
-                            runS[i].x += (d0.x + d1.x) + (d2.x + d3.x);
-                            runS[i].y += (d0.y + d1.y) + (d2.y + d3.y);
                         } else {
-                            const double2 d = row[0];
-                            runS[i].x += d.x; runS[i].y += d.y;
+                            if (n & 4) {
+                                const double2 d0 = row[0], d1 = row[1], d2 = row[2], d3 = row[3];
+                                runS[i].x += (d0.x + d1.x) + (d2.x + d3.x);
+                                runS[i].y += (d0.y + d1.y) + (d2.y + d3.y);
+                                row += 4;
+                            }
+                            if (n & 2) {
+                                const double2 d0 = row[0], d1 = row[1];
+                                runS[i].x += d0.x + d1.x;
+                                runS[i].y += d0.y + d1.y;
+                                row += 2;
+                            }
+                            if (n & 1) { const double2 d = row[0]; runS[i].x += d.x; runS[i].y += d.y; }
                         }
                     }
                 }
-                j += step;
+                j += n;
                 if (!((smask >> (j - 1)) & 1u)) continue;
                 const int jb = j - 1;                                    // node jb ends a (t, c) segment
 #pragma unroll
@@ -311,7 +319,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 }
             }
             __syncwarp();
-            mC = mN; tC = tN; mN = mF; tN = tF;
+            kC = kN; kN = kF;
         }
         if (kcur > kdone) write_rows(kdone, kcur - kdone);
     }

@@ -120,10 +120,9 @@ __global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_be
         __syncwarp();
     }
     __syncthreads();
-    unsigned short* g_sorted = nl.sorted + (size_t)blockIdx.x * L.nnode;
+    unsigned* g_key = nl.key + (size_t)blockIdx.x * L.nnode;
     unsigned short* g_rkpos = nl.rkpos + (size_t)blockIdx.x * L.nnode;
-    int* g_tcell = nl.tcell + (size_t)blockIdx.x * L.nnode;
-    for (int k = tid; k < ntot; k += T) { g_sorted[k] = s_sorted[k]; g_rkpos[k] = s_rkpos[k]; g_tcell[k] = s_tcpos[k]; }
+    for (int k = tid; k < ntot; k += T) { g_key[k] = ((unsigned)s_tcpos[k] << 14) | s_sorted[k]; g_rkpos[k] = s_rkpos[k]; }
     // (target, x-node) segments of the sorted list: the fill pass applies the bra harmonics once per segment
     int seg = 0;
     for (int k = tid; k < ntot; k += T) {
@@ -206,10 +205,10 @@ __global__ void __launch_bounds__(kThreads) k_emit_cols(DevLattice L, NodeLists 
     int* hitcell = (int*)smem;
     const int H = nl.hits[blockIdx.x], ntot = nl.ntot[blockIdx.x];
     const unsigned short* g_rkpos = nl.rkpos + (size_t)blockIdx.x * L.nnode;
-    const int* g_tcell = nl.tcell + (size_t)blockIdx.x * L.nnode;
+    const unsigned* g_key = nl.key + (size_t)blockIdx.x * L.nnode;
     for (int pos = tid; pos < ntot; pos += T) {
         const int r = g_rkpos[pos];
-        if (pos == 0 || g_rkpos[pos - 1] != r) hitcell[r] = g_tcell[pos];
+        if (pos == 0 || g_rkpos[pos - 1] != r) hitcell[r] = (int)(g_key[pos] >> 14);
     }
     __syncthreads();
     for (int a = 0; a < L.n_ch; ++a) {
