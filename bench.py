@@ -14,7 +14,6 @@ import json
 import os
 import subprocess
 import sys
-import threading
 import time
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
@@ -29,6 +28,9 @@ METRIC = "P-matrix nonzeros/sec (pattern + fill, FP64)"
 UNIT = "nnz/s"
 # FP64 ALU peak used for the roofline: SMs x 64 DFMA lanes x 2 flop x max SM clock
 FP64_LANES_PER_SM = 64
+# dram__bytes_read.sum + dram__bytes_write.sum of one fill launch from the committed `ncu --set full` capture
+# (profiles/r1_fill.md), per workload; None where no capture exists.
+FILL_DRAM_TRAFFIC = {"cfg4_3N_Jhalf+_jle3_26ch_150x150": 7.097e9 + 0.449e9}
 
 
 def _peaks():
@@ -40,46 +42,45 @@ def _peaks():
 
 
 class ClockSampler:
-    """Samples nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    """Samples nvidia-smi clocks / throttle reasons every 50 ms during the timed region (B200_PROFILING.md clocks line)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index=0):
-        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
-
-    def _run(self):
-        while not self._stop.is_set():
-            try:
-                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
-                                     capture_output=True, text=True, timeout=5).stdout.strip()
-                if out:
-                    self.rows.append([c.strip() for c in out.split(",")])
-            except Exception:
-                pass
-            self._stop.wait(0.2)
+        self.index, self.proc, self.out = index, None, ""
 
     def __enter__(self):
-        self._t = threading.Thread(target=self._run, daemon=True)
-        self._t.start()
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "50"], stdout=subprocess.PIPE, text=True)
+            time.sleep(0.25)                        # let the first samples arrive before the timed region starts
+        except Exception:
+            self.proc = None
         return self
 
     def __exit__(self, *a):
-        self._stop.set()
-        self._t.join(timeout=6)
+        if self.proc is not None:
+            time.sleep(0.1)
+            self.proc.terminate()
+            try:
+                self.out = self.proc.communicate(timeout=5)[0]
+            except Exception:
+                self.out = ""
 
     def summary(self):
-        sm, mx, reasons = [], 0.0, set()
+        sm, mx, pw, reasons = [], 0.0, [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
+        for line in self.out.strip().splitlines():
+            r = [c.strip() for c in line.split(",")]
             try:
-                sm.append(float(r[0])); mx = max(mx, float(r[1]))
+                sm.append(float(r[0])); mx = max(mx, float(r[1])); pw.append(float(r[2]))
                 for n, v in zip(names, r[3:7]):
                     if v.lower().startswith("active"):
                         reasons.add(n)
             except Exception:
                 continue
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons),
-                "samples": len(sm)}
+                "power_w_max": max(pw) if pw else None, "samples": len(sm)}
 
 
 def build_flops(lat_api, h):
@@ -91,7 +92,7 @@ def build_flops(lat_api, h):
                                                                  "segments": segs, "hit_cells": hits}
 
 
-def oracle_sample(wl, seconds_target=15.0, max_cells=64):
+def oracle_sample(wl, seconds_target=15.0, max_cells=512):
     """Times the oracle as it stands on evenly spaced source cells of `wl` (bounded CPU work)."""
     from oracle.pm_oracle import Oracle
     o = Oracle()
@@ -115,10 +116,10 @@ def run_reference(args):
     wl = inputs.config(args.config)
     per_step = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
     for _ in range(args.warmup):
-        oracle_sample(wl, per_step, 16)
+        oracle_sample(wl, per_step, 256)
     tot_nnz, tot_t, info = 0, 0.0, None
     for _ in range(args.steps):
-        info, nnz, dt = oracle_sample(wl, per_step, 16)
+        info, nnz, dt = oracle_sample(wl, per_step, 256)
         tot_nnz += nnz; tot_t += dt
     v = tot_nnz / tot_t
     info["value"] = v
@@ -209,7 +210,7 @@ def main():
     achieved_tf = flops / fill_avg * 1e-12
     dfma = api.pm_diag_dfma_tflops()
     roof = {"bound": "alu", "kernel": "pm_fill", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
-            "frac": achieved_tf / peak_tf, "traffic": None,
+            "frac": achieved_tf / peak_tf, "traffic": FILL_DRAM_TRAFFIC.get(wl.name),
             "peak_source": f"{n_sm} SM x {FP64_LANES_PER_SM} DFMA lanes x 2 x {pk['sm_max_mhz']:.0f} MHz ({pk['src']} clock); "
                            f"DFMA microbenchmark on this box: {dfma:.1f} TFLOP/s",
             "flops_per_launch": flops, "work": work, "fill_ms": fill_avg * 1e3,

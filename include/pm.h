@@ -121,6 +121,15 @@ int32_t pm_lattice_work(const pm_lattice* lat, double* flop_per_node, double* fl
  * PM_ERR_STATE before the first pm_pattern. */
 int32_t pm_pattern_counts(const pm_lattice* lat, int64_t* nodes_on_grid, int64_t* segments, int64_t* hit_cells);
 
+/* Name of the fill kernel this lattice's channel set selects: "Spec_<set>" when csrc/build.py generated straight-line
+ * ket code for it (the channel sets of BASELINE.json's configs), "generic" for the table-driven kernel every other
+ * channel set uses.  Host only; library-owned string, never NULL. */
+const char* pm_lattice_fill_kernel(const pm_lattice* lat);
+
+/* Diagnostic (host only): the smallest double y with sqrt(y) >= edge under IEEE round-to-nearest — the threshold
+ * the kernels compare p'^2 with instead of taking sqrt(p'^2) and comparing with the edge. */
+double pm_diag_sqrt_threshold(double edge);
+
 /* Diagnostic: measured FP64 FMA throughput of the current device in TFLOP/s (a dependent-free DFMA loop on every
  * SM, timed with CUDA events on `cuda_stream`); the roofline denominator is stated beside it in DESIGN.md sec. 7. */
 int32_t pm_diag_dfma_tflops(double* tflops, void* cuda_stream);

@@ -22,7 +22,8 @@ ERRORS = {-1: "PM_ERR_ARG", -2: "PM_ERR_GRID", -3: "PM_ERR_CHANNEL", -4: "PM_ERR
           -6: "PM_ERR_NOMEM", -7: "PM_ERR_STATE", -8: "PM_ERR_OVERFLOW", -9: "PM_ERR_DEVICE"}
 
 EXPORTS = ["pm_lattice_create", "pm_lattice_destroy", "pm_lattice_dims", "pm_lattice_rule", "pm_lattice_set_rule",
-           "pm_lattice_coupling", "pm_lattice_work", "pm_pattern_counts", "pm_diag_dfma_tflops", "pm_pattern", "pm_fill", "pm_spmv", "pm_build_host_count", "pm_build_host",
+           "pm_lattice_coupling", "pm_lattice_work", "pm_pattern_counts", "pm_lattice_fill_kernel", "pm_diag_sqrt_threshold",
+           "pm_diag_dfma_tflops", "pm_pattern", "pm_fill", "pm_spmv", "pm_build_host_count", "pm_build_host",
            "pm_launch_count", "pm_last_error"]
 
 
@@ -61,13 +62,17 @@ def lib():
     L.pm_lattice_work.argtypes = [_vp, _dp, _dp, _dp, _i32p]
     L.pm_pattern_counts.argtypes = [_vp, _i64p, _i64p, _i64p]
     L.pm_diag_dfma_tflops.argtypes = [_dp, _vp]
+    L.pm_lattice_fill_kernel.argtypes = [_vp]
+    L.pm_lattice_fill_kernel.restype = C.c_char_p
+    L.pm_diag_sqrt_threshold.argtypes = [C.c_double]
+    L.pm_diag_sqrt_threshold.restype = C.c_double
     L.pm_pattern.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, C.c_int64, _i64p, _vp]
     L.pm_fill.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, _vp]
     L.pm_spmv.argtypes = [_vp, C.c_int64, _vp, _vp, _vp, _vp, _vp, _vp]
     L.pm_build_host_count.argtypes = [_vp, C.c_int64, _i64p, _i32p]
     L.pm_build_host.argtypes = [_vp, C.c_int64, _vp, _vp, _vp, C.c_int64, _i64p, _i32p]
     for name in EXPORTS:
-        if name not in ("pm_last_error", "pm_launch_count"):
+        if name not in ("pm_last_error", "pm_launch_count", "pm_lattice_fill_kernel", "pm_diag_sqrt_threshold"):
             getattr(L, name).restype = C.c_int32
     _lib = L
     return L
@@ -142,6 +147,14 @@ def pm_pattern_counts(h):
     a, s_, b = C.c_int64(), C.c_int64(), C.c_int64()
     _check(lib().pm_pattern_counts(h, C.byref(a), C.byref(s_), C.byref(b)))
     return a.value, s_.value, b.value
+
+
+def pm_lattice_fill_kernel(h):
+    return lib().pm_lattice_fill_kernel(h).decode()
+
+
+def pm_diag_sqrt_threshold(edge):
+    return lib().pm_diag_sqrt_threshold(float(edge))
 
 
 def pm_diag_dfma_tflops(stream=None):

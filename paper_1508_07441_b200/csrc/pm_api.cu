@@ -316,6 +316,13 @@ int32_t pm_pattern_counts(const pm_lattice* lat, int64_t* nodes_on_grid, int64_t
     return PM_OK;
 }
 
+const char* pm_lattice_fill_kernel(const pm_lattice* lat)
+{
+    return lat ? pm::fill_variant_name(lat->hash) : "";
+}
+
+double pm_diag_sqrt_threshold(double edge) { return pm::sqrt_threshold(edge); }
+
 int32_t pm_diag_dfma_tflops(double* tflops, void* cuda_stream)
 {
     if (!tflops) return fail(PM_ERR_ARG, "NULL argument");

@@ -39,6 +39,12 @@ bool fill_has_spec(unsigned long long hash)
     return false;
 }
 
+const char* fill_variant_name(unsigned long long hash)
+{
+    for (const FillVariant& v : kVariants) if (v.hash == hash && hash != 0ull) return v.name;
+    return "generic";
+}
+
 // Picks the variant (specialised when `hash` matches a generated kernel, else table-driven; the preferred warp count
 // if its shared memory fits, else a smaller one) and the persistent grid.  Returns cudaErrorInvalidConfiguration
 // when no variant fits in shared memory.

@@ -27,6 +27,7 @@ cudaError_t launch_emit_cols(const DevLattice& L, int n_blk, const NodeLists& nl
 // fill pass (pm_fill.cuh): variant selection and launch
 struct FillLaunch { const void* fn; int nw, grid; FillSmem smem; const char* name; };
 bool fill_has_spec(unsigned long long tables_hash);
+const char* fill_variant_name(unsigned long long tables_hash);
 cudaError_t fill_plan(const DevLattice& L, unsigned long long tables_hash, int n_sm, FillLaunch* out);
 cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl,
                         const int64_t* rowptr, double* vals, int* counter, cudaStream_t st);

@@ -79,6 +79,29 @@ def test_bitwise_reproducible(api):
     assert all(np.array_equal(x, y) for x, y in zip(a, b))
 
 
+def test_generic_kernel_parity_on_reordered_channels(api, oracle):
+    """A channel order with no generated kernel runs the table-driven fill; same bar."""
+    wl = I.small_coupled(N=6, jmax=2, orders=(3, 4, 6))
+    wl.channels = wl.channels[::-1].copy()
+    lat = api.Lattice(wl)
+    assert api.pm_lattice_fill_kernel(lat.h) == "generic"
+    rp, ci, v = lat.build()
+    rpo, cio, vo = oracle.build_csr(wl)
+    assert np.array_equal(rp.cpu().numpy(), rpo) and np.array_equal(ci.cpu().numpy(), cio)
+    _assert_values(v.cpu().numpy(), vo)
+    lat.close()
+
+
+def test_pattern_counts(api):
+    wl = I.config(1)
+    lat = api.Lattice(wl)
+    rp, ci, nnz = lat.pattern()
+    nodes, segs, hits = api.pm_pattern_counts(lat.h)
+    assert hits * 4 == nnz and hits <= segs <= nodes <= wl.n_cells * wl.nodes_per_cell
+    assert nodes > 0.9 * wl.n_cells * wl.nodes_per_cell          # fewer than 10 % of the nodes leave the grid
+    lat.close()
+
+
 def test_fill_requires_pattern(api):
     import torch
     wl = I.config(0)

@@ -123,6 +123,43 @@ def test_compute_calls_fail_loudly_without_gpu():
     api.pm_lattice_destroy(h)
 
 
+def test_fill_kernel_selection_and_work_model():
+    """configs[0..4] select a generated (channel-specialised) fill kernel; another channel ORDER of the same set has
+    other tables and falls back to the table-driven kernel.  The work model is positive and grows with the set."""
+    names, work = [], []
+    for k in range(5):
+        wl = I.config(k)
+        h = _create(wl)
+        names.append(api.pm_lattice_fill_kernel(h))
+        work.append(api.pm_lattice_work(h))
+        with pytest.raises(api.PmError) as e:
+            api.pm_pattern_counts(h)
+        assert e.value.code == -7
+        api.pm_lattice_destroy(h)
+    assert names == ["Spec_boson_s", "Spec_boson_s", "Spec_nnn_j2", "Spec_nnn_j3", "Spec_nnn_j3"]
+    assert all(w[0] > 40 and w[1] > 0 and w[2] > 0 for w in work)
+    assert work[4][0] > work[2][0] > work[1][0] and work[4][3] == 580 and work[2][3] == 276
+    wl = I.config(2)
+    h = _create(wl, channels=wl.channels[::-1].copy())
+    assert api.pm_lattice_fill_kernel(h) == "generic"
+    api.pm_lattice_destroy(h)
+
+
+def test_sqrt_threshold_is_the_exact_boundary():
+    """'edge <= sqrt(y)'  <=>  'y >= thr(edge)' for IEEE doubles: checked on the neighbours of thr for every edge of the
+    five lattices and for random edges (numpy's sqrt is correctly rounded)."""
+    rng = np.random.default_rng(7)
+    edges = np.concatenate([I.config(k).p_edges for k in range(5)] + [I.config(2).q_edges, rng.uniform(1e-6, 1e3, 2000),
+                           10.0 ** rng.uniform(-12, 12, 2000)])
+    for e in edges:
+        t = api.pm_diag_sqrt_threshold(e)
+        if e == 0.0:
+            assert t == 0.0
+            continue
+        assert np.sqrt(t) >= e
+        assert np.sqrt(np.nextafter(t, 0.0)) < e
+
+
 def test_product_does_not_import_oracle():
     """The product path must never route through the oracle (or any CPU fallback)."""
     pkg = os.path.join(ROOT, "paper_1508_07441_b200")
