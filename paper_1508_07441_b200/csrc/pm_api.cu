@@ -124,6 +124,10 @@ int32_t ensure_device(pm_lattice* L)
 
     const size_t o_pe = put(pe.data(), 8 * pe.size()), o_qe = put(qe.data(), 8 * qe.size());
     const size_t o_thp = put(thp.data(), 8 * thp.size()), o_thq = put(thq.data(), 8 * thq.size());
+    std::vector<uint16_t> bkp, bkq;
+    pm::bucket_table(thp, L->Np + 1, pm::kBuckets, D.bk_hmin_p, D.bk_sh_p, bkp);
+    pm::bucket_table(thq, L->Nq + 1, pm::kBuckets, D.bk_hmin_q, D.bk_sh_q, bkq);
+    const size_t o_bkp = put(bkp.data(), 2 * bkp.size()), o_bkq = put(bkq.data(), 2 * bkq.size());
     size_t o_t[3], o_w[3];
     for (int k = 0; k < 3; ++k) { o_t[k] = put(L->rule_t[k].data(), 8 * L->rule_t[k].size()); o_w[k] = put(L->rule_w[k].data(), 8 * L->rule_w[k].size()); }
     const size_t o_sx = put(sx.data(), 8 * sx.size());
@@ -146,6 +150,7 @@ int32_t ensure_device(pm_lattice* L)
     char* b = L->d_blob;
     D.pe = (const double*)(b + o_pe); D.qe = (const double*)(b + o_qe);
     D.thr_p = (const double*)(b + o_thp); D.thr_q = (const double*)(b + o_thq);
+    D.bk_p = (const unsigned short*)(b + o_bkp); D.bk_q = (const unsigned short*)(b + o_bkq);
     D.tp = (const double*)(b + o_t[0]); D.wp = (const double*)(b + o_w[0]);
     D.tq = (const double*)(b + o_t[1]); D.wq = (const double*)(b + o_w[1]);
     D.tx = (const double*)(b + o_t[2]); D.wx = (const double*)(b + o_w[2]);

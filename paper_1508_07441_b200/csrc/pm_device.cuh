@@ -18,6 +18,8 @@ struct DevLattice {
     unsigned mg_npq, mg_nq;                     // ceil(2^32 / (n_p*n_q)), ceil(2^32 / n_q): exact division of node ids
     const double *pe, *qe;                      // edges, Np+1 / Nq+1 entries (padded with +inf to pe_pad / qe_pad)
     const double *thr_p, *thr_q;                // sqrt_threshold(edge), padded with +inf to a power of two
+    const unsigned short *bk_p, *bk_q;          // kBuckets entries each: first threshold a value of that bucket can meet
+    int bk_hmin_p, bk_sh_p, bk_hmin_q, bk_sh_q; // bucket(v) = clamp((hi32(v) - hmin) >> sh, 0, kBuckets-1)
     const double *tp, *wp, *tq, *wq, *tx, *wx;  // Gauss-Legendre rules on [-1,1]
     const double *sx;                           // sqrt(1-x^2) per x-node
     const int *cl_off, *cl, *o_alpha;           // coupled lists; o_alpha[o] = alpha of output o
@@ -74,23 +76,28 @@ __device__ __forceinline__ void map_node_sq(const CellGeom& g, double ta, double
     Q2 = Q2 < 0.0 ? 0.0 : Q2;
 }
 
-// number of thresholds <= v, minus one; thr has `pad` (power of two) entries, the tail filled with +inf
-__device__ __forceinline__ int locate(const double* __restrict__ thr, int pad, double v)
+constexpr int kBuckets = 1024;
+
+// Number of thresholds <= v, minus one.  The upper 32 bits of a non-negative double grow with its value, so
+// bucket(v) = clamp((hi32(v) - hmin) >> sh) is monotone: every threshold in a lower bucket is < v and start[bucket]
+// counts exactly those; the few thresholds of v's own bucket are compared one by one (thr ends with +inf).
+__device__ __forceinline__ int locate(const double* __restrict__ thr, const unsigned short* __restrict__ start, int hmin, int sh,
+                                      double v)
 {
-    int lo = 0;
-#pragma unroll 1
-    for (int s = pad >> 1; s > 0; s >>= 1) lo += (thr[lo + s - 1] <= v) ? s : 0;
-    lo += (thr[lo] <= v) ? 1 : 0;          // entries beyond N+1 are +inf, so lo <= N+1
-    return lo - 1;
+    const int b = max(0, min(kBuckets - 1, (__double2hiint(v) - hmin) >> sh));
+    int i = start[b];
+    while (thr[i] <= v) ++i;
+    return i - 1;
 }
 
+struct Locator { const double *thr_p, *thr_q; const unsigned short *bk_p, *bk_q; int hmin_p, sh_p, hmin_q, sh_q, Np, Nq; };
+
 // target cell of a mapped node, or -1 (outside the grid, or p' = 0 / q' = 0): readings R5, R6.  sqrt(y) = 0 <=> y = 0.
-__device__ __forceinline__ int target_cell_sq(const double* thr_p, int pe_pad, int Np, const double* thr_q, int qe_pad, int Nq,
-                                              double P2, double Q2)
+__device__ __forceinline__ int target_cell_sq(const Locator& lc, double P2, double Q2)
 {
-    const int ic = locate(thr_p, pe_pad, P2), jc = locate(thr_q, qe_pad, Q2);
-    const bool ok = (ic >= 0) & (ic < Np) & (jc >= 0) & (jc < Nq) & (P2 != 0.0) & (Q2 != 0.0);
-    return ok ? ic * Nq + jc : -1;
+    const int ic = locate(lc.thr_p, lc.bk_p, lc.hmin_p, lc.sh_p, P2), jc = locate(lc.thr_q, lc.bk_q, lc.hmin_q, lc.sh_q, Q2);
+    const bool ok = (ic >= 0) & (ic < lc.Np) & (jc >= 0) & (jc < lc.Nq) & (P2 != 0.0) & (Q2 != 0.0);
+    return ok ? ic * lc.Nq + jc : -1;
 }
 
 // In-place exclusive scan of n ints in shared memory by the whole block; returns the total.

@@ -26,7 +26,7 @@ size_t map_sort_smem(const DevLattice& L)
 {
     const int nw = kThreads / 32;
     const int hcap = std::min(L.nnode, L.n_cells);
-    return al16(8 * (size_t)L.pe_pad) + al16(8 * (size_t)L.qe_pad) + al16(8 * (size_t)L.n_p) + al16(8 * (size_t)L.n_q)
+    return al16(8 * (size_t)L.pe_pad) + al16(8 * (size_t)L.qe_pad) + 2 * al16(2 * (size_t)kBuckets) + al16(8 * (size_t)L.n_p) + al16(8 * (size_t)L.n_q)
          + al16(8 * (size_t)L.n_x) + 2 * al16(4 * (size_t)L.n_words) + al16(4 * (size_t)(kThreads + 1))
          + 2 * al16(4 * (size_t)L.nnode) + 3 * al16(2 * (size_t)L.nnode) + al16(4 * (size_t)(hcap + 1))
          + al16(4 * (size_t)std::max(nw * std::min(hcap, kHitsFast), hcap));
@@ -41,6 +41,8 @@ __global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_be
     char* sp = smem;
     double* s_thr_p = (double*)carve(sp, 8 * (size_t)L.pe_pad);
     double* s_thr_q = (double*)carve(sp, 8 * (size_t)L.qe_pad);
+    unsigned short* s_bk_p = (unsigned short*)carve(sp, 2 * (size_t)kBuckets);
+    unsigned short* s_bk_q = (unsigned short*)carve(sp, 2 * (size_t)kBuckets);
     double* s_tp = (double*)carve(sp, 8 * (size_t)L.n_p);
     double* s_tq = (double*)carve(sp, 8 * (size_t)L.n_q);
     double* s_tx = (double*)carve(sp, 8 * (size_t)L.n_x);
@@ -58,6 +60,8 @@ __global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_be
 
     for (int k = tid; k < L.pe_pad; k += T) s_thr_p[k] = L.thr_p[k];
     for (int k = tid; k < L.qe_pad; k += T) s_thr_q[k] = L.thr_q[k];
+    for (int k = tid; k < kBuckets; k += T) { s_bk_p[k] = L.bk_p[k]; s_bk_q[k] = L.bk_q[k]; }
+    const Locator lc{s_thr_p, s_thr_q, s_bk_p, s_bk_q, L.bk_hmin_p, L.bk_sh_p, L.bk_hmin_q, L.bk_sh_q, L.Np, L.Nq};
     for (int k = tid; k < L.n_p; k += T) s_tp[k] = L.tp[k];
     for (int k = tid; k < L.n_q; k += T) s_tq[k] = L.tq[k];
     for (int k = tid; k < L.n_x; k += T) s_tx[k] = L.tx[k];
@@ -72,7 +76,7 @@ __global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_be
         split_node(L, m, c, a, b);
         double p, q, P2, Q2;
         map_node_sq(g, s_tp[a], s_tq[b], s_tx[c], p, q, P2, Q2);
-        const int t = target_cell_sq(s_thr_p, L.pe_pad, L.Np, s_thr_q, L.qe_pad, L.Nq, P2, Q2);
+        const int t = target_cell_sq(lc, P2, Q2);
         if (t >= 0) atomicOr(&hs.bits[t >> 5], 1u << (t & 31));
         s_tgt[m] = t;
     }
@@ -195,33 +199,33 @@ __global__ void __launch_bounds__(256) k_write_rowptr(DevLattice L, int n_blk, c
 }
 
 // Pattern pass, kernel B: column indices, ascending within each row.  The hit cells of a source cell are read
-// off its node lists (the target cell at the first sorted position of every rank).
-__global__ void __launch_bounds__(kThreads) k_emit_cols(DevLattice L, NodeLists nl, int hmax,
-                                                       const int64_t* __restrict__ rowptr, int32_t* __restrict__ colidx)
+// off its node lists (the target cell at the first sorted position of every rank).  Thread = output (alpha, m-th
+// coupled alpha'), looping over the hit cells k: entry k of row alpha sits at row_start + k*nc + m, so the threads
+// of a warp write runs of consecutive m and consecutive k fill the gaps (the same store pattern as the fill's rows).
+__global__ void __launch_bounds__(1024) k_emit_cols(DevLattice L, NodeLists nl, int hmax,
+                                                   const int64_t* __restrict__ rowptr, int32_t* __restrict__ colidx)
 {
     extern __shared__ __align__(16) char smem[];
-    constexpr int T = kThreads;
-    const int tid = threadIdx.x;
-    int* hitcell = (int*)smem;
+    const int T = blockDim.x, tid = threadIdx.x;
+    int* hitcol = (int*)smem;                        // first column of every hit cell: cell * n_ch
     const int H = nl.hits[blockIdx.x], ntot = nl.ntot[blockIdx.x];
     const unsigned short* g_rkpos = nl.rkpos + (size_t)blockIdx.x * L.nnode;
     const unsigned* g_key = nl.key + (size_t)blockIdx.x * L.nnode;
     for (int pos = tid; pos < ntot; pos += T) {
         const int r = g_rkpos[pos];
-        if (pos == 0 || g_rkpos[pos - 1] != r) hitcell[r] = (int)(g_key[pos] >> 14);
+        if (pos == 0 || g_rkpos[pos - 1] != r) hitcol[r] = (int)(g_key[pos] >> 14) * L.n_ch;
     }
     __syncthreads();
-    for (int a = 0; a < L.n_ch; ++a) {
-        const int off = L.cl_off[a], nc = L.cl_off[a + 1] - off;
-        int32_t* out = colidx + rowptr[(int64_t)blockIdx.x * L.n_ch + a];
-        const int len = H * nc;
-        const unsigned mg = nc > 1 ? (unsigned)(((1ull << 32) + (unsigned)nc - 1) / (unsigned)nc) : 0u;   // idx*nc < 2^32
-        const int* cl = L.cl + off;
-        for (int idx = tid; idx < len; idx += T) {
-            const int k = mg ? (int)__umulhi((unsigned)idx, mg) : idx, m = idx - k * nc;
-            out[idx] = hitcell[k] * L.n_ch + cl[m];
+    int32_t* __restrict__ row0 = colidx + rowptr[(int64_t)blockIdx.x * L.n_ch];
+    // the block is G groups of `ow` threads: a group covers all outputs (in passes if totcoup > ow) for k = g, g+G, ...
+    const int ow = min(T, (L.totcoup + 31) & ~31), G = T / ow, g = tid / ow;
+    if (g < G)
+        for (int o = tid - g * ow; o < L.totcoup; o += ow) {
+            const int al = L.o_alpha[o], off = L.cl_off[al], nc = L.cl_off[al + 1] - off, ap = L.cl[o];
+            int32_t* out = row0 + ((size_t)H * off + (o - off));
+#pragma unroll 4
+            for (int k = g; k < H; k += G) out[(size_t)k * nc] = hitcol[k] + ap;
         }
-    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -276,7 +280,8 @@ cudaError_t launch_emit_cols(const DevLattice& L, int n_blk, const NodeLists& nl
     const size_t sm = al16(4 * (size_t)std::max(hmax, 1));
     cudaError_t e = cudaFuncSetAttribute(k_emit_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
-    k_emit_cols<<<n_blk, kThreads, sm, st>>>(L, nl, hmax, rowptr, colidx);
+    const int threads = std::min(1024, std::max(128, (L.totcoup + 31) & ~31));
+    k_emit_cols<<<n_blk, threads, sm, st>>>(L, nl, hmax, rowptr, colidx);
     ++g_launches;
     return cudaGetLastError();
 }

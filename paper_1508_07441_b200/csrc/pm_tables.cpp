@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdlib>
+#include <cstring>
 #include <limits>
 #include <map>
 #include <tuple>
@@ -356,6 +357,24 @@ double sqrt_threshold(double e)
     while (std::sqrt(y) >= e && y > 0.0) y = std::nextafter(y, 0.0);
     while (std::sqrt(y) < e) y = std::nextafter(y, std::numeric_limits<double>::infinity());
     return y;
+}
+
+void bucket_table(const std::vector<double>& thr, int n, int n_buckets, int& hmin, int& sh, std::vector<uint16_t>& start)
+{
+    auto hi32 = [](double x) { int64_t b; std::memcpy(&b, &x, 8); return (int)(b >> 32); };
+    int first = 0;
+    while (first < n - 1 && !(thr[(size_t)first] > 0.0)) ++first;      // smallest positive threshold (zero has its own bucket 0)
+    hmin = hi32(thr[(size_t)first]);
+    const int64_t span = (int64_t)hi32(thr[(size_t)n - 1]) - hmin;
+    sh = 0;
+    while ((span >> sh) >= n_buckets - 1) ++sh;
+    auto bucket = [&](double x) { int64_t b = ((int64_t)hi32(x) - hmin) >> sh; return (int)std::max<int64_t>(0, std::min<int64_t>(n_buckets - 1, b)); };
+    start.assign((size_t)n_buckets, 0);
+    for (int b = 0; b < n_buckets; ++b) {
+        int c = 0;
+        while (c < n && bucket(thr[(size_t)c]) < b) ++c;
+        start[(size_t)b] = (uint16_t)c;
+    }
 }
 
 }  // namespace pm

@@ -74,4 +74,8 @@ double ket_flops(const Tables& T);
 // so a node is located from p'^2 with the very decisions the oracle takes on p' = sqrt(p'^2) (reading R6).
 double sqrt_threshold(double e);
 
+// Bucket table over thresholds thr[0..n) (ascending, thr[0] >= 0) for the device-side locate (pm_device.cuh):
+// bucket(v) = clamp((hi32(v) - hmin) >> sh, 0, n_buckets-1); start[b] = number of thresholds in buckets below b.
+void bucket_table(const std::vector<double>& thr, int n, int n_buckets, int& hmin, int& sh, std::vector<uint16_t>& start);
+
 }  // namespace pm
