@@ -1,8 +1,8 @@
 #!/usr/bin/env python
 """bench.py — P-matrix build throughput on B200 (BASELINE.json metric: nonzeros/s, build time, % FP64 peak).
 
-A "step" is one pass of the whole hot path — pm_pattern (count, scan, emit columns) + pm_fill — over one
-lattice; the default workload is BASELINE.json configs[4] (the largest lattice; its CSR fits HBM, one block).
+A "step" is one pass of the whole hot path over one lattice through pm_build: the pattern pass (map and sort every
+quadrature node, scan, row pointers) and the fill kernel, which writes the column index and the value of every nonzero; the default workload is BASELINE.json configs[4] (the largest lattice; its CSR fits HBM, one block).
 `value` times the device-resident path with CUDA events; `e2e` times pm_build_host (host buffers, D2H copies
 inside the timed region); `roofline` is for the dominant kernel (the fill); `cpu_baseline` times the oracle on
 a bounded sample of source cells on the host cores.  `--impl reference` times the oracle alone.
@@ -171,13 +171,8 @@ def main():
     vals = torch.empty(nnz, dtype=torch.float64, device="cuda")
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
 
-    def step(ev=None):
-        api.pm_pattern(lat.h, 0, wl.n_cells, rowptr, colidx)
-        if ev:
-            ev[0].record(st)
-        api.pm_fill(lat.h, 0, wl.n_cells, rowptr, vals)
-        if ev:
-            ev[1].record(st)
+    def step():
+        api.pm_build(lat.h, 0, wl.n_cells, rowptr, colidx, vals)
 
     for _ in range(max(args.warmup, 3)):
         step()
@@ -187,12 +182,14 @@ def main():
     with ClockSampler(local) as clocks:
         for _ in range(args.steps):
             flush.zero_()                                     # L2 flush between timed iterations (untimed)
-            e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            e0, e1 = (torch.cuda.Event(enable_timing=True) for _ in range(2))
             barrier()
             e0.record(st)
-            step((e1, e2))
+            step()
+            e1.record(st)
             torch.cuda.synchronize()
-            step_ms.append(e0.elapsed_time(e2)); fill_ms.append(e1.elapsed_time(e2))
+            step_ms.append(e0.elapsed_time(e1))
+            fill_ms.append(api.pm_last_fill_ms(lat.h))        # CUDA events around the fill kernel, on its stream
         barrier()
     launches = api.pm_launch_count() - l0
     tot = torch.tensor([sum(step_ms)], dtype=torch.float64, device="cuda")
@@ -209,12 +206,12 @@ def main():
     fill_avg = float(np.mean(fill_ms)) * 1e-3
     achieved_tf = flops / fill_avg * 1e-12
     dfma = api.pm_diag_dfma_tflops()
-    roof = {"bound": "alu", "kernel": "pm_fill", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
+    roof = {"bound": "alu", "kernel": "k_fill_warp (values + column indices)", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
             "frac": achieved_tf / peak_tf, "traffic": FILL_DRAM_TRAFFIC.get(wl.name),
             "peak_source": f"{n_sm} SM x {FP64_LANES_PER_SM} DFMA lanes x 2 x {pk['sm_max_mhz']:.0f} MHz ({pk['src']} clock); "
                            f"DFMA microbenchmark on this box: {dfma:.1f} TFLOP/s",
             "flops_per_launch": flops, "work": work, "fill_ms": fill_avg * 1e3,
-            "csr_write_gbs": 8.0 * nnz / fill_avg * 1e-9, "hbm_peak_gbs": pk["hbm_gbs"]}
+            "csr_write_gbs": 12.0 * nnz / fill_avg * 1e-9, "hbm_peak_gbs": pk["hbm_gbs"]}
 
     # ---- end to end through the C ABI with HOST buffers (D2H copies inside the timed region)
     e2e = None

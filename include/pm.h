@@ -93,6 +93,18 @@ int32_t pm_pattern(pm_lattice* lat, int32_t cell_begin, int32_t cell_end,
 int32_t pm_fill(pm_lattice* lat, int32_t cell_begin, int32_t cell_end,
                 const int64_t* d_rowptr, double* d_vals, void* cuda_stream);
 
+/* Pattern and fill of one block in one call: the pattern pass up to rowptr and nnz (the stream is synchronised for
+ * *nnz_host), then ONE kernel writes both the column index and the value of every nonzero — the separate column
+ * kernel of pm_pattern is not run.  Same results as pm_pattern + pm_fill, bit for bit.
+ *   d_rowptr, d_colidx, d_vals : device, as in pm_pattern / pm_fill;  capacity : entries d_colidx and d_vals can hold;
+ *   PM_ERR_OVERFLOW (with *nnz_host valid, nothing written to d_colidx / d_vals) if nnz exceeds it. */
+int32_t pm_build(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int64_t* d_rowptr, int32_t* d_colidx, double* d_vals,
+                 int64_t capacity, int64_t* nnz_host, void* cuda_stream);
+
+/* Device time of the last fill kernel launched for this lattice (by pm_fill, pm_build or pm_build_host), from CUDA
+ * events recorded around it on its stream; waits for that kernel.  PM_ERR_STATE before the first fill. */
+int32_t pm_last_fill_ms(pm_lattice* lat, float* ms);
+
 /* y = A x for a CSR block (convenience check only): n_rows rows, GLOBAL columns. */
 int32_t pm_spmv(pm_lattice* lat, int64_t n_rows, const int64_t* d_rowptr, const int32_t* d_colidx,
                 const double* d_vals, const double* d_x, double* d_y, void* cuda_stream);

@@ -23,7 +23,7 @@ ERRORS = {-1: "PM_ERR_ARG", -2: "PM_ERR_GRID", -3: "PM_ERR_CHANNEL", -4: "PM_ERR
 
 EXPORTS = ["pm_lattice_create", "pm_lattice_destroy", "pm_lattice_dims", "pm_lattice_rule", "pm_lattice_set_rule",
            "pm_lattice_coupling", "pm_lattice_work", "pm_pattern_counts", "pm_lattice_fill_kernel", "pm_diag_sqrt_threshold",
-           "pm_diag_dfma_tflops", "pm_pattern", "pm_fill", "pm_spmv", "pm_build_host_count", "pm_build_host",
+           "pm_diag_dfma_tflops", "pm_pattern", "pm_fill", "pm_build", "pm_last_fill_ms", "pm_spmv", "pm_build_host_count", "pm_build_host",
            "pm_launch_count", "pm_last_error"]
 
 
@@ -68,6 +68,8 @@ def lib():
     L.pm_diag_sqrt_threshold.restype = C.c_double
     L.pm_pattern.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, C.c_int64, _i64p, _vp]
     L.pm_fill.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, _vp]
+    L.pm_last_fill_ms.argtypes = [_vp, C.POINTER(C.c_float)]
+    L.pm_build.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, _vp, C.c_int64, _i64p, _vp]
     L.pm_spmv.argtypes = [_vp, C.c_int64, _vp, _vp, _vp, _vp, _vp, _vp]
     L.pm_build_host_count.argtypes = [_vp, C.c_int64, _i64p, _i32p]
     L.pm_build_host.argtypes = [_vp, C.c_int64, _vp, _vp, _vp, C.c_int64, _i64p, _i32p]
@@ -176,6 +178,20 @@ def pm_fill(h, cell_begin, cell_end, d_rowptr, d_vals, stream=None):
     _check(lib().pm_fill(h, cell_begin, cell_end, d_rowptr.data_ptr(), d_vals.data_ptr(), _stream_ptr(stream)))
 
 
+def pm_build(h, cell_begin, cell_end, d_rowptr, d_colidx, d_vals, stream=None):
+    """Pattern + fill of one block, columns and values written by one kernel.  Returns nnz."""
+    nnz = C.c_int64()
+    _check(lib().pm_build(h, cell_begin, cell_end, d_rowptr.data_ptr(), d_colidx.data_ptr(), d_vals.data_ptr(),
+                          min(d_colidx.numel(), d_vals.numel()), C.byref(nnz), _stream_ptr(stream)))
+    return nnz.value
+
+
+def pm_last_fill_ms(h):
+    ms = C.c_float()
+    _check(lib().pm_last_fill_ms(h, C.byref(ms)))
+    return ms.value
+
+
 def pm_spmv(h, d_rowptr, d_colidx, d_vals, d_x, d_y, stream=None):
     _check(lib().pm_spmv(h, d_rowptr.numel() - 1, d_rowptr.data_ptr(), d_colidx.data_ptr(), d_vals.data_ptr(),
                          d_x.data_ptr(), d_y.data_ptr(), _stream_ptr(stream)))
@@ -248,6 +264,17 @@ class Lattice:
     def build(self, cell_begin=0, cell_end=None):
         rowptr, colidx, nnz = self.pattern(cell_begin, cell_end)
         return rowptr, colidx, self.fill(rowptr, nnz, cell_begin, cell_end)
+
+    def build_fused(self, cell_begin=0, cell_end=None):
+        """pm_build: count (rowptr, nnz), allocate, then one call that writes columns and values together."""
+        import torch
+        cell_end = self.n_cells if cell_end is None else cell_end
+        rowptr, _, nnz = self.pattern(cell_begin, cell_end, count_only=True)
+        colidx = torch.empty(max(nnz, 1), dtype=torch.int32, device="cuda")[:nnz]
+        vals = torch.empty(max(nnz, 1), dtype=torch.float64, device="cuda")[:nnz]
+        if nnz:
+            pm_build(self.h, cell_begin, cell_end, rowptr, colidx, vals)
+        return rowptr, colidx, vals
 
     def spmv(self, rowptr, colidx, vals, x):
         import torch

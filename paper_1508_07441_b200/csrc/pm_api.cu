@@ -51,6 +51,8 @@ struct pm_lattice {
     bool have_plan = false;
     pm::FillLaunch plan{};
     int* d_counter = nullptr;          // work counter of the fill kernel
+    cudaEvent_t ev_fill0 = nullptr, ev_fill1 = nullptr;   // around the last fill kernel, on its stream (pm_last_fill_ms)
+    bool fill_timed = false;
     unsigned long long hash = 0;       // pm::tables_hash of T (selects a generated fill kernel)
     int n_sm = 0;
     pm::DevLattice dev{};
@@ -71,6 +73,9 @@ void free_device(pm_lattice* L)
     if (L->h_summary) cudaFreeHost(L->h_summary);
     if (L->d_counter) cudaFree(L->d_counter);
     L->d_counter = nullptr;
+    if (L->ev_fill0) cudaEventDestroy(L->ev_fill0);
+    if (L->ev_fill1) cudaEventDestroy(L->ev_fill1);
+    L->ev_fill0 = L->ev_fill1 = nullptr; L->fill_timed = false;
     L->d_blob = nullptr; L->nl = pm::NodeLists{}; L->d_cellbase = nullptr; L->d_summary = nullptr; L->h_summary = nullptr;
     L->hits_cap = 0;
 }
@@ -146,6 +151,7 @@ int32_t ensure_device(pm_lattice* L)
     if ((e = cudaMemcpy(L->d_blob, blob.data(), blob.size(), cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_fail(e, "cudaMemcpy(tables)");
     if ((e = cudaMalloc(&L->d_summary, 4 * sizeof(int64_t))) != cudaSuccess) return cuda_fail(e, "cudaMalloc(summary)");
     if ((e = cudaMalloc(&L->d_counter, sizeof(int))) != cudaSuccess) return cuda_fail(e, "cudaMalloc(counter)");
+    if ((e = cudaEventCreate(&L->ev_fill0)) != cudaSuccess || (e = cudaEventCreate(&L->ev_fill1)) != cudaSuccess) return cuda_fail(e, "cudaEventCreate");
     if ((e = cudaMallocHost(&L->h_summary, 4 * sizeof(int64_t))) != cudaSuccess) return cuda_fail(e, "cudaMallocHost(summary)");
     char* b = L->d_blob;
     D.pe = (const double*)(b + o_pe); D.qe = (const double*)(b + o_qe);
@@ -386,17 +392,17 @@ int32_t pm_pattern(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int64_
     return PM_OK;
 }
 
-int32_t pm_fill(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const int64_t* d_rowptr, double* d_vals, void* cuda_stream)
+}  // extern "C"
+
+namespace {
+
+// values (and, when d_colidx is given, column indices) of the block of the last pattern call
+int32_t fill_block(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const int64_t* d_rowptr, double* d_vals,
+                   int32_t* d_colidx, cudaStream_t st)
 {
-    if (!lat || !d_rowptr || !d_vals) return fail(PM_ERR_ARG, "NULL argument");
-    const int n_cells = lat->Np * lat->Nq;
-    if (cell_begin < 0 || cell_end > n_cells || cell_begin > cell_end) return fail(PM_ERR_ARG, "bad cell range");
-    int32_t rc = ensure_device(lat);
-    if (rc) return rc;
     if (lat->hmax < 0 || cell_begin != lat->pat_begin || cell_end != lat->pat_end)
         return fail(PM_ERR_STATE, "pm_fill needs a preceding pm_pattern of the same cell range on this lattice");
     if (cell_begin == cell_end) return PM_OK;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
     const int n_blk = cell_end - cell_begin;
     cudaError_t e;
     if (!lat->have_plan) {
@@ -405,9 +411,48 @@ int32_t pm_fill(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const int
         if (e != cudaSuccess) return cuda_fail(e, "fill_plan");
         lat->have_plan = true;
     }
-    e = pm::launch_fill(lat->dev, lat->plan, cell_begin, n_blk, lat->nl, d_rowptr, d_vals, lat->d_counter, st);
+    cudaEventRecord(lat->ev_fill0, st);
+    e = pm::launch_fill(lat->dev, lat->plan, cell_begin, n_blk, lat->nl, d_rowptr, d_vals, d_colidx, lat->d_counter, st);
+    cudaEventRecord(lat->ev_fill1, st);
     if (e != cudaSuccess) return cuda_fail(e, "k_fill");
+    lat->fill_timed = true;
     return PM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int32_t pm_fill(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const int64_t* d_rowptr, double* d_vals, void* cuda_stream)
+{
+    if (!lat || !d_rowptr || !d_vals) return fail(PM_ERR_ARG, "NULL argument");
+    const int n_cells = lat->Np * lat->Nq;
+    if (cell_begin < 0 || cell_end > n_cells || cell_begin > cell_end) return fail(PM_ERR_ARG, "bad cell range");
+    int32_t rc = ensure_device(lat);
+    if (rc) return rc;
+    return fill_block(lat, cell_begin, cell_end, d_rowptr, d_vals, nullptr, (cudaStream_t)cuda_stream);
+}
+
+int32_t pm_last_fill_ms(pm_lattice* lat, float* ms)
+{
+    if (!lat || !ms) return fail(PM_ERR_ARG, "NULL argument");
+    if (!lat->fill_timed) return fail(PM_ERR_STATE, "no fill kernel has been launched on this lattice");
+    cudaError_t e = cudaEventSynchronize(lat->ev_fill1);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(ms, lat->ev_fill0, lat->ev_fill1);
+    if (e != cudaSuccess) return cuda_fail(e, "pm_last_fill_ms");
+    return PM_OK;
+}
+
+int32_t pm_build(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int64_t* d_rowptr, int32_t* d_colidx, double* d_vals,
+                 int64_t capacity, int64_t* nnz_host, void* cuda_stream)
+{
+    if (!lat || !d_rowptr || !d_colidx || !d_vals || !nnz_host) return fail(PM_ERR_ARG, "NULL argument");
+    // pattern pass without the column kernel: node lists, rowptr, nnz ...
+    int32_t rc = pm_pattern(lat, cell_begin, cell_end, d_rowptr, nullptr, 0, nnz_host, cuda_stream);
+    if (rc) return rc;
+    if (*nnz_host > capacity) return fail(PM_ERR_OVERFLOW, "d_colidx / d_vals too small for this block's nnz");
+    // ... then one kernel writes the column index and the value of every nonzero
+    return fill_block(lat, cell_begin, cell_end, d_rowptr, d_vals, d_colidx, (cudaStream_t)cuda_stream);
 }
 
 int32_t pm_spmv(pm_lattice* lat, int64_t n_rows, const int64_t* d_rowptr, const int32_t* d_colidx, const double* d_vals,

@@ -13,16 +13,18 @@ namespace {
 
 constexpr int kSmemLimit = 227 * 1024;
 
-using FillKernel = void (*)(DevLattice, FillSmem, NodeLists, int, int, const int64_t*, double*, int*);
+using FillKernel = void (*)(DevLattice, FillSmem, NodeLists, int, int, const int64_t*, double*, int32_t*, int*);
 
-struct FillVariant { unsigned long long hash; int nw; FillKernel fn; const char* name; };
+struct FillVariant { unsigned long long hash; int nw, rb; FillKernel fn, fn_cols; const char* name; };
 
-#define PM_SPEC(S) {gen::S::kHash, 4, k_fill_warp<gen::S, 4>, #S}, {gen::S::kHash, 6, k_fill_warp<gen::S, 6>, #S}, \
-                   {gen::S::kHash, 8, k_fill_warp<gen::S, 8>, #S}, {gen::S::kHash, 12, k_fill_warp<gen::S, 12>, #S},
+#define PM_VAR(S, NW, RB) {gen::S::kHash, NW, RB, k_fill_warp<gen::S, NW, RB, false>, k_fill_warp<gen::S, NW, RB, true>, #S}
+#define PM_SPEC(S) PM_VAR(S, 4, 4), PM_VAR(S, 8, 4), PM_VAR(S, 12, 4),
 const FillVariant kVariants[] = {
     PM_SPEC_LIST
-    {0ull, 4, k_fill_warp<SpecGeneric, 4>, "generic"}, {0ull, 8, k_fill_warp<SpecGeneric, 8>, "generic"},
+    {0ull, 4, 4, k_fill_warp<SpecGeneric, 4, 4, false>, k_fill_warp<SpecGeneric, 4, 4, true>, "generic"},
+    {0ull, 8, 4, k_fill_warp<SpecGeneric, 8, 4, false>, k_fill_warp<SpecGeneric, 8, 4, true>, "generic"},
 };
+#undef PM_VAR
 #undef PM_SPEC
 
 int preferred_warps()
@@ -54,18 +56,20 @@ cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int n_sm, Fi
     const int want = preferred_warps();
     const FillVariant* best = nullptr;          // largest warp count <= want whose shared memory fits, else the smallest that fits
     for (const FillVariant& v : kVariants) {
-        if (v.hash != key || fill_smem_plan(L, v.nw).total > kSmemLimit) continue;
+        if (v.hash != key || fill_smem_plan(L, v.nw, v.rb).total > kSmemLimit) continue;
         if (!best) { best = &v; continue; }
         const bool v_ok = v.nw <= want, b_ok = best->nw <= want;
         if ((v_ok && (!b_ok || v.nw > best->nw)) || (!v_ok && !b_ok && v.nw < best->nw)) best = &v;
     }
     if (!best) return cudaErrorInvalidConfiguration;
     out->fn = (const void*)best->fn;
+    out->fn_cols = (const void*)best->fn_cols;
     out->nw = best->nw;
     out->name = best->name;
-    out->smem = fill_smem_plan(L, best->nw);
+    out->smem = fill_smem_plan(L, best->nw, best->rb);
     cudaError_t e = cudaFuncSetAttribute(out->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, out->smem.total);
     if (e != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(out->fn_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, out->smem.total)) != cudaSuccess) return e;
     int per_sm = 1;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, out->fn, best->nw * 32, (size_t)out->smem.total);
     if (e != cudaSuccess) return e;
@@ -74,7 +78,7 @@ cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int n_sm, Fi
 }
 
 cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl,
-                        const int64_t* rowptr, double* vals, int* counter, cudaStream_t st)
+                        const int64_t* rowptr, double* vals, int32_t* colidx, int* counter, cudaStream_t st)
 {
     const int need = (n_blk + F.nw - 1) / F.nw;                        // one cell per warp at a time
     const int grid = need < F.grid ? need : F.grid;
@@ -83,8 +87,8 @@ cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin
     NodeLists N = nl;
     cudaError_t e = cudaMemsetAsync(counter, 0, sizeof(int), st);      // the work counter the warps draw cells from
     if (e != cudaSuccess) return e;
-    void* args[] = {&Lc, &S, &N, &cell_begin, &n_blk, (void*)&rowptr, &vals, &counter};
-    e = cudaLaunchKernel(F.fn, dim3((unsigned)grid), dim3((unsigned)(F.nw * 32)), args, (size_t)S.total, st);
+    void* args[] = {&Lc, &S, &N, &cell_begin, &n_blk, (void*)&rowptr, &vals, &colidx, &counter};
+    e = cudaLaunchKernel(colidx ? F.fn_cols : F.fn, dim3((unsigned)grid), dim3((unsigned)(F.nw * 32)), args, (size_t)S.total, st);
     count_launch();
     return e != cudaSuccess ? e : cudaGetLastError();
 }

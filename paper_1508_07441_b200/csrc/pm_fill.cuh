@@ -47,16 +47,15 @@ struct SpecGeneric {
 };
 
 struct FillSmem {           // byte offsets into dynamic shared memory, computed on the host
-    int dp, dq, tp, tq, tx, sx, wx, bra, odesc, ofi, oc, warp0, warp_bytes, w_tile, w_sseg, w_acc, w_norm, w_wpa, w_wqb, total;
+    int dp, dq, tp, tq, tx, sx, wx, bra, odesc, ofi, oc, warp0, warp_bytes, w_tile, w_sseg, w_acc, w_norm, w_hcol, w_wpa, w_wqb, total;
 };
 
-constexpr int kRowBatch = 4;           // finished targets held per warp before their row entries are written
 constexpr int kTileStride = 33;        // double2 per K-tile row: 32 nodes + 1 pad (conflict-free rows and columns)
 
 inline int fill_align16(int b) { return (b + 15) & ~15; }
 
 // shared-memory plan for nw warps: tables shared by the CTA, then one private area per warp
-inline FillSmem fill_smem_plan(const DevLattice& L, int nw)
+inline FillSmem fill_smem_plan(const DevLattice& L, int nw, int row_batch)
 {
     FillSmem s{};
     int o = 0;
@@ -70,8 +69,9 @@ inline FillSmem fill_smem_plan(const DevLattice& L, int nw)
     auto wtake = [&](int bytes) { int r = w; w += fill_align16(bytes); return r; };
     s.w_tile = wtake(16 * kTileStride * np);
     s.w_sseg = wtake(16 * np);
-    s.w_acc = wtake(8 * L.n_fun * kRowBatch);
-    s.w_norm = wtake(8 * kRowBatch);
+    s.w_acc = wtake(8 * L.n_fun * row_batch);      // sums of finished targets waiting for their rows to be written
+    s.w_norm = wtake(8 * row_batch);
+    s.w_hcol = wtake(4 * row_batch);
     s.w_wpa = wtake(8 * L.n_p); s.w_wqb = wtake(8 * L.n_q);
     s.warp_bytes = w;
     s.warp0 = take(w * nw);
@@ -79,10 +79,10 @@ inline FillSmem fill_smem_plan(const DevLattice& L, int nw)
     return s;
 }
 
-template <class Spec, int NW>
+template <class Spec, int NW, int kRowBatch, bool kCols>
 __global__ void __launch_bounds__(NW * 32, 1)
 k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, const int64_t* __restrict__ rowptr,
-            double* __restrict__ vals, int* __restrict__ counter)
+            double* __restrict__ vals, int32_t* __restrict__ colidx, int* __restrict__ counter)
 {
     constexpr int T = NW * 32;
     constexpr int NP = (Spec::NS + 1) / 2;              // slot pairs (one double2 per pair and node in the K tile)
@@ -96,7 +96,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
     double* s_tp = (double*)(smem + S.tp);   double* s_tq = (double*)(smem + S.tq);   double* s_tx = (double*)(smem + S.tx);
     double* s_sx = (double*)(smem + S.sx);   double* s_wx = (double*)(smem + S.wx);
     double* s_bra = (double*)(smem + S.bra);
-    int* s_odesc = (int*)(smem + S.odesc);             // per output o: cl_off[alpha] | nc << 12 | m << 19
+    int* s_odesc = (int*)(smem + S.odesc);             // per output o: cl_off[alpha] | nc << 12 | m << 19 | alpha' << 25
     int* s_ofi = (int*)(smem + S.ofi);                 // f0 | f1 << 8 | f2 << 16 | n_terms << 24
     double* s_oc = (double*)(smem + S.oc);             // [o][3] coefficients c^L (0 where there is no term)
     char* wsm = smem + S.warp0 + warp * S.warp_bytes;
@@ -105,6 +105,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
     const double* s_sseg = (const double*)s_sseg2;
     double* s_acc = (double*)(wsm + S.w_acc);         // [kRowBatch][nf] sums of finished targets
     double* s_norm = (double*)(wsm + S.w_norm);
+    int* s_hcol = (int*)(wsm + S.w_hcol);               // first column of each finished target: cell * n_ch (kCols)
     double* s_wpa = (double*)(wsm + S.w_wpa);
     double* s_wqb = (double*)(wsm + S.w_wqb);
 
@@ -119,7 +120,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
     for (int o = tid; o < L.totcoup; o += T) {
         const int al = L.o_alpha[o], off = L.cl_off[al], nc = L.cl_off[al + 1] - off;
         const int t0 = L.ot_off[o], nt = L.ot_off[o + 1] - t0;
-        s_odesc[o] = off | (nc << 12) | ((o - off) << 19);
+        s_odesc[o] = off | (nc << 12) | ((o - off) << 19) | (L.cl[o] << 25);
         int fi = nt << 24;
         for (int i = 0; i < 3; ++i) {
             s_oc[3 * o + i] = i < nt ? L.ot_c[t0 + i] : 0.0;
@@ -159,7 +160,9 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         const CellGeom g = cell_geom(L.pe, L.qe, ci, cj);
         const int H = nl.hits[cb], we = nl.ntot[cb];
         const unsigned* __restrict__ g_key = nl.key + (size_t)cb * L.nnode;       // target cell << 14 | node id
-        double* __restrict__ row0 = vals + rowptr[(int64_t)cb * L.n_ch];
+        const int64_t rbase = rowptr[(int64_t)cb * L.n_ch];
+        double* __restrict__ row0 = vals + rbase;
+        int32_t* __restrict__ col0 = kCols ? colidx + rbase : nullptr;
         const double dsrc = s_dp[ci] * s_dq[cj];
         for (int k = lane; k < L.n_p; k += 32) s_wpa[k] = __dmul_rn(g.hp, L.wp[k]);
         for (int k = lane; k < L.n_q; k += 32) s_wqb[k] = __dmul_rn(g.hq, L.wq[k]);
@@ -169,10 +172,11 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         auto write_rows = [&](int k0, int nb) {
             for (int o = lane; o < L.totcoup; o += 32) {
                 const int od = s_odesc[o], fi = s_ofi[o];
-                const int clo = od & 4095, nc = (od >> 12) & 127, mm = od >> 19;
+                const int clo = od & 4095, nc = (od >> 12) & 127, mm = (od >> 19) & 63, ap = (unsigned)od >> 25;
                 const double c0 = s_oc[3 * o], c1 = s_oc[3 * o + 1], c2 = s_oc[3 * o + 2];
                 const int f0 = fi & 255, f1 = (fi >> 8) & 255, f2 = (fi >> 16) & 255, nt = fi >> 24;
-                double* out = row0 + ((size_t)H * clo + (size_t)k0 * nc + mm);
+                const size_t idx0 = (size_t)H * clo + (size_t)k0 * nc + mm;
+                double* out = row0 + idx0;
 #pragma unroll
                 for (int bb = 0; bb < kRowBatch; ++bb) {
                     if (bb < nb) {
@@ -183,6 +187,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                             for (int t = 3; t < nt; ++t) v = fma(L.ot_c[t0 + t], acc[L.ot_f[t0 + t]], v);
                         }
                         out[(size_t)bb * nc] = v * s_norm[bb];
+                        if (kCols) col0[idx0 + (size_t)bb * nc] = s_hcol[bb] + ap;
                     }
                 }
             }
@@ -312,7 +317,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                     }
                     const int tcell = __shfl_sync(0xffffffffu, tC, jb);
                     const int ic = tcell / L.Nq, jc = tcell - ic * L.Nq;
-                    if (lane == 0) s_norm[slot] = 1.0 / sqrt(dsrc * (s_dp[ic] * s_dq[jc]));
+                    if (lane == 0) { s_norm[slot] = 1.0 / sqrt(dsrc * (s_dp[ic] * s_dq[jc])); s_hcol[slot] = tcell * L.n_ch; }
                     ++kcur;
                     __syncwarp();
                     if (kcur - kdone == kRowBatch) { write_rows(kdone, kRowBatch); kdone = kcur; }

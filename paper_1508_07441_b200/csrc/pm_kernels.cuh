@@ -25,12 +25,12 @@ cudaError_t launch_emit_cols(const DevLattice& L, int n_blk, const NodeLists& nl
                              int32_t* colidx, cudaStream_t st);
 
 // fill pass (pm_fill.cuh): variant selection and launch
-struct FillLaunch { const void* fn; int nw, grid; FillSmem smem; const char* name; };
+struct FillLaunch { const void *fn, *fn_cols; int nw, grid; FillSmem smem; const char* name; };   // fn_cols also writes colidx
 bool fill_has_spec(unsigned long long tables_hash);
 const char* fill_variant_name(unsigned long long tables_hash);
 cudaError_t fill_plan(const DevLattice& L, unsigned long long tables_hash, int n_sm, FillLaunch* out);
 cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl,
-                        const int64_t* rowptr, double* vals, int* counter, cudaStream_t st);
+                        const int64_t* rowptr, double* vals, int32_t* colidx, int* counter, cudaStream_t st);
 
 cudaError_t launch_spmv(int64_t n_rows, const int64_t* rowptr, const int32_t* colidx, const double* vals,
                         const double* x, double* y, cudaStream_t st);

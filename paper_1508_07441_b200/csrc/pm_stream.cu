@@ -104,11 +104,9 @@ int32_t pm_build_host(pm_lattice* lat, int64_t device_budget_bytes, int64_t* h_r
         const int64_t off = P.rowptr[(size_t)cb * P.n_ch];
         int64_t nnz = 0;
         // the stream of this buffer set is idle here: pm_pattern synchronises it before reusing the buffers
-        rc = pm_pattern(lat, cb, ce, B.rowptr, B.col, P.max_blk, &nnz, B.st);
+        rc = pm_build(lat, cb, ce, B.rowptr, B.col, B.val, P.max_blk, &nnz, B.st);
         if (rc) break;
         if (nnz != P.rowptr[(size_t)ce * P.n_ch] - off) { rc = PM_ERR_STATE; break; }
-        rc = pm_fill(lat, cb, ce, B.rowptr, B.val, B.st);
-        if (rc) break;
         if (cudaEventRecord(filled, B.st) != cudaSuccess) { rc = PM_ERR_CUDA; break; }
         if (cudaMemcpyAsync(h_colidx + off, B.col, sizeof(int32_t) * (size_t)nnz, cudaMemcpyDeviceToHost, B.st) != cudaSuccess ||
             cudaMemcpyAsync(h_vals + off, B.val, sizeof(double) * (size_t)nnz, cudaMemcpyDeviceToHost, B.st) != cudaSuccess)

@@ -92,6 +92,20 @@ def test_generic_kernel_parity_on_reordered_channels(api, oracle):
     lat.close()
 
 
+@pytest.mark.parametrize("wl", [I.config(1), I.small_coupled(N=7, jmax=3, orders=(4, 5, 7))], ids=lambda w: w.name)
+def test_pm_build_equals_pattern_plus_fill(api, wl):
+    """pm_build (columns and values from one kernel) is bit-identical to pm_pattern + pm_fill."""
+    lat = api.Lattice(wl)
+    a = [t.cpu().numpy() for t in lat.build()]
+    b = [t.cpu().numpy() for t in lat.build_fused()]
+    assert all(np.array_equal(x, y) for x, y in zip(a, b))
+    c = [t.cpu().numpy() for t in lat.build_fused(3, 11)]
+    d = [t.cpu().numpy() for t in lat.build(3, 11)]
+    assert all(np.array_equal(x, y) for x, y in zip(c, d))
+    assert api.pm_last_fill_ms(lat.h) > 0.0
+    lat.close()
+
+
 def test_pattern_counts(api):
     wl = I.config(1)
     lat = api.Lattice(wl)
