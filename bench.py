@@ -83,6 +83,23 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm)}
 
 
+def max_over_ranks(x: float, world: int, device="cuda") -> float:
+    """Max of a per-rank scalar over all ranks (device time of the slowest rank); identity for one rank."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(units_per_rank_step: float, steps: int, total_ms: float, world: int) -> float:
+    """Whole-job units per second: every rank processes `units_per_rank_step` per step (replicas, weak scaling),
+    `total_ms` is the max over ranks of the time for `steps` steps."""
+    return world * units_per_rank_step * steps / (total_ms * 1e-3)
+
+
 def build_flops(lat_api, h):
     """Algorithmic FP64 flops of one build: pm_lattice_work x pm_pattern_counts."""
     per_node, per_seg, per_hit, _ = lat_api.pm_lattice_work(h)
@@ -192,11 +209,8 @@ def main():
             fill_ms.append(api.pm_last_fill_ms(lat.h))        # CUDA events around the fill kernel, on its stream
         barrier()
     launches = api.pm_launch_count() - l0
-    tot = torch.tensor([sum(step_ms)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tot, op=dist.ReduceOp.MAX)
-    total_ms = float(tot.item())
-    value = world * nnz * args.steps / (total_ms * 1e-3)
+    total_ms = max_over_ranks(sum(step_ms), world)
+    value = job_throughput(nnz, args.steps, total_ms, world)
 
     # ---- roofline of the dominant kernel (fill): FP64 ALU bound
     pk = _peaks()
@@ -236,11 +250,9 @@ def main():
         for _ in range(args.e2e_steps):
             _, nb = e2e_step()
         barrier()
-        dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+        dt_s = max_over_ranks(time.perf_counter() - t0, world)
         h2d = wl.p_edges.nbytes + wl.q_edges.nbytes + wl.channels.nbytes + sum(a.nbytes + b.nbytes for a, b in wl.rules.values())
-        e2e = {"value": world * nnz * args.e2e_steps / float(dt.item()), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+        e2e = {"value": job_throughput(nnz, args.e2e_steps, dt_s * 1e3, world), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(12 * nnz + 8 * (wl.M + 1)), "blocks": nb, "steps": args.e2e_steps,
                "api": "pm_lattice_create + pm_lattice_set_rule + pm_build_host (pinned host buffers) + pm_lattice_destroy"}
 
