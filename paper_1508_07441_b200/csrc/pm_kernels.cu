@@ -7,6 +7,8 @@
 // cell-major row order makes every row segment contiguous, so no repack exists.
 #include "pm_kernels.cuh"
 
+#include <cstdlib>
+
 namespace pm {
 
 __device__ __forceinline__ char* carve(char*& p, size_t bytes)
@@ -22,17 +24,17 @@ static size_t al16(size_t b) { return (b + 15) & ~size_t(15); }
 // Pattern pass, kernel A: map every node of a source cell, rank the hit cells, stable counting sort of the
 // node ids by rank.  Node id m = c*(n_p*n_q) + a*n_q + b, so the sorted list is ordered by (target, x-node, a, b).
 // ------------------------------------------------------------------------------------------------
-size_t map_sort_smem(const DevLattice& L)
+size_t map_sort_smem(const DevLattice& L, int hits_fast)
 {
     const int nw = kThreads / 32;
     const int hcap = std::min(L.nnode, L.n_cells);
     return al16(8 * (size_t)L.pe_pad) + al16(8 * (size_t)L.qe_pad) + 2 * al16(2 * (size_t)kBuckets) + al16(8 * (size_t)L.n_p) + al16(8 * (size_t)L.n_q)
          + al16(8 * (size_t)L.n_x) + 2 * al16(4 * (size_t)L.n_words) + al16(4 * (size_t)(kThreads + 1))
          + 2 * al16(4 * (size_t)L.nnode) + 3 * al16(2 * (size_t)L.nnode) + al16(4 * (size_t)(hcap + 1))
-         + al16(4 * (size_t)std::max(nw * std::min(hcap, kHitsFast), hcap));
+         + al16(4 * (size_t)std::max(nw * std::min(hcap, hits_fast), hcap));
 }
 
-__global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_begin, NodeLists nl)
+__global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_begin, NodeLists nl, int hits_fast)
 {
     extern __shared__ __align__(16) char smem[];
     constexpr int T = kThreads, NW = kThreads / 32;
@@ -56,7 +58,7 @@ __global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_be
     unsigned short* s_rk = (unsigned short*)carve(sp, 2 * (size_t)L.nnode);     // rank of each node's target (0xffff: off the grid)
     int* s_tcpos = (int*)carve(sp, 4 * (size_t)L.nnode);                         // target cell at each sorted position
     int* s_start = (int*)carve(sp, 4 * (size_t)(hcap + 1));
-    int* s_hist = (int*)carve(sp, 4 * (size_t)max(NW * min(hcap, kHitsFast), hcap));
+    int* s_hist = (int*)carve(sp, 4 * (size_t)max(NW * min(hcap, hits_fast), hcap));
 
     for (int k = tid; k < L.pe_pad; k += T) s_thr_p[k] = L.thr_p[k];
     for (int k = tid; k < L.qe_pad; k += T) s_thr_q[k] = L.thr_q[k];
@@ -83,8 +85,8 @@ __global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_be
     __syncthreads();
     const int H = rank_bits_n(L.n_words, hs);
     // stable counting sort: each of `nwe` warps owns a contiguous slice of node ids and a histogram of H counters
-    // (all warps when H <= kHitsFast, else warp 0 alone: rare, slow, same result)
-    const int nwe = (H <= kHitsFast) ? NW : 1;
+    // (all warps when H <= hits_fast, else warp 0 alone: rare, slow, same result)
+    const int nwe = (H <= hits_fast) ? NW : 1;
     for (int k = tid; k < nwe * H; k += T) s_hist[k] = 0;
     __syncthreads();
     const int slice = (((L.nnode + nwe - 1) / nwe) + 31) & ~31;
@@ -255,10 +257,12 @@ void count_launch() { ++g_launches; }
 
 cudaError_t launch_map_sort(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, cudaStream_t st)
 {
-    const size_t sm = map_sort_smem(L);
+    // per-warp histograms up to this many hit cells per source cell, one warp beyond (PM_HITS_FAST: test hook)
+    static const int hits_fast = [] { const char* e = std::getenv("PM_HITS_FAST"); return e ? std::max(1, std::atoi(e)) : kHitsFast; }();
+    const size_t sm = map_sort_smem(L, hits_fast);
     cudaError_t e = cudaFuncSetAttribute(k_map_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
-    k_map_sort<<<n_blk, kThreads, sm, st>>>(L, cell_begin, nl);
+    k_map_sort<<<n_blk, kThreads, sm, st>>>(L, cell_begin, nl, hits_fast);
     ++g_launches;
     return cudaGetLastError();
 }

@@ -13,7 +13,7 @@ namespace pm {
 constexpr int kThreads = 256;
 constexpr int kHitsFast = 512;      // k_map_sort: per-warp histograms up to this many hit cells, one warp beyond
 
-size_t map_sort_smem(const DevLattice& L);
+size_t map_sort_smem(const DevLattice& L, int hits_fast);
 int64_t launch_count();
 void count_launch();
 

@@ -2,12 +2,15 @@
 
 Bar (BASELINE.json north_star): rowptr and colidx bit-exact; |dP| <= max(1e-11*|P_ref|, 1e-14*max|P|).
 """
+import os
+
 import numpy as np
 import pytest
 
 from paper_1508_07441_b200 import inputs as I
 
 pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 REL, FLOOR = 1e-11, 1e-14
 
@@ -106,6 +109,27 @@ def test_pm_build_equals_pattern_plus_fill(api, wl):
     lat.close()
 
 
+def test_single_warp_sort_path(oracle):
+    """Source cells with more hit cells than the per-warp histograms hold are sorted by one warp; the test hook
+    PM_HITS_FAST=8 sends almost every cell of configs[1] down that path (own process: the hook is read once)."""
+    import subprocess
+    import sys
+    import tempfile
+    code = (
+        "import sys, numpy as np; sys.path.insert(0, %r)\n"
+        "from paper_1508_07441_b200 import api, inputs\n"
+        "wl = inputs.config(1); lat = api.Lattice(wl); rp, ci, v = lat.build_fused()\n"
+        "np.savez(sys.argv[1], rp=rp.cpu().numpy(), ci=ci.cpu().numpy(), v=v.cpu().numpy())\n"
+    ) % ROOT
+    with tempfile.TemporaryDirectory() as d:
+        out = os.path.join(d, "r.npz")
+        subprocess.run([sys.executable, "-c", code, out], check=True, env=dict(os.environ, PM_HITS_FAST="8"), timeout=600)
+        r = np.load(out)
+        rpo, cio, vo = oracle.build_csr(I.config(1))
+        assert np.array_equal(r["rp"], rpo) and np.array_equal(r["ci"], cio)
+        _assert_values(r["v"], vo)
+
+
 def test_pattern_counts(api):
     wl = I.config(1)
     lat = api.Lattice(wl)
@@ -136,7 +160,7 @@ def test_full_size_sampled_rows(api, oracle, k):
     import torch
     wl = I.config(k)
     lat = api.Lattice(wl)
-    rp, ci, v = lat.build()
+    rp, ci, v = lat.build_fused()                  # pm_build: the call bench.py times
     rp_h = rp.cpu().numpy()
     rng = np.random.default_rng(100 + k)
     cells = sorted(set(rng.integers(0, wl.n_cells, size=5).tolist()) | {0, wl.n_cells - 1, wl.Nq * (wl.Np // 2) + 3})
