@@ -71,9 +71,9 @@ std::string emit_spec(const std::string& name, const Tables& T, Stats& st)
     const int nf = (int)T.fun.size();
     o << "struct Spec_" << name << " {\n";
     o << "    static constexpr bool kStatic = true;\n";
-    int maxm = 1;
-    for (const OrbFun& f : T.fun) maxm = std::max(maxm, f.nM);
-    o << "    static constexpr int NS = " << T.n_slot << ", NF = " << nf << ", NCH = " << (nf + 31) / 32 << ", MAXM = " << maxm << ";\n";
+    int maxm = 1, maxl1 = 1;                        // most M-terms of a function; number of L values (terms per output)
+    for (const OrbFun& f : T.fun) { maxm = std::max(maxm, f.nM); maxl1 = std::max(maxl1, f.L + 1); }
+    o << "    static constexpr int NS = " << T.n_slot << ", NF = " << nf << ", NCH = " << (nf + 31) / 32 << ", MAXM = " << maxm << ", MAXL1 = " << maxl1 << ";\n";
     char hb[32]; std::snprintf(hb, sizeof hb, "0x%016" PRIx64 "ull", tables_hash(T));
     o << "    static constexpr unsigned long long kHash = " << hb << ";\n";
     o << "    // K[s] = omega * (ket bipolar harmonic of slot s) at directions a = p'^ = (uxa,0,uza), b = q'^ = (uxb,0,uzb)\n";

@@ -16,6 +16,7 @@
 // (PAPER.md:L341, L348-356, L376).
 #pragma once
 #include <cstdint>
+#include <type_traits>
 #include <cuda_runtime.h>
 
 #include "pm_device.cuh"
@@ -30,7 +31,7 @@ constexpr int kFillMaxY = 45;
 // Table-driven ket code for channel sets without a generated kernel (slow: local arrays, table loads).
 struct SpecGeneric {
     static constexpr bool kStatic = false;
-    static constexpr int NS = kFillMaxSlot, NF = kFillMaxFun, NCH = kFillMaxFun / 32, MAXM = 99;
+    static constexpr int NS = kFillMaxSlot, NF = kFillMaxFun, NCH = kFillMaxFun / 32, MAXM = 99, MAXL1 = 99;
     static constexpr unsigned long long kHash = 0ull;
     static __device__ __noinline__ void ket(const DevLattice& L, double om, double uxa, double uza, double uxb, double uzb,
                                             double (&K)[NS])
@@ -169,29 +170,38 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         __syncwarp();
         int kcur = 0, kdone = 0;                        // targets finished / written; a target's rank is its position in every row
         // ---- E: lane = output (alpha, m-th coupled alpha'): P = norm_t * sum_L c^L acc_t[f] for targets k0 .. k0+nb-1
-        auto write_rows = [&](int k0, int nb) {
+        auto write_rows_t = [&](int k0, int nb, auto full_tag) {
+            constexpr bool kFull = decltype(full_tag)::value;           // all kRowBatch slots hold a target
+            double nrm[kRowBatch];
+            int hcl[kRowBatch];
+#pragma unroll
+            for (int bb = 0; bb < kRowBatch; ++bb) { nrm[bb] = s_norm[bb]; hcl[bb] = kCols ? s_hcol[bb] : 0; }
             for (int o = lane; o < L.totcoup; o += 32) {
                 const int od = s_odesc[o], fi = s_ofi[o];
                 const int clo = od & 4095, nc = (od >> 12) & 127, mm = (od >> 19) & 63, ap = (unsigned)od >> 25;
                 const double c0 = s_oc[3 * o], c1 = s_oc[3 * o + 1], c2 = s_oc[3 * o + 2];
-                const int f0 = fi & 255, f1 = (fi >> 8) & 255, f2 = (fi >> 16) & 255, nt = fi >> 24;
+                const int f0 = fi & 255, f1 = (fi >> 8) & 255, f2 = (fi >> 16) & 255;
                 const size_t idx0 = (size_t)H * clo + (size_t)k0 * nc + mm;
                 double* out = row0 + idx0;
+                int32_t* outc = kCols ? col0 + idx0 : nullptr;
 #pragma unroll
                 for (int bb = 0; bb < kRowBatch; ++bb) {
-                    if (bb < nb) {
+                    if (kFull || bb < nb) {
                         const double* acc = s_acc + bb * nf;
                         double v = fma(c2, acc[f2], fma(c1, acc[f1], c0 * acc[f0]));
-                        if (nt > 3) {
-                            const int t0 = L.ot_off[o];
+                        if (Spec::MAXL1 > 3) {                           // more than three L values: the tail comes from the tables
+                            const int t0 = L.ot_off[o], nt = fi >> 24;
                             for (int t = 3; t < nt; ++t) v = fma(L.ot_c[t0 + t], acc[L.ot_f[t0 + t]], v);
                         }
-                        out[(size_t)bb * nc] = v * s_norm[bb];
-                        if (kCols) col0[idx0 + (size_t)bb * nc] = s_hcol[bb] + ap;
+                        out[bb * nc] = v * nrm[bb];
+                        if (kCols) outc[bb * nc] = hcl[bb] + ap;
                     }
                 }
             }
             __syncwarp();
+        };
+        auto write_rows = [&](int k0, int nb) {
+            if (nb == kRowBatch) write_rows_t(k0, nb, std::true_type{}); else write_rows_t(k0, nb, std::false_type{});
         };
 
         // ---- C + D: 32 sorted nodes per step; the node ids of the next two steps are already in flight
