@@ -99,7 +99,7 @@ int32_t ensure_device(pm_lattice* L)
     pm::DevLattice D{};
     D.Np = L->Np; D.Nq = L->Nq; D.n_ch = L->n_ch; D.n_p = L->n_p; D.n_q = L->n_q; D.n_x = L->n_x;
     D.nnode = L->n_p * L->n_q * L->n_x; D.n_cells = L->Np * L->Nq; D.n_words = (D.n_cells + 31) / 32;
-    D.pe_pad = next_pow2(L->Np + 1); D.qe_pad = next_pow2(L->Nq + 1);
+    D.pe_pad = next_pow2(L->Np + 2); D.qe_pad = next_pow2(L->Nq + 2);     // at least one +inf sentinel after the last edge
     D.totcoup = T.totcoup; D.n_slot = T.n_slot; D.n_fun = (int)T.fun.size(); D.lmax = T.lmax;
     D.ny = pm::ylm_index(T.lmax, T.lmax) + 1;
     auto magic = [](int d) { return d <= 1 ? 0u : (unsigned)(((1ull << 32) + (unsigned)d - 1) / (unsigned)d); };

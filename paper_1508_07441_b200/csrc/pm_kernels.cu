@@ -30,7 +30,7 @@ size_t map_sort_smem(const DevLattice& L, int hits_fast)
     const int hcap = std::min(L.nnode, L.n_cells);
     return al16(8 * (size_t)L.pe_pad) + al16(8 * (size_t)L.qe_pad) + 2 * al16(2 * (size_t)kBuckets) + al16(8 * (size_t)L.n_p) + al16(8 * (size_t)L.n_q)
          + al16(8 * (size_t)L.n_x) + 2 * al16(4 * (size_t)L.n_words) + al16(4 * (size_t)(kThreads + 1))
-         + 2 * al16(4 * (size_t)L.nnode) + 3 * al16(2 * (size_t)L.nnode) + al16(4 * (size_t)(hcap + 1))
+         + al16(4 * (size_t)L.nnode) + al16(2 * (size_t)L.nnode) + al16(4 * (size_t)(hcap + 1))
          + al16(4 * (size_t)std::max(nw * std::min(hcap, hits_fast), hcap));
 }
 
@@ -53,10 +53,7 @@ __global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_be
     hs.wpre = (int*)carve(sp, 4 * (size_t)L.n_words);
     hs.scratch = (int*)carve(sp, 4 * (size_t)(T + 1));
     int* s_tgt = (int*)carve(sp, 4 * (size_t)L.nnode);
-    unsigned short* s_sorted = (unsigned short*)carve(sp, 2 * (size_t)L.nnode);
-    unsigned short* s_rkpos = (unsigned short*)carve(sp, 2 * (size_t)L.nnode);
     unsigned short* s_rk = (unsigned short*)carve(sp, 2 * (size_t)L.nnode);     // rank of each node's target (0xffff: off the grid)
-    int* s_tcpos = (int*)carve(sp, 4 * (size_t)L.nnode);                         // target cell at each sorted position
     int* s_start = (int*)carve(sp, 4 * (size_t)(hcap + 1));
     int* s_hist = (int*)carve(sp, 4 * (size_t)max(NW * min(hcap, hits_fast), hcap));
 
@@ -111,30 +108,30 @@ __global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_be
         for (int w = 0; w < nwe; ++w) { const int v = s_hist[w * H + k]; s_hist[w * H + k] = run; run += v; }
     }
     __syncthreads();
+    // placement straight into the node lists (scattered 4- and 2-byte stores inside the cell's 19 KB; L2 merges them)
+    unsigned* g_key = nl.key + (size_t)blockIdx.x * L.nnode;
+    unsigned short* g_rkpos = nl.rkpos + (size_t)blockIdx.x * L.nnode;
     for (int m0 = nb; m0 < ne; m0 += 32) {
         const int m = m0 + lane;
         const int key = (m < ne) ? (int)s_rk[m] : 0xffff;
         const unsigned same = __match_any_sync(0xffffffffu, key);
         if (key != 0xffff) {
             const int pos = s_hist[warp * H + key] + __popc(same & ((1u << lane) - 1u));
-            s_sorted[pos] = (unsigned short)m;
-            s_rkpos[pos] = (unsigned short)key;
-            s_tcpos[pos] = s_tgt[m];
+            g_key[pos] = ((unsigned)s_tgt[m] << 14) | (unsigned)m;
+            g_rkpos[pos] = (unsigned short)key;
         }
         __syncwarp();
         if (key != 0xffff && lane == (__ffs(same) - 1)) s_hist[warp * H + key] += __popc(same);
         __syncwarp();
     }
     __syncthreads();
-    unsigned* g_key = nl.key + (size_t)blockIdx.x * L.nnode;
-    unsigned short* g_rkpos = nl.rkpos + (size_t)blockIdx.x * L.nnode;
-    for (int k = tid; k < ntot; k += T) { g_key[k] = ((unsigned)s_tcpos[k] << 14) | s_sorted[k]; g_rkpos[k] = s_rkpos[k]; }
-    // (target, x-node) segments of the sorted list: the fill pass applies the bra harmonics once per segment
+    // (target, x-node) segments of the sorted list (statistics for the work model): read back what this CTA just wrote
     int seg = 0;
     for (int k = tid; k < ntot; k += T) {
-        const int ck = L.mg_npq ? (int)__umulhi((unsigned)s_sorted[k], L.mg_npq) : (int)s_sorted[k];
-        const int cp = k ? (L.mg_npq ? (int)__umulhi((unsigned)s_sorted[k - 1], L.mg_npq) : (int)s_sorted[k - 1]) : -1;
-        seg += (k == 0 || s_rkpos[k] != s_rkpos[k - 1] || ck != cp) ? 1 : 0;
+        const unsigned kk = g_key[k], kp = k ? g_key[k - 1] : 0u;
+        const int mk = (int)(kk & 16383u), mp = (int)(kp & 16383u);
+        const int ck = L.mg_npq ? (int)__umulhi((unsigned)mk, L.mg_npq) : mk, cp = L.mg_npq ? (int)__umulhi((unsigned)mp, L.mg_npq) : mp;
+        seg += (k == 0 || (kk >> 14) != (kp >> 14) || ck != cp) ? 1 : 0;
     }
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) seg += __shfl_xor_sync(0xffffffffu, seg, d);
