@@ -257,34 +257,47 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 }
             }
             __syncwarp();
-            // lane = slot pair: walks the tile's nodes, up to 8 per step, stopping at every segment end (and at the tile end)
+            // lane = slot pair: walks the tile's nodes, up to 16 per step, stopping at every segment end (and at the tile end)
             const unsigned stops = smask | (1u << (cnt - 1));
             for (int j = 0; j < cnt;) {
-                const int n = min(__ffs(stops >> j), 8);                 // nodes up to and including the next stop, at most 8
+                const int n = min(__ffs(stops >> j), 16);                // nodes up to and including the next stop, at most 16
 #pragma unroll
                 for (int i = 0; i < NPC; ++i) {
                     const int sp = i * 32 + lane;
                     if (sp < np) {
                         const double2* row = s_tile + sp * kTileStride + j;
-                        if (n == 8) {
-                            const double2 d0 = row[0], d1 = row[1], d2 = row[2], d3 = row[3], d4 = row[4], d5 = row[5], d6 = row[6], d7 = row[7];
-                            runS[i].x += ((d0.x + d1.x) + (d2.x + d3.x)) + ((d4.x + d5.x) + (d6.x + d7.x));
-                            runS[i].y += ((d0.y + d1.y) + (d2.y + d3.y)) + ((d4.y + d5.y) + (d6.y + d7.y));
+                        double2 r = runS[i];
+                        if (n & 16) {
+                            double2 d[16];
+#pragma unroll
+                            for (int k = 0; k < 16; ++k) d[k] = row[k];
+#pragma unroll
+                            for (int w = 8; w > 0; w >>= 1)
+#pragma unroll
+                                for (int k = 0; k < w; ++k) { d[k].x += d[k + w].x; d[k].y += d[k + w].y; }
+                            r.x += d[0].x; r.y += d[0].y;
                         } else {
+                            if (n & 8) {
+                                const double2 d0 = row[0], d1 = row[1], d2 = row[2], d3 = row[3], d4 = row[4], d5 = row[5], d6 = row[6], d7 = row[7];
+                                r.x += ((d0.x + d1.x) + (d2.x + d3.x)) + ((d4.x + d5.x) + (d6.x + d7.x));
+                                r.y += ((d0.y + d1.y) + (d2.y + d3.y)) + ((d4.y + d5.y) + (d6.y + d7.y));
+                                row += 8;
+                            }
                             if (n & 4) {
                                 const double2 d0 = row[0], d1 = row[1], d2 = row[2], d3 = row[3];
-                                runS[i].x += (d0.x + d1.x) + (d2.x + d3.x);
-                                runS[i].y += (d0.y + d1.y) + (d2.y + d3.y);
+                                r.x += (d0.x + d1.x) + (d2.x + d3.x);
+                                r.y += (d0.y + d1.y) + (d2.y + d3.y);
                                 row += 4;
                             }
                             if (n & 2) {
                                 const double2 d0 = row[0], d1 = row[1];
-                                runS[i].x += d0.x + d1.x;
-                                runS[i].y += d0.y + d1.y;
+                                r.x += d0.x + d1.x;
+                                r.y += d0.y + d1.y;
                                 row += 2;
                             }
-                            if (n & 1) { const double2 d = row[0]; runS[i].x += d.x; runS[i].y += d.y; }
+                            if (n & 1) { const double2 d = row[0]; r.x += d.x; r.y += d.y; }
                         }
+                        runS[i] = r;
                     }
                 }
                 j += n;
