@@ -29,8 +29,8 @@ UNIT = "nnz/s"
 # FP64 ALU peak used for the roofline: SMs x 64 DFMA lanes x 2 flop x max SM clock
 FP64_LANES_PER_SM = 64
 # dram__bytes_read.sum + dram__bytes_write.sum of one fill launch from the committed `ncu --set full` capture
-# (profiles/r1_fill.md), per workload; None where no capture exists.
-FILL_DRAM_TRAFFIC = {"cfg4_3N_Jhalf+_jle3_26ch_150x150": 7.097e9 + 0.449e9}
+# (profiles/r1_final_fill.md), per workload; None where no capture exists.
+FILL_DRAM_TRAFFIC = {"cfg4_3N_Jhalf+_jle3_26ch_150x150": 10.777e9 + 0.443e9}
 
 
 def _peaks():
