@@ -176,6 +176,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
             int hcl[kRowBatch];
 #pragma unroll
             for (int bb = 0; bb < kRowBatch; ++bb) { nrm[bb] = s_norm[bb]; hcl[bb] = kCols ? s_hcol[bb] : 0; }
+#pragma unroll 2
             for (int o = lane; o < L.totcoup; o += 32) {
                 const int od = s_odesc[o], fi = s_ofi[o];
                 const int clo = od & 4095, nc = (od >> 12) & 127, mm = (od >> 19) & 63, ap = (unsigned)od >> 25;
