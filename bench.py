@@ -227,6 +227,24 @@ def main():
             "flops_per_launch": flops, "work": work, "fill_ms": fill_avg * 1e3,
             "csr_write_gbs": 12.0 * nnz / fill_avg * 1e-9, "hbm_peak_gbs": pk["hbm_gbs"]}
 
+    # ---- the SpMV check (row a9): y = P0 x on the matrix just built; HBM bound, 12 B per nonzero
+    xv = torch.rand(wl.M, dtype=torch.float64, device="cuda")
+    yv = torch.empty(wl.M, dtype=torch.float64, device="cuda")
+    spmv_ms = []
+    for it in range(6):
+        flush.zero_()
+        s0, s1 = (torch.cuda.Event(enable_timing=True) for _ in range(2))
+        s0.record(st)
+        api.pm_spmv(lat.h, rowptr, colidx, vals, xv, yv)
+        s1.record(st)
+        torch.cuda.synchronize()
+        if it:
+            spmv_ms.append(s0.elapsed_time(s1))
+    spmv_gbs = 12.0 * nnz / (min(spmv_ms) * 1e-3) * 1e-9
+    spmv = {"ms": min(spmv_ms), "bound": "hbm", "achieved": spmv_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
+            "frac": spmv_gbs / pk["hbm_gbs"]}
+    del xv, yv
+
     # ---- end to end through the C ABI with HOST buffers (D2H copies inside the timed region)
     e2e = None
     if not args.no_e2e:
@@ -271,7 +289,7 @@ def main():
                             "pattern_median": float(np.median(np.array(step_ms) - np.array(fill_ms))),
                             "fill_median": float(np.median(fill_ms)), "fill_best": float(np.min(fill_ms)),
                             "fill_all": [round(float(x), 3) for x in fill_ms]},
-               "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
+               "roofline": roof, "spmv": spmv, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
                "clocks": clocks.summary()}
         print(json.dumps(out))
     lat.close()
