@@ -168,6 +168,14 @@ def main():
 
     rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    # explicit build step (no-op when libpm.so is newer than its sources); local rank 0 builds, the others wait for it
+    from paper_1508_07441_b200.csrc import build as lib_build
+    if local == 0:
+        lib_build.build()
+    else:
+        t_wait = time.time()
+        while lib_build.stale() and time.time() - t_wait < 600:
+            time.sleep(1.0)
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))

@@ -12,6 +12,14 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
 
 
+@pytest.fixture(scope="session", autouse=True)
+def _libpm_built():
+    """Build libpm.so (and the generated kernels) if it is missing or older than its sources: an explicit build step,
+    not a fallback — the library itself still refuses to run without its CUDA extension."""
+    from paper_1508_07441_b200.csrc import build
+    build.build()
+
+
 @pytest.fixture(scope="session")
 def oracle():
     from oracle.pm_oracle import Oracle
