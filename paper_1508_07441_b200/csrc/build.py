@@ -63,8 +63,14 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         generate(verbose)
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", LIB, *[os.path.join(HERE, s) for s in SOURCES]]
-        subprocess.check_call(cmd)
+        tmp = LIB + f".{os.getpid()}.tmp"                 # link beside the target, then rename: readers never see a partial file
+        cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", tmp, *[os.path.join(HERE, s) for s in SOURCES]]
+        try:
+            subprocess.check_call(cmd)
+            os.replace(tmp, LIB)
+        finally:
+            if os.path.exists(tmp):
+                os.remove(tmp)
     return LIB
 
 
