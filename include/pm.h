@@ -134,9 +134,21 @@ int32_t pm_lattice_work(const pm_lattice* lat, double* flop_per_node, double* fl
 int32_t pm_pattern_counts(const pm_lattice* lat, int64_t* nodes_on_grid, int64_t* segments, int64_t* hit_cells);
 
 /* Name of the fill kernel this lattice's channel set selects: "Spec_<set>" when csrc/build.py generated straight-line
- * ket code for it (the channel sets of BASELINE.json's configs), "generic" for the table-driven kernel every other
- * channel set uses.  Host only; library-owned string, never NULL. */
+ * ket code for it at build time (the channel sets of BASELINE.json's configs); "jit" when the same kind of code is
+ * generated from the lattice's tables and compiled with NVRTC at the first fill (any other channel set; needs
+ * libnvrtc and the CUDA driver at run time, about a second once per channel set and process); "generic" for the
+ * table-driven kernel used when run-time compilation is switched off or failed.  All three give the same results
+ * within the value tolerance and the same pattern.  Host only; library-owned string, never NULL. */
 const char* pm_lattice_fill_kernel(const pm_lattice* lat);
+
+/* Switches run-time compilation on (default, unless the environment variable PM_NO_JIT is set) or off for lattices
+ * that have not run a fill yet. */
+int32_t pm_set_jit(int32_t enabled);
+
+/* Diagnostic (host only, no GPU needed): generates this lattice's run-time kernel source and compiles it with NVRTC
+ * for sm_100a; *cubin_bytes receives the size of the binary.  PM_ERR_STATE with the compiler log as message on failure
+ * (also when libnvrtc cannot be loaded). */
+int32_t pm_diag_jit_compile(const pm_lattice* lat, int64_t* cubin_bytes);
 
 /* Diagnostic (host only): the smallest double y with sqrt(y) >= edge under IEEE round-to-nearest — the threshold
  * the kernels compare p'^2 with instead of taking sqrt(p'^2) and comparing with the edge. */

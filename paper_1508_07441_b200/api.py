@@ -22,7 +22,7 @@ ERRORS = {-1: "PM_ERR_ARG", -2: "PM_ERR_GRID", -3: "PM_ERR_CHANNEL", -4: "PM_ERR
           -6: "PM_ERR_NOMEM", -7: "PM_ERR_STATE", -8: "PM_ERR_OVERFLOW", -9: "PM_ERR_DEVICE"}
 
 EXPORTS = ["pm_lattice_create", "pm_lattice_destroy", "pm_lattice_dims", "pm_lattice_rule", "pm_lattice_set_rule",
-           "pm_lattice_coupling", "pm_lattice_work", "pm_pattern_counts", "pm_lattice_fill_kernel", "pm_diag_sqrt_threshold",
+           "pm_lattice_coupling", "pm_lattice_work", "pm_pattern_counts", "pm_lattice_fill_kernel", "pm_set_jit", "pm_diag_jit_compile", "pm_diag_sqrt_threshold",
            "pm_diag_dfma_tflops", "pm_pattern", "pm_fill", "pm_build", "pm_last_fill_ms", "pm_spmv", "pm_build_host_count", "pm_build_host",
            "pm_launch_count", "pm_last_error"]
 
@@ -62,6 +62,8 @@ def lib():
     L.pm_lattice_work.argtypes = [_vp, _dp, _dp, _dp, _i32p]
     L.pm_pattern_counts.argtypes = [_vp, _i64p, _i64p, _i64p]
     L.pm_diag_dfma_tflops.argtypes = [_dp, _vp]
+    L.pm_set_jit.argtypes = [C.c_int32]
+    L.pm_diag_jit_compile.argtypes = [_vp, _i64p]
     L.pm_lattice_fill_kernel.argtypes = [_vp]
     L.pm_lattice_fill_kernel.restype = C.c_char_p
     L.pm_diag_sqrt_threshold.argtypes = [C.c_double]
@@ -153,6 +155,17 @@ def pm_pattern_counts(h):
 
 def pm_lattice_fill_kernel(h):
     return lib().pm_lattice_fill_kernel(h).decode()
+
+
+def pm_set_jit(enabled):
+    _check(lib().pm_set_jit(1 if enabled else 0))
+
+
+def pm_diag_jit_compile(h):
+    """Compiles the lattice's run-time kernel with NVRTC (no GPU needed); returns the cubin size in bytes."""
+    n = C.c_int64()
+    _check(lib().pm_diag_jit_compile(h, C.byref(n)))
+    return n.value
 
 
 def pm_diag_sqrt_threshold(edge):

@@ -12,6 +12,7 @@
 #include <cuda_runtime.h>
 
 #include "../../include/pm.h"
+#include "pm_jit.hpp"
 #include "pm_kernels.cuh"
 #include "pm_tables.hpp"
 
@@ -49,6 +50,8 @@ struct pm_lattice {
     bool pat_count_only = false;       // the last pattern call only counted: an emit call for the same range reuses its lists
     int64_t counts[3] = {0, 0, 0};     // nodes on the grid, (target, x-node) segments, hit cells of the last pattern call
     bool have_plan = false;
+    bool jit_failed = false;           // run-time compilation was tried for this lattice and failed (jit_error says why)
+    std::string jit_error;
     pm::FillLaunch plan{};
     int* d_counter = nullptr;          // work counter of the fill kernel
     cudaEvent_t ev_fill0 = nullptr, ev_fill1 = nullptr;   // around the last fill kernel, on its stream (pm_last_fill_ms)
@@ -329,7 +332,26 @@ int32_t pm_pattern_counts(const pm_lattice* lat, int64_t* nodes_on_grid, int64_t
 
 const char* pm_lattice_fill_kernel(const pm_lattice* lat)
 {
-    return lat ? pm::fill_variant_name(lat->hash) : "";
+    if (!lat) return "";
+    if (pm::fill_has_spec(lat->hash)) return pm::fill_variant_name(lat->hash);
+    if (lat->have_plan) return lat->plan.name;                              // what the last fill ran: "jit" or "generic"
+    return (pm::jit_enabled() && !lat->jit_failed) ? "jit" : "generic";
+}
+
+int32_t pm_set_jit(int32_t enabled)
+{
+    pm::jit_set_enabled(enabled != 0);
+    return PM_OK;
+}
+
+int32_t pm_diag_jit_compile(const pm_lattice* lat, int64_t* cubin_bytes)
+{
+    if (!lat) return fail(PM_ERR_ARG, "lat is NULL");
+    std::string err;
+    size_t n = 0;
+    if (!pm::jit_compile_check(lat->T, 12, 4, &n, err)) return fail(PM_ERR_STATE, err);
+    if (cubin_bytes) *cubin_bytes = (int64_t)n;
+    return PM_OK;
 }
 
 double pm_diag_sqrt_threshold(double edge) { return pm::sqrt_threshold(edge); }
@@ -405,6 +427,11 @@ int32_t fill_block(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const 
     if (cell_begin == cell_end) return PM_OK;
     const int n_blk = cell_end - cell_begin;
     cudaError_t e;
+    if (!lat->have_plan && !pm::fill_has_spec(lat->hash) && pm::jit_enabled() && !lat->jit_failed) {
+        // no build-time kernel for this channel set: specialise at run time (pm_jit.hpp), else fall back below
+        if (pm::fill_plan_jit(lat->dev, lat->T, lat->hash, lat->n_sm, &lat->plan, lat->jit_error)) lat->have_plan = true;
+        else lat->jit_failed = true;
+    }
     if (!lat->have_plan) {
         e = pm::fill_plan(lat->dev, lat->hash, lat->n_sm, &lat->plan);
         if (e == cudaErrorInvalidConfiguration) { cudaGetLastError(); return fail(PM_ERR_NOMEM, "channel set needs more shared memory than one SM has"); }

@@ -7,8 +7,22 @@
 // compares it with the edges; here p'^2 is compared with sqrt_threshold(edge) (pm_tables.hpp), the smallest
 // double whose correctly rounded square root reaches the edge — the same decision without the square root.
 #pragma once
+#ifdef __CUDACC_RTC__                  // compiled at run time by NVRTC (pm_jit.cpp): no host headers there
+typedef int int32_t;
+typedef unsigned int uint32_t;
+typedef long long int64_t;
+typedef unsigned long long uint64_t;
+typedef unsigned long size_t;
+namespace std {
+template <bool B> struct pm_bool_constant { static constexpr bool value = B; };
+typedef pm_bool_constant<true> true_type;
+typedef pm_bool_constant<false> false_type;
+}
+#else
 #include <cstdint>
+#include <type_traits>
 #include <cuda_runtime.h>
+#endif
 
 namespace pm {
 

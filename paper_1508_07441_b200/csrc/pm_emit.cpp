@@ -1,0 +1,93 @@
+// pm_emit.cpp — emits the channel-specialised ket code of the fill kernel as CUDA source text (see pm_emit.hpp).
+#include "pm_emit.hpp"
+
+#include <cinttypes>
+#include <cstdio>
+#include <map>
+#include <sstream>
+
+namespace pm {
+
+namespace {
+
+std::string num(double v)
+{
+    char buf[64];
+    std::snprintf(buf, sizeof buf, "%.17g", v);
+    std::string s(buf);
+    if (s.find_first_of(".eEn") == std::string::npos) s += ".0";
+    return s;
+}
+
+std::string yname(char side, int idx)
+{
+    int l = 0;
+    while (ylm_index(l + 1, 0) <= idx) ++l;
+    return std::string(1, side) + std::to_string(l) + "_" + std::to_string(idx - ylm_index(l, 0));
+}
+
+// scaled harmonics Q_lm of one direction, seed `seed` (omega for the p' side, 1 for the q' side)
+void emit_q(std::ostringstream& o, char side, int lmax, const std::string& seed, const std::string& ux, const std::string& uz,
+            const std::vector<double>& beta)
+{
+    o << "        const double " << yname(side, 0) << " = " << seed << ";\n";
+    for (int m = 0; m <= lmax; ++m) {
+        if (m > 0)
+            o << "        const double " << yname(side, ylm_index(m, m)) << " = " << ux << " * " << yname(side, ylm_index(m - 1, m - 1)) << ";\n";
+        for (int l = m + 1; l <= lmax; ++l) {
+            o << "        const double " << yname(side, ylm_index(l, m)) << " = ";
+            if (l == m + 1) o << uz << " * " << yname(side, ylm_index(l - 1, m)) << ";\n";
+            else o << "fma(" << uz << ", " << yname(side, ylm_index(l - 1, m)) << ", " << num(-beta[(size_t)ylm_index(l, m)]) << " * "
+                   << yname(side, ylm_index(l - 2, m)) << ");\n";
+        }
+    }
+}
+
+}  // namespace
+
+std::string emit_spec(const std::string& name, const Tables& T, EmitStats& st)
+{
+    std::vector<double> ynorm, ybeta;
+    scaled_harmonics(T.lmax, ynorm, ybeta);
+    int la = 0, lb = 0;
+    for (const Triple& t : T.tri) { la = std::max(la, t.l); lb = std::max(lb, t.lam); }
+    std::ostringstream o;
+    const int nf = (int)T.fun.size();
+    o << "struct Spec_" << name << " {\n";
+    o << "    static constexpr bool kStatic = true;\n";
+    int maxm = 1, maxl1 = 1;                        // most M-terms of a function; number of L values (terms per output)
+    for (const OrbFun& f : T.fun) { maxm = std::max(maxm, f.nM); maxl1 = std::max(maxl1, f.L + 1); }
+    o << "    static constexpr int NS = " << T.n_slot << ", NF = " << nf << ", NCH = " << (nf + 31) / 32 << ", MAXM = " << maxm << ", MAXL1 = " << maxl1 << ";\n";
+    char hb[32]; std::snprintf(hb, sizeof hb, "0x%016" PRIx64 "ull", tables_hash(T));
+    o << "    static constexpr unsigned long long kHash = " << hb << ";\n";
+    o << "    // K[s] = omega * (ket bipolar harmonic of slot s) at directions a = p'^ = (uxa,0,uza), b = q'^ = (uxb,0,uzb)\n";
+    o << "    static __device__ __forceinline__ void ket(const DevLattice&, double om, double uxa, double uza, double uxb, double uzb,\n"
+         "                                               double (&K)[NS])\n    {\n";
+    emit_q(o, 'a', la, "om", "uxa", "uza", ybeta);
+    emit_q(o, 'b', lb, "1.0", "uxb", "uzb", ybeta);
+    // products shared by several terms
+    std::map<std::pair<int, int>, int> uses;
+    for (size_t t = 0; t < T.kt_c.size(); ++t) uses[{T.kt_ip[t], T.kt_iq[t]}]++;
+    for (auto& kv : uses) {
+        o << "        const double t" << kv.first.first << "_" << kv.first.second << " = " << yname('a', kv.first.first) << " * "
+          << yname('b', kv.first.second) << ";\n";
+        st.n_prod++;
+    }
+    for (int s = 0; s < T.n_slot; ++s) {
+        const int b = T.kt_off[(size_t)s], e = T.kt_off[(size_t)s + 1];
+        if (b == e) { o << "        K[" << s << "] = 0.0;\n"; continue; }
+        std::string expr;
+        for (int t = b; t < e; ++t) {
+            const double c = T.kt_c[(size_t)t] * ynorm[(size_t)T.kt_ip[(size_t)t]] * ynorm[(size_t)T.kt_iq[(size_t)t]];
+            const std::string p = "t" + std::to_string(T.kt_ip[(size_t)t]) + "_" + std::to_string(T.kt_iq[(size_t)t]);
+            if (t == b) { expr = num(c) + " * " + p; st.n_mul++; }
+            else { expr = "fma(" + num(c) + ", " + p + ", " + expr + ")"; st.n_fma++; }
+        }
+        o << "        K[" << s << "] = " << expr << ";\n";
+    }
+    o << "    }\n};\n\n";
+    return o.str();
+}
+
+
+}  // namespace pm

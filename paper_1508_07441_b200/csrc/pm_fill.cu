@@ -5,6 +5,7 @@
 #include <cstdlib>
 
 #include "gen/pm_spec_gen.cuh"
+#include "pm_jit.hpp"
 #include "pm_kernels.cuh"
 
 namespace pm {
@@ -66,6 +67,7 @@ cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int n_sm, Fi
     out->fn_cols = (const void*)best->fn_cols;
     out->nw = best->nw;
     out->name = best->name;
+    out->jit = false;
     out->smem = fill_smem_plan(L, best->nw, best->rb);
     cudaError_t e = cudaFuncSetAttribute(out->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, out->smem.total);
     if (e != cudaSuccess) return e;
@@ -75,6 +77,23 @@ cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int n_sm, Fi
     if (e != cudaSuccess) return e;
     out->grid = n_sm * (per_sm > 0 ? per_sm : 1);
     return cudaSuccess;
+}
+
+bool fill_plan_jit(const DevLattice& L, const Tables& T, unsigned long long hash, int n_sm, FillLaunch* out, std::string& err)
+{
+    const int rb = 4;
+    int nw = 0;
+    for (int w : {preferred_warps(), 12, 8, 4})
+        if (w >= 1 && w <= 32 && fill_smem_plan(L, w, rb).total <= kSmemLimit) { nw = w; break; }
+    if (!nw) { err = "no warp count fits in shared memory"; return false; }
+    JitFill k;
+    if (!jit_fill(T, hash, nw, rb, &k, err)) return false;
+    out->fn = k.fn; out->fn_cols = k.fn_cols; out->nw = nw; out->name = "jit"; out->jit = true;
+    out->smem = fill_smem_plan(L, nw, rb);
+    const int per_sm = jit_prepare(k, false, out->smem.total), per_sm_c = jit_prepare(k, true, out->smem.total);
+    if (per_sm < 1 || per_sm_c < 1) { err = "the compiled kernel does not fit on an SM"; return false; }
+    out->grid = n_sm * (per_sm < per_sm_c ? per_sm : per_sm_c);
+    return true;
 }
 
 cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl,
@@ -88,6 +107,11 @@ cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin
     cudaError_t e = cudaMemsetAsync(counter, 0, sizeof(int), st);      // the work counter the warps draw cells from
     if (e != cudaSuccess) return e;
     void* args[] = {&Lc, &S, &N, &cell_begin, &n_blk, (void*)&rowptr, &vals, &colidx, &counter};
+    if (F.jit) {
+        const int cr = jit_launch(const_cast<void*>(colidx ? F.fn_cols : F.fn), grid, F.nw * 32, S.total, (void*)st, args);
+        count_launch();
+        return cr == 0 ? cudaGetLastError() : cudaErrorLaunchFailure;
+    }
     e = cudaLaunchKernel(colidx ? F.fn_cols : F.fn, dim3((unsigned)grid), dim3((unsigned)(F.nw * 32)), args, (size_t)S.total, st);
     count_launch();
     return e != cudaSuccess ? e : cudaGetLastError();

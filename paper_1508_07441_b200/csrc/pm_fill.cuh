@@ -15,10 +15,6 @@
 // Prior art this replaces: one thread per element / per cell pair, constants in global memory, CPU repack
 // (PAPER.md:L341, L348-356, L376).
 #pragma once
-#include <cstdint>
-#include <type_traits>
-#include <cuda_runtime.h>
-
 #include "pm_device.cuh"
 #include "pm_ylm.h"
 

@@ -1,0 +1,41 @@
+// pm_jit.hpp — run-time specialisation of the fill kernel for channel sets that have no build-time kernel.
+//
+// csrc/build.py generates straight-line ket code only for the channel sets of BASELINE.json's configs.  Any other
+// channel set (another J^pi, another order) would run the table-driven `SpecGeneric` kernel, 8x slower.  Instead the
+// library emits the same kind of struct from the lattice's tables (pm_emit.cpp), compiles `k_fill_warp<Spec_jit, ...>`
+// with NVRTC for sm_100a from the very headers nvcc compiled (embedded as text in gen/pm_jit_src.inc) and launches it
+// through the driver API.  libnvrtc and libcuda are opened with dlopen on first use, so libpm.so loads on machines
+// without them; if either is missing or the compilation fails, pm_fill falls back to the table-driven kernel and
+// `pm_lattice_fill_kernel` says so.  Compiled kernels are cached per tables hash for the life of the process.
+#pragma once
+#include <cstddef>
+#include <string>
+
+#include "pm_tables.hpp"
+
+namespace pm {
+
+struct JitFill {
+    void* fn = nullptr;        // CUfunction of k_fill_warp<Spec_jit, nw, rb, false>
+    void* fn_cols = nullptr;   // ... <..., true>
+    int nw = 0, rb = 0;
+};
+
+// Enables / disables run-time compilation for lattices planned from now on (default: enabled unless PM_NO_JIT is set).
+void jit_set_enabled(bool on);
+bool jit_enabled();
+
+// Compiles (or fetches from the cache) the two kernel variants for tables T with `nw` warps and row batch `rb`.
+// Returns false and a message if NVRTC / the driver API is unavailable or the compilation fails.
+bool jit_fill(const Tables& T, unsigned long long hash, int nw, int rb, JitFill* out, std::string& err);
+
+// NVRTC only, no device needed: does the kernel for tables T compile for sm_100a?  (diagnostic, CPU tests)
+bool jit_compile_check(const Tables& T, int nw, int rb, size_t* cubin_bytes, std::string& err);
+
+// cuFuncSetAttribute(max dynamic shared memory) + occupancy; returns CTAs per SM (0 on error)
+int jit_prepare(const JitFill& k, bool cols, int smem_bytes);
+
+// cuLaunchKernel on `stream` (a cudaStream_t); returns 0 on success, else a CUresult value
+int jit_launch(void* fn, int grid, int block, int smem_bytes, void* stream, void** args);
+
+}  // namespace pm

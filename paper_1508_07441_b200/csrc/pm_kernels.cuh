@@ -4,9 +4,11 @@
 #include <atomic>
 #include <cstddef>
 #include <cstdint>
+#include <string>
 
 #include "pm_device.cuh"
 #include "pm_fill.cuh"
+#include "pm_tables.hpp"
 
 namespace pm {
 
@@ -25,10 +27,13 @@ cudaError_t launch_emit_cols(const DevLattice& L, int n_blk, const NodeLists& nl
                              int32_t* colidx, cudaStream_t st);
 
 // fill pass (pm_fill.cuh): variant selection and launch
-struct FillLaunch { const void *fn, *fn_cols; int nw, grid; FillSmem smem; const char* name; };   // fn_cols also writes colidx
+struct FillLaunch { const void *fn, *fn_cols; int nw, grid; FillSmem smem; const char* name; bool jit; };   // fn_cols also writes colidx;
+                                                      // jit: fn / fn_cols are CUfunction handles of run-time compiled kernels (pm_jit.hpp)
 bool fill_has_spec(unsigned long long tables_hash);
 const char* fill_variant_name(unsigned long long tables_hash);
 cudaError_t fill_plan(const DevLattice& L, unsigned long long tables_hash, int n_sm, FillLaunch* out);
+// run-time compiled kernel for tables T (no build-time kernel): false + message when NVRTC / the driver API fails
+bool fill_plan_jit(const DevLattice& L, const Tables& T, unsigned long long tables_hash, int n_sm, FillLaunch* out, std::string& err);
 cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl,
                         const int64_t* rowptr, double* vals, int32_t* colidx, int* counter, cudaStream_t st);
 

@@ -82,17 +82,30 @@ def test_bitwise_reproducible(api):
     assert all(np.array_equal(x, y) for x, y in zip(a, b))
 
 
-def test_generic_kernel_parity_on_reordered_channels(api, oracle):
-    """A channel order with no generated kernel runs the table-driven fill; same bar."""
+@pytest.mark.parametrize("jit", [True, False], ids=["jit", "generic"])
+def test_kernels_for_channel_sets_without_a_build_time_kernel(api, oracle, jit):
+    """A channel order with no build-time kernel is specialised at run time (NVRTC) or, with that switched off, runs
+    the table-driven fill; same bar for both, and both are what pm_lattice_fill_kernel reports."""
     wl = I.small_coupled(N=6, jmax=2, orders=(3, 4, 6))
     wl.channels = wl.channels[::-1].copy()
-    lat = api.Lattice(wl)
-    assert api.pm_lattice_fill_kernel(lat.h) == "generic"
-    rp, ci, v = lat.build()
+    api.pm_set_jit(jit)
+    try:
+        lat = api.Lattice(wl)
+        rp, ci, v = lat.build()
+        assert api.pm_lattice_fill_kernel(lat.h) == ("jit" if jit else "generic")
+        rp2, ci2, v2 = lat.build_fused()
+        assert torch_equal(rp, rp2) and torch_equal(ci, ci2) and torch_equal(v, v2)
+    finally:
+        api.pm_set_jit(True)
     rpo, cio, vo = oracle.build_csr(wl)
     assert np.array_equal(rp.cpu().numpy(), rpo) and np.array_equal(ci.cpu().numpy(), cio)
     _assert_values(v.cpu().numpy(), vo)
     lat.close()
+
+
+def torch_equal(a, b):
+    import torch
+    return torch.equal(a, b)
 
 
 @pytest.mark.parametrize("wl", [I.config(1), I.small_coupled(N=7, jmax=3, orders=(4, 5, 7))], ids=lambda w: w.name)

@@ -141,8 +141,37 @@ def test_fill_kernel_selection_and_work_model():
     assert work[4][0] > work[2][0] > work[1][0] and work[4][3] == 580 and work[2][3] == 276
     wl = I.config(2)
     h = _create(wl, channels=wl.channels[::-1].copy())
-    assert api.pm_lattice_fill_kernel(h) == "generic"
+    assert api.pm_lattice_fill_kernel(h) == "jit"             # specialised at run time (NVRTC) at the first fill
+    api.pm_set_jit(False)
+    try:
+        assert api.pm_lattice_fill_kernel(h) == "generic"     # table-driven kernel when run-time compilation is off
+    finally:
+        api.pm_set_jit(True)
     api.pm_lattice_destroy(h)
+
+
+def test_runtime_kernel_source_compiles_for_sm100a():
+    """The source generated at run time for channel sets without a build-time kernel compiles with NVRTC for sm_100a
+    (no GPU needed): J = 3/2-, a reordered 18-channel set, bosons with d-waves."""
+    g7 = I.tan_grid(7, 1.0)
+    cases = [
+        I.Workload("3N_J3half-", g7, 0.9 * g7, I.enumerate_3n_channels(3, -1, 1, 1), 3, -1, 1, 0, 3, 4, 8),
+        I.Workload("boson_dwave", g7, g7, np.concatenate([I.boson_channel(0, 0), I.boson_channel(2, 2)]), 0, +1, 0,
+                   I.PM_SPINLESS_BOSON, 5, 5, 9),
+    ]
+    wl = I.config(2)
+    wl.channels = wl.channels[::-1].copy()
+    cases.append(wl)
+    for wl in cases:
+        h = _create(wl)
+        try:
+            n = api.pm_diag_jit_compile(h)
+        except api.PmError as e:
+            if "libnvrtc not found" in str(e):
+                pytest.skip("libnvrtc is not installed here")
+            raise
+        assert n > 10000
+        api.pm_lattice_destroy(h)
 
 
 def test_sqrt_threshold_is_the_exact_boundary():
