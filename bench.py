@@ -220,7 +220,7 @@ def main():
     total_ms = max_over_ranks(sum(step_ms), world)
     value = job_throughput(nnz, args.steps, total_ms, world)
 
-    # ---- roofline of the dominant kernel (fill): FP64 ALU bound
+    # ---- roofline of the dominant kernel (the fill): both roofs, the binding one first
     pk = _peaks()
     n_sm = torch.cuda.get_device_properties(local).multi_processor_count
     peak_tf = n_sm * FP64_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 * 1e-12
@@ -228,12 +228,20 @@ def main():
     fill_avg = float(np.mean(fill_ms)) * 1e-3
     achieved_tf = flops / fill_avg * 1e-12
     dfma = api.pm_diag_dfma_tflops()
-    roof = {"bound": "alu", "kernel": "k_fill_warp (values + column indices)", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
-            "frac": achieved_tf / peak_tf, "traffic": FILL_DRAM_TRAFFIC.get(wl.name),
-            "peak_source": f"{n_sm} SM x {FP64_LANES_PER_SM} DFMA lanes x 2 x {pk['sm_max_mhz']:.0f} MHz ({pk['src']} clock); "
-                           f"DFMA microbenchmark on this box: {dfma:.1f} TFLOP/s",
-            "flops_per_launch": flops, "work": work, "fill_ms": fill_avg * 1e3,
-            "csr_write_gbs": 12.0 * nnz / fill_avg * 1e-9, "hbm_peak_gbs": pk["hbm_gbs"]}
+    # algorithmic bytes of one launch: 8 B value + 4 B column index per nonzero written once, 4 B key per node on the grid read once
+    alg_bytes = 12.0 * nnz + 4.0 * work["nodes_on_grid"]
+    achieved_gbs = alg_bytes / fill_avg * 1e-9
+    t_alu, t_hbm = flops / (peak_tf * 1e12), alg_bytes / (pk["hbm_gbs"] * 1e9)
+    alu = {"achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
+           "peak_source": f"{n_sm} SM x {FP64_LANES_PER_SM} DFMA lanes x 2 x {pk['sm_max_mhz']:.0f} MHz ({pk['src']} clock); "
+                          f"DFMA microbenchmark on this box: {dfma:.1f} TFLOP/s"}
+    hbm = {"achieved": achieved_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": achieved_gbs / pk["hbm_gbs"],
+           "peak_source": f"copy bandwidth, MEASURED_PEAKS.json ({pk['src']})"}
+    bound = "hbm" if t_hbm >= t_alu else "alu"
+    roof = {"bound": bound, "kernel": "k_fill_warp (values + column indices)", **(hbm if bound == "hbm" else alu),
+            "traffic": FILL_DRAM_TRAFFIC.get(wl.name), "algorithmic_bytes": alg_bytes, "flops_per_launch": flops,
+            "flop_per_byte": flops / alg_bytes, "ridge_flop_per_byte": peak_tf * 1e3 / pk["hbm_gbs"],
+            "min_ms": {"alu": t_alu * 1e3, "hbm": t_hbm * 1e3}, "alu": alu, "hbm": hbm, "work": work, "fill_ms": fill_avg * 1e3}
 
     # ---- the SpMV check (row a9): y = P0 x on the matrix just built; HBM bound, 12 B per nonzero
     xv = torch.rand(wl.M, dtype=torch.float64, device="cuda")
