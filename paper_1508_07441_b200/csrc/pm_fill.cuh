@@ -87,7 +87,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
     constexpr int NCH = Spec::NCH;                      // function chunks of the lane = function stage
     extern __shared__ __align__(16) char smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int ns = Spec::kStatic ? Spec::NS : L.n_slot, nf = L.n_fun, np = (ns + 1) >> 1;
+    const int ns = Spec::kStatic ? Spec::NS : L.n_slot, nf = Spec::kStatic ? Spec::NF : L.n_fun, np = (ns + 1) >> 1;
 
     double* s_dp = (double*)(smem + S.dp);   double* s_dq = (double*)(smem + S.dq);
     double* s_tp = (double*)(smem + S.tp);   double* s_tq = (double*)(smem + S.tq);   double* s_tx = (double*)(smem + S.tx);
@@ -178,20 +178,22 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 const int clo = od & 4095, nc = (od >> 12) & 127, mm = (od >> 19) & 63, ap = (unsigned)od >> 25;
                 const double c0 = s_oc[3 * o], c1 = s_oc[3 * o + 1], c2 = s_oc[3 * o + 2];
                 const int f0 = fi & 255, f1 = (fi >> 8) & 255, f2 = (fi >> 16) & 255;
-                const size_t idx0 = (size_t)H * clo + (size_t)k0 * nc + mm;
-                double* out = row0 + idx0;
-                int32_t* outc = kCols ? col0 + idx0 : nullptr;
+                // entry of target k0+bb in row alpha: element H*clo + (k0+bb)*nc + m of the cell's block (fits 32 bits)
+                const unsigned idx0 = (unsigned)(H * clo + k0 * nc + mm);
+                const char* acc0 = (const char*)s_acc;
+                const unsigned a0 = 8u * f0, a1 = 8u * f1, a2 = 8u * f2;
 #pragma unroll
                 for (int bb = 0; bb < kRowBatch; ++bb) {
                     if (kFull || bb < nb) {
-                        const double* acc = s_acc + bb * nf;
-                        double v = fma(c2, acc[f2], fma(c1, acc[f1], c0 * acc[f0]));
+                        const char* acc = acc0 + bb * (8 * nf);
+                        double v = fma(c2, *(const double*)(acc + a2), fma(c1, *(const double*)(acc + a1), c0 * *(const double*)(acc + a0)));
                         if (Spec::MAXL1 > 3) {                           // more than three L values: the tail comes from the tables
                             const int t0 = L.ot_off[o], nt = fi >> 24;
-                            for (int t = 3; t < nt; ++t) v = fma(L.ot_c[t0 + t], acc[L.ot_f[t0 + t]], v);
+                            for (int t = 3; t < nt; ++t) v = fma(L.ot_c[t0 + t], ((const double*)acc)[L.ot_f[t0 + t]], v);
                         }
-                        out[bb * nc] = v * nrm[bb];
-                        if (kCols) outc[bb * nc] = hcl[bb] + ap;
+                        const unsigned e = idx0 + (unsigned)(bb * nc);
+                        row0[e] = v * nrm[bb];
+                        if (kCols) col0[e] = hcl[bb] + ap;
                     }
                 }
             }
