@@ -1,15 +1,25 @@
 """Input generators: channel counts the paper prints, grids, rules."""
+import os
+
 import numpy as np
 
 from paper_1508_07441_b200 import inputs as I
 
 
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
 def test_channel_counts_match_paper():
-    # PAPER.md:L378 "18-channel Faddeev equation ... J = 1/2+" ; L374 "up to 62 channels if ... j <= 3"
-    assert len(I.enumerate_3n_channels(1, +1, 1, 2)) == 18
+    """tests/golden/paper_channel_counts.txt holds the two channel counts the paper prints (with their citations)."""
+    rows = [ln.split() for ln in open(os.path.join(GOLDEN, "paper_channel_counts.txt")) if ln.strip() and not ln.startswith("#")]
+    assert len(rows) == 2
+    for J2, par, T2, jmax, n in (tuple(int(x) for x in r) for r in rows):
+        if J2 == 0:                                  # maximum over all J <= 17/2 and both parities
+            counts = [len(I.enumerate_3n_channels(j2, p, T2, jmax)) for j2 in range(1, 19, 2) for p in (+1, -1)]
+            assert max(counts) == n
+        else:
+            assert len(I.enumerate_3n_channels(J2, par, T2, jmax)) == n
     assert len(I.enumerate_3n_channels(1, +1, 1, 3)) == 26
-    counts = [len(I.enumerate_3n_channels(J2, par, 1, 3)) for J2 in range(1, 19, 2) for par in (+1, -1)]
-    assert max(counts) == 62
 
 
 def test_channels_obey_selection_rules():

@@ -209,3 +209,22 @@ def test_integral_three_ways_on_4x4(oracle):
     coarse = _csr(_boson(4, (12, 12, 24)), oracle).toarray()
     assert np.abs(A - V).max() < np.abs(coarse - V).max()
     assert np.array_equal(A != 0, V > 1e-9 * scale) or np.sum((A != 0) != (V > 1e-9 * scale)) <= 4
+
+
+def test_oracle_reproduces_its_stored_rows(oracle):
+    """Regression fixture written by tests/golden/make_cfg0_rows.py (oracle only): the oracle's arithmetic has not moved.
+    A deliberate change of the oracle regenerates the file and says why in its commit message."""
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg0_rows.txt")
+    stored = {}
+    for ln in open(path):
+        if ln.startswith("#"):
+            continue
+        c, col, hx, _ = ln.split()
+        stored.setdefault(int(c), []).append((int(col), float.fromhex(hx)))
+    wl = I.config(0)
+    for c, entries in stored.items():
+        rp, ci, v = oracle.build_csr(wl, c, c + 1)
+        assert ci.tolist() == [e[0] for e in entries]
+        ref = np.array([e[1] for e in entries])
+        assert np.max(np.abs(v - ref)) <= 1e-15 * np.max(np.abs(ref))
