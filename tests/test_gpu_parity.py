@@ -143,6 +143,29 @@ def test_single_warp_sort_path(oracle):
         _assert_values(r["v"], vo)
 
 
+def test_values_do_not_depend_on_the_block_shape(api):
+    """One warp owns one source cell and sums in sorted node order, so the bits of every value are the same whatever the
+    number of warps per block (PM_FILL_WARPS is read once per process: the 4-warp run is a subprocess)."""
+    import subprocess
+    import sys
+    import tempfile
+    wl = I.small_coupled(N=7, jmax=3, orders=(4, 5, 7))
+    lat = api.Lattice(wl)
+    rp, ci, v = (t.cpu().numpy() for t in lat.build_fused())
+    lat.close()
+    code = (
+        "import sys, numpy as np; sys.path.insert(0, %r)\n"
+        "from paper_1508_07441_b200 import api, inputs\n"
+        "wl = inputs.small_coupled(N=7, jmax=3, orders=(4, 5, 7)); lat = api.Lattice(wl); rp, ci, v = lat.build_fused()\n"
+        "np.savez(sys.argv[1], rp=rp.cpu().numpy(), ci=ci.cpu().numpy(), v=v.cpu().numpy())\n"
+    ) % ROOT
+    with tempfile.TemporaryDirectory() as d:
+        out = os.path.join(d, "r.npz")
+        subprocess.run([sys.executable, "-c", code, out], check=True, env=dict(os.environ, PM_FILL_WARPS="4"), timeout=600)
+        r = np.load(out)
+        assert np.array_equal(r["rp"], rp) and np.array_equal(r["ci"], ci) and np.array_equal(r["v"], v)
+
+
 def test_pattern_counts(api):
     wl = I.config(1)
     lat = api.Lattice(wl)
