@@ -109,6 +109,23 @@ int32_t pm_last_fill_ms(pm_lattice* lat, float* ms);
 int32_t pm_spmv(pm_lattice* lat, int64_t n_rows, const int64_t* d_rowptr, const int32_t* d_colidx,
                 const double* d_vals, const double* d_x, double* d_y, void* cuda_stream);
 
+/* ---- The iteration step that consumes P0 (eq. 24) -------------------
+ * K = O P0 V~1 G1 : G1 diagonal, P0 "highly sparse" (the CSR built above, whole lattice, global columns), O and
+ * V~1 = O^T V1 "block matrices with the block dimension (N x N)": one (Np x Np) block per channel alpha acting on
+ * the pair index i for fixed (j, alpha).  The paper keeps the four factors in memory and applies them one after the
+ * other (L239-241); its iterations are what remains its bottleneck after P0 moved to the GPU (L408-410).
+ *
+ * pm_block_apply : d_out[(i,j,a)] = sum_i' B_a[i][i'] * (d_diag ? d_diag[(i',j,a)] : 1) * d_in[(i',j,a)]
+ *   d_blocks : device, n_ch*Np*Np doubles, B_a row-major, a-major;  d_diag : device, M doubles, or NULL;
+ *   d_in, d_out : device, M doubles in the lattice's row order r = (i*Nq + j)*n_ch + a, distinct buffers.
+ * pm_kernel_apply : d_out = O (P0 (V~1 (G1 u))) — three launches; d_work : device scratch of 2*M doubles.
+ * Both are asynchronous on `cuda_stream`. */
+int32_t pm_block_apply(pm_lattice* lat, const double* d_blocks, const double* d_diag, const double* d_in, double* d_out,
+                       void* cuda_stream);
+int32_t pm_kernel_apply(pm_lattice* lat, const int64_t* d_rowptr, const int32_t* d_colidx, const double* d_vals,
+                        const double* d_O, const double* d_Vt, const double* d_g1, const double* d_u, double* d_out,
+                        double* d_work, void* cuda_stream);
+
 /* Whole build with HOST output buffers and row-block streaming: source-cell ranges are
  * chosen so that one block's CSR (12 B per nonzero) fits `device_budget_bytes` (0 = 3/4 of free device memory);
  * each block is built on the device and copied to the host arrays.

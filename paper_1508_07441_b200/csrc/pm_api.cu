@@ -460,6 +460,32 @@ int32_t pm_fill(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const int
     return fill_block(lat, cell_begin, cell_end, d_rowptr, d_vals, nullptr, (cudaStream_t)cuda_stream);
 }
 
+int32_t pm_block_apply(pm_lattice* lat, const double* d_blocks, const double* d_diag, const double* d_in, double* d_out, void* cuda_stream)
+{
+    if (!lat || !d_blocks || !d_in || !d_out) return fail(PM_ERR_ARG, "NULL argument");
+    if (d_in == d_out) return fail(PM_ERR_ARG, "pm_block_apply cannot work in place");
+    int32_t rc = ensure_device(lat);
+    if (rc) return rc;
+    cudaError_t e = pm::launch_block_apply(lat->Np, lat->Nq, lat->n_ch, d_blocks, d_diag, d_in, d_out, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e, "k_block_apply");
+    return PM_OK;
+}
+
+int32_t pm_kernel_apply(pm_lattice* lat, const int64_t* d_rowptr, const int32_t* d_colidx, const double* d_vals,
+                        const double* d_O, const double* d_Vt, const double* d_g1, const double* d_u, double* d_out,
+                        double* d_work, void* cuda_stream)
+{
+    if (!lat || !d_rowptr || !d_colidx || !d_vals || !d_O || !d_Vt || !d_g1 || !d_u || !d_out || !d_work)
+        return fail(PM_ERR_ARG, "NULL argument");
+    const int64_t M = (int64_t)lat->Np * lat->Nq * lat->n_ch;
+    double* t1 = d_work;                                   // V~1 G1 u
+    double* t2 = d_work + M;                               // P0 V~1 G1 u
+    int32_t rc = pm_block_apply(lat, d_Vt, d_g1, d_u, t1, cuda_stream);
+    if (rc) return rc;
+    if ((rc = pm_spmv(lat, M, d_rowptr, d_colidx, d_vals, t1, t2, cuda_stream))) return rc;
+    return pm_block_apply(lat, d_O, nullptr, t2, d_out, cuda_stream);
+}
+
 int32_t pm_last_fill_ms(pm_lattice* lat, float* ms)
 {
     if (!lat || !ms) return fail(PM_ERR_ARG, "NULL argument");

@@ -340,4 +340,41 @@ cudaError_t measure_dfma(int n_sm, double* tflops, cudaStream_t st)
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------------
+// Iteration step (eq. 24):  K u = O P0 V~1 G1 u  with G1 diagonal,
+// P0 the CSR matrix of this library and O, V~1 block matrices with (Np x Np) blocks acting on the pair index i for fixed
+// (j, alpha).  k_block_apply is one block-matrix factor with an optional diagonal factor folded in:
+//   out[(i,j,a)] = sum_i' B_a[i][i'] * (diag ? diag[(i',j,a)] : 1) * in[(i',j,a)] ,  index (i*Nq + j)*n_ch + a.
+// Thread = output element; consecutive threads read consecutive `in` entries for every i'.  The vectors (8 M bytes)
+// and the blocks stay in L2; the step is bound by the P0 SpMV (12 B per nonzero from HBM).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_block_apply(int Np, int Nq, int n_ch, const double* __restrict__ B,
+                                                    const double* __restrict__ diag, const double* __restrict__ in,
+                                                    double* __restrict__ out)
+{
+    const int64_t M = (int64_t)Np * Nq * n_ch, stride = (int64_t)Nq * n_ch;
+    for (int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; r < M; r += (int64_t)gridDim.x * blockDim.x) {
+        const int i = (int)(r / stride);
+        const int64_t ja = r - (int64_t)i * stride;
+        const int a = (int)(ja % n_ch);
+        const double* row = B + ((size_t)a * Np + i) * Np;
+        double s = 0.0;
+        for (int ip = 0; ip < Np; ++ip) {
+            const int64_t c = (int64_t)ip * stride + ja;
+            s = fma(row[ip], diag ? diag[c] * in[c] : in[c], s);
+        }
+        out[r] = s;
+    }
+}
+
+cudaError_t launch_block_apply(int Np, int Nq, int n_ch, const double* B, const double* diag, const double* in, double* out,
+                               cudaStream_t st)
+{
+    const int64_t M = (int64_t)Np * Nq * n_ch;
+    const int64_t blocks = std::min<int64_t>((M + 255) / 256, 148 * 16);
+    k_block_apply<<<(unsigned)std::max<int64_t>(blocks, 1), 256, 0, st>>>(Np, Nq, n_ch, B, diag, in, out);
+    count_launch();
+    return cudaGetLastError();
+}
+
 }  // namespace pm

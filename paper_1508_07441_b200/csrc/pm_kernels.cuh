@@ -40,6 +40,10 @@ cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin
 cudaError_t launch_spmv(int64_t n_rows, const int64_t* rowptr, const int32_t* colidx, const double* vals,
                         const double* x, double* y, cudaStream_t st);
 
+// one block-matrix factor of the iteration step (eq. 24) with an optional diagonal factor
+cudaError_t launch_block_apply(int Np, int Nq, int n_ch, const double* B, const double* diag, const double* in, double* out,
+                               cudaStream_t st);
+
 // dependent-free DFMA loop on every SM: measured FP64 FMA throughput in TFLOP/s (diagnostic)
 cudaError_t measure_dfma(int n_sm, double* tflops, cudaStream_t st);
 

@@ -179,3 +179,20 @@ def small_coupled(N: int = 6, jmax: int = 2, orders=(3, 3, 6), c: float = 1.0) -
     structure as configs[2]/[3], small grids so that the oracle runs in seconds)."""
     return Workload(f"small_3N_jle{jmax}_{N}x{N}", tan_grid(N, c), tan_grid(N, 0.8 * c),
                     enumerate_3n_channels(1, +1, 1, jmax), 1, +1, 1, PM_FERMION_ISOSPIN, *orders)
+
+
+# --------------------------------------------------------------------------- iteration-step inputs (eq. 24)
+def iteration_factors(wl: Workload, seed: int = 2025):
+    """Seeded synthetic factors of K = O P0 V~1 G1 (eq. 24), standing in for the pair-interaction data that is
+    not in the container: per channel an orthogonal (Np x Np) rotation O_a (QR of a Gaussian matrix), a symmetric
+    short-ranged V1_a, a diagonal G1 in [-1, 1] and a start vector u.  Data only — V~1 = O^T V1 is formed by whoever
+    uses them."""
+    rng = np.random.default_rng(seed)
+    Np = wl.Np
+    O = np.stack([np.linalg.qr(rng.standard_normal((Np, Np)))[0] for _ in range(wl.n_ch)])
+    idx = np.arange(Np)
+    decay = np.exp(-0.15 * np.abs(idx[:, None] - idx[None, :]))
+    V1 = np.stack([(lambda A: 0.5 * (A + A.T) * decay)(rng.standard_normal((Np, Np))) for _ in range(wl.n_ch)])
+    g1 = rng.uniform(-1.0, 1.0, wl.M)
+    u = rng.uniform(-1.0, 1.0, wl.M)
+    return np.ascontiguousarray(O), np.ascontiguousarray(V1), g1, u
