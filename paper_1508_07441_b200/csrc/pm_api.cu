@@ -106,7 +106,7 @@ int32_t ensure_device(pm_lattice* L)
     D.totcoup = T.totcoup; D.n_slot = T.n_slot; D.n_fun = (int)T.fun.size(); D.lmax = T.lmax;
     D.ny = pm::ylm_index(T.lmax, T.lmax) + 1;
     auto magic = [](int d) { return d <= 1 ? 0u : (unsigned)(((1ull << 32) + (unsigned)d - 1) / (unsigned)d); };
-    D.mg_npq = magic(L->n_p * L->n_q); D.mg_nq = magic(L->n_q);
+    D.mg_npq = magic(L->n_p * L->n_q); D.mg_nq = magic(L->n_q); D.mg_Nq = magic(L->Nq);
 
     std::vector<char> blob;
     auto put = [&](const void* src, size_t bytes) {

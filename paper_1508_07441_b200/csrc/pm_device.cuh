@@ -29,7 +29,7 @@ namespace pm {
 struct DevLattice {
     int Np, Nq, n_ch, n_p, n_q, n_x, nnode, n_cells, n_words, pe_pad, qe_pad;
     int totcoup, n_slot, n_fun, lmax, ny;
-    unsigned mg_npq, mg_nq;                     // ceil(2^32 / (n_p*n_q)), ceil(2^32 / n_q): exact division of node ids
+    unsigned mg_npq, mg_nq, mg_Nq;              // ceil(2^32 / d) for d = n_p*n_q, n_q, Nq: exact division of node and cell ids (x*d < 2^32)
     const double *pe, *qe;                      // edges, Np+1 / Nq+1 entries (padded with +inf to pe_pad / qe_pad)
     const double *thr_p, *thr_q;                // sqrt_threshold(edge), padded with +inf to a power of two
     const unsigned short *bk_p, *bk_q;          // kBuckets entries each: first threshold a value of that bucket can meet

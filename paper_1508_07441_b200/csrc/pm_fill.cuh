@@ -338,8 +338,9 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                         runT[ch] = 0.0;
                     }
                     const int tcell = __shfl_sync(0xffffffffu, tC, jb);
-                    const int ic = tcell / L.Nq, jc = tcell - ic * L.Nq;
-                    if (lane == 0) { s_norm[slot] = 1.0 / sqrt(dsrc * (s_dp[ic] * s_dq[jc])); s_hcol[slot] = tcell * L.n_ch; }
+                    const int ic = L.mg_Nq ? (int)__umulhi((unsigned)tcell, L.mg_Nq) : tcell, jc = tcell - ic * L.Nq;
+                    // (d_i dbar_j d_i' dbar_j')^(-1/2); rsqrt is within 2 ulp of the oracle's 1/sqrt
+                    if (lane == 0) { s_norm[slot] = rsqrt(dsrc * (s_dp[ic] * s_dq[jc])); s_hcol[slot] = tcell * L.n_ch; }
                     ++kcur;
                     __syncwarp();
                     if (kcur - kdone == kRowBatch) { write_rows(kdone, kRowBatch); kdone = kcur; }
