@@ -345,34 +345,61 @@ cudaError_t measure_dfma(int n_sm, double* tflops, cudaStream_t st)
 // P0 the CSR matrix of this library and O, V~1 block matrices with (Np x Np) blocks acting on the pair index i for fixed
 // (j, alpha).  k_block_apply is one block-matrix factor with an optional diagonal factor folded in:
 //   out[(i,j,a)] = sum_i' B_a[i][i'] * (diag ? diag[(i',j,a)] : 1) * in[(i',j,a)] ,  index (i*Nq + j)*n_ch + a.
-// Thread = output element; consecutive threads read consecutive `in` entries for every i'.  The vectors (8 M bytes)
-// and the blocks stay in L2; the step is bound by the P0 SpMV (12 B per nonzero from HBM).
+// The vectors (8 M bytes) and the blocks stay in L2; the step is bound by the P0 SpMV (12 B per nonzero from HBM).
 // ------------------------------------------------------------------------------------------------
+// Per channel a this is the product Out_a (Np x Nq) = B_a (Np x Np) * In_a (Np x Nq) on strided data.  CTA = (a, 32 x 32
+// tile of (i, j)): the 32 rows of B_a and the Np x 32 slab of (diag*)in are staged in shared memory (each reused 32
+// times), thread = 2 x 2 outputs.
+constexpr int kBlkT = 32;
+
 __global__ void __launch_bounds__(256) k_block_apply(int Np, int Nq, int n_ch, const double* __restrict__ B,
                                                     const double* __restrict__ diag, const double* __restrict__ in,
                                                     double* __restrict__ out)
 {
-    const int64_t M = (int64_t)Np * Nq * n_ch, stride = (int64_t)Nq * n_ch;
-    for (int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; r < M; r += (int64_t)gridDim.x * blockDim.x) {
-        const int i = (int)(r / stride);
-        const int64_t ja = r - (int64_t)i * stride;
-        const int a = (int)(ja % n_ch);
-        const double* row = B + ((size_t)a * Np + i) * Np;
-        double s = 0.0;
-        for (int ip = 0; ip < Np; ++ip) {
-            const int64_t c = (int64_t)ip * stride + ja;
-            s = fma(row[ip], diag ? diag[c] * in[c] : in[c], s);
-        }
-        out[r] = s;
+    extern __shared__ __align__(16) char smem[];
+    const int ld = Np + 1;                                     // padded row length of the B tile
+    double* sB = (double*)smem;                                 // [kBlkT][Np + 1]
+    double* sX = sB + kBlkT * ld;                               // [Np][kBlkT]
+    const int ti = (Np + kBlkT - 1) / kBlkT, tj = (Nq + kBlkT - 1) / kBlkT;
+    const int a = blockIdx.x / (ti * tj), rem = blockIdx.x - a * ti * tj, i0 = (rem / tj) * kBlkT, j0 = (rem % tj) * kBlkT;
+    const int64_t stride = (int64_t)Nq * n_ch;
+    const double* Ba = B + (size_t)a * Np * Np;
+    for (int k = threadIdx.x; k < kBlkT * Np; k += blockDim.x) {
+        const int r = k / Np, c = k - r * Np;
+        sB[r * ld + c] = (i0 + r < Np) ? Ba[(size_t)(i0 + r) * Np + c] : 0.0;
     }
+    for (int k = threadIdx.x; k < Np * kBlkT; k += blockDim.x) {
+        const int ip = k / kBlkT, jj = k - ip * kBlkT;
+        double x = 0.0;
+        if (j0 + jj < Nq) { const int64_t c = (int64_t)ip * stride + (int64_t)(j0 + jj) * n_ch + a; x = diag ? diag[c] * in[c] : in[c]; }
+        sX[k] = x;
+    }
+    __syncthreads();
+    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;     // outputs (i0 + ty, +16) x (j0 + tx, +16)
+    double s00 = 0.0, s01 = 0.0, s10 = 0.0, s11 = 0.0;
+    const double* b0 = sB + ty * ld;
+    const double* b1 = sB + (ty + 16) * ld;
+    for (int ip = 0; ip < Np; ++ip) {
+        const double x0 = sX[ip * kBlkT + tx], x1 = sX[ip * kBlkT + tx + 16], v0 = b0[ip], v1 = b1[ip];
+        s00 = fma(v0, x0, s00); s01 = fma(v0, x1, s01);
+        s10 = fma(v1, x0, s10); s11 = fma(v1, x1, s11);
+    }
+    const int i = i0 + ty, j = j0 + tx;
+    if (i < Np && j < Nq) out[(int64_t)i * stride + (int64_t)j * n_ch + a] = s00;
+    if (i < Np && j + 16 < Nq) out[(int64_t)i * stride + (int64_t)(j + 16) * n_ch + a] = s01;
+    if (i + 16 < Np && j < Nq) out[(int64_t)(i + 16) * stride + (int64_t)j * n_ch + a] = s10;
+    if (i + 16 < Np && j + 16 < Nq) out[(int64_t)(i + 16) * stride + (int64_t)(j + 16) * n_ch + a] = s11;
 }
 
 cudaError_t launch_block_apply(int Np, int Nq, int n_ch, const double* B, const double* diag, const double* in, double* out,
                                cudaStream_t st)
 {
-    const int64_t M = (int64_t)Np * Nq * n_ch;
-    const int64_t blocks = std::min<int64_t>((M + 255) / 256, 148 * 16);
-    k_block_apply<<<(unsigned)std::max<int64_t>(blocks, 1), 256, 0, st>>>(Np, Nq, n_ch, B, diag, in, out);
+    const int ti = (Np + kBlkT - 1) / kBlkT, tj = (Nq + kBlkT - 1) / kBlkT;
+    const size_t sm = sizeof(double) * ((size_t)kBlkT * (Np + 1) + (size_t)Np * kBlkT);
+    if (sm > 227 * 1024) return cudaErrorInvalidConfiguration;
+    cudaError_t e = cudaFuncSetAttribute(k_block_apply, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (e != cudaSuccess) return e;
+    k_block_apply<<<(unsigned)(n_ch * ti * tj), 256, sm, st>>>(Np, Nq, n_ch, B, diag, in, out);
     count_launch();
     return cudaGetLastError();
 }
