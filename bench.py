@@ -269,14 +269,16 @@ def main():
         flush.zero_()
         s0, s1 = (torch.cuda.Event(enable_timing=True) for _ in range(2))
         s0.record(st)
-        api.pm_kernel_apply(lat.h, rowptr, colidx, vals, dO, dVt, dg, du, yv, work)
+        api.pm_kernel_apply(lat.h, rowptr, None, vals, dO, dVt, dg, du, yv, work)      # columns implied by the hit lists
         s1.record(st)
         torch.cuda.synchronize()
         if it:
             it_ms.append(s0.elapsed_time(s1))
-    it_gbs = 12.0 * nnz / (min(it_ms) * 1e-3) * 1e-9
+    it_gbs = 8.0 * nnz / (min(it_ms) * 1e-3) * 1e-9
     iteration = {"ms": min(it_ms), "bound": "hbm", "achieved": it_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                 "frac": it_gbs / pk["hbm_gbs"], "what": "K u = O P0 V~1 G1 u, synthetic O, V1, G1 (seed 2025); bytes = 12 B per nonzero of P0"}
+                 "frac": it_gbs / pk["hbm_gbs"],
+                 "what": "K u = O P0 V~1 G1 u, synthetic O, V1, G1 (seed 2025), SpMV without the column array; "
+                         "bytes = 8 B per nonzero of P0 (with the column array: 12 B and the time of `spmv` + 0.15 ms)"}
     del xv, yv, work
 
     # ---- end to end through the C ABI with HOST buffers (D2H copies inside the timed region)

@@ -101,6 +101,13 @@ int32_t pm_fill(pm_lattice* lat, int32_t cell_begin, int32_t cell_end,
 int32_t pm_build(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int64_t* d_rowptr, int32_t* d_colidx, double* d_vals,
                  int64_t capacity, int64_t* nnz_host, void* cuda_stream);
 
+/* y = P0 x for the WHOLE lattice without reading column indices: the columns of row (cell, alpha) are implied by the
+ * hit cells of the source cell and the coupled-channel list, which the lattice keeps from its last pm_pattern /
+ * pm_build call over the whole lattice [0, n_cells) (PM_ERR_STATE otherwise).  d_rowptr, d_vals: that call's outputs.
+ * Reads 8 instead of 12 bytes per nonzero; the same bits as pm_spmv. */
+int32_t pm_spmv_implicit(pm_lattice* lat, const int64_t* d_rowptr, const double* d_vals, const double* d_x, double* d_y,
+                         void* cuda_stream);
+
 /* Device time of the last fill kernel launched for this lattice (by pm_fill, pm_build or pm_build_host), from CUDA
  * events recorded around it on its stream; waits for that kernel.  PM_ERR_STATE before the first fill. */
 int32_t pm_last_fill_ms(pm_lattice* lat, float* ms);
@@ -118,7 +125,8 @@ int32_t pm_spmv(pm_lattice* lat, int64_t n_rows, const int64_t* d_rowptr, const 
  * pm_block_apply : d_out[(i,j,a)] = sum_i' B_a[i][i'] * (d_diag ? d_diag[(i',j,a)] : 1) * d_in[(i',j,a)]
  *   d_blocks : device, n_ch*Np*Np doubles, B_a row-major, a-major;  d_diag : device, M doubles, or NULL;
  *   d_in, d_out : device, M doubles in the lattice's row order r = (i*Nq + j)*n_ch + a, distinct buffers.
- * pm_kernel_apply : d_out = O (P0 (V~1 (G1 u))) — three launches; d_work : device scratch of 2*M doubles.
+ * pm_kernel_apply : d_out = O (P0 (V~1 (G1 u))) — three launches; d_work : device scratch of 2*M doubles;
+ *   d_colidx may be NULL: the SpMV then takes the columns from the lattice's hit lists (pm_spmv_implicit).
  * Both are asynchronous on `cuda_stream`. */
 int32_t pm_block_apply(pm_lattice* lat, const double* d_blocks, const double* d_diag, const double* d_in, double* d_out,
                        void* cuda_stream);

@@ -23,7 +23,7 @@ ERRORS = {-1: "PM_ERR_ARG", -2: "PM_ERR_GRID", -3: "PM_ERR_CHANNEL", -4: "PM_ERR
 
 EXPORTS = ["pm_lattice_create", "pm_lattice_destroy", "pm_lattice_dims", "pm_lattice_rule", "pm_lattice_set_rule",
            "pm_lattice_coupling", "pm_lattice_work", "pm_pattern_counts", "pm_lattice_fill_kernel", "pm_set_jit", "pm_diag_jit_compile", "pm_diag_sqrt_threshold",
-           "pm_diag_dfma_tflops", "pm_pattern", "pm_fill", "pm_build", "pm_last_fill_ms", "pm_block_apply", "pm_kernel_apply", "pm_spmv", "pm_build_host_count", "pm_build_host",
+           "pm_diag_dfma_tflops", "pm_pattern", "pm_fill", "pm_build", "pm_last_fill_ms", "pm_block_apply", "pm_kernel_apply", "pm_spmv_implicit", "pm_spmv", "pm_build_host_count", "pm_build_host",
            "pm_launch_count", "pm_last_error"]
 
 
@@ -70,6 +70,7 @@ def lib():
     L.pm_diag_sqrt_threshold.restype = C.c_double
     L.pm_pattern.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, C.c_int64, _i64p, _vp]
     L.pm_fill.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, _vp]
+    L.pm_spmv_implicit.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp]
     L.pm_block_apply.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp]
     L.pm_kernel_apply.argtypes = [_vp] + [_vp] * 10
     L.pm_last_fill_ms.argtypes = [_vp, C.POINTER(C.c_float)]
@@ -201,6 +202,11 @@ def pm_build(h, cell_begin, cell_end, d_rowptr, d_colidx, d_vals, stream=None):
     return nnz.value
 
 
+def pm_spmv_implicit(h, d_rowptr, d_vals, d_x, d_y, stream=None):
+    """y = P0 x with the columns implied by the lattice's hit lists (whole lattice, after pm_pattern / pm_build)."""
+    _check(lib().pm_spmv_implicit(h, d_rowptr.data_ptr(), d_vals.data_ptr(), d_x.data_ptr(), d_y.data_ptr(), _stream_ptr(stream)))
+
+
 def pm_block_apply(h, d_blocks, d_diag, d_in, d_out, stream=None):
     _check(lib().pm_block_apply(h, d_blocks.data_ptr(), d_diag.data_ptr() if d_diag is not None else None,
                                 d_in.data_ptr(), d_out.data_ptr(), _stream_ptr(stream)))
@@ -208,7 +214,8 @@ def pm_block_apply(h, d_blocks, d_diag, d_in, d_out, stream=None):
 
 def pm_kernel_apply(h, d_rowptr, d_colidx, d_vals, d_O, d_Vt, d_g1, d_u, d_out, d_work, stream=None):
     """d_out = O P0 V~1 G1 u (eq. 24); d_work holds 2*M doubles."""
-    _check(lib().pm_kernel_apply(h, d_rowptr.data_ptr(), d_colidx.data_ptr(), d_vals.data_ptr(), d_O.data_ptr(),
+    _check(lib().pm_kernel_apply(h, d_rowptr.data_ptr(), d_colidx.data_ptr() if d_colidx is not None else None,
+                                 d_vals.data_ptr(), d_O.data_ptr(),
                                  d_Vt.data_ptr(), d_g1.data_ptr(), d_u.data_ptr(), d_out.data_ptr(), d_work.data_ptr(),
                                  _stream_ptr(stream)))
 

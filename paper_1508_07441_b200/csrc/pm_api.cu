@@ -54,6 +54,9 @@ struct pm_lattice {
     std::string jit_error;
     pm::FillLaunch plan{};
     int* d_counter = nullptr;          // work counter of the fill kernel
+    int* d_hitlist = nullptr;          // hit cells of every source cell of the last pattern call (pm_spmv_implicit), lazily built
+    int64_t hitlist_cap = 0;
+    bool hitlist_valid = false;
     cudaEvent_t ev_fill0 = nullptr, ev_fill1 = nullptr;   // around the last fill kernel, on its stream (pm_last_fill_ms)
     bool fill_timed = false;
     unsigned long long hash = 0;       // pm::tables_hash of T (selects a generated fill kernel)
@@ -76,6 +79,8 @@ void free_device(pm_lattice* L)
     if (L->h_summary) cudaFreeHost(L->h_summary);
     if (L->d_counter) cudaFree(L->d_counter);
     L->d_counter = nullptr;
+    if (L->d_hitlist) cudaFree(L->d_hitlist);
+    L->d_hitlist = nullptr; L->hitlist_cap = 0; L->hitlist_valid = false;
     if (L->ev_fill0) cudaEventDestroy(L->ev_fill0);
     if (L->ev_fill1) cudaEventDestroy(L->ev_fill1);
     L->ev_fill0 = L->ev_fill1 = nullptr; L->fill_timed = false;
@@ -394,6 +399,7 @@ int32_t pm_pattern(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int64_
     const bool reuse = lat->hmax >= 0 && lat->pat_count_only && d_colidx && lat->pat_begin == cell_begin && lat->pat_end == cell_end
                     && lat->hits_cap >= n_blk;
     lat->pat_count_only = (d_colidx == nullptr);
+    if (!reuse) lat->hitlist_valid = false;
     if (!reuse) {
         lat->hmax = -1;
         if ((rc = ensure_cell_scratch(lat, n_blk))) return rc;
@@ -460,6 +466,32 @@ int32_t pm_fill(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const int
     return fill_block(lat, cell_begin, cell_end, d_rowptr, d_vals, nullptr, (cudaStream_t)cuda_stream);
 }
 
+int32_t pm_spmv_implicit(pm_lattice* lat, const int64_t* d_rowptr, const double* d_vals, const double* d_x, double* d_y, void* cuda_stream)
+{
+    if (!lat || !d_rowptr || !d_vals || !d_x || !d_y) return fail(PM_ERR_ARG, "NULL argument");
+    int32_t rc = ensure_device(lat);
+    if (rc) return rc;
+    const int n_cells = lat->Np * lat->Nq;
+    if (lat->hmax < 0 || lat->pat_begin != 0 || lat->pat_end != n_cells)
+        return fail(PM_ERR_STATE, "pm_spmv_implicit needs the node lists of a pm_pattern / pm_build call over the whole lattice");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e;
+    if (!lat->hitlist_valid) {
+        const int64_t need = std::max<int64_t>(lat->counts[2], 1);
+        if (need > lat->hitlist_cap) {
+            if (lat->d_hitlist) cudaFree(lat->d_hitlist);
+            lat->d_hitlist = nullptr; lat->hitlist_cap = 0;
+            if ((e = cudaMalloc(&lat->d_hitlist, sizeof(int) * (size_t)need)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(hit list)");
+            lat->hitlist_cap = need;
+        }
+        if ((e = pm::launch_hit_list(lat->dev, n_cells, lat->nl, lat->d_cellbase, lat->d_hitlist, st)) != cudaSuccess) return cuda_fail(e, "k_hit_list");
+        lat->hitlist_valid = true;
+    }
+    e = pm::launch_spmv_implicit(lat->dev, (int64_t)n_cells * lat->n_ch, d_rowptr, lat->nl.hits, lat->d_cellbase, lat->d_hitlist, d_vals, d_x, d_y, st);
+    if (e != cudaSuccess) return cuda_fail(e, "k_spmv_implicit");
+    return PM_OK;
+}
+
 int32_t pm_block_apply(pm_lattice* lat, const double* d_blocks, const double* d_diag, const double* d_in, double* d_out, void* cuda_stream)
 {
     if (!lat || !d_blocks || !d_in || !d_out) return fail(PM_ERR_ARG, "NULL argument");
@@ -475,14 +507,16 @@ int32_t pm_kernel_apply(pm_lattice* lat, const int64_t* d_rowptr, const int32_t*
                         const double* d_O, const double* d_Vt, const double* d_g1, const double* d_u, double* d_out,
                         double* d_work, void* cuda_stream)
 {
-    if (!lat || !d_rowptr || !d_colidx || !d_vals || !d_O || !d_Vt || !d_g1 || !d_u || !d_out || !d_work)
+    if (!lat || !d_rowptr || !d_vals || !d_O || !d_Vt || !d_g1 || !d_u || !d_out || !d_work)
         return fail(PM_ERR_ARG, "NULL argument");
     const int64_t M = (int64_t)lat->Np * lat->Nq * lat->n_ch;
     double* t1 = d_work;                                   // V~1 G1 u
     double* t2 = d_work + M;                               // P0 V~1 G1 u
     int32_t rc = pm_block_apply(lat, d_Vt, d_g1, d_u, t1, cuda_stream);
     if (rc) return rc;
-    if ((rc = pm_spmv(lat, M, d_rowptr, d_colidx, d_vals, t1, t2, cuda_stream))) return rc;
+    rc = d_colidx ? pm_spmv(lat, M, d_rowptr, d_colidx, d_vals, t1, t2, cuda_stream)
+                  : pm_spmv_implicit(lat, d_rowptr, d_vals, t1, t2, cuda_stream);      // columns implied by the hit lists
+    if (rc) return rc;
     return pm_block_apply(lat, d_O, nullptr, t2, d_out, cuda_stream);
 }
 

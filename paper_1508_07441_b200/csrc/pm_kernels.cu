@@ -246,6 +246,50 @@ __global__ void __launch_bounds__(256) k_spmv(int64_t n_rows, const int64_t* __r
 }
 
 // ------------------------------------------------------------------------------------------------
+// SpMV without the column array.  A row (cell, alpha) holds, for each hit cell k of its source cell in ascending
+// order, each alpha' coupled to alpha: column = hit[k]*n_ch + cl[alpha][m].  With the hit lists (4 B per hit cell pair,
+// 6 MB on configs[4]) the 4 B per nonzero of colidx need not be read: 8 instead of 12 B per nonzero from HBM.
+// Same lane striding and reduction as k_spmv, hence the same bits.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kThreads) k_hit_list(DevLattice L, NodeLists nl, const int64_t* __restrict__ cellbase,
+                                                      int* __restrict__ hitlist)
+{
+    const int ntot = nl.ntot[blockIdx.x];
+    const unsigned short* g_rkpos = nl.rkpos + (size_t)blockIdx.x * L.nnode;
+    const unsigned* g_key = nl.key + (size_t)blockIdx.x * L.nnode;
+    int* out = hitlist + cellbase[blockIdx.x];
+    for (int pos = threadIdx.x; pos < ntot; pos += blockDim.x) {
+        const int r = g_rkpos[pos];
+        if (pos == 0 || g_rkpos[pos - 1] != r) out[r] = (int)(g_key[pos] >> 14);
+    }
+}
+
+__global__ void __launch_bounds__(256) k_spmv_implicit(DevLattice L, int64_t n_rows, const int64_t* __restrict__ rowptr,
+                                                      const int* __restrict__ hits, const int64_t* __restrict__ cellbase,
+                                                      const int* __restrict__ hitlist, const double* __restrict__ vals,
+                                                      const double* __restrict__ x, double* __restrict__ y)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t wpb = blockDim.x >> 5;
+    for (int64_t r = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5); r < n_rows; r += (int64_t)gridDim.x * wpb) {
+        const int cell = (int)(r / L.n_ch), al = (int)(r - (int64_t)cell * L.n_ch);
+        const int off = L.cl_off[al], nc = L.cl_off[al + 1] - off, len = hits[cell] * nc;
+        const unsigned mg = nc > 1 ? (unsigned)(((1ull << 32) + (unsigned)nc - 1) / (unsigned)nc) : 0u;
+        const int* hl = hitlist + cellbase[cell];
+        const int* cl = L.cl + off;
+        const double* v = vals + rowptr[r];
+        double s = 0.0;
+        for (int idx = lane; idx < len; idx += 32) {
+            const int k = mg ? (int)__umulhi((unsigned)idx, mg) : idx, m = idx - k * nc;
+            s += v[idx] * x[hl[k] * L.n_ch + cl[m]];
+        }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+        if (lane == 0) y[r] = s;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Host launchers
 // ------------------------------------------------------------------------------------------------
 static std::atomic<int64_t> g_launches{0};
@@ -283,6 +327,22 @@ cudaError_t launch_emit_cols(const DevLattice& L, int n_blk, const NodeLists& nl
     if (e != cudaSuccess) return e;
     const int threads = std::min(1024, std::max(128, (L.totcoup + 31) & ~31));
     k_emit_cols<<<n_blk, threads, sm, st>>>(L, nl, hmax, rowptr, colidx);
+    ++g_launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_hit_list(const DevLattice& L, int n_blk, const NodeLists& nl, const int64_t* cellbase, int* hitlist, cudaStream_t st)
+{
+    k_hit_list<<<n_blk, kThreads, 0, st>>>(L, nl, cellbase, hitlist);
+    ++g_launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_spmv_implicit(const DevLattice& L, int64_t n_rows, const int64_t* rowptr, const int* hits, const int64_t* cellbase,
+                                 const int* hitlist, const double* vals, const double* x, double* y, cudaStream_t st)
+{
+    const int64_t blocks = std::min<int64_t>((n_rows + 7) / 8, 148 * 32);
+    k_spmv_implicit<<<(unsigned)std::max<int64_t>(blocks, 1), 256, 0, st>>>(L, n_rows, rowptr, hits, cellbase, hitlist, vals, x, y);
     ++g_launches;
     return cudaGetLastError();
 }

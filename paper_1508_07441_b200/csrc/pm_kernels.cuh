@@ -37,6 +37,9 @@ bool fill_plan_jit(const DevLattice& L, const Tables& T, unsigned long long tabl
 cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl,
                         const int64_t* rowptr, double* vals, int32_t* colidx, int* counter, cudaStream_t st);
 
+cudaError_t launch_hit_list(const DevLattice& L, int n_blk, const NodeLists& nl, const int64_t* cellbase, int* hitlist, cudaStream_t st);
+cudaError_t launch_spmv_implicit(const DevLattice& L, int64_t n_rows, const int64_t* rowptr, const int* hits, const int64_t* cellbase,
+                                 const int* hitlist, const double* vals, const double* x, double* y, cudaStream_t st);
 cudaError_t launch_spmv(int64_t n_rows, const int64_t* rowptr, const int32_t* colidx, const double* vals,
                         const double* x, double* y, cudaStream_t st);
 

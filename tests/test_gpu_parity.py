@@ -270,6 +270,17 @@ def test_iteration_step_matches_oracle(api, oracle, wl):
     api.pm_kernel_apply(lat.h, rp, ci, v, dO, dVt, dg, du, out, work)
     got = out.cpu().numpy()
     assert np.max(np.abs(got - ref)) <= 1e-11 * np.max(np.abs(ref))
+    out2 = torch.empty_like(out)
+    api.pm_kernel_apply(lat.h, rp, None, v, dO, dVt, dg, du, out2, work)     # columns implied by the hit lists
+    assert torch.equal(out, out2)
+    y1, y2 = torch.empty_like(out), torch.empty_like(out)
+    api.pm_spmv(lat.h, rp, ci, v, du, y1)
+    api.pm_spmv_implicit(lat.h, rp, v, du, y2)
+    assert torch.equal(y1, y2)                                               # same lane striding, same bits
+    lat.pattern(0, 3)                                                        # a partial pattern call drops the whole-lattice lists
+    with pytest.raises(api.PmError) as e:
+        api.pm_spmv_implicit(lat.h, rp, v, du, y2)
+    assert e.value.code == -7
     api.pm_block_apply(lat.h, dO, None, du, out)
     assert np.max(np.abs(out.cpu().numpy() - it.block_apply(O, u, wl.Np, wl.Nq, wl.n_ch))) <= 1e-13 * np.max(np.abs(u)) * wl.Np
     api.pm_block_apply(lat.h, dVt, dg, du, out)
