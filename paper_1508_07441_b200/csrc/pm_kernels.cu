@@ -149,39 +149,56 @@ __global__ void __launch_bounds__(1024) k_scan_cells(DevLattice L, int n_blk, co
                                                     const int* __restrict__ ntot, const int* __restrict__ nseg,
                                                     int64_t* __restrict__ cellbase, int64_t* __restrict__ summary)
 {
-    __shared__ long long part[1024];
-    __shared__ int pmax[1024];
-    if (blockDim.x == 1024 && threadIdx.x >= 992) {  // last warp: totals of nodes on the grid and of segments (statistics)
-        long long a = 0, s2 = 0;
-        for (int k = threadIdx.x - 992; k < n_blk; k += 32) { a += ntot[k]; s2 += nseg[k]; }
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, d); s2 += __shfl_xor_sync(0xffffffffu, s2, d); }
-        if (threadIdx.x == 992) { summary[2] = a; summary[3] = s2; }
-    }
-    const int T = blockDim.x, t = threadIdx.x;
-    const int chunk = (n_blk + T - 1) / T, b = min(t * chunk, n_blk), e = min(b + chunk, n_blk);
-    long long sum = 0; int mx = 0;
-    for (int k = b; k < e; ++k) { sum += hits[k]; mx = max(mx, hits[k]); }
-    part[t] = sum; pmax[t] = mx;
+    // tiles of 1024 consecutive cells (coalesced reads and writes): warp scans, then the 32 warp totals, then the carry
+    __shared__ long long wsum[32];
+    __shared__ long long s_carry;
+    __shared__ long long s_stat[3][32];
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    long long nodes = 0, segs = 0;
+    int mx = 0;
+    if (t == 0) s_carry = 0;
     __syncthreads();
-    if (t < 32) {                                   // warp 0 scans the 1024 partial sums, 32 per lane
-        long long run = 0; int m = 0;
-        for (int k = t * 32; k < t * 32 + 32; ++k) { run += part[k]; m = max(m, pmax[k]); }
-        long long inc = run;
+    for (int base = 0; base < n_blk; base += 1024) {
+        const int k = base + t;
+        const int h = k < n_blk ? hits[k] : 0;
+        if (k < n_blk) { nodes += ntot[k]; segs += nseg[k]; mx = max(mx, h); }
+        long long inc = h;
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const long long y = __shfl_up_sync(0xffffffffu, inc, d);
-            const int my = __shfl_xor_sync(0xffffffffu, m, d);
-            if (t >= d) inc += y;
-            m = max(m, my);
+        for (int d = 1; d < 32; d <<= 1) { const long long y = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += y; }
+        if (lane == 31) wsum[warp] = inc;
+        __syncthreads();
+        if (warp == 0) {
+            const long long v = wsum[lane];
+            long long x = v;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) { const long long y = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += y; }
+            wsum[lane] = x - v;                         // exclusive prefix of the warp totals
+            if (lane == 31) s_stat[0][0] = x;           // tile total
         }
-        long long ex = inc - run;
-        for (int k = t * 32; k < t * 32 + 32; ++k) { const long long v = part[k]; part[k] = ex; ex += v; }
-        if (t == 31) { summary[0] = inc * L.totcoup; summary[1] = m; cellbase[n_blk] = inc; }
+        __syncthreads();
+        const long long carry = s_carry;
+        if (k < n_blk) cellbase[k] = carry + wsum[warp] + inc - h;
+        __syncthreads();
+        if (t == 0) s_carry = carry + s_stat[0][0];
+        __syncthreads();
     }
+    // statistics: nodes on the grid, segments, max hits
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        nodes += __shfl_xor_sync(0xffffffffu, nodes, d); segs += __shfl_xor_sync(0xffffffffu, segs, d);
+        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+    }
+    if (lane == 0) { s_stat[0][warp] = nodes; s_stat[1][warp] = segs; s_stat[2][warp] = mx; }
     __syncthreads();
-    long long run = part[t];
-    for (int k = b; k < e; ++k) { cellbase[k] = run; run += hits[k]; }
+    if (t == 0) {
+        long long a = 0, s2 = 0, m = 0;
+        for (int w = 0; w < 32; ++w) { a += s_stat[0][w]; s2 += s_stat[1][w]; m = max(m, s_stat[2][w]); }
+        const long long total = s_carry;
+        summary[0] = total * L.totcoup;                 // nnz of the block
+        summary[1] = m;                                 // max hit cells of any source cell
+        summary[2] = a; summary[3] = s2;
+        cellbase[n_blk] = total;
+    }
 }
 
 // Pattern pass, kernel R: rowptr (block-local) from cellbase: row (cell k, alpha) starts at
