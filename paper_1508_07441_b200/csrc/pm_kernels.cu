@@ -1,4 +1,4 @@
-// pm_kernels.cu — CUDA kernels of libpm for sm_100a: pattern pass (a6), SpMV (a9), FP64 peak diagnostic.
+// pm_kernels.cu — CUDA kernels of libpm for sm_100a: pattern pass (a6), SpMV (a9) with and without the column array, the block factors of the iteration step, FP64 peak diagnostic.
 // One CTA per source cell D_ij; the node map and location live in pm_device.cuh.
 // Paper's prior art: pre-selection of the nonzero elements by a separate GPU pass,
 // one thread per element, constants in global memory (L341), CPU repack into CSR for coupled channels (L376).
