@@ -174,11 +174,24 @@ def config(k: int) -> Workload:
     raise ValueError(f"no config {k}")
 
 
-def small_coupled(N: int = 6, jmax: int = 2, orders=(3, 3, 6), c: float = 1.0) -> Workload:
+def small_coupled(N: int = 6, jmax: int = 2, orders=(3, 3, 6), c: float = 1.0, Nq: int | None = None,
+                  J2: int = 1, parity: int = +1) -> Workload:
     """A reduced coupled-channel lattice for element-by-element parity tests (same channel
-    structure as configs[2]/[3], small grids so that the oracle runs in seconds)."""
-    return Workload(f"small_3N_jle{jmax}_{N}x{N}", tan_grid(N, c), tan_grid(N, 0.8 * c),
-                    enumerate_3n_channels(1, +1, 1, jmax), 1, +1, 1, PM_FERMION_ISOSPIN, *orders)
+    structure as configs[2]/[3], small grids so that the oracle runs in seconds).  `Nq` (default N) gives a
+    rectangular lattice with N cells in p and Nq cells in q; (J2, parity) selects another J^pi."""
+    Nq = N if Nq is None else Nq
+    tag = "" if (J2, parity) == (1, +1) else f"_J{J2}half{'+' if parity > 0 else '-'}"
+    return Workload(f"small_3N_jle{jmax}{tag}_{N}x{Nq}", tan_grid(N, c), tan_grid(Nq, 0.8 * c),
+                    enumerate_3n_channels(J2, parity, 1, jmax), J2, parity, 1, PM_FERMION_ISOSPIN, *orders)
+
+
+def boson_lattice(Np: int, Nq: int, waves=((0, 0),), J: int = 0, orders=(4, 4, 8), cp: float = 1.0, cq: float = 1.0) -> Workload:
+    """Spinless-boson lattice with Np x Nq cells (tangent-mapped grids with scales cp, cq) and the channels
+    (l, lam) in `waves` coupled to total J = L."""
+    ch = np.concatenate([boson_channel(l, lam) for l, lam in waves])
+    w = "".join(f"{l}{lam}" for l, lam in waves)
+    return Workload(f"boson_w{w}_J{J}_{Np}x{Nq}", tan_grid(Np, cp), tan_grid(Nq, cq), ch, 2 * J, +1 if all((l + lam) % 2 == 0 for l, lam in waves) else -1,
+                    0, PM_SPINLESS_BOSON, *orders)
 
 
 # --------------------------------------------------------------------------- iteration-step inputs (eq. 24)

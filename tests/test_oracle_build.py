@@ -228,3 +228,130 @@ def test_oracle_reproduces_its_stored_rows(oracle):
         assert ci.tolist() == [e[0] for e in entries]
         ref = np.array([e[1] for e in entries])
         assert np.max(np.abs(v - ref)) <= 1e-15 * np.max(np.abs(ref))
+
+
+# ---- po_build's coupled-channel assembly against the pinned coefficient po_G, node by node ---------------------
+def _rebuild_from_G(wl, oracle):
+    """Every CSR entry from its definition (eq. 21-22):
+    P0[(ij a),(i'j' a')] = sum_{nodes of (i,j) landing in (i',j')} w * pq/(p'q') * 2*G2_{a a'}(p,q,x) / sqrt(d_i dbar_j d_i' dbar_j'),
+    nodes from po_cell_nodes, the coefficient from po_G (one call per node and channel pair — nothing of po_build's
+    own tables is used).  Returns a dict (row, col) -> value."""
+    pe, qe, nc = wl.p_edges, wl.q_edges, wl.n_ch
+    ch = wl.channels
+    coupled = [[oracle.coupled(a, b, wl.J2, wl.statistics) for b in ch] for a in ch]
+    out = {}
+    for cell in range(wl.n_cells):
+        i, j = divmod(cell, wl.Nq)
+        nd = oracle.cell_nodes(wl, cell)
+        for n in range(wl.nodes_per_cell):
+            t = int(nd["target"][n])
+            if t < 0:
+                continue
+            ic, jc = divmod(t, wl.Nq)
+            p, q, x = float(nd["p"][n]), float(nd["q"][n]), float(nd["x"][n])
+            om = nd["w"][n] * (p * q / (nd["pp"][n] * nd["qq"][n]))
+            nrm = math.sqrt((pe[i + 1] - pe[i]) * (qe[j + 1] - qe[j]) * (pe[ic + 1] - pe[ic]) * (qe[jc + 1] - qe[jc]))
+            for a in range(nc):
+                for b in range(nc):
+                    if coupled[a][b]:
+                        key = (cell * nc + a, t * nc + b)
+                        out[key] = out.get(key, 0.0) + om * 2.0 * oracle.G(ch[a], ch[b], wl.J2, wl.T2, wl.statistics, p, q, x, 2) / nrm
+    return out
+
+
+@pytest.mark.parametrize("wl", [
+    I.small_coupled(N=4, jmax=3, orders=(2, 3, 4)),                            # 26 channels, unequal orders
+    I.small_coupled(N=3, jmax=2, orders=(2, 2, 4), Nq=5),                      # 18 channels, Np != Nq
+    I.small_coupled(N=3, jmax=1, orders=(2, 3, 4), Nq=4, J2=3, parity=-1),     # J = 3/2-, L up to 3
+    I.boson_lattice(4, 6, waves=((0, 0), (2, 2)), J=0, orders=(3, 2, 5), cq=0.7),   # bosons with d-waves, Np != Nq
+    I.boson_lattice(3, 3, waves=((0, 2), (2, 0), (2, 2)), J=2, orders=(2, 2, 4)),   # J = L = 2
+], ids=lambda w: w.name)
+def test_build_equals_node_sum_of_pinned_G(oracle, wl):
+    """po_build has its own tabulated route to the coefficient (po_tables_init, po_eval_bipolar, tri_of / coef);
+    po_G is the function pinned by tests/test_oracle_algebra.py (product-basis construction, sympy, scipy).  Here every
+    entry of po_build's CSR is recomputed from po_cell_nodes and po_G alone and must agree to rounding: a swapped
+    bra/ket triple, a lost 1/(2L+1), a wrong factor 2 or a transposed (alpha, alpha') in the assembly would fail.
+    Cites eq. (21)-(22); DESIGN.md sec. 3.1 / 3.2."""
+    rp, ci, v = oracle.build_csr(wl)
+    ref = _rebuild_from_G(wl, oracle)
+    assert len(ref) == len(v)                                   # same structural pattern: hit cells x coupled mask
+    rows = np.repeat(np.arange(len(rp) - 1), np.diff(rp))
+    want = np.array([ref[(int(r), int(c))] for r, c in zip(rows, ci)])
+    assert np.max(np.abs(v - want)) <= 1e-14 * np.max(np.abs(want)), np.max(np.abs(v - want)) / np.max(np.abs(want))
+    assert np.max(np.abs(want)) > 1e-3
+
+
+# ---- rectangular lattices (Np != Nq): every index formula that could mix the two axes --------------------------
+RECT = [
+    I.boson_lattice(5, 9, orders=(3, 4, 6), cp=1.0, cq=0.6),
+    I.boson_lattice(9, 5, orders=(4, 3, 6), cp=0.7, cq=1.3),
+    I.small_coupled(N=5, jmax=1, orders=(3, 2, 5), Nq=8),
+]
+
+
+@pytest.mark.parametrize("wl", RECT, ids=lambda w: w.name)
+def test_rectangular_lattice_pins(oracle, wl):
+    """Np != Nq: cell = i*Nq + j on both the source and the target side.  (1) measure conservation per source cell with
+    the cell's own (i, j) = divmod(cell, Nq); (2) the target of every node re-derived in numpy with searchsorted on the
+    p- and the q-edges separately; (3) the pattern of po_build is exactly {targets of the cell's nodes} x coupled mask,
+    with row = cell*n_ch + a and column = target*n_ch + b; (4) energy invariant of every entry."""
+    pe, qe, nc = wl.p_edges, wl.q_edges, wl.n_ch
+    (tp, wp), (tq, wq), (tx, wx) = wl.rules["p"], wl.rules["q"], wl.rules["x"]
+    rp, ci, v = oracle.build_csr(wl)
+    assert len(rp) == wl.Np * wl.Nq * nc + 1
+    cmask = np.array([[oracle.coupled(a, b, wl.J2, wl.statistics) for b in wl.channels] for a in wl.channels])
+    for cell in range(wl.n_cells):
+        i, j = divmod(cell, wl.Nq)
+        nd = oracle.cell_nodes(wl, cell)
+        exact = (pe[i + 1] ** 3 - pe[i] ** 3) * (qe[j + 1] ** 3 - qe[j] ** 3) / 9.0
+        assert abs(0.5 * np.sum(nd["w"] * nd["p"] ** 2 * nd["q"] ** 2) - exact) <= 1e-13 * exact
+        assert np.all((nd["p"] > pe[i]) & (nd["p"] < pe[i + 1]) & (nd["q"] > qe[j]) & (nd["q"] < qe[j + 1]))
+        ic = np.searchsorted(pe, nd["pp"], side="right") - 1
+        jc = np.searchsorted(qe, nd["qq"], side="right") - 1
+        ok = (ic >= 0) & (ic < wl.Np) & (jc >= 0) & (jc < wl.Nq) & (nd["pp"] > 0) & (nd["qq"] > 0)
+        tgt = np.where(ok, ic * wl.Nq + jc, -1)
+        assert np.array_equal(tgt, nd["target"])
+        hit = np.unique(tgt[tgt >= 0])
+        for a in range(nc):
+            r = cell * nc + a
+            want = (hit[:, None] * nc + np.nonzero(cmask[a])[0][None, :]).ravel()
+            assert np.array_equal(ci[rp[r]:rp[r + 1]], want)
+    rows = np.repeat(np.arange(len(rp) - 1), np.diff(rp))
+    src, dst = rows // nc, ci // nc
+    i, j, ic, jc = src // wl.Nq, src % wl.Nq, dst // wl.Nq, dst % wl.Nq
+    assert ic.max() < wl.Np and jc.max() < wl.Nq
+    Elo, Ehi = pe[i] ** 2 + 0.75 * qe[j] ** 2, pe[i + 1] ** 2 + 0.75 * qe[j + 1] ** 2
+    Flo, Fhi = pe[ic] ** 2 + 0.75 * qe[jc] ** 2, pe[ic + 1] ** 2 + 0.75 * qe[jc + 1] ** 2
+    assert np.all((Elo <= Fhi * (1 + 1e-14)) & (Flo <= Ehi * (1 + 1e-14)))
+
+
+def test_rectangular_transpose_symmetry(oracle):
+    """The exact s-wave matrix is symmetric; at high orders the node-binned one on a 4 x 6 lattice approaches its own
+    transpose — an (i, j) / (i', j') index mix-up between the axes would not."""
+    a = [_asym(_csr(I.boson_lattice(4, 6, orders=o, cq=0.8), oracle)) for o in ((6, 6, 12), (24, 24, 48))]
+    assert a[1] < a[0] / 4 and a[1] < 2e-2, a
+
+
+def test_single_p_node_is_the_two_axis_rule(oracle):
+    """Reading R1: n_p = 1 (the midpoint of the p-cell, weight = the cell width) is north_star's literal 'quadrature in q
+    and x'.  The node table has p = the cell midpoint for every node, weights (d_i)(hq wq_b) wx_c, and po_build of the
+    s-wave boson lattice equals the direct node sum."""
+    wl = I.boson_lattice(5, 4, orders=(1, 3, 6), cq=0.9)
+    pe, qe = wl.p_edges, wl.q_edges
+    (tq, wq), (tx, wx) = wl.rules["q"], wl.rules["x"]
+    assert wl.rules["p"][0].tolist() == [0.0] and wl.rules["p"][1].tolist() == [2.0]
+    A = _csr(wl, oracle).toarray()
+    B = np.zeros_like(A)
+    for cell in range(wl.n_cells):
+        i, j = divmod(cell, wl.Nq)
+        nd = oracle.cell_nodes(wl, cell)
+        assert np.all(nd["p"] == 0.5 * (pe[i] + pe[i + 1]))
+        b, c = np.meshgrid(np.arange(wl.n_q), np.arange(wl.n_x), indexing="ij")
+        w = ((0.5 * (pe[i + 1] - pe[i]) * 2.0) * (0.5 * (qe[j + 1] - qe[j]) * wq[b]) * wx[c]).ravel()
+        assert np.array_equal(w, nd["w"])
+        for n in np.nonzero(nd["target"] >= 0)[0]:
+            t = nd["target"][n]
+            ic, jc = divmod(int(t), wl.Nq)
+            nrm = math.sqrt((pe[i + 1] - pe[i]) * (qe[j + 1] - qe[j]) * (pe[ic + 1] - pe[ic]) * (qe[jc + 1] - qe[jc]))
+            B[cell, t] += nd["w"][n] * nd["p"][n] * nd["q"][n] / (nd["pp"][n] * nd["qq"][n]) / nrm
+    assert np.max(np.abs(A - B)) <= 1e-14 * np.max(np.abs(B))
