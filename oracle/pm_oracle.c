@@ -556,6 +556,55 @@ int po_build(const double* pe, int Np, const double* qe, int Nq,
     return 0;
 }
 
+/* ------------------------------------------------------------------------------------------
+ * Pattern only (no values): the hit cells of every source cell in [cell_begin, cell_end), ascending —
+ * the geometric half of the pattern  {hit cells} x {coupled(alpha,alpha')}  of DESIGN.md sec. 3.1
+ * (the paper's step 2a 'pre-selection').  Same node loop and the same po_make_node as
+ * po_build, nothing else.  hitptr[nblk+1] is always written; hitcell (capacity cap) may be NULL to count.
+ * Returns 0, -1 on bad arguments, -3 when cap is too small.
+ * ---------------------------------------------------------------------------------------- */
+int po_hit_cells(const double* pe, int Np, const double* qe, int Nq,
+                 const double* tp, const double* wp, int n_p, const double* tq, const double* wq, int n_q,
+                 const double* tx, const double* wx, int n_x,
+                 int cell_begin, int cell_end, int64_t* hitptr, int32_t* hitcell, int64_t cap)
+{
+    const int n_cells = Np * Nq;
+    if (cell_begin < 0 || cell_end > n_cells || cell_begin > cell_end) return -1;
+    const int nblk = cell_end - cell_begin;
+    for (int pass = 0; pass < 2; ++pass) {
+        if (pass == 1) {
+            hitptr[0] = 0;
+            for (int cb = 0; cb < nblk; ++cb) hitptr[cb + 1] += hitptr[cb];     /* counts -> offsets */
+            if (!hitcell) return 0;
+            if (hitptr[nblk] > cap) return -3;
+        }
+#pragma omp parallel
+        {
+            unsigned char* flag = (unsigned char*)malloc((size_t)n_cells);
+#pragma omp for schedule(dynamic, 8)
+            for (int cb = 0; cb < nblk; ++cb) {
+                int cell = cell_begin + cb, i = cell / Nq, j = cell % Nq;
+                memset(flag, 0, (size_t)n_cells);
+                for (int a = 0; a < n_p; ++a) for (int b = 0; b < n_q; ++b) for (int c = 0; c < n_x; ++c) {
+                    po_node nd;
+                    po_make_node(pe, Np, qe, Nq, i, j, tp[a], wp[a], tq[b], wq[b], tx[c], wx[c], &nd);
+                    if (nd.ic >= 0) flag[nd.ic * Nq + nd.jc] = 1;
+                }
+                if (pass == 0) {
+                    int64_t h = 0;
+                    for (int k = 0; k < n_cells; ++k) h += flag[k];
+                    hitptr[cb + 1] = h;
+                } else {
+                    int64_t pos = hitptr[cb];
+                    for (int k = 0; k < n_cells; ++k) if (flag[k]) hitcell[pos++] = k;
+                }
+            }
+            free(flag);
+        }
+    }
+    return 0;
+}
+
 int po_threads(void)
 {
 #ifdef _OPENMP

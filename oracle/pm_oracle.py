@@ -81,6 +81,9 @@ class Oracle:
         lib.po_build.argtypes = [_dp, C.c_int, _dp, C.c_int, _chp, C.c_int, C.c_int, C.c_int, C.c_int,
                                  _dp, _dp, C.c_int, _dp, _dp, C.c_int, _dp, _dp, C.c_int,
                                  C.c_int, C.c_int, _i64p, _i32p, _dp, C.c_int64, _i64p]
+        lib.po_hit_cells.restype = C.c_int
+        lib.po_hit_cells.argtypes = [_dp, C.c_int, _dp, C.c_int, _dp, _dp, C.c_int, _dp, _dp, C.c_int, _dp, _dp, C.c_int,
+                                     C.c_int, C.c_int, _i64p, _i32p, C.c_int64]
         lib.po_threads.restype = C.c_int
         lib.po_set_threads.argtypes = [C.c_int]
 
@@ -168,3 +171,39 @@ class Oracle:
         vals = np.empty(nnz.value, dtype=np.float64)
         call(colidx.ctypes.data_as(_i32p), _d(vals), nnz.value)
         return rowptr, colidx, vals
+
+    # ---- the geometric pattern alone ----
+    def hit_cells(self, wl, cell_begin=0, cell_end=None):
+        """(hitptr int64[n+1], hitcell int32[]) — the ascending hit cells of every source cell of the range (no values)."""
+        if cell_end is None:
+            cell_end = wl.n_cells
+        (tp, wp), (tq, wq), (tx, wx) = wl.rules["p"], wl.rules["q"], wl.rules["x"]
+        hitptr = np.zeros(cell_end - cell_begin + 1, dtype=np.int64)
+
+        def call(hc, cap):
+            rc = self.lib.po_hit_cells(_d(wl.p_edges), wl.Np, _d(wl.q_edges), wl.Nq, _d(tp), _d(wp), wl.n_p, _d(tq), _d(wq), wl.n_q,
+                                       _d(tx), _d(wx), wl.n_x, cell_begin, cell_end, hitptr.ctypes.data_as(_i64p), hc, cap)
+            if rc != 0:
+                raise RuntimeError(f"po_hit_cells failed: {rc}")
+
+        call(None, 0)
+        hitcell = np.empty(int(hitptr[-1]), dtype=np.int32)
+        call(hitcell.ctypes.data_as(_i32p), hitcell.size)
+        return hitptr, hitcell
+
+    # ---- scattered source cells, one po_build call per cell, several calls at a time ----
+    def build_cells(self, wl, cells, workers=None):
+        """[(rowptr, colidx, vals)] of the single-cell blocks `cells`.  po_build's OpenMP loop runs over the source cells of
+        ONE call, so a one-cell call uses one thread; here `workers` host threads (default: the OpenMP thread count) each
+        issue one-cell calls (ctypes releases the GIL), every call single-threaded.  The arithmetic is po_build's, untouched."""
+        from concurrent.futures import ThreadPoolExecutor
+        workers = workers or self.threads()
+
+        def one(c):
+            self.lib.po_set_threads(1)             # the calling thread's own setting
+            return self.build_csr(wl, int(c), int(c) + 1)
+
+        if workers <= 1:
+            return [one(c) for c in cells]
+        with ThreadPoolExecutor(max_workers=workers) as ex:
+            return list(ex.map(one, cells))

@@ -31,6 +31,12 @@ int next_pow2(int n) { int p = 1; while (p < n) p <<= 1; return p; }
 
 }  // namespace
 
+namespace pm {
+// used by the other translation units of the library (pm_stream.cu): every failing path leaves a message for pm_last_error()
+int32_t set_error(int32_t code, const std::string& msg) { return fail(code, msg); }
+int32_t set_cuda_error(cudaError_t e, const char* where) { cudaGetLastError(); return cuda_fail(e, where); }
+}  // namespace pm
+
 struct pm_lattice {
     int Np = 0, Nq = 0, n_ch = 0, J2 = 0, parity = 1, T2 = 0, stat = 0, n_p = 0, n_q = 0, n_x = 0;
     std::vector<double> pe, qe;
@@ -208,7 +214,7 @@ int32_t ensure_cell_scratch(pm_lattice* L, int n_blk)
 bool bad_edges(const double* e, int N)
 {
     if (!(e[0] >= 0.0)) return true;
-    for (int k = 0; k <= N; ++k) if (!std::isfinite(e[k])) return true;
+    for (int k = 0; k <= N; ++k) if (!std::isfinite(e[k]) || e[k] > 1e150) return true;      // e*e must stay finite
     for (int k = 0; k < N; ++k) if (!(e[k + 1] > e[k])) return true;
     return false;
 }
@@ -229,8 +235,9 @@ int32_t pm_lattice_create(const double* p_edges, int32_t Np, const double* q_edg
     if (!p_edges || !q_edges || !ch) return fail(PM_ERR_ARG, "NULL input pointer");
     if (Np < 1 || Nq < 1) return fail(PM_ERR_GRID, "need at least one cell per axis");
     if ((int64_t)Np * Nq > 262144) return fail(PM_ERR_GRID, "Np*Nq exceeds 262144");
-    if (bad_edges(p_edges, Np)) return fail(PM_ERR_GRID, "p_edges must be finite, strictly increasing, p_edges[0] >= 0");
-    if (bad_edges(q_edges, Nq)) return fail(PM_ERR_GRID, "q_edges must be finite, strictly increasing, q_edges[0] >= 0");
+    if ((int64_t)Np * Nq * Nq >= (int64_t(1) << 32)) return fail(PM_ERR_GRID, "Np*Nq*Nq must be below 2^32 (exact division of cell ids by Nq)");
+    if (bad_edges(p_edges, Np)) return fail(PM_ERR_GRID, "p_edges must be finite (at most 1e150), strictly increasing, p_edges[0] >= 0");
+    if (bad_edges(q_edges, Nq)) return fail(PM_ERR_GRID, "q_edges must be finite (at most 1e150), strictly increasing, q_edges[0] >= 0");
     if (n_ch < 1 || n_ch > PM_MAX_CHANNELS) return fail(PM_ERR_CHANNEL, "n_ch out of range");
     if (n_p < 1 || n_q < 1 || n_x < 1 || n_p > PM_MAX_ORDER || n_q > PM_MAX_ORDER || n_x > PM_MAX_ORDER)
         return fail(PM_ERR_ORDER, "quadrature order out of range 1..64");
@@ -444,10 +451,10 @@ int32_t fill_block(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const 
         if (e != cudaSuccess) return cuda_fail(e, "fill_plan");
         lat->have_plan = true;
     }
-    cudaEventRecord(lat->ev_fill0, st);
+    if ((e = cudaEventRecord(lat->ev_fill0, st)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
     e = pm::launch_fill(lat->dev, lat->plan, cell_begin, n_blk, lat->nl, d_rowptr, d_vals, d_colidx, lat->d_counter, st);
-    cudaEventRecord(lat->ev_fill1, st);
     if (e != cudaSuccess) return cuda_fail(e, "k_fill");
+    if ((e = cudaEventRecord(lat->ev_fill1, st)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
     lat->fill_timed = true;
     return PM_OK;
 }

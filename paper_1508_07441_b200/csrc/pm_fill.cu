@@ -3,6 +3,8 @@
 #include "pm_fill.cuh"
 
 #include <cstdlib>
+#include <map>
+#include <mutex>
 
 #include "gen/pm_spec_gen.cuh"
 #include "pm_jit.hpp"
@@ -27,6 +29,25 @@ const FillVariant kVariants[] = {
 };
 #undef PM_VAR
 #undef PM_SPEC
+
+// The dynamic shared-memory limit is an attribute of the kernel FUNCTION, shared by every lattice that selects it, while
+// the bytes a launch needs depend on the lattice (grids, orders): keep a per-function monotone maximum and raise it
+// before any launch that needs more (never lowered, so interleaved lattices of different shape cannot starve each other).
+std::mutex g_attr_mu;
+std::map<const void*, int> g_attr_max;
+
+cudaError_t ensure_smem_limit(const void* fn, int bytes)
+{
+    std::lock_guard<std::mutex> g(g_attr_mu);
+    int dev = 0;
+    cudaGetDevice(&dev);
+    const void* key = (const char*)fn + dev;              // per (function, device)
+    auto it = g_attr_max.find(key);
+    if (it != g_attr_max.end() && it->second >= bytes) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) g_attr_max[key] = bytes;
+    return e;
+}
 
 int preferred_warps()
 {
@@ -69,9 +90,9 @@ cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int n_sm, Fi
     out->name = best->name;
     out->jit = false;
     out->smem = fill_smem_plan(L, best->nw, best->rb);
-    cudaError_t e = cudaFuncSetAttribute(out->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, out->smem.total);
+    cudaError_t e = ensure_smem_limit(out->fn, out->smem.total);
     if (e != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(out->fn_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, out->smem.total)) != cudaSuccess) return e;
+    if ((e = ensure_smem_limit(out->fn_cols, out->smem.total)) != cudaSuccess) return e;
     int per_sm = 1;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, out->fn, best->nw * 32, (size_t)out->smem.total);
     if (e != cudaSuccess) return e;
@@ -108,10 +129,12 @@ cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin
     if (e != cudaSuccess) return e;
     void* args[] = {&Lc, &S, &N, &cell_begin, &n_blk, (void*)&rowptr, &vals, &colidx, &counter};
     if (F.jit) {
+        if (jit_prepare_fn(const_cast<void*>(colidx ? F.fn_cols : F.fn), S.total) != 0) return cudaErrorInvalidValue;
         const int cr = jit_launch(const_cast<void*>(colidx ? F.fn_cols : F.fn), grid, F.nw * 32, S.total, (void*)st, args);
         count_launch();
         return cr == 0 ? cudaGetLastError() : cudaErrorLaunchFailure;
     }
+    if ((e = ensure_smem_limit(colidx ? F.fn_cols : F.fn, S.total)) != cudaSuccess) return e;
     e = cudaLaunchKernel(colidx ? F.fn_cols : F.fn, dim3((unsigned)grid), dim3((unsigned)(F.nw * 32)), args, (size_t)S.total, st);
     count_launch();
     return e != cudaSuccess ? e : cudaGetLastError();

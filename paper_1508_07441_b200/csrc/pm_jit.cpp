@@ -42,11 +42,13 @@ struct Api {
     CUresult (*funcSetAttribute)(CUfunction, CUfunction_attribute, int) = nullptr;
     CUresult (*launchKernel)(CUfunction, unsigned, unsigned, unsigned, unsigned, unsigned, unsigned, unsigned, CUstream, void**, void**) = nullptr;
     CUresult (*occupancy)(int*, CUfunction, int, size_t) = nullptr;
+    CUresult (*ctxGetDevice)(int*) = nullptr;
 };
 
 Api g_api;
 std::mutex g_mu;
-std::map<std::string, JitFill> g_cache;          // key: hash / nw / rb
+std::map<std::string, JitFill> g_cache;          // key: device / hash / nw / rb (a CUfunction belongs to the context it was loaded in)
+std::map<void*, int> g_fn_smem;                  // per function: the dynamic shared-memory limit set so far
 bool g_enabled = std::getenv("PM_NO_JIT") == nullptr;
 
 template <class F>
@@ -83,7 +85,7 @@ bool load_driver()
     if (!hc) { a.why = "libcuda.so.1 not found"; return false; }
     a.ok_cu = sym(hc, "cuModuleLoadData", a.moduleLoadData, a.why) && sym(hc, "cuModuleGetFunction", a.moduleGetFunction, a.why)
         && sym(hc, "cuFuncSetAttribute", a.funcSetAttribute, a.why) && sym(hc, "cuLaunchKernel", a.launchKernel, a.why)
-        && sym(hc, "cuOccupancyMaxActiveBlocksPerMultiprocessor", a.occupancy, a.why);
+        && sym(hc, "cuOccupancyMaxActiveBlocksPerMultiprocessor", a.occupancy, a.why) && sym(hc, "cuCtxGetDevice", a.ctxGetDevice, a.why);
     return a.ok_cu;
 }
 
@@ -147,8 +149,10 @@ bool jit_fill(const Tables& T, unsigned long long hash, int nw, int rb, JitFill*
 {
     std::lock_guard<std::mutex> g(g_mu);
     if (!g_enabled) { err = "run-time compilation is disabled"; return false; }
-    char key[64];
-    std::snprintf(key, sizeof key, "%016llx/%d/%d", hash, nw, rb);
+    char key[80];
+    int dev = -1;
+    if (load_driver() && g_api.ctxGetDevice) g_api.ctxGetDevice(&dev);
+    std::snprintf(key, sizeof key, "%d/%016llx/%d/%d", dev, hash, nw, rb);
     auto it = g_cache.find(key);
     if (it != g_cache.end()) { *out = it->second; return true; }
     std::vector<char> cubin;
@@ -172,11 +176,22 @@ bool jit_fill(const Tables& T, unsigned long long hash, int nw, int rb, JitFill*
     return true;
 }
 
+int jit_prepare_fn(void* fn, int smem_bytes)
+{
+    std::lock_guard<std::mutex> g(g_mu);
+    if (!g_api.ok_cu) return -1;
+    auto it = g_fn_smem.find(fn);
+    if (it != g_fn_smem.end() && it->second >= smem_bytes) return 0;
+    if (g_api.funcSetAttribute((CUfunction)fn, CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, smem_bytes) != CUDA_SUCCESS) return -1;
+    g_fn_smem[fn] = smem_bytes;
+    return 0;
+}
+
 int jit_prepare(const JitFill& k, bool cols, int smem_bytes)
 {
     if (!g_api.ok_cu) return 0;
     CUfunction f = (CUfunction)(cols ? k.fn_cols : k.fn);
-    if (g_api.funcSetAttribute(f, CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, smem_bytes) != CUDA_SUCCESS) return 0;
+    if (jit_prepare_fn((void*)f, smem_bytes) != 0) return 0;
     int per_sm = 0;
     if (g_api.occupancy(&per_sm, f, k.nw * 32, (size_t)smem_bytes) != CUDA_SUCCESS) return 0;
     return per_sm;

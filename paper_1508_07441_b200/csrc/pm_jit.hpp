@@ -35,6 +35,10 @@ bool jit_compile_check(const Tables& T, int nw, int rb, size_t* cubin_bytes, std
 // cuFuncSetAttribute(max dynamic shared memory) + occupancy; returns CTAs per SM (0 on error)
 int jit_prepare(const JitFill& k, bool cols, int smem_bytes);
 
+// Raises (never lowers) the dynamic shared-memory limit of a run-time compiled function to at least `smem_bytes`;
+// returns 0 on success.  Called before every launch: the function is shared by all lattices with the same tables.
+int jit_prepare_fn(void* fn, int smem_bytes);
+
 // cuLaunchKernel on `stream` (a cudaStream_t); returns 0 on success, else a CUresult value
 int jit_launch(void* fn, int grid, int block, int smem_bytes, void* stream, void** args);
 

@@ -355,3 +355,29 @@ def test_single_p_node_is_the_two_axis_rule(oracle):
             nrm = math.sqrt((pe[i + 1] - pe[i]) * (qe[j + 1] - qe[j]) * (pe[ic + 1] - pe[ic]) * (qe[jc + 1] - qe[jc]))
             B[cell, t] += nd["w"][n] * nd["p"][n] * nd["q"][n] / (nd["pp"][n] * nd["qq"][n]) / nrm
     assert np.max(np.abs(A - B)) <= 1e-14 * np.max(np.abs(B))
+
+
+@pytest.mark.parametrize("wl", [I.config(1), RECT[0], RECT[2]], ids=lambda w: w.name)
+def test_hit_cells_is_the_geometric_pattern(oracle, wl):
+    """po_hit_cells (pattern without values) against the node table (unique targets per source cell) and against the
+    column indices of po_build; sub-ranges are slices of the whole."""
+    hp, hc = oracle.hit_cells(wl)
+    rp, ci, _ = oracle.build_csr(wl)
+    nc = wl.n_ch
+    assert hp[0] == 0 and len(hp) == wl.n_cells + 1 and hp[-1] == len(hc)
+    for cell in range(0, wl.n_cells, max(1, wl.n_cells // 97)):
+        t = oracle.cell_nodes(wl, cell)["target"]
+        assert np.array_equal(hc[hp[cell]:hp[cell + 1]], np.unique(t[t >= 0]))
+        assert np.array_equal(np.unique(ci[rp[cell * nc]:rp[cell * nc + 1]] // nc), hc[hp[cell]:hp[cell + 1]])
+    b, e = wl.n_cells // 5, wl.n_cells // 2
+    hp2, hc2 = oracle.hit_cells(wl, b, e)
+    assert np.array_equal(hp2, hp[b:e + 1] - hp[b]) and np.array_equal(hc2, hc[hp[b]:hp[e]])
+    assert oracle.hit_cells(wl, 3, 3)[0].tolist() == [0]
+
+
+def test_build_cells_is_build_csr_per_cell(oracle):
+    wl = I.small_coupled(N=5, jmax=2, orders=(3, 3, 5), Nq=6)
+    cells = [0, 7, 29, 13]
+    for (rp, ci, v), c in zip(oracle.build_cells(wl, cells, workers=3), cells):
+        rp2, ci2, v2 = oracle.build_csr(wl, c, c + 1)
+        assert np.array_equal(rp, rp2) and np.array_equal(ci, ci2) and np.array_equal(v, v2)
