@@ -44,7 +44,7 @@ enum {
     PM_ERR_NOMEM = -6, PM_ERR_STATE = -7, PM_ERR_OVERFLOW = -8, PM_ERR_DEVICE = -9
 };
 enum { PM_FERMION_ISOSPIN = 0, PM_SPINLESS_BOSON = 1 };      /* `statistics` */
-enum { PM_MAX_CHANNELS = 64, PM_MAX_ORDER = 64, PM_MAX_L = 8 };
+enum { PM_MAX_CHANNELS = 64, PM_MAX_ORDER = 64, PM_MAX_L = 12 };
 
 /* Create a lattice (host work only: validation, Gauss-Legendre rules, recoupling tables — PAPER.md:L247-256
  * step 1, 'calculation of algebraic coefficients g').
@@ -58,6 +58,15 @@ int32_t pm_lattice_create(const double* p_edges, int32_t Np, const double* q_edg
                           int32_t J2, int32_t parity, int32_t T2, int32_t statistics,
                           int32_t n_p, int32_t n_q, int32_t n_x, pm_lattice** out);
 int32_t pm_lattice_destroy(pm_lattice* lat);
+
+/* A lattice for ANOTHER channel set (another J^pi) on the grids, orders and rules of `base` (
+ * PAPER.md:L374 "up to 62 channels", L394 + Table 1 "all states ... up to J_max = 17/2").  The two share, by reference
+ * count, everything that does not depend on the channels: device tables of the grids and the node lists of the pattern
+ * pass.  pm_build_reuse on any lattice of such a group reuses the node lists the group already holds for that cell
+ * range, so a sweep over J^pi maps and sorts the quadrature nodes once.  pm_lattice_set_rule on one member changes the
+ * rule of all.  Each member is destroyed with pm_lattice_destroy, in any order.  Errors as pm_lattice_create. */
+int32_t pm_lattice_attach(pm_lattice* base, const pm_channel* ch, int32_t n_ch, int32_t J2, int32_t parity, int32_t T2,
+                          int32_t statistics, pm_lattice** out);
 
 /* M = n_ch*Np*Nq (matrix dimension) and the number of lattice cells. */
 int32_t pm_lattice_dims(const pm_lattice* lat, int64_t* M, int32_t* n_cells);
@@ -93,13 +102,38 @@ int32_t pm_pattern(pm_lattice* lat, int32_t cell_begin, int32_t cell_end,
 int32_t pm_fill(pm_lattice* lat, int32_t cell_begin, int32_t cell_end,
                 const int64_t* d_rowptr, double* d_vals, void* cuda_stream);
 
-/* Pattern and fill of one block in one call: the pattern pass up to rowptr and nnz (the stream is synchronised for
- * *nnz_host), then ONE kernel writes both the column index and the value of every nonzero — the separate column
- * kernel of pm_pattern is not run.  Same results as pm_pattern + pm_fill, bit for bit.
+/* Pattern and fill of one block in one call: the pattern pass up to rowptr and nnz, then ONE kernel writes both the
+ * column index and the value of every nonzero — the separate column kernel of pm_pattern is not run.  The kernels are
+ * queued back to back; the host reads nnz back once, after the fill has been queued (the capacity check runs on the device).  Same results as pm_pattern + pm_fill, bit for bit.
  *   d_rowptr, d_colidx, d_vals : device, as in pm_pattern / pm_fill;  capacity : entries d_colidx and d_vals can hold;
  *   PM_ERR_OVERFLOW (with *nnz_host valid, nothing written to d_colidx / d_vals) if nnz exceeds it. */
 int32_t pm_build(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int64_t* d_rowptr, int32_t* d_colidx, double* d_vals,
                  int64_t capacity, int64_t* nnz_host, void* cuda_stream);
+
+/* pm_build without any host synchronisation: the pattern pass, the capacity check and the fill are queued on the stream
+ * back to back; nnz stays on the device until pm_build_wait.  If the block's nnz exceeds `capacity` the fill kernel
+ * writes nothing (checked on the device) and pm_build_wait returns PM_ERR_OVERFLOW.  reuse_lists != 0: as pm_build_reuse.
+ * At most one un-waited build per lattice group: the next pattern / build call on the group waits for it first. */
+int32_t pm_build_async(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int64_t* d_rowptr, int32_t* d_colidx, double* d_vals,
+                       int64_t capacity, int32_t reuse_lists, void* cuda_stream);
+/* Waits for the pattern pass of the last pm_build_async (not for its fill kernel) and returns the block's nnz. */
+int32_t pm_build_wait(pm_lattice* lat, int64_t* nnz_host);
+
+/* pm_build that skips the node map and sort when the lattice group (pm_lattice_attach) already holds the node lists of
+ * [cell_begin, cell_end) from its last pattern / build call; otherwise identical to pm_build, bit for bit. */
+int32_t pm_build_reuse(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int64_t* d_rowptr, int32_t* d_colidx, double* d_vals,
+                       int64_t capacity, int64_t* nnz_host, void* cuda_stream);
+
+/* ---- Sharded build over several GPUs (the elements are "calculated ... fully
+ * independently from each other").  Rows of different source cells are independent, so every rank builds a contiguous
+ * range of source cells; the only exchange is one all-gather of the per-rank nnz (8 bytes), done by the caller.
+ *   pm_pattern_cell_hits : hit cells of every source cell of the last pm_pattern / pm_build call, h_hits[cell_end-cell_begin] (HOST out)
+ *   pm_partition_cells   : host only.  cuts[n_parts+1] with cuts[0] = 0, cuts[n_parts] = n_cells: contiguous ranges of
+ *                          (almost) equal weight sum(hits[k] + cell_cost); deterministic, identical on every rank
+ *   pm_rowptr_offset     : d_rowptr[0..n) += offset (block-local row pointers -> global ones)                         */
+int32_t pm_pattern_cell_hits(pm_lattice* lat, int32_t* h_hits, void* cuda_stream);
+int32_t pm_partition_cells(const int32_t* hits, int32_t n_cells, double cell_cost, int32_t n_parts, int32_t* cuts);
+int32_t pm_rowptr_offset(int64_t* d_rowptr, int64_t n, int64_t offset, void* cuda_stream);
 
 /* y = P0 x for the WHOLE lattice without reading column indices: the columns of row (cell, alpha) are implied by the
  * hit cells of the source cell and the coupled-channel list, which the lattice keeps from its last pm_pattern /
@@ -130,6 +164,13 @@ int32_t pm_spmv(pm_lattice* lat, int64_t n_rows, const int64_t* d_rowptr, const 
  * Both are asynchronous on `cuda_stream`. */
 int32_t pm_block_apply(pm_lattice* lat, const double* d_blocks, const double* d_diag, const double* d_in, double* d_out,
                        void* cuda_stream);
+/* the same with the transposed blocks: d_out[(i,j,a)] = sum_i' B_a[i'][i] * d_in[(i',j,a)] */
+int32_t pm_block_apply_t(pm_lattice* lat, const double* d_blocks, const double* d_in, double* d_out, void* cuda_stream);
+/* Rotation to the channel basis, eq. (20): P = O P0 O^T applied to a vector,
+ * d_out = O (P0 (O^T x)); O as in pm_block_apply (one orthogonal (Np x Np) block per channel); d_work: 2*M doubles;
+ * d_colidx may be NULL (columns from the hit lists, as pm_spmv_implicit). */
+int32_t pm_rotate_apply(pm_lattice* lat, const int64_t* d_rowptr, const int32_t* d_colidx, const double* d_vals,
+                        const double* d_O, const double* d_x, double* d_out, double* d_work, void* cuda_stream);
 int32_t pm_kernel_apply(pm_lattice* lat, const int64_t* d_rowptr, const int32_t* d_colidx, const double* d_vals,
                         const double* d_O, const double* d_Vt, const double* d_g1, const double* d_u, double* d_out,
                         double* d_work, void* cuda_stream);

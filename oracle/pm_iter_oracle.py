@@ -41,3 +41,20 @@ def kernel_apply(rowptr, colidx, vals, O, V1, g1, u, Np, Nq, n_ch) -> np.ndarray
     y = block_apply(vtilde(O, V1), y, Np, Nq, n_ch)
     y = csr_matvec(rowptr, colidx, vals, y)
     return block_apply(O, y, Np, Nq, n_ch)
+
+
+def block_apply_t(B: np.ndarray, x: np.ndarray, Np: int, Nq: int, n_ch: int) -> np.ndarray:
+    """y[(i,j,a)] = sum_i' B[a][i'][i] x[(i',j,a)] — the transposed blocks."""
+    x3 = x.reshape(Np, Nq, n_ch)
+    y3 = np.empty_like(x3)
+    for a in range(n_ch):
+        y3[:, :, a] = B[a].T @ x3[:, :, a]
+    return y3.reshape(-1)
+
+
+def rotate_apply(rowptr, colidx, vals, O, x, Np, Nq, n_ch) -> np.ndarray:
+    """P x with P = O P0 O^T, eq. (20): the permutation matrix rotated from the lattice (free
+    wave-packet) basis to the channel basis, applied factor by factor, right to left."""
+    y = block_apply_t(O, x, Np, Nq, n_ch)
+    y = csr_matvec(rowptr, colidx, vals, y)
+    return block_apply(O, y, Np, Nq, n_ch)

@@ -24,7 +24,8 @@ ERRORS = {-1: "PM_ERR_ARG", -2: "PM_ERR_GRID", -3: "PM_ERR_CHANNEL", -4: "PM_ERR
 EXPORTS = ["pm_lattice_create", "pm_lattice_destroy", "pm_lattice_dims", "pm_lattice_rule", "pm_lattice_set_rule",
            "pm_lattice_coupling", "pm_lattice_work", "pm_pattern_counts", "pm_lattice_fill_kernel", "pm_set_jit", "pm_diag_jit_compile", "pm_diag_sqrt_threshold",
            "pm_diag_dfma_tflops", "pm_pattern", "pm_fill", "pm_build", "pm_last_fill_ms", "pm_block_apply", "pm_kernel_apply", "pm_spmv_implicit", "pm_spmv", "pm_build_host_count", "pm_build_host",
-           "pm_launch_count", "pm_last_error"]
+           "pm_launch_count", "pm_last_error", "pm_lattice_attach", "pm_build_async", "pm_build_wait", "pm_build_reuse",
+           "pm_pattern_cell_hits", "pm_partition_cells", "pm_rowptr_offset", "pm_block_apply_t", "pm_rotate_apply"]
 
 
 class PmError(RuntimeError):
@@ -55,6 +56,15 @@ def lib():
                                     C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
                                     C.POINTER(_vp)]
     L.pm_lattice_destroy.argtypes = [_vp]
+    L.pm_lattice_attach.argtypes = [_vp, C.POINTER(_Channel), C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.POINTER(_vp)]
+    L.pm_build_async.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, _vp, C.c_int64, C.c_int32, _vp]
+    L.pm_build_wait.argtypes = [_vp, _i64p]
+    L.pm_build_reuse.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, _vp, C.c_int64, _i64p, _vp]
+    L.pm_pattern_cell_hits.argtypes = [_vp, _i32p, _vp]
+    L.pm_partition_cells.argtypes = [_i32p, C.c_int32, C.c_double, C.c_int32, _i32p]
+    L.pm_rowptr_offset.argtypes = [_vp, C.c_int64, C.c_int64, _vp]
+    L.pm_block_apply_t.argtypes = [_vp, _vp, _vp, _vp, _vp]
+    L.pm_rotate_apply.argtypes = [_vp] + [_vp] * 8
     L.pm_lattice_dims.argtypes = [_vp, _i64p, _i32p]
     L.pm_lattice_rule.argtypes = [_vp, C.c_int32, _dp, _dp]
     L.pm_lattice_set_rule.argtypes = [_vp, C.c_int32, _dp, _dp]
@@ -110,6 +120,14 @@ def pm_lattice_create(p_edges, q_edges, channels, J2, parity, T2, statistics, n_
     _check(lib().pm_lattice_create(_d(pe), len(pe) - 1, _d(qe), len(qe) - 1, ch, len(channels),
                                    int(J2), int(parity), int(T2), int(statistics), int(n_p), int(n_q), int(n_x),
                                    C.byref(h)))
+    return h
+
+
+def pm_lattice_attach(base, channels, J2, parity, T2, statistics):
+    """Another channel set (another J^pi) on the grids and rules of `base`; shares its geometric pattern."""
+    ch = (_Channel * len(channels))(*[_Channel(*(int(c[k]) for k in ("l", "s", "j", "t", "lam", "I2"))) for c in channels])
+    h = _vp()
+    _check(lib().pm_lattice_attach(base, ch, len(channels), int(J2), int(parity), int(T2), int(statistics), C.byref(h)))
     return h
 
 
@@ -200,6 +218,55 @@ def pm_build(h, cell_begin, cell_end, d_rowptr, d_colidx, d_vals, stream=None):
     _check(lib().pm_build(h, cell_begin, cell_end, d_rowptr.data_ptr(), d_colidx.data_ptr(), d_vals.data_ptr(),
                           min(d_colidx.numel(), d_vals.numel()), C.byref(nnz), _stream_ptr(stream)))
     return nnz.value
+
+
+def pm_build_reuse(h, cell_begin, cell_end, d_rowptr, d_colidx, d_vals, stream=None):
+    """pm_build that reuses the node lists the lattice group already holds for this cell range.  Returns nnz."""
+    nnz = C.c_int64()
+    _check(lib().pm_build_reuse(h, cell_begin, cell_end, d_rowptr.data_ptr(), d_colidx.data_ptr(), d_vals.data_ptr(),
+                                min(d_colidx.numel(), d_vals.numel()), C.byref(nnz), _stream_ptr(stream)))
+    return nnz.value
+
+
+def pm_build_async(h, cell_begin, cell_end, d_rowptr, d_colidx, d_vals, reuse_lists=False, stream=None):
+    """Queues pattern + fill on the stream without any host synchronisation; pm_build_wait returns nnz."""
+    _check(lib().pm_build_async(h, cell_begin, cell_end, d_rowptr.data_ptr(), d_colidx.data_ptr(), d_vals.data_ptr(),
+                                min(d_colidx.numel(), d_vals.numel()), 1 if reuse_lists else 0, _stream_ptr(stream)))
+
+
+def pm_build_wait(h):
+    nnz = C.c_int64()
+    _check(lib().pm_build_wait(h, C.byref(nnz)))
+    return nnz.value
+
+
+def pm_pattern_cell_hits(h, n_cells_in_block, stream=None):
+    """Hit cells per source cell of the last pattern / build call (numpy int32)."""
+    out = np.empty(n_cells_in_block, dtype=np.int32)
+    _check(lib().pm_pattern_cell_hits(h, out.ctypes.data_as(_i32p), _stream_ptr(stream) if n_cells_in_block else None))
+    return out
+
+
+def pm_partition_cells(hits, n_parts, cell_cost=0.0):
+    """cuts[n_parts+1]: contiguous source-cell ranges of (almost) equal weight sum(hits + cell_cost).  Host only."""
+    h = np.ascontiguousarray(hits, dtype=np.int32)
+    cuts = np.empty(n_parts + 1, dtype=np.int32)
+    _check(lib().pm_partition_cells(h.ctypes.data_as(_i32p), len(h), float(cell_cost), int(n_parts), cuts.ctypes.data_as(_i32p)))
+    return cuts
+
+
+def pm_rowptr_offset(d_rowptr, offset, stream=None):
+    _check(lib().pm_rowptr_offset(d_rowptr.data_ptr(), d_rowptr.numel(), int(offset), _stream_ptr(stream)))
+
+
+def pm_block_apply_t(h, d_blocks, d_in, d_out, stream=None):
+    _check(lib().pm_block_apply_t(h, d_blocks.data_ptr(), d_in.data_ptr(), d_out.data_ptr(), _stream_ptr(stream)))
+
+
+def pm_rotate_apply(h, d_rowptr, d_colidx, d_vals, d_O, d_x, d_out, d_work, stream=None):
+    """d_out = O P0 O^T x (eq. 20); d_work holds 2*M doubles."""
+    _check(lib().pm_rotate_apply(h, d_rowptr.data_ptr(), d_colidx.data_ptr() if d_colidx is not None else None, d_vals.data_ptr(),
+                                 d_O.data_ptr(), d_x.data_ptr(), d_out.data_ptr(), d_work.data_ptr(), _stream_ptr(stream)))
 
 
 def pm_spmv_implicit(h, d_rowptr, d_vals, d_x, d_y, stream=None):

@@ -34,6 +34,7 @@ struct DevLattice {
     const double *thr_p, *thr_q;                // sqrt_threshold(edge), padded with +inf to a power of two
     const unsigned short *bk_p, *bk_q;          // kBuckets entries each: first threshold a value of that bucket can meet
     int bk_hmin_p, bk_sh_p, bk_hmin_q, bk_sh_q; // bucket(v) = clamp((hi32(v) - hmin) >> sh, 0, kBuckets-1)
+    int bk_kmax;                                // most thresholds any bucket of either axis holds
     const double *tp, *wp, *tq, *wq, *tx, *wx;  // Gauss-Legendre rules on [-1,1]
     const double *sx;                           // sqrt(1-x^2) per x-node
     const int *cl_off, *cl, *o_alpha;           // coupled lists; o_alpha[o] = alpha of output o
@@ -45,15 +46,13 @@ struct DevLattice {
 };
 
 // Per-source-cell node lists written by the pattern pass and read by the fill pass (library-owned scratch), stride
-// nnode per source cell: for every node that hit the grid, in the order (rank of target cell, node id),
-//   key   = target cell << 14 | node id     (node id m = c*(n_p*n_q) + a*n_q + b < 2^14, cell < 2^18)
-//   rkpos = rank of the target cell among the source cell's hit cells.
+// nnode per source cell: for every node that hit the grid, in the order (target cell, node id),
+//   key   = target cell << 14 | node id     (node id m = c*(n_p*n_q) + a*n_q + b < 2^14, cell < 2^18).
+// The rank of a target among the source cell's hit cells is the number of target changes before it.
 struct NodeLists {
     unsigned* key;              // [n_blk][nnode]
-    unsigned short* rkpos;      // [n_blk][nnode]
     int* ntot;                  // [n_blk] nodes on the grid
     int* hits;                  // [n_blk] hit cells H
-    int* nseg;                  // [n_blk] (target, x-node) segments of the sorted list
 };
 
 struct CellGeom { double cp, hp, cq, hq; };
@@ -104,59 +103,31 @@ __device__ __forceinline__ int locate(const double* __restrict__ thr, const unsi
     return i - 1;
 }
 
+// The same count when no bucket holds more than K thresholds: K independent comparisons instead of a dependent scan
+// (the tables carry K entries of +inf behind the last threshold).
+template <int K>
+__device__ __forceinline__ int locate_k(const double* __restrict__ thr, const unsigned short* __restrict__ start, int hmin, int sh, double v)
+{
+    const int b = max(0, min(kBuckets - 1, (__double2hiint(v) - hmin) >> sh));
+    const int i = start[b];
+    int c = 0;
+#pragma unroll
+    for (int k = 0; k < K; ++k) c += (thr[i + k] <= v) ? 1 : 0;
+    return i + c - 1;
+}
+
+constexpr int kLocK = 4;
+
 struct Locator { const double *thr_p, *thr_q; const unsigned short *bk_p, *bk_q; int hmin_p, sh_p, hmin_q, sh_q, Np, Nq; };
 
 // target cell of a mapped node, or -1 (outside the grid, or p' = 0 / q' = 0): readings R5, R6.  sqrt(y) = 0 <=> y = 0.
+template <bool kFast>
 __device__ __forceinline__ int target_cell_sq(const Locator& lc, double P2, double Q2)
 {
-    const int ic = locate(lc.thr_p, lc.bk_p, lc.hmin_p, lc.sh_p, P2), jc = locate(lc.thr_q, lc.bk_q, lc.hmin_q, lc.sh_q, Q2);
+    const int ic = kFast ? locate_k<kLocK>(lc.thr_p, lc.bk_p, lc.hmin_p, lc.sh_p, P2) : locate(lc.thr_p, lc.bk_p, lc.hmin_p, lc.sh_p, P2);
+    const int jc = kFast ? locate_k<kLocK>(lc.thr_q, lc.bk_q, lc.hmin_q, lc.sh_q, Q2) : locate(lc.thr_q, lc.bk_q, lc.hmin_q, lc.sh_q, Q2);
     const bool ok = (ic >= 0) & (ic < lc.Np) & (jc >= 0) & (jc < lc.Nq) & (P2 != 0.0) & (Q2 != 0.0);
     return ok ? ic * lc.Nq + jc : -1;
-}
-
-// In-place exclusive scan of n ints in shared memory by the whole block; returns the total.
-// `scratch` holds blockDim.x + 1 ints.  All threads must call.
-__device__ inline int block_exclusive_scan(int* data, int n, int* scratch)
-{
-    const int T = blockDim.x, t = threadIdx.x;
-    const int chunk = (n + T - 1) / T;
-    const int b = min(t * chunk, n), e = min(b + chunk, n);
-    int s = 0;
-    for (int k = b; k < e; ++k) s += data[k];
-    scratch[t] = s;
-    __syncthreads();
-    if (t < 32) {
-        int carry = 0;
-        for (int base = 0; base < T; base += 32) {
-            int v = scratch[base + t], x = v;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, d); if (t >= d) x += y; }
-            scratch[base + t] = carry + x - v;
-            carry += __shfl_sync(0xffffffffu, x, 31);
-        }
-        if (t == 0) scratch[T] = carry;
-    }
-    __syncthreads();
-    int run = scratch[t];
-    for (int k = b; k < e; ++k) { int v = data[k]; data[k] = run; run += v; }
-    const int total = scratch[T];
-    __syncthreads();
-    return total;
-}
-
-// hit bitset of one source cell with word-prefix popcounts (ranks of the hit cells)
-struct HitSet { unsigned* bits; int* wpre; int* scratch; };
-
-__device__ inline int rank_bits_n(int n_words, const HitSet& s)
-{
-    for (int k = threadIdx.x; k < n_words; k += blockDim.x) s.wpre[k] = __popc(s.bits[k]);
-    __syncthreads();
-    return block_exclusive_scan(s.wpre, n_words, s.scratch);
-}
-
-__device__ __forceinline__ int rank_of(const HitSet& s, int t)
-{
-    return s.wpre[t >> 5] + __popc(s.bits[t >> 5] & ((1u << (t & 31)) - 1u));
 }
 
 }  // namespace pm

@@ -16,7 +16,7 @@ namespace {
 
 constexpr int kSmemLimit = 227 * 1024;
 
-using FillKernel = void (*)(DevLattice, FillSmem, NodeLists, int, int, const int64_t*, double*, int32_t*, int*);
+using FillKernel = void (*)(DevLattice, FillSmem, NodeLists, int, int, const int64_t*, double*, int32_t*, int*, const int64_t*);
 
 struct FillVariant { unsigned long long hash; int nw, rb; FillKernel fn, fn_cols; const char* name; };
 
@@ -118,7 +118,7 @@ bool fill_plan_jit(const DevLattice& L, const Tables& T, unsigned long long hash
 }
 
 cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl,
-                        const int64_t* rowptr, double* vals, int32_t* colidx, int* counter, cudaStream_t st)
+                        const int64_t* rowptr, double* vals, int32_t* colidx, int* counter, const int64_t* guard, cudaStream_t st)
 {
     const int need = (n_blk + F.nw - 1) / F.nw;                        // one cell per warp at a time
     const int grid = need < F.grid ? need : F.grid;
@@ -127,7 +127,7 @@ cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin
     NodeLists N = nl;
     cudaError_t e = cudaMemsetAsync(counter, 0, sizeof(int), st);      // the work counter the warps draw cells from
     if (e != cudaSuccess) return e;
-    void* args[] = {&Lc, &S, &N, &cell_begin, &n_blk, (void*)&rowptr, &vals, &colidx, &counter};
+    void* args[] = {&Lc, &S, &N, &cell_begin, &n_blk, (void*)&rowptr, &vals, &colidx, &counter, (void*)&guard};
     if (F.jit) {
         if (jit_prepare_fn(const_cast<void*>(colidx ? F.fn_cols : F.fn), S.total) != 0) return cudaErrorInvalidValue;
         const int cr = jit_launch(const_cast<void*>(colidx ? F.fn_cols : F.fn), grid, F.nw * 32, S.total, (void*)st, args);

@@ -79,8 +79,11 @@ inline FillSmem fill_smem_plan(const DevLattice& L, int nw, int row_batch)
 template <class Spec, int NW, int kRowBatch, bool kCols>
 __global__ void __launch_bounds__(NW * 32, 1)
 k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, const int64_t* __restrict__ rowptr,
-            double* __restrict__ vals, int32_t* __restrict__ colidx, int* __restrict__ counter)
+            double* __restrict__ vals, int32_t* __restrict__ colidx, int* __restrict__ counter, const int64_t* __restrict__ guard)
 {
+    // pm_build launches this kernel before the host has seen nnz: the scan kernel left guard[4] != 0 when the block's
+    // nnz exceeds the caller's capacity, and then nothing may be written
+    if (guard != nullptr && guard[4] != 0) return;
     constexpr int T = NW * 32;
     constexpr int NP = (Spec::NS + 1) / 2;              // slot pairs (one double2 per pair and node in the K tile)
     constexpr int NPC = (NP + 31) / 32;                 // pair chunks of the lane = slot-pair walk

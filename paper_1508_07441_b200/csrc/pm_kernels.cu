@@ -21,183 +21,195 @@ __device__ __forceinline__ char* carve(char*& p, size_t bytes)
 static size_t al16(size_t b) { return (b + 15) & ~size_t(15); }
 
 // ------------------------------------------------------------------------------------------------
-// Pattern pass, kernel A: map every node of a source cell, rank the hit cells, stable counting sort of the
-// node ids by rank.  Node id m = c*(n_p*n_q) + a*n_q + b, so the sorted list is ordered by (target, x-node, a, b).
+// Pattern pass, kernel A: ONE WARP per source cell (cells drawn from a work counter, tables staged once per CTA, no
+// block barrier after start-up).  Pass 1 maps every node (exact ops, bucketed location), marks the hit cells in a bitset
+// and keeps each node's target in shared memory; word-prefix popcounts turn a target into its rank; pass 2 counts the
+// nodes per rank, pass 3 places the node ids in node order (a stable counting sort).  Node id m = c*(n_p*n_q) + a*n_q + b,
+// so the sorted list is ordered by (target, x-node, a, b).  Lanes that meet the same rank in a step are grouped with
+// match_any (32 consecutive nodes fall into one to three targets), so no shared-memory atomics are needed for the counts.
+// Ranks are processed in windows of kHistCap counters: one window for every realistic lattice, any number otherwise.
 // ------------------------------------------------------------------------------------------------
-size_t map_sort_smem(const DevLattice& L, int hits_fast)
+MapSortSmem map_sort_plan(const DevLattice& L, int max_warps)
 {
-    const int nw = kThreads / 32;
-    const int hcap = std::min(L.nnode, L.n_cells);
-    return al16(8 * (size_t)L.pe_pad) + al16(8 * (size_t)L.qe_pad) + 2 * al16(2 * (size_t)kBuckets) + al16(8 * (size_t)L.n_p) + al16(8 * (size_t)L.n_q)
-         + al16(8 * (size_t)L.n_x) + 2 * al16(4 * (size_t)L.n_words) + al16(4 * (size_t)(kThreads + 1))
-         + al16(4 * (size_t)L.nnode) + al16(2 * (size_t)L.nnode) + al16(4 * (size_t)(hcap + 1))
-         + al16(4 * (size_t)std::max(nw * std::min(hcap, hits_fast), hcap));
+    // rank counters per window (PM_HIST_CAP: test hook that forces several windows on small lattices)
+    static const int hist_cap = [] { const char* e = std::getenv("PM_HIST_CAP"); return e ? std::max(1, std::min(kHistCap, std::atoi(e))) : kHistCap; }();
+    MapSortSmem S{};
+    S.hist_cap = hist_cap;
+    int o = 0;
+    auto take = [&](size_t bytes) { int r = o; o += (int)al16(bytes); return r; };
+    S.thr_p = take(8 * (size_t)(L.pe_pad + kLocK)); S.thr_q = take(8 * (size_t)(L.qe_pad + kLocK));      // + sentinels of locate_k
+    S.bk_p = take(2 * (size_t)kBuckets); S.bk_q = take(2 * (size_t)kBuckets);
+    S.tp = take(8 * (size_t)L.n_p); S.tq = take(8 * (size_t)L.n_q); S.tx = take(8 * (size_t)L.n_x);
+    S.wide = L.n_cells > 65535 ? 1 : 0;                 // targets kept as 16-bit ids when they fit
+    int w = 0;
+    auto wtake = [&](size_t bytes) { int r = w; w += (int)al16(bytes); return r; };
+    S.w_bits = wtake(4 * (size_t)L.n_words);
+    S.w_wpre = wtake(2 * (size_t)L.n_words);
+    S.w_t = wtake((S.wide ? 4 : 2) * (size_t)L.nnode);
+    S.w_hist = wtake(4 * (size_t)S.hist_cap);
+    S.warp_bytes = w;
+    const int room = 227 * 1024 - o;
+    S.nw = std::max(0, std::min(max_warps, room / w));
+    S.warp0 = take((size_t)w * std::max(S.nw, 1));
+    S.total = o;
+    return S;
 }
 
-__global__ void __launch_bounds__(kThreads) k_map_sort(DevLattice L, int cell_begin, NodeLists nl, int hits_fast)
+template <class TT, bool kFast>
+__global__ void __launch_bounds__(kMapSortMaxWarps * 32, 1)
+k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl, int* __restrict__ counter)
 {
     extern __shared__ __align__(16) char smem[];
-    constexpr int T = kThreads, NW = kThreads / 32;
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int hcap = min(L.nnode, L.n_cells);
-    char* sp = smem;
-    double* s_thr_p = (double*)carve(sp, 8 * (size_t)L.pe_pad);
-    double* s_thr_q = (double*)carve(sp, 8 * (size_t)L.qe_pad);
-    unsigned short* s_bk_p = (unsigned short*)carve(sp, 2 * (size_t)kBuckets);
-    unsigned short* s_bk_q = (unsigned short*)carve(sp, 2 * (size_t)kBuckets);
-    double* s_tp = (double*)carve(sp, 8 * (size_t)L.n_p);
-    double* s_tq = (double*)carve(sp, 8 * (size_t)L.n_q);
-    double* s_tx = (double*)carve(sp, 8 * (size_t)L.n_x);
-    HitSet hs;
-    hs.bits = (unsigned*)carve(sp, 4 * (size_t)L.n_words);
-    hs.wpre = (int*)carve(sp, 4 * (size_t)L.n_words);
-    hs.scratch = (int*)carve(sp, 4 * (size_t)(T + 1));
-    int* s_tgt = (int*)carve(sp, 4 * (size_t)L.nnode);
-    unsigned short* s_rk = (unsigned short*)carve(sp, 2 * (size_t)L.nnode);     // rank of each node's target (0xffff: off the grid)
-    int* s_start = (int*)carve(sp, 4 * (size_t)(hcap + 1));
-    int* s_hist = (int*)carve(sp, 4 * (size_t)max(NW * min(hcap, hits_fast), hcap));
+    constexpr unsigned kOff = (unsigned)(TT)~(TT)0;             // marker of a node that left the grid
+    const int T = blockDim.x, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    double* s_thr_p = (double*)(smem + S.thr_p); double* s_thr_q = (double*)(smem + S.thr_q);
+    unsigned short* s_bk_p = (unsigned short*)(smem + S.bk_p); unsigned short* s_bk_q = (unsigned short*)(smem + S.bk_q);
+    double* s_tp = (double*)(smem + S.tp); double* s_tq = (double*)(smem + S.tq); double* s_tx = (double*)(smem + S.tx);
+    char* wsm = smem + S.warp0 + warp * S.warp_bytes;
+    unsigned* bits = (unsigned*)(wsm + S.w_bits);
+    unsigned short* wpre = (unsigned short*)(wsm + S.w_wpre);
+    TT* s_t = (TT*)(wsm + S.w_t);
+    int* hist = (int*)(wsm + S.w_hist);
 
-    for (int k = tid; k < L.pe_pad; k += T) s_thr_p[k] = L.thr_p[k];
-    for (int k = tid; k < L.qe_pad; k += T) s_thr_q[k] = L.thr_q[k];
+    for (int k = tid; k < L.pe_pad + kLocK; k += T) s_thr_p[k] = k < L.pe_pad ? L.thr_p[k] : __longlong_as_double(0x7ff0000000000000ll);
+    for (int k = tid; k < L.qe_pad + kLocK; k += T) s_thr_q[k] = k < L.qe_pad ? L.thr_q[k] : __longlong_as_double(0x7ff0000000000000ll);
     for (int k = tid; k < kBuckets; k += T) { s_bk_p[k] = L.bk_p[k]; s_bk_q[k] = L.bk_q[k]; }
-    const Locator lc{s_thr_p, s_thr_q, s_bk_p, s_bk_q, L.bk_hmin_p, L.bk_sh_p, L.bk_hmin_q, L.bk_sh_q, L.Np, L.Nq};
     for (int k = tid; k < L.n_p; k += T) s_tp[k] = L.tp[k];
     for (int k = tid; k < L.n_q; k += T) s_tq[k] = L.tq[k];
     for (int k = tid; k < L.n_x; k += T) s_tx[k] = L.tx[k];
-    for (int k = tid; k < L.n_words; k += T) hs.bits[k] = 0u;
-    const int cell = cell_begin + blockIdx.x;
-    const int ci = cell / L.Nq, cj = cell - ci * L.Nq;
-    const CellGeom g = cell_geom(L.pe, L.qe, ci, cj);
-    __syncthreads();
+    const Locator lc{s_thr_p, s_thr_q, s_bk_p, s_bk_q, L.bk_hmin_p, L.bk_sh_p, L.bk_hmin_q, L.bk_sh_q, L.Np, L.Nq};
+    __syncthreads();                                            // the only block-level barrier
 
-    for (int m = tid; m < L.nnode; m += T) {
-        int c, a, b;
-        split_node(L, m, c, a, b);
-        double p, q, P2, Q2;
-        map_node_sq(g, s_tp[a], s_tq[b], s_tx[c], p, q, P2, Q2);
-        const int t = target_cell_sq(lc, P2, Q2);
-        if (t >= 0) atomicOr(&hs.bits[t >> 5], 1u << (t & 31));
-        s_tgt[m] = t;
-    }
-    __syncthreads();
-    const int H = rank_bits_n(L.n_words, hs);
-    // stable counting sort: each of `nwe` warps owns a contiguous slice of node ids and a histogram of H counters
-    // (all warps when H <= hits_fast, else warp 0 alone: rare, slow, same result)
-    const int nwe = (H <= hits_fast) ? NW : 1;
-    for (int k = tid; k < nwe * H; k += T) s_hist[k] = 0;
-    __syncthreads();
-    const int slice = (((L.nnode + nwe - 1) / nwe) + 31) & ~31;
-    const int nb = min(warp * slice, L.nnode), ne = (warp < nwe) ? min(nb + slice, L.nnode) : nb;
-    for (int m = nb + lane; m < ne; m += 32) {
-        const int t = s_tgt[m];
-        const int r = (t >= 0) ? rank_of(hs, t) : 0xffff;
-        s_rk[m] = (unsigned short)r;
-        if (t >= 0) atomicAdd(&s_hist[warp * H + r], 1);
-    }
-    __syncthreads();
-    for (int k = tid; k < H; k += T) {
-        int tot = 0;
-        for (int w = 0; w < nwe; ++w) tot += s_hist[w * H + k];
-        s_start[k] = tot;
-    }
-    if (tid == 0) s_start[H] = 0;
-    __syncthreads();
-    const int ntot = block_exclusive_scan(s_start, H + 1, hs.scratch);
-    for (int k = tid; k < H; k += T) {
-        int run = s_start[k];
-        for (int w = 0; w < nwe; ++w) { const int v = s_hist[w * H + k]; s_hist[w * H + k] = run; run += v; }
-    }
-    __syncthreads();
-    // placement straight into the node lists (scattered 4- and 2-byte stores inside the cell's 19 KB; L2 merges them)
-    unsigned* g_key = nl.key + (size_t)blockIdx.x * L.nnode;
-    unsigned short* g_rkpos = nl.rkpos + (size_t)blockIdx.x * L.nnode;
-    for (int m0 = nb; m0 < ne; m0 += 32) {
-        const int m = m0 + lane;
-        const int key = (m < ne) ? (int)s_rk[m] : 0xffff;
-        const unsigned same = __match_any_sync(0xffffffffu, key);
-        if (key != 0xffff) {
-            const int pos = s_hist[warp * H + key] + __popc(same & ((1u << lane) - 1u));
-            g_key[pos] = ((unsigned)s_tgt[m] << 14) | (unsigned)m;
-            g_rkpos[pos] = (unsigned short)key;
+    const unsigned lt = (1u << lane) - 1u;
+    const int wchunk = (L.n_words + 31) >> 5;                   // bitset words per lane in the rank prefix
+    const int nsteps = (L.nnode + 31) >> 5;
+    for (;;) {
+        int cb = 0;
+        if (lane == 0) cb = atomicAdd(counter, 1);
+        cb = __shfl_sync(0xffffffffu, cb, 0);
+        if (cb >= n_blk) break;
+        const int cell = cell_begin + cb;
+        const int ci = cell / L.Nq, cj = cell - ci * L.Nq;
+        const CellGeom g = cell_geom(L.pe, L.qe, ci, cj);
+        for (int k = lane; k < L.n_words; k += 32) bits[k] = 0u;
+        __syncwarp();
+        // ---- pass 1: map, locate, mark (two independent nodes per lane and iteration)
+        for (int m0 = lane; m0 < L.nnode; m0 += 64) {
+            int t[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int m = min(m0 + 32 * u, L.nnode - 1);
+                int c, a, b;
+                split_node(L, m, c, a, b);
+                double p, q, P2, Q2;
+                map_node_sq(g, s_tp[a], s_tq[b], s_tx[c], p, q, P2, Q2);
+                t[u] = target_cell_sq<kFast>(lc, P2, Q2);
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int m = m0 + 32 * u;
+                if (m < L.nnode) {
+                    if (t[u] >= 0) atomicOr(&bits[t[u] >> 5], 1u << (t[u] & 31));
+                    s_t[m] = t[u] >= 0 ? (TT)t[u] : (TT)~(TT)0;
+                }
+            }
         }
         __syncwarp();
-        if (key != 0xffff && lane == (__ffs(same) - 1)) s_hist[warp * H + key] += __popc(same);
-        __syncwarp();
-    }
-    __syncthreads();
-    // (target, x-node) segments of the sorted list (statistics for the work model): read back what this CTA just wrote
-    int seg = 0;
-    for (int k = tid; k < ntot; k += T) {
-        const unsigned kk = g_key[k], kp = k ? g_key[k - 1] : 0u;
-        const int mk = (int)(kk & 16383u), mp = (int)(kp & 16383u);
-        const int ck = L.mg_npq ? (int)__umulhi((unsigned)mk, L.mg_npq) : mk, cp = L.mg_npq ? (int)__umulhi((unsigned)mp, L.mg_npq) : mp;
-        seg += (k == 0 || (kk >> 14) != (kp >> 14) || ck != cp) ? 1 : 0;
-    }
+        // ---- ranks: exclusive prefix of the word popcounts (lane = a contiguous run of words)
+        int H;
+        {
+            const int k0 = min(lane * wchunk, L.n_words), k1 = min(k0 + wchunk, L.n_words);
+            int mine = 0;
+            for (int k = k0; k < k1; ++k) mine += __popc(bits[k]);
+            int x = mine;
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) seg += __shfl_xor_sync(0xffffffffu, seg, d);
-    if (lane == 0) hs.scratch[warp] = seg;
-    __syncthreads();
-    if (tid == 0) {
-        int tot = 0;
-        for (int w = 0; w < NW; ++w) tot += hs.scratch[w];
-        nl.hits[blockIdx.x] = H; nl.ntot[blockIdx.x] = ntot; nl.nseg[blockIdx.x] = tot;
+            for (int d = 1; d < 32; d <<= 1) { const int y = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += y; }
+            H = __shfl_sync(0xffffffffu, x, 31);
+            int run = x - mine;
+            for (int k = k0; k < k1; ++k) { wpre[k] = (unsigned short)run; run += __popc(bits[k]); }
+        }
+        __syncwarp();
+        unsigned* g_key = nl.key + (size_t)cb * L.nnode;
+        int placed = 0;
+        for (int r0 = 0; r0 < H; r0 += S.hist_cap) {
+            const int nr = min(S.hist_cap, H - r0);
+            for (int k = lane; k < nr; k += 32) hist[k] = 0;
+            __syncwarp();
+            // ---- pass 2: nodes per rank
+            for (int st = 0; st < nsteps; ++st) {
+                const int m = st * 32 + lane;
+                const unsigned t = m < L.nnode ? (unsigned)s_t[m] : kOff;
+                int r = -1;
+                if (t != kOff) r = (int)wpre[t >> 5] + __popc(bits[t >> 5] & ((1u << (t & 31)) - 1u)) - r0;
+                const bool in = r >= 0 && r < nr;
+                const unsigned same = __match_any_sync(0xffffffffu, in ? r : -1 - lane);
+                if (in && (same & lt) == 0u) hist[r] += __popc(same);
+                __syncwarp();
+            }
+            // ---- exclusive scan of the counts, offset by what earlier windows placed
+            for (int k0 = 0; k0 < nr; k0 += 32) {
+                const int k = k0 + lane, v = k < nr ? hist[k] : 0;
+                int x = v;
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) { const int y = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += y; }
+                if (k < nr) hist[k] = placed + x - v;
+                placed += __shfl_sync(0xffffffffu, x, 31);
+            }
+            __syncwarp();
+            // ---- pass 3: placement in node order (stable)
+            for (int st = 0; st < nsteps; ++st) {
+                const int m = st * 32 + lane;
+                const unsigned t = m < L.nnode ? (unsigned)s_t[m] : kOff;
+                int r = -1;
+                if (t != kOff) r = (int)wpre[t >> 5] + __popc(bits[t >> 5] & ((1u << (t & 31)) - 1u)) - r0;
+                const bool in = r >= 0 && r < nr;
+                const unsigned same = __match_any_sync(0xffffffffu, in ? r : -1 - lane);
+                int base = 0;
+                if (in) { base = hist[r]; g_key[base + __popc(same & lt)] = (t << 14) | (unsigned)m; }
+                __syncwarp();
+                if (in && (same & lt) == 0u) hist[r] = base + __popc(same);
+                __syncwarp();
+            }
+        }
+        if (lane == 0) { nl.hits[cb] = H; nl.ntot[cb] = placed; }
     }
 }
 
-// Pattern pass, kernel S: exclusive scan of the hit counts -> cellbase, nnz and max hits.  One CTA.
+// Pattern pass, kernel S: exclusive scan of the hit counts -> cellbase, nnz, max hits, nodes on the grid.  One CTA;
+// thread = a contiguous run of cells (one load phase, one block scan, one store phase).
 __global__ void __launch_bounds__(1024) k_scan_cells(DevLattice L, int n_blk, const int* __restrict__ hits,
-                                                    const int* __restrict__ ntot, const int* __restrict__ nseg,
-                                                    int64_t* __restrict__ cellbase, int64_t* __restrict__ summary)
+                                                    const int* __restrict__ ntot, int64_t* __restrict__ cellbase,
+                                                    int64_t* __restrict__ summary, int64_t capacity)
 {
-    // tiles of 1024 consecutive cells (coalesced reads and writes): warp scans, then the 32 warp totals, then the carry
-    __shared__ long long wsum[32];
-    __shared__ long long s_carry;
-    __shared__ long long s_stat[3][32];
+    __shared__ long long wsum[32], wnod[32];
+    __shared__ int wmax[32];
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-    long long nodes = 0, segs = 0;
+    const int chunk = (n_blk + 1023) >> 10;
+    const int k0 = min(t * chunk, n_blk), k1 = min(k0 + chunk, n_blk);
+    long long mine = 0, nodes = 0;
     int mx = 0;
-    if (t == 0) s_carry = 0;
+    for (int k = k0; k < k1; ++k) { const int h = hits[k]; mine += h; mx = max(mx, h); nodes += ntot[k]; }
+    long long x = mine;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const long long y = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += y; }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) { nodes += __shfl_xor_sync(0xffffffffu, nodes, d); mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, d)); }
+    if (lane == 31) wsum[warp] = x;
+    if (lane == 0) { wnod[warp] = nodes; wmax[warp] = mx; }
     __syncthreads();
-    for (int base = 0; base < n_blk; base += 1024) {
-        const int k = base + t;
-        const int h = k < n_blk ? hits[k] : 0;
-        if (k < n_blk) { nodes += ntot[k]; segs += nseg[k]; mx = max(mx, h); }
-        long long inc = h;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) { const long long y = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += y; }
-        if (lane == 31) wsum[warp] = inc;
-        __syncthreads();
-        if (warp == 0) {
-            const long long v = wsum[lane];
-            long long x = v;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) { const long long y = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += y; }
-            wsum[lane] = x - v;                         // exclusive prefix of the warp totals
-            if (lane == 31) s_stat[0][0] = x;           // tile total
-        }
-        __syncthreads();
-        const long long carry = s_carry;
-        if (k < n_blk) cellbase[k] = carry + wsum[warp] + inc - h;
-        __syncthreads();
-        if (t == 0) s_carry = carry + s_stat[0][0];
-        __syncthreads();
-    }
-    // statistics: nodes on the grid, segments, max hits
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) {
-        nodes += __shfl_xor_sync(0xffffffffu, nodes, d); segs += __shfl_xor_sync(0xffffffffu, segs, d);
-        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, d));
-    }
-    if (lane == 0) { s_stat[0][warp] = nodes; s_stat[1][warp] = segs; s_stat[2][warp] = mx; }
-    __syncthreads();
-    if (t == 0) {
-        long long a = 0, s2 = 0, m = 0;
-        for (int w = 0; w < 32; ++w) { a += s_stat[0][w]; s2 += s_stat[1][w]; m = max(m, s_stat[2][w]); }
-        const long long total = s_carry;
+    long long carry = 0;
+    for (int w = 0; w < warp; ++w) carry += wsum[w];
+    long long run = carry + x - mine;
+    for (int k = k0; k < k1; ++k) { cellbase[k] = run; run += hits[k]; }
+    if (t == 1023) {
+        long long nn = 0; int m = 0;
+        for (int w = 0; w < 32; ++w) { nn += wnod[w]; m = max(m, wmax[w]); }
+        const long long total = carry + x;
+        cellbase[n_blk] = total;
         summary[0] = total * L.totcoup;                 // nnz of the block
         summary[1] = m;                                 // max hit cells of any source cell
-        summary[2] = a; summary[3] = s2;
-        cellbase[n_blk] = total;
+        summary[2] = nn;                                // nodes on the grid
+        summary[4] = (capacity >= 0 && total * L.totcoup > capacity) ? 1 : 0;      // the fill of pm_build must not run
     }
 }
 
@@ -214,24 +226,60 @@ __global__ void __launch_bounds__(256) k_write_rowptr(DevLattice L, int n_blk, c
     }
 }
 
-// Pattern pass, kernel B: column indices, ascending within each row.  The hit cells of a source cell are read
-// off its node lists (the target cell at the first sorted position of every rank).  Thread = output (alpha, m-th
+// Hit cells of every source cell, ascending, at hitlist[cellbase[k] ..): the target at every change of target in the
+// sorted node list.  One warp per source cell.  (Not on pm_build's path: pm_pattern with d_colidx and the SpMV without
+// the column array use it.)
+__global__ void __launch_bounds__(kThreads) k_hit_list(DevLattice L, int n_blk, NodeLists nl, const int64_t* __restrict__ cellbase,
+                                                      int* __restrict__ hitlist)
+{
+    const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+    for (int cb = blockIdx.x * wpb + (threadIdx.x >> 5); cb < n_blk; cb += gridDim.x * wpb) {
+        const int ntot = nl.ntot[cb];
+        const unsigned* g_key = nl.key + (size_t)cb * L.nnode;
+        int* out = hitlist + cellbase[cb];
+        int rank = 0;
+        for (int p0 = 0; p0 < ntot; p0 += 32) {
+            const int pos = p0 + lane;
+            unsigned t = 0, tp = 0xffffffffu;
+            if (pos < ntot) { t = g_key[pos] >> 14; if (pos) tp = g_key[pos - 1] >> 14; }
+            const bool first = pos < ntot && t != tp;
+            const unsigned b = __ballot_sync(0xffffffffu, first);
+            if (first) out[rank + __popc(b & ((1u << lane) - 1u))] = (int)t;
+            rank += __popc(b);
+        }
+    }
+}
+
+// (target, x-node) segments of the sorted lists (statistics for the work model only; run on demand)
+__global__ void __launch_bounds__(kThreads) k_count_segments(DevLattice L, int n_blk, NodeLists nl, unsigned long long* __restrict__ total)
+{
+    const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+    unsigned long long seg = 0;
+    for (int cb = blockIdx.x * wpb + (threadIdx.x >> 5); cb < n_blk; cb += gridDim.x * wpb) {
+        const int ntot = nl.ntot[cb];
+        const unsigned* g_key = nl.key + (size_t)cb * L.nnode;
+        for (int k = lane; k < ntot; k += 32) {
+            const unsigned kk = g_key[k], kp = k ? g_key[k - 1] : 0u;
+            const int mk = (int)(kk & 16383u), mp = (int)(kp & 16383u);
+            const int ck = L.mg_npq ? (int)__umulhi((unsigned)mk, L.mg_npq) : mk, cp = L.mg_npq ? (int)__umulhi((unsigned)mp, L.mg_npq) : mp;
+            seg += (k == 0 || (kk >> 14) != (kp >> 14) || ck != cp) ? 1 : 0;
+        }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) seg += __shfl_xor_sync(0xffffffffu, seg, d);
+    if (lane == 0 && seg) atomicAdd(total, seg);
+}
+
+// Pattern pass, kernel B: column indices, ascending within each row, from the hit lists.  Thread = output (alpha, m-th
 // coupled alpha'), looping over the hit cells k: entry k of row alpha sits at row_start + k*nc + m, so the threads
 // of a warp write runs of consecutive m and consecutive k fill the gaps (the same store pattern as the fill's rows).
-__global__ void __launch_bounds__(1024) k_emit_cols(DevLattice L, NodeLists nl, int hmax,
-                                                   const int64_t* __restrict__ rowptr, int32_t* __restrict__ colidx)
+__global__ void __launch_bounds__(1024) k_emit_cols(DevLattice L, NodeLists nl, const int64_t* __restrict__ cellbase,
+                                                   const int* __restrict__ hitlist, const int64_t* __restrict__ rowptr,
+                                                   int32_t* __restrict__ colidx)
 {
-    extern __shared__ __align__(16) char smem[];
     const int T = blockDim.x, tid = threadIdx.x;
-    int* hitcol = (int*)smem;                        // first column of every hit cell: cell * n_ch
-    const int H = nl.hits[blockIdx.x], ntot = nl.ntot[blockIdx.x];
-    const unsigned short* g_rkpos = nl.rkpos + (size_t)blockIdx.x * L.nnode;
-    const unsigned* g_key = nl.key + (size_t)blockIdx.x * L.nnode;
-    for (int pos = tid; pos < ntot; pos += T) {
-        const int r = g_rkpos[pos];
-        if (pos == 0 || g_rkpos[pos - 1] != r) hitcol[r] = (int)(g_key[pos] >> 14) * L.n_ch;
-    }
-    __syncthreads();
+    const int H = nl.hits[blockIdx.x];
+    const int* __restrict__ hit = hitlist + cellbase[blockIdx.x];
     int32_t* __restrict__ row0 = colidx + rowptr[(int64_t)blockIdx.x * L.n_ch];
     // the block is G groups of `ow` threads: a group covers all outputs (in passes if totcoup > ow) for k = g, g+G, ...
     const int ow = min(T, (L.totcoup + 31) & ~31), G = T / ow, g = tid / ow;
@@ -240,7 +288,7 @@ __global__ void __launch_bounds__(1024) k_emit_cols(DevLattice L, NodeLists nl, 
             const int al = L.o_alpha[o], off = L.cl_off[al], nc = L.cl_off[al + 1] - off, ap = L.cl[o];
             int32_t* out = row0 + ((size_t)H * off + (o - off));
 #pragma unroll 4
-            for (int k = g; k < H; k += G) out[(size_t)k * nc] = hitcol[k] + ap;
+            for (int k = g; k < H; k += G) out[(size_t)k * nc] = hit[k] * L.n_ch + ap;
         }
 }
 
@@ -268,19 +316,6 @@ __global__ void __launch_bounds__(256) k_spmv(int64_t n_rows, const int64_t* __r
 // 6 MB on configs[4]) the 4 B per nonzero of colidx need not be read: 8 instead of 12 B per nonzero from HBM.
 // Same lane striding and reduction as k_spmv, hence the same bits.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kThreads) k_hit_list(DevLattice L, NodeLists nl, const int64_t* __restrict__ cellbase,
-                                                      int* __restrict__ hitlist)
-{
-    const int ntot = nl.ntot[blockIdx.x];
-    const unsigned short* g_rkpos = nl.rkpos + (size_t)blockIdx.x * L.nnode;
-    const unsigned* g_key = nl.key + (size_t)blockIdx.x * L.nnode;
-    int* out = hitlist + cellbase[blockIdx.x];
-    for (int pos = threadIdx.x; pos < ntot; pos += blockDim.x) {
-        const int r = g_rkpos[pos];
-        if (pos == 0 || g_rkpos[pos - 1] != r) out[r] = (int)(g_key[pos] >> 14);
-    }
-}
-
 __global__ void __launch_bounds__(256) k_spmv_implicit(DevLattice L, int64_t n_rows, const int64_t* __restrict__ rowptr,
                                                       const int* __restrict__ hits, const int64_t* __restrict__ cellbase,
                                                       const int* __restrict__ hitlist, const double* __restrict__ vals,
@@ -313,22 +348,28 @@ static std::atomic<int64_t> g_launches{0};
 int64_t launch_count() { return g_launches.load(); }
 void count_launch() { ++g_launches; }
 
-cudaError_t launch_map_sort(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, cudaStream_t st)
+cudaError_t launch_map_sort(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, int n_sm, int* counter, cudaStream_t st)
 {
-    // per-warp histograms up to this many hit cells per source cell, one warp beyond (PM_HITS_FAST: test hook)
-    static const int hits_fast = [] { const char* e = std::getenv("PM_HITS_FAST"); return e ? std::max(1, std::atoi(e)) : kHitsFast; }();
-    const size_t sm = map_sort_smem(L, hits_fast);
-    cudaError_t e = cudaFuncSetAttribute(k_map_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    // warps per CTA: as many as shared memory holds, at most kMapSortMaxWarps (PM_MAPSORT_WARPS: test hook)
+    static const int want = [] { const char* e = std::getenv("PM_MAPSORT_WARPS"); return e ? std::max(1, std::min(kMapSortMaxWarps, std::atoi(e))) : kMapSortMaxWarps; }();
+    const MapSortSmem S = map_sort_plan(L, want);
+    if (S.nw < 1) return cudaErrorInvalidConfiguration;
+    using Fn = void (*)(DevLattice, MapSortSmem, int, int, NodeLists, int*);
+    const bool fast = L.bk_kmax <= kLocK;
+    const Fn fn = S.wide ? (fast ? k_map_sort<unsigned, true> : k_map_sort<unsigned, false>)
+                         : (fast ? k_map_sort<unsigned short, true> : k_map_sort<unsigned short, false>);
+    cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
-    k_map_sort<<<n_blk, kThreads, sm, st>>>(L, cell_begin, nl, hits_fast);
+    const int grid = std::max(1, std::min(n_sm, (n_blk + S.nw - 1) / S.nw));
+    fn<<<grid, S.nw * 32, S.total, st>>>(L, S, cell_begin, n_blk, nl, counter);
     ++g_launches;
     return cudaGetLastError();
 }
 
 cudaError_t launch_scan_rows(const DevLattice& L, int n_blk, const NodeLists& nl, int64_t* cellbase, int64_t* rowptr,
-                             int64_t* summary, cudaStream_t st)
+                             int64_t* summary, int64_t capacity, cudaStream_t st)
 {
-    k_scan_cells<<<1, 1024, 0, st>>>(L, n_blk, nl.hits, nl.ntot, nl.nseg, cellbase, summary);
+    k_scan_cells<<<1, 1024, 0, st>>>(L, n_blk, nl.hits, nl.ntot, cellbase, summary, capacity);
     ++g_launches;
     const int64_t n = (int64_t)n_blk * L.n_ch + 1;
     k_write_rowptr<<<(unsigned)std::min<int64_t>((n + 255) / 256, 148 * 8), 256, 0, st>>>(L, n_blk, nl.hits, cellbase, rowptr);
@@ -336,21 +377,27 @@ cudaError_t launch_scan_rows(const DevLattice& L, int n_blk, const NodeLists& nl
     return cudaGetLastError();
 }
 
-cudaError_t launch_emit_cols(const DevLattice& L, int n_blk, const NodeLists& nl, int hmax, const int64_t* rowptr,
-                             int32_t* colidx, cudaStream_t st)
+cudaError_t launch_emit_cols(const DevLattice& L, int n_blk, const NodeLists& nl, const int64_t* cellbase, const int* hitlist,
+                             const int64_t* rowptr, int32_t* colidx, cudaStream_t st)
 {
-    const size_t sm = al16(4 * (size_t)std::max(hmax, 1));
-    cudaError_t e = cudaFuncSetAttribute(k_emit_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    if (e != cudaSuccess) return e;
     const int threads = std::min(1024, std::max(128, (L.totcoup + 31) & ~31));
-    k_emit_cols<<<n_blk, threads, sm, st>>>(L, nl, hmax, rowptr, colidx);
+    k_emit_cols<<<n_blk, threads, 0, st>>>(L, nl, cellbase, hitlist, rowptr, colidx);
     ++g_launches;
     return cudaGetLastError();
 }
 
 cudaError_t launch_hit_list(const DevLattice& L, int n_blk, const NodeLists& nl, const int64_t* cellbase, int* hitlist, cudaStream_t st)
 {
-    k_hit_list<<<n_blk, kThreads, 0, st>>>(L, nl, cellbase, hitlist);
+    k_hit_list<<<std::max(1, std::min((n_blk + 7) / 8, 148 * 8)), kThreads, 0, st>>>(L, n_blk, nl, cellbase, hitlist);
+    ++g_launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_count_segments(const DevLattice& L, int n_blk, const NodeLists& nl, unsigned long long* total, cudaStream_t st)
+{
+    cudaError_t e = cudaMemsetAsync(total, 0, sizeof(unsigned long long), st);
+    if (e != cudaSuccess) return e;
+    k_count_segments<<<std::max(1, std::min((n_blk + 7) / 8, 148 * 8)), kThreads, 0, st>>>(L, n_blk, nl, total);
     ++g_launches;
     return cudaGetLastError();
 }
@@ -431,7 +478,7 @@ constexpr int kBlkT = 32;
 
 __global__ void __launch_bounds__(256) k_block_apply(int Np, int Nq, int n_ch, const double* __restrict__ B,
                                                     const double* __restrict__ diag, const double* __restrict__ in,
-                                                    double* __restrict__ out)
+                                                    double* __restrict__ out, int transpose)
 {
     extern __shared__ __align__(16) char smem[];
     const int ld = Np + 1;                                     // padded row length of the B tile
@@ -443,7 +490,7 @@ __global__ void __launch_bounds__(256) k_block_apply(int Np, int Nq, int n_ch, c
     const double* Ba = B + (size_t)a * Np * Np;
     for (int k = threadIdx.x; k < kBlkT * Np; k += blockDim.x) {
         const int r = k / Np, c = k - r * Np;
-        sB[r * ld + c] = (i0 + r < Np) ? Ba[(size_t)(i0 + r) * Np + c] : 0.0;
+        sB[r * ld + c] = (i0 + r < Np) ? (transpose ? Ba[(size_t)c * Np + (i0 + r)] : Ba[(size_t)(i0 + r) * Np + c]) : 0.0;   // B_a or its transpose
     }
     for (int k = threadIdx.x; k < Np * kBlkT; k += blockDim.x) {
         const int ip = k / kBlkT, jj = k - ip * kBlkT;
@@ -469,14 +516,27 @@ __global__ void __launch_bounds__(256) k_block_apply(int Np, int Nq, int n_ch, c
 }
 
 cudaError_t launch_block_apply(int Np, int Nq, int n_ch, const double* B, const double* diag, const double* in, double* out,
-                               cudaStream_t st)
+                               int transpose, cudaStream_t st)
 {
     const int ti = (Np + kBlkT - 1) / kBlkT, tj = (Nq + kBlkT - 1) / kBlkT;
     const size_t sm = sizeof(double) * ((size_t)kBlkT * (Np + 1) + (size_t)Np * kBlkT);
     if (sm > 227 * 1024) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaFuncSetAttribute(k_block_apply, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
-    k_block_apply<<<(unsigned)(n_ch * ti * tj), 256, sm, st>>>(Np, Nq, n_ch, B, diag, in, out);
+    k_block_apply<<<(unsigned)(n_ch * ti * tj), 256, sm, st>>>(Np, Nq, n_ch, B, diag, in, out, transpose);
+    count_launch();
+    return cudaGetLastError();
+}
+
+// rowptr of a shard -> global offsets (sharded multi-GPU build: add the nonzeros of the shards before it)
+__global__ void __launch_bounds__(256) k_add_offset(int64_t* __restrict__ a, int64_t n, int64_t off)
+{
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) a[k] += off;
+}
+
+cudaError_t launch_add_offset(int64_t* a, int64_t n, int64_t off, cudaStream_t st)
+{
+    k_add_offset<<<(unsigned)std::max<int64_t>(1, std::min<int64_t>((n + 255) / 256, 148 * 8)), 256, 0, st>>>(a, n, off);
     count_launch();
     return cudaGetLastError();
 }

@@ -13,18 +13,23 @@
 namespace pm {
 
 constexpr int kThreads = 256;
-constexpr int kHitsFast = 512;      // k_map_sort: per-warp histograms up to this many hit cells, one warp beyond
+constexpr int kMapSortMaxWarps = 16;  // k_map_sort: warps (= source cells in flight) per CTA, one CTA per SM
+constexpr int kHistCap = 512;         // k_map_sort: rank counters per window (one window unless a source cell hits more cells)
 
-size_t map_sort_smem(const DevLattice& L, int hits_fast);
+// shared-memory plan of k_map_sort: tables shared by the CTA, then one private area per warp (byte offsets)
+struct MapSortSmem { int thr_p, thr_q, bk_p, bk_q, tp, tq, tx, warp0, warp_bytes, w_bits, w_wpre, w_t, w_hist, nw, wide, hist_cap, total; };
+MapSortSmem map_sort_plan(const DevLattice& L, int max_warps);
 int64_t launch_count();
 void count_launch();
 
 // pattern pass
-cudaError_t launch_map_sort(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, cudaStream_t st);
+cudaError_t launch_map_sort(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, int n_sm, int* counter, cudaStream_t st);
+// scan of the hit counts + rowptr; summary = {nnz, max hits, nodes on the grid, (segments), overflow flag: nnz > capacity >= 0}
 cudaError_t launch_scan_rows(const DevLattice& L, int n_blk, const NodeLists& nl, int64_t* cellbase, int64_t* rowptr,
-                             int64_t* summary, cudaStream_t st);
-cudaError_t launch_emit_cols(const DevLattice& L, int n_blk, const NodeLists& nl, int hmax, const int64_t* rowptr,
-                             int32_t* colidx, cudaStream_t st);
+                             int64_t* summary, int64_t capacity, cudaStream_t st);
+cudaError_t launch_emit_cols(const DevLattice& L, int n_blk, const NodeLists& nl, const int64_t* cellbase, const int* hitlist,
+                             const int64_t* rowptr, int32_t* colidx, cudaStream_t st);
+cudaError_t launch_count_segments(const DevLattice& L, int n_blk, const NodeLists& nl, unsigned long long* total, cudaStream_t st);
 
 // fill pass (pm_fill.cuh): variant selection and launch
 struct FillLaunch { const void *fn, *fn_cols; int nw, grid; FillSmem smem; const char* name; bool jit; };   // fn_cols also writes colidx;
@@ -35,7 +40,7 @@ cudaError_t fill_plan(const DevLattice& L, unsigned long long tables_hash, int n
 // run-time compiled kernel for tables T (no build-time kernel): false + message when NVRTC / the driver API fails
 bool fill_plan_jit(const DevLattice& L, const Tables& T, unsigned long long tables_hash, int n_sm, FillLaunch* out, std::string& err);
 cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl,
-                        const int64_t* rowptr, double* vals, int32_t* colidx, int* counter, cudaStream_t st);
+                        const int64_t* rowptr, double* vals, int32_t* colidx, int* counter, const int64_t* guard, cudaStream_t st);
 
 cudaError_t launch_hit_list(const DevLattice& L, int n_blk, const NodeLists& nl, const int64_t* cellbase, int* hitlist, cudaStream_t st);
 cudaError_t launch_spmv_implicit(const DevLattice& L, int64_t n_rows, const int64_t* rowptr, const int* hits, const int64_t* cellbase,
@@ -45,7 +50,8 @@ cudaError_t launch_spmv(int64_t n_rows, const int64_t* rowptr, const int32_t* co
 
 // one block-matrix factor of the iteration step (eq. 24) with an optional diagonal factor
 cudaError_t launch_block_apply(int Np, int Nq, int n_ch, const double* B, const double* diag, const double* in, double* out,
-                               cudaStream_t st);
+                               int transpose, cudaStream_t st);
+cudaError_t launch_add_offset(int64_t* a, int64_t n, int64_t off, cudaStream_t st);
 
 // dependent-free DFMA loop on every SM: measured FP64 FMA throughput in TFLOP/s (diagnostic)
 cudaError_t measure_dfma(int n_sm, double* tflops, cudaStream_t st);

@@ -1,9 +1,12 @@
 // pm_stream.cu — row-block streaming build with host outputs (hot-path step a8).
 // PAPER.md:L340 "subdivide the whole calculation of this matrix into some blocks using an external CPU cycle",
 // L351-354 (copy a block in, launch, copy the block's values back).  Here a block is a contiguous range of
-// source cells whose CSR (12 B per nonzero) fits the caller's device budget; two buffer sets on two streams
-// let block b's device->host copies overlap block b+1's kernels.
+// source cells whose CSR (12 B per nonzero) plus node lists fit the caller's device budget; two buffer sets on two
+// streams let block b's device->host copies overlap block b+1's kernels.  The count pass that sizes the blocks runs in
+// bounded cell chunks (its node-list scratch never exceeds kCountScratch bytes) and its result is kept per lattice, so
+// pm_build_host after pm_build_host_count does not count again.
 #include <algorithm>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -11,9 +14,23 @@
 
 #include "../../include/pm.h"
 
+namespace pm {
+int32_t set_error(int32_t code, const std::string& msg);
+int32_t set_cuda_error(cudaError_t e, const char* where);
+void lattice_stamp(const pm_lattice* lat, uint64_t* id, uint64_t* version, int* nnode);
+}  // namespace pm
+
 namespace {
 
-struct Plan { std::vector<int64_t> rowptr; std::vector<int> cuts; int64_t nnz = 0, max_blk = 0; int n_ch = 0; };
+constexpr int64_t kCountScratch = int64_t(256) << 20;
+
+struct Plan {
+    uint64_t id = 0, version = 0; int64_t budget = -1;      // what it was made for
+    std::vector<int64_t> rowptr; std::vector<int> cuts; int64_t nnz = 0, max_blk = 0; int n_ch = 0, max_cells = 0;
+};
+
+std::mutex g_plan_mu;
+Plan g_plan;                      // the last plan made in this process (one entry: count -> build is the use)
 
 struct DevBuf {
     int64_t* rowptr = nullptr; int32_t* col = nullptr; double* val = nullptr; cudaStream_t st = nullptr;
@@ -25,32 +42,64 @@ int32_t make_plan(pm_lattice* lat, int64_t budget, Plan& P)
     int64_t M = 0; int32_t n_cells = 0;
     int32_t rc = pm_lattice_dims(lat, &M, &n_cells);
     if (rc) return rc;
-    P.n_ch = (int)(M / n_cells);
+    uint64_t id = 0, version = 0; int nnode = 0;
+    pm::lattice_stamp(lat, &id, &version, &nnode);
+    {
+        std::lock_guard<std::mutex> g(g_plan_mu);
+        if (g_plan.id == id && g_plan.version == version && g_plan.budget == budget && !g_plan.rowptr.empty()) { P = g_plan; return PM_OK; }
+    }
+    const int n_ch = (int)(M / n_cells);
+    const int64_t budget_in = budget;
     if (budget <= 0) {
         size_t fr = 0, tot = 0;
-        if (cudaMemGetInfo(&fr, &tot) != cudaSuccess) { cudaGetLastError(); return PM_ERR_DEVICE; }
+        cudaError_t e = cudaMemGetInfo(&fr, &tot);
+        if (e != cudaSuccess) { cudaGetLastError(); return pm::set_error(PM_ERR_DEVICE, std::string("cudaMemGetInfo: ") + cudaGetErrorString(e)); }
         budget = (int64_t)(fr / 4) * 3 / 2;            // two buffer sets share 3/4 of the free memory
     }
+    // coupled channels per row (host tables)
+    std::vector<uint8_t> mask((size_t)n_ch * n_ch);
+    if ((rc = pm_lattice_coupling(lat, mask.data(), nullptr))) return rc;
+    std::vector<int64_t> ncoup((size_t)n_ch, 0);
+    int64_t totcoup = 0;
+    for (int a = 0; a < n_ch; ++a) { for (int b = 0; b < n_ch; ++b) ncoup[(size_t)a] += mask[(size_t)a * n_ch + b]; totcoup += ncoup[(size_t)a]; }
+    // count pass in bounded chunks: hit cells per source cell
+    const int chunk = (int)std::max<int64_t>(1, std::min<int64_t>(n_cells, kCountScratch / (4 * (int64_t)std::max(nnode, 1))));
+    std::vector<int32_t> hits((size_t)n_cells);
     int64_t* d_rowptr = nullptr;
-    if (cudaMalloc(&d_rowptr, sizeof(int64_t) * (size_t)(M + 1)) != cudaSuccess) { cudaGetLastError(); return PM_ERR_NOMEM; }
-    int64_t nnz = 0;
-    rc = pm_pattern(lat, 0, n_cells, d_rowptr, nullptr, 0, &nnz, nullptr);
-    if (rc == PM_OK) {
-        P.rowptr.resize((size_t)M + 1);
-        if (cudaMemcpy(P.rowptr.data(), d_rowptr, sizeof(int64_t) * (size_t)(M + 1), cudaMemcpyDeviceToHost) != cudaSuccess) rc = PM_ERR_CUDA;
+    cudaError_t e = cudaMalloc(&d_rowptr, sizeof(int64_t) * ((size_t)chunk * n_ch + 1));
+    if (e != cudaSuccess) return pm::set_cuda_error(e, "cudaMalloc(count pass rowptr)");
+    for (int cb = 0; cb < n_cells && rc == PM_OK; cb += chunk) {
+        const int ce = std::min(n_cells, cb + chunk);
+        int64_t nnz = 0;
+        rc = pm_pattern(lat, cb, ce, d_rowptr, nullptr, 0, &nnz, nullptr);
+        if (rc == PM_OK) rc = pm_pattern_cell_hits(lat, hits.data() + cb, nullptr);
     }
     cudaFree(d_rowptr);
     if (rc) return rc;
-    P.nnz = nnz;
+    P = Plan();
+    P.id = id; P.version = version; P.budget = budget_in; P.n_ch = n_ch;
+    P.rowptr.resize((size_t)M + 1);
+    int64_t run = 0;
+    for (int c = 0; c < n_cells; ++c)
+        for (int a = 0; a < n_ch; ++a) { P.rowptr[(size_t)c * n_ch + a] = run; run += (int64_t)hits[(size_t)c] * ncoup[(size_t)a]; }
+    P.rowptr[(size_t)M] = run;
+    P.nnz = run;
+    // blocks: CSR bytes of the block plus its node lists (4 B per node) within the budget
     P.cuts.assign(1, 0);
-    int64_t cur = 0;
+    int64_t cur = 0, cur_bytes = 0;
+    int cur_cells = 0;
     for (int c = 0; c < n_cells; ++c) {
-        const int64_t nz = P.rowptr[(size_t)(c + 1) * P.n_ch] - P.rowptr[(size_t)c * P.n_ch];
-        if (cur > 0 && 12 * (cur + nz) > budget) { P.cuts.push_back(c); P.max_blk = std::max(P.max_blk, cur); cur = 0; }
-        cur += nz;
+        const int64_t nz = (int64_t)hits[(size_t)c] * totcoup, bytes = 12 * nz + 4 * (int64_t)nnode;
+        if (cur_cells > 0 && cur_bytes + bytes > budget) {
+            P.cuts.push_back(c); P.max_blk = std::max(P.max_blk, cur); P.max_cells = std::max(P.max_cells, cur_cells);
+            cur = 0; cur_bytes = 0; cur_cells = 0;
+        }
+        cur += nz; cur_bytes += bytes; ++cur_cells;
     }
     P.cuts.push_back(n_cells);
-    P.max_blk = std::max(P.max_blk, cur);
+    P.max_blk = std::max(P.max_blk, cur); P.max_cells = std::max(P.max_cells, cur_cells);
+    std::lock_guard<std::mutex> g(g_plan_mu);
+    g_plan = P;
     return PM_OK;
 }
 
@@ -60,7 +109,7 @@ extern "C" {
 
 int32_t pm_build_host_count(pm_lattice* lat, int64_t device_budget_bytes, int64_t* nnz_total, int32_t* n_blocks)
 {
-    if (!lat || !nnz_total || !n_blocks) return PM_ERR_ARG;
+    if (!lat || !nnz_total || !n_blocks) return pm::set_error(PM_ERR_ARG, "NULL argument");
     Plan P;
     int32_t rc = make_plan(lat, device_budget_bytes, P);
     if (rc) return rc;
@@ -72,49 +121,51 @@ int32_t pm_build_host_count(pm_lattice* lat, int64_t device_budget_bytes, int64_
 int32_t pm_build_host(pm_lattice* lat, int64_t device_budget_bytes, int64_t* h_rowptr, int32_t* h_colidx, double* h_vals,
                       int64_t capacity, int64_t* nnz_total, int32_t* n_blocks)
 {
-    if (!lat || !h_rowptr || !h_colidx || !h_vals || !nnz_total || !n_blocks) return PM_ERR_ARG;
+    if (!lat || !h_rowptr || !h_colidx || !h_vals || !nnz_total || !n_blocks) return pm::set_error(PM_ERR_ARG, "NULL argument");
     Plan P;
     int32_t rc = make_plan(lat, device_budget_bytes, P);
     if (rc) return rc;
     *nnz_total = P.nnz;
     *n_blocks = (int32_t)P.cuts.size() - 1;
-    if (P.nnz > capacity) return PM_ERR_OVERFLOW;
+    if (P.nnz > capacity) return pm::set_error(PM_ERR_OVERFLOW, "h_colidx / h_vals too small for the matrix's nnz");
     std::copy(P.rowptr.begin(), P.rowptr.end(), h_rowptr);
     const int nb = *n_blocks, nset = nb > 1 ? 2 : 1;
-    int max_cells = 0;
-    for (int b = 0; b < nb; ++b) max_cells = std::max(max_cells, P.cuts[(size_t)b + 1] - P.cuts[(size_t)b]);
     DevBuf buf[2];
+    cudaError_t e;
     for (int s = 0; s < nset; ++s) {
-        if (cudaStreamCreate(&buf[s].st) != cudaSuccess ||
-            cudaMalloc(&buf[s].rowptr, sizeof(int64_t) * ((size_t)max_cells * P.n_ch + 1)) != cudaSuccess ||
-            cudaMalloc(&buf[s].col, sizeof(int32_t) * (size_t)std::max<int64_t>(P.max_blk, 1)) != cudaSuccess ||
-            cudaMalloc(&buf[s].val, sizeof(double) * (size_t)std::max<int64_t>(P.max_blk, 1)) != cudaSuccess) {
-            cudaGetLastError();
-            return PM_ERR_NOMEM;
-        }
+        if ((e = cudaStreamCreate(&buf[s].st)) != cudaSuccess) return pm::set_cuda_error(e, "cudaStreamCreate");
+        if ((e = cudaMalloc(&buf[s].rowptr, sizeof(int64_t) * ((size_t)P.max_cells * P.n_ch + 1))) != cudaSuccess ||
+            (e = cudaMalloc(&buf[s].col, sizeof(int32_t) * (size_t)std::max<int64_t>(P.max_blk, 1))) != cudaSuccess ||
+            (e = cudaMalloc(&buf[s].val, sizeof(double) * (size_t)std::max<int64_t>(P.max_blk, 1))) != cudaSuccess)
+            return pm::set_cuda_error(e, "cudaMalloc(block buffers)");
     }
-    // The lattice's node lists and work counter serve one block at a time: block b+1's kernels wait for block b's
+    // The lattice's node lists and work counters serve one block at a time: block b+1's kernels wait for block b's
     // fill (event), so only the device->host copies of block b overlap the kernels of block b+1.
     cudaEvent_t filled = nullptr;
-    if (cudaEventCreateWithFlags(&filled, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return PM_ERR_CUDA; }
+    if ((e = cudaEventCreateWithFlags(&filled, cudaEventDisableTiming)) != cudaSuccess) return pm::set_cuda_error(e, "cudaEventCreate");
     for (int b = 0; b < nb && rc == PM_OK; ++b) {
         DevBuf& B = buf[b % nset];
-        if (b > 0 && cudaStreamWaitEvent(B.st, filled, 0) != cudaSuccess) { rc = PM_ERR_CUDA; break; }
+        if (b > 0 && (e = cudaStreamWaitEvent(B.st, filled, 0)) != cudaSuccess) { rc = pm::set_cuda_error(e, "cudaStreamWaitEvent"); break; }
+        // (this buffer set was last used by block b-2 on the same stream: its copies precede these kernels in stream order)
         const int cb = P.cuts[(size_t)b], ce = P.cuts[(size_t)b + 1];
         const int64_t off = P.rowptr[(size_t)cb * P.n_ch];
-        int64_t nnz = 0;
-        // the stream of this buffer set is idle here: pm_pattern synchronises it before reusing the buffers
-        rc = pm_build(lat, cb, ce, B.rowptr, B.col, B.val, P.max_blk, &nnz, B.st);
+        const int64_t nnz = P.rowptr[(size_t)ce * P.n_ch] - off;
+        // pattern and fill back to back on the stream; the nnz is known from the plan, the device checks it against the capacity
+        rc = pm_build_async(lat, cb, ce, B.rowptr, B.col, B.val, P.max_blk, 0, B.st);
         if (rc) break;
-        if (nnz != P.rowptr[(size_t)ce * P.n_ch] - off) { rc = PM_ERR_STATE; break; }
-        if (cudaEventRecord(filled, B.st) != cudaSuccess) { rc = PM_ERR_CUDA; break; }
-        if (cudaMemcpyAsync(h_colidx + off, B.col, sizeof(int32_t) * (size_t)nnz, cudaMemcpyDeviceToHost, B.st) != cudaSuccess ||
-            cudaMemcpyAsync(h_vals + off, B.val, sizeof(double) * (size_t)nnz, cudaMemcpyDeviceToHost, B.st) != cudaSuccess)
-            rc = PM_ERR_CUDA;
+        if ((e = cudaEventRecord(filled, B.st)) != cudaSuccess) { rc = pm::set_cuda_error(e, "cudaEventRecord"); break; }
+        if ((e = cudaMemcpyAsync(h_colidx + off, B.col, sizeof(int32_t) * (size_t)nnz, cudaMemcpyDeviceToHost, B.st)) != cudaSuccess ||
+            (e = cudaMemcpyAsync(h_vals + off, B.val, sizeof(double) * (size_t)nnz, cudaMemcpyDeviceToHost, B.st)) != cudaSuccess) {
+            rc = pm::set_cuda_error(e, "cudaMemcpyAsync(block)");
+            break;
+        }
+        int64_t got = 0;
+        rc = pm_build_wait(lat, &got);                  // host state of this block (waits for its pattern pass only)
+        if (rc == PM_OK && got != nnz) rc = pm::set_error(PM_ERR_STATE, "block nnz differs from the count pass");
     }
     cudaEventDestroy(filled);
     for (int s = 0; s < nset; ++s)
-        if (buf[s].st && cudaStreamSynchronize(buf[s].st) != cudaSuccess && rc == PM_OK) rc = PM_ERR_CUDA;
+        if (buf[s].st && (e = cudaStreamSynchronize(buf[s].st)) != cudaSuccess && rc == PM_OK) rc = pm::set_cuda_error(e, "streaming build");
     return rc;
 }
 

@@ -56,6 +56,8 @@ def _small_cases():
         I.small_coupled(N=9, jmax=3, orders=(4, 3, 5), Nq=4),                                        # 26 channels, 9 x 4
         I.boson_lattice(6, 5, orders=(1, 4, 8), cq=0.9),                                             # n_p = 1 (reading R1)
         I.small_coupled(N=6, jmax=2, orders=(1, 5, 6), Nq=7),
+        # 300 uniform p-cells: more than four sqrt-thresholds per bucket of the location table (the scanning locate path)
+        I.Workload("uniform_fine_300x3", np.linspace(0.0, 1.2, 301), I.tan_grid(3, 1.0), I.boson_channel(), 0, +1, 0, I.PM_SPINLESS_BOSON, 2, 3, 4),
     ]
 
 
@@ -129,9 +131,12 @@ def test_pm_build_equals_pattern_plus_fill(api, wl):
     lat.close()
 
 
-def test_single_warp_sort_path(oracle):
-    """Source cells with more hit cells than the per-warp histograms hold are sorted by one warp; the test hook
-    PM_HITS_FAST=8 sends almost every cell of configs[1] down that path (own process: the hook is read once)."""
+@pytest.mark.parametrize("env", [{"PM_HIST_CAP": "8"}, {"PM_MAPSORT_WARPS": "1"}, {"PM_HIST_CAP": "5", "PM_MAPSORT_WARPS": "3"}],
+                         ids=lambda e: "-".join(f"{k[3:].lower()}{v}" for k, v in e.items()))
+def test_sort_windows_and_warp_counts(oracle, env):
+    """k_map_sort counts and places the nodes rank window by rank window (512 counters per window: one window on every
+    realistic lattice).  The test hook PM_HIST_CAP forces up to 14 windows per source cell of configs[1]; PM_MAPSORT_WARPS
+    changes the warps (source cells in flight) per CTA.  Own process: the hooks are read once."""
     import subprocess
     import sys
     import tempfile
@@ -143,7 +148,7 @@ def test_single_warp_sort_path(oracle):
     ) % ROOT
     with tempfile.TemporaryDirectory() as d:
         out = os.path.join(d, "r.npz")
-        subprocess.run([sys.executable, "-c", code, out], check=True, env=dict(os.environ, PM_HITS_FAST="8"), timeout=600)
+        subprocess.run([sys.executable, "-c", code, out], check=True, env=dict(os.environ, **env), timeout=600)
         r = np.load(out)
         rpo, cio, vo = oracle.build_csr(I.config(1))
         assert np.array_equal(r["rp"], rpo) and np.array_equal(r["ci"], cio)
@@ -301,7 +306,7 @@ def test_streaming_build_identical(api, oracle, budget_blocks, wl):
     rectangular lattice)."""
     lat = api.Lattice(wl)
     nnz, _ = api.pm_build_host_count(lat.h, 1 << 40)
-    budget = (1 << 40) if budget_blocks == 1 else int(12 * nnz / budget_blocks) + 1
+    budget = (1 << 40) if budget_blocks == 1 else int((12 * nnz + 4 * wl.nodes_per_cell * wl.n_cells) / budget_blocks) + 1   # CSR + node lists
     rp, ci, v, nnz2, nb = lat.build_host(budget, pinned=(budget_blocks != 3))
     assert nnz2 == nnz and (nb == 1 if budget_blocks == 1 else budget_blocks <= nb <= 2 * budget_blocks + 2)
     rpo, cio, vo = oracle.build_csr(wl)
@@ -346,4 +351,121 @@ def test_iteration_step_matches_oracle(api, oracle, wl):
     assert np.max(np.abs(out.cpu().numpy() - it.block_apply(O, u, wl.Np, wl.Nq, wl.n_ch))) <= 1e-13 * np.max(np.abs(u)) * wl.Np
     api.pm_block_apply(lat.h, dVt, dg, du, out)
     assert np.max(np.abs(out.cpu().numpy() - it.block_apply(Vt, g1 * u, wl.Np, wl.Nq, wl.n_ch))) <= 1e-12 * np.max(np.abs(Vt)) * wl.Np
+    lat.close()
+
+
+def test_build_async_and_device_side_capacity_check(api, oracle):
+    """pm_build_async queues pattern + fill without a host synchronisation; pm_build_wait returns nnz.  With a capacity
+    below nnz the device-side check stops the fill: nothing is written and the wait reports PM_ERR_OVERFLOW."""
+    import torch
+    wl = I.small_coupled(N=6, jmax=2, orders=(3, 4, 6), Nq=7)
+    lat = api.Lattice(wl)
+    rp0, ci0, v0 = lat.build_fused()
+    nnz = ci0.numel()
+    rp = torch.empty_like(rp0); ci = torch.full_like(ci0, -7); v = torch.full_like(v0, -7.0)
+    api.pm_build_async(lat.h, 0, wl.n_cells, rp, ci, v)
+    assert api.pm_build_wait(lat.h) == nnz
+    assert torch.equal(rp, rp0) and torch.equal(ci, ci0) and torch.equal(v, v0)
+    ci_s = torch.full((nnz - 1,), -7, dtype=torch.int32, device="cuda"); v_s = torch.full((nnz - 1,), -7.0, dtype=torch.float64, device="cuda")
+    api.pm_build_async(lat.h, 0, wl.n_cells, rp, ci_s, v_s)
+    with pytest.raises(api.PmError) as e:
+        api.pm_build_wait(lat.h)
+    assert e.value.code == -8 and "too small" in str(e.value)
+    torch.cuda.synchronize()
+    assert bool((ci_s == -7).all()) and bool((v_s == -7.0).all())
+    with pytest.raises(api.PmError) as e:                      # the synchronous call reports the same
+        api.pm_build(lat.h, 0, wl.n_cells, rp, ci_s, v_s)
+    assert e.value.code == -8
+    lat.close()
+
+
+@pytest.mark.parametrize("wl", [I.config(1), I.small_coupled(N=9, jmax=3, orders=(4, 3, 5), Nq=7)], ids=lambda w: w.name)
+@pytest.mark.parametrize("world", [2, 3, 8])
+def test_shards_concatenate_to_the_whole_build(api, wl, world):
+    """contiguous source-cell ranges balanced by hit count, one shard per rank, the per-shard nnz turned
+    into global row-pointer offsets.  Here the shards are built one after the other on one GPU and must concatenate, bit
+    for bit, to the single-block build."""
+    import torch
+    lat = api.Lattice(wl)
+    rp0, ci0, v0 = lat.build_fused()
+    hits = api.pm_pattern_cell_hits(lat.h, wl.n_cells)
+    assert hits.sum() * int(api.pm_lattice_coupling(lat.h, wl.n_ch)[0].sum()) == ci0.numel()
+    cuts = api.pm_partition_cells(hits, world, cell_cost=2.0)
+    assert cuts[0] == 0 and cuts[-1] == wl.n_cells and np.all(np.diff(cuts) >= 0)
+    w = hits.astype(np.float64) + 2.0
+    loads = np.array([w[cuts[r]:cuts[r + 1]].sum() for r in range(world)])
+    assert loads.max() <= w.sum() / world + w.max()                 # balanced to within one cell
+    parts, nnz_r = [], []
+    for r in range(world):
+        rp, ci, v = lat.build_fused(int(cuts[r]), int(cuts[r + 1]))
+        parts.append((rp, ci, v)); nnz_r.append(ci.numel())
+    offs = np.concatenate([[0], np.cumsum(nnz_r)])                   # what the all-gather of the per-rank nnz yields
+    rows = []
+    for r, (rp, ci, v) in enumerate(parts):
+        api.pm_rowptr_offset(rp, int(offs[r]))
+        rows.append(rp[:-1] if r < world - 1 else rp)
+    assert torch.equal(torch.cat(rows), rp0)
+    assert torch.equal(torch.cat([p[1] for p in parts]), ci0) and torch.equal(torch.cat([p[2] for p in parts]), v0)
+    lat.close()
+
+
+@pytest.mark.parametrize("wl", [I.small_coupled(N=6, jmax=2, orders=(3, 3, 6)), I.small_coupled(N=5, jmax=3, orders=(3, 4, 6), Nq=9)],
+                         ids=lambda w: w.name)
+def test_rotation_to_the_channel_basis(api, oracle, wl):
+    """eq. (20), P = O P0 O^T: pm_rotate_apply on the GPU-built P0 against the numpy oracle on the
+    oracle-built P0; the transposed block factor alone; with and without the column array."""
+    import torch
+    from oracle import pm_iter_oracle as it
+    O, _, _, x = I.iteration_factors(wl, seed=23)
+    rpo, cio, vo = oracle.build_csr(wl)
+    ref = it.rotate_apply(rpo, cio, vo, O, x, wl.Np, wl.Nq, wl.n_ch)
+    lat = api.Lattice(wl)
+    rp, ci, v = lat.build_fused()
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    dO, dx = dev(O), dev(x)
+    out = torch.empty(wl.M, dtype=torch.float64, device="cuda")
+    work = torch.empty(2 * wl.M, dtype=torch.float64, device="cuda")
+    api.pm_rotate_apply(lat.h, rp, ci, v, dO, dx, out, work)
+    assert np.max(np.abs(out.cpu().numpy() - ref)) <= 1e-11 * np.max(np.abs(ref))
+    out2 = torch.empty_like(out)
+    api.pm_rotate_apply(lat.h, rp, None, v, dO, dx, out2, work)
+    assert torch.equal(out, out2)
+    api.pm_block_apply_t(lat.h, dO, dx, out)
+    assert np.max(np.abs(out.cpu().numpy() - it.block_apply_t(O, x, wl.Np, wl.Nq, wl.n_ch))) <= 1e-13 * np.max(np.abs(x)) * wl.Np
+    lat.close()
+
+
+def test_attached_lattices_share_the_geometric_pattern(api, oracle):
+    """SURVEY sec. 8(f) rank 3: several J^pi on one grid.  Lattices attached to a base share its node lists;
+    pm_build_reuse maps and sorts the nodes once for the whole group (the launch counter shows it) and every member's CSR
+    meets the oracle's."""
+    import torch
+    base = I.small_coupled(N=6, jmax=2, orders=(3, 4, 6), Nq=7)
+    others = [I.small_coupled(N=6, jmax=2, orders=(3, 4, 6), Nq=7, J2=1, parity=-1),
+              I.small_coupled(N=6, jmax=1, orders=(3, 4, 6), Nq=7, J2=3, parity=+1),
+              I.small_coupled(N=6, jmax=1, orders=(3, 4, 6), Nq=7, J2=3, parity=-1)]
+    lat = api.Lattice(base)
+    hs = [api.pm_lattice_attach(lat.h, w.channels, w.J2, w.parity, w.T2, w.statistics) for w in others]
+    results = []
+    l0 = api.pm_launch_count()
+    for h, w in zip([lat.h] + hs, [base] + others):
+        rp = torch.empty(w.M + 1, dtype=torch.int64, device="cuda")
+        nnz = api.pm_pattern(h, 0, w.n_cells, rp, None) if h is lat.h else None     # the base counts (and maps) first
+        cap = base.n_cells * base.nodes_per_cell * w.n_ch * w.n_ch                   # an upper bound: no count needed
+        ci = torch.empty(min(cap, 1 << 26), dtype=torch.int32, device="cuda"); v = torch.empty(ci.numel(), dtype=torch.float64, device="cuda")
+        n = api.pm_build_reuse(h, 0, w.n_cells, rp, ci, v)
+        assert nnz is None or nnz == n
+        results.append((rp.cpu().numpy(), ci[:n].cpu().numpy(), v[:n].cpu().numpy()))
+    launches = api.pm_launch_count() - l0
+    # one map_sort in all (the base's count call); per member scan + rowptr + fill, plus the base's own scan + rowptr
+    assert launches == 1 + 2 + 3 * 4, launches
+    for (rp, ci, v), w in zip(results, [base] + others):
+        rpo, cio, vo = oracle.build_csr(w)
+        assert np.array_equal(rp, rpo) and np.array_equal(ci, cio)
+        _assert_values(v, vo)
+    for h in hs:
+        api.pm_lattice_destroy(h)
+    # the base still works after its group is gone, and pm_build (no reuse) maps afresh
+    rp, ci, v = lat.build_fused()
+    assert np.array_equal(ci.cpu().numpy(), results[0][1]) and np.array_equal(v.cpu().numpy(), results[0][2])
     lat.close()

@@ -197,3 +197,58 @@ def test_product_does_not_import_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".cpp", ".hpp", ".h")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert "pm_oracle" not in src and "from oracle" not in src and "import oracle" not in src, f
+
+
+def test_partition_cells_is_balanced_and_deterministic():
+    """pm_partition_cells (host only): contiguous ranges, every cell in exactly one, loads within one cell of the mean,
+    degenerate inputs (more parts than cells, zero hits, one part)."""
+    rng = np.random.default_rng(5)
+    for n, parts, cost in ((22500, 8, 40.0), (100, 3, 0.0), (5, 8, 1.0), (1, 1, 0.0), (0, 4, 1.0), (1000, 7, 0.5)):
+        hits = rng.integers(0, 174, size=n).astype(np.int32)
+        cuts = api.pm_partition_cells(hits, parts, cost)
+        assert len(cuts) == parts + 1 and cuts[0] == 0 and cuts[-1] == n and np.all(np.diff(cuts) >= 0)
+        assert np.array_equal(cuts, api.pm_partition_cells(hits.copy(), parts, cost))
+        if n:
+            w = hits + cost
+            loads = np.array([w[cuts[r]:cuts[r + 1]].sum() for r in range(parts)])
+            assert loads.sum() == pytest.approx(w.sum()) and loads.max() <= w.sum() / parts + w.max() + 1e-9
+    with pytest.raises(api.PmError):
+        api.pm_partition_cells(np.zeros(3, np.int32), 0)
+
+
+def test_failing_calls_leave_a_message():
+    """Every failing path across the ABI sets pm_last_error (also the streaming build of pm_stream.cu)."""
+    import torch
+    wl = I.config(0)
+    h = _create(wl)
+    L = api.lib()
+    for call in (lambda: L.pm_build_host_count(h, 0, None, None),
+                 lambda: L.pm_build_host(h, 0, None, None, None, 0, None, None),
+                 lambda: L.pm_build_wait(h, None),
+                 lambda: L.pm_pattern_cell_hits(h, None, None),
+                 lambda: L.pm_rowptr_offset(None, 4, 1, None)):
+        L.pm_lattice_dims(h, None, None)               # a succeeding call in between does not clear or set anything
+        rc = call()
+        assert rc != 0 and L.pm_last_error().decode() != "", rc
+    if not torch.cuda.is_available():
+        import ctypes as C
+        nnz, nb = C.c_int64(), C.c_int32()
+        buf = np.zeros(8, dtype=np.int64)
+        rc = L.pm_build_host(h, 0, buf.ctypes.data, buf.ctypes.data, buf.ctypes.data, 1, C.byref(nnz), C.byref(nb))
+        assert rc in (-9, -6, -5) and "CUDA" in L.pm_last_error().decode() or "device" in L.pm_last_error().decode()
+    api.pm_lattice_destroy(h)
+
+
+def test_attach_validates_like_create():
+    wl = I.config(1)
+    h = _create(wl)
+    other = I.enumerate_3n_channels(3, -1, 1, 1)
+    h2 = api.pm_lattice_attach(h, other, 3, -1, 1, 0)
+    assert api.pm_lattice_dims(h2) == (wl.n_cells * len(other), wl.n_cells)
+    with pytest.raises(api.PmError) as e:
+        api.pm_lattice_attach(h, other, 3, +1, 1, 0)          # wrong parity for these channels
+    assert e.value.code == -3
+    api.pm_lattice_destroy(h)                                  # base first: the group lives on
+    t, w = api.pm_lattice_rule(h2, 2, wl.n_x)
+    assert len(t) == wl.n_x
+    api.pm_lattice_destroy(h2)

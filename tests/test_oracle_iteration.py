@@ -35,6 +35,18 @@ def test_kernel_apply_equals_dense_product(oracle):
     # P V1 G1 with P = O P0 O^T (eq. 20): the same operator
     ref2 = (Of @ P @ Of.T) @ Vf @ G @ u
     assert np.max(np.abs(got - ref2)) < 1e-12 * np.max(np.abs(ref))
+    # eq. (20) alone: rotate_apply is the dense P = O P0 O^T, which has P0's spectrum (O is orthogonal)
+    Pd = Of @ P @ Of.T
+    rot = it.rotate_apply(rp, ci, v, O, u, wl.Np, wl.Nq, wl.n_ch)
+    assert np.max(np.abs(rot - Pd @ u)) < 1e-12 * np.max(np.abs(Pd @ u))
+    assert np.max(np.abs(Of @ Of.T - np.eye(wl.M))) < 1e-12
+    e0, e1 = np.sort(np.linalg.eigvals(P).real), np.sort(np.linalg.eigvals(Pd).real)
+    assert np.max(np.abs(e0 - e1)) < 1e-9 * np.max(np.abs(e0))
+    # transposed blocks: <y, B x> = <B^T y, x>
+    y = np.random.default_rng(5).uniform(-1, 1, wl.M)
+    lhs = y @ it.block_apply(O, u, wl.Np, wl.Nq, wl.n_ch)
+    rhs = it.block_apply_t(O, y, wl.Np, wl.Nq, wl.n_ch) @ u
+    assert abs(lhs - rhs) < 1e-12 * abs(lhs)
 
 
 def test_identity_factors_reduce_to_the_spmv(oracle):
