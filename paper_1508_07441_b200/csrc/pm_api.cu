@@ -66,6 +66,8 @@ struct pm_geometry {
     cudaEvent_t ev_summary = nullptr;  // recorded after the copy
     bool summary_pending = false;      // the host has not looked at h_summary yet
     int* d_counter = nullptr;          // [0] work counter of the fill kernel, [1] of k_map_sort
+    void* d_sort_scratch = nullptr;    // k_map_sort: targets of the cells in flight (a few MB)
+    size_t sort_scratch_bytes = 0;
     int* d_hitlist = nullptr;          // hit cells of every source cell of the last pattern call, lazily built
     int64_t hitlist_cap = 0;
     bool hitlist_valid = false;
@@ -119,6 +121,8 @@ void free_geometry_device(pm_geometry* G)
     if (G->ev_summary) cudaEventDestroy(G->ev_summary);
     if (G->d_counter) cudaFree(G->d_counter);
     if (G->d_hitlist) cudaFree(G->d_hitlist);
+    if (G->d_sort_scratch) cudaFree(G->d_sort_scratch);
+    G->d_sort_scratch = nullptr; G->sort_scratch_bytes = 0;
     G->d_blob = nullptr; G->d_summary = nullptr; G->h_summary = nullptr; G->ev_summary = nullptr; G->d_counter = nullptr;
     G->d_hitlist = nullptr; G->hitlist_cap = 0; G->summary_pending = false; G->dev_version = 0;
 }
@@ -537,7 +541,14 @@ int32_t pattern_async(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int
         G->lists_valid = false; G->hitlist_valid = false; G->segments = -1;
         if ((rc = ensure_cell_scratch(G, n_blk))) return rc;
         if ((e = cudaMemsetAsync(G->d_counter, 0, 2 * sizeof(int), st)) != cudaSuccess) return cuda_fail(e, "memset(counters)");
-        e = pm::launch_map_sort(lat->dev, cell_begin, n_blk, G->nl, G->n_sm, G->d_counter + 1, st);
+        const size_t need = pm::map_sort_scratch_bytes(lat->dev, G->n_sm);
+        if (need > G->sort_scratch_bytes) {
+            if (G->d_sort_scratch) cudaFree(G->d_sort_scratch);
+            G->d_sort_scratch = nullptr; G->sort_scratch_bytes = 0;
+            if ((e = cudaMalloc(&G->d_sort_scratch, need)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(sort scratch)");
+            G->sort_scratch_bytes = need;
+        }
+        e = pm::launch_map_sort(lat->dev, cell_begin, n_blk, G->nl, G->n_sm, G->d_counter + 1, G->d_sort_scratch, st);
         if (e == cudaErrorInvalidConfiguration) { cudaGetLastError(); return fail(PM_ERR_NOMEM, "lattice needs more shared memory per source cell than one SM has"); }
         if (e != cudaSuccess) return cuda_fail(e, "k_map_sort");
     }

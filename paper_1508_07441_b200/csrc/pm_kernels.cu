@@ -28,6 +28,8 @@ static size_t al16(size_t b) { return (b + 15) & ~size_t(15); }
 // so the sorted list is ordered by (target, x-node, a, b).  Lanes that meet the same rank in a step are grouped with
 // match_any (32 consecutive nodes fall into one to three targets), so no shared-memory atomics are needed for the counts.
 // Ranks are processed in windows of kHistCap counters: one window for every realistic lattice, any number otherwise.
+// The targets of pass 1 wait for passes 2 and 3 in a per-warp global scratch (L2-resident, 2-4 bytes per node), which
+// keeps the shared memory per warp small enough for 32 warps per SM.
 // ------------------------------------------------------------------------------------------------
 MapSortSmem map_sort_plan(const DevLattice& L, int max_warps)
 {
@@ -45,19 +47,20 @@ MapSortSmem map_sort_plan(const DevLattice& L, int max_warps)
     auto wtake = [&](size_t bytes) { int r = w; w += (int)al16(bytes); return r; };
     S.w_bits = wtake(4 * (size_t)L.n_words);
     S.w_wpre = wtake(2 * (size_t)L.n_words);
-    S.w_t = wtake((S.wide ? 4 : 2) * (size_t)L.nnode);
     S.w_hist = wtake(4 * (size_t)S.hist_cap);
     S.warp_bytes = w;
-    const int room = 227 * 1024 - o;
-    S.nw = std::max(0, std::min(max_warps, room / w));
+    // two CTAs per SM when 2 x (tables + max_warps warps) fit, else one CTA with as many warps as fit
+    const int limit = 227 * 1024;
+    if (2 * (o + w * max_warps + 1024) <= limit) { S.nw = max_warps; S.ctas = 2; }
+    else { S.nw = std::max(0, std::min(max_warps, (limit - o) / w)); S.ctas = 1; }
     S.warp0 = take((size_t)w * std::max(S.nw, 1));
     S.total = o;
     return S;
 }
 
 template <class TT, bool kFast>
-__global__ void __launch_bounds__(kMapSortMaxWarps * 32, 1)
-k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl, int* __restrict__ counter)
+__global__ void __launch_bounds__(kMapSortMaxWarps * 32, 2)
+k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl, int* __restrict__ counter, void* __restrict__ scratch)
 {
     extern __shared__ __align__(16) char smem[];
     constexpr unsigned kOff = (unsigned)(TT)~(TT)0;             // marker of a node that left the grid
@@ -68,7 +71,7 @@ k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl,
     char* wsm = smem + S.warp0 + warp * S.warp_bytes;
     unsigned* bits = (unsigned*)(wsm + S.w_bits);
     unsigned short* wpre = (unsigned short*)(wsm + S.w_wpre);
-    TT* s_t = (TT*)(wsm + S.w_t);
+    TT* __restrict__ s_t = (TT*)scratch + (size_t)(blockIdx.x * (T >> 5) + warp) * (size_t)((L.nnode + 31) & ~31);   // this warp's targets
     int* hist = (int*)(wsm + S.w_hist);
 
     for (int k = tid; k < L.pe_pad + kLocK; k += T) s_thr_p[k] = k < L.pe_pad ? L.thr_p[k] : __longlong_as_double(0x7ff0000000000000ll);
@@ -348,20 +351,31 @@ static std::atomic<int64_t> g_launches{0};
 int64_t launch_count() { return g_launches.load(); }
 void count_launch() { ++g_launches; }
 
-cudaError_t launch_map_sort(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, int n_sm, int* counter, cudaStream_t st)
+static int map_sort_warps()
+{
+    static const int want = [] { const char* e = std::getenv("PM_MAPSORT_WARPS"); return e ? std::max(1, std::min(kMapSortMaxWarps, std::atoi(e))) : kMapSortMaxWarps; }();
+    return want;
+}
+
+size_t map_sort_scratch_bytes(const DevLattice& L, int n_sm)
+{
+    const MapSortSmem S = map_sort_plan(L, map_sort_warps());
+    return (size_t)n_sm * S.ctas * std::max(S.nw, 1) * (size_t)((L.nnode + 31) & ~31) * (S.wide ? 4 : 2);
+}
+
+cudaError_t launch_map_sort(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, int n_sm, int* counter, void* scratch, cudaStream_t st)
 {
     // warps per CTA: as many as shared memory holds, at most kMapSortMaxWarps (PM_MAPSORT_WARPS: test hook)
-    static const int want = [] { const char* e = std::getenv("PM_MAPSORT_WARPS"); return e ? std::max(1, std::min(kMapSortMaxWarps, std::atoi(e))) : kMapSortMaxWarps; }();
-    const MapSortSmem S = map_sort_plan(L, want);
+    const MapSortSmem S = map_sort_plan(L, map_sort_warps());
     if (S.nw < 1) return cudaErrorInvalidConfiguration;
-    using Fn = void (*)(DevLattice, MapSortSmem, int, int, NodeLists, int*);
+    using Fn = void (*)(DevLattice, MapSortSmem, int, int, NodeLists, int*, void*);
     const bool fast = L.bk_kmax <= kLocK;
     const Fn fn = S.wide ? (fast ? k_map_sort<unsigned, true> : k_map_sort<unsigned, false>)
                          : (fast ? k_map_sort<unsigned short, true> : k_map_sort<unsigned short, false>);
     cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
-    const int grid = std::max(1, std::min(n_sm, (n_blk + S.nw - 1) / S.nw));
-    fn<<<grid, S.nw * 32, S.total, st>>>(L, S, cell_begin, n_blk, nl, counter);
+    const int grid = std::max(1, std::min(n_sm * S.ctas, (n_blk + S.nw - 1) / S.nw));
+    fn<<<grid, S.nw * 32, S.total, st>>>(L, S, cell_begin, n_blk, nl, counter, scratch);
     ++g_launches;
     return cudaGetLastError();
 }

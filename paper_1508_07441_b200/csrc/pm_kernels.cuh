@@ -17,13 +17,14 @@ constexpr int kMapSortMaxWarps = 16;  // k_map_sort: warps (= source cells in fl
 constexpr int kHistCap = 512;         // k_map_sort: rank counters per window (one window unless a source cell hits more cells)
 
 // shared-memory plan of k_map_sort: tables shared by the CTA, then one private area per warp (byte offsets)
-struct MapSortSmem { int thr_p, thr_q, bk_p, bk_q, tp, tq, tx, warp0, warp_bytes, w_bits, w_wpre, w_t, w_hist, nw, wide, hist_cap, total; };
+struct MapSortSmem { int thr_p, thr_q, bk_p, bk_q, tp, tq, tx, warp0, warp_bytes, w_bits, w_wpre, w_hist, nw, ctas, wide, hist_cap, total; };
 MapSortSmem map_sort_plan(const DevLattice& L, int max_warps);
 int64_t launch_count();
 void count_launch();
 
 // pattern pass
-cudaError_t launch_map_sort(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, int n_sm, int* counter, cudaStream_t st);
+size_t map_sort_scratch_bytes(const DevLattice& L, int n_sm);      // per-warp target scratch of k_map_sort (global memory)
+cudaError_t launch_map_sort(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, int n_sm, int* counter, void* scratch, cudaStream_t st);
 // scan of the hit counts + rowptr; summary = {nnz, max hits, nodes on the grid, (segments), overflow flag: nnz > capacity >= 0}
 cudaError_t launch_scan_rows(const DevLattice& L, int n_blk, const NodeLists& nl, int64_t* cellbase, int64_t* rowptr,
                              int64_t* summary, int64_t capacity, cudaStream_t st);
