@@ -350,7 +350,7 @@ int po_cell_nodes(const double* pe, int Np, const double* qe, int Nq, int cell,
  * Tables that depend on the channel list only (computed once per build): coupled mask, the
  * coefficients c^L, and Clebsch-Gordan tables of the bipolar harmonics that occur.
  * ---------------------------------------------------------------------------------------- */
-#define PO_MAXL 8      /* max total orbital L kept in tables */
+#define PO_MAXL 10     /* max total orbital L kept in tables: L <= J + 3/2 = 10 for J = 17/2 (Table 1) */
 typedef struct { int l, lam, L; double cg[2 * PO_MAXL + 1][2 * PO_LMAX + 1]; } po_triple;
 typedef struct {
     int n_ch, n_tri, lmax;

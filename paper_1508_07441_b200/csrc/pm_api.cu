@@ -90,10 +90,12 @@ struct pm_lattice {
     uint64_t geo_version = 0;          // geometry version the channel tables were uploaded for
     int device = -1;
     char* d_blob = nullptr;            // channel tables (coupled lists, bra harmonics, term lists)
-    bool have_plan = false;
+    bool have_plan = false;            // every group has its launch plan
     bool jit_failed = false;           // run-time compilation was tried for this lattice and failed (jit_error says why)
     std::string jit_error;
-    pm::FillLaunch plan{};
+    std::vector<pm::GroupTables> groups;   // column-channel groups (one unless the set exceeds what one kernel holds)
+    struct GroupDev { pm::DevLattice dev; pm::FillLaunch plan; };
+    std::vector<GroupDev> gdev;
     cudaEvent_t ev_fill0 = nullptr, ev_fill1 = nullptr;   // around the last fill kernel, on its stream (pm_last_fill_ms)
     bool fill_timed = false;
     unsigned long long hash = 0;       // pm::tables_hash of T (selects a generated fill kernel)
@@ -225,25 +227,32 @@ int32_t ensure_device(pm_lattice* L)
     const pm::Tables& T = L->T;
     pm::DevLattice D = G->geo;
     D.n_ch = L->n_ch;
-    D.totcoup = T.totcoup; D.n_slot = T.n_slot; D.n_fun = (int)T.fun.size(); D.lmax = T.lmax;
+    D.totcoup = T.totcoup; D.n_bra = T.n_slot; D.lmax = T.lmax;
     D.ny = pm::ylm_index(T.lmax, T.lmax) + 1;
     std::vector<double> bra;
     pm::build_bra(T, G->rule_t[2], bra);
     std::vector<int32_t> o_alpha(T.totcoup);
     for (int a = 0; a < L->n_ch; ++a) for (int o = T.cl_off[a]; o < T.cl_off[a + 1]; ++o) o_alpha[o] = a;
-    std::vector<int4> fun(T.fun.size());
-    for (size_t f = 0; f < T.fun.size(); ++f) fun[f] = make_int4(T.fun[f].sa0, T.fun[f].sb0, T.fun[f].nM, T.fun[f].L);
     Blob B;
     const size_t o_cloff = B.put(T.cl_off.data(), 4 * T.cl_off.size()), o_cl = B.put(T.cl.data(), 4 * T.cl.size());
     const size_t o_oa = B.put(o_alpha.data(), 4 * o_alpha.size());
     const size_t o_bra = B.put(bra.data(), 8 * bra.size());
-    const size_t o_ktoff = B.put(T.kt_off.data(), 4 * T.kt_off.size()), o_ktip = B.put(T.kt_ip.data(), 4 * T.kt_ip.size());
-    const size_t o_ktiq = B.put(T.kt_iq.data(), 4 * T.kt_iq.size()), o_ktc = B.put(T.kt_c.data(), 8 * T.kt_c.size());
-    const size_t o_fun = B.put(fun.data(), sizeof(int4) * fun.size());
-    const size_t o_otoff = B.put(T.ot_off.data(), 4 * T.ot_off.size()), o_otf = B.put(T.ot_f.data(), 4 * T.ot_f.size());
-    const size_t o_otc = B.put(T.ot_c.data(), 8 * T.ot_c.size());
     const size_t o_ya = B.put(T.ya.data(), 8 * T.ya.size()), o_yb = B.put(T.yb.data(), 8 * T.yb.size());
     const size_t o_yd = B.put(T.ydiag.data(), 8 * T.ydiag.size());
+    struct GOff { size_t ktoff, ktip, ktiq, ktc, fun, otoff, otf, otc, ga, gm, gap; };
+    std::vector<GOff> go(L->groups.size());
+    for (size_t g = 0; g < L->groups.size(); ++g) {
+        const pm::GroupTables& Gt = L->groups[g];
+        std::vector<int4> fun(Gt.fun.size());
+        for (size_t f = 0; f < Gt.fun.size(); ++f) fun[f] = make_int4(Gt.fun[f].sa0, Gt.fun[f].sb0, Gt.fun[f].nM, Gt.fun[f].L);
+        go[g].ktoff = B.put(Gt.kt_off.data(), 4 * Gt.kt_off.size()); go[g].ktip = B.put(Gt.kt_ip.data(), 4 * Gt.kt_ip.size());
+        go[g].ktiq = B.put(Gt.kt_iq.data(), 4 * Gt.kt_iq.size()); go[g].ktc = B.put(Gt.kt_c.data(), 8 * Gt.kt_c.size());
+        go[g].fun = B.put(fun.data(), sizeof(int4) * fun.size());
+        go[g].otoff = B.put(Gt.ot_off.data(), 4 * Gt.ot_off.size()); go[g].otf = B.put(Gt.ot_f.data(), 4 * Gt.ot_f.size());
+        go[g].otc = B.put(Gt.ot_c.data(), 8 * Gt.ot_c.size());
+        go[g].ga = B.put(Gt.o_alpha.data(), 4 * Gt.o_alpha.size()); go[g].gm = B.put(Gt.o_m.data(), 4 * Gt.o_m.size());
+        go[g].gap = B.put(Gt.o_ap.data(), 4 * Gt.o_ap.size());
+    }
     cudaError_t e;
     if ((e = cudaMalloc(&L->d_blob, B.b.size())) != cudaSuccess) return cuda_fail(e, "cudaMalloc(channel tables)");
     if ((e = cudaMemcpy(L->d_blob, B.b.data(), B.b.size(), cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_fail(e, "cudaMemcpy(channel tables)");
@@ -251,11 +260,20 @@ int32_t ensure_device(pm_lattice* L)
     char* b = L->d_blob;
     D.cl_off = (const int*)(b + o_cloff); D.cl = (const int*)(b + o_cl); D.o_alpha = (const int*)(b + o_oa);
     D.bra = (const double*)(b + o_bra);
-    D.kt_off = (const int*)(b + o_ktoff); D.kt_ip = (const int*)(b + o_ktip); D.kt_iq = (const int*)(b + o_ktiq);
-    D.kt_c = (const double*)(b + o_ktc);
-    D.fun = (const int4*)(b + o_fun);
-    D.ot_off = (const int*)(b + o_otoff); D.ot_f = (const int*)(b + o_otf); D.ot_c = (const double*)(b + o_otc);
     D.ya = (const double*)(b + o_ya); D.yb = (const double*)(b + o_yb); D.ydiag = (const double*)(b + o_yd);
+    L->gdev.assign(L->groups.size(), pm_lattice::GroupDev{});
+    for (size_t g = 0; g < L->groups.size(); ++g) {
+        const pm::GroupTables& Gt = L->groups[g];
+        pm::DevLattice Dg = D;
+        Dg.n_slot = Gt.n_slot; Dg.n_fun = (int)Gt.fun.size(); Dg.n_out = (int)Gt.o_alpha.size();
+        Dg.kt_off = (const int*)(b + go[g].ktoff); Dg.kt_ip = (const int*)(b + go[g].ktip); Dg.kt_iq = (const int*)(b + go[g].ktiq);
+        Dg.kt_c = (const double*)(b + go[g].ktc);
+        Dg.fun = (const int4*)(b + go[g].fun);
+        Dg.ot_off = (const int*)(b + go[g].otoff); Dg.ot_f = (const int*)(b + go[g].otf); Dg.ot_c = (const double*)(b + go[g].otc);
+        Dg.g_alpha = (const int*)(b + go[g].ga); Dg.g_m = (const int*)(b + go[g].gm); Dg.g_ap = (const int*)(b + go[g].gap);
+        L->gdev[g].dev = Dg;
+    }
+    D = L->gdev[0].dev;                                 // (the pattern kernels read the geometric and coupled-list fields only)
     L->dev = D;
     L->geo_version = G->version;
     L->have_plan = false;
@@ -311,9 +329,11 @@ int32_t make_lattice(pm_geometry* G, const pm_channel* ch, int32_t n_ch, int32_t
     msg = pm::build_tables(ch, n_ch, J2, T2, statistics, L->T);
     if (!msg.empty()) { delete L; return fail(PM_ERR_CHANNEL, msg); }
     L->hash = pm::tables_hash(L->T);
-    if ((int)L->T.fun.size() > pm::kFillMaxFun || L->T.n_slot > pm::kFillMaxSlot) {
-        delete L; return fail(PM_ERR_CHANNEL, "channel set needs more orbital functions than this build supports");
-    }
+    pm::build_groups(L->T, ch, pm::kFillMaxSlot, pm::kFillMaxFun, L->groups);
+    for (const pm::GroupTables& Gt : L->groups)
+        if (Gt.n_slot > pm::kFillMaxSlot || (int)Gt.fun.size() > pm::kFillMaxFun) {
+            delete L; return fail(PM_ERR_CHANNEL, "one orbital pair (l', lambda') of this channel set needs more ket slots than a kernel holds");
+        }
     static std::atomic<uint64_t> next_id{1};
     L->id = next_id++;
     L->G = G;
@@ -474,7 +494,8 @@ const char* pm_lattice_fill_kernel(const pm_lattice* lat)
 {
     if (!lat) return "";
     if (pm::fill_has_spec(lat->hash)) return pm::fill_variant_name(lat->hash);
-    if (lat->have_plan) return lat->plan.name;                              // what the last fill ran: "jit" or "generic"
+    if (lat->groups.size() > 1) return "generic-grouped";                   // table-driven kernel, one launch per column-channel group
+    if (lat->have_plan && !lat->gdev.empty()) return lat->gdev[0].plan.name; // what the last fill ran: "jit" or "generic"
     return (pm::jit_enabled() && !lat->jit_failed) ? "jit" : "generic";
 }
 
@@ -489,6 +510,7 @@ int32_t pm_diag_jit_compile(const pm_lattice* lat, int64_t* cubin_bytes)
     if (!lat) return fail(PM_ERR_ARG, "lat is NULL");
     std::string err;
     size_t n = 0;
+    if (lat->groups.size() > 1) return fail(PM_ERR_STATE, "this channel set runs the table-driven kernel group by group; nothing to compile");
     if (!pm::jit_compile_check(lat->T, 12, 4, &n, err)) return fail(PM_ERR_STATE, err);
     if (cubin_bytes) *cubin_bytes = (int64_t)n;
     return PM_OK;
@@ -593,20 +615,25 @@ int32_t fill_block(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const 
     if (cell_begin == cell_end) return PM_OK;
     const int n_blk = cell_end - cell_begin;
     cudaError_t e;
-    if (!lat->have_plan && !pm::fill_has_spec(lat->hash) && pm::jit_enabled() && !lat->jit_failed) {
+    const bool grouped = lat->gdev.size() > 1;         // big channel sets: one table-driven launch per column-channel group
+    if (!lat->have_plan && !grouped && !pm::fill_has_spec(lat->hash) && pm::jit_enabled() && !lat->jit_failed) {
         // no build-time kernel for this channel set: specialise at run time (pm_jit.hpp), else fall back below
-        if (pm::fill_plan_jit(lat->dev, lat->T, lat->hash, G->n_sm, &lat->plan, lat->jit_error)) lat->have_plan = true;
+        if (pm::fill_plan_jit(lat->gdev[0].dev, lat->T, lat->hash, G->n_sm, &lat->gdev[0].plan, lat->jit_error)) lat->have_plan = true;
         else lat->jit_failed = true;
     }
     if (!lat->have_plan) {
-        e = pm::fill_plan(lat->dev, lat->hash, G->n_sm, &lat->plan);
-        if (e == cudaErrorInvalidConfiguration) { cudaGetLastError(); return fail(PM_ERR_NOMEM, "channel set needs more shared memory than one SM has"); }
-        if (e != cudaSuccess) return cuda_fail(e, "fill_plan");
+        for (auto& gd : lat->gdev) {
+            e = pm::fill_plan(gd.dev, grouped ? 0ull : lat->hash, G->n_sm, &gd.plan);
+            if (e == cudaErrorInvalidConfiguration) { cudaGetLastError(); return fail(PM_ERR_NOMEM, "channel set needs more shared memory than one SM has"); }
+            if (e != cudaSuccess) return cuda_fail(e, "fill_plan");
+        }
         lat->have_plan = true;
     }
     if ((e = cudaEventRecord(lat->ev_fill0, st)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
-    e = pm::launch_fill(lat->dev, lat->plan, cell_begin, n_blk, G->nl, d_rowptr, d_vals, d_colidx, G->d_counter, guard, st);
-    if (e != cudaSuccess) return cuda_fail(e, "k_fill");
+    for (auto& gd : lat->gdev) {
+        e = pm::launch_fill(gd.dev, gd.plan, cell_begin, n_blk, G->nl, d_rowptr, d_vals, d_colidx, G->d_counter, guard, st);
+        if (e != cudaSuccess) return cuda_fail(e, "k_fill");
+    }
     if ((e = cudaEventRecord(lat->ev_fill1, st)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
     lat->fill_timed = true;
     return PM_OK;

@@ -28,7 +28,8 @@ namespace pm {
 
 struct DevLattice {
     int Np, Nq, n_ch, n_p, n_q, n_x, nnode, n_cells, n_words, pe_pad, qe_pad;
-    int totcoup, n_slot, n_fun, lmax, ny;
+    int totcoup, n_slot, n_fun, lmax, ny;       // n_slot / n_fun: ket slots and orbital functions of THIS column-channel group
+    int n_out, n_bra;                           // outputs (alpha, alpha') of this group; bra slots of the whole channel set
     unsigned mg_npq, mg_nq, mg_Nq;              // ceil(2^32 / d) for d = n_p*n_q, n_q, Nq: exact division of node and cell ids (x*d < 2^32)
     const double *pe, *qe;                      // edges, Np+1 / Nq+1 entries (padded with +inf to pe_pad / qe_pad)
     const double *thr_p, *thr_q;                // sqrt_threshold(edge), padded with +inf to a power of two
@@ -37,8 +38,9 @@ struct DevLattice {
     int bk_kmax;                                // most thresholds any bucket of either axis holds
     const double *tp, *wp, *tq, *wq, *tx, *wx;  // Gauss-Legendre rules on [-1,1]
     const double *sx;                           // sqrt(1-x^2) per x-node
-    const int *cl_off, *cl, *o_alpha;           // coupled lists; o_alpha[o] = alpha of output o
-    const double *bra;                          // [n_x][n_slot]
+    const int *cl_off, *cl, *o_alpha;           // coupled lists of the whole set; o_alpha[o] = alpha of global output o
+    const int *g_alpha, *g_m, *g_ap;            // outputs of this group: row channel, position in the row's coupled list, column channel
+    const double *bra;                          // [n_x][n_bra]
     const int *kt_off, *kt_ip, *kt_iq; const double *kt_c;
     const int4 *fun;                            // (sa0, sb0, nM, L)
     const int *ot_off, *ot_f; const double *ot_c;

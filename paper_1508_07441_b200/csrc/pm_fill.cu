@@ -77,8 +77,13 @@ cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int n_sm, Fi
     const unsigned long long key = fill_has_spec(hash) ? hash : 0ull;
     const int want = preferred_warps();
     const FillVariant* best = nullptr;          // largest warp count <= want whose shared memory fits, else the smallest that fits
+    auto plan_of = [&](const FillVariant& v) {         // the bra table moves to global memory when it does not fit beside the tiles
+        FillSmem s = fill_smem_plan(L, v.nw, v.rb, true);
+        if (s.total > kSmemLimit && v.hash == 0ull) s = fill_smem_plan(L, v.nw, v.rb, false);
+        return s;
+    };
     for (const FillVariant& v : kVariants) {
-        if (v.hash != key || fill_smem_plan(L, v.nw, v.rb).total > kSmemLimit) continue;
+        if (v.hash != key || plan_of(v).total > kSmemLimit) continue;
         if (!best) { best = &v; continue; }
         const bool v_ok = v.nw <= want, b_ok = best->nw <= want;
         if ((v_ok && (!b_ok || v.nw > best->nw)) || (!v_ok && !b_ok && v.nw < best->nw)) best = &v;
@@ -89,7 +94,7 @@ cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int n_sm, Fi
     out->nw = best->nw;
     out->name = best->name;
     out->jit = false;
-    out->smem = fill_smem_plan(L, best->nw, best->rb);
+    out->smem = plan_of(*best);
     cudaError_t e = ensure_smem_limit(out->fn, out->smem.total);
     if (e != cudaSuccess) return e;
     if ((e = ensure_smem_limit(out->fn_cols, out->smem.total)) != cudaSuccess) return e;

@@ -20,25 +20,34 @@
 
 namespace pm {
 
-constexpr int kFillMaxSlot = 160;      // table-driven fallback: slots / functions it can hold
-constexpr int kFillMaxFun = 256;
-constexpr int kFillMaxY = 45;
+constexpr int kFillMaxSlot = 96;       // ket slots / orbital functions one kernel launch holds (larger channel sets are
+constexpr int kFillMaxFun = 320;       // split into column-channel groups, pm_tables.hpp)
+constexpr int kFillMaxY = 91;          // harmonics per direction up to l = PM_MAX_L = 12
 
 // Table-driven ket code for channel sets without a generated kernel (slow: local arrays, table loads).
 struct SpecGeneric {
     static constexpr bool kStatic = false;
     static constexpr int NS = kFillMaxSlot, NF = kFillMaxFun, NCH = kFillMaxFun / 32, MAXM = 99, MAXL1 = 99;
     static constexpr unsigned long long kHash = 0ull;
-    static __device__ __noinline__ void ket(const DevLattice& L, double om, double uxa, double uza, double uxb, double uzb,
-                                            double (&K)[NS])
+    // writes the node's column of the K tile directly (no per-thread K array): col = tile + lane, np slot pairs
+    static __device__ __noinline__ void ket_tile(const DevLattice& L, double om, double uxa, double uza, double uxb, double uzb,
+                                                 double2* __restrict__ col, int stride, int np, int ns)
     {
         double Yp[kFillMaxY], Yq[kFillMaxY];
         ylm_fill(L.lmax, uxa, uza, L.ya, L.yb, L.ydiag, Yp);
         ylm_fill(L.lmax, uxb, uzb, L.ya, L.yb, L.ydiag, Yq);
-        for (int s = 0; s < L.n_slot; ++s) {
-            double v = 0.0;
-            for (int t = L.kt_off[s]; t < L.kt_off[s + 1]; ++t) v += L.kt_c[t] * Yp[L.kt_ip[t]] * Yq[L.kt_iq[t]];
-            K[s] = v * om;
+        for (int i = 0; i < np; ++i) {
+            double v[2] = {0.0, 0.0};
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int s = 2 * i + h;
+                if (s < ns) {
+                    double a = 0.0;
+                    for (int t = L.kt_off[s]; t < L.kt_off[s + 1]; ++t) a += L.kt_c[t] * Yp[L.kt_ip[t]] * Yq[L.kt_iq[t]];
+                    v[h] = a * om;
+                }
+            }
+            col[i * stride] = make_double2(v[0], v[1]);
         }
     }
 };
@@ -52,15 +61,15 @@ constexpr int kTileStride = 33;        // double2 per K-tile row: 32 nodes + 1 p
 inline int fill_align16(int b) { return (b + 15) & ~15; }
 
 // shared-memory plan for nw warps: tables shared by the CTA, then one private area per warp
-inline FillSmem fill_smem_plan(const DevLattice& L, int nw, int row_batch)
+inline FillSmem fill_smem_plan(const DevLattice& L, int nw, int row_batch, bool bra_in_smem = true)
 {
     FillSmem s{};
     int o = 0;
     auto take = [&](int bytes) { int r = o; o += fill_align16(bytes); return r; };
     s.dp = take(8 * L.Np); s.dq = take(8 * L.Nq);
     s.tp = take(8 * L.n_p); s.tq = take(8 * L.n_q); s.tx = take(8 * L.n_x); s.sx = take(8 * L.n_x); s.wx = take(8 * L.n_x);
-    s.bra = take(8 * L.n_x * (L.n_slot + 1));       // rows padded with one zero slot
-    s.odesc = take(4 * L.totcoup); s.ofi = take(4 * L.totcoup); s.oc = take(24 * L.totcoup);
+    s.bra = bra_in_smem ? take(8 * L.n_x * (L.n_bra + 1)) : -1;      // rows padded with one zero slot; -1: read from global memory
+    s.odesc = take(4 * L.n_out); s.ofi = take(4 * L.n_out); s.oc = take(24 * L.n_out);
     const int np = (L.n_slot + 1) / 2;              // slot pairs
     int w = 0;
     auto wtake = [&](int bytes) { int r = w; w += fill_align16(bytes); return r; };
@@ -95,9 +104,9 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
     double* s_dp = (double*)(smem + S.dp);   double* s_dq = (double*)(smem + S.dq);
     double* s_tp = (double*)(smem + S.tp);   double* s_tq = (double*)(smem + S.tq);   double* s_tx = (double*)(smem + S.tx);
     double* s_sx = (double*)(smem + S.sx);   double* s_wx = (double*)(smem + S.wx);
-    double* s_bra = (double*)(smem + S.bra);
+    double* s_bra = (double*)(smem + (S.bra >= 0 ? S.bra : 0));
     int* s_odesc = (int*)(smem + S.odesc);             // per output o: cl_off[alpha] | nc << 12 | m << 19 | alpha' << 25
-    int* s_ofi = (int*)(smem + S.ofi);                 // f0 | f1 << 8 | f2 << 16 | n_terms << 24
+    int* s_ofi = (int*)(smem + S.ofi);                 // f0 | f1 << 10 | f2 << 20 | (n_terms - 1) << 30
     double* s_oc = (double*)(smem + S.oc);             // [o][3] coefficients c^L (0 where there is no term)
     char* wsm = smem + S.warp0 + warp * S.warp_bytes;
     double2* s_tile = (double2*)(wsm + S.w_tile);
@@ -115,37 +124,41 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
     for (int k = tid; k < L.n_p; k += T) s_tp[k] = L.tp[k];
     for (int k = tid; k < L.n_q; k += T) s_tq[k] = L.tq[k];
     for (int k = tid; k < L.n_x; k += T) { s_tx[k] = L.tx[k]; s_sx[k] = L.sx[k]; s_wx[k] = L.wx[k]; }
-    const int nsb = ns + 1;                             // bra rows carry one trailing zero slot (index ns)
-    for (int k = tid; k < L.n_x * nsb; k += T) { const int c = k / nsb, sl = k - c * nsb; s_bra[k] = sl < ns ? L.bra[c * ns + sl] : 0.0; }
-    for (int o = tid; o < L.totcoup; o += T) {
-        const int al = L.o_alpha[o], off = L.cl_off[al], nc = L.cl_off[al + 1] - off;
+    const int nb_ = Spec::kStatic ? Spec::NS : L.n_bra; // bra slots (the whole channel set's)
+    const int nsb = nb_ + 1;                            // shared-memory bra rows carry one trailing zero slot (index nb_)
+    if (S.bra >= 0)
+        for (int k = tid; k < L.n_x * nsb; k += T) { const int c = k / nsb, sl = k - c * nsb; s_bra[k] = sl < nb_ ? L.bra[c * nb_ + sl] : 0.0; }
+    const double* __restrict__ bra_tab = S.bra >= 0 ? s_bra : L.bra;      // big channel sets: the bra table stays in global memory
+    const int bra_stride = S.bra >= 0 ? nsb : nb_;
+    for (int o = tid; o < L.n_out; o += T) {
+        const int al = L.g_alpha[o], off = L.cl_off[al], nc = L.cl_off[al + 1] - off;
         const int t0 = L.ot_off[o], nt = L.ot_off[o + 1] - t0;
-        s_odesc[o] = off | (nc << 12) | ((o - off) << 19) | (L.cl[o] << 25);
-        int fi = nt << 24;
+        s_odesc[o] = off | (nc << 12) | (L.g_m[o] << 19) | (L.g_ap[o] << 25);
+        int fi = (nt > 0 ? nt - 1 : 0) << 30;
         for (int i = 0; i < 3; ++i) {
             s_oc[3 * o + i] = i < nt ? L.ot_c[t0 + i] : 0.0;
-            fi |= (i < nt ? L.ot_f[t0 + i] : 0) << (8 * i);
+            fi |= (i < nt ? L.ot_f[t0 + i] : 0) << (10 * i);
         }
         s_ofi[o] = fi;
     }
     // per-lane descriptors of function f = ch*32 + lane.  kPacked (at most 3 M-terms per function): byte i of fa / fb =
-    // bra / ket slot of term i, unused terms point at the zero bra slot; else fa = sa | sb << 8 | nM << 16.
+    // bra / ket slot of term i, unused terms point at the zero bra slot; else fa = sa | nM << 16, fb = sb.
     constexpr bool kPacked = Spec::MAXM <= 3;
     int fa[NCH], fb[NCH];
 #pragma unroll
     for (int ch = 0; ch < NCH; ++ch) {
         const int f = ch * 32 + lane;
-        fa[ch] = kPacked ? (ns | (ns << 8) | (ns << 16)) : 0;
+        fa[ch] = kPacked ? (nb_ | (nb_ << 8) | (nb_ << 16)) : 0;
         fb[ch] = 0;
         if (f < nf) {
             const int4 fn = L.fun[f];
             if (kPacked) {
                 fa[ch] = 0;
                 for (int i = 0; i < 3; ++i) {
-                    fa[ch] |= (i < fn.z ? fn.x + i : ns) << (8 * i);
+                    fa[ch] |= (i < fn.z ? fn.x + i : nb_) << (8 * i);
                     fb[ch] |= (i < fn.z ? fn.y + i : 0) << (8 * i);
                 }
-            } else fa[ch] = fn.x | (fn.y << 8) | (fn.z << 16);
+            } else { fa[ch] = fn.x | (fn.z << 16); fb[ch] = fn.y; }
         }
     }
     __syncthreads();                                    // the only block-level barrier
@@ -176,11 +189,11 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
 #pragma unroll
             for (int bb = 0; bb < kRowBatch; ++bb) { nrm[bb] = s_norm[bb]; hcl[bb] = kCols ? s_hcol[bb] : 0; }
 #pragma unroll 2
-            for (int o = lane; o < L.totcoup; o += 32) {
+            for (int o = lane; o < L.n_out; o += 32) {
                 const int od = s_odesc[o], fi = s_ofi[o];
                 const int clo = od & 4095, nc = (od >> 12) & 127, mm = (od >> 19) & 63, ap = (unsigned)od >> 25;
                 const double c0 = s_oc[3 * o], c1 = s_oc[3 * o + 1], c2 = s_oc[3 * o + 2];
-                const int f0 = fi & 255, f1 = (fi >> 8) & 255, f2 = (fi >> 16) & 255;
+                const int f0 = fi & 1023, f1 = (fi >> 10) & 1023, f2 = (fi >> 20) & 1023;
                 // entry of target k0+bb in row alpha: element H*clo + (k0+bb)*nc + m of the cell's block (fits 32 bits)
                 const unsigned idx0 = (unsigned)(H * clo + k0 * nc + mm);
                 const char* acc0 = (const char*)s_acc;
@@ -191,7 +204,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                         const char* acc = acc0 + bb * (8 * nf);
                         double v = fma(c2, *(const double*)(acc + a2), fma(c1, *(const double*)(acc + a1), c0 * *(const double*)(acc + a0)));
                         if (Spec::MAXL1 > 3) {                           // more than three L values: the tail comes from the tables
-                            const int t0 = L.ot_off[o], nt = fi >> 24;
+                            const int t0 = L.ot_off[o], nt = (int)((unsigned)fi >> 30) + 1;
                             for (int t = 3; t < nt; ++t) v = fma(L.ot_c[t0 + t], ((const double*)acc)[L.ot_f[t0 + t]], v);
                         }
                         const unsigned e = idx0 + (unsigned)(bb * nc);
@@ -247,15 +260,14 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 const double ax = -0.5 * psx, az = fma(-0.5, px, -0.75 * q);
                 const double bx = psx, bz = fma(-0.5, q, px);
                 const double ra = rsqrt(fma(ax, ax, az * az)), rb = rsqrt(fma(bx, bx, bz * bz));
-                double K[Spec::NS];
-                Spec::ket(L, om, ax * ra, az * ra, bx * rb, bz * rb, K);
-                if (Spec::kStatic) {
+                if constexpr (Spec::kStatic) {
+                    double K[Spec::NS];
+                    Spec::ket(L, om, ax * ra, az * ra, bx * rb, bz * rb, K);
 #pragma unroll
                     for (int i = 0; i < NP; ++i)
                         s_tile[i * kTileStride + lane] = make_double2(K[2 * i], (2 * i + 1 < Spec::NS) ? K[(2 * i + 1) % Spec::NS] : 0.0);
                 } else {
-                    for (int i = 0; i < np; ++i)
-                        s_tile[i * kTileStride + lane] = make_double2(K[2 * i], (2 * i + 1 < ns) ? K[2 * i + 1] : 0.0);
+                    Spec::ket_tile(L, om, ax * ra, az * ra, bx * rb, bz * rb, s_tile + lane, kTileStride, np, ns);
                 }
             }
             __syncwarp();
@@ -313,7 +325,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 }
                 __syncwarp();
                 const int cseg = __shfl_sync(0xffffffffu, c, jb);
-                const double* bra = s_bra + cseg * nsb;
+                const double* bra = bra_tab + cseg * bra_stride;
 #pragma unroll
                 for (int ch = 0; ch < NCH; ++ch) {
                     if (kPacked) {
@@ -323,7 +335,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                         v = fma(bra[ia >> 16], s_sseg[ib >> 16], v);
                         runT[ch] += v;
                     } else {
-                        const int sa = fa[ch] & 255, sb = (fa[ch] >> 8) & 255, nM = fa[ch] >> 16;
+                        const int sa = fa[ch] & 65535, sb = fb[ch], nM = fa[ch] >> 16;
                         double v = 0.0;
                         for (int i = 0; i < nM; ++i) v = fma(bra[sa + i], s_sseg[sb + i], v);
                         runT[ch] += v;

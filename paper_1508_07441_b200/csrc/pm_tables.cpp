@@ -279,6 +279,71 @@ std::string build_tables(const pm_channel* ch, int n_ch, int J2, int T2, int sta
     return "";
 }
 
+void build_groups(const Tables& T, const pm_channel* ch, int max_slot, int max_fun, std::vector<GroupTables>& groups)
+{
+    groups.clear();
+    const int n_tri = (int)T.tri.size(), n_fun = (int)T.fun.size();
+    // classes of ket triples by (l', lam'), in order of first appearance
+    std::map<std::pair<int, int>, int> cls_id;
+    std::vector<int> tri_cls((size_t)n_tri), cls_slots, cls_funs;
+    for (int t = 0; t < n_tri; ++t) {
+        auto key = std::make_pair(T.tri[(size_t)t].l, T.tri[(size_t)t].lam);
+        auto it = cls_id.find(key);
+        if (it == cls_id.end()) { it = cls_id.emplace(key, (int)cls_slots.size()).first; cls_slots.push_back(0); cls_funs.push_back(0); }
+        tri_cls[(size_t)t] = it->second;
+        cls_slots[(size_t)it->second] += T.tri[(size_t)t].nM;
+    }
+    for (const OrbFun& f : T.fun) cls_funs[(size_t)tri_cls[(size_t)f.tb]]++;
+    const int n_cls = (int)cls_slots.size();
+    std::vector<int> cls_grp((size_t)n_cls, 0);
+    int n_grp = 1;
+    if (T.n_slot > max_slot || n_fun > max_fun) {
+        int gs = 0, gf = 0;
+        n_grp = 0;
+        for (int c = 0; c < n_cls; ++c) {
+            if (n_grp == 0 || gs + cls_slots[(size_t)c] > max_slot || gf + cls_funs[(size_t)c] > max_fun) { ++n_grp; gs = 0; gf = 0; }
+            cls_grp[(size_t)c] = n_grp - 1;
+            gs += cls_slots[(size_t)c]; gf += cls_funs[(size_t)c];
+        }
+    }
+    groups.resize((size_t)n_grp);
+    std::vector<int> slot_local((size_t)T.n_slot, -1), fun_local((size_t)n_fun, -1);
+    for (int g = 0; g < n_grp; ++g) groups[(size_t)g].kt_off.assign(1, 0);
+    for (int t = 0; t < n_tri; ++t) {                  // local ket slots in triple order (one group: the global numbering)
+        GroupTables& G = groups[(size_t)cls_grp[(size_t)tri_cls[(size_t)t]]];
+        const Triple& tr = T.tri[(size_t)t];
+        for (int i = 0; i < tr.nM; ++i) {
+            const int s = tr.slot0 + i;
+            slot_local[(size_t)s] = G.n_slot++;
+            for (int k = T.kt_off[(size_t)s]; k < T.kt_off[(size_t)s + 1]; ++k) {
+                G.kt_ip.push_back(T.kt_ip[(size_t)k]); G.kt_iq.push_back(T.kt_iq[(size_t)k]); G.kt_c.push_back(T.kt_c[(size_t)k]);
+            }
+            G.kt_off.push_back((int32_t)G.kt_c.size());
+        }
+    }
+    for (int f = 0; f < n_fun; ++f) {
+        const OrbFun& F = T.fun[(size_t)f];
+        GroupTables& G = groups[(size_t)cls_grp[(size_t)tri_cls[(size_t)F.tb]]];
+        fun_local[(size_t)f] = (int)G.fun.size();
+        OrbFun L = F;
+        L.sb0 = slot_local[(size_t)F.sb0];
+        G.fun.push_back(L);
+    }
+    for (int g = 0; g < n_grp; ++g) groups[(size_t)g].ot_off.assign(1, 0);
+    for (int a = 0; a < T.n_ch; ++a)
+        for (int o = T.cl_off[(size_t)a]; o < T.cl_off[(size_t)a + 1]; ++o) {
+            const int b = T.cl[(size_t)o];
+            const auto it = cls_id.find(std::make_pair(ch[b].l, ch[b].lam));
+            // a column channel whose orbital pair carries no triple at all has only structural zeros: any group may write them
+            GroupTables& G = groups[(size_t)(it == cls_id.end() ? 0 : cls_grp[(size_t)it->second])];
+            G.o_alpha.push_back(a); G.o_m.push_back(o - T.cl_off[(size_t)a]); G.o_ap.push_back(b);
+            for (int k = T.ot_off[(size_t)o]; k < T.ot_off[(size_t)o + 1]; ++k) {
+                G.ot_f.push_back(fun_local[(size_t)T.ot_f[(size_t)k]]); G.ot_c.push_back(T.ot_c[(size_t)k]);
+            }
+            G.ot_off.push_back((int32_t)G.ot_f.size());
+        }
+}
+
 void build_bra(const Tables& T, const std::vector<double>& tx, std::vector<double>& bra)
 {
     const int ny = ylm_index(T.lmax, T.lmax) + 1;

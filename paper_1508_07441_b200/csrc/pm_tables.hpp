@@ -40,6 +40,23 @@ struct Tables {
     std::vector<double> ya, yb, ydiag;
 };
 
+// A column-channel group: the channels alpha' whose orbital pair (l', lam') falls into one set of classes.  Every ket
+// triple (l', lam', L), every orbital function and every output (alpha, alpha') belongs to exactly one group, so a group
+// is a complete sub-problem of the fill: it writes its own columns of every row.  Channel sets whose ket tables exceed
+// what one kernel holds (62 channels, J up to 17/2: 422 slots, 546 functions) are filled group by group.
+struct GroupTables {
+    int n_slot = 0;                                   // ket slots of the group, numbered locally
+    std::vector<int32_t> kt_off, kt_ip, kt_iq;        // ket terms per local slot
+    std::vector<double> kt_c;
+    std::vector<OrbFun> fun;                          // sa0: GLOBAL bra slot, sb0: LOCAL ket slot
+    std::vector<int32_t> o_alpha, o_m, o_ap;          // outputs: row channel, position in the row's coupled list, column channel
+    std::vector<int32_t> ot_off, ot_f;                // terms per output, f numbered locally
+    std::vector<double> ot_c;
+};
+
+// One group holding everything when the set fits (max_slot, max_fun), else a greedy packing of the (l', lam') classes.
+void build_groups(const Tables& T, const pm_channel* ch, int max_slot, int max_fun, std::vector<GroupTables>& groups);
+
 // Algebra (doubled arguments), exposed for host tests through the C ABI indirectly (pm_lattice_coupling).
 double clebsch(int j1, int m1, int j2, int m2, int j3, int m3);
 double sixj(int a, int b, int c, int d, int e, int f);

@@ -265,6 +265,7 @@ def _rebuild_from_G(wl, oracle):
     I.small_coupled(N=3, jmax=1, orders=(2, 3, 4), Nq=4, J2=3, parity=-1),     # J = 3/2-, L up to 3
     I.boson_lattice(4, 6, waves=((0, 0), (2, 2)), J=0, orders=(3, 2, 5), cq=0.7),   # bosons with d-waves, Np != Nq
     I.boson_lattice(3, 3, waves=((0, 2), (2, 0), (2, 2)), J=2, orders=(2, 2, 4)),   # J = L = 2
+    I.small_coupled(N=3, jmax=1, orders=(2, 2, 3), Nq=2, J2=9, parity=-1),          # J = 9/2-: lambda up to 6, L up to 6
 ], ids=lambda w: w.name)
 def test_build_equals_node_sum_of_pinned_G(oracle, wl):
     """po_build has its own tabulated route to the coefficient (po_tables_init, po_eval_bipolar, tri_of / coef);
