@@ -44,6 +44,7 @@ enum {
     PM_ERR_NOMEM = -6, PM_ERR_STATE = -7, PM_ERR_OVERFLOW = -8, PM_ERR_DEVICE = -9
 };
 enum { PM_FERMION_ISOSPIN = 0, PM_SPINLESS_BOSON = 1 };      /* `statistics` */
+enum { PM_NORM_WIDTH = 0, PM_NORM_P2 = 1 };                  /* cell normalisation, pm_lattice_set_normalisation */
 enum { PM_MAX_CHANNELS = 64, PM_MAX_ORDER = 64, PM_MAX_L = 12 };
 
 /* Create a lattice (host work only: validation, Gauss-Legendre rules, recoupling tables — PAPER.md:L247-256
@@ -76,6 +77,13 @@ int32_t pm_lattice_dims(const pm_lattice* lat, int64_t* M, int32_t* n_cells);
  * (reading R12); nodes must be strictly increasing inside (-1,1); the x-rule must be symmetric. */
 int32_t pm_lattice_rule(const pm_lattice* lat, int32_t axis, double* nodes, double* weights);
 int32_t pm_lattice_set_rule(pm_lattice* lat, int32_t axis, const double* nodes, const double* weights);
+
+/* Normalisation of the lattice states (eq. 21, is garbled there; reading R2):
+ *   PM_NORM_WIDTH (default, reading A): radial states normalised to delta(p - p'), cell norm B_k = e_{k+1} - e_k;
+ *                 node weight w * pq/(p'q'), prefactor (B_i Bbar_j B_i' Bbar_j')^(-1/2)
+ *   PM_NORM_P2    (reading B): states normalised in the p^2 dp measure, B_k = (e_{k+1}^3 - e_k^3)/3; node weight w * p^2 q^2.
+ * Both bases are orthonormal; the pattern does not depend on the choice.  Takes effect at the next pm_fill / pm_build. */
+int32_t pm_lattice_set_normalisation(pm_lattice* lat, int32_t normalisation);
 
 /* Channel tables (host out): coupled[n_ch*n_ch] (1 iff the integer selection rules couple alpha, alpha');
  * *n_functions = number of distinct orbital functions A^L_{l lam, l' lam'} the fill evaluates per node. */

@@ -437,12 +437,22 @@ static void po_eval_bipolar(const po_tables* T, real ax, real az, real bx, real 
  * Call with colidx = vals = NULL to count (rowptr and *nnz_out are still filled).
  * Returns 0, or <0 on bad arguments / capacity overflow.
  * ---------------------------------------------------------------------------------------- */
-int po_build(const double* pe, int Np, const double* qe, int Nq,
+/* Cell norm B_k of the radial basis (reading R2; eq. 21 is garbled in PAPER.md:L208):
+ *   norm = 0, reading A: delta(p-p')-normalised radial states, f = 1, B_k = e[k+1] - e[k] (the width);
+ *   norm = 1, reading B: states normalised in the p^2 dp measure,  B_k = (e[k+1]^3 - e[k]^3)/3.
+ * Node weight: A  w * pq/(p'q') ;  B  w * p^2 q^2.  Prefactor (B_i Bbar_j B_i' Bbar_j')^(-1/2) in both. */
+static real po_cell_norm(const double* e, int k, int norm)
+{
+    if (norm == 1) return ((real)e[k + 1] * (real)e[k + 1] * (real)e[k + 1] - (real)e[k] * (real)e[k] * (real)e[k]) / 3;
+    return (real)e[k + 1] - (real)e[k];
+}
+
+int po_build_norm(const double* pe, int Np, const double* qe, int Nq,
              const po_channel* ch, int n_ch, int J2, int T2, int stat,
              const double* tp, const double* wp, int n_p, const double* tq, const double* wq, int n_q,
              const double* tx, const double* wx, int n_x,
              int cell_begin, int cell_end,
-             int64_t* rowptr, int32_t* colidx, double* vals, int64_t cap, int64_t* nnz_out)
+             int64_t* rowptr, int32_t* colidx, double* vals, int64_t cap, int64_t* nnz_out, int norm)
 {
     const int n_cells = Np * Nq;
     if (cell_begin < 0 || cell_end > n_cells || cell_begin > cell_end) return -1;
@@ -512,7 +522,8 @@ int po_build(const double* pe, int Np, const double* qe, int Nq,
                 const po_node* nd = &nodes[n];
                 if (nd->ic < 0) continue;
                 real p = nd->p, q = nd->q, x = nd->x;
-                real omega = (real)(nd->w * ((nd->p * nd->q) / (nd->pp * nd->qq)));
+                real omega = norm == 1 ? (real)(nd->w * ((nd->p * nd->q) * (nd->p * nd->q)))
+                                       : (real)(nd->w * ((nd->p * nd->q) / (nd->pp * nd->qq)));
                 real sx = RSQRT((1 - x) * (1 + x));
                 real ppx, ppz, qpx, qpz;
                 po_rotated_dirs(p, q, x, 2, &ppx, &ppz, &qpx, &qpz);
@@ -534,12 +545,12 @@ int po_build(const double* pe, int Np, const double* qe, int Nq,
                 }
             }
             /* emit rows of this source cell */
-            real di = (real)pe[i + 1] - (real)pe[i], dj = (real)qe[j + 1] - (real)qe[j];
+            real di = po_cell_norm(pe, i, norm), dj = po_cell_norm(qe, j, norm);
             for (int a = 0; a < n_ch; ++a) {
                 int64_t pos = rowptr[(int64_t)cb * n_ch + a];
                 for (int h = 0; h < H; ++h) {
                     int ic = hitcell[h] / Nq, jc = hitcell[h] % Nq;
-                    real dic = (real)pe[ic + 1] - (real)pe[ic], djc = (real)qe[jc + 1] - (real)qe[jc];
+                    real dic = po_cell_norm(pe, ic, norm), djc = po_cell_norm(qe, jc, norm);
                     real norm = RSQRT(di * dj * dic * djc);
                     for (int b = 0; b < n_ch; ++b) {
                         if (!T.coupled[a * n_ch + b]) continue;
@@ -553,6 +564,151 @@ int po_build(const double* pe, int Np, const double* qe, int Nq,
         free(flag); free(local); free(hitcell); free(nodes); free(bra); free(ket); free(acc);
     }
     free(nhit); free(ncoup); po_tables_free(&T);
+    return 0;
+}
+
+int po_build(const double* pe, int Np, const double* qe, int Nq,
+             const po_channel* ch, int n_ch, int J2, int T2, int stat,
+             const double* tp, const double* wp, int n_p, const double* tq, const double* wq, int n_q,
+             const double* tx, const double* wx, int n_x,
+             int cell_begin, int cell_end,
+             int64_t* rowptr, int32_t* colidx, double* vals, int64_t cap, int64_t* nnz_out)
+{
+    return po_build_norm(pe, Np, qe, Nq, ch, n_ch, J2, T2, stat, tp, wp, n_p, tq, wq, n_q, tx, wx, n_x, cell_begin, cell_end,
+                         rowptr, colidx, vals, cap, nnz_out, 0);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Exact-overlap evaluation — the paper's own route: "a double integral with variable limits"
+ * (sec. 3.2).  For a fixed outer node (p, q) of the source cell the image moves along
+ *   p'^2 = A + B x ,  q'^2 = C - D x ,   A = p^2/4 + 9q^2/16, B = 3pq/4, C = p^2 + q^2/4, D = pq  (B, D > 0),
+ * both linear in x, so the x-values landing in target cell (i', j') form ONE interval
+ *   x_lo = max(-1, (pe[i']^2 - A)/B, (C - qe[j'+1]^2)/D) ,  x_hi = min(1, (pe[i'+1]^2 - A)/B, (C - qe[j']^2)/D),
+ * and the smooth integrand is integrated over it with the n_x-point rule mapped to [x_lo, x_hi].  The outer (p, q)
+ * rule is the tensor rule of the node-binning scheme.  Pattern: target cells with a non-empty interval (x_hi > x_lo)
+ * for at least one outer node, times the coupled-channel mask.  Plain loops over ALL target cells — slow, obvious.
+ * Same output conventions as po_build; norm as in po_build_norm.
+ * ---------------------------------------------------------------------------------------- */
+static int po_xo_interval(const double* pe, const double* qe, int ic, int jc, double A, double B, double C, double D,
+                          double* x_lo, double* x_hi)
+{
+    double lo = -1.0, hi = 1.0, v;
+    v = (pe[ic] * pe[ic] - A) / B;         if (v > lo) lo = v;
+    v = (C - qe[jc + 1] * qe[jc + 1]) / D; if (v > lo) lo = v;
+    v = (pe[ic + 1] * pe[ic + 1] - A) / B; if (v < hi) hi = v;
+    v = (C - qe[jc] * qe[jc]) / D;         if (v < hi) hi = v;
+    *x_lo = lo; *x_hi = hi;
+    return hi > lo;
+}
+
+int po_build_xo(const double* pe, int Np, const double* qe, int Nq,
+                const po_channel* ch, int n_ch, int J2, int T2, int stat,
+                const double* tp, const double* wp, int n_p, const double* tq, const double* wq, int n_q,
+                const double* tx, const double* wx, int n_x,
+                int cell_begin, int cell_end,
+                int64_t* rowptr, int32_t* colidx, double* vals, int64_t cap, int64_t* nnz_out, int norm)
+{
+    const int n_cells = Np * Nq;
+    if (cell_begin < 0 || cell_end > n_cells || cell_begin > cell_end) return -1;
+    po_tables T;
+    int rc = po_tables_init(&T, ch, n_ch, J2, T2, stat);
+    if (rc) { po_tables_free(&T); return rc; }
+    const int nblk = cell_end - cell_begin;
+    int* ncoup = (int*)calloc((size_t)n_ch, sizeof(int));
+    for (int a = 0; a < n_ch; ++a) for (int b = 0; b < n_ch; ++b) ncoup[a] += T.coupled[a * n_ch + b];
+    unsigned char* hit = (unsigned char*)calloc((size_t)nblk * n_cells + 1, 1);     /* [source][target] */
+    /* pass 1: which targets have a non-empty interval */
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int cb = 0; cb < nblk; ++cb) {
+        int cell = cell_begin + cb, i = cell / Nq, j = cell % Nq;
+        double cp = 0.5 * (pe[i] + pe[i + 1]), hp = 0.5 * (pe[i + 1] - pe[i]);
+        double cq = 0.5 * (qe[j] + qe[j + 1]), hq = 0.5 * (qe[j + 1] - qe[j]);
+        for (int a = 0; a < n_p; ++a) for (int b = 0; b < n_q; ++b) {
+            double p = cp + hp * tp[a], q = cq + hq * tq[b];
+            double A = 0.25 * (p * p) + 0.5625 * (q * q), B = 0.75 * (p * q), C = (p * p) + 0.25 * (q * q), D = p * q;
+            for (int t = 0; t < n_cells; ++t) {
+                double lo, hi;
+                if (po_xo_interval(pe, qe, t / Nq, t % Nq, A, B, C, D, &lo, &hi)) hit[(size_t)cb * n_cells + t] = 1;
+            }
+        }
+    }
+    rowptr[0] = 0;
+    for (int cb = 0; cb < nblk; ++cb) {
+        int64_t h = 0;
+        for (int t = 0; t < n_cells; ++t) h += hit[(size_t)cb * n_cells + t];
+        for (int a = 0; a < n_ch; ++a) rowptr[(int64_t)cb * n_ch + a + 1] = rowptr[(int64_t)cb * n_ch + a] + h * ncoup[a];
+    }
+    const int64_t nnz = rowptr[(int64_t)nblk * n_ch];
+    *nnz_out = nnz;
+    if ((!colidx && !vals) || nnz > cap) { int r = (!colidx && !vals) ? 0 : -3; free(hit); free(ncoup); po_tables_free(&T); return r; }
+    /* pass 2: values */
+#pragma omp parallel
+    {
+        real (*bra)[2 * PO_MAXL + 1] = malloc(sizeof(real[2 * PO_MAXL + 1]) * (size_t)(T.n_tri + 1));
+        real (*ket)[2 * PO_MAXL + 1] = malloc(sizeof(real[2 * PO_MAXL + 1]) * (size_t)(T.n_tri + 1));
+        real* acc = (real*)malloc(sizeof(real) * (size_t)n_ch * n_ch);
+#pragma omp for schedule(dynamic, 2)
+        for (int cb = 0; cb < nblk; ++cb) {
+            int cell = cell_begin + cb, i = cell / Nq, j = cell % Nq;
+            double cp = 0.5 * (pe[i] + pe[i + 1]), hp = 0.5 * (pe[i + 1] - pe[i]);
+            double cq = 0.5 * (qe[j] + qe[j + 1]), hq = 0.5 * (qe[j + 1] - qe[j]);
+            int h = 0;
+            for (int t = 0; t < n_cells; ++t) {
+                if (!hit[(size_t)cb * n_cells + t]) continue;
+                int ic = t / Nq, jc = t % Nq;
+                for (int k = 0; k < n_ch * n_ch; ++k) acc[k] = 0;
+                for (int a = 0; a < n_p; ++a) for (int b = 0; b < n_q; ++b) {
+                    double p = cp + hp * tp[a], q = cq + hq * tq[b];
+                    double A = 0.25 * (p * p) + 0.5625 * (q * q), B = 0.75 * (p * q), C = (p * p) + 0.25 * (q * q), D = p * q;
+                    double lo, hi;
+                    if (!po_xo_interval(pe, qe, ic, jc, A, B, C, D, &lo, &hi)) continue;
+                    double xm = 0.5 * (lo + hi), xh = 0.5 * (hi - lo);
+                    for (int c = 0; c < n_x; ++c) {
+                        double x = xm + xh * tx[c];
+                        double w = ((hp * wp[a]) * (hq * wq[b])) * (xh * wx[c]);
+                        double P2 = A + B * x, Q2 = C - D * x;
+                        real omega;
+                        if (norm == 1) omega = (real)(w * ((p * q) * (p * q)));
+                        else {
+                            if (P2 <= 0.0 || Q2 <= 0.0) continue;       /* only at an interval end that touches p' = 0 or q' = 0 */
+                            omega = (real)(w * ((p * q) / (sqrt(P2) * sqrt(Q2))));
+                        }
+                        real sx = RSQRT((1 - (real)x) * (1 + (real)x));
+                        real ppx, ppz, qpx, qpz;
+                        po_rotated_dirs((real)p, (real)q, (real)x, 2, &ppx, &ppz, &qpx, &qpz);
+                        po_eval_bipolar(&T, sx, (real)x, 0, 1, bra);
+                        po_eval_bipolar(&T, ppx, ppz, qpx, qpz, ket);
+                        for (int al = 0; al < n_ch; ++al) for (int be = 0; be < n_ch; ++be) {
+                            if (!T.coupled[al * n_ch + be]) continue;
+                            real G = 0;
+                            for (int L = 0; L <= PO_MAXL; ++L) {
+                                double cL = T.coef[((size_t)al * n_ch + be) * (PO_MAXL + 1) + L];
+                                if (cL == 0.0) continue;
+                                int ta = T.tri_of[al * (PO_MAXL + 1) + L], tb = T.tri_of[be * (PO_MAXL + 1) + L];
+                                real AL = 0;
+                                for (int M = -L; M <= L; ++M) AL += bra[ta][M + L] * ket[tb][M + L];
+                                G += (real)cL * (AL / (real)(2 * L + 1));
+                            }
+                            acc[al * n_ch + be] += omega * G;
+                        }
+                    }
+                }
+                real nrm = RSQRT(po_cell_norm(pe, i, norm) * po_cell_norm(qe, j, norm) * po_cell_norm(pe, ic, norm) * po_cell_norm(qe, jc, norm));
+                for (int al = 0; al < n_ch; ++al) {
+                    int64_t pos = rowptr[(int64_t)cb * n_ch + al] + (int64_t)h * ncoup[al];
+                    for (int be = 0; be < n_ch; ++be) {
+                        if (!T.coupled[al * n_ch + be]) continue;
+                        if (colidx) colidx[pos] = t * n_ch + be;
+                        if (vals) vals[pos] = (double)(acc[al * n_ch + be] / nrm);
+                        ++pos;
+                    }
+                }
+                ++h;
+            }
+        }
+        free(bra); free(ket); free(acc);
+    }
+    free(hit); free(ncoup); po_tables_free(&T);
     return 0;
 }
 

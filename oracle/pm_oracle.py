@@ -81,6 +81,10 @@ class Oracle:
         lib.po_build.argtypes = [_dp, C.c_int, _dp, C.c_int, _chp, C.c_int, C.c_int, C.c_int, C.c_int,
                                  _dp, _dp, C.c_int, _dp, _dp, C.c_int, _dp, _dp, C.c_int,
                                  C.c_int, C.c_int, _i64p, _i32p, _dp, C.c_int64, _i64p]
+        for name in ("po_build_norm", "po_build_xo"):
+            f = getattr(lib, name)
+            f.restype = C.c_int
+            f.argtypes = lib.po_build.argtypes + [C.c_int]
         lib.po_hit_cells.restype = C.c_int
         lib.po_hit_cells.argtypes = [_dp, C.c_int, _dp, C.c_int, _dp, _dp, C.c_int, _dp, _dp, C.c_int, _dp, _dp, C.c_int,
                                      C.c_int, C.c_int, _i64p, _i32p, C.c_int64]
@@ -145,8 +149,10 @@ class Oracle:
         return out
 
     # ---- the build ----
-    def build_csr(self, wl, cell_begin=0, cell_end=None, values=True):
-        """CSR block of rows of source cells [cell_begin, cell_end): (rowptr int64, colidx int32, vals f64)."""
+    def build_csr(self, wl, cell_begin=0, cell_end=None, values=True, norm=0, exact_overlap=False):
+        """CSR block of rows of source cells [cell_begin, cell_end): (rowptr int64, colidx int32, vals f64).
+        norm: 0 = reading A (cell widths), 1 = reading B (p^2 dp measure); exact_overlap: the paper's 'double integral
+        with variable limits' (po_build_xo) instead of node binning."""
         if cell_end is None:
             cell_end = wl.n_cells
         chs = np.ascontiguousarray(wl.channels)
@@ -157,10 +163,11 @@ class Oracle:
         nnz = C.c_int64(0)
 
         def call(col, val, cap):
-            rc = self.lib.po_build(_d(wl.p_edges), wl.Np, _d(wl.q_edges), wl.Nq, chp, wl.n_ch,
-                                   wl.J2, wl.T2, wl.statistics,
-                                   _d(tp), _d(wp), wl.n_p, _d(tq), _d(wq), wl.n_q, _d(tx), _d(wx), wl.n_x,
-                                   cell_begin, cell_end, rowptr.ctypes.data_as(_i64p), col, val, cap, C.byref(nnz))
+            fn = self.lib.po_build_xo if exact_overlap else self.lib.po_build_norm
+            rc = fn(_d(wl.p_edges), wl.Np, _d(wl.q_edges), wl.Nq, chp, wl.n_ch,
+                    wl.J2, wl.T2, wl.statistics,
+                    _d(tp), _d(wp), wl.n_p, _d(tq), _d(wq), wl.n_q, _d(tx), _d(wx), wl.n_x,
+                    cell_begin, cell_end, rowptr.ctypes.data_as(_i64p), col, val, cap, C.byref(nnz), int(norm))
             if rc != 0:
                 raise RuntimeError(f"po_build failed: {rc}")
 

@@ -25,7 +25,8 @@ EXPORTS = ["pm_lattice_create", "pm_lattice_destroy", "pm_lattice_dims", "pm_lat
            "pm_lattice_coupling", "pm_lattice_work", "pm_pattern_counts", "pm_lattice_fill_kernel", "pm_set_jit", "pm_diag_jit_compile", "pm_diag_sqrt_threshold",
            "pm_diag_dfma_tflops", "pm_pattern", "pm_fill", "pm_build", "pm_last_fill_ms", "pm_block_apply", "pm_kernel_apply", "pm_spmv_implicit", "pm_spmv", "pm_build_host_count", "pm_build_host",
            "pm_launch_count", "pm_last_error", "pm_lattice_attach", "pm_build_async", "pm_build_wait", "pm_build_reuse",
-           "pm_pattern_cell_hits", "pm_partition_cells", "pm_rowptr_offset", "pm_block_apply_t", "pm_rotate_apply"]
+           "pm_pattern_cell_hits", "pm_partition_cells", "pm_rowptr_offset", "pm_block_apply_t", "pm_rotate_apply",
+           "pm_lattice_set_normalisation"]
 
 
 class PmError(RuntimeError):
@@ -56,6 +57,7 @@ def lib():
                                     C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
                                     C.POINTER(_vp)]
     L.pm_lattice_destroy.argtypes = [_vp]
+    L.pm_lattice_set_normalisation.argtypes = [_vp, C.c_int32]
     L.pm_lattice_attach.argtypes = [_vp, C.POINTER(_Channel), C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.POINTER(_vp)]
     L.pm_build_async.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, _vp, C.c_int64, C.c_int32, _vp]
     L.pm_build_wait.argtypes = [_vp, _i64p]
@@ -133,6 +135,11 @@ def pm_lattice_attach(base, channels, J2, parity, T2, statistics):
 
 def pm_lattice_destroy(h):
     _check(lib().pm_lattice_destroy(h))
+
+
+def pm_lattice_set_normalisation(h, normalisation):
+    """0 = PM_NORM_WIDTH (reading A, default), 1 = PM_NORM_P2 (reading B: p^2 dp measure)."""
+    _check(lib().pm_lattice_set_normalisation(h, int(normalisation)))
 
 
 def pm_lattice_dims(h):
@@ -323,10 +330,12 @@ def pm_launch_count():
 class Lattice:
     """Owns a pm_lattice handle created from a `inputs.Workload`; allocates outputs with torch."""
 
-    def __init__(self, wl, use_workload_rules: bool = True):
+    def __init__(self, wl, use_workload_rules: bool = True, normalisation: int = 0):
         self.wl = wl
         self.h = pm_lattice_create(wl.p_edges, wl.q_edges, wl.channels, wl.J2, wl.parity, wl.T2, wl.statistics,
                                    wl.n_p, wl.n_q, wl.n_x)
+        if normalisation:
+            pm_lattice_set_normalisation(self.h, normalisation)
         if use_workload_rules:                      # feed the very arrays the oracle gets (reading R12)
             for axis, key in enumerate(("p", "q", "x")):
                 pm_lattice_set_rule(self.h, axis, *wl.rules[key])

@@ -84,6 +84,7 @@ struct pm_lattice {
     uint64_t id = 0;                   // unique per created lattice (pm_stream.cu keys its cached block plan with it)
     pm_geometry* G = nullptr;
     int n_ch = 0, J2 = 0, parity = 1, T2 = 0, stat = 0;
+    int norm = 0;                      // cell normalisation (pm_lattice_set_normalisation)
     std::vector<pm_channel> ch;
     pm::Tables T;
     // device side
@@ -226,7 +227,7 @@ int32_t ensure_device(pm_lattice* L)
     L->device = G->device;
     const pm::Tables& T = L->T;
     pm::DevLattice D = G->geo;
-    D.n_ch = L->n_ch;
+    D.n_ch = L->n_ch; D.norm = L->norm;
     D.totcoup = T.totcoup; D.n_bra = T.n_slot; D.lmax = T.lmax;
     D.ny = pm::ylm_index(T.lmax, T.lmax) + 1;
     std::vector<double> bra;
@@ -435,6 +436,14 @@ int32_t pm_lattice_set_rule(pm_lattice* lat, int32_t axis, const double* nodes, 
     G->rule_t[axis].assign(nodes, nodes + n);
     G->rule_w[axis].assign(weights, weights + n);
     ++G->version;                      // every lattice of the group re-uploads its tables; the node lists are stale
+    return PM_OK;
+}
+
+int32_t pm_lattice_set_normalisation(pm_lattice* lat, int32_t normalisation)
+{
+    if (!lat) return fail(PM_ERR_ARG, "lat is NULL");
+    if (normalisation != PM_NORM_WIDTH && normalisation != PM_NORM_P2) return fail(PM_ERR_ARG, "unknown normalisation");
+    if (lat->norm != normalisation) { lat->norm = normalisation; lat->geo_version = 0; }      // the device tables are rebuilt at the next call
     return PM_OK;
 }
 

@@ -29,6 +29,7 @@ namespace pm {
 struct DevLattice {
     int Np, Nq, n_ch, n_p, n_q, n_x, nnode, n_cells, n_words, pe_pad, qe_pad;
     int totcoup, n_slot, n_fun, lmax, ny;       // n_slot / n_fun: ket slots and orbital functions of THIS column-channel group
+    int norm;                                   // cell normalisation: 0 reading A (widths), 1 reading B (p^2 dp measure) — DESIGN.md R2
     int n_out, n_bra;                           // outputs (alpha, alpha') of this group; bra slots of the whole channel set
     unsigned mg_npq, mg_nq, mg_Nq;              // ceil(2^32 / d) for d = n_p*n_q, n_q, Nq: exact division of node and cell ids (x*d < 2^32)
     const double *pe, *qe;                      // edges, Np+1 / Nq+1 entries (padded with +inf to pe_pad / qe_pad)

@@ -119,8 +119,9 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
     double* s_wqb = (double*)(wsm + S.w_wqb);
 
     // ---- once per CTA: widths, rules, bra harmonics, output descriptors
-    for (int k = tid; k < L.Np; k += T) s_dp[k] = L.pe[k + 1] - L.pe[k];
-    for (int k = tid; k < L.Nq; k += T) s_dq[k] = L.qe[k + 1] - L.qe[k];
+    // cell norms B_k: widths (reading A) or (e_{k+1}^3 - e_k^3)/3 (reading B, states normalised in the p^2 dp measure)
+    for (int k = tid; k < L.Np; k += T) { const double e0 = L.pe[k], e1 = L.pe[k + 1]; s_dp[k] = L.norm ? (e1 * e1 * e1 - e0 * e0 * e0) / 3.0 : e1 - e0; }
+    for (int k = tid; k < L.Nq; k += T) { const double e0 = L.qe[k], e1 = L.qe[k + 1]; s_dq[k] = L.norm ? (e1 * e1 * e1 - e0 * e0 * e0) / 3.0 : e1 - e0; }
     for (int k = tid; k < L.n_p; k += T) s_tp[k] = L.tp[k];
     for (int k = tid; k < L.n_q; k += T) s_tq[k] = L.tq[k];
     for (int k = tid; k < L.n_x; k += T) { s_tx[k] = L.tx[k]; s_sx[k] = L.sx[k]; s_wx[k] = L.wx[k]; }
@@ -253,7 +254,8 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 map_node_sq(g, s_tp[a], s_tq[b], x, p, q, P2, Q2);
                 // omega = w * p q / (p' q'),  w = ((hp wp_a)(hq wq_b)) wx_c
                 const double w = __dmul_rn(__dmul_rn(s_wpa[a], s_wqb[b]), s_wx[c]);
-                const double om = w * (p * q) * rsqrt(P2 * Q2);
+                // (reading B: omega = w * p^2 q^2, no Jacobian of the delta functions)
+                const double om = L.norm ? w * ((p * q) * (p * q)) : w * (p * q) * rsqrt(P2 * Q2);
                 // rotated directions from vector components (frame: q^ = z, p^ = (sx, 0, x)):
                 //   p' = -p/2 - 3q/4 ,  q' = p - q/2
                 const double sx = s_sx[c], psx = p * sx, px = p * x;
@@ -325,7 +327,8 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 }
                 __syncwarp();
                 const int cseg = __shfl_sync(0xffffffffu, c, jb);
-                const double* bra = bra_tab + cseg * bra_stride;
+                const double* bra;                                     // (shared-memory loads for the specialised kernels)
+                if constexpr (Spec::kStatic) bra = s_bra + cseg * nsb; else bra = bra_tab + cseg * bra_stride;
 #pragma unroll
                 for (int ch = 0; ch < NCH; ++ch) {
                     if (kPacked) {

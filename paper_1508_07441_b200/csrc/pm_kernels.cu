@@ -43,6 +43,19 @@ MapSortSmem map_sort_plan(const DevLattice& L, int max_warps)
     S.bk_p = take(2 * (size_t)kBuckets); S.bk_q = take(2 * (size_t)kBuckets);
     S.tp = take(8 * (size_t)L.n_p); S.tq = take(8 * (size_t)L.n_q); S.tx = take(8 * (size_t)L.n_x);
     S.wide = L.n_cells > 65535 ? 1 : 0;                 // targets kept as 16-bit ids when they fit
+    // pass 1 items = (a, b) pairs x runs of n_x / nchunk consecutive x-nodes: the fewest runs that keep >= 90 % of the lanes busy
+    S.nchunk = 1;
+    {
+        const int npq = L.n_p * L.n_q;
+        double best = 0.0;
+        for (int nc = 1; nc <= L.n_x; ++nc) {
+            if (L.n_x % nc) continue;
+            const int items = npq * nc;
+            const double util = (double)items / (32.0 * ((items + 31) / 32));
+            if (util > best + 1e-9) { best = util; S.nchunk = nc; }
+            if (util >= 0.9) break;
+        }
+    }
     int w = 0;
     auto wtake = [&](size_t bytes) { int r = w; w += (int)al16(bytes); return r; };
     S.w_bits = wtake(4 * (size_t)L.n_words);
@@ -71,7 +84,7 @@ k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl,
     char* wsm = smem + S.warp0 + warp * S.warp_bytes;
     unsigned* bits = (unsigned*)(wsm + S.w_bits);
     unsigned short* wpre = (unsigned short*)(wsm + S.w_wpre);
-    TT* __restrict__ s_t = (TT*)scratch + (size_t)(blockIdx.x * (T >> 5) + warp) * (size_t)((L.nnode + 31) & ~31);   // this warp's targets
+    TT* s_t = (TT*)scratch + (size_t)(blockIdx.x * (T >> 5) + warp) * (size_t)((L.nnode + 31) & ~31);   // this warp's targets
     int* hist = (int*)(wsm + S.w_hist);
 
     for (int k = tid; k < L.pe_pad + kLocK; k += T) s_thr_p[k] = k < L.pe_pad ? L.thr_p[k] : __longlong_as_double(0x7ff0000000000000ll);
@@ -96,24 +109,35 @@ k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl,
         const CellGeom g = cell_geom(L.pe, L.qe, ci, cj);
         for (int k = lane; k < L.n_words; k += 32) bits[k] = 0u;
         __syncwarp();
-        // ---- pass 1: map, locate, mark (two independent nodes per lane and iteration)
-        for (int m0 = lane; m0 < L.nnode; m0 += 64) {
-            int t[2];
-#pragma unroll
-            for (int u = 0; u < 2; ++u) {
-                const int m = min(m0 + 32 * u, L.nnode - 1);
-                int c, a, b;
-                split_node(L, m, c, a, b);
-                double p, q, P2, Q2;
-                map_node_sq(g, s_tp[a], s_tq[b], s_tx[c], p, q, P2, Q2);
-                t[u] = target_cell_sq<kFast>(lc, P2, Q2);
-            }
-#pragma unroll
-            for (int u = 0; u < 2; ++u) {
-                const int m = m0 + 32 * u;
-                if (m < L.nnode) {
-                    if (t[u] >= 0) atomicOr(&bits[t[u] >> 5], 1u << (t[u] & 31));
-                    s_t[m] = t[u] >= 0 ? (TT)t[u] : (TT)~(TT)0;
+        // ---- pass 1: map, locate, mark.  Lane = one (a, b) pair and one run of consecutive x-nodes: p, q and the
+        // x-independent sums of the map are formed once per run (the very operations of map_node_sq, in its order), and
+        // since p'^2 grows and q'^2 falls with x, the cell indices of a node follow from the previous node's by a few
+        // comparisons (the first node of a run is located through the bucket tables).
+        {
+            const int npq = L.n_p * L.n_q, cpc = L.n_x / S.nchunk, items = npq * S.nchunk;
+            for (int item = lane; item < items; item += 32) {
+                const int ck = item / npq, ab = item - ck * npq;
+                const int a = L.mg_nq ? (int)__umulhi((unsigned)ab, L.mg_nq) : ab, b = ab - a * L.n_q;
+                const double p = __dadd_rn(g.cp, __dmul_rn(g.hp, s_tp[a])), q = __dadd_rn(g.cq, __dmul_rn(g.hq, s_tq[b]));
+                const double pq = __dmul_rn(p, q), p2 = __dmul_rn(p, p), q2 = __dmul_rn(q, q);
+                const double PA = __dadd_rn(__dmul_rn(0.25, p2), __dmul_rn(0.5625, q2)), QA = __dadd_rn(p2, __dmul_rn(0.25, q2));
+                int ip = 0, iq = 0;
+                for (int c = ck * cpc; c < (ck + 1) * cpc; ++c) {
+                    const double pqx = __dmul_rn(pq, s_tx[c]);
+                    double P2 = __dadd_rn(PA, __dmul_rn(0.75, pqx)), Q2 = __dsub_rn(QA, pqx);
+                    P2 = P2 < 0.0 ? 0.0 : P2;
+                    Q2 = Q2 < 0.0 ? 0.0 : Q2;
+                    if (c == ck * cpc) {
+                        ip = kFast ? locate_k<kLocK>(s_thr_p, s_bk_p, L.bk_hmin_p, L.bk_sh_p, P2) : locate(s_thr_p, s_bk_p, L.bk_hmin_p, L.bk_sh_p, P2);
+                        iq = kFast ? locate_k<kLocK>(s_thr_q, s_bk_q, L.bk_hmin_q, L.bk_sh_q, Q2) : locate(s_thr_q, s_bk_q, L.bk_hmin_q, L.bk_sh_q, Q2);
+                    } else {
+                        while (s_thr_p[ip + 1] <= P2) ++ip;              // (+inf sentinel behind the last threshold)
+                        while (iq >= 0 && s_thr_q[iq] > Q2) --iq;
+                    }
+                    const bool ok = (ip >= 0) & (ip < L.Np) & (iq >= 0) & (iq < L.Nq) & (P2 != 0.0) & (Q2 != 0.0);
+                    const int t = ok ? ip * L.Nq + iq : -1;
+                    if (t >= 0) atomicOr(&bits[t >> 5], 1u << (t & 31));
+                    s_t[c * npq + ab] = t >= 0 ? (TT)t : (TT)~(TT)0;
                 }
             }
         }

@@ -17,7 +17,7 @@ constexpr int kMapSortMaxWarps = 16;  // k_map_sort: warps (= source cells in fl
 constexpr int kHistCap = 512;         // k_map_sort: rank counters per window (one window unless a source cell hits more cells)
 
 // shared-memory plan of k_map_sort: tables shared by the CTA, then one private area per warp (byte offsets)
-struct MapSortSmem { int thr_p, thr_q, bk_p, bk_q, tp, tq, tx, warp0, warp_bytes, w_bits, w_wpre, w_hist, nw, ctas, wide, hist_cap, total; };
+struct MapSortSmem { int thr_p, thr_q, bk_p, bk_q, tp, tq, tx, warp0, warp_bytes, w_bits, w_wpre, w_hist, nw, ctas, wide, hist_cap, nchunk, total; };
 MapSortSmem map_sort_plan(const DevLattice& L, int max_warps);
 int64_t launch_count();
 void count_launch();

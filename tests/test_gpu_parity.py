@@ -500,3 +500,24 @@ def test_every_Jpi_up_to_17_halves_on_one_grid(api, oracle):
     assert kinds[(17, +1)] == (62, "generic-grouped") and kinds[(5, +1)][1] == "generic-grouped", kinds
     assert max(k[0] for k in kinds.values()) == 62
     lat.close()
+
+
+@pytest.mark.parametrize("wl", [I.config(1), I.small_coupled(N=7, jmax=3, orders=(4, 5, 7), Nq=5),
+                                I.boson_lattice(9, 5, waves=((0, 0), (2, 2)), orders=(4, 3, 6), cp=0.7, cq=1.3)], ids=lambda w: w.name)
+def test_reading_B_normalisation(api, oracle, wl):
+    """pm_lattice_set_normalisation(PM_NORM_P2): states normalised in the p^2 dp measure (reading R2-B): the same
+    pattern, values against po_build_norm(norm = 1); switching back restores reading A bit for bit."""
+    lat = api.Lattice(wl)
+    a0 = [t.cpu().numpy() for t in lat.build_fused()]
+    api.pm_lattice_set_normalisation(lat.h, 1)
+    rp, ci, v = (t.cpu().numpy() for t in lat.build_fused())
+    rpo, cio, vo = oracle.build_csr(wl, norm=1)
+    assert np.array_equal(rp, rpo) and np.array_equal(ci, cio) and np.array_equal(rp, a0[0]) and np.array_equal(ci, a0[1])
+    _assert_values(v, vo)
+    assert np.max(np.abs(v - a0[2])) > 1e-3 * np.max(np.abs(vo))            # it is a different matrix
+    api.pm_lattice_set_normalisation(lat.h, 0)
+    a1 = [t.cpu().numpy() for t in lat.build_fused()]
+    assert all(np.array_equal(x, y) for x, y in zip(a0, a1))
+    with pytest.raises(api.PmError):
+        api.pm_lattice_set_normalisation(lat.h, 7)
+    lat.close()

@@ -382,3 +382,135 @@ def test_build_cells_is_build_csr_per_cell(oracle):
     for (rp, ci, v), c in zip(oracle.build_cells(wl, cells, workers=3), cells):
         rp2, ci2, v2 = oracle.build_csr(wl, c, c + 1)
         assert np.array_equal(rp, rp2) and np.array_equal(ci, ci2) and np.array_equal(v, v2)
+
+
+# ---- reading-B normalisation and the exact-overlap ("variable limits") evaluation ------
+def _variable_limits_matrix_B(g, sub=16, order=6):
+    """Reading B for s-wave bosons (G = 1): P = int p^2 dp q^2 dq (length of the x-interval landing in the target cell)
+    / sqrt(B_i B_j B_i' B_j'), B_k = (g[k+1]^3 - g[k]^3)/3.  Outer composite Gauss-Legendre, inner x exact."""
+    N = len(g) - 1
+    t, w = np.polynomial.legendre.leggauss(order)
+    Bk = (g[1:] ** 3 - g[:-1] ** 3) / 3.0
+    P = np.zeros((N * N, N * N))
+    for i in range(N):
+        for j in range(N):
+            ep = np.linspace(g[i], g[i + 1], sub + 1); eq = np.linspace(g[j], g[j + 1], sub + 1)
+            pn = (0.5 * (ep[:-1] + ep[1:])[:, None] + 0.5 * np.diff(ep)[:, None] * t[None, :]).ravel()
+            pw = (0.5 * np.diff(ep)[:, None] * w[None, :]).ravel()
+            qn = (0.5 * (eq[:-1] + eq[1:])[:, None] + 0.5 * np.diff(eq)[:, None] * t[None, :]).ravel()
+            qw = (0.5 * np.diff(eq)[:, None] * w[None, :]).ravel()
+            pg, qg = np.meshgrid(pn, qn, indexing="ij"); wg = pw[:, None] * qw[None, :]
+            a, b = 0.25 * pg * pg + 0.5625 * qg * qg, 0.75 * pg * qg
+            c, d = pg * pg + 0.25 * qg * qg, pg * qg
+            for ic in range(N):
+                for jc in range(N):
+                    lo = np.maximum.reduce([np.full_like(pg, -1.0), (g[ic] ** 2 - a) / b, (c - g[jc + 1] ** 2) / d])
+                    hi = np.minimum.reduce([np.full_like(pg, 1.0), (g[ic + 1] ** 2 - a) / b, (c - g[jc] ** 2) / d])
+                    val = np.sum(wg * pg ** 2 * qg ** 2 * np.maximum(hi - lo, 0.0))
+                    P[i * N + j, ic * N + jc] = val / math.sqrt(Bk[i] * Bk[j] * Bk[ic] * Bk[jc])
+    return P
+
+
+def test_reading_B_and_exact_overlap_on_4x4(oracle):
+    """Pins of po_build_norm(norm = 1) and po_build_xo (PAPER.md:L215 'double integral with variable limits') on the 4x4
+    s-wave lattice, against numpy routes that share nothing with the oracle:
+    * reading A, exact overlap  vs  the variable-limits matrix (inner x analytic) of test_integral_three_ways_on_4x4;
+    * reading B, exact overlap  vs  the same route with weight p^2 q^2 (inner x exact: the interval length);
+    * node binning in reading B converges to it; both readings give spectra inside [-1, 2];
+    * at equal orders the exact-overlap matrix is far more symmetric than the node-binned one."""
+    g = I.tan_grid(4, 1.0)
+    VA, VB = _variable_limits_matrix(g), _variable_limits_matrix_B(g)
+    xo = I.boson_lattice(4, 4, orders=(48, 48, 32))
+    XA = _csr(xo, oracle, exact_overlap=True).toarray()
+    XB = _csr(xo, oracle, exact_overlap=True, norm=1).toarray()
+    # (the interval length is only piecewise smooth in (p, q): the outer rule converges algebraically; 3.5e-4 / 8e-5 observed)
+    assert np.abs(XA - VA).max() < 1e-3 * np.abs(VA).max()
+    assert np.abs(XB - VB).max() < 2.5e-4 * np.abs(VB).max()
+    coarse = I.boson_lattice(4, 4, orders=(24, 24, 16))
+    assert np.abs(XB - VB).max() < np.abs(_csr(coarse, oracle, exact_overlap=True, norm=1).toarray() - VB).max()
+    assert np.abs(VB - VB.T).max() < 1e-4 * np.abs(VB).max()                 # the exact reading-B matrix is symmetric too
+    hi = I.boson_lattice(4, 4, orders=(48, 48, 96))
+    BB = _csr(hi, oracle, norm=1).toarray()
+    assert np.abs(BB - VB).max() < 3e-3 * np.abs(VB).max()
+    for M in (XA, XB, BB):
+        ev = np.linalg.eigvalsh(0.5 * (M + M.T))
+        assert ev.min() > -1.05 and 1.2 < ev.max() < 2.05
+    lo_orders = I.boson_lattice(4, 4, orders=(8, 8, 8))
+    assert _asym(_csr(lo_orders, oracle, exact_overlap=True)) < 0.2 * _asym(_csr(lo_orders, oracle))
+    # patterns: every node-binned entry lies inside the exact-overlap pattern (a node that lands in a cell proves the overlap)
+    pa = _csr(I.boson_lattice(4, 4, orders=(8, 8, 8)), oracle).toarray() != 0
+    px = _csr(I.boson_lattice(4, 4, orders=(8, 8, 8)), oracle, exact_overlap=True).toarray() != 0
+    assert np.all(px[pa])
+
+
+def _rebuild_xo_from_G(wl, oracle, norm):
+    """Every entry of the exact-overlap matrix from its definition: outer nodes (p, q) of the source cell, the x-interval
+    landing in the target cell from the two linear maps p'^2 = A + Bx, q'^2 = C - Dx, the n_x-point rule mapped to it,
+    the coefficient from po_G.  numpy + po_G only."""
+    pe, qe, nc = wl.p_edges, wl.q_edges, wl.n_ch
+    (tp, wp), (tq, wq), (tx, wx) = wl.rules["p"], wl.rules["q"], wl.rules["x"]
+    ch = wl.channels
+    coupled = [[oracle.coupled(a, b, wl.J2, wl.statistics) for b in ch] for a in ch]
+    nk = (lambda e, k: (e[k + 1] ** 3 - e[k] ** 3) / 3.0) if norm else (lambda e, k: e[k + 1] - e[k])
+    out = {}
+    for cell in range(wl.n_cells):
+        i, j = divmod(cell, wl.Nq)
+        for a in range(wl.n_p):
+            for b in range(wl.n_q):
+                p = 0.5 * (pe[i] + pe[i + 1]) + 0.5 * (pe[i + 1] - pe[i]) * tp[a]
+                q = 0.5 * (qe[j] + qe[j + 1]) + 0.5 * (qe[j + 1] - qe[j]) * tq[b]
+                wab = (0.5 * (pe[i + 1] - pe[i]) * wp[a]) * (0.5 * (qe[j + 1] - qe[j]) * wq[b])
+                A, B, Cc, D = 0.25 * p * p + 0.5625 * q * q, 0.75 * p * q, p * p + 0.25 * q * q, p * q
+                for t in range(wl.n_cells):
+                    ic, jc = divmod(t, wl.Nq)
+                    lo = max(-1.0, (pe[ic] ** 2 - A) / B, (Cc - qe[jc + 1] ** 2) / D)
+                    hi = min(1.0, (pe[ic + 1] ** 2 - A) / B, (Cc - qe[jc] ** 2) / D)
+                    if not hi > lo:
+                        continue
+                    nrm = math.sqrt(nk(pe, i) * nk(qe, j) * nk(pe, ic) * nk(qe, jc))
+                    for c in range(wl.n_x):
+                        x = 0.5 * (lo + hi) + 0.5 * (hi - lo) * tx[c]
+                        w = wab * 0.5 * (hi - lo) * wx[c]
+                        om = w * (p * q) ** 2 if norm else w * p * q / math.sqrt((A + B * x) * (Cc - D * x))
+                        for al in range(nc):
+                            for be in range(nc):
+                                if coupled[al][be]:
+                                    key = (cell * nc + al, t * nc + be)
+                                    out[key] = out.get(key, 0.0) + om * 2.0 * oracle.G(ch[al], ch[be], wl.J2, wl.T2, wl.statistics, p, q, float(x), 2) / nrm
+    return out
+
+
+@pytest.mark.parametrize("norm", [0, 1])
+@pytest.mark.parametrize("wl", [I.small_coupled(N=3, jmax=1, orders=(2, 2, 3), Nq=4),
+                                I.boson_lattice(4, 3, waves=((0, 0), (2, 2)), J=0, orders=(2, 3, 3), cq=0.7)], ids=lambda w: w.name)
+def test_exact_overlap_build_equals_its_definition(oracle, wl, norm):
+    """po_build_xo and po_build_norm entry by entry from numpy + the pinned po_G: intervals, mapped rule, weights, the two
+    normalisations, the coupled-channel assembly, the pattern (readings R2, R17)."""
+    rp, ci, v = oracle.build_csr(wl, norm=norm, exact_overlap=True)
+    ref = _rebuild_xo_from_G(wl, oracle, norm)
+    assert len(ref) == len(v)
+    rows = np.repeat(np.arange(len(rp) - 1), np.diff(rp))
+    want = np.array([ref[(int(r), int(c))] for r, c in zip(rows, ci)])
+    assert np.max(np.abs(v - want)) <= 1e-13 * np.max(np.abs(want))
+    if norm:                                               # node binning in reading B: the same check through po_build's node table
+        rp, ci, v = oracle.build_csr(wl, norm=1)
+        rpA, ciA, vA = oracle.build_csr(wl, norm=0)
+        assert np.array_equal(rp, rpA) and np.array_equal(ci, ciA)       # the normalisation does not touch the pattern
+        pe, qe = wl.p_edges, wl.q_edges
+        Bn = lambda e, k: (e[k + 1] ** 3 - e[k] ** 3) / 3.0
+        rows = np.repeat(np.arange(len(rp) - 1), np.diff(rp))
+        got = {}
+        for cell in range(wl.n_cells):
+            i, j = divmod(cell, wl.Nq)
+            nd = oracle.cell_nodes(wl, cell)
+            for n in np.nonzero(nd["target"] >= 0)[0]:
+                t = int(nd["target"][n]); ic, jc = divmod(t, wl.Nq)
+                om = nd["w"][n] * (nd["p"][n] * nd["q"][n]) ** 2 / math.sqrt(Bn(pe, i) * Bn(qe, j) * Bn(pe, ic) * Bn(qe, jc))
+                for al in range(wl.n_ch):
+                    for be in range(wl.n_ch):
+                        if oracle.coupled(wl.channels[al], wl.channels[be], wl.J2, wl.statistics):
+                            key = (cell * wl.n_ch + al, t * wl.n_ch + be)
+                            got[key] = got.get(key, 0.0) + om * 2.0 * oracle.G(wl.channels[al], wl.channels[be], wl.J2, wl.T2, wl.statistics,
+                                                                                float(nd["p"][n]), float(nd["q"][n]), float(nd["x"][n]), 2)
+        want = np.array([got[(int(r), int(c))] for r, c in zip(rows, ci)])
+        assert np.max(np.abs(v - want)) <= 1e-13 * np.max(np.abs(want))
