@@ -262,6 +262,42 @@ def fill_roofline(api, lat, wl, nnz, fill_ms, pk, n_sm, dfma):
             "min_ms": {"alu": t_alu * 1e3, "hbm": t_hbm * 1e3}, "alu": alu, "hbm": hbm, "work": work, "fill_ms": fill_avg * 1e3}
 
 
+def jpi_sweep(api, torch, lat, wl, flush, st):
+    """SURVEY sec. 8(f) rank 3 / PAPER.md Table 1 (L396-404: '62 spin-orbital channels and all states ... up to J_max = 17/2'):
+    every J^pi <= 17/2 (pair j <= 3) on the grid of `wl`, each attached to the base lattice and built with pm_build_reuse into
+    one pair of buffers sized for the largest set; the geometric pattern (map + sort) is computed once, before the sweep."""
+    rp = torch.empty(wl.n_cells * 64 + 1, dtype=torch.int64, device="cuda")
+    e0, e1 = (torch.cuda.Event(enable_timing=True) for _ in range(2))
+    e0.record(st)
+    nnz0 = api.pm_pattern(lat.h, 0, wl.n_cells, rp, None)                # the one node map + sort of the sweep
+    e1.record(st); torch.cuda.synchronize()
+    pattern_ms = e0.elapsed_time(e1)
+    hits = nnz0 // int(api.pm_lattice_coupling(lat.h, wl.n_ch)[0].sum())
+    sets = [(J2, par, inputs.enumerate_3n_channels(J2, par, 1, 3)) for J2 in range(1, 19, 2) for par in (+1, -1)]
+    handles = [api.pm_lattice_attach(lat.h, ch, J2, par, 1, inputs.PM_FERMION_ISOSPIN) for J2, par, ch in sets]
+    cap = hits * max(int(api.pm_lattice_coupling(h, len(ch))[0].sum()) for h, (_, _, ch) in zip(handles, sets))
+    ci = torch.empty(cap, dtype=torch.int32, device="cuda")
+    v = torch.empty(cap, dtype=torch.float64, device="cuda")
+    rows, total_ms, total_nnz = [], 0.0, 0
+    for h, (J2, par, ch) in zip(handles, sets):
+        rpj = rp[: wl.n_cells * len(ch) + 1]
+        api.pm_build_reuse(h, 0, wl.n_cells, rpj, ci, v)                 # untimed: run-time compilation of the set's kernel, if any
+        flush.zero_()
+        e0.record(st)
+        n = api.pm_build_reuse(h, 0, wl.n_cells, rpj, ci, v)
+        e1.record(st); torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        rows.append({"J2": J2, "parity": par, "channels": len(ch), "nnz": n, "ms": ms, "kernel": api.pm_lattice_fill_kernel(h)})
+        total_ms += ms; total_nnz += n
+        api.pm_lattice_destroy(h)
+    del ci, v, rp
+    torch.cuda.empty_cache()
+    return {"what": f"all 18 J^pi <= 17/2, pair j <= 3, T = 1/2 on {wl.name}'s grid; pattern pass once + one pm_build_reuse per J^pi",
+            "pattern_ms_once": pattern_ms, "fill_ms_total": total_ms, "total_ms": pattern_ms + total_ms, "total_nnz": total_nnz,
+            "nnz_per_s": total_nnz / ((pattern_ms + total_ms) * 1e-3), "max_channels": max(r["channels"] for r in rows),
+            "csr_bytes_largest": 12 * max(r["nnz"] for r in rows), "sets": rows}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -272,6 +308,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-lattices", action="store_true", help="skip the five-lattice table")
+    ap.add_argument("--sweep", action="store_true", help="also time the sweep over all J^pi <= 17/2 (62 channels) on the workload's grid")
     ap.add_argument("--e2e-steps", type=int, default=2)
     args = ap.parse_args()
     args.config = int(args.config)
@@ -418,6 +455,18 @@ def main():
             lk.close()
             del rpk, cik, vk
 
+    # ---- every J^pi <= 17/2 on this grid (on request: ~70 GB of device buffers, ~25 s)
+    sweep = None
+    if args.sweep:
+        try:
+            del colidx, vals
+            torch.cuda.empty_cache()
+            sweep = jpi_sweep(api, torch, lat, wl, flush, st)
+            colidx = torch.empty(nnz, dtype=torch.int32, device="cuda")
+            vals = torch.empty(nnz, dtype=torch.float64, device="cuda")
+        except Exception as ex:                                  # the headline line must not depend on it
+            sweep = {"error": repr(ex)}
+
     # ---- end to end through the C ABI with HOST buffers (D2H copies inside the timed region)
     e2e = None
     if not args.no_e2e:
@@ -462,7 +511,7 @@ def main():
                         "pattern_median": float(np.median(np.array(step_ms) - np.array(fill_ms))),
                         "fill_median": float(np.median(fill_ms)), "fill_best": float(np.min(fill_ms)),
                         "fill_all": [round(float(x), 3) for x in fill_ms]},
-           "roofline": roof, "spmv": spmv, "iteration": iteration, "rotation": rotation, "lattices": lattices,
+           "roofline": roof, "spmv": spmv, "iteration": iteration, "rotation": rotation, "lattices": lattices, "sweep": sweep,
            "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks.summary()}
     print(json.dumps(out))
     lat.close()

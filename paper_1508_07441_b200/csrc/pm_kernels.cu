@@ -330,7 +330,16 @@ __global__ void __launch_bounds__(256) k_spmv(int64_t n_rows, const int64_t* __r
     const int64_t wpb = blockDim.x >> 5;
     for (int64_t r = (int64_t)blockIdx.x * wpb + (threadIdx.x >> 5); r < n_rows; r += (int64_t)gridDim.x * wpb) {
         double s = 0.0;
-        for (int64_t k = rowptr[r] + lane; k < rowptr[r + 1]; k += 32) s += vals[k] * x[colidx[k]];
+        int64_t k = rowptr[r] + lane;
+        const int64_t ke = rowptr[r + 1];
+        for (; k + 96 < ke; k += 128) {                    // four independent element chains in flight per lane
+            double vv[4], xx[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) { vv[u] = vals[k + 32 * u]; xx[u] = x[colidx[k + 32 * u]]; }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) s += vv[u] * xx[u];
+        }
+        for (; k < ke; k += 32) s += vals[k] * x[colidx[k]];
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
         if (lane == 0) y[r] = s;
