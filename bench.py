@@ -458,14 +458,14 @@ def main():
     # ---- every J^pi <= 17/2 on this grid (on request: ~70 GB of device buffers, ~25 s)
     sweep = None
     if args.sweep:
+        colidx = vals = None                                     # (the sweep needs ~70 GB of its own)
+        torch.cuda.empty_cache()
         try:
-            del colidx, vals
-            torch.cuda.empty_cache()
             sweep = jpi_sweep(api, torch, lat, wl, flush, st)
-            colidx = torch.empty(nnz, dtype=torch.int32, device="cuda")
-            vals = torch.empty(nnz, dtype=torch.float64, device="cuda")
         except Exception as ex:                                  # the headline line must not depend on it
             sweep = {"error": repr(ex)}
+            print("sweep failed:", repr(ex), file=sys.stderr)
+        torch.cuda.empty_cache()
 
     # ---- end to end through the C ABI with HOST buffers (D2H copies inside the timed region)
     e2e = None
@@ -473,7 +473,7 @@ def main():
         h_rp = torch.empty(wl.M + 1, dtype=torch.int64, pin_memory=True)
         h_ci = torch.empty(nnz, dtype=torch.int32, pin_memory=True)
         h_v = torch.empty(nnz, dtype=torch.float64, pin_memory=True)
-        del colidx, vals
+        colidx = vals = None
         torch.cuda.empty_cache()
 
         def e2e_step():

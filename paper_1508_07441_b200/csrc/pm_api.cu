@@ -94,9 +94,11 @@ struct pm_lattice {
     bool have_plan = false;            // every group has its launch plan
     bool jit_failed = false;           // run-time compilation was tried for this lattice and failed (jit_error says why)
     std::string jit_error;
-    std::vector<pm::GroupTables> groups;   // column-channel groups (one unless the set exceeds what one kernel holds)
+    std::vector<pm::GroupTables> groups;   // column-channel groups the table-driven kernel can hold (one for small sets)
+    std::vector<pm::GroupTables> whole;    // the whole set as one group, for a run-time specialised kernel (empty when groups is that already)
     struct GroupDev { pm::DevLattice dev; pm::FillLaunch plan; };
-    std::vector<GroupDev> gdev;
+    std::vector<GroupDev> gdev, gdev_whole;
+    bool use_whole = false;            // the last plan runs the whole set through one run-time specialised kernel
     cudaEvent_t ev_fill0 = nullptr, ev_fill1 = nullptr;   // around the last fill kernel, on its stream (pm_last_fill_ms)
     bool fill_timed = false;
     unsigned long long hash = 0;       // pm::tables_hash of T (selects a generated fill kernel)
@@ -135,7 +137,7 @@ void free_lattice_device(pm_lattice* L)
     if (L->d_blob) cudaFree(L->d_blob);
     if (L->ev_fill0) cudaEventDestroy(L->ev_fill0);
     if (L->ev_fill1) cudaEventDestroy(L->ev_fill1);
-    L->d_blob = nullptr; L->ev_fill0 = L->ev_fill1 = nullptr; L->fill_timed = false; L->geo_version = 0; L->have_plan = false;
+    L->d_blob = nullptr; L->ev_fill0 = L->ev_fill1 = nullptr; L->fill_timed = false; L->geo_version = 0; L->have_plan = false; L->use_whole = false;
 }
 
 struct Blob {
@@ -241,9 +243,12 @@ int32_t ensure_device(pm_lattice* L)
     const size_t o_ya = B.put(T.ya.data(), 8 * T.ya.size()), o_yb = B.put(T.yb.data(), 8 * T.yb.size());
     const size_t o_yd = B.put(T.ydiag.data(), 8 * T.ydiag.size());
     struct GOff { size_t ktoff, ktip, ktiq, ktc, fun, otoff, otf, otc, ga, gm, gap; };
-    std::vector<GOff> go(L->groups.size());
-    for (size_t g = 0; g < L->groups.size(); ++g) {
-        const pm::GroupTables& Gt = L->groups[g];
+    std::vector<const pm::GroupTables*> all;           // the groups, then the whole-set group (if kept)
+    for (const pm::GroupTables& Gt : L->groups) all.push_back(&Gt);
+    for (const pm::GroupTables& Gt : L->whole) all.push_back(&Gt);
+    std::vector<GOff> go(all.size());
+    for (size_t g = 0; g < all.size(); ++g) {
+        const pm::GroupTables& Gt = *all[g];
         std::vector<int4> fun(Gt.fun.size());
         for (size_t f = 0; f < Gt.fun.size(); ++f) fun[f] = make_int4(Gt.fun[f].sa0, Gt.fun[f].sb0, Gt.fun[f].nM, Gt.fun[f].L);
         go[g].ktoff = B.put(Gt.kt_off.data(), 4 * Gt.kt_off.size()); go[g].ktip = B.put(Gt.kt_ip.data(), 4 * Gt.kt_ip.size());
@@ -263,8 +268,9 @@ int32_t ensure_device(pm_lattice* L)
     D.bra = (const double*)(b + o_bra);
     D.ya = (const double*)(b + o_ya); D.yb = (const double*)(b + o_yb); D.ydiag = (const double*)(b + o_yd);
     L->gdev.assign(L->groups.size(), pm_lattice::GroupDev{});
-    for (size_t g = 0; g < L->groups.size(); ++g) {
-        const pm::GroupTables& Gt = L->groups[g];
+    L->gdev_whole.assign(L->whole.size(), pm_lattice::GroupDev{});
+    for (size_t g = 0; g < all.size(); ++g) {
+        const pm::GroupTables& Gt = *all[g];
         pm::DevLattice Dg = D;
         Dg.n_slot = Gt.n_slot; Dg.n_fun = (int)Gt.fun.size(); Dg.n_out = (int)Gt.o_alpha.size();
         Dg.kt_off = (const int*)(b + go[g].ktoff); Dg.kt_ip = (const int*)(b + go[g].ktip); Dg.kt_iq = (const int*)(b + go[g].ktiq);
@@ -272,7 +278,7 @@ int32_t ensure_device(pm_lattice* L)
         Dg.fun = (const int4*)(b + go[g].fun);
         Dg.ot_off = (const int*)(b + go[g].otoff); Dg.ot_f = (const int*)(b + go[g].otf); Dg.ot_c = (const double*)(b + go[g].otc);
         Dg.g_alpha = (const int*)(b + go[g].ga); Dg.g_m = (const int*)(b + go[g].gm); Dg.g_ap = (const int*)(b + go[g].gap);
-        L->gdev[g].dev = Dg;
+        (g < L->groups.size() ? L->gdev[g] : L->gdev_whole[g - L->groups.size()]).dev = Dg;
     }
     D = L->gdev[0].dev;                                 // (the pattern kernels read the geometric and coupled-list fields only)
     L->dev = D;
@@ -330,7 +336,9 @@ int32_t make_lattice(pm_geometry* G, const pm_channel* ch, int32_t n_ch, int32_t
     msg = pm::build_tables(ch, n_ch, J2, T2, statistics, L->T);
     if (!msg.empty()) { delete L; return fail(PM_ERR_CHANNEL, msg); }
     L->hash = pm::tables_hash(L->T);
-    pm::build_groups(L->T, ch, pm::kFillMaxSlot, pm::kFillMaxFun, L->groups);
+    pm::build_groups(L->T, ch, pm::kFillMaxSlot, pm::kFillMaxFun, pm::kFillMaxOut, L->groups);
+    if (L->groups.size() > 1 && L->T.n_slot <= pm::kFillMaxSlot && (int)L->T.fun.size() <= pm::kFillMaxFun)
+        pm::build_groups(L->T, ch, 1 << 30, 1 << 30, 1 << 30, L->whole);
     for (const pm::GroupTables& Gt : L->groups)
         if (Gt.n_slot > pm::kFillMaxSlot || (int)Gt.fun.size() > pm::kFillMaxFun) {
             delete L; return fail(PM_ERR_CHANNEL, "one orbital pair (l', lambda') of this channel set needs more ket slots than a kernel holds");
@@ -503,9 +511,9 @@ const char* pm_lattice_fill_kernel(const pm_lattice* lat)
 {
     if (!lat) return "";
     if (pm::fill_has_spec(lat->hash)) return pm::fill_variant_name(lat->hash);
-    if (lat->groups.size() > 1) return "generic-grouped";                   // table-driven kernel, one launch per column-channel group
-    if (lat->have_plan && !lat->gdev.empty()) return lat->gdev[0].plan.name; // what the last fill ran: "jit" or "generic"
-    return (pm::jit_enabled() && !lat->jit_failed) ? "jit" : "generic";
+    const bool may_jit = (lat->groups.size() == 1 || !lat->whole.empty()) && pm::jit_enabled() && !lat->jit_failed;
+    if (lat->have_plan) return lat->use_whole ? "jit" : (lat->groups.size() > 1 ? "generic-grouped" : lat->gdev[0].plan.name);
+    return may_jit ? "jit" : (lat->groups.size() > 1 ? "generic-grouped" : "generic");
 }
 
 int32_t pm_set_jit(int32_t enabled)
@@ -519,7 +527,7 @@ int32_t pm_diag_jit_compile(const pm_lattice* lat, int64_t* cubin_bytes)
     if (!lat) return fail(PM_ERR_ARG, "lat is NULL");
     std::string err;
     size_t n = 0;
-    if (lat->groups.size() > 1) return fail(PM_ERR_STATE, "this channel set runs the table-driven kernel group by group; nothing to compile");
+    if (lat->groups.size() > 1 && lat->whole.empty()) return fail(PM_ERR_STATE, "this channel set runs the table-driven kernel group by group; nothing to compile");
     if (!pm::jit_compile_check(lat->T, 12, 4, &n, err)) return fail(PM_ERR_STATE, err);
     if (cubin_bytes) *cubin_bytes = (int64_t)n;
     return PM_OK;
@@ -625,12 +633,14 @@ int32_t fill_block(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const 
     const int n_blk = cell_end - cell_begin;
     cudaError_t e;
     const bool grouped = lat->gdev.size() > 1;         // big channel sets: one table-driven launch per column-channel group
-    if (!lat->have_plan && !grouped && !pm::fill_has_spec(lat->hash) && pm::jit_enabled() && !lat->jit_failed) {
+    std::vector<pm_lattice::GroupDev>& one = lat->gdev_whole.empty() ? lat->gdev : lat->gdev_whole;     // the whole set as one group, if it may be
+    if (!lat->have_plan && one.size() == 1 && !pm::fill_has_spec(lat->hash) && pm::jit_enabled() && !lat->jit_failed) {
         // no build-time kernel for this channel set: specialise at run time (pm_jit.hpp), else fall back below
-        if (pm::fill_plan_jit(lat->gdev[0].dev, lat->T, lat->hash, G->n_sm, &lat->gdev[0].plan, lat->jit_error)) lat->have_plan = true;
+        if (pm::fill_plan_jit(one[0].dev, lat->T, lat->hash, G->n_sm, &one[0].plan, lat->jit_error)) { lat->have_plan = true; lat->use_whole = &one == &lat->gdev_whole; }
         else lat->jit_failed = true;
     }
     if (!lat->have_plan) {
+        lat->use_whole = false;
         for (auto& gd : lat->gdev) {
             e = pm::fill_plan(gd.dev, grouped ? 0ull : lat->hash, G->n_sm, &gd.plan);
             if (e == cudaErrorInvalidConfiguration) { cudaGetLastError(); return fail(PM_ERR_NOMEM, "channel set needs more shared memory than one SM has"); }
@@ -639,7 +649,7 @@ int32_t fill_block(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const 
         lat->have_plan = true;
     }
     if ((e = cudaEventRecord(lat->ev_fill0, st)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
-    for (auto& gd : lat->gdev) {
+    for (auto& gd : (lat->use_whole ? lat->gdev_whole : lat->gdev)) {
         e = pm::launch_fill(gd.dev, gd.plan, cell_begin, n_blk, G->nl, d_rowptr, d_vals, d_colidx, G->d_counter, guard, st);
         if (e != cudaSuccess) return cuda_fail(e, "k_fill");
     }

@@ -24,6 +24,7 @@ struct FillVariant { unsigned long long hash; int nw, rb; FillKernel fn, fn_cols
 #define PM_SPEC(S) PM_VAR(S, 4, 4), PM_VAR(S, 8, 4), PM_VAR(S, 12, 4),
 const FillVariant kVariants[] = {
     PM_SPEC_LIST
+    {0ull, 2, 4, k_fill_warp<SpecGeneric, 2, 4, false>, k_fill_warp<SpecGeneric, 2, 4, true>, "generic"},
     {0ull, 4, 4, k_fill_warp<SpecGeneric, 4, 4, false>, k_fill_warp<SpecGeneric, 4, 4, true>, "generic"},
     {0ull, 8, 4, k_fill_warp<SpecGeneric, 8, 4, false>, k_fill_warp<SpecGeneric, 8, 4, true>, "generic"},
 };

@@ -22,6 +22,7 @@ namespace pm {
 
 constexpr int kFillMaxSlot = 96;       // ket slots / orbital functions one kernel launch holds (larger channel sets are
 constexpr int kFillMaxFun = 320;       // split into column-channel groups, pm_tables.hpp)
+constexpr int kFillMaxOut = 1400;      // outputs (alpha, alpha') per launch of the table-driven kernel (their tables live in shared memory)
 constexpr int kFillMaxY = 91;          // harmonics per direction up to l = PM_MAX_L = 12
 
 // Table-driven ket code for channel sets without a generated kernel (slow: local arrays, table loads).

@@ -279,7 +279,7 @@ std::string build_tables(const pm_channel* ch, int n_ch, int J2, int T2, int sta
     return "";
 }
 
-void build_groups(const Tables& T, const pm_channel* ch, int max_slot, int max_fun, std::vector<GroupTables>& groups)
+void build_groups(const Tables& T, const pm_channel* ch, int max_slot, int max_fun, int max_out, std::vector<GroupTables>& groups)
 {
     groups.clear();
     const int n_tri = (int)T.tri.size(), n_fun = (int)T.fun.size();
@@ -295,15 +295,22 @@ void build_groups(const Tables& T, const pm_channel* ch, int max_slot, int max_f
     }
     for (const OrbFun& f : T.fun) cls_funs[(size_t)tri_cls[(size_t)f.tb]]++;
     const int n_cls = (int)cls_slots.size();
+    std::vector<int> cls_outs((size_t)n_cls, 0);       // outputs (alpha, alpha') whose column channel has the class's orbital pair
+    for (int o = 0; o < T.totcoup; ++o) {
+        const auto it = cls_id.find(std::make_pair(ch[T.cl[(size_t)o]].l, ch[T.cl[(size_t)o]].lam));
+        if (it != cls_id.end()) cls_outs[(size_t)it->second]++;
+    }
     std::vector<int> cls_grp((size_t)n_cls, 0);
     int n_grp = 1;
-    if (T.n_slot > max_slot || n_fun > max_fun) {
-        int gs = 0, gf = 0;
+    if (T.n_slot > max_slot || n_fun > max_fun || T.totcoup > max_out) {
+        int gs = 0, gf = 0, go = 0;
         n_grp = 0;
         for (int c = 0; c < n_cls; ++c) {
-            if (n_grp == 0 || gs + cls_slots[(size_t)c] > max_slot || gf + cls_funs[(size_t)c] > max_fun) { ++n_grp; gs = 0; gf = 0; }
+            if (n_grp == 0 || gs + cls_slots[(size_t)c] > max_slot || gf + cls_funs[(size_t)c] > max_fun || go + cls_outs[(size_t)c] > max_out) {
+                ++n_grp; gs = 0; gf = 0; go = 0;
+            }
             cls_grp[(size_t)c] = n_grp - 1;
-            gs += cls_slots[(size_t)c]; gf += cls_funs[(size_t)c];
+            gs += cls_slots[(size_t)c]; gf += cls_funs[(size_t)c]; go += cls_outs[(size_t)c];
         }
     }
     groups.resize((size_t)n_grp);

@@ -54,8 +54,9 @@ struct GroupTables {
     std::vector<double> ot_c;
 };
 
-// One group holding everything when the set fits (max_slot, max_fun), else a greedy packing of the (l', lam') classes.
-void build_groups(const Tables& T, const pm_channel* ch, int max_slot, int max_fun, std::vector<GroupTables>& groups);
+// One group holding everything when the set fits (max_slot, max_fun, max_out outputs), else a greedy packing of the
+// (l', lam') classes under the three limits.
+void build_groups(const Tables& T, const pm_channel* ch, int max_slot, int max_fun, int max_out, std::vector<GroupTables>& groups);
 
 // Algebra (doubled arguments), exposed for host tests through the C ABI indirectly (pm_lattice_coupling).
 double clebsch(int j1, int m1, int j2, int m2, int j3, int m3);
