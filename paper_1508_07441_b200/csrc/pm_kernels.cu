@@ -162,16 +162,27 @@ k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl,
             const int nr = min(S.hist_cap, H - r0);
             for (int k = lane; k < nr; k += 32) hist[k] = 0;
             __syncwarp();
-            // ---- pass 2: nodes per rank
-            for (int st = 0; st < nsteps; ++st) {
-                const int m = st * 32 + lane;
-                const unsigned t = m < L.nnode ? (unsigned)s_t[m] : kOff;
-                int r = -1;
-                if (t != kOff) r = (int)wpre[t >> 5] + __popc(bits[t >> 5] & ((1u << (t & 31)) - 1u)) - r0;
-                const bool in = r >= 0 && r < nr;
-                const unsigned same = __match_any_sync(0xffffffffu, in ? r : -1 - lane);
-                if (in && (same & lt) == 0u) hist[r] += __popc(same);
-                __syncwarp();
+            // ---- pass 2: nodes per rank (the targets of the next four steps are fetched while four are processed)
+            {
+                unsigned tn[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) { const int m = u * 32 + lane; tn[u] = m < L.nnode ? (unsigned)s_t[m] : kOff; }
+                for (int st0 = 0; st0 < nsteps; st0 += 4) {
+                    unsigned tt[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) { tt[u] = tn[u]; const int m = (st0 + 4 + u) * 32 + lane; tn[u] = m < L.nnode ? (unsigned)s_t[m] : kOff; }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        if (st0 + u >= nsteps) break;
+                        const unsigned t = tt[u];
+                        int r = -1;
+                        if (t != kOff) r = (int)wpre[t >> 5] + __popc(bits[t >> 5] & ((1u << (t & 31)) - 1u)) - r0;
+                        const bool in = r >= 0 && r < nr;
+                        const unsigned same = __match_any_sync(0xffffffffu, in ? r : -1 - lane);
+                        if (in && (same & lt) == 0u) hist[r] += __popc(same);
+                        __syncwarp();
+                    }
+                }
             }
             // ---- exclusive scan of the counts, offset by what earlier windows placed
             for (int k0 = 0; k0 < nr; k0 += 32) {
@@ -184,18 +195,30 @@ k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl,
             }
             __syncwarp();
             // ---- pass 3: placement in node order (stable)
-            for (int st = 0; st < nsteps; ++st) {
-                const int m = st * 32 + lane;
-                const unsigned t = m < L.nnode ? (unsigned)s_t[m] : kOff;
-                int r = -1;
-                if (t != kOff) r = (int)wpre[t >> 5] + __popc(bits[t >> 5] & ((1u << (t & 31)) - 1u)) - r0;
-                const bool in = r >= 0 && r < nr;
-                const unsigned same = __match_any_sync(0xffffffffu, in ? r : -1 - lane);
-                int base = 0;
-                if (in) { base = hist[r]; g_key[base + __popc(same & lt)] = (t << 14) | (unsigned)m; }
-                __syncwarp();
-                if (in && (same & lt) == 0u) hist[r] = base + __popc(same);
-                __syncwarp();
+            {
+                unsigned tn[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) { const int m = u * 32 + lane; tn[u] = m < L.nnode ? (unsigned)s_t[m] : kOff; }
+                for (int st0 = 0; st0 < nsteps; st0 += 4) {
+                    unsigned tt[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) { tt[u] = tn[u]; const int m = (st0 + 4 + u) * 32 + lane; tn[u] = m < L.nnode ? (unsigned)s_t[m] : kOff; }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        if (st0 + u >= nsteps) break;
+                        const int m = (st0 + u) * 32 + lane;
+                        const unsigned t = tt[u];
+                        int r = -1;
+                        if (t != kOff) r = (int)wpre[t >> 5] + __popc(bits[t >> 5] & ((1u << (t & 31)) - 1u)) - r0;
+                        const bool in = r >= 0 && r < nr;
+                        const unsigned same = __match_any_sync(0xffffffffu, in ? r : -1 - lane);
+                        int base = 0;
+                        if (in) { base = hist[r]; g_key[base + __popc(same & lt)] = (t << 14) | (unsigned)m; }
+                        __syncwarp();
+                        if (in && (same & lt) == 0u) hist[r] = base + __popc(same);
+                        __syncwarp();
+                    }
+                }
             }
         }
         if (lane == 0) { nl.hits[cb] = H; nl.ntot[cb] = placed; }
