@@ -112,6 +112,8 @@ void free_lists(pm_geometry* G)
     if (G->nl.key) cudaFree(G->nl.key);
     if (G->nl.ntot) cudaFree(G->nl.ntot);
     if (G->nl.hits) cudaFree(G->nl.hits);
+    if (G->nl.chunk) cudaFree(G->nl.chunk);
+    if (G->nl.nchunk) cudaFree(G->nl.nchunk);
     if (G->d_cellbase) cudaFree(G->d_cellbase);
     G->nl = pm::NodeLists{}; G->d_cellbase = nullptr; G->cells_cap = 0;
     G->lists_valid = false; G->hitlist_valid = false; G->hmax = -1;
@@ -287,6 +289,13 @@ int32_t ensure_device(pm_lattice* L)
     return PM_OK;
 }
 
+// nodes one lane of the fill kernel sums before the cross-lane segment sums (PM_CHUNK_LEN: tuning / test hook)
+int chunk_len()
+{
+    static const int v = [] { const char* e = std::getenv("PM_CHUNK_LEN"); const int x = e ? std::atoi(e) : 4; return x < 1 ? 1 : (x > pm::kMaxChunkLen ? pm::kMaxChunkLen : x); }();
+    return v;
+}
+
 int32_t ensure_cell_scratch(pm_geometry* G, int n_blk)
 {
     if (n_blk <= G->cells_cap) return PM_OK;
@@ -296,6 +305,14 @@ int32_t ensure_cell_scratch(pm_geometry* G, int n_blk)
     if ((e = cudaMalloc(&G->nl.key, sizeof(unsigned) * nn)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(node lists)");
     if ((e = cudaMalloc(&G->nl.ntot, sizeof(int) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(ntot)");
     if ((e = cudaMalloc(&G->nl.hits, sizeof(int) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(hits)");
+    if ((e = cudaMalloc(&G->nl.chunk, sizeof(uint2) * nn)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(chunk lists)");
+    if ((e = cudaMalloc(&G->nl.nchunk, sizeof(int) * (size_t)n_blk)) != cudaSuccess) return cuda_fail(e, "cudaMalloc(nchunk)");
+    {   // (a, b) indices are packed into 32 bits per chunk
+        int bits = 1;
+        while ((1 << bits) < G->geo.n_p * G->geo.n_q) ++bits;
+        G->nl.ab_bits = bits;
+        G->nl.chunk_len = std::max(1, std::min(chunk_len(), 32 / bits));
+    }
     if ((e = cudaMalloc(&G->d_cellbase, sizeof(int64_t) * ((size_t)n_blk + 1))) != cudaSuccess) return cuda_fail(e, "cudaMalloc(cellbase)");
     G->cells_cap = n_blk;
     return PM_OK;

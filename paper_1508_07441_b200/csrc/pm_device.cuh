@@ -52,11 +52,21 @@ struct DevLattice {
 // nnode per source cell: for every node that hit the grid, in the order (target cell, node id),
 //   key   = target cell << 14 | node id     (node id m = c*(n_p*n_q) + a*n_q + b < 2^14, cell < 2^18).
 // The rank of a target among the source cell's hit cells is the number of target changes before it.
+// Chunks: the sorted list cut into runs of at most chunk_len consecutive nodes that never cross a (target, x-node)
+// segment; one lane of the fill kernel sums the ket harmonics of one chunk in registers (pm_fill.cuh).  A chunk carries
+// the (a, b) indices of its nodes, so the fill reads no node key on its per-node path:
+//   chunk.x = first sorted position | (len - 1) << 14 | ends a segment << 18 | ends a target << 19 | x-node c << 20
+//   chunk.y = ab_0 | ab_1 << ab_bits | ...        (ab = a*n_q + b < 2^ab_bits, len * ab_bits <= 32)
 struct NodeLists {
     unsigned* key;              // [n_blk][nnode]
     int* ntot;                  // [n_blk] nodes on the grid
     int* hits;                  // [n_blk] hit cells H
+    uint2* chunk;               // [n_blk][nnode] (at most one chunk per node)
+    int* nchunk;                // [n_blk]
+    int chunk_len;              // longest chunk the pattern pass cuts: min(wanted, 32 / ab_bits)
+    int ab_bits;                // bits of one (a, b) index in chunk.y
 };
+constexpr int kMaxChunkLen = 16;
 
 struct CellGeom { double cp, hp, cq, hq; };
 
@@ -80,11 +90,17 @@ __device__ __forceinline__ void split_node(const DevLattice& L, int m, int& c, i
 
 // DESIGN.md sec. 3.1, exactly:  p = cp + hp*t_a ; q = cq + hq*t_b ; x = t_c ; pq = p*q
 //   P2 = (0.25*(p*p) + 0.5625*(q*q)) + 0.75*(pq*x) ;  Q2 = ((p*p) + 0.25*(q*q)) - pq*x ; clamp at 0
+__device__ __forceinline__ void map_pq_sq(double p, double q, double tc, double& P2, double& Q2);
 __device__ __forceinline__ void map_node_sq(const CellGeom& g, double ta, double tb, double tc,
                                             double& p, double& q, double& P2, double& Q2)
 {
     p = __dadd_rn(g.cp, __dmul_rn(g.hp, ta));
     q = __dadd_rn(g.cq, __dmul_rn(g.hq, tb));
+    map_pq_sq(p, q, tc, P2, Q2);
+}
+// the map from a node's (p, q, x) on
+__device__ __forceinline__ void map_pq_sq(double p, double q, double tc, double& P2, double& Q2)
+{
     const double pq = __dmul_rn(p, q), p2 = __dmul_rn(p, p), q2 = __dmul_rn(q, q), pqx = __dmul_rn(pq, tc);
     P2 = __dadd_rn(__dadd_rn(__dmul_rn(0.25, p2), __dmul_rn(0.5625, q2)), __dmul_rn(0.75, pqx));
     Q2 = __dsub_rn(__dadd_rn(p2, __dmul_rn(0.25, q2)), pqx);

@@ -5,6 +5,7 @@
 #include <cstdio>
 #include <map>
 #include <sstream>
+#include <vector>
 
 namespace pm {
 
@@ -60,30 +61,42 @@ std::string emit_spec(const std::string& name, const Tables& T, EmitStats& st)
     o << "    static constexpr int NS = " << T.n_slot << ", NF = " << nf << ", NCH = " << (nf + 31) / 32 << ", MAXM = " << maxm << ", MAXL1 = " << maxl1 << ";\n";
     char hb[32]; std::snprintf(hb, sizeof hb, "0x%016" PRIx64 "ull", tables_hash(T));
     o << "    static constexpr unsigned long long kHash = " << hb << ";\n";
-    o << "    // K[s] = omega * (ket bipolar harmonic of slot s) at directions a = p'^ = (uxa,0,uza), b = q'^ = (uxb,0,uzb)\n";
-    o << "    static __device__ __forceinline__ void ket(const DevLattice&, double om, double uxa, double uza, double uxb, double uzb,\n"
-         "                                               double (&K)[NS])\n    {\n";
+    o << "    // K[s] += omega * (ket bipolar harmonic of slot s) at directions a = p'^ = (uxa,0,uza), b = q'^ = (uxb,0,uzb)\n";
+    o << "    static __device__ __forceinline__ void ket_acc(const DevLattice&, double om, double uxa, double uza, double uxb, double uzb,\n"
+         "                                                   double (&K)[NS])\n    {\n";
     emit_q(o, 'a', la, "om", "uxa", "uza", ybeta);
-    emit_q(o, 'b', lb, "1.0", "uxb", "uzb", ybeta);
-    // products shared by several terms
-    std::map<std::pair<int, int>, int> uses;
-    for (size_t t = 0; t < T.kt_c.size(); ++t) uses[{T.kt_ip[t], T.kt_iq[t]}]++;
-    for (auto& kv : uses) {
-        o << "        const double t" << kv.first.first << "_" << kv.first.second << " = " << yname('a', kv.first.first) << " * "
-          << yname('b', kv.first.second) << ";\n";
-        st.n_prod++;
-    }
-    for (int s = 0; s < T.n_slot; ++s) {
-        const int b = T.kt_off[(size_t)s], e = T.kt_off[(size_t)s + 1];
-        if (b == e) { o << "        K[" << s << "] = 0.0;\n"; continue; }
-        std::string expr;
-        for (int t = b; t < e; ++t) {
-            const double c = T.kt_c[(size_t)t] * ynorm[(size_t)T.kt_ip[(size_t)t]] * ynorm[(size_t)T.kt_iq[(size_t)t]];
-            const std::string p = "t" + std::to_string(T.kt_ip[(size_t)t]) + "_" + std::to_string(T.kt_iq[(size_t)t]);
-            if (t == b) { expr = num(c) + " * " + p; st.n_mul++; }
-            else { expr = "fma(" + num(c) + ", " + p + ", " + expr + ")"; st.n_fma++; }
+    // The q' side harmonic by harmonic (m-major recurrence): each b_lm is multiplied into its products and those into the
+    // running sums K[s] at once, so only the p' side harmonics and two or three b values are live at any point (the
+    // accumulators K take 2*NS registers; short live ranges are what keeps the rest of the kernel out of local memory).
+    std::map<std::pair<int, int>, std::vector<size_t>> terms;             // (iq, ip) -> ket terms
+    for (int s = 0; s < T.n_slot; ++s)
+        for (int t = T.kt_off[(size_t)s]; t < T.kt_off[(size_t)s + 1]; ++t) terms[{T.kt_iq[(size_t)t], T.kt_ip[(size_t)t]}].push_back((size_t)t);
+    std::vector<int> slot_of(T.kt_c.size());
+    for (int s = 0; s < T.n_slot; ++s)
+        for (int t = T.kt_off[(size_t)s]; t < T.kt_off[(size_t)s + 1]; ++t) slot_of[(size_t)t] = s;
+    for (int m = 0; m <= lb; ++m) {
+        for (int l = m; l <= lb; ++l) {
+            const int iq = ylm_index(l, m);
+            const std::string bn = yname('b', iq);
+            o << "        const double " << bn << " = ";
+            if (l == 0) o << "1.0;\n";
+            else if (l == m) o << "uxb * " << yname('b', ylm_index(m - 1, m - 1)) << ";\n";
+            else if (l == m + 1) o << "uzb * " << yname('b', ylm_index(l - 1, m)) << ";\n";
+            else o << "fma(uzb, " << yname('b', ylm_index(l - 1, m)) << ", " << num(-ybeta[(size_t)iq]) << " * " << yname('b', ylm_index(l - 2, m)) << ");\n";
+            for (auto it = terms.lower_bound({iq, -1}); it != terms.end() && it->first.first == iq; ++it) {
+                const int ip = it->first.second;
+                const std::string p = "t" + std::to_string(ip) + "_" + std::to_string(iq);
+                o << "        { const double " << p << " = " << yname('a', ip) << " * " << bn << ";";
+                st.n_prod++;
+                for (size_t t : it->second) {
+                    const double c = T.kt_c[t] * ynorm[(size_t)T.kt_ip[t]] * ynorm[(size_t)T.kt_iq[t]];
+                    const int s = slot_of[t];
+                    o << " K[" << s << "] = fma(" << num(c) << ", " << p << ", K[" << s << "]);";
+                    st.n_fma++;
+                }
+                o << " }\n";
+            }
         }
-        o << "        K[" << s << "] = " << expr << ";\n";
     }
     o << "    }\n};\n\n";
     return o.str();

@@ -32,7 +32,7 @@ struct SpecGeneric {
     static constexpr unsigned long long kHash = 0ull;
     // writes the node's column of the K tile directly (no per-thread K array): col = tile + lane, np slot pairs
     static __device__ __noinline__ void ket_tile(const DevLattice& L, double om, double uxa, double uza, double uxb, double uzb,
-                                                 double2* __restrict__ col, int stride, int np, int ns)
+                                                 double2* __restrict__ col, int stride, int np, int ns, bool first)
     {
         double Yp[kFillMaxY], Yq[kFillMaxY];
         ylm_fill(L.lmax, uxa, uza, L.ya, L.yb, L.ydiag, Yp);
@@ -48,13 +48,14 @@ struct SpecGeneric {
                     v[h] = a * om;
                 }
             }
+            if (!first) { const double2 o = col[i * stride]; v[0] += o.x; v[1] += o.y; }       // running sum of the lane's chunk
             col[i * stride] = make_double2(v[0], v[1]);
         }
     }
 };
 
 struct FillSmem {           // byte offsets into dynamic shared memory, computed on the host
-    int dp, dq, tp, tq, tx, sx, wx, bra, odesc, ofi, oc, warp0, warp_bytes, w_tile, w_sseg, w_acc, w_norm, w_hcol, w_wpa, w_wqb, total;
+    int dp, dq, tx, sx, wx, bra, odesc, ofi, oc, fa, fb, warp0, warp_bytes, w_tile, w_sseg, w_acc, w_norm, w_hcol, w_wpa, w_wqb, w_pa, w_qb, total;
 };
 
 constexpr int kTileStride = 33;        // double2 per K-tile row: 32 nodes + 1 pad (conflict-free rows and columns)
@@ -68,9 +69,10 @@ inline FillSmem fill_smem_plan(const DevLattice& L, int nw, int row_batch, bool 
     int o = 0;
     auto take = [&](int bytes) { int r = o; o += fill_align16(bytes); return r; };
     s.dp = take(8 * L.Np); s.dq = take(8 * L.Nq);
-    s.tp = take(8 * L.n_p); s.tq = take(8 * L.n_q); s.tx = take(8 * L.n_x); s.sx = take(8 * L.n_x); s.wx = take(8 * L.n_x);
+    s.tx = take(8 * L.n_x); s.sx = take(8 * L.n_x); s.wx = take(8 * L.n_x);
     s.bra = bra_in_smem ? take(8 * L.n_x * (L.n_bra + 1)) : -1;      // rows padded with one zero slot; -1: read from global memory
     s.odesc = take(4 * L.n_out); s.ofi = take(4 * L.n_out); s.oc = take(24 * L.n_out);
+    s.fa = take(4 * kFillMaxFun); s.fb = take(4 * kFillMaxFun);        // (every function chunk of the stage reads its entry)
     const int np = (L.n_slot + 1) / 2;              // slot pairs
     int w = 0;
     auto wtake = [&](int bytes) { int r = w; w += fill_align16(bytes); return r; };
@@ -79,7 +81,7 @@ inline FillSmem fill_smem_plan(const DevLattice& L, int nw, int row_batch, bool 
     s.w_acc = wtake(8 * L.n_fun * row_batch);      // sums of finished targets waiting for their rows to be written
     s.w_norm = wtake(8 * row_batch);
     s.w_hcol = wtake(4 * row_batch);
-    s.w_wpa = wtake(8 * L.n_p); s.w_wqb = wtake(8 * L.n_q);
+    s.w_wpa = wtake(8 * L.n_p); s.w_wqb = wtake(8 * L.n_q); s.w_pa = wtake(8 * L.n_p); s.w_qb = wtake(8 * L.n_q);
     s.warp_bytes = w;
     s.warp0 = take(w * nw);
     s.total = o;
@@ -103,7 +105,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
     const int ns = Spec::kStatic ? Spec::NS : L.n_slot, nf = Spec::kStatic ? Spec::NF : L.n_fun, np = (ns + 1) >> 1;
 
     double* s_dp = (double*)(smem + S.dp);   double* s_dq = (double*)(smem + S.dq);
-    double* s_tp = (double*)(smem + S.tp);   double* s_tq = (double*)(smem + S.tq);   double* s_tx = (double*)(smem + S.tx);
+    double* s_tx = (double*)(smem + S.tx);
     double* s_sx = (double*)(smem + S.sx);   double* s_wx = (double*)(smem + S.wx);
     double* s_bra = (double*)(smem + (S.bra >= 0 ? S.bra : 0));
     int* s_odesc = (int*)(smem + S.odesc);             // per output o: cl_off[alpha] | nc << 12 | m << 19 | alpha' << 25
@@ -118,13 +120,13 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
     int* s_hcol = (int*)(wsm + S.w_hcol);               // first column of each finished target: cell * n_ch (kCols)
     double* s_wpa = (double*)(wsm + S.w_wpa);
     double* s_wqb = (double*)(wsm + S.w_wqb);
+    double* s_pa = (double*)(wsm + S.w_pa);
+    double* s_qb = (double*)(wsm + S.w_qb);
 
     // ---- once per CTA: widths, rules, bra harmonics, output descriptors
     // cell norms B_k: widths (reading A) or (e_{k+1}^3 - e_k^3)/3 (reading B, states normalised in the p^2 dp measure)
     for (int k = tid; k < L.Np; k += T) { const double e0 = L.pe[k], e1 = L.pe[k + 1]; s_dp[k] = L.norm ? (e1 * e1 * e1 - e0 * e0 * e0) / 3.0 : e1 - e0; }
     for (int k = tid; k < L.Nq; k += T) { const double e0 = L.qe[k], e1 = L.qe[k + 1]; s_dq[k] = L.norm ? (e1 * e1 * e1 - e0 * e0 * e0) / 3.0 : e1 - e0; }
-    for (int k = tid; k < L.n_p; k += T) s_tp[k] = L.tp[k];
-    for (int k = tid; k < L.n_q; k += T) s_tq[k] = L.tq[k];
     for (int k = tid; k < L.n_x; k += T) { s_tx[k] = L.tx[k]; s_sx[k] = L.sx[k]; s_wx[k] = L.wx[k]; }
     const int nb_ = Spec::kStatic ? Spec::NS : L.n_bra; // bra slots (the whole channel set's)
     const int nsb = nb_ + 1;                            // shared-memory bra rows carry one trailing zero slot (index nb_)
@@ -143,25 +145,25 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         }
         s_ofi[o] = fi;
     }
-    // per-lane descriptors of function f = ch*32 + lane.  kPacked (at most 3 M-terms per function): byte i of fa / fb =
-    // bra / ket slot of term i, unused terms point at the zero bra slot; else fa = sa | nM << 16, fb = sb.
+    // descriptors of function f (lane = f & 31 in the stage), kept in shared memory (registers are what limits the
+    // warps per SM here).  kPacked (at most 3 M-terms per function): byte i of fa / fb = bra / ket slot of term i,
+    // unused terms point at the zero bra slot; else fa = sa | nM << 16, fb = sb.
     constexpr bool kPacked = Spec::MAXM <= 3;
-    int fa[NCH], fb[NCH];
-#pragma unroll
-    for (int ch = 0; ch < NCH; ++ch) {
-        const int f = ch * 32 + lane;
-        fa[ch] = kPacked ? (nb_ | (nb_ << 8) | (nb_ << 16)) : 0;
-        fb[ch] = 0;
+    int* s_fa = (int*)(smem + S.fa);
+    int* s_fb = (int*)(smem + S.fb);
+    for (int f = tid; f < NCH * 32; f += T) {
+        int va = kPacked ? (nb_ | (nb_ << 8) | (nb_ << 16)) : 0, vb = 0;
         if (f < nf) {
             const int4 fn = L.fun[f];
             if (kPacked) {
-                fa[ch] = 0;
+                va = 0;
                 for (int i = 0; i < 3; ++i) {
-                    fa[ch] |= (i < fn.z ? fn.x + i : nb_) << (8 * i);
-                    fb[ch] |= (i < fn.z ? fn.y + i : 0) << (8 * i);
+                    va |= (i < fn.z ? fn.x + i : nb_) << (8 * i);
+                    vb |= (i < fn.z ? fn.y + i : 0) << (8 * i);
                 }
-            } else { fa[ch] = fn.x | (fn.z << 16); fb[ch] = fn.y; }
+            } else { va = fn.x | (fn.z << 16); vb = fn.y; }
         }
+        s_fa[f] = va; s_fb[f] = vb;
     }
     __syncthreads();                                    // the only block-level barrier
 
@@ -172,15 +174,18 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         if (cb >= n_blk) break;
         const int cell = cell_begin + cb;
         const int ci = cell / L.Nq, cj = cell - ci * L.Nq;
-        const CellGeom g = cell_geom(L.pe, L.qe, ci, cj);
-        const int H = nl.hits[cb], we = nl.ntot[cb];
+        const int H = nl.hits[cb], nck = nl.nchunk[cb];
         const unsigned* __restrict__ g_key = nl.key + (size_t)cb * L.nnode;       // target cell << 14 | node id
+        const uint2* __restrict__ g_chunk = nl.chunk + (size_t)cb * L.nnode;      // NodeLists (pm_device.cuh)
         const int64_t rbase = rowptr[(int64_t)cb * L.n_ch];
         double* __restrict__ row0 = vals + rbase;
         int32_t* __restrict__ col0 = kCols ? colidx + rbase : nullptr;
         const double dsrc = s_dp[ci] * s_dq[cj];
-        for (int k = lane; k < L.n_p; k += 32) s_wpa[k] = __dmul_rn(g.hp, L.wp[k]);
-        for (int k = lane; k < L.n_q; k += 32) s_wqb[k] = __dmul_rn(g.hq, L.wq[k]);
+        {   // the cell's nodes p_a = cp + hp t_a, q_b = cq + hq t_b (the operations of map_node_sq) and weights hp wp_a, hq wq_b
+            const CellGeom g = cell_geom(L.pe, L.qe, ci, cj);
+            for (int k = lane; k < L.n_p; k += 32) { s_wpa[k] = __dmul_rn(g.hp, L.wp[k]); s_pa[k] = __dadd_rn(g.cp, __dmul_rn(g.hp, L.tp[k])); }
+            for (int k = lane; k < L.n_q; k += 32) { s_wqb[k] = __dmul_rn(g.hq, L.wq[k]); s_qb[k] = __dadd_rn(g.cq, __dmul_rn(g.hq, L.tq[k])); }
+        }
         __syncwarp();
         int kcur = 0, kdone = 0;                        // targets finished / written; a target's rank is its position in every row
         // ---- E: lane = output (alpha, m-th coupled alpha'): P = norm_t * sum_L c^L acc_t[f] for targets k0 .. k0+nb-1
@@ -221,56 +226,74 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
             if (nb == kRowBatch) write_rows_t(k0, nb, std::true_type{}); else write_rows_t(k0, nb, std::false_type{});
         };
 
-        // ---- C + D: 32 sorted nodes per step; the node ids of the next two steps are already in flight
+        // ---- C + D: 32 chunks per step, lane = chunk (at most chunk_len consecutive sorted nodes of one (t, c) segment,
+        // cut by the pattern pass): the lane sums the ket harmonics of its nodes in registers, so the K tile holds one
+        // column per chunk and the shared-memory traffic of the segment sums falls by the chunk length.
+        // The chunk words of the next two steps are already in flight.
         double runT[NCH];
 #pragma unroll
         for (int ch = 0; ch < NCH; ++ch) runT[ch] = 0.0;
         double2 runS[NPC];
 #pragma unroll
         for (int i = 0; i < NPC; ++i) runS[i] = make_double2(0.0, 0.0);
-        unsigned kC = 0, kN = 0;                        // this step's and the next step's keys
-        if (lane < we) kC = g_key[lane];
-        if (32 + lane < we) kN = g_key[32 + lane];
-        for (int base = 0; base < we; base += 32) {
-            unsigned kF = 0;
-            if (base + 64 + lane < we) kF = g_key[base + 64 + lane];
-            const bool active = base + lane < we;
-            const int tC = (int)(kC >> 14);
-            int c, a, b;
-            split_node(L, (int)(kC & 16383u), c, a, b);
-            // the node after this one (next lane, or lane 0 of the next step)
-            unsigned k1 = __shfl_down_sync(0xffffffffu, kC, 1);
-            const unsigned k1n = __shfl_sync(0xffffffffu, kN, 0);
-            if (lane == 31) k1 = k1n;
-            const int m1 = (int)(k1 & 16383u);
-            const int c1 = L.mg_npq ? (int)__umulhi((unsigned)m1, L.mg_npq) : m1;
-            // target ends: t changes after this node (or the list ends); segment ends: (t, c) changes
-            const bool tend = active && (base + lane + 1 >= we || (int)(k1 >> 14) != tC);
-            const bool send = active && (tend || c1 != c);
-            const unsigned tmask = __ballot_sync(0xffffffffu, tend), smask = __ballot_sync(0xffffffffu, send);
-            const int cnt = min(32, we - base);
+        uint2 dC = make_uint2(0u, 0u), dN = dC;         // this step's and the next step's chunk words
+        if (lane < nck) dC = g_chunk[lane];
+        if (32 + lane < nck) dN = g_chunk[32 + lane];
+        const unsigned abmask = (1u << nl.ab_bits) - 1u;
+        for (int base = 0; base < nck; base += 32) {
+            uint2 dF = make_uint2(0u, 0u);
+            if (base + 64 + lane < nck) dF = g_chunk[base + 64 + lane];
+            const bool active = base + lane < nck;
+            const int len = active ? (int)((dC.x >> 14) & 15u) + 1 : 0;
+            // segment ends: (t, c) changes behind this chunk; target ends: t changes (or the list ends)
+            const unsigned smask = __ballot_sync(0xffffffffu, (dC.x >> 18) & 1u), tmask = __ballot_sync(0xffffffffu, (dC.x >> 19) & 1u);
+            const int cnt = min(32, nck - base);
+            int tC = 0;                                                     // the target cell, fetched by the chunks that end one
+            if ((dC.x >> 19) & 1u) tC = (int)(g_key[dC.x & 16383u] >> 14);
+            const int c = (int)(dC.x >> 20);                                // the chunk's x-node
+            const int maxlen = __reduce_max_sync(0xffffffffu, len);
             {
-                double p, q, P2, Q2;
-                const double x = s_tx[c];
-                map_node_sq(g, s_tp[a], s_tq[b], x, p, q, P2, Q2);
-                // omega = w * p q / (p' q'),  w = ((hp wp_a)(hq wq_b)) wx_c
-                const double w = __dmul_rn(__dmul_rn(s_wpa[a], s_wqb[b]), s_wx[c]);
-                // (reading B: omega = w * p^2 q^2, no Jacobian of the delta functions)
-                const double om = L.norm ? w * ((p * q) * (p * q)) : w * (p * q) * rsqrt(P2 * Q2);
-                // rotated directions from vector components (frame: q^ = z, p^ = (sx, 0, x)):
-                //   p' = -p/2 - 3q/4 ,  q' = p - q/2
-                const double sx = s_sx[c], psx = p * sx, px = p * x;
-                const double ax = -0.5 * psx, az = fma(-0.5, px, -0.75 * q);
-                const double bx = psx, bz = fma(-0.5, q, px);
-                const double ra = rsqrt(fma(ax, ax, az * az)), rb = rsqrt(fma(bx, bx, bz * bz));
+                double K[Spec::kStatic ? Spec::NS : 1];
                 if constexpr (Spec::kStatic) {
-                    double K[Spec::NS];
-                    Spec::ket(L, om, ax * ra, az * ra, bx * rb, bz * rb, K);
+#pragma unroll
+                    for (int i = 0; i < Spec::NS; ++i) K[i] = 0.0;
+                }
+                // One node of the chunk: omega and the rotated directions.  Branch-free (a lane whose chunk is shorter
+                // runs node 0 again with omega = 0), so the map of node r + 1 can be scheduled into the ket code of node r.
+                struct NodeIn { double om, uxa, uza, uxb, uzb; };
+                auto node_in = [&](unsigned abw, bool valid) {
+                    const int ab = (int)(abw & abmask);
+                    const int a = L.mg_nq ? (int)__umulhi((unsigned)ab, L.mg_nq) : ab, b = ab - a * L.n_q;
+                    const double x = s_tx[c], sx = s_sx[c];
+                    const double p = s_pa[a], q = s_qb[b];                  // cp + hp t_a, cq + hq t_b: the node of DESIGN.md sec. 3.1
+                    double P2, Q2;
+                    map_pq_sq(p, q, x, P2, Q2);
+                    // omega = w * p q / (p' q'),  w = ((hp wp_a)(hq wq_b)) wx_c
+                    const double w = __dmul_rn(__dmul_rn(s_wpa[a], s_wqb[b]), s_wx[c]);
+                    // rotated directions from vector components (frame: q^ = z, p^ = (sx, 0, x)):
+                    //   p' = -p/2 - 3q/4 ,  q' = p - q/2
+                    const double psx = p * sx, px = p * x;
+                    const double ax = -0.5 * psx, az = fma(-0.5, px, -0.75 * q);
+                    const double bx = psx, bz = fma(-0.5, q, px);
+                    const double ra = rsqrt(fma(ax, ax, az * az)), rb = rsqrt(fma(bx, bx, bz * bz));
+                    // (reading B: omega = w * p^2 q^2, no Jacobian of the delta functions)
+                    const double om = L.norm ? w * ((p * q) * (p * q)) : w * (p * q) * rsqrt(P2 * Q2);
+                    return NodeIn{valid ? om : 0.0, ax * ra, az * ra, bx * rb, bz * rb};
+                };
+                unsigned abs_ = dC.y;
+                NodeIn cur = node_in(abs_, 0 < len);
+#pragma unroll 1
+                for (int r = 0; r < maxlen; ++r) {
+                    abs_ >>= nl.ab_bits;
+                    const NodeIn nxt = node_in(abs_, r + 1 < len);
+                    if constexpr (Spec::kStatic) Spec::ket_acc(L, cur.om, cur.uxa, cur.uza, cur.uxb, cur.uzb, K);
+                    else Spec::ket_tile(L, cur.om, cur.uxa, cur.uza, cur.uxb, cur.uzb, s_tile + lane, kTileStride, np, ns, r == 0);
+                    cur = nxt;
+                }
+                if constexpr (Spec::kStatic) {
 #pragma unroll
                     for (int i = 0; i < NP; ++i)
                         s_tile[i * kTileStride + lane] = make_double2(K[2 * i], (2 * i + 1 < Spec::NS) ? K[(2 * i + 1) % Spec::NS] : 0.0);
-                } else {
-                    Spec::ket_tile(L, om, ax * ra, az * ra, bx * rb, bz * rb, s_tile + lane, kTileStride, np, ns);
                 }
             }
             __syncwarp();
@@ -333,13 +356,13 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
 #pragma unroll
                 for (int ch = 0; ch < NCH; ++ch) {
                     if (kPacked) {
-                        const int ia = fa[ch], ib = fb[ch];
+                        const int ia = s_fa[ch * 32 + lane], ib = s_fb[ch * 32 + lane];
                         double v = bra[ia & 255] * s_sseg[ib & 255];
                         v = fma(bra[(ia >> 8) & 255], s_sseg[(ib >> 8) & 255], v);
                         v = fma(bra[ia >> 16], s_sseg[ib >> 16], v);
                         runT[ch] += v;
                     } else {
-                        const int sa = fa[ch] & 65535, sb = fb[ch], nM = fa[ch] >> 16;
+                        const int fav = s_fa[ch * 32 + lane], sa = fav & 65535, sb = s_fb[ch * 32 + lane], nM = fav >> 16;
                         double v = 0.0;
                         for (int i = 0; i < nM; ++i) v = fma(bra[sa + i], s_sseg[sb + i], v);
                         runT[ch] += v;
@@ -366,7 +389,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 }
             }
             __syncwarp();
-            kC = kN; kN = kF;
+            dC = dN; dN = dF;
         }
         if (kcur > kdone) write_rows(kdone, kcur - kdone);
     }

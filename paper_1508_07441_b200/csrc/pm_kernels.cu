@@ -221,7 +221,56 @@ k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl,
                 }
             }
         }
-        if (lane == 0) { nl.hits[cb] = H; nl.ntot[cb] = placed; }
+        // ---- chunks of the sorted list (NodeLists): a chunk ends with its segment or after chunk_len nodes of it.
+        // Lane = sorted position; a position's offset in its segment follows from the last segment start at or before it;
+        // the lane that ends a chunk collects the (a, b) indices of the chunk's nodes from the lanes below it (those of
+        // the previous step when the chunk began there).
+        __syncwarp();
+        int nck = 0;
+        {
+            uint2* g_chunk = nl.chunk + (size_t)cb * L.nnode;
+            const unsigned R = (unsigned)nl.chunk_len, bits = (unsigned)nl.ab_bits;
+            const unsigned npq = (unsigned)(L.n_p * L.n_q);
+            int seg_start = 0;                                  // first position of the segment that is open at the start of a step
+            unsigned carry = 1u;                                // the step's first position starts a segment
+            unsigned ab_prev = 0u;                              // this lane's (a, b) index in the previous step
+            unsigned kn = lane < placed ? g_key[lane] : 0u;     // keys of the next step, fetched one step ahead
+            for (int base = 0; base < placed; base += 32) {
+                const int pos = base + lane;
+                const bool act = pos < placed;
+                const unsigned k = kn;
+                kn = pos + 32 < placed ? g_key[pos + 32] : 0u;
+                unsigned k1 = __shfl_down_sync(0xffffffffu, k, 1);
+                const unsigned k1n = __shfl_sync(0xffffffffu, kn, 0);
+                if (lane == 31) k1 = k1n;
+                const unsigned mk = k & 16383u, m1 = k1 & 16383u;
+                const unsigned ck = L.mg_npq ? __umulhi(mk, L.mg_npq) : mk, c1 = L.mg_npq ? __umulhi(m1, L.mg_npq) : m1;
+                const unsigned ab = mk - ck * npq;
+                const bool tend = act && (pos + 1 >= placed || (k1 >> 14) != (k >> 14));
+                const bool send = act && (tend || c1 != ck);
+                const unsigned smask = __ballot_sync(0xffffffffu, send);
+                const unsigned starts = (smask << 1) | carry;               // positions of this step that start a segment
+                const unsigned below = starts & (0xffffffffu >> (31 - lane));
+                const int start = below ? base + 31 - __clz(below) : seg_start;
+                const unsigned off = (unsigned)(pos - start) % R;           // position in its chunk
+                const bool cend = act && (send || off == R - 1u);
+                const unsigned cmask = __ballot_sync(0xffffffffu, cend);
+                const unsigned maxoff = __reduce_max_sync(0xffffffffu, cend ? off : 0u);
+                unsigned abs_ = ab << (off * bits);                         // (only lanes that end a chunk use it)
+                for (unsigned j = 1; j <= maxoff; ++j) {
+                    const unsigned src = (unsigned)(lane - (int)j) & 31u;
+                    const unsigned va = __shfl_sync(0xffffffffu, ab, src), vb = __shfl_sync(0xffffffffu, ab_prev, src);
+                    if (j <= off) abs_ |= ((unsigned)lane >= j ? va : vb) << ((off - j) * bits);
+                }
+                if (cend) g_chunk[nck + __popc(cmask & lt)] =
+                    make_uint2((unsigned)(pos - (int)off) | (off << 14) | ((unsigned)send << 18) | ((unsigned)tend << 19) | (ck << 20), abs_);
+                nck += __popc(cmask);
+                if (starts) seg_start = base + 31 - __clz(starts);
+                carry = smask >> 31;
+                ab_prev = ab;
+            }
+        }
+        if (lane == 0) { nl.hits[cb] = H; nl.ntot[cb] = placed; nl.nchunk[cb] = nck; }
     }
 }
 
