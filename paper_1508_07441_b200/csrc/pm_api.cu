@@ -274,7 +274,7 @@ int32_t ensure_device(pm_lattice* L)
     for (size_t g = 0; g < all.size(); ++g) {
         const pm::GroupTables& Gt = *all[g];
         pm::DevLattice Dg = D;
-        Dg.n_slot = Gt.n_slot; Dg.n_fun = (int)Gt.fun.size(); Dg.n_out = (int)Gt.o_alpha.size();
+        Dg.n_slot = Gt.n_slot; Dg.n_fun = (int)Gt.fun.size(); Dg.n_out = (int)Gt.o_alpha.size(); Dg.n_out1 = Gt.n_out1; Dg.n_out2 = Gt.n_out2;
         Dg.kt_off = (const int*)(b + go[g].ktoff); Dg.kt_ip = (const int*)(b + go[g].ktip); Dg.kt_iq = (const int*)(b + go[g].ktiq);
         Dg.kt_c = (const double*)(b + go[g].ktc);
         Dg.fun = (const int4*)(b + go[g].fun);
@@ -311,7 +311,9 @@ int32_t ensure_cell_scratch(pm_geometry* G, int n_blk)
         int bits = 1;
         while ((1 << bits) < G->geo.n_p * G->geo.n_q) ++bits;
         G->nl.ab_bits = bits;
-        G->nl.chunk_len = std::max(1, std::min(chunk_len(), 32 / bits));
+        int r = 1;                                      // a power of two, r * bits <= 32
+        while (2 * r <= chunk_len() && 2 * r * bits <= 32) r *= 2;
+        G->nl.chunk_len = r;
     }
     if ((e = cudaMalloc(&G->d_cellbase, sizeof(int64_t) * ((size_t)n_blk + 1))) != cudaSuccess) return cuda_fail(e, "cudaMalloc(cellbase)");
     G->cells_cap = n_blk;

@@ -17,6 +17,7 @@ namespace std {
 template <bool B> struct pm_bool_constant { static constexpr bool value = B; };
 typedef pm_bool_constant<true> true_type;
 typedef pm_bool_constant<false> false_type;
+template <class T, T v> struct integral_constant { static constexpr T value = v; };
 }
 #else
 #include <cstdint>
@@ -31,6 +32,7 @@ struct DevLattice {
     int totcoup, n_slot, n_fun, lmax, ny;       // n_slot / n_fun: ket slots and orbital functions of THIS column-channel group
     int norm;                                   // cell normalisation: 0 reading A (widths), 1 reading B (p^2 dp measure) — DESIGN.md R2
     int n_out, n_bra;                           // outputs (alpha, alpha') of this group; bra slots of the whole channel set
+    int n_out1, n_out2;                         // the group's rows are ordered by the most terms of their outputs: outputs of rows with at most 1 / at most 2
     unsigned mg_npq, mg_nq, mg_Nq;              // ceil(2^32 / d) for d = n_p*n_q, n_q, Nq: exact division of node and cell ids (x*d < 2^32)
     const double *pe, *qe;                      // edges, Np+1 / Nq+1 entries (padded with +inf to pe_pad / qe_pad)
     const double *thr_p, *thr_q;                // sqrt_threshold(edge), padded with +inf to a power of two
@@ -55,8 +57,9 @@ struct DevLattice {
 // Chunks: the sorted list cut into runs of at most chunk_len consecutive nodes that never cross a (target, x-node)
 // segment; one lane of the fill kernel sums the ket harmonics of one chunk in registers (pm_fill.cuh).  A chunk carries
 // the (a, b) indices of its nodes, so the fill reads no node key on its per-node path:
-//   chunk.x = first sorted position | (len - 1) << 14 | ends a segment << 18 | ends a target << 19 | x-node c << 20
+//   chunk.x = target cell | (len - 1) << 18 | ends a segment << 22 | ends a target << 23 | x-node c << 24
 //   chunk.y = ab_0 | ab_1 << ab_bits | ...        (ab = a*n_q + b < 2^ab_bits, len * ab_bits <= 32)
+// (cell < 2^18, len <= 16, c < PM_MAX_ORDER = 64)
 struct NodeLists {
     unsigned* key;              // [n_blk][nnode]
     int* ntot;                  // [n_blk] nodes on the grid

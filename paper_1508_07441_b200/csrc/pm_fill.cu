@@ -79,8 +79,8 @@ cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int n_sm, Fi
     const int want = preferred_warps();
     const FillVariant* best = nullptr;          // largest warp count <= want whose shared memory fits, else the smallest that fits
     auto plan_of = [&](const FillVariant& v) {         // the bra table moves to global memory when it does not fit beside the tiles
-        FillSmem s = fill_smem_plan(L, v.nw, v.rb, true);
-        if (s.total > kSmemLimit && v.hash == 0ull) s = fill_smem_plan(L, v.nw, v.rb, false);
+        FillSmem s = fill_smem_plan(L, v.nw, v.rb, true, v.hash == 0ull);
+        if (s.total > kSmemLimit && v.hash == 0ull) s = fill_smem_plan(L, v.nw, v.rb, false, true);
         return s;
     };
     for (const FillVariant& v : kVariants) {

@@ -55,7 +55,7 @@ struct SpecGeneric {
 };
 
 struct FillSmem {           // byte offsets into dynamic shared memory, computed on the host
-    int dp, dq, tx, sx, wx, bra, odesc, ofi, oc, fa, fb, warp0, warp_bytes, w_tile, w_sseg, w_acc, w_norm, w_hcol, w_wpa, w_wqb, w_pa, w_qb, total;
+    int tx, sx, wx, bra, odesc, ofi, oc, fa, fb, warp0, warp_bytes, w_tile, w_sseg, w_acc, w_hcol, w_wpa, w_wqb, w_pa, w_qb, w_ring, w_cell, total;
 };
 
 constexpr int kTileStride = 33;        // double2 per K-tile row: 32 nodes + 1 pad (conflict-free rows and columns)
@@ -63,29 +63,36 @@ constexpr int kTileStride = 33;        // double2 per K-tile row: 32 nodes + 1 p
 inline int fill_align16(int b) { return (b + 15) & ~15; }
 
 // shared-memory plan for nw warps: tables shared by the CTA, then one private area per warp
-inline FillSmem fill_smem_plan(const DevLattice& L, int nw, int row_batch, bool bra_in_smem = true)
+inline FillSmem fill_smem_plan(const DevLattice& L, int nw, int row_batch, bool bra_in_smem = true, bool generic = false)
 {
+    const int nfun_pad = generic ? kFillMaxFun : (L.n_fun + 31) & ~31;     // NCH * 32 of the kernel that runs
     FillSmem s{};
     int o = 0;
     auto take = [&](int bytes) { int r = o; o += fill_align16(bytes); return r; };
-    s.dp = take(8 * L.Np); s.dq = take(8 * L.Nq);
     s.tx = take(8 * L.n_x); s.sx = take(8 * L.n_x); s.wx = take(8 * L.n_x);
     s.bra = bra_in_smem ? take(8 * L.n_x * (L.n_bra + 1)) : -1;      // rows padded with one zero slot; -1: read from global memory
     s.odesc = take(4 * L.n_out); s.ofi = take(4 * L.n_out); s.oc = take(24 * L.n_out);
-    s.fa = take(4 * kFillMaxFun); s.fb = take(4 * kFillMaxFun);        // (every function chunk of the stage reads its entry)
+    s.fa = take(4 * nfun_pad); s.fb = take(4 * nfun_pad);             // (every function chunk of the stage reads its entry)
     const int np = (L.n_slot + 1) / 2;              // slot pairs
     int w = 0;
     auto wtake = [&](int bytes) { int r = w; w += fill_align16(bytes); return r; };
     s.w_tile = wtake(16 * kTileStride * np);
     s.w_sseg = wtake(16 * np);
     s.w_acc = wtake(8 * L.n_fun * row_batch);      // sums of finished targets waiting for their rows to be written
-    s.w_norm = wtake(8 * row_batch);
     s.w_hcol = wtake(4 * row_batch);
     s.w_wpa = wtake(8 * L.n_p); s.w_wqb = wtake(8 * L.n_q); s.w_pa = wtake(8 * L.n_p); s.w_qb = wtake(8 * L.n_q);
+    s.w_ring = wtake(2 * 32 * 8); s.w_cell = wtake(32);
     s.warp_bytes = w;
     s.warp0 = take(w * nw);
     s.total = o;
     return s;
+}
+
+// cell norm B_k: width (reading A) or (e_{k+1}^3 - e_k^3)/3 (reading B, states normalised in the p^2 dp measure)
+__device__ __forceinline__ double cell_norm(const double* __restrict__ e, int k, int norm)
+{
+    const double e0 = e[k], e1 = e[k + 1];
+    return norm ? (e1 * e1 * e1 - e0 * e0 * e0) / 3.0 : e1 - e0;
 }
 
 template <class Spec, int NW, int kRowBatch, bool kCols>
@@ -104,7 +111,6 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int ns = Spec::kStatic ? Spec::NS : L.n_slot, nf = Spec::kStatic ? Spec::NF : L.n_fun, np = (ns + 1) >> 1;
 
-    double* s_dp = (double*)(smem + S.dp);   double* s_dq = (double*)(smem + S.dq);
     double* s_tx = (double*)(smem + S.tx);
     double* s_sx = (double*)(smem + S.sx);   double* s_wx = (double*)(smem + S.wx);
     double* s_bra = (double*)(smem + (S.bra >= 0 ? S.bra : 0));
@@ -116,17 +122,16 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
     double2* s_sseg2 = (double2*)(wsm + S.w_sseg);
     const double* s_sseg = (const double*)s_sseg2;
     double* s_acc = (double*)(wsm + S.w_acc);         // [kRowBatch][nf] sums of finished targets
-    double* s_norm = (double*)(wsm + S.w_norm);
     int* s_hcol = (int*)(wsm + S.w_hcol);               // first column of each finished target: cell * n_ch (kCols)
     double* s_wpa = (double*)(wsm + S.w_wpa);
     double* s_wqb = (double*)(wsm + S.w_wqb);
     double* s_pa = (double*)(wsm + S.w_pa);
     double* s_qb = (double*)(wsm + S.w_qb);
+    uint2* s_ring = (uint2*)(wsm + S.w_ring);           // chunk words of two steps
+    struct CellInfo { int64_t rbase; double dsrc; int H; };
+    CellInfo* s_cell = (CellInfo*)(wsm + S.w_cell);
 
     // ---- once per CTA: widths, rules, bra harmonics, output descriptors
-    // cell norms B_k: widths (reading A) or (e_{k+1}^3 - e_k^3)/3 (reading B, states normalised in the p^2 dp measure)
-    for (int k = tid; k < L.Np; k += T) { const double e0 = L.pe[k], e1 = L.pe[k + 1]; s_dp[k] = L.norm ? (e1 * e1 * e1 - e0 * e0 * e0) / 3.0 : e1 - e0; }
-    for (int k = tid; k < L.Nq; k += T) { const double e0 = L.qe[k], e1 = L.qe[k + 1]; s_dq[k] = L.norm ? (e1 * e1 * e1 - e0 * e0 * e0) / 3.0 : e1 - e0; }
     for (int k = tid; k < L.n_x; k += T) { s_tx[k] = L.tx[k]; s_sx[k] = L.sx[k]; s_wx[k] = L.wx[k]; }
     const int nb_ = Spec::kStatic ? Spec::NS : L.n_bra; // bra slots (the whole channel set's)
     const int nsb = nb_ + 1;                            // shared-memory bra rows carry one trailing zero slot (index nb_)
@@ -175,12 +180,9 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         const int cell = cell_begin + cb;
         const int ci = cell / L.Nq, cj = cell - ci * L.Nq;
         const int H = nl.hits[cb], nck = nl.nchunk[cb];
-        const unsigned* __restrict__ g_key = nl.key + (size_t)cb * L.nnode;       // target cell << 14 | node id
         const uint2* __restrict__ g_chunk = nl.chunk + (size_t)cb * L.nnode;      // NodeLists (pm_device.cuh)
-        const int64_t rbase = rowptr[(int64_t)cb * L.n_ch];
-        double* __restrict__ row0 = vals + rbase;
-        int32_t* __restrict__ col0 = kCols ? colidx + rbase : nullptr;
-        const double dsrc = s_dp[ci] * s_dq[cj];
+        // what only the row phase and the target ends need of the cell waits in shared memory (registers are the limit here)
+        if (lane == 0) { s_cell->rbase = rowptr[(int64_t)cb * L.n_ch]; s_cell->dsrc = cell_norm(L.pe, ci, L.norm) * cell_norm(L.qe, cj, L.norm); s_cell->H = H; }
         {   // the cell's nodes p_a = cp + hp t_a, q_b = cq + hq t_b (the operations of map_node_sq) and weights hp wp_a, hq wq_b
             const CellGeom g = cell_geom(L.pe, L.qe, ci, cj);
             for (int k = lane; k < L.n_p; k += 32) { s_wpa[k] = __dmul_rn(g.hp, L.wp[k]); s_pa[k] = __dadd_rn(g.cp, __dmul_rn(g.hp, L.tp[k])); }
@@ -189,36 +191,54 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         __syncwarp();
         int kcur = 0, kdone = 0;                        // targets finished / written; a target's rank is its position in every row
         // ---- E: lane = output (alpha, m-th coupled alpha'): P = norm_t * sum_L c^L acc_t[f] for targets k0 .. k0+nb-1
+        // The rows are ordered by the most terms of their outputs (pm_tables.cpp): a 32-output step inside the one-term
+        // (two-term) rows loads one (two) sums per target.  The cell normalisation is already in the sums (target end, below).
         auto write_rows_t = [&](int k0, int nb, auto full_tag) {
             constexpr bool kFull = decltype(full_tag)::value;           // all kRowBatch slots hold a target
-            double nrm[kRowBatch];
             int hcl[kRowBatch];
 #pragma unroll
-            for (int bb = 0; bb < kRowBatch; ++bb) { nrm[bb] = s_norm[bb]; hcl[bb] = kCols ? s_hcol[bb] : 0; }
+            for (int bb = 0; bb < kRowBatch; ++bb) hcl[bb] = kCols ? s_hcol[bb] : 0;
+            const int64_t rbase = s_cell->rbase;
+            double* __restrict__ row0 = vals + rbase;
+            int32_t* __restrict__ col0 = kCols ? colidx + rbase : nullptr;
+            const int Hc = s_cell->H;
+            auto outputs = [&](int o_begin, int o_end, auto nt_tag) {
+                constexpr int NT = decltype(nt_tag)::value;
 #pragma unroll 2
-            for (int o = lane; o < L.n_out; o += 32) {
-                const int od = s_odesc[o], fi = s_ofi[o];
-                const int clo = od & 4095, nc = (od >> 12) & 127, mm = (od >> 19) & 63, ap = (unsigned)od >> 25;
-                const double c0 = s_oc[3 * o], c1 = s_oc[3 * o + 1], c2 = s_oc[3 * o + 2];
-                const int f0 = fi & 1023, f1 = (fi >> 10) & 1023, f2 = (fi >> 20) & 1023;
-                // entry of target k0+bb in row alpha: element H*clo + (k0+bb)*nc + m of the cell's block (fits 32 bits)
-                const unsigned idx0 = (unsigned)(H * clo + k0 * nc + mm);
-                const char* acc0 = (const char*)s_acc;
-                const unsigned a0 = 8u * f0, a1 = 8u * f1, a2 = 8u * f2;
+                for (int o = o_begin + lane; o < o_end; o += 32) {
+                    const int od = s_odesc[o], fi = s_ofi[o];
+                    const int clo = od & 4095, nc = (od >> 12) & 127, mm = (od >> 19) & 63, ap = (unsigned)od >> 25;
+                    const double c0 = s_oc[3 * o], c1 = NT > 1 ? s_oc[3 * o + 1] : 0.0, c2 = NT > 2 ? s_oc[3 * o + 2] : 0.0;
+                    const int f0 = fi & 1023, f1 = (fi >> 10) & 1023, f2 = (fi >> 20) & 1023;
+                    // entry of target k0+bb in row alpha: element H*clo + (k0+bb)*nc + m of the cell's block (fits 32 bits)
+                    const unsigned idx0 = (unsigned)(Hc * clo + k0 * nc + mm);
+                    const char* acc0 = (const char*)s_acc;
+                    const unsigned a0 = 8u * f0, a1 = 8u * f1, a2 = 8u * f2;
 #pragma unroll
-                for (int bb = 0; bb < kRowBatch; ++bb) {
-                    if (kFull || bb < nb) {
-                        const char* acc = acc0 + bb * (8 * nf);
-                        double v = fma(c2, *(const double*)(acc + a2), fma(c1, *(const double*)(acc + a1), c0 * *(const double*)(acc + a0)));
-                        if (Spec::MAXL1 > 3) {                           // more than three L values: the tail comes from the tables
-                            const int t0 = L.ot_off[o], nt = (int)((unsigned)fi >> 30) + 1;
-                            for (int t = 3; t < nt; ++t) v = fma(L.ot_c[t0 + t], ((const double*)acc)[L.ot_f[t0 + t]], v);
+                    for (int bb = 0; bb < kRowBatch; ++bb) {
+                        if (kFull || bb < nb) {
+                            const char* acc = acc0 + bb * (8 * nf);
+                            double v = c0 * *(const double*)(acc + a0);
+                            if (NT > 1) v = fma(c1, *(const double*)(acc + a1), v);
+                            if (NT > 2) v = fma(c2, *(const double*)(acc + a2), v);
+                            if (Spec::MAXL1 > 3) {                       // more than three L values: the tail comes from the tables
+                                const int t0 = L.ot_off[o], nt = (int)((unsigned)fi >> 30) + 1;
+                                for (int t = 3; t < nt; ++t) v = fma(L.ot_c[t0 + t], ((const double*)acc)[L.ot_f[t0 + t]], v);
+                            }
+                            const unsigned e = idx0 + (unsigned)(bb * nc);
+                            row0[e] = v;
+                            if (kCols) col0[e] = hcl[bb] + ap;
                         }
-                        const unsigned e = idx0 + (unsigned)(bb * nc);
-                        row0[e] = v * nrm[bb];
-                        if (kCols) col0[e] = hcl[bb] + ap;
                     }
                 }
+            };
+            if constexpr (kFull) {
+                const int e1 = L.n_out1 & ~31, e2 = max(e1, L.n_out2 & ~31);
+                outputs(0, e1, std::integral_constant<int, 1>{});
+                outputs(e1, e2, std::integral_constant<int, 2>{});
+                outputs(e2, L.n_out, std::integral_constant<int, 3>{});
+            } else {
+                outputs(0, L.n_out, std::integral_constant<int, 3>{});
             }
             __syncwarp();
         };
@@ -236,21 +256,26 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         double2 runS[NPC];
 #pragma unroll
         for (int i = 0; i < NPC; ++i) runS[i] = make_double2(0.0, 0.0);
-        uint2 dC = make_uint2(0u, 0u), dN = dC;         // this step's and the next step's chunk words
-        if (lane < nck) dC = g_chunk[lane];
-        if (32 + lane < nck) dN = g_chunk[32 + lane];
+        // The chunk words travel global -> shared memory by cp.async into a per-warp ring of two steps (the words of step
+        // s + 2 are requested when step s is finished): no register holds a word in flight across the ket code, and the
+        // step's own words stay readable for the segment and target ends behind it.
+        const unsigned ring = (unsigned)__cvta_generic_to_shared(s_ring) + 8u * lane;
+        auto fetch = [&](int step, int slot) {          // chunk word of this lane in step `step` -> ring slot `slot`
+            const int k = step * 32 + lane;
+            if (k < nck) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(ring + 256u * slot), "l"(g_chunk + k) : "memory");
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        };
+        fetch(0, 0);
+        fetch(1, 1);
         const unsigned abmask = (1u << nl.ab_bits) - 1u;
         for (int base = 0; base < nck; base += 32) {
-            uint2 dF = make_uint2(0u, 0u);
-            if (base + 64 + lane < nck) dF = g_chunk[base + 64 + lane];
-            const bool active = base + lane < nck;
-            const int len = active ? (int)((dC.x >> 14) & 15u) + 1 : 0;
-            // segment ends: (t, c) changes behind this chunk; target ends: t changes (or the list ends)
-            const unsigned smask = __ballot_sync(0xffffffffu, (dC.x >> 18) & 1u), tmask = __ballot_sync(0xffffffffu, (dC.x >> 19) & 1u);
-            const int cnt = min(32, nck - base);
-            int tC = 0;                                                     // the target cell, fetched by the chunks that end one
-            if ((dC.x >> 19) & 1u) tC = (int)(g_key[dC.x & 16383u] >> 14);
-            const int c = (int)(dC.x >> 20);                                // the chunk's x-node
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+            uint2* s_step = s_ring + (base & 32);                           // this step's chunk words
+            if (base + lane >= nck) s_step[lane] = make_uint2(0u, 0u);      // (a lane without a chunk)
+            __syncwarp();
+            const uint2 dC = s_step[lane];
+            const int len = base + lane < nck ? (int)((dC.x >> 18) & 15u) + 1 : 0;
+            const int c = (int)(dC.x >> 24);                                // the chunk's x-node
             const int maxlen = __reduce_max_sync(0xffffffffu, len);
             {
                 double K[Spec::kStatic ? Spec::NS : 1];
@@ -297,6 +322,10 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 }
             }
             __syncwarp();
+            // segment ends: (t, c) changes behind a chunk; target ends: t changes (or the list ends)
+            const unsigned dx = s_step[lane].x;
+            const unsigned smask = __ballot_sync(0xffffffffu, (dx >> 22) & 1u), tmask = __ballot_sync(0xffffffffu, (dx >> 23) & 1u);
+            const int cnt = min(32, nck - base);
             // lane = slot pair: walks the tile's nodes, up to 16 per step, stopping at every segment end (and at the tile end)
             const unsigned stops = smask | (1u << (cnt - 1));
             for (int j = 0; j < cnt;) {
@@ -350,7 +379,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                     runS[i] = make_double2(0.0, 0.0);
                 }
                 __syncwarp();
-                const int cseg = __shfl_sync(0xffffffffu, c, jb);
+                const int cseg = (int)(s_step[jb].x >> 24);
                 const double* bra;                                     // (shared-memory loads for the specialised kernels)
                 if constexpr (Spec::kStatic) bra = s_bra + cseg * nsb; else bra = bra_tab + cseg * bra_stride;
 #pragma unroll
@@ -373,23 +402,24 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 // node jb also ends target t: its sums are complete; kRowBatch finished targets are written together
                 {
                     const int slot = kcur - kdone;
+                    const int tcell = (int)(s_step[jb].x & 262143u);
+                    const int ic = L.mg_Nq ? (int)__umulhi((unsigned)tcell, L.mg_Nq) : tcell, jc = tcell - ic * L.Nq;
+                    // (d_i dbar_j d_i' dbar_j')^(-1/2), folded into the sums; rsqrt is within 2 ulp of the oracle's 1/sqrt
+                    const double nrm = rsqrt(s_cell->dsrc * (cell_norm(L.pe, ic, L.norm) * cell_norm(L.qe, jc, L.norm)));
 #pragma unroll
                     for (int ch = 0; ch < NCH; ++ch) {
                         const int f = ch * 32 + lane;
-                        if (f < nf) s_acc[slot * nf + f] = runT[ch];
+                        if (f < nf) s_acc[slot * nf + f] = runT[ch] * nrm;
                         runT[ch] = 0.0;
                     }
-                    const int tcell = __shfl_sync(0xffffffffu, tC, jb);
-                    const int ic = L.mg_Nq ? (int)__umulhi((unsigned)tcell, L.mg_Nq) : tcell, jc = tcell - ic * L.Nq;
-                    // (d_i dbar_j d_i' dbar_j')^(-1/2); rsqrt is within 2 ulp of the oracle's 1/sqrt
-                    if (lane == 0) { s_norm[slot] = rsqrt(dsrc * (s_dp[ic] * s_dq[jc])); s_hcol[slot] = tcell * L.n_ch; }
+                    if (lane == 0) s_hcol[slot] = tcell * L.n_ch;
                     ++kcur;
                     __syncwarp();
                     if (kcur - kdone == kRowBatch) { write_rows(kdone, kRowBatch); kdone = kcur; }
                 }
             }
             __syncwarp();
-            dC = dN; dN = dF;
+            fetch((base >> 5) + 2, (base >> 5) & 1);
         }
         if (kcur > kdone) write_rows(kdone, kcur - kdone);
     }

@@ -229,11 +229,11 @@ k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl,
         int nck = 0;
         {
             uint2* g_chunk = nl.chunk + (size_t)cb * L.nnode;
-            const unsigned R = (unsigned)nl.chunk_len, bits = (unsigned)nl.ab_bits;
+            const unsigned R = (unsigned)nl.chunk_len, bits = (unsigned)nl.ab_bits;      // R: a power of two, R * bits <= 32
             const unsigned npq = (unsigned)(L.n_p * L.n_q);
             int seg_start = 0;                                  // first position of the segment that is open at the start of a step
             unsigned carry = 1u;                                // the step's first position starts a segment
-            unsigned ab_prev = 0u;                              // this lane's (a, b) index in the previous step
+            unsigned prev[4] = {0u, 0u, 0u, 0u};                // the previous step's packed indices, level by level
             unsigned kn = lane < placed ? g_key[lane] : 0u;     // keys of the next step, fetched one step ahead
             for (int base = 0; base < placed; base += 32) {
                 const int pos = base + lane;
@@ -245,29 +245,33 @@ k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl,
                 if (lane == 31) k1 = k1n;
                 const unsigned mk = k & 16383u, m1 = k1 & 16383u;
                 const unsigned ck = L.mg_npq ? __umulhi(mk, L.mg_npq) : mk, c1 = L.mg_npq ? __umulhi(m1, L.mg_npq) : m1;
-                const unsigned ab = mk - ck * npq;
                 const bool tend = act && (pos + 1 >= placed || (k1 >> 14) != (k >> 14));
                 const bool send = act && (tend || c1 != ck);
                 const unsigned smask = __ballot_sync(0xffffffffu, send);
                 const unsigned starts = (smask << 1) | carry;               // positions of this step that start a segment
                 const unsigned below = starts & (0xffffffffu >> (31 - lane));
                 const int start = below ? base + 31 - __clz(below) : seg_start;
-                const unsigned off = (unsigned)(pos - start) % R;           // position in its chunk
+                const unsigned off = (unsigned)(pos - start) & (R - 1u);    // position in its chunk
                 const bool cend = act && (send || off == R - 1u);
                 const unsigned cmask = __ballot_sync(0xffffffffu, cend);
-                const unsigned maxoff = __reduce_max_sync(0xffffffffu, cend ? off : 0u);
-                unsigned abs_ = ab << (off * bits);                         // (only lanes that end a chunk use it)
-                for (unsigned j = 1; j <= maxoff; ++j) {
-                    const unsigned src = (unsigned)(lane - (int)j) & 31u;
-                    const unsigned va = __shfl_sync(0xffffffffu, ab, src), vb = __shfl_sync(0xffffffffu, ab_prev, src);
-                    if (j <= off) abs_ |= ((unsigned)lane >= j ? va : vb) << ((off - j) * bits);
+                // v = the (a, b) indices of the R positions that end here, oldest in the low bits (doubling: 1, 2, 4, ... positions)
+                unsigned v = mk - ck * npq;
+#pragma unroll
+                for (int lv = 0; lv < 4; ++lv) {
+                    const unsigned d = 1u << lv;
+                    if (d < R) {
+                        const unsigned src = (unsigned)(lane - (int)d) & 31u;
+                        const unsigned va = __shfl_sync(0xffffffffu, v, src), vb = __shfl_sync(0xffffffffu, prev[lv], src);
+                        prev[lv] = v;
+                        v = ((unsigned)lane >= d ? va : vb) | (v << (d * bits));
+                    }
                 }
                 if (cend) g_chunk[nck + __popc(cmask & lt)] =
-                    make_uint2((unsigned)(pos - (int)off) | (off << 14) | ((unsigned)send << 18) | ((unsigned)tend << 19) | (ck << 20), abs_);
+                    make_uint2((k >> 14) | (off << 18) | ((unsigned)send << 22) | ((unsigned)tend << 23) | (ck << 24),
+                               v >> ((R - 1u - off) * bits));
                 nck += __popc(cmask);
                 if (starts) seg_start = base + 31 - __clz(starts);
                 carry = smask >> 31;
-                ab_prev = ab;
             }
         }
         if (lane == 0) { nl.hits[cb] = H; nl.ntot[cb] = placed; nl.nchunk[cb] = nck; }

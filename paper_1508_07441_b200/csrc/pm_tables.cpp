@@ -349,6 +349,31 @@ void build_groups(const Tables& T, const pm_channel* ch, int max_slot, int max_f
             }
             G.ot_off.push_back((int32_t)G.ot_f.size());
         }
+    // Whole rows (all outputs of one alpha, which the fill stores as one contiguous run per target) ordered by the largest
+    // number of terms any of their outputs has (stable), so that the fill kernel's 32-output steps over the one-term
+    // (two-term) rows load no padded terms while every store still covers consecutive entries of a row.
+    for (GroupTables& G : groups) {
+        const int n = (int)G.o_alpha.size();
+        std::vector<int> ord((size_t)n);
+        for (int o = 0; o < n; ++o) ord[(size_t)o] = o;
+        auto nt = [&](int o) { return G.ot_off[(size_t)o + 1] - G.ot_off[(size_t)o]; };
+        std::map<int, int> row_nt;                                     // alpha -> most terms of its outputs in this group
+        for (int o = 0; o < n; ++o) row_nt[G.o_alpha[(size_t)o]] = std::max(row_nt[G.o_alpha[(size_t)o]], nt(o));
+        std::stable_sort(ord.begin(), ord.end(), [&](int x, int y) { return row_nt[G.o_alpha[(size_t)x]] < row_nt[G.o_alpha[(size_t)y]]; });
+        GroupTables R = G;
+        R.ot_off.assign(1, 0); R.ot_f.clear(); R.ot_c.clear();
+        G.n_out1 = G.n_out2 = 0;
+        for (int i = 0; i < n; ++i) {
+            const int o = ord[(size_t)i];
+            R.o_alpha[(size_t)i] = G.o_alpha[(size_t)o]; R.o_m[(size_t)i] = G.o_m[(size_t)o]; R.o_ap[(size_t)i] = G.o_ap[(size_t)o];
+            for (int k = G.ot_off[(size_t)o]; k < G.ot_off[(size_t)o + 1]; ++k) { R.ot_f.push_back(G.ot_f[(size_t)k]); R.ot_c.push_back(G.ot_c[(size_t)k]); }
+            R.ot_off.push_back((int32_t)R.ot_f.size());
+            if (row_nt[G.o_alpha[(size_t)o]] <= 1) ++G.n_out1;
+            if (row_nt[G.o_alpha[(size_t)o]] <= 2) ++G.n_out2;
+        }
+        R.n_out1 = G.n_out1; R.n_out2 = G.n_out2;
+        G = R;
+    }
 }
 
 void build_bra(const Tables& T, const std::vector<double>& tx, std::vector<double>& bra)

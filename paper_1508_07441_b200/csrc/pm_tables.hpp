@@ -49,7 +49,9 @@ struct GroupTables {
     std::vector<int32_t> kt_off, kt_ip, kt_iq;        // ket terms per local slot
     std::vector<double> kt_c;
     std::vector<OrbFun> fun;                          // sa0: GLOBAL bra slot, sb0: LOCAL ket slot
-    std::vector<int32_t> o_alpha, o_m, o_ap;          // outputs: row channel, position in the row's coupled list, column channel
+    std::vector<int32_t> o_alpha, o_m, o_ap;          // outputs: row channel, position in the row's coupled list, column channel;
+                                                      // rows ordered by the most terms of their outputs
+    int n_out1 = 0, n_out2 = 0;                       // outputs in rows with at most one / at most two terms per output
     std::vector<int32_t> ot_off, ot_f;                // terms per output, f numbered locally
     std::vector<double> ot_c;
 };
