@@ -310,7 +310,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
 #pragma unroll 1
                 for (int r = 0; r < maxlen; ++r) {
                     abs_ >>= nl.ab_bits;
-                    const NodeIn nxt = node_in(abs_, r + 1 < len);
+                    const NodeIn nxt = node_in(abs_, r + 1 < len);      // (peeling the last iteration doubles the ket code: slower)
                     if constexpr (Spec::kStatic) Spec::ket_acc(L, cur.om, cur.uxa, cur.uza, cur.uxb, cur.uzb, K);
                     else Spec::ket_tile(L, cur.om, cur.uxa, cur.uza, cur.uxb, cur.uzb, s_tile + lane, kTileStride, np, ns, r == 0);
                     cur = nxt;

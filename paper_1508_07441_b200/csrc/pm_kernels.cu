@@ -234,19 +234,27 @@ k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl,
             int seg_start = 0;                                  // first position of the segment that is open at the start of a step
             unsigned carry = 1u;                                // the step's first position starts a segment
             unsigned prev[4] = {0u, 0u, 0u, 0u};                // the previous step's packed indices, level by level
-            unsigned kn = lane < placed ? g_key[lane] : 0u;     // keys of the next step, fetched one step ahead
+            // keys of this step and of the next two (the last position's successor is the next step's first key, so the
+            // loads run two steps ahead of their use)
+            unsigned k = lane < placed ? g_key[lane] : 0u, kn = 32 + lane < placed ? g_key[32 + lane] : 0u;
             for (int base = 0; base < placed; base += 32) {
                 const int pos = base + lane;
                 const bool act = pos < placed;
-                const unsigned k = kn;
-                kn = pos + 32 < placed ? g_key[pos + 32] : 0u;
+                const unsigned knn = pos + 64 < placed ? g_key[pos + 64] : 0u;
                 unsigned k1 = __shfl_down_sync(0xffffffffu, k, 1);
                 const unsigned k1n = __shfl_sync(0xffffffffu, kn, 0);
                 if (lane == 31) k1 = k1n;
-                const unsigned mk = k & 16383u, m1 = k1 & 16383u;
-                const unsigned ck = L.mg_npq ? __umulhi(mk, L.mg_npq) : mk, c1 = L.mg_npq ? __umulhi(m1, L.mg_npq) : m1;
+                // (target, x-node) of a position = key with the (a, b) part removed: tc = t << 14 | c * npq
+                const unsigned mk = k & 16383u;
+                const unsigned ck = L.mg_npq ? __umulhi(mk, L.mg_npq) : mk;
+                const unsigned ab = mk - ck * npq, tc = k - ab;
+                unsigned tc1 = __shfl_down_sync(0xffffffffu, tc, 1);
+                {   // lane 31's successor: the next step's first position
+                    const unsigned mn = k1n & 16383u, cn = L.mg_npq ? __umulhi(mn, L.mg_npq) : mn;
+                    if (lane == 31) tc1 = k1n - (mn - cn * npq);
+                }
                 const bool tend = act && (pos + 1 >= placed || (k1 >> 14) != (k >> 14));
-                const bool send = act && (tend || c1 != ck);
+                const bool send = act && (tend || tc1 != tc);
                 const unsigned smask = __ballot_sync(0xffffffffu, send);
                 const unsigned starts = (smask << 1) | carry;               // positions of this step that start a segment
                 const unsigned below = starts & (0xffffffffu >> (31 - lane));
@@ -255,7 +263,7 @@ k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl,
                 const bool cend = act && (send || off == R - 1u);
                 const unsigned cmask = __ballot_sync(0xffffffffu, cend);
                 // v = the (a, b) indices of the R positions that end here, oldest in the low bits (doubling: 1, 2, 4, ... positions)
-                unsigned v = mk - ck * npq;
+                unsigned v = ab;
 #pragma unroll
                 for (int lv = 0; lv < 4; ++lv) {
                     const unsigned d = 1u << lv;
@@ -272,6 +280,7 @@ k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl,
                 nck += __popc(cmask);
                 if (starts) seg_start = base + 31 - __clz(starts);
                 carry = smask >> 31;
+                k = kn; kn = knn;
             }
         }
         if (lane == 0) { nl.hits[cb] = H; nl.ntot[cb] = placed; nl.nchunk[cb] = nck; }
