@@ -59,6 +59,15 @@ std::string emit_spec(const std::string& name, const Tables& T, EmitStats& st)
     int maxm = 1, maxl1 = 1;                        // most M-terms of a function; number of L values (terms per output)
     for (const OrbFun& f : T.fun) { maxm = std::max(maxm, f.nM); maxl1 = std::max(maxl1, f.L + 1); }
     o << "    static constexpr int NS = " << T.n_slot << ", NF = " << nf << ", NCH = " << (nf + 31) / 32 << ", MAXM = " << maxm << ", MAXL1 = " << maxl1 << ";\n";
+    o << "    // most M-terms of the 32 functions step ch of the stage handles\n"
+         "    static __device__ __forceinline__ constexpr int terms(int ch) { return ";
+    for (int c = 0; c < (nf + 31) / 32; ++c) {
+        int m = 1;
+        for (int f = 32 * c; f < std::min(nf, 32 * c + 32); ++f) m = std::max(m, T.fun[(size_t)f].nM);
+        if (c + 1 < (nf + 31) / 32) o << "ch == " << c << " ? " << m << " : ";
+        else o << m;
+    }
+    o << "; }\n";
     char hb[32]; std::snprintf(hb, sizeof hb, "0x%016" PRIx64 "ull", tables_hash(T));
     o << "    static constexpr unsigned long long kHash = " << hb << ";\n";
     o << "    // K[s] += omega * (ket bipolar harmonic of slot s) at directions a = p'^ = (uxa,0,uza), b = q'^ = (uxb,0,uzb)\n";

@@ -30,6 +30,7 @@ struct SpecGeneric {
     static constexpr bool kStatic = false;
     static constexpr int NS = kFillMaxSlot, NF = kFillMaxFun, NCH = kFillMaxFun / 32, MAXM = 99, MAXL1 = 99;
     static constexpr unsigned long long kHash = 0ull;
+    static __device__ __forceinline__ constexpr int terms(int) { return 3; }      // (unused: MAXM > 3 loops over the function's own terms)
     // writes the node's column of the K tile directly (no per-thread K array): col = tile + lane, np slot pairs
     static __device__ __noinline__ void ket_tile(const DevLattice& L, double om, double uxa, double uza, double uxb, double uzb,
                                                  double2* __restrict__ col, int stride, int np, int ns, bool first)
@@ -54,13 +55,36 @@ struct SpecGeneric {
     }
 };
 
-struct FillSmem {           // byte offsets into dynamic shared memory, computed on the host
-    int tx, sx, wx, bra, odesc, ofi, oc, fa, fb, warp0, warp_bytes, w_tile, w_sseg, w_acc, w_hcol, w_wpa, w_wqb, w_pa, w_qb, w_ring, w_cell, total;
-};
 
 constexpr int kTileStride = 33;        // double2 per K-tile row: 32 nodes + 1 pad (conflict-free rows and columns)
 
+// Private shared-memory area of one warp, byte offsets: everything whose size follows from (slot pairs, functions, row
+// batch) first, so that a specialised kernel addresses it with compile-time offsets from ONE base register (the kernel
+// runs at the register limit); the per-cell node tables (sizes n_p, n_q) come last.
+struct WarpLayout { int tile, sseg, acc, hcol, ring, cell, p2, fixed_bytes; };
+__host__ __device__ constexpr int fill_al16(int b) { return (b + 15) & ~15; }
+__host__ __device__ constexpr WarpLayout warp_layout(int np, int nf, int row_batch)
+{
+    WarpLayout w{};
+    int o = 0;
+    w.tile = o; o += fill_al16(16 * kTileStride * np);
+    w.sseg = o; o += fill_al16(16 * np);
+    w.acc = o;  o += fill_al16(8 * nf * row_batch);      // sums of finished targets waiting for their rows to be written
+    w.hcol = o; o += fill_al16(4 * row_batch);
+    w.ring = o; o += 2 * 32 * 8;                         // chunk words of two steps
+    w.cell = o; o += 32;
+    w.p2 = o;                                            // double2 (p_a, hp wp_a) [n_p], then (q_b, hq wq_b) [n_q]
+    w.fixed_bytes = o;
+    return w;
+}
+
+struct FillSmem {           // byte offsets into dynamic shared memory, computed on the host
+    int dp, dq, tx, sx, wx, bra, odesc, ofi, oc, fa, fb, warp0, warp_bytes, total;
+    WarpLayout w;
+};
+
 inline int fill_align16(int b) { return (b + 15) & ~15; }
+
 
 // shared-memory plan for nw warps: tables shared by the CTA, then one private area per warp
 inline FillSmem fill_smem_plan(const DevLattice& L, int nw, int row_batch, bool bra_in_smem = true, bool generic = false)
@@ -69,21 +93,18 @@ inline FillSmem fill_smem_plan(const DevLattice& L, int nw, int row_batch, bool 
     FillSmem s{};
     int o = 0;
     auto take = [&](int bytes) { int r = o; o += fill_align16(bytes); return r; };
+    // cell norms of both axes: in shared memory when they fit beside everything else (decided below), else read from the edges
+    s.dp = s.dq = -1;
     s.tx = take(8 * L.n_x); s.sx = take(8 * L.n_x); s.wx = take(8 * L.n_x);
     s.bra = bra_in_smem ? take(8 * L.n_x * (L.n_bra + 1)) : -1;      // rows padded with one zero slot; -1: read from global memory
     s.odesc = take(4 * L.n_out); s.ofi = take(4 * L.n_out); s.oc = take(24 * L.n_out);
     s.fa = take(4 * nfun_pad); s.fb = take(4 * nfun_pad);             // (every function chunk of the stage reads its entry)
     const int np = (L.n_slot + 1) / 2;              // slot pairs
-    int w = 0;
-    auto wtake = [&](int bytes) { int r = w; w += fill_align16(bytes); return r; };
-    s.w_tile = wtake(16 * kTileStride * np);
-    s.w_sseg = wtake(16 * np);
-    s.w_acc = wtake(8 * L.n_fun * row_batch);      // sums of finished targets waiting for their rows to be written
-    s.w_hcol = wtake(4 * row_batch);
-    s.w_wpa = wtake(8 * L.n_p); s.w_wqb = wtake(8 * L.n_q); s.w_pa = wtake(8 * L.n_p); s.w_qb = wtake(8 * L.n_q);
-    s.w_ring = wtake(2 * 32 * 8); s.w_cell = wtake(32);
+    s.w = warp_layout(np, L.n_fun, row_batch);
+    const int w = s.w.fixed_bytes + 16 * (L.n_p + L.n_q);
     s.warp_bytes = w;
     s.warp0 = take(w * nw);
+    if (o + fill_align16(8 * L.Np) + fill_align16(8 * L.Nq) <= 227 * 1024) { s.dp = take(8 * L.Np); s.dq = take(8 * L.Nq); }
     s.total = o;
     return s;
 }
@@ -118,20 +139,26 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
     int* s_ofi = (int*)(smem + S.ofi);                 // f0 | f1 << 10 | f2 << 20 | (n_terms - 1) << 30
     double* s_oc = (double*)(smem + S.oc);             // [o][3] coefficients c^L (0 where there is no term)
     char* wsm = smem + S.warp0 + warp * S.warp_bytes;
-    double2* s_tile = (double2*)(wsm + S.w_tile);
-    double2* s_sseg2 = (double2*)(wsm + S.w_sseg);
+    // compile-time offsets for a specialised kernel (the host plan computes the same numbers from the lattice's tables)
+    constexpr WarpLayout kW = warp_layout(NP, Spec::NF, kRowBatch);
+    const WarpLayout W = Spec::kStatic ? kW : S.w;
+    double2* s_tile = (double2*)(wsm + W.tile);
+    double2* s_sseg2 = (double2*)(wsm + W.sseg);
     const double* s_sseg = (const double*)s_sseg2;
-    double* s_acc = (double*)(wsm + S.w_acc);         // [kRowBatch][nf] sums of finished targets
-    int* s_hcol = (int*)(wsm + S.w_hcol);               // first column of each finished target: cell * n_ch (kCols)
-    double* s_wpa = (double*)(wsm + S.w_wpa);
-    double* s_wqb = (double*)(wsm + S.w_wqb);
-    double* s_pa = (double*)(wsm + S.w_pa);
-    double* s_qb = (double*)(wsm + S.w_qb);
-    uint2* s_ring = (uint2*)(wsm + S.w_ring);           // chunk words of two steps
+    double* s_acc = (double*)(wsm + W.acc);           // [kRowBatch][nf] sums of finished targets
+    int* s_hcol = (int*)(wsm + W.hcol);                 // first column of each finished target: cell * n_ch (kCols)
+    double2* s_p2 = (double2*)(wsm + W.p2);             // (p_a, hp wp_a) of the cell's p-nodes, then (q_b, hq wq_b) at s_p2 + n_p
+    uint2* s_ring = (uint2*)(wsm + W.ring);             // chunk words of two steps
     struct CellInfo { int64_t rbase; double dsrc; int H; };
-    CellInfo* s_cell = (CellInfo*)(wsm + S.w_cell);
+    CellInfo* s_cell = (CellInfo*)(wsm + W.cell);
 
     // ---- once per CTA: widths, rules, bra harmonics, output descriptors
+    const double* s_dp = S.dp >= 0 ? (const double*)(smem + S.dp) : nullptr;
+    const double* s_dq = S.dq >= 0 ? (const double*)(smem + S.dq) : nullptr;
+    if (S.dp >= 0) {
+        for (int k = tid; k < L.Np; k += T) ((double*)(smem + S.dp))[k] = cell_norm(L.pe, k, L.norm);
+        for (int k = tid; k < L.Nq; k += T) ((double*)(smem + S.dq))[k] = cell_norm(L.qe, k, L.norm);
+    }
     for (int k = tid; k < L.n_x; k += T) { s_tx[k] = L.tx[k]; s_sx[k] = L.sx[k]; s_wx[k] = L.wx[k]; }
     const int nb_ = Spec::kStatic ? Spec::NS : L.n_bra; // bra slots (the whole channel set's)
     const int nsb = nb_ + 1;                            // shared-memory bra rows carry one trailing zero slot (index nb_)
@@ -185,8 +212,8 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         if (lane == 0) { s_cell->rbase = rowptr[(int64_t)cb * L.n_ch]; s_cell->dsrc = cell_norm(L.pe, ci, L.norm) * cell_norm(L.qe, cj, L.norm); s_cell->H = H; }
         {   // the cell's nodes p_a = cp + hp t_a, q_b = cq + hq t_b (the operations of map_node_sq) and weights hp wp_a, hq wq_b
             const CellGeom g = cell_geom(L.pe, L.qe, ci, cj);
-            for (int k = lane; k < L.n_p; k += 32) { s_wpa[k] = __dmul_rn(g.hp, L.wp[k]); s_pa[k] = __dadd_rn(g.cp, __dmul_rn(g.hp, L.tp[k])); }
-            for (int k = lane; k < L.n_q; k += 32) { s_wqb[k] = __dmul_rn(g.hq, L.wq[k]); s_qb[k] = __dadd_rn(g.cq, __dmul_rn(g.hq, L.tq[k])); }
+            for (int k = lane; k < L.n_p; k += 32) s_p2[k] = make_double2(__dadd_rn(g.cp, __dmul_rn(g.hp, L.tp[k])), __dmul_rn(g.hp, L.wp[k]));
+            for (int k = lane; k < L.n_q; k += 32) s_p2[L.n_p + k] = make_double2(__dadd_rn(g.cq, __dmul_rn(g.hq, L.tq[k])), __dmul_rn(g.hq, L.wq[k]));
         }
         __syncwarp();
         int kcur = 0, kdone = 0;                        // targets finished / written; a target's rank is its position in every row
@@ -250,12 +277,13 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         // cut by the pattern pass): the lane sums the ket harmonics of its nodes in registers, so the K tile holds one
         // column per chunk and the shared-memory traffic of the segment sums falls by the chunk length.
         // The chunk words of the next two steps are already in flight.
-        double runT[NCH];
+        // The running sums of the open segment (runS) and of the open target (runT) live in registers only while a step's
+        // segment sums are formed; across the ket code of the next step they wait in shared memory (the open target's
+        // slot of the row batch and the segment buffer), which is what keeps the ket code's accumulators out of local memory.
 #pragma unroll
-        for (int ch = 0; ch < NCH; ++ch) runT[ch] = 0.0;
-        double2 runS[NPC];
+        for (int ch = 0; ch < NCH; ++ch) { const int f = ch * 32 + lane; if (f < nf) s_acc[f] = 0.0; }
 #pragma unroll
-        for (int i = 0; i < NPC; ++i) runS[i] = make_double2(0.0, 0.0);
+        for (int i = 0; i < NPC; ++i) { const int sp = i * 32 + lane; if (sp < np) s_sseg2[sp] = make_double2(0.0, 0.0); }
         // The chunk words travel global -> shared memory by cp.async into a per-warp ring of two steps (the words of step
         // s + 2 are requested when step s is finished): no register holds a word in flight across the ket code, and the
         // step's own words stay readable for the segment and target ends behind it.
@@ -290,11 +318,12 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                     const int ab = (int)(abw & abmask);
                     const int a = L.mg_nq ? (int)__umulhi((unsigned)ab, L.mg_nq) : ab, b = ab - a * L.n_q;
                     const double x = s_tx[c], sx = s_sx[c];
-                    const double p = s_pa[a], q = s_qb[b];                  // cp + hp t_a, cq + hq t_b: the node of DESIGN.md sec. 3.1
+                    const double2 pw = s_p2[a], qw = s_p2[L.n_p + b];
+                    const double p = pw.x, q = qw.x;                        // cp + hp t_a, cq + hq t_b: the node of DESIGN.md sec. 3.1
                     double P2, Q2;
                     map_pq_sq(p, q, x, P2, Q2);
                     // omega = w * p q / (p' q'),  w = ((hp wp_a)(hq wq_b)) wx_c
-                    const double w = __dmul_rn(__dmul_rn(s_wpa[a], s_wqb[b]), s_wx[c]);
+                    const double w = __dmul_rn(__dmul_rn(pw.y, qw.y), s_wx[c]);
                     // rotated directions from vector components (frame: q^ = z, p^ = (sx, 0, x)):
                     //   p' = -p/2 - 3q/4 ,  q' = p - q/2
                     const double psx = p * sx, px = p * x;
@@ -326,6 +355,15 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
             const unsigned dx = s_step[lane].x;
             const unsigned smask = __ballot_sync(0xffffffffu, (dx >> 22) & 1u), tmask = __ballot_sync(0xffffffffu, (dx >> 23) & 1u);
             const int cnt = min(32, nck - base);
+            double runT[NCH];
+            double2 runS[NPC];
+            {
+                const int slot = kcur - kdone;
+#pragma unroll
+                for (int ch = 0; ch < NCH; ++ch) { const int f = ch * 32 + lane; runT[ch] = f < nf ? s_acc[slot * nf + f] : 0.0; }
+#pragma unroll
+                for (int i = 0; i < NPC; ++i) { const int sp = i * 32 + lane; runS[i] = sp < np ? s_sseg2[sp] : make_double2(0.0, 0.0); }
+            }
             // lane = slot pair: walks the tile's nodes, up to 16 per step, stopping at every segment end (and at the tile end)
             const unsigned stops = smask | (1u << (cnt - 1));
             for (int j = 0; j < cnt;) {
@@ -387,8 +425,8 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                     if (kPacked) {
                         const int ia = s_fa[ch * 32 + lane], ib = s_fb[ch * 32 + lane];
                         double v = bra[ia & 255] * s_sseg[ib & 255];
-                        v = fma(bra[(ia >> 8) & 255], s_sseg[(ib >> 8) & 255], v);
-                        v = fma(bra[ia >> 16], s_sseg[ib >> 16], v);
+                        if (Spec::terms(ch) > 1) v = fma(bra[(ia >> 8) & 255], s_sseg[(ib >> 8) & 255], v);
+                        if (Spec::terms(ch) > 2) v = fma(bra[ia >> 16], s_sseg[ib >> 16], v);
                         runT[ch] += v;
                     } else {
                         const int fav = s_fa[ch * 32 + lane], sa = fav & 65535, sb = s_fb[ch * 32 + lane], nM = fav >> 16;
@@ -405,7 +443,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                     const int tcell = (int)(s_step[jb].x & 262143u);
                     const int ic = L.mg_Nq ? (int)__umulhi((unsigned)tcell, L.mg_Nq) : tcell, jc = tcell - ic * L.Nq;
                     // (d_i dbar_j d_i' dbar_j')^(-1/2), folded into the sums; rsqrt is within 2 ulp of the oracle's 1/sqrt
-                    const double nrm = rsqrt(s_cell->dsrc * (cell_norm(L.pe, ic, L.norm) * cell_norm(L.qe, jc, L.norm)));
+                    const double nrm = rsqrt(s_cell->dsrc * (s_dp ? s_dp[ic] * s_dq[jc] : cell_norm(L.pe, ic, L.norm) * cell_norm(L.qe, jc, L.norm)));
 #pragma unroll
                     for (int ch = 0; ch < NCH; ++ch) {
                         const int f = ch * 32 + lane;
@@ -417,6 +455,13 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                     __syncwarp();
                     if (kcur - kdone == kRowBatch) { write_rows(kdone, kRowBatch); kdone = kcur; }
                 }
+            }
+            {   // park the running sums
+                const int slot = kcur - kdone;
+#pragma unroll
+                for (int ch = 0; ch < NCH; ++ch) { const int f = ch * 32 + lane; if (f < nf) s_acc[slot * nf + f] = runT[ch]; }
+#pragma unroll
+                for (int i = 0; i < NPC; ++i) { const int sp = i * 32 + lane; if (sp < np) s_sseg2[sp] = runS[i]; }
             }
             __syncwarp();
             fetch((base >> 5) + 2, (base >> 5) & 1);

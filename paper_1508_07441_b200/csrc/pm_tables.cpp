@@ -238,6 +238,47 @@ std::string build_tables(const pm_channel* ch, int n_ch, int J2, int T2, int sta
             T.ot_off.push_back((int32_t)T.ot_f.size());
         }
 
+    // Triples renumbered by (L, l, lambda), so that the slots of all triples with one L are contiguous and evenly strided:
+    // with the function order below, neighbouring lanes of the stage read evenly strided ket slots.
+    {
+        const int nt = (int)T.tri.size();
+        std::vector<int> ord((size_t)nt), inv((size_t)nt);
+        for (int t = 0; t < nt; ++t) ord[(size_t)t] = t;
+        std::stable_sort(ord.begin(), ord.end(), [&](int x, int y) {
+            const Triple &A = T.tri[(size_t)x], &B = T.tri[(size_t)y];
+            return std::make_tuple(A.L, A.l, A.lam) < std::make_tuple(B.L, B.l, B.lam);
+        });
+        std::vector<Triple> sorted((size_t)nt);
+        int slot = 0;
+        for (int i = 0; i < nt; ++i) {
+            sorted[(size_t)i] = T.tri[(size_t)ord[(size_t)i]];
+            sorted[(size_t)i].slot0 = slot;
+            slot += sorted[(size_t)i].nM;
+            inv[(size_t)ord[(size_t)i]] = i;
+        }
+        T.tri.swap(sorted);
+        for (OrbFun& f : T.fun) {
+            f.ta = inv[(size_t)f.ta]; f.tb = inv[(size_t)f.tb];
+            f.sa0 = T.tri[(size_t)f.ta].slot0; f.sb0 = T.tri[(size_t)f.tb].slot0;
+        }
+    }
+    // Functions ordered by (number of M-terms, L, bra triple, ket triple): the fill kernel's stage handles 32 functions at
+    // a time with as many terms as the largest of them has, neighbouring lanes then read the same bra slots and evenly
+    // strided ket slots (few shared-memory bank conflicts), and the outputs of one row read neighbouring sums.
+    {
+        const int nf = (int)T.fun.size();
+        std::vector<int> ord((size_t)nf), inv((size_t)nf);
+        for (int f = 0; f < nf; ++f) ord[(size_t)f] = f;
+        std::stable_sort(ord.begin(), ord.end(), [&](int x, int y) {
+            const OrbFun &A = T.fun[(size_t)x], &B = T.fun[(size_t)y];
+            return std::make_tuple(A.nM, A.L, A.ta, A.tb) < std::make_tuple(B.nM, B.L, B.ta, B.tb);
+        });
+        std::vector<OrbFun> sorted((size_t)nf);
+        for (int i = 0; i < nf; ++i) { sorted[(size_t)i] = T.fun[(size_t)ord[(size_t)i]]; inv[(size_t)ord[(size_t)i]] = i; }
+        T.fun.swap(sorted);
+        for (int32_t& f : T.ot_f) f = inv[(size_t)f];
+    }
+
     // per-slot bra weights and ket term lists
     T.slot_w.assign((size_t)T.n_slot, 0.0); T.slot_l.assign((size_t)T.n_slot, 0); T.slot_M.assign((size_t)T.n_slot, 0);
     T.kt_off.assign(1, 0);

@@ -93,9 +93,10 @@ def test_bitwise_reproducible(api):
 
 @pytest.mark.parametrize("jit", [True, False], ids=["jit", "generic"])
 def test_kernels_for_channel_sets_without_a_build_time_kernel(api, oracle, jit):
-    """A channel order with no build-time kernel is specialised at run time (NVRTC) or, with that switched off, runs
-    the table-driven fill; same bar for both, and both are what pm_lattice_fill_kernel reports."""
-    wl = I.small_coupled(N=6, jmax=2, orders=(3, 4, 6))
+    """A channel set with no build-time kernel (pair j <= 1, in reversed channel order) is specialised at run time
+    (NVRTC) or, with that switched off, runs the table-driven fill; same bar for both, and both are what
+    pm_lattice_fill_kernel reports."""
+    wl = I.small_coupled(N=6, jmax=1, orders=(3, 4, 6))
     wl.channels = wl.channels[::-1].copy()
     api.pm_set_jit(jit)
     try:

@@ -124,8 +124,9 @@ def test_compute_calls_fail_loudly_without_gpu():
 
 
 def test_fill_kernel_selection_and_work_model():
-    """configs[0..4] select a generated (channel-specialised) fill kernel; another channel ORDER of the same set has
-    other tables and falls back to the table-driven kernel.  The work model is positive and grows with the set."""
+    """configs[0..4] select a generated (channel-specialised) fill kernel, in any channel ORDER (triples and functions
+    are numbered canonically, so the ket tables do not depend on it); another channel SET is specialised at run time or,
+    with that switched off, runs the table-driven kernel.  The work model is positive and grows with the set."""
     names, work = [], []
     for k in range(5):
         wl = I.config(k)
@@ -141,6 +142,9 @@ def test_fill_kernel_selection_and_work_model():
     assert work[4][0] > work[2][0] > work[1][0] and work[4][3] == 580 and work[2][3] == 276
     wl = I.config(2)
     h = _create(wl, channels=wl.channels[::-1].copy())
+    assert api.pm_lattice_fill_kernel(h) == "Spec_nnn_j2"
+    api.pm_lattice_destroy(h)
+    h = _create(wl, channels=I.enumerate_3n_channels(1, +1, 1, 1))
     assert api.pm_lattice_fill_kernel(h) == "jit"             # specialised at run time (NVRTC) at the first fill
     api.pm_set_jit(False)
     try:
@@ -152,7 +156,7 @@ def test_fill_kernel_selection_and_work_model():
 
 def test_runtime_kernel_source_compiles_for_sm100a():
     """The source generated at run time for channel sets without a build-time kernel compiles with NVRTC for sm_100a
-    (no GPU needed): J = 3/2-, a reordered 18-channel set, bosons with d-waves."""
+    (no GPU needed): J = 3/2-, the pair j <= 1 set of J = 1/2+ in reversed order, bosons with d-waves."""
     g7 = I.tan_grid(7, 1.0)
     cases = [
         I.Workload("3N_J3half-", g7, 0.9 * g7, I.enumerate_3n_channels(3, -1, 1, 1), 3, -1, 1, 0, 3, 4, 8),
@@ -160,7 +164,7 @@ def test_runtime_kernel_source_compiles_for_sm100a():
                    I.PM_SPINLESS_BOSON, 5, 5, 9),
     ]
     wl = I.config(2)
-    wl.channels = wl.channels[::-1].copy()
+    wl.channels = I.enumerate_3n_channels(1, +1, 1, 1)[::-1].copy()
     cases.append(wl)
     for wl in cases:
         h = _create(wl)
