@@ -95,10 +95,11 @@ struct pm_lattice {
     bool jit_failed = false;           // run-time compilation was tried for this lattice and failed (jit_error says why)
     std::string jit_error;
     std::vector<pm::GroupTables> groups;   // column-channel groups the table-driven kernel can hold (one for small sets)
-    std::vector<pm::GroupTables> whole;    // the whole set as one group, for a run-time specialised kernel (empty when groups is that already)
+    std::vector<pm::GroupTables> jgroups;  // the groups a specialised kernel can hold (ket slots in registers): one for the sets of
+                                           // BASELINE.json's configs, up to 13 for the 62-channel sets
     struct GroupDev { pm::DevLattice dev; pm::FillLaunch plan; };
-    std::vector<GroupDev> gdev, gdev_whole;
-    bool use_whole = false;            // the last plan runs the whole set through one run-time specialised kernel
+    std::vector<GroupDev> gdev, gdev_j;
+    bool use_j = false;                // the last plan runs the specialised kernels of jgroups
     cudaEvent_t ev_fill0 = nullptr, ev_fill1 = nullptr;   // around the last fill kernel, on its stream (pm_last_fill_ms)
     bool fill_timed = false;
     unsigned long long hash = 0;       // pm::tables_hash of T (selects a generated fill kernel)
@@ -139,7 +140,7 @@ void free_lattice_device(pm_lattice* L)
     if (L->d_blob) cudaFree(L->d_blob);
     if (L->ev_fill0) cudaEventDestroy(L->ev_fill0);
     if (L->ev_fill1) cudaEventDestroy(L->ev_fill1);
-    L->d_blob = nullptr; L->ev_fill0 = L->ev_fill1 = nullptr; L->fill_timed = false; L->geo_version = 0; L->have_plan = false; L->use_whole = false;
+    L->d_blob = nullptr; L->ev_fill0 = L->ev_fill1 = nullptr; L->fill_timed = false; L->geo_version = 0; L->have_plan = false; L->use_j = false;
 }
 
 struct Blob {
@@ -235,7 +236,13 @@ int32_t ensure_device(pm_lattice* L)
     D.totcoup = T.totcoup; D.n_bra = T.n_slot; D.lmax = T.lmax;
     D.ny = pm::ylm_index(T.lmax, T.lmax) + 1;
     std::vector<double> bra;
-    pm::build_bra(T, G->rule_t[2], bra);
+    {   // rows of n_slot + 1 entries: one trailing zero slot for the unused terms of a function
+        std::vector<double> b0;
+        pm::build_bra(T, G->rule_t[2], b0);
+        const size_t ns = (size_t)T.n_slot, nx = G->rule_t[2].size();
+        bra.assign(nx * (ns + 1), 0.0);
+        for (size_t c = 0; c < nx; ++c) std::copy(b0.begin() + (ptrdiff_t)(c * ns), b0.begin() + (ptrdiff_t)((c + 1) * ns), bra.begin() + (ptrdiff_t)(c * (ns + 1)));
+    }
     std::vector<int32_t> o_alpha(T.totcoup);
     for (int a = 0; a < L->n_ch; ++a) for (int o = T.cl_off[a]; o < T.cl_off[a + 1]; ++o) o_alpha[o] = a;
     Blob B;
@@ -245,9 +252,9 @@ int32_t ensure_device(pm_lattice* L)
     const size_t o_ya = B.put(T.ya.data(), 8 * T.ya.size()), o_yb = B.put(T.yb.data(), 8 * T.yb.size());
     const size_t o_yd = B.put(T.ydiag.data(), 8 * T.ydiag.size());
     struct GOff { size_t ktoff, ktip, ktiq, ktc, fun, otoff, otf, otc, ga, gm, gap; };
-    std::vector<const pm::GroupTables*> all;           // the groups, then the whole-set group (if kept)
+    std::vector<const pm::GroupTables*> all;           // the groups of the table-driven kernel, then those of the specialised kernels
     for (const pm::GroupTables& Gt : L->groups) all.push_back(&Gt);
-    for (const pm::GroupTables& Gt : L->whole) all.push_back(&Gt);
+    for (const pm::GroupTables& Gt : L->jgroups) all.push_back(&Gt);
     std::vector<GOff> go(all.size());
     for (size_t g = 0; g < all.size(); ++g) {
         const pm::GroupTables& Gt = *all[g];
@@ -270,17 +277,17 @@ int32_t ensure_device(pm_lattice* L)
     D.bra = (const double*)(b + o_bra);
     D.ya = (const double*)(b + o_ya); D.yb = (const double*)(b + o_yb); D.ydiag = (const double*)(b + o_yd);
     L->gdev.assign(L->groups.size(), pm_lattice::GroupDev{});
-    L->gdev_whole.assign(L->whole.size(), pm_lattice::GroupDev{});
+    L->gdev_j.assign(L->jgroups.size(), pm_lattice::GroupDev{});
     for (size_t g = 0; g < all.size(); ++g) {
         const pm::GroupTables& Gt = *all[g];
         pm::DevLattice Dg = D;
-        Dg.n_slot = Gt.n_slot; Dg.n_fun = (int)Gt.fun.size(); Dg.n_out = (int)Gt.o_alpha.size(); Dg.n_out1 = Gt.n_out1; Dg.n_out2 = Gt.n_out2;
+        Dg.n_slot = Gt.n_slot; Dg.n_fun = (int)Gt.fun.size(); Dg.n_out = (int)Gt.o_alpha.size(); Dg.n_out1 = Gt.n_out1; Dg.n_out2 = Gt.n_out2; Dg.n_out3 = Gt.n_out3;
         Dg.kt_off = (const int*)(b + go[g].ktoff); Dg.kt_ip = (const int*)(b + go[g].ktip); Dg.kt_iq = (const int*)(b + go[g].ktiq);
         Dg.kt_c = (const double*)(b + go[g].ktc);
         Dg.fun = (const int4*)(b + go[g].fun);
         Dg.ot_off = (const int*)(b + go[g].otoff); Dg.ot_f = (const int*)(b + go[g].otf); Dg.ot_c = (const double*)(b + go[g].otc);
         Dg.g_alpha = (const int*)(b + go[g].ga); Dg.g_m = (const int*)(b + go[g].gm); Dg.g_ap = (const int*)(b + go[g].gap);
-        (g < L->groups.size() ? L->gdev[g] : L->gdev_whole[g - L->groups.size()]).dev = Dg;
+        (g < L->groups.size() ? L->gdev[g] : L->gdev_j[g - L->groups.size()]).dev = Dg;
     }
     D = L->gdev[0].dev;                                 // (the pattern kernels read the geometric and coupled-list fields only)
     L->dev = D;
@@ -356,8 +363,9 @@ int32_t make_lattice(pm_geometry* G, const pm_channel* ch, int32_t n_ch, int32_t
     if (!msg.empty()) { delete L; return fail(PM_ERR_CHANNEL, msg); }
     L->hash = pm::tables_hash(L->T);
     pm::build_groups(L->T, ch, pm::kFillMaxSlot, pm::kFillMaxFun, pm::kFillMaxOut, L->groups);
-    if (L->groups.size() > 1 && L->T.n_slot <= pm::kFillMaxSlot && (int)L->T.fun.size() <= pm::kFillMaxFun)
-        pm::build_groups(L->T, ch, 1 << 30, 1 << 30, 1 << 30, L->whole);
+    pm::build_groups(L->T, ch, pm::kFillJitSlot, pm::kFillJitFun, pm::kFillJitOut, L->jgroups);
+    for (const pm::GroupTables& Gt : L->jgroups)
+        if (Gt.n_slot > pm::kFillJitSlot || (int)Gt.fun.size() > pm::kFillJitFun) { L->jgroups.clear(); break; }   // (one class too big: table-driven only)
     for (const pm::GroupTables& Gt : L->groups)
         if (Gt.n_slot > pm::kFillMaxSlot || (int)Gt.fun.size() > pm::kFillMaxFun) {
             delete L; return fail(PM_ERR_CHANNEL, "one orbital pair (l', lambda') of this channel set needs more ket slots than a kernel holds");
@@ -530,9 +538,10 @@ const char* pm_lattice_fill_kernel(const pm_lattice* lat)
 {
     if (!lat) return "";
     if (pm::fill_has_spec(lat->hash)) return pm::fill_variant_name(lat->hash);
-    const bool may_jit = (lat->groups.size() == 1 || !lat->whole.empty()) && pm::jit_enabled() && !lat->jit_failed;
-    if (lat->have_plan) return lat->use_whole ? "jit" : (lat->groups.size() > 1 ? "generic-grouped" : lat->gdev[0].plan.name);
-    return may_jit ? "jit" : (lat->groups.size() > 1 ? "generic-grouped" : "generic");
+    const bool may_jit = !lat->jgroups.empty() && pm::jit_enabled() && !lat->jit_failed;
+    const char* jname = lat->jgroups.size() > 1 ? "jit-grouped" : "jit";
+    if (lat->have_plan) return lat->use_j ? jname : (lat->groups.size() > 1 ? "generic-grouped" : lat->gdev[0].plan.name);
+    return may_jit ? jname : (lat->groups.size() > 1 ? "generic-grouped" : "generic");
 }
 
 int32_t pm_set_jit(int32_t enabled)
@@ -546,8 +555,12 @@ int32_t pm_diag_jit_compile(const pm_lattice* lat, int64_t* cubin_bytes)
     if (!lat) return fail(PM_ERR_ARG, "lat is NULL");
     std::string err;
     size_t n = 0;
-    if (lat->groups.size() > 1 && lat->whole.empty()) return fail(PM_ERR_STATE, "this channel set runs the table-driven kernel group by group; nothing to compile");
-    if (!pm::jit_compile_check(lat->T, 12, 4, &n, err)) return fail(PM_ERR_STATE, err);
+    if (lat->jgroups.empty()) return fail(PM_ERR_STATE, "one orbital pair of this channel set needs more ket slots than a specialised kernel holds: table-driven kernel only");
+    for (const pm::GroupTables& Gt : lat->jgroups) {           // every column-channel group is one kernel
+        size_t k = 0;
+        if (!pm::jit_compile_check(pm::ket_view(Gt, lat->T.n_slot, lat->jgroups.size() == 1), 12, 4, &k, err)) return fail(PM_ERR_STATE, err);
+        n += k;
+    }
     if (cubin_bytes) *cubin_bytes = (int64_t)n;
     return PM_OK;
 }
@@ -651,15 +664,25 @@ int32_t fill_block(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const 
     if (cell_begin == cell_end) return PM_OK;
     const int n_blk = cell_end - cell_begin;
     cudaError_t e;
-    const bool grouped = lat->gdev.size() > 1;         // big channel sets: one table-driven launch per column-channel group
-    std::vector<pm_lattice::GroupDev>& one = lat->gdev_whole.empty() ? lat->gdev : lat->gdev_whole;     // the whole set as one group, if it may be
-    if (!lat->have_plan && one.size() == 1 && !pm::fill_has_spec(lat->hash) && pm::jit_enabled() && !lat->jit_failed) {
-        // no build-time kernel for this channel set: specialise at run time (pm_jit.hpp), else fall back below
-        if (pm::fill_plan_jit(one[0].dev, lat->T, lat->hash, G->n_sm, &one[0].plan, lat->jit_error)) { lat->have_plan = true; lat->use_whole = &one == &lat->gdev_whole; }
-        else lat->jit_failed = true;
+    const bool grouped = lat->gdev.size() > 1;         // big channel sets: one launch per column-channel group
+    const bool has_spec = !grouped && pm::fill_has_spec(lat->hash);
+    const bool cols = d_colidx != nullptr;
+    const bool need_variant = lat->have_plan && lat->use_j && !(cols ? lat->gdev_j[0].plan.fn_cols : lat->gdev_j[0].plan.fn);
+    if ((!lat->have_plan || need_variant) && !has_spec && !lat->gdev_j.empty() && pm::jit_enabled() && !lat->jit_failed) {
+        // no build-time kernel for this channel set: specialise at run time (pm_jit.hpp), one kernel per group of jgroups
+        // and only the variant this call launches; else fall back to the table-driven kernel below
+        std::vector<pm::DevLattice> devs;
+        std::vector<pm::KetView> views;
+        for (size_t g = 0; g < lat->gdev_j.size(); ++g) { devs.push_back(lat->gdev_j[g].dev); views.push_back(pm::ket_view(lat->jgroups[g], lat->T.n_slot, true)); }
+        std::vector<pm::FillLaunch> plans;
+        if (need_variant) for (auto& gd : lat->gdev_j) plans.push_back(gd.plan);
+        if (pm::fill_plan_jit(devs, views, G->n_sm, cols, plans, lat->jit_error)) {
+            for (size_t g = 0; g < plans.size(); ++g) lat->gdev_j[g].plan = plans[g];
+            lat->have_plan = true; lat->use_j = true;
+        } else { lat->jit_failed = true; lat->have_plan = false; }
     }
     if (!lat->have_plan) {
-        lat->use_whole = false;
+        lat->use_j = false;
         for (auto& gd : lat->gdev) {
             e = pm::fill_plan(gd.dev, grouped ? 0ull : lat->hash, G->n_sm, &gd.plan);
             if (e == cudaErrorInvalidConfiguration) { cudaGetLastError(); return fail(PM_ERR_NOMEM, "channel set needs more shared memory than one SM has"); }
@@ -668,7 +691,7 @@ int32_t fill_block(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const 
         lat->have_plan = true;
     }
     if ((e = cudaEventRecord(lat->ev_fill0, st)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
-    for (auto& gd : (lat->use_whole ? lat->gdev_whole : lat->gdev)) {
+    for (auto& gd : (lat->use_j ? lat->gdev_j : lat->gdev)) {
         e = pm::launch_fill(gd.dev, gd.plan, cell_begin, n_blk, G->nl, d_rowptr, d_vals, d_colidx, G->d_counter, guard, st);
         if (e != cudaSuccess) return cuda_fail(e, "k_fill");
     }

@@ -32,7 +32,7 @@ struct DevLattice {
     int totcoup, n_slot, n_fun, lmax, ny;       // n_slot / n_fun: ket slots and orbital functions of THIS column-channel group
     int norm;                                   // cell normalisation: 0 reading A (widths), 1 reading B (p^2 dp measure) — DESIGN.md R2
     int n_out, n_bra;                           // outputs (alpha, alpha') of this group; bra slots of the whole channel set
-    int n_out1, n_out2;                         // the group's rows are ordered by the most terms of their outputs: outputs of rows with at most 1 / at most 2
+    int n_out1, n_out2, n_out3;                       // the group's rows are ordered by the most terms of their outputs: outputs of rows with at most 1 / 2 / 3
     unsigned mg_npq, mg_nq, mg_Nq;              // ceil(2^32 / d) for d = n_p*n_q, n_q, Nq: exact division of node and cell ids (x*d < 2^32)
     const double *pe, *qe;                      // edges, Np+1 / Nq+1 entries (padded with +inf to pe_pad / qe_pad)
     const double *thr_p, *thr_q;                // sqrt_threshold(edge), padded with +inf to a power of two
@@ -43,7 +43,7 @@ struct DevLattice {
     const double *sx;                           // sqrt(1-x^2) per x-node
     const int *cl_off, *cl, *o_alpha;           // coupled lists of the whole set; o_alpha[o] = alpha of global output o
     const int *g_alpha, *g_m, *g_ap;            // outputs of this group: row channel, position in the row's coupled list, column channel
-    const double *bra;                          // [n_x][n_bra]
+    const double *bra;                          // [n_x][n_bra + 1], every row ends with a zero slot
     const int *kt_off, *kt_ip, *kt_iq; const double *kt_c;
     const int4 *fun;                            // (sa0, sb0, nM, L)
     const int *ot_off, *ot_f; const double *ot_c;

@@ -46,18 +46,22 @@ void emit_q(std::ostringstream& o, char side, int lmax, const std::string& seed,
 
 }  // namespace
 
-std::string emit_spec(const std::string& name, const Tables& T, EmitStats& st)
+std::string emit_spec(const std::string& name, const KetView& V, EmitStats& st)
 {
-    std::vector<double> ynorm, ybeta;
-    scaled_harmonics(T.lmax, ynorm, ybeta);
+    struct { int n_slot; const std::vector<int32_t>&kt_off, &kt_ip, &kt_iq; const std::vector<double>& kt_c; const std::vector<OrbFun>& fun; }
+        T{V.n_slot, *V.kt_off, *V.kt_ip, *V.kt_iq, *V.kt_c, *V.fun};
+    auto l_of = [](int idx) { int l = 0; while (ylm_index(l + 1, 0) <= idx) ++l; return l; };
     int la = 0, lb = 0;
-    for (const Triple& t : T.tri) { la = std::max(la, t.l); lb = std::max(lb, t.lam); }
+    for (size_t t = 0; t < T.kt_c.size(); ++t) { la = std::max(la, l_of(T.kt_ip[t])); lb = std::max(lb, l_of(T.kt_iq[t])); }
+    std::vector<double> ynorm, ybeta;
+    scaled_harmonics(std::max(la, lb), ynorm, ybeta);
     std::ostringstream o;
     const int nf = (int)T.fun.size();
     o << "struct Spec_" << name << " {\n";
     o << "    static constexpr bool kStatic = true;\n";
     int maxm = 1, maxl1 = 1;                        // most M-terms of a function; number of L values (terms per output)
     for (const OrbFun& f : T.fun) { maxm = std::max(maxm, f.nM); maxl1 = std::max(maxl1, f.L + 1); }
+    if (V.n_bra > 254) maxm = std::max(maxm, 4);   // the packed descriptors (MAXM <= 3) hold bra slots in 8 bits
     o << "    static constexpr int NS = " << T.n_slot << ", NF = " << nf << ", NCH = " << (nf + 31) / 32 << ", MAXM = " << maxm << ", MAXL1 = " << maxl1 << ";\n";
     o << "    // most M-terms of the 32 functions step ch of the stage handles\n"
          "    static __device__ __forceinline__ constexpr int terms(int ch) { return ";
@@ -68,7 +72,10 @@ std::string emit_spec(const std::string& name, const Tables& T, EmitStats& st)
         else o << m;
     }
     o << "; }\n";
-    char hb[32]; std::snprintf(hb, sizeof hb, "0x%016" PRIx64 "ull", tables_hash(T));
+    o << "    static constexpr int NOT = " << V.n_oterm << ";            // terms per output kept in shared memory\n";
+    o << "    static constexpr bool kOutTail = " << (V.oterm_tail ? "true" : "false") << ";     // some output has more terms than that\n";
+    o << "    static constexpr bool kBraSmem = " << (V.bra_smem ? "true" : "false") << ";      // bra harmonics in shared / global memory\n";
+    char hb[32]; std::snprintf(hb, sizeof hb, "0x%016" PRIx64 "ull", (uint64_t)V.hash);
     o << "    static constexpr unsigned long long kHash = " << hb << ";\n";
     o << "    // K[s] += omega * (ket bipolar harmonic of slot s) at directions a = p'^ = (uxa,0,uza), b = q'^ = (uxb,0,uzb)\n";
     o << "    static __device__ __forceinline__ void ket_acc(const DevLattice&, double om, double uxa, double uza, double uxb, double uzb,\n"

@@ -10,7 +10,7 @@ namespace pm {
 
 struct EmitStats { int n_prod = 0, n_fma = 0, n_mul = 0; };
 
-// `struct Spec_<name> { ... static __device__ void ket(...) }` for tables T (no namespace around it)
-std::string emit_spec(const std::string& name, const Tables& T, EmitStats& st);
+// `struct Spec_<name> { ... static __device__ void ket_acc(...) }` for the ket tables in V (no namespace around it)
+std::string emit_spec(const std::string& name, const KetView& V, EmitStats& st);
 
 }  // namespace pm

@@ -18,15 +18,15 @@ constexpr int kSmemLimit = 227 * 1024;
 
 using FillKernel = void (*)(DevLattice, FillSmem, NodeLists, int, int, const int64_t*, double*, int32_t*, int*, const int64_t*);
 
-struct FillVariant { unsigned long long hash; int nw, rb; FillKernel fn, fn_cols; const char* name; };
+struct FillVariant { unsigned long long hash; int nw, rb, n_oterm; FillKernel fn, fn_cols; const char* name; };
 
-#define PM_VAR(S, NW, RB) {gen::S::kHash, NW, RB, k_fill_warp<gen::S, NW, RB, false>, k_fill_warp<gen::S, NW, RB, true>, #S}
+#define PM_VAR(S, NW, RB) {gen::S::kHash, NW, RB, gen::S::NOT, k_fill_warp<gen::S, NW, RB, false>, k_fill_warp<gen::S, NW, RB, true>, #S}
 #define PM_SPEC(S) PM_VAR(S, 4, 4), PM_VAR(S, 8, 4), PM_VAR(S, 12, 4),
 const FillVariant kVariants[] = {
     PM_SPEC_LIST
-    {0ull, 2, 4, k_fill_warp<SpecGeneric, 2, 4, false>, k_fill_warp<SpecGeneric, 2, 4, true>, "generic"},
-    {0ull, 4, 4, k_fill_warp<SpecGeneric, 4, 4, false>, k_fill_warp<SpecGeneric, 4, 4, true>, "generic"},
-    {0ull, 8, 4, k_fill_warp<SpecGeneric, 8, 4, false>, k_fill_warp<SpecGeneric, 8, 4, true>, "generic"},
+    {0ull, 2, 4, SpecGeneric::NOT, k_fill_warp<SpecGeneric, 2, 4, false>, k_fill_warp<SpecGeneric, 2, 4, true>, "generic"},
+    {0ull, 4, 4, SpecGeneric::NOT, k_fill_warp<SpecGeneric, 4, 4, false>, k_fill_warp<SpecGeneric, 4, 4, true>, "generic"},
+    {0ull, 8, 4, SpecGeneric::NOT, k_fill_warp<SpecGeneric, 8, 4, false>, k_fill_warp<SpecGeneric, 8, 4, true>, "generic"},
 };
 #undef PM_VAR
 #undef PM_SPEC
@@ -79,8 +79,8 @@ cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int n_sm, Fi
     const int want = preferred_warps();
     const FillVariant* best = nullptr;          // largest warp count <= want whose shared memory fits, else the smallest that fits
     auto plan_of = [&](const FillVariant& v) {         // the bra table moves to global memory when it does not fit beside the tiles
-        FillSmem s = fill_smem_plan(L, v.nw, v.rb, true, v.hash == 0ull);
-        if (s.total > kSmemLimit && v.hash == 0ull) s = fill_smem_plan(L, v.nw, v.rb, false, true);
+        FillSmem s = fill_smem_plan(L, v.nw, v.rb, v.n_oterm, true, v.hash == 0ull);
+        if (s.total > kSmemLimit && v.hash == 0ull) s = fill_smem_plan(L, v.nw, v.rb, v.n_oterm, false, true);
         return s;
     };
     for (const FillVariant& v : kVariants) {
@@ -106,20 +106,40 @@ cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int n_sm, Fi
     return cudaSuccess;
 }
 
-bool fill_plan_jit(const DevLattice& L, const Tables& T, unsigned long long hash, int n_sm, FillLaunch* out, std::string& err)
+// Run-time compiled kernels for the column-channel groups `views` of one lattice (devs[g]: the group's device view).
+// One warp count and one bra placement for all groups: the most warps whose shared memory fits with the bra harmonics
+// beside them, else the most warps with the bra harmonics read from global memory.
+bool fill_plan_jit(const std::vector<DevLattice>& devs, std::vector<KetView> views, int n_sm, bool cols, std::vector<FillLaunch>& out, std::string& err)
 {
     const int rb = 4;
+    const size_t n = devs.size();
+    auto fits = [&](int w, bool bra_smem) {
+        for (size_t g = 0; g < n; ++g) if (fill_smem_plan(devs[g], w, rb, views[g].n_oterm, bra_smem).total > kSmemLimit) return false;
+        return true;
+    };
     int nw = 0;
-    for (int w : {preferred_warps(), 12, 8, 4})
-        if (w >= 1 && w <= 32 && fill_smem_plan(L, w, rb).total <= kSmemLimit) { nw = w; break; }
+    bool bra_smem = true;
+    const int want = preferred_warps();
+    for (int w : {want, 12, 8, 4}) {
+        if (w < 1 || w > 32) continue;
+        if (fits(w, true)) { nw = w; bra_smem = true; break; }
+        if (w >= 8 && fits(w, false)) { nw = w; bra_smem = false; break; }
+    }
+    if (!nw) for (int w : {4, 2}) if (fits(w, false)) { nw = w; bra_smem = false; break; }
     if (!nw) { err = "no warp count fits in shared memory"; return false; }
-    JitFill k;
-    if (!jit_fill(T, hash, nw, rb, &k, err)) return false;
-    out->fn = k.fn; out->fn_cols = k.fn_cols; out->nw = nw; out->name = "jit"; out->jit = true;
-    out->smem = fill_smem_plan(L, nw, rb);
-    const int per_sm = jit_prepare(k, false, out->smem.total), per_sm_c = jit_prepare(k, true, out->smem.total);
-    if (per_sm < 1 || per_sm_c < 1) { err = "the compiled kernel does not fit on an SM"; return false; }
-    out->grid = n_sm * (per_sm < per_sm_c ? per_sm : per_sm_c);
+    for (KetView& v : views) v.bra_smem = bra_smem;
+    std::vector<JitFill> k;
+    if (!jit_fill_many(views, nw, rb, cols, k, err)) return false;
+    if (out.size() != n) out.assign(n, FillLaunch{});       // (a second call adds the other variant to the plans of the first)
+    for (size_t g = 0; g < n; ++g) {
+        FillLaunch& F = out[g];
+        (cols ? F.fn_cols : F.fn) = cols ? k[g].fn_cols : k[g].fn;
+        F.nw = nw; F.name = n > 1 ? "jit-grouped" : "jit"; F.jit = true;
+        F.smem = fill_smem_plan(devs[g], nw, rb, views[g].n_oterm, bra_smem);
+        const int per_sm = jit_prepare(k[g], cols, F.smem.total);
+        if (per_sm < 1) { err = "the compiled kernel does not fit on an SM"; return false; }
+        F.grid = n_sm * per_sm;
+    }
     return true;
 }
 

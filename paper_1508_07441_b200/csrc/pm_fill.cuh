@@ -23,6 +23,9 @@ namespace pm {
 constexpr int kFillMaxSlot = 96;       // ket slots / orbital functions one kernel launch holds (larger channel sets are
 constexpr int kFillMaxFun = 320;       // split into column-channel groups, pm_tables.hpp)
 constexpr int kFillMaxOut = 1400;      // outputs (alpha, alpha') per launch of the table-driven kernel (their tables live in shared memory)
+constexpr int kFillJitSlot = 40;       // ... and what one SPECIALISED kernel holds: its ket slots are accumulators in registers,
+constexpr int kFillJitFun = 160;       // its functions five stage steps, its output tables share the SM's shared memory with
+constexpr int kFillJitOut = 700;       // twelve warps' tiles
 constexpr int kFillMaxY = 91;          // harmonics per direction up to l = PM_MAX_L = 12
 
 // Table-driven ket code for channel sets without a generated kernel (slow: local arrays, table loads).
@@ -30,6 +33,9 @@ struct SpecGeneric {
     static constexpr bool kStatic = false;
     static constexpr int NS = kFillMaxSlot, NF = kFillMaxFun, NCH = kFillMaxFun / 32, MAXM = 99, MAXL1 = 99;
     static constexpr unsigned long long kHash = 0ull;
+    static constexpr bool kBraSmem = false;             // (decided at run time for this kernel: FillSmem::bra)
+    static constexpr int NOT = 3;                       // terms per output kept in shared memory (more come from the global tables)
+    static constexpr bool kOutTail = true;
     static __device__ __forceinline__ constexpr int terms(int) { return 3; }      // (unused: MAXM > 3 loops over the function's own terms)
     // writes the node's column of the K tile directly (no per-thread K array): col = tile + lane, np slot pairs
     static __device__ __noinline__ void ket_tile(const DevLattice& L, double om, double uxa, double uza, double uxb, double uzb,
@@ -87,7 +93,7 @@ inline int fill_align16(int b) { return (b + 15) & ~15; }
 
 
 // shared-memory plan for nw warps: tables shared by the CTA, then one private area per warp
-inline FillSmem fill_smem_plan(const DevLattice& L, int nw, int row_batch, bool bra_in_smem = true, bool generic = false)
+inline FillSmem fill_smem_plan(const DevLattice& L, int nw, int row_batch, int n_oterm, bool bra_in_smem = true, bool generic = false)
 {
     const int nfun_pad = generic ? kFillMaxFun : (L.n_fun + 31) & ~31;     // NCH * 32 of the kernel that runs
     FillSmem s{};
@@ -96,8 +102,8 @@ inline FillSmem fill_smem_plan(const DevLattice& L, int nw, int row_batch, bool 
     // cell norms of both axes: in shared memory when they fit beside everything else (decided below), else read from the edges
     s.dp = s.dq = -1;
     s.tx = take(8 * L.n_x); s.sx = take(8 * L.n_x); s.wx = take(8 * L.n_x);
-    s.bra = bra_in_smem ? take(8 * L.n_x * (L.n_bra + 1)) : -1;      // rows padded with one zero slot; -1: read from global memory
-    s.odesc = take(4 * L.n_out); s.ofi = take(4 * L.n_out); s.oc = take(24 * L.n_out);
+    s.bra = bra_in_smem ? take(8 * L.n_x * (L.n_bra + 1)) : -1;      // rows end with one zero slot; -1: read from global memory
+    s.odesc = take(4 * L.n_out); s.ofi = take(4 * L.n_out); s.oc = take(8 * n_oterm * L.n_out);
     s.fa = take(4 * nfun_pad); s.fb = take(4 * nfun_pad);             // (every function chunk of the stage reads its entry)
     const int np = (L.n_slot + 1) / 2;              // slot pairs
     s.w = warp_layout(np, L.n_fun, row_batch);
@@ -136,8 +142,8 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
     double* s_sx = (double*)(smem + S.sx);   double* s_wx = (double*)(smem + S.wx);
     double* s_bra = (double*)(smem + (S.bra >= 0 ? S.bra : 0));
     int* s_odesc = (int*)(smem + S.odesc);             // per output o: cl_off[alpha] | nc << 12 | m << 19 | alpha' << 25
-    int* s_ofi = (int*)(smem + S.ofi);                 // f0 | f1 << 10 | f2 << 20 | (n_terms - 1) << 30
-    double* s_oc = (double*)(smem + S.oc);             // [o][3] coefficients c^L (0 where there is no term)
+    int* s_ofi = (int*)(smem + S.ofi);                 // f0 | f1 << 10 | f2 << 20 | (n_terms - 1) << 30, or four f of 8 bits
+    double* s_oc = (double*)(smem + S.oc);             // [o][NOT] coefficients c^L (0 where there is no term)
     char* wsm = smem + S.warp0 + warp * S.warp_bytes;
     // compile-time offsets for a specialised kernel (the host plan computes the same numbers from the lattice's tables)
     constexpr WarpLayout kW = warp_layout(NP, Spec::NF, kRowBatch);
@@ -160,20 +166,21 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         for (int k = tid; k < L.Nq; k += T) ((double*)(smem + S.dq))[k] = cell_norm(L.qe, k, L.norm);
     }
     for (int k = tid; k < L.n_x; k += T) { s_tx[k] = L.tx[k]; s_sx[k] = L.sx[k]; s_wx[k] = L.wx[k]; }
-    const int nb_ = Spec::kStatic ? Spec::NS : L.n_bra; // bra slots (the whole channel set's)
-    const int nsb = nb_ + 1;                            // shared-memory bra rows carry one trailing zero slot (index nb_)
+    const int nb_ = L.n_bra;                            // bra slots (the whole channel set's)
+    const int nsb = nb_ + 1;                            // bra rows carry one trailing zero slot (index nb_), in global memory too
     if (S.bra >= 0)
-        for (int k = tid; k < L.n_x * nsb; k += T) { const int c = k / nsb, sl = k - c * nsb; s_bra[k] = sl < nb_ ? L.bra[c * nb_ + sl] : 0.0; }
+        for (int k = tid; k < L.n_x * nsb; k += T) s_bra[k] = L.bra[k];
     const double* __restrict__ bra_tab = S.bra >= 0 ? s_bra : L.bra;      // big channel sets: the bra table stays in global memory
-    const int bra_stride = S.bra >= 0 ? nsb : nb_;
+    const int bra_stride = nsb;
+    constexpr int NOT = Spec::NOT;                      // terms per output kept in shared memory: 3 (f in 10 bits each + count) or 4 (8 bits each)
     for (int o = tid; o < L.n_out; o += T) {
         const int al = L.g_alpha[o], off = L.cl_off[al], nc = L.cl_off[al + 1] - off;
         const int t0 = L.ot_off[o], nt = L.ot_off[o + 1] - t0;
         s_odesc[o] = off | (nc << 12) | (L.g_m[o] << 19) | (L.g_ap[o] << 25);
-        int fi = (nt > 0 ? nt - 1 : 0) << 30;
-        for (int i = 0; i < 3; ++i) {
-            s_oc[3 * o + i] = i < nt ? L.ot_c[t0 + i] : 0.0;
-            fi |= (i < nt ? L.ot_f[t0 + i] : 0) << (10 * i);
+        int fi = NOT == 3 ? (nt > 0 ? nt - 1 : 0) << 30 : 0;
+        for (int i = 0; i < NOT; ++i) {
+            s_oc[NOT * o + i] = i < nt ? L.ot_c[t0 + i] : 0.0;
+            fi |= (i < nt ? L.ot_f[t0 + i] : 0) << ((NOT == 3 ? 10 : 8) * i);
         }
         s_ofi[o] = fi;
     }
@@ -235,12 +242,14 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 for (int o = o_begin + lane; o < o_end; o += 32) {
                     const int od = s_odesc[o], fi = s_ofi[o];
                     const int clo = od & 4095, nc = (od >> 12) & 127, mm = (od >> 19) & 63, ap = (unsigned)od >> 25;
-                    const double c0 = s_oc[3 * o], c1 = NT > 1 ? s_oc[3 * o + 1] : 0.0, c2 = NT > 2 ? s_oc[3 * o + 2] : 0.0;
-                    const int f0 = fi & 1023, f1 = (fi >> 10) & 1023, f2 = (fi >> 20) & 1023;
+                    const double c0 = s_oc[NOT * o], c1 = NT > 1 ? s_oc[NOT * o + 1] : 0.0, c2 = NT > 2 ? s_oc[NOT * o + 2] : 0.0,
+                                 c3 = NT > 3 ? s_oc[NOT * o + 3] : 0.0;
+                    constexpr int FB = NOT == 3 ? 10 : 8, FM = (1 << FB) - 1;
+                    const int f0 = fi & FM, f1 = (fi >> FB) & FM, f2 = (fi >> (2 * FB)) & FM, f3 = NOT > 3 ? (int)((unsigned)fi >> 24) : 0;
                     // entry of target k0+bb in row alpha: element H*clo + (k0+bb)*nc + m of the cell's block (fits 32 bits)
                     const unsigned idx0 = (unsigned)(Hc * clo + k0 * nc + mm);
                     const char* acc0 = (const char*)s_acc;
-                    const unsigned a0 = 8u * f0, a1 = 8u * f1, a2 = 8u * f2;
+                    const unsigned a0 = 8u * f0, a1 = 8u * f1, a2 = 8u * f2, a3 = 8u * f3;
 #pragma unroll
                     for (int bb = 0; bb < kRowBatch; ++bb) {
                         if (kFull || bb < nb) {
@@ -248,9 +257,10 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                             double v = c0 * *(const double*)(acc + a0);
                             if (NT > 1) v = fma(c1, *(const double*)(acc + a1), v);
                             if (NT > 2) v = fma(c2, *(const double*)(acc + a2), v);
-                            if (Spec::MAXL1 > 3) {                       // more than three L values: the tail comes from the tables
-                                const int t0 = L.ot_off[o], nt = (int)((unsigned)fi >> 30) + 1;
-                                for (int t = 3; t < nt; ++t) v = fma(L.ot_c[t0 + t], ((const double*)acc)[L.ot_f[t0 + t]], v);
+                            if (NT > 3) v = fma(c3, *(const double*)(acc + a3), v);
+                            if (Spec::kOutTail) {                     // more L values than the shared-memory tables hold: the tail comes from the global ones
+                                const int t0 = L.ot_off[o], nt = L.ot_off[o + 1] - t0;
+                                for (int t = NOT; t < nt; ++t) v = fma(L.ot_c[t0 + t], ((const double*)acc)[L.ot_f[t0 + t]], v);
                             }
                             const unsigned e = idx0 + (unsigned)(bb * nc);
                             row0[e] = v;
@@ -260,12 +270,13 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 }
             };
             if constexpr (kFull) {
-                const int e1 = L.n_out1 & ~31, e2 = max(e1, L.n_out2 & ~31);
+                const int e1 = L.n_out1 & ~31, e2 = max(e1, L.n_out2 & ~31), e3 = NOT > 3 ? max(e2, L.n_out3 & ~31) : L.n_out;
                 outputs(0, e1, std::integral_constant<int, 1>{});
                 outputs(e1, e2, std::integral_constant<int, 2>{});
-                outputs(e2, L.n_out, std::integral_constant<int, 3>{});
+                outputs(e2, e3, std::integral_constant<int, 3>{});
+                if constexpr (NOT > 3) outputs(e3, L.n_out, std::integral_constant<int, 4>{});
             } else {
-                outputs(0, L.n_out, std::integral_constant<int, 3>{});
+                outputs(0, L.n_out, std::integral_constant<int, NOT>{});
             }
             __syncwarp();
         };
@@ -419,7 +430,8 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 __syncwarp();
                 const int cseg = (int)(s_step[jb].x >> 24);
                 const double* bra;                                     // (shared-memory loads for the specialised kernels)
-                if constexpr (Spec::kStatic) bra = s_bra + cseg * nsb; else bra = bra_tab + cseg * bra_stride;
+                if constexpr (Spec::kStatic) { if (Spec::kBraSmem) bra = s_bra + cseg * nsb; else bra = L.bra + cseg * nsb; }
+                else bra = bra_tab + cseg * bra_stride;
 #pragma unroll
                 for (int ch = 0; ch < NCH; ++ch) {
                     if (kPacked) {

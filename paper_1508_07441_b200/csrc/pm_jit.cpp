@@ -3,8 +3,11 @@
 
 #include <cstdio>
 #include <cstdlib>
+#include <algorithm>
+#include <atomic>
 #include <map>
 #include <mutex>
+#include <thread>
 #include <sstream>
 #include <vector>
 
@@ -90,14 +93,17 @@ bool load_driver()
 }
 
 // NVRTC only (no device needed): cubin and the lowered names of the two kernel variants
-bool compile_cubin(const Tables& T, int nw, int rb, std::vector<char>& cubin, std::string low[2], std::string& err)
+bool compile_cubin(const KetView& T, int nw, int rb, int variants, std::vector<char>& cubin, std::string low[2], std::string& err)
 {
-    if (!load_nvrtc()) { err = g_api.why; return false; }
+    if (!g_api.ok) { err = g_api.why.empty() ? "NVRTC is not loaded" : g_api.why; return false; }      // (load_nvrtc() ran under the lock)
     const Api& a = g_api;
     EmitStats st;
     std::ostringstream src;
     src << "#include \"pm_fill.cuh\"\nnamespace pm {\nnamespace gen {\n" << emit_spec("jit", T, st) << "}\n}\n";
     const std::string text = src.str();
+    if (const char* dump = std::getenv("PM_JIT_DUMP")) {        // debugging aid: the generated translation unit
+        if (FILE* f = std::fopen(dump, "w")) { std::fputs(text.c_str(), f); std::fclose(f); }
+    }
     const char* hdr_src[] = {kJitDeviceCuh, kJitYlmH, kJitFillCuh};
     const char* hdr_name[] = {"pm_device.cuh", "pm_ylm.h", "pm_fill.cuh"};
     nvrtcProgram prog = nullptr;
@@ -105,6 +111,7 @@ bool compile_cubin(const Tables& T, int nw, int rb, std::vector<char>& cubin, st
     if (r != NVRTC_SUCCESS) { err = std::string("nvrtcCreateProgram: ") + a.errString(r); return false; }
     std::string names[2];
     for (int c = 0; c < 2; ++c) {
+        if (!(variants & (1 << c))) continue;
         std::ostringstream n;
         n << "pm::k_fill_warp<pm::gen::Spec_jit, " << nw << ", " << rb << ", " << (c ? "true" : "false") << ">";
         names[c] = n.str();
@@ -125,7 +132,13 @@ bool compile_cubin(const Tables& T, int nw, int rb, std::vector<char>& cubin, st
     a.getCubinSize(prog, &nbin);
     cubin.resize(nbin);
     a.getCubin(prog, cubin.data());
-    for (int c = 0; c < 2; ++c) { const char* l = nullptr; a.getLowered(prog, names[c].c_str(), &l); low[c] = l ? l : ""; }
+    for (int c = 0; c < 2; ++c) {
+        low[c].clear();
+        if (!(variants & (1 << c))) continue;
+        const char* l = nullptr;
+        a.getLowered(prog, names[c].c_str(), &l);
+        low[c] = l ? l : "";
+    }
     a.destroyProgram(&prog);
     return true;
 }
@@ -135,44 +148,86 @@ bool compile_cubin(const Tables& T, int nw, int rb, std::vector<char>& cubin, st
 void jit_set_enabled(bool on) { std::lock_guard<std::mutex> g(g_mu); g_enabled = on; }
 bool jit_enabled() { std::lock_guard<std::mutex> g(g_mu); return g_enabled; }
 
-bool jit_compile_check(const Tables& T, int nw, int rb, size_t* cubin_bytes, std::string& err)
+bool jit_compile_check(const KetView& V, int nw, int rb, size_t* cubin_bytes, std::string& err)
 {
-    std::lock_guard<std::mutex> g(g_mu);
+    {
+        std::lock_guard<std::mutex> g(g_mu);
+        if (!load_nvrtc()) { err = g_api.why; return false; }
+    }
     std::vector<char> cubin;
     std::string low[2];
-    if (!compile_cubin(T, nw, rb, cubin, low, err)) return false;
+    if (!compile_cubin(V, nw, rb, 2, cubin, low, err)) return false;      // the variant pm_build launches
     if (cubin_bytes) *cubin_bytes = cubin.size();
-    return !low[0].empty() && !low[1].empty();
+    return !low[1].empty();
 }
 
-bool jit_fill(const Tables& T, unsigned long long hash, int nw, int rb, JitFill* out, std::string& err)
+bool jit_fill_many(const std::vector<KetView>& views, int nw, int rb, bool cols, std::vector<JitFill>& out, std::string& err)
 {
-    std::lock_guard<std::mutex> g(g_mu);
-    if (!g_enabled) { err = "run-time compilation is disabled"; return false; }
-    char key[80];
-    int dev = -1;
-    if (load_driver() && g_api.ctxGetDevice) g_api.ctxGetDevice(&dev);
-    std::snprintf(key, sizeof key, "%d/%016llx/%d/%d", dev, hash, nw, rb);
-    auto it = g_cache.find(key);
-    if (it != g_cache.end()) { *out = it->second; return true; }
-    std::vector<char> cubin;
-    std::string low[2];
-    if (!compile_cubin(T, nw, rb, cubin, low, err)) return false;
-    if (!load_driver()) { err = g_api.why; return false; }
-    const Api& a = g_api;
-    CUmodule mod = nullptr;
-    CUresult cr = a.moduleLoadData(&mod, cubin.data());
-    JitFill k;
-    k.nw = nw; k.rb = rb;
-    if (cr == CUDA_SUCCESS) {
-        CUfunction f0 = nullptr, f1 = nullptr;
-        cr = a.moduleGetFunction(&f0, mod, low[0].c_str());
-        if (cr == CUDA_SUCCESS) cr = a.moduleGetFunction(&f1, mod, low[1].c_str());
-        k.fn = f0; k.fn_cols = f1;
+    const size_t n = views.size();
+    out.assign(n, JitFill{});
+    std::vector<std::string> keys(n);
+    std::vector<size_t> todo;
+    {
+        std::lock_guard<std::mutex> g(g_mu);
+        if (!g_enabled) { err = "run-time compilation is disabled"; return false; }
+        int dev = -1;
+        if (load_driver() && g_api.ctxGetDevice) g_api.ctxGetDevice(&dev);
+        for (size_t i = 0; i < n; ++i) {
+            char key[96];
+            std::snprintf(key, sizeof key, "%d/%016llx/%d/%d/%d/%d/%d", dev, (unsigned long long)views[i].hash, nw, rb, views[i].bra_smem ? 1 : 0, views[i].n_bra > 254 ? 1 : 0, cols ? 1 : 0);
+            keys[i] = key;
+            auto it = g_cache.find(keys[i]);
+            if (it != g_cache.end()) out[i] = it->second; else todo.push_back(i);
+        }
+        if (todo.empty()) return true;
+        if (!load_nvrtc()) { err = g_api.why; return false; }
+        if (!load_driver()) { err = g_api.why; return false; }
     }
-    if (cr != CUDA_SUCCESS) { err = "loading the compiled kernel failed (CUresult " + std::to_string((int)cr) + ")"; return false; }
-    g_cache[key] = k;                                // the module stays loaded for the life of the process
-    *out = k;
+    // NVRTC runs outside the lock, one host thread per kernel (the programs are independent)
+    std::vector<std::vector<char>> cubin(todo.size());
+    std::vector<std::string> low0(todo.size()), low1(todo.size()), errs(todo.size());
+    std::vector<char> ok(todo.size(), 0);
+    {
+        const size_t nt = std::min<size_t>(todo.size(), std::max(1u, std::thread::hardware_concurrency()));
+        std::atomic<size_t> next{0};
+        auto work = [&] {
+            for (size_t j = next++; j < todo.size(); j = next++) {
+                std::string low[2];
+                ok[j] = compile_cubin(views[todo[j]], nw, rb, cols ? 2 : 1, cubin[j], low, errs[j]) ? 1 : 0;
+                low0[j] = low[0]; low1[j] = low[1];
+            }
+        };
+        std::vector<std::thread> th;
+        for (size_t t = 1; t < nt; ++t) th.emplace_back(work);
+        work();
+        for (std::thread& t : th) t.join();
+    }
+    // modules are loaded by the calling thread (it holds the CUDA context)
+    std::lock_guard<std::mutex> g(g_mu);
+    const Api& a = g_api;
+    for (size_t j = 0; j < todo.size(); ++j) {
+        if (!ok[j]) { err = errs[j]; return false; }
+        CUmodule mod = nullptr;
+        CUresult cr = a.moduleLoadData(&mod, cubin[j].data());
+        JitFill k;
+        k.nw = nw; k.rb = rb;
+        if (cr == CUDA_SUCCESS) {
+            CUfunction f = nullptr;
+            cr = a.moduleGetFunction(&f, mod, (cols ? low1[j] : low0[j]).c_str());
+            (cols ? k.fn_cols : k.fn) = f;
+        }
+        if (cr != CUDA_SUCCESS) { err = "loading the compiled kernel failed (CUresult " + std::to_string((int)cr) + ")"; return false; }
+        g_cache[keys[todo[j]]] = k;                  // the module stays loaded for the life of the process
+        out[todo[j]] = k;
+    }
+    return true;
+}
+
+bool jit_fill(const KetView& V, int nw, int rb, bool cols, JitFill* out, std::string& err)
+{
+    std::vector<JitFill> r;
+    if (!jit_fill_many(std::vector<KetView>{V}, nw, rb, cols, r, err)) return false;
+    *out = r[0];
     return true;
 }
 

@@ -5,6 +5,7 @@
 #include <cstddef>
 #include <cstdint>
 #include <string>
+#include <vector>
 
 #include "pm_device.cuh"
 #include "pm_fill.cuh"
@@ -38,8 +39,9 @@ struct FillLaunch { const void *fn, *fn_cols; int nw, grid; FillSmem smem; const
 bool fill_has_spec(unsigned long long tables_hash);
 const char* fill_variant_name(unsigned long long tables_hash);
 cudaError_t fill_plan(const DevLattice& L, unsigned long long tables_hash, int n_sm, FillLaunch* out);
-// run-time compiled kernel for tables T (no build-time kernel): false + message when NVRTC / the driver API fails
-bool fill_plan_jit(const DevLattice& L, const Tables& T, unsigned long long tables_hash, int n_sm, FillLaunch* out, std::string& err);
+// run-time compiled kernels for the column-channel groups of one lattice (no build-time kernel): false + message when
+// NVRTC / the driver API fails
+bool fill_plan_jit(const std::vector<DevLattice>& devs, std::vector<KetView> views, int n_sm, bool cols, std::vector<FillLaunch>& out, std::string& err);
 cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl,
                         const int64_t* rowptr, double* vals, int32_t* colidx, int* counter, const int64_t* guard, cudaStream_t st);
 

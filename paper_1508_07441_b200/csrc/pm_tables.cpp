@@ -403,7 +403,8 @@ void build_groups(const Tables& T, const pm_channel* ch, int max_slot, int max_f
         std::stable_sort(ord.begin(), ord.end(), [&](int x, int y) { return row_nt[G.o_alpha[(size_t)x]] < row_nt[G.o_alpha[(size_t)y]]; });
         GroupTables R = G;
         R.ot_off.assign(1, 0); R.ot_f.clear(); R.ot_c.clear();
-        G.n_out1 = G.n_out2 = 0;
+        G.n_out1 = G.n_out2 = G.n_out3 = 0;
+        int max_nt = 0;
         for (int i = 0; i < n; ++i) {
             const int o = ord[(size_t)i];
             R.o_alpha[(size_t)i] = G.o_alpha[(size_t)o]; R.o_m[(size_t)i] = G.o_m[(size_t)o]; R.o_ap[(size_t)i] = G.o_ap[(size_t)o];
@@ -411,9 +412,24 @@ void build_groups(const Tables& T, const pm_channel* ch, int max_slot, int max_f
             R.ot_off.push_back((int32_t)R.ot_f.size());
             if (row_nt[G.o_alpha[(size_t)o]] <= 1) ++G.n_out1;
             if (row_nt[G.o_alpha[(size_t)o]] <= 2) ++G.n_out2;
+            if (row_nt[G.o_alpha[(size_t)o]] <= 3) ++G.n_out3;
+            max_nt = std::max(max_nt, nt(o));
         }
-        R.n_out1 = G.n_out1; R.n_out2 = G.n_out2;
+        R.n_out1 = G.n_out1; R.n_out2 = G.n_out2; R.n_out3 = G.n_out3;
+        R.n_oterm = max_nt > 3 ? 4 : 3;
+        R.oterm_tail = max_nt > 4;
         G = R;
+        uint64_t h = 1469598103934665603ull;
+        auto mix = [&](const void* p, size_t n) {
+            const unsigned char* b = (const unsigned char*)p;
+            for (size_t i = 0; i < n; ++i) { h ^= b[i]; h *= 1099511628211ull; }
+        };
+        auto mixi = [&](int64_t v) { mix(&v, sizeof v); };
+        mixi(G.n_slot); mixi((int64_t)G.fun.size()); mixi(G.n_oterm); mixi(G.oterm_tail ? 1 : 0);
+        for (const OrbFun& f : G.fun) { mixi(f.sb0); mixi(f.nM); mixi(f.L); }
+        mix(G.kt_off.data(), 4 * G.kt_off.size()); mix(G.kt_ip.data(), 4 * G.kt_ip.size());
+        mix(G.kt_iq.data(), 4 * G.kt_iq.size()); mix(G.kt_c.data(), 8 * G.kt_c.size());
+        G.hash = h;
     }
 }
 
@@ -445,6 +461,27 @@ uint64_t tables_hash(const Tables& T)
     mix(T.kt_off.data(), 4 * T.kt_off.size()); mix(T.kt_ip.data(), 4 * T.kt_ip.size());
     mix(T.kt_iq.data(), 4 * T.kt_iq.size()); mix(T.kt_c.data(), 8 * T.kt_c.size());
     return h;
+}
+
+KetView ket_view(const Tables& T)
+{
+    KetView v;
+    v.n_slot = T.n_slot; v.n_bra = T.n_slot; v.kt_off = &T.kt_off; v.kt_ip = &T.kt_ip; v.kt_iq = &T.kt_iq; v.kt_c = &T.kt_c; v.fun = &T.fun;
+    v.hash = tables_hash(T); v.bra_smem = true;
+    for (size_t o = 0; o + 1 < T.ot_off.size(); ++o) {
+        if (T.ot_off[o + 1] - T.ot_off[o] > 3) v.n_oterm = 4;
+        if (T.ot_off[o + 1] - T.ot_off[o] > 4) v.oterm_tail = true;
+    }
+    return v;
+}
+
+KetView ket_view(const GroupTables& G, int n_bra, bool bra_smem)
+{
+    KetView v;
+    v.n_bra = n_bra;
+    v.n_slot = G.n_slot; v.kt_off = &G.kt_off; v.kt_ip = &G.kt_ip; v.kt_iq = &G.kt_iq; v.kt_c = &G.kt_c; v.fun = &G.fun;
+    v.hash = G.hash; v.bra_smem = bra_smem; v.n_oterm = G.n_oterm; v.oterm_tail = G.oterm_tail;
+    return v;
 }
 
 void scaled_harmonics(int lmax, std::vector<double>& ynorm, std::vector<double>& ybeta)

@@ -51,10 +51,28 @@ struct GroupTables {
     std::vector<OrbFun> fun;                          // sa0: GLOBAL bra slot, sb0: LOCAL ket slot
     std::vector<int32_t> o_alpha, o_m, o_ap;          // outputs: row channel, position in the row's coupled list, column channel;
                                                       // rows ordered by the most terms of their outputs
-    int n_out1 = 0, n_out2 = 0;                       // outputs in rows with at most one / at most two terms per output
+    int n_out1 = 0, n_out2 = 0, n_out3 = 0;           // outputs in rows with at most one / two / three terms per output
+    int n_oterm = 3;                                  // terms per output a specialised kernel keeps in shared memory: 3, or 4 when an output has more than 3
+    bool oterm_tail = false;                          // some output has more terms than that (never for three spin-1/2 particles: at most four L per pair)
     std::vector<int32_t> ot_off, ot_f;                // terms per output, f numbered locally
     std::vector<double> ot_c;
+    uint64_t hash = 0;                                // FNV-1a of what the group's ket code depends on (keys run-time compiled kernels)
 };
+
+// What the generated ket code of one kernel depends on: a whole channel set (Tables) or one column-channel group.
+struct KetView {
+    int n_slot = 0;
+    int n_bra = 0;                                    // bra slots of the whole channel set (the functions' sa0 index them)
+    const std::vector<int32_t> *kt_off = nullptr, *kt_ip = nullptr, *kt_iq = nullptr;
+    const std::vector<double>* kt_c = nullptr;
+    const std::vector<OrbFun>* fun = nullptr;
+    uint64_t hash = 0;
+    int n_oterm = 3;                                  // (GroupTables::n_oterm, oterm_tail)
+    bool oterm_tail = false;
+    bool bra_smem = true;                             // the kernel reads the bra harmonics from shared memory (else from global memory)
+};
+KetView ket_view(const Tables& T);
+KetView ket_view(const GroupTables& G, int n_bra, bool bra_smem);
 
 // One group holding everything when the set fits (max_slot, max_fun, max_out outputs), else a greedy packing of the
 // (l', lam') classes under the three limits.

@@ -472,14 +472,16 @@ def test_attached_lattices_share_the_geometric_pattern(api, oracle):
     lat.close()
 
 
-JPI = [(3, +1), (3, -1), (5, +1), (5, -1), (9, -1), (17, +1), (17, -1)]
+JPI = [(3, -1), (17, +1)]                                   # run-time specialised kernels (3 + 13 of them: NVRTC takes a minute)
+JPI_GENERIC = [(3, +1), (5, +1), (5, -1), (9, -1), (17, -1)]  # table-driven kernel, group by group
 
 
 def test_every_Jpi_up_to_17_halves_on_one_grid(api, oracle):
     """SURVEY sec. 8(f) rank 3 ("up to 62 channels", L394 + Table 1 "all states ... up to J_max = 17/2"):
     the j <= 3 channel sets of J^pi = 3/2+- ... 17/2+- attached to one J = 1/2+ base lattice, built with pm_build_reuse
     (the geometric pattern is mapped once), element by element against the oracle.  Sets beyond one kernel's tables
-    (up to 422 ket slots, 546 orbital functions, 3694 coupled channel pairs) run column-channel group by group."""
+    (up to 422 ket slots, 546 orbital functions, 3694 coupled channel pairs) run column-channel group by group, each group
+    through its own run-time specialised kernel or, with that switched off, through the table-driven one."""
     import torch
     base = I.small_coupled(N=4, jmax=3, orders=(3, 2, 5), Nq=5)
     lat = api.Lattice(base)
@@ -498,8 +500,24 @@ def test_every_Jpi_up_to_17_halves_on_one_grid(api, oracle):
         assert np.array_equal(rp.cpu().numpy(), rpo) and np.array_equal(ci.cpu().numpy(), cio), (J2, par)
         _assert_values(v.cpu().numpy(), vo)
         api.pm_lattice_destroy(h)
-    assert kinds[(17, +1)] == (62, "generic-grouped") and kinds[(5, +1)][1] == "generic-grouped", kinds
+    assert kinds[(17, +1)] == (62, "jit-grouped") and kinds[(3, -1)] == (46, "jit-grouped"), kinds
     assert max(k[0] for k in kinds.values()) == 62
+    # the same with run-time compilation switched off: the table-driven kernel, group by group, same bar
+    api.pm_set_jit(False)
+    try:
+        for J2, par in JPI_GENERIC:
+            w = I.small_coupled(N=4, jmax=3, orders=(3, 2, 5), Nq=5, J2=J2, parity=par)
+            h = api.pm_lattice_attach(lat.h, w.channels, w.J2, w.parity, w.T2, w.statistics)
+            rpo, cio, vo = oracle.build_csr(w)
+            rp = torch.empty(w.M + 1, dtype=torch.int64, device="cuda")
+            ci = torch.empty(len(cio), dtype=torch.int32, device="cuda"); v = torch.empty(len(cio), dtype=torch.float64, device="cuda")
+            assert api.pm_build_reuse(h, 0, w.n_cells, rp, ci, v) == len(cio)
+            assert api.pm_lattice_fill_kernel(h) == "generic-grouped"
+            assert np.array_equal(rp.cpu().numpy(), rpo) and np.array_equal(ci.cpu().numpy(), cio), (J2, par)
+            _assert_values(v.cpu().numpy(), vo)
+            api.pm_lattice_destroy(h)
+    finally:
+        api.pm_set_jit(True)
     lat.close()
 
 
