@@ -33,7 +33,7 @@ UNIT = "nnz/s"
 FP64_LANES_PER_SM = 64
 # dram__bytes_read.sum + dram__bytes_write.sum of one fill launch, QUOTED from the committed `ncu --set full` capture
 # named beside it (bench.py cannot run under the profiler); None where no capture exists.
-FILL_DRAM_TRAFFIC = {"cfg4_3N_Jhalf+_jle3_26ch_150x150": (10.777e9 + 0.443e9, "profiles/r1_final_fill.md (ncu --set full, round 1; quoted, not measured in this run)")}
+FILL_DRAM_TRAFFIC = {"cfg4_3N_Jhalf+_jle3_26ch_150x150": (10.779e9 + 0.311e9, "profiles/r2_final.md (ncu --set full of this kernel, round 2; quoted, not measured in this run)")}
 
 
 def _peaks():
@@ -240,13 +240,14 @@ class _Null:
 
 def fill_roofline(api, lat, wl, nnz, fill_ms, pk, n_sm, dfma):
     """Both roofs of the fill kernel, the binding one first.  HBM: algorithmic bytes = 12 B per nonzero
-    written once; the 4 B node key the kernel reads per node on the grid is listed separately."""
+    written once; the 8-byte chunk words the kernel reads (one per run of at most four nodes) are listed
+    separately."""
     peak_tf = n_sm * FP64_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 * 1e-12
     flops, work = build_flops(api, lat.h)
     fill_avg = float(np.mean(fill_ms)) * 1e-3
     achieved_tf = flops / fill_avg * 1e-12
     alg_bytes = 12.0 * nnz
-    key_bytes = 4.0 * work["nodes_on_grid"]
+    key_bytes = 8.0 * api.pm_pattern_chunks(lat.h)
     achieved_gbs = alg_bytes / fill_avg * 1e-9
     t_alu, t_hbm = flops / (peak_tf * 1e12), alg_bytes / (pk["hbm_gbs"] * 1e9)
     alu = {"achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
@@ -257,7 +258,7 @@ def fill_roofline(api, lat, wl, nnz, fill_ms, pk, n_sm, dfma):
     bound = "hbm" if t_hbm >= t_alu else "alu"
     traffic, traffic_src = FILL_DRAM_TRAFFIC.get(wl.name, (None, None))
     return {"bound": bound, "kernel": "k_fill_warp (values + column indices)", **(hbm if bound == "hbm" else alu),
-            "traffic": traffic, "traffic_source": traffic_src, "algorithmic_bytes": alg_bytes, "node_key_bytes_read": key_bytes,
+            "traffic": traffic, "traffic_source": traffic_src, "algorithmic_bytes": alg_bytes, "chunk_word_bytes_read": key_bytes,
             "flops_per_launch": flops, "flop_per_byte": flops / alg_bytes, "ridge_flop_per_byte": peak_tf * 1e3 / pk["hbm_gbs"],
             "min_ms": {"alu": t_alu * 1e3, "hbm": t_hbm * 1e3}, "alu": alu, "hbm": hbm, "work": work, "fill_ms": fill_avg * 1e3}
 

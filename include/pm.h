@@ -207,6 +207,12 @@ int32_t pm_lattice_work(const pm_lattice* lat, double* flop_per_node, double* fl
  * PM_ERR_STATE before the first pm_pattern. */
 int32_t pm_pattern_counts(const pm_lattice* lat, int64_t* nodes_on_grid, int64_t* segments, int64_t* hit_cells);
 
+/* Chunks of the last pm_pattern call on this lattice (host out): the pattern pass cuts every source cell's sorted node
+ * list into runs of at most four nodes of one (target cell, x-node) segment (one lane of the fill kernel sums one chunk in
+ * registers) and leaves one 8-byte word per chunk, which the fill reads once: 8 * chunks are the fill's input bytes.
+ * PM_ERR_STATE before the first pm_pattern. */
+int32_t pm_pattern_chunks(const pm_lattice* lat, int64_t* chunks);
+
 /* Name of the fill kernel this lattice's channel set selects: "Spec_<set>" when csrc/build.py generated straight-line
  * ket code for it at build time (the channel sets of BASELINE.json's configs); "jit" when the same kind of code is
  * generated from the lattice's tables and compiled with NVRTC at the first fill (any other channel set; needs

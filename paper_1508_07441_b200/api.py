@@ -22,7 +22,7 @@ ERRORS = {-1: "PM_ERR_ARG", -2: "PM_ERR_GRID", -3: "PM_ERR_CHANNEL", -4: "PM_ERR
           -6: "PM_ERR_NOMEM", -7: "PM_ERR_STATE", -8: "PM_ERR_OVERFLOW", -9: "PM_ERR_DEVICE"}
 
 EXPORTS = ["pm_lattice_create", "pm_lattice_destroy", "pm_lattice_dims", "pm_lattice_rule", "pm_lattice_set_rule",
-           "pm_lattice_coupling", "pm_lattice_work", "pm_pattern_counts", "pm_lattice_fill_kernel", "pm_set_jit", "pm_diag_jit_compile", "pm_diag_sqrt_threshold",
+           "pm_lattice_coupling", "pm_lattice_work", "pm_pattern_counts", "pm_pattern_chunks", "pm_lattice_fill_kernel", "pm_set_jit", "pm_diag_jit_compile", "pm_diag_sqrt_threshold",
            "pm_diag_dfma_tflops", "pm_pattern", "pm_fill", "pm_build", "pm_last_fill_ms", "pm_block_apply", "pm_kernel_apply", "pm_spmv_implicit", "pm_spmv", "pm_build_host_count", "pm_build_host",
            "pm_launch_count", "pm_last_error", "pm_lattice_attach", "pm_build_async", "pm_build_wait", "pm_build_reuse",
            "pm_pattern_cell_hits", "pm_partition_cells", "pm_rowptr_offset", "pm_block_apply_t", "pm_rotate_apply",
@@ -73,6 +73,7 @@ def lib():
     L.pm_lattice_coupling.argtypes = [_vp, C.POINTER(C.c_uint8), _i32p]
     L.pm_lattice_work.argtypes = [_vp, _dp, _dp, _dp, _i32p]
     L.pm_pattern_counts.argtypes = [_vp, _i64p, _i64p, _i64p]
+    L.pm_pattern_chunks.argtypes = [_vp, _i64p]
     L.pm_diag_dfma_tflops.argtypes = [_dp, _vp]
     L.pm_set_jit.argtypes = [C.c_int32]
     L.pm_diag_jit_compile.argtypes = [_vp, _i64p]
@@ -179,6 +180,13 @@ def pm_pattern_counts(h):
     a, s_, b = C.c_int64(), C.c_int64(), C.c_int64()
     _check(lib().pm_pattern_counts(h, C.byref(a), C.byref(s_), C.byref(b)))
     return a.value, s_.value, b.value
+
+
+def pm_pattern_chunks(h):
+    """Chunks (8-byte words the fill reads) of the last pm_pattern call."""
+    a = C.c_int64()
+    _check(lib().pm_pattern_chunks(h, C.byref(a)))
+    return a.value
 
 
 def pm_lattice_fill_kernel(h):

@@ -76,7 +76,7 @@ struct pm_geometry {
     int pat_begin = -1, pat_end = -1;
     int totcoup_of_scan = 0;           // the channel-pair count the last scan multiplied the hit counts with
     int hmax = -1;
-    int64_t nnz = 0, nodes_on_grid = 0, hit_cells = 0, segments = -1, overflow = 0;
+    int64_t nnz = 0, nodes_on_grid = 0, hit_cells = 0, segments = -1, overflow = 0, chunks = 0;
     cudaStream_t last_stream = nullptr;
 };
 
@@ -100,6 +100,13 @@ struct pm_lattice {
     struct GroupDev { pm::DevLattice dev; pm::FillLaunch plan; };
     std::vector<GroupDev> gdev, gdev_j;
     bool use_j = false;                // the last plan runs the specialised kernels of jgroups
+    // several groups: the fill goes through the per-pair sums (pm_fill.cuh mode 2 + k_op_expand)
+    int op_stride = 0;                 // doubles per hit cell pair: the groups' functions, each group's range padded to 4
+    std::vector<int> op_off;           // first position of each group of jgroups
+    const unsigned short* d_xpos = nullptr;    // [totcoup][4] position of each term's function in a pair's sums (in d_blob)
+    const double* d_xc = nullptr;              // [totcoup][4] coefficients
+    double* d_opA = nullptr;           // the sums of the last fill, library-owned scratch
+    int64_t opA_cap = 0;
     cudaEvent_t ev_fill0 = nullptr, ev_fill1 = nullptr;   // around the last fill kernel, on its stream (pm_last_fill_ms)
     bool fill_timed = false;
     unsigned long long hash = 0;       // pm::tables_hash of T (selects a generated fill kernel)
@@ -140,6 +147,8 @@ void free_lattice_device(pm_lattice* L)
     if (L->d_blob) cudaFree(L->d_blob);
     if (L->ev_fill0) cudaEventDestroy(L->ev_fill0);
     if (L->ev_fill1) cudaEventDestroy(L->ev_fill1);
+    if (L->d_opA) cudaFree(L->d_opA);
+    L->d_opA = nullptr; L->opA_cap = 0;
     L->d_blob = nullptr; L->ev_fill0 = L->ev_fill1 = nullptr; L->fill_timed = false; L->geo_version = 0; L->have_plan = false; L->use_j = false;
 }
 
@@ -268,6 +277,27 @@ int32_t ensure_device(pm_lattice* L)
         go[g].ga = B.put(Gt.o_alpha.data(), 4 * Gt.o_alpha.size()); go[g].gm = B.put(Gt.o_m.data(), 4 * Gt.o_m.size());
         go[g].gap = B.put(Gt.o_ap.data(), 4 * Gt.o_ap.size());
     }
+    // per-pair sums layout of jgroups and the whole set's outputs in terms of it (k_op_expand)
+    size_t o_xpos = 0, o_xc = 0;
+    L->op_off.clear(); L->op_stride = 0;
+    if (L->jgroups.size() > 1) {
+        std::vector<int> pos(T.fun.size(), 0);
+        for (const pm::GroupTables& Gt : L->jgroups) {
+            L->op_off.push_back(L->op_stride);
+            for (size_t f = 0; f < Gt.f_global.size(); ++f) pos[(size_t)Gt.f_global[f]] = L->op_stride + (int)f;
+            L->op_stride += ((int)Gt.fun.size() + 3) & ~3;
+        }
+        std::vector<uint16_t> xpos(4 * (size_t)T.totcoup, 0);
+        std::vector<double> xc(4 * (size_t)T.totcoup, 0.0);
+        bool ok = L->op_stride < 65536;
+        for (int o = 0; o < T.totcoup && ok; ++o) {
+            const int t0 = T.ot_off[(size_t)o], nt = T.ot_off[(size_t)o + 1] - t0;
+            if (nt > 4) { ok = false; break; }
+            for (int i = 0; i < nt; ++i) { xpos[4 * (size_t)o + i] = (uint16_t)pos[(size_t)T.ot_f[(size_t)(t0 + i)]]; xc[4 * (size_t)o + i] = T.ot_c[(size_t)(t0 + i)]; }
+        }
+        if (ok) { o_xpos = B.put(xpos.data(), 2 * xpos.size()); o_xc = B.put(xc.data(), 8 * xc.size()); }
+        else { L->op_stride = 0; L->op_off.clear(); }          // (more than four terms per output: group by group into the CSR)
+    }
     cudaError_t e;
     if ((e = cudaMalloc(&L->d_blob, B.b.size())) != cudaSuccess) return cuda_fail(e, "cudaMalloc(channel tables)");
     if ((e = cudaMemcpy(L->d_blob, B.b.data(), B.b.size(), cudaMemcpyHostToDevice)) != cudaSuccess) return cuda_fail(e, "cudaMemcpy(channel tables)");
@@ -275,6 +305,7 @@ int32_t ensure_device(pm_lattice* L)
     char* b = L->d_blob;
     D.cl_off = (const int*)(b + o_cloff); D.cl = (const int*)(b + o_cl); D.o_alpha = (const int*)(b + o_oa);
     D.bra = (const double*)(b + o_bra);
+    L->d_xpos = L->op_stride ? (const unsigned short*)(b + o_xpos) : nullptr; L->d_xc = L->op_stride ? (const double*)(b + o_xc) : nullptr;
     D.ya = (const double*)(b + o_ya); D.yb = (const double*)(b + o_yb); D.ydiag = (const double*)(b + o_yd);
     L->gdev.assign(L->groups.size(), pm_lattice::GroupDev{});
     L->gdev_j.assign(L->jgroups.size(), pm_lattice::GroupDev{});
@@ -286,6 +317,7 @@ int32_t ensure_device(pm_lattice* L)
         Dg.kt_c = (const double*)(b + go[g].ktc);
         Dg.fun = (const int4*)(b + go[g].fun);
         Dg.ot_off = (const int*)(b + go[g].otoff); Dg.ot_f = (const int*)(b + go[g].otf); Dg.ot_c = (const double*)(b + go[g].otc);
+        Dg.op_stride = L->op_stride; Dg.op_off = (g >= L->groups.size() && L->op_stride) ? L->op_off[g - L->groups.size()] : 0;
         Dg.g_alpha = (const int*)(b + go[g].ga); Dg.g_m = (const int*)(b + go[g].gm); Dg.g_ap = (const int*)(b + go[g].gap);
         (g < L->groups.size() ? L->gdev[g] : L->gdev_j[g - L->groups.size()]).dev = Dg;
     }
@@ -336,6 +368,7 @@ int32_t sync_summary(pm_geometry* G)
     G->summary_pending = false;
     G->nnz = G->h_summary[0]; G->hmax = (int)G->h_summary[1]; G->nodes_on_grid = G->h_summary[2];
     G->overflow = G->h_summary[4];
+    G->chunks = G->h_summary[5];
     G->hit_cells = G->totcoup_of_scan ? G->nnz / G->totcoup_of_scan : 0;
     return PM_OK;
 }
@@ -534,6 +567,17 @@ int32_t pm_pattern_counts(const pm_lattice* lat_c, int64_t* nodes_on_grid, int64
     return PM_OK;
 }
 
+int32_t pm_pattern_chunks(const pm_lattice* lat_c, int64_t* chunks)
+{
+    if (!lat_c || !chunks) return fail(PM_ERR_ARG, "NULL argument");
+    pm_geometry* G = const_cast<pm_lattice*>(lat_c)->G;
+    if (!G->lists_valid) return fail(PM_ERR_STATE, "pm_pattern_chunks needs a preceding pm_pattern");
+    int32_t rc = sync_summary(G);
+    if (rc) return rc;
+    *chunks = G->chunks;
+    return PM_OK;
+}
+
 const char* pm_lattice_fill_kernel(const pm_lattice* lat)
 {
     if (!lat) return "";
@@ -625,7 +669,7 @@ int32_t pattern_async(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int
     }
     if ((e = pm::launch_scan_rows(lat->dev, n_blk, G->nl, G->d_cellbase, d_rowptr, G->d_summary, capacity, st)) != cudaSuccess)
         return cuda_fail(e, "k_scan_rows");
-    if ((e = cudaMemcpyAsync(G->h_summary, G->d_summary, 5 * sizeof(int64_t), cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+    if ((e = cudaMemcpyAsync(G->h_summary, G->d_summary, 6 * sizeof(int64_t), cudaMemcpyDeviceToHost, st)) != cudaSuccess)
         return cuda_fail(e, "cudaMemcpyAsync(summary)");
     if ((e = cudaEventRecord(G->ev_summary, st)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
     G->summary_pending = true;
@@ -666,8 +710,11 @@ int32_t fill_block(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const 
     cudaError_t e;
     const bool grouped = lat->gdev.size() > 1;         // big channel sets: one launch per column-channel group
     const bool has_spec = !grouped && pm::fill_has_spec(lat->hash);
-    const bool cols = d_colidx != nullptr;
-    const bool need_variant = lat->have_plan && lat->use_j && !(cols ? lat->gdev_j[0].plan.fn_cols : lat->gdev_j[0].plan.fn);
+    // several specialised groups: each writes the per-pair sums of its functions, one kernel then writes whole CSR rows
+    const bool via_sums = lat->gdev_j.size() > 1 && lat->op_stride > 0;
+    const int mode = via_sums ? 2 : (d_colidx != nullptr ? 1 : 0);
+    auto have_fn = [&](const pm::FillLaunch& F) { return mode == 2 ? F.fn_op != nullptr : mode == 1 ? F.fn_cols != nullptr : F.fn != nullptr; };
+    const bool need_variant = lat->have_plan && lat->use_j && !have_fn(lat->gdev_j[0].plan);
     if ((!lat->have_plan || need_variant) && !has_spec && !lat->gdev_j.empty() && pm::jit_enabled() && !lat->jit_failed) {
         // no build-time kernel for this channel set: specialise at run time (pm_jit.hpp), one kernel per group of jgroups
         // and only the variant this call launches; else fall back to the table-driven kernel below
@@ -676,7 +723,7 @@ int32_t fill_block(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const 
         for (size_t g = 0; g < lat->gdev_j.size(); ++g) { devs.push_back(lat->gdev_j[g].dev); views.push_back(pm::ket_view(lat->jgroups[g], lat->T.n_slot, true)); }
         std::vector<pm::FillLaunch> plans;
         if (need_variant) for (auto& gd : lat->gdev_j) plans.push_back(gd.plan);
-        if (pm::fill_plan_jit(devs, views, G->n_sm, cols, plans, lat->jit_error)) {
+        if (pm::fill_plan_jit(devs, views, G->n_sm, mode, plans, lat->jit_error)) {
             for (size_t g = 0; g < plans.size(); ++g) lat->gdev_j[g].plan = plans[g];
             lat->have_plan = true; lat->use_j = true;
         } else { lat->jit_failed = true; lat->have_plan = false; }
@@ -691,6 +738,27 @@ int32_t fill_block(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const 
         lat->have_plan = true;
     }
     if ((e = cudaEventRecord(lat->ev_fill0, st)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
+    if (lat->use_j && via_sums) {
+        int32_t rc = ensure_hitlist(lat, st);           // (waits for the pattern pass: the number of hit cell pairs sizes the sums)
+        if (rc) return rc;
+        if (G->overflow) return PM_OK;                  // (the caller reports it)
+        const int64_t need = std::max<int64_t>(G->hit_cells, 1) * lat->op_stride;
+        if (need > lat->opA_cap) {
+            if (lat->d_opA) cudaFree(lat->d_opA);
+            lat->d_opA = nullptr; lat->opA_cap = 0;
+            if ((e = cudaMalloc(&lat->d_opA, sizeof(double) * (size_t)need)) != cudaSuccess) { cudaGetLastError(); return fail(PM_ERR_NOMEM, "out of device memory for the per-pair sums of this channel set"); }
+            lat->opA_cap = need;
+        }
+        for (auto& gd : lat->gdev_j) {
+            e = pm::launch_fill(gd.dev, gd.plan, cell_begin, n_blk, G->nl, G->d_cellbase, lat->d_opA, nullptr, G->d_counter, guard, st, true);
+            if (e != cudaSuccess) return cuda_fail(e, "k_fill (per-pair sums)");
+        }
+        pm::DevLattice De = lat->dev;
+        De.op_stride = lat->op_stride;
+        e = pm::launch_op_expand(De, cell_begin, n_blk, G->nl, G->d_cellbase, G->d_hitlist, lat->d_opA, lat->d_xpos, lat->d_xc, d_rowptr, d_vals,
+                                 d_colidx, G->d_counter, guard, G->n_sm, st);
+        if (e != cudaSuccess) return cuda_fail(e, "k_op_expand");
+    } else
     for (auto& gd : (lat->use_j ? lat->gdev_j : lat->gdev)) {
         e = pm::launch_fill(gd.dev, gd.plan, cell_begin, n_blk, G->nl, d_rowptr, d_vals, d_colidx, G->d_counter, guard, st);
         if (e != cudaSuccess) return cuda_fail(e, "k_fill");

@@ -32,6 +32,7 @@ struct DevLattice {
     int totcoup, n_slot, n_fun, lmax, ny;       // n_slot / n_fun: ket slots and orbital functions of THIS column-channel group
     int norm;                                   // cell normalisation: 0 reading A (widths), 1 reading B (p^2 dp measure) — DESIGN.md R2
     int n_out, n_bra;                           // outputs (alpha, alpha') of this group; bra slots of the whole channel set
+    int op_stride, op_off;                      // per-pair sums form (pm_fill.cuh, mode 2): doubles per hit cell pair, this group's first
     int n_out1, n_out2, n_out3;                       // the group's rows are ordered by the most terms of their outputs: outputs of rows with at most 1 / 2 / 3
     unsigned mg_npq, mg_nq, mg_Nq;              // ceil(2^32 / d) for d = n_p*n_q, n_q, Nq: exact division of node and cell ids (x*d < 2^32)
     const double *pe, *qe;                      // edges, Np+1 / Nq+1 entries (padded with +inf to pe_pad / qe_pad)

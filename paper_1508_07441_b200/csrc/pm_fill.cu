@@ -92,6 +92,7 @@ cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int n_sm, Fi
     if (!best) return cudaErrorInvalidConfiguration;
     out->fn = (const void*)best->fn;
     out->fn_cols = (const void*)best->fn_cols;
+    out->fn_op = nullptr;
     out->nw = best->nw;
     out->name = best->name;
     out->jit = false;
@@ -109,7 +110,7 @@ cudaError_t fill_plan(const DevLattice& L, unsigned long long hash, int n_sm, Fi
 // Run-time compiled kernels for the column-channel groups `views` of one lattice (devs[g]: the group's device view).
 // One warp count and one bra placement for all groups: the most warps whose shared memory fits with the bra harmonics
 // beside them, else the most warps with the bra harmonics read from global memory.
-bool fill_plan_jit(const std::vector<DevLattice>& devs, std::vector<KetView> views, int n_sm, bool cols, std::vector<FillLaunch>& out, std::string& err)
+bool fill_plan_jit(const std::vector<DevLattice>& devs, std::vector<KetView> views, int n_sm, int mode, std::vector<FillLaunch>& out, std::string& err)
 {
     const int rb = 4;
     const size_t n = devs.size();
@@ -129,14 +130,14 @@ bool fill_plan_jit(const std::vector<DevLattice>& devs, std::vector<KetView> vie
     if (!nw) { err = "no warp count fits in shared memory"; return false; }
     for (KetView& v : views) v.bra_smem = bra_smem;
     std::vector<JitFill> k;
-    if (!jit_fill_many(views, nw, rb, cols, k, err)) return false;
+    if (!jit_fill_many(views, nw, rb, mode, k, err)) return false;
     if (out.size() != n) out.assign(n, FillLaunch{});       // (a second call adds the other variant to the plans of the first)
     for (size_t g = 0; g < n; ++g) {
         FillLaunch& F = out[g];
-        (cols ? F.fn_cols : F.fn) = cols ? k[g].fn_cols : k[g].fn;
+        (mode == 2 ? F.fn_op : mode == 1 ? F.fn_cols : F.fn) = mode == 2 ? k[g].fn_op : mode == 1 ? k[g].fn_cols : k[g].fn;
         F.nw = nw; F.name = n > 1 ? "jit-grouped" : "jit"; F.jit = true;
         F.smem = fill_smem_plan(devs[g], nw, rb, views[g].n_oterm, bra_smem);
-        const int per_sm = jit_prepare(k[g], cols, F.smem.total);
+        const int per_sm = jit_prepare(k[g], mode, F.smem.total);
         if (per_sm < 1) { err = "the compiled kernel does not fit on an SM"; return false; }
         F.grid = n_sm * per_sm;
     }
@@ -144,7 +145,7 @@ bool fill_plan_jit(const std::vector<DevLattice>& devs, std::vector<KetView> vie
 }
 
 cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl,
-                        const int64_t* rowptr, double* vals, int32_t* colidx, int* counter, const int64_t* guard, cudaStream_t st)
+                        const int64_t* rowptr, double* vals, int32_t* colidx, int* counter, const int64_t* guard, cudaStream_t st, bool op_mode)
 {
     const int need = (n_blk + F.nw - 1) / F.nw;                        // one cell per warp at a time
     const int grid = need < F.grid ? need : F.grid;
@@ -155,8 +156,9 @@ cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin
     if (e != cudaSuccess) return e;
     void* args[] = {&Lc, &S, &N, &cell_begin, &n_blk, (void*)&rowptr, &vals, &colidx, &counter, (void*)&guard};
     if (F.jit) {
-        if (jit_prepare_fn(const_cast<void*>(colidx ? F.fn_cols : F.fn), S.total) != 0) return cudaErrorInvalidValue;
-        const int cr = jit_launch(const_cast<void*>(colidx ? F.fn_cols : F.fn), grid, F.nw * 32, S.total, (void*)st, args);
+        void* fn = const_cast<void*>(op_mode ? F.fn_op : colidx ? F.fn_cols : F.fn);
+        if (!fn || jit_prepare_fn(fn, S.total) != 0) return cudaErrorInvalidValue;
+        const int cr = jit_launch(fn, grid, F.nw * 32, S.total, (void*)st, args);
         count_launch();
         return cr == 0 ? cudaGetLastError() : cudaErrorLaunchFailure;
     }

@@ -122,7 +122,11 @@ __device__ __forceinline__ double cell_norm(const double* __restrict__ e, int k,
     return norm ? (e1 * e1 * e1 - e0 * e0 * e0) / 3.0 : e1 - e0;
 }
 
-template <class Spec, int NW, int kRowBatch, bool kCols>
+// kMode: 0 values, 1 values and column indices, 2 the PER-PAIR SUMS: for every hit cell pair (source cell, k-th hit cell) the
+// normalised sums of the group's orbital functions, vals[(cellbase + k) * op_stride + op_off + f] (`rowptr` is then the
+// exclusive scan of the hit counts): the operator form of P0 (every nonzero is a combination of at most four of them) that
+// k_op_expand turns into CSR rows for channel sets filled group by group.
+template <class Spec, int NW, int kRowBatch, int kMode>
 __global__ void __launch_bounds__(NW * 32, 1)
 k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, const int64_t* __restrict__ rowptr,
             double* __restrict__ vals, int32_t* __restrict__ colidx, int* __restrict__ counter, const int64_t* __restrict__ guard)
@@ -131,6 +135,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
     // nnz exceeds the caller's capacity, and then nothing may be written
     if (guard != nullptr && guard[4] != 0) return;
     constexpr int T = NW * 32;
+    constexpr bool kCols = kMode == 1;
     constexpr int NP = (Spec::NS + 1) / 2;              // slot pairs (one double2 per pair and node in the K tile)
     constexpr int NPC = (NP + 31) / 32;                 // pair chunks of the lane = slot-pair walk
     constexpr int NCH = Spec::NCH;                      // function chunks of the lane = function stage
@@ -216,7 +221,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         const int H = nl.hits[cb], nck = nl.nchunk[cb];
         const uint2* __restrict__ g_chunk = nl.chunk + (size_t)cb * L.nnode;      // NodeLists (pm_device.cuh)
         // what only the row phase and the target ends need of the cell waits in shared memory (registers are the limit here)
-        if (lane == 0) { s_cell->rbase = rowptr[(int64_t)cb * L.n_ch]; s_cell->dsrc = cell_norm(L.pe, ci, L.norm) * cell_norm(L.qe, cj, L.norm); s_cell->H = H; }
+        if (lane == 0) { s_cell->rbase = kMode == 2 ? rowptr[cb] : rowptr[(int64_t)cb * L.n_ch]; s_cell->dsrc = cell_norm(L.pe, ci, L.norm) * cell_norm(L.qe, cj, L.norm); s_cell->H = H; }
         {   // the cell's nodes p_a = cp + hp t_a, q_b = cq + hq t_b (the operations of map_node_sq) and weights hp wp_a, hq wq_b
             const CellGeom g = cell_geom(L.pe, L.qe, ci, cj);
             for (int k = lane; k < L.n_p; k += 32) s_p2[k] = make_double2(__dadd_rn(g.cp, __dmul_rn(g.hp, L.tp[k])), __dmul_rn(g.hp, L.wp[k]));
@@ -443,7 +448,16 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                     } else {
                         const int fav = s_fa[ch * 32 + lane], sa = fav & 65535, sb = s_fb[ch * 32 + lane], nM = fav >> 16;
                         double v = 0.0;
-                        for (int i = 0; i < nM; ++i) v = fma(bra[sa + i], s_sseg[sb + i], v);
+                        if constexpr (Spec::kStatic && Spec::MAXM <= 12) {
+                            // all bra harmonics of the function first (they may come from global memory: one latency, not nM)
+                            double bv[Spec::MAXM];
+#pragma unroll
+                            for (int i = 0; i < Spec::MAXM; ++i) bv[i] = i < nM ? bra[sa + i] : 0.0;
+#pragma unroll
+                            for (int i = 0; i < Spec::MAXM; ++i) if (i < nM) v = fma(bv[i], s_sseg[sb + i], v);
+                        } else {
+                            for (int i = 0; i < nM; ++i) v = fma(bra[sa + i], s_sseg[sb + i], v);
+                        }
                         runT[ch] += v;
                     }
                 }
@@ -456,16 +470,27 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                     const int ic = L.mg_Nq ? (int)__umulhi((unsigned)tcell, L.mg_Nq) : tcell, jc = tcell - ic * L.Nq;
                     // (d_i dbar_j d_i' dbar_j')^(-1/2), folded into the sums; rsqrt is within 2 ulp of the oracle's 1/sqrt
                     const double nrm = rsqrt(s_cell->dsrc * (s_dp ? s_dp[ic] * s_dq[jc] : cell_norm(L.pe, ic, L.norm) * cell_norm(L.qe, jc, L.norm)));
+                    if constexpr (kMode == 2) {
+                        double* __restrict__ Ah = vals + (s_cell->rbase + kcur) * (int64_t)L.op_stride + L.op_off;
 #pragma unroll
-                    for (int ch = 0; ch < NCH; ++ch) {
-                        const int f = ch * 32 + lane;
-                        if (f < nf) s_acc[slot * nf + f] = runT[ch] * nrm;
-                        runT[ch] = 0.0;
+                        for (int ch = 0; ch < NCH; ++ch) {
+                            const int f = ch * 32 + lane;
+                            if (f < nf) Ah[f] = runT[ch] * nrm;
+                            runT[ch] = 0.0;
+                        }
+                        ++kcur; kdone = kcur;                              // (nothing waits in the row batch)
+                    } else {
+#pragma unroll
+                        for (int ch = 0; ch < NCH; ++ch) {
+                            const int f = ch * 32 + lane;
+                            if (f < nf) s_acc[slot * nf + f] = runT[ch] * nrm;
+                            runT[ch] = 0.0;
+                        }
+                        if (lane == 0) s_hcol[slot] = tcell * L.n_ch;
+                        ++kcur;
+                        __syncwarp();
+                        if (kcur - kdone == kRowBatch) { write_rows(kdone, kRowBatch); kdone = kcur; }
                     }
-                    if (lane == 0) s_hcol[slot] = tcell * L.n_ch;
-                    ++kcur;
-                    __syncwarp();
-                    if (kcur - kdone == kRowBatch) { write_rows(kdone, kRowBatch); kdone = kcur; }
                 }
             }
             {   // park the running sums

@@ -93,7 +93,7 @@ bool load_driver()
 }
 
 // NVRTC only (no device needed): cubin and the lowered names of the two kernel variants
-bool compile_cubin(const KetView& T, int nw, int rb, int variants, std::vector<char>& cubin, std::string low[2], std::string& err)
+bool compile_cubin(const KetView& T, int nw, int rb, int variants, std::vector<char>& cubin, std::string low[3], std::string& err)
 {
     if (!g_api.ok) { err = g_api.why.empty() ? "NVRTC is not loaded" : g_api.why; return false; }      // (load_nvrtc() ran under the lock)
     const Api& a = g_api;
@@ -109,11 +109,11 @@ bool compile_cubin(const KetView& T, int nw, int rb, int variants, std::vector<c
     nvrtcProgram prog = nullptr;
     nvrtcResult r = a.createProgram(&prog, text.c_str(), "pm_fill_jit.cu", 3, hdr_src, hdr_name);
     if (r != NVRTC_SUCCESS) { err = std::string("nvrtcCreateProgram: ") + a.errString(r); return false; }
-    std::string names[2];
-    for (int c = 0; c < 2; ++c) {
+    std::string names[3];
+    for (int c = 0; c < 3; ++c) {
         if (!(variants & (1 << c))) continue;
         std::ostringstream n;
-        n << "pm::k_fill_warp<pm::gen::Spec_jit, " << nw << ", " << rb << ", " << (c ? "true" : "false") << ">";
+        n << "pm::k_fill_warp<pm::gen::Spec_jit, " << nw << ", " << rb << ", " << c << ">";
         names[c] = n.str();
         a.addName(prog, names[c].c_str());
     }
@@ -132,7 +132,7 @@ bool compile_cubin(const KetView& T, int nw, int rb, int variants, std::vector<c
     a.getCubinSize(prog, &nbin);
     cubin.resize(nbin);
     a.getCubin(prog, cubin.data());
-    for (int c = 0; c < 2; ++c) {
+    for (int c = 0; c < 3; ++c) {
         low[c].clear();
         if (!(variants & (1 << c))) continue;
         const char* l = nullptr;
@@ -155,13 +155,13 @@ bool jit_compile_check(const KetView& V, int nw, int rb, size_t* cubin_bytes, st
         if (!load_nvrtc()) { err = g_api.why; return false; }
     }
     std::vector<char> cubin;
-    std::string low[2];
+    std::string low[3];
     if (!compile_cubin(V, nw, rb, 2, cubin, low, err)) return false;      // the variant pm_build launches
     if (cubin_bytes) *cubin_bytes = cubin.size();
     return !low[1].empty();
 }
 
-bool jit_fill_many(const std::vector<KetView>& views, int nw, int rb, bool cols, std::vector<JitFill>& out, std::string& err)
+bool jit_fill_many(const std::vector<KetView>& views, int nw, int rb, int mode, std::vector<JitFill>& out, std::string& err)
 {
     const size_t n = views.size();
     out.assign(n, JitFill{});
@@ -174,7 +174,7 @@ bool jit_fill_many(const std::vector<KetView>& views, int nw, int rb, bool cols,
         if (load_driver() && g_api.ctxGetDevice) g_api.ctxGetDevice(&dev);
         for (size_t i = 0; i < n; ++i) {
             char key[96];
-            std::snprintf(key, sizeof key, "%d/%016llx/%d/%d/%d/%d/%d", dev, (unsigned long long)views[i].hash, nw, rb, views[i].bra_smem ? 1 : 0, views[i].n_bra > 254 ? 1 : 0, cols ? 1 : 0);
+            std::snprintf(key, sizeof key, "%d/%016llx/%d/%d/%d/%d/%d", dev, (unsigned long long)views[i].hash, nw, rb, views[i].bra_smem ? 1 : 0, views[i].n_bra > 254 ? 1 : 0, mode);
             keys[i] = key;
             auto it = g_cache.find(keys[i]);
             if (it != g_cache.end()) out[i] = it->second; else todo.push_back(i);
@@ -185,16 +185,16 @@ bool jit_fill_many(const std::vector<KetView>& views, int nw, int rb, bool cols,
     }
     // NVRTC runs outside the lock, one host thread per kernel (the programs are independent)
     std::vector<std::vector<char>> cubin(todo.size());
-    std::vector<std::string> low0(todo.size()), low1(todo.size()), errs(todo.size());
+    std::vector<std::string> lowm(todo.size()), errs(todo.size());
     std::vector<char> ok(todo.size(), 0);
     {
         const size_t nt = std::min<size_t>(todo.size(), std::max(1u, std::thread::hardware_concurrency()));
         std::atomic<size_t> next{0};
         auto work = [&] {
             for (size_t j = next++; j < todo.size(); j = next++) {
-                std::string low[2];
-                ok[j] = compile_cubin(views[todo[j]], nw, rb, cols ? 2 : 1, cubin[j], low, errs[j]) ? 1 : 0;
-                low0[j] = low[0]; low1[j] = low[1];
+                std::string low[3];
+                ok[j] = compile_cubin(views[todo[j]], nw, rb, 1 << mode, cubin[j], low, errs[j]) ? 1 : 0;
+                lowm[j] = low[mode];
             }
         };
         std::vector<std::thread> th;
@@ -213,8 +213,8 @@ bool jit_fill_many(const std::vector<KetView>& views, int nw, int rb, bool cols,
         k.nw = nw; k.rb = rb;
         if (cr == CUDA_SUCCESS) {
             CUfunction f = nullptr;
-            cr = a.moduleGetFunction(&f, mod, (cols ? low1[j] : low0[j]).c_str());
-            (cols ? k.fn_cols : k.fn) = f;
+            cr = a.moduleGetFunction(&f, mod, lowm[j].c_str());
+            (mode == 2 ? k.fn_op : mode == 1 ? k.fn_cols : k.fn) = f;
         }
         if (cr != CUDA_SUCCESS) { err = "loading the compiled kernel failed (CUresult " + std::to_string((int)cr) + ")"; return false; }
         g_cache[keys[todo[j]]] = k;                  // the module stays loaded for the life of the process
@@ -223,10 +223,10 @@ bool jit_fill_many(const std::vector<KetView>& views, int nw, int rb, bool cols,
     return true;
 }
 
-bool jit_fill(const KetView& V, int nw, int rb, bool cols, JitFill* out, std::string& err)
+bool jit_fill(const KetView& V, int nw, int rb, int mode, JitFill* out, std::string& err)
 {
     std::vector<JitFill> r;
-    if (!jit_fill_many(std::vector<KetView>{V}, nw, rb, cols, r, err)) return false;
+    if (!jit_fill_many(std::vector<KetView>{V}, nw, rb, mode, r, err)) return false;
     *out = r[0];
     return true;
 }
@@ -242,10 +242,10 @@ int jit_prepare_fn(void* fn, int smem_bytes)
     return 0;
 }
 
-int jit_prepare(const JitFill& k, bool cols, int smem_bytes)
+int jit_prepare(const JitFill& k, int mode, int smem_bytes)
 {
     if (!g_api.ok_cu) return 0;
-    CUfunction f = (CUfunction)(cols ? k.fn_cols : k.fn);
+    CUfunction f = (CUfunction)(mode == 2 ? k.fn_op : mode == 1 ? k.fn_cols : k.fn);
     if (jit_prepare_fn((void*)f, smem_bytes) != 0) return 0;
     int per_sm = 0;
     if (g_api.occupancy(&per_sm, f, k.nw * 32, (size_t)smem_bytes) != CUDA_SUCCESS) return 0;

@@ -17,8 +17,9 @@
 namespace pm {
 
 struct JitFill {
-    void* fn = nullptr;        // CUfunction of k_fill_warp<Spec_jit, nw, rb, false>, or NULL (compiled when first needed)
-    void* fn_cols = nullptr;   // ... <..., true>
+    void* fn = nullptr;        // CUfunction of k_fill_warp<Spec_jit, nw, rb, 0>, or NULL (compiled when first needed)
+    void* fn_cols = nullptr;   // ... <..., 1>: values and column indices
+    void* fn_op = nullptr;     // ... <..., 2>: per-pair sums (pm_fill.cuh)
     int nw = 0, rb = 0;
 };
 
@@ -26,18 +27,18 @@ struct JitFill {
 void jit_set_enabled(bool on);
 bool jit_enabled();
 
-// Compiles (or fetches from the cache) ONE kernel variant (cols: the one that also writes column indices; the other
-// member of JitFill stays NULL) for the ket tables in V with `nw` warps and row batch `rb`.  Returns false and a message if NVRTC / the driver API is unavailable or the compilation fails.
-bool jit_fill(const KetView& V, int nw, int rb, bool cols, JitFill* out, std::string& err);
+// Compiles (or fetches from the cache) ONE kernel variant (mode 0 values, 1 values and column indices, 2 per-pair sums;
+// the other members of JitFill stay NULL) for the ket tables in V with `nw` warps and row batch `rb`.  Returns false and a message if NVRTC / the driver API is unavailable or the compilation fails.
+bool jit_fill(const KetView& V, int nw, int rb, int mode, JitFill* out, std::string& err);
 // The same for several kernels at once (the column-channel groups of a big channel set): the NVRTC compilations run
 // on one host thread each, the modules are loaded by the caller's thread.
-bool jit_fill_many(const std::vector<KetView>& views, int nw, int rb, bool cols, std::vector<JitFill>& out, std::string& err);
+bool jit_fill_many(const std::vector<KetView>& views, int nw, int rb, int mode, std::vector<JitFill>& out, std::string& err);
 
 // NVRTC only, no device needed: does the kernel for V compile for sm_100a?  (diagnostic, CPU tests)
 bool jit_compile_check(const KetView& V, int nw, int rb, size_t* cubin_bytes, std::string& err);
 
 // cuFuncSetAttribute(max dynamic shared memory) + occupancy; returns CTAs per SM (0 on error)
-int jit_prepare(const JitFill& k, bool cols, int smem_bytes);
+int jit_prepare(const JitFill& k, int mode, int smem_bytes);
 
 // Raises (never lowers) the dynamic shared-memory limit of a run-time compiled function to at least `smem_bytes`;
 // returns 0 on success.  Called before every launch: the function is shared by all lattices with the same tables.

@@ -290,37 +290,41 @@ k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl,
 // Pattern pass, kernel S: exclusive scan of the hit counts -> cellbase, nnz, max hits, nodes on the grid.  One CTA;
 // thread = a contiguous run of cells (one load phase, one block scan, one store phase).
 __global__ void __launch_bounds__(1024) k_scan_cells(DevLattice L, int n_blk, const int* __restrict__ hits,
-                                                    const int* __restrict__ ntot, int64_t* __restrict__ cellbase,
-                                                    int64_t* __restrict__ summary, int64_t capacity)
+                                                    const int* __restrict__ ntot, const int* __restrict__ nchunk,
+                                                    int64_t* __restrict__ cellbase, int64_t* __restrict__ summary, int64_t capacity)
 {
-    __shared__ long long wsum[32], wnod[32];
+    __shared__ long long wsum[32], wnod[32], wchk[32];
     __shared__ int wmax[32];
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
     const int chunk = (n_blk + 1023) >> 10;
     const int k0 = min(t * chunk, n_blk), k1 = min(k0 + chunk, n_blk);
-    long long mine = 0, nodes = 0;
+    long long mine = 0, nodes = 0, chunks = 0;
     int mx = 0;
-    for (int k = k0; k < k1; ++k) { const int h = hits[k]; mine += h; mx = max(mx, h); nodes += ntot[k]; }
+    for (int k = k0; k < k1; ++k) { const int h = hits[k]; mine += h; mx = max(mx, h); nodes += ntot[k]; chunks += nchunk[k]; }
     long long x = mine;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) { const long long y = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += y; }
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) { nodes += __shfl_xor_sync(0xffffffffu, nodes, d); mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, d)); }
+    for (int d = 16; d > 0; d >>= 1) {
+        nodes += __shfl_xor_sync(0xffffffffu, nodes, d); chunks += __shfl_xor_sync(0xffffffffu, chunks, d);
+        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+    }
     if (lane == 31) wsum[warp] = x;
-    if (lane == 0) { wnod[warp] = nodes; wmax[warp] = mx; }
+    if (lane == 0) { wnod[warp] = nodes; wchk[warp] = chunks; wmax[warp] = mx; }
     __syncthreads();
     long long carry = 0;
     for (int w = 0; w < warp; ++w) carry += wsum[w];
     long long run = carry + x - mine;
     for (int k = k0; k < k1; ++k) { cellbase[k] = run; run += hits[k]; }
     if (t == 1023) {
-        long long nn = 0; int m = 0;
-        for (int w = 0; w < 32; ++w) { nn += wnod[w]; m = max(m, wmax[w]); }
+        long long nn = 0, nc = 0; int m = 0;
+        for (int w = 0; w < 32; ++w) { nn += wnod[w]; nc += wchk[w]; m = max(m, wmax[w]); }
         const long long total = carry + x;
         cellbase[n_blk] = total;
         summary[0] = total * L.totcoup;                 // nnz of the block
         summary[1] = m;                                 // max hit cells of any source cell
         summary[2] = nn;                                // nodes on the grid
+        summary[5] = nc;                                // chunks of the sorted node lists (8 B each, read once by the fill)
         summary[4] = (capacity >= 0 && total * L.totcoup > capacity) ? 1 : 0;      // the fill of pm_build must not run
     }
 }
@@ -380,6 +384,98 @@ __global__ void __launch_bounds__(kThreads) k_count_segments(DevLattice L, int n
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) seg += __shfl_xor_sync(0xffffffffu, seg, d);
     if (lane == 0 && seg) atomicAdd(total, seg);
+}
+
+// CSR rows from the per-pair sums (pm_fill.cuh, mode 2), for channel sets whose fill runs group by group: every nonzero
+// of (source cell, k-th hit cell) is a combination of at most four of the pair's sums,
+//   P[(cell, alpha), (cell_k, alpha')] = sum_i xc[4 o + i] * A[(cellbase + k) * stride + xpos[4 o + i]],   o = cl_off[alpha] + m.
+// One warp per source cell; the pair's sums wait in shared memory, lane = output, and a warp store covers consecutive
+// alpha' of one row: every 32-byte sector of vals / colidx is written once, in full (group-by-group fills of the CSR would
+// write a few entries of every sector per group, which DRAM pays with a read-modify-write each time).
+struct ExpandSmem { int odesc, xpos, xc, warp0, warp_bytes, total; };
+
+__global__ void __launch_bounds__(512, 1)
+k_op_expand(DevLattice L, ExpandSmem S, int cell_begin, int n_blk, const int* __restrict__ hits, const int64_t* __restrict__ cellbase,
+            const int* __restrict__ hitlist, const double* __restrict__ A, const unsigned short* __restrict__ g_xpos,
+            const double* __restrict__ g_xc, const int64_t* __restrict__ rowptr, double* __restrict__ vals,
+            int32_t* __restrict__ colidx, int* __restrict__ counter, const int64_t* __restrict__ guard)
+{
+    if (guard != nullptr && guard[4] != 0) return;
+    extern __shared__ __align__(16) char smem[];
+    const int T = blockDim.x, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    int* s_odesc = (int*)(smem + S.odesc);                      // cl_off[alpha] | nc << 12 | m << 19 | alpha' << 25
+    uint2* s_xpos = (uint2*)(smem + S.xpos);                    // four positions of 16 bits
+    double* s_xc = (double*)(smem + S.xc);                      // [o][4]
+    double* s_A = (double*)(smem + S.warp0 + warp * S.warp_bytes);      // the sums of two hit cell pairs
+    const int nout = L.totcoup, stride = L.op_stride;
+    for (int o = tid; o < nout; o += T) {
+        const int al = L.o_alpha[o], off = L.cl_off[al], nc = L.cl_off[al + 1] - off;
+        s_odesc[o] = off | (nc << 12) | ((o - off) << 19) | (L.cl[o] << 25);
+        s_xpos[o] = make_uint2((unsigned)g_xpos[4 * o] | ((unsigned)g_xpos[4 * o + 1] << 16), (unsigned)g_xpos[4 * o + 2] | ((unsigned)g_xpos[4 * o + 3] << 16));
+        for (int i = 0; i < 4; ++i) s_xc[4 * o + i] = g_xc[4 * o + i];
+    }
+    __syncthreads();
+    for (;;) {
+        int cb = 0;
+        if (lane == 0) cb = atomicAdd(counter, 1);
+        cb = __shfl_sync(0xffffffffu, cb, 0);
+        if (cb >= n_blk) break;
+        const int H = hits[cb];
+        const int64_t hbase = cellbase[cb], rbase = rowptr[(int64_t)cb * L.n_ch];
+        double* __restrict__ row0 = vals + rbase;
+        int32_t* __restrict__ col0 = colidx ? colidx + rbase : nullptr;
+        for (int k0 = 0; k0 < H; k0 += 2) {
+            const int nb = min(2, H - k0);
+            const double* __restrict__ Ak = A + (hbase + k0) * (int64_t)stride;
+            for (int i = lane; i < nb * stride; i += 32) s_A[i] = Ak[i];
+            const int t0 = hitlist[hbase + k0] * L.n_ch, t1 = nb > 1 ? hitlist[hbase + k0 + 1] * L.n_ch : 0;
+            __syncwarp();
+#pragma unroll 2
+            for (int o = lane; o < nout; o += 32) {
+                const int od = s_odesc[o];
+                const uint2 xp = s_xpos[o];
+                const double c0 = s_xc[4 * o], c1 = s_xc[4 * o + 1], c2 = s_xc[4 * o + 2], c3 = s_xc[4 * o + 3];
+                const int clo = od & 4095, nc = (od >> 12) & 127, mm = (od >> 19) & 63, ap = (unsigned)od >> 25;
+                const unsigned p0 = xp.x & 65535u, p1 = xp.x >> 16, p2 = xp.y & 65535u, p3 = xp.y >> 16;
+                const unsigned e = (unsigned)(H * clo + k0 * nc + mm);
+                {
+                    const double v = fma(c3, s_A[p3], fma(c2, s_A[p2], fma(c1, s_A[p1], c0 * s_A[p0])));
+                    row0[e] = v;
+                    if (col0) col0[e] = t0 + ap;
+                }
+                if (nb > 1) {
+                    const double* A1 = s_A + stride;
+                    const double v = fma(c3, A1[p3], fma(c2, A1[p2], fma(c1, A1[p1], c0 * A1[p0])));
+                    row0[e + nc] = v;
+                    if (col0) col0[e + nc] = t1 + ap;
+                }
+            }
+            __syncwarp();
+        }
+    }
+}
+
+cudaError_t launch_op_expand(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, const int64_t* cellbase, const int* hitlist,
+                             const double* A, const unsigned short* xpos, const double* xc, const int64_t* rowptr, double* vals,
+                             int32_t* colidx, int* counter, const int64_t* guard, int n_sm, cudaStream_t st)
+{
+    ExpandSmem S{};
+    int o = 0;
+    auto take = [&](size_t bytes) { int r = o; o += (int)al16(bytes); return r; };
+    S.odesc = take(4 * (size_t)L.totcoup); S.xpos = take(8 * (size_t)L.totcoup); S.xc = take(32 * (size_t)L.totcoup);
+    S.warp_bytes = (int)al16(2 * 8 * (size_t)L.op_stride);
+    const int limit = 227 * 1024;
+    int nw = std::min(16, (limit - o) / std::max(S.warp_bytes, 16));
+    if (nw < 1) return cudaErrorInvalidConfiguration;
+    S.warp0 = take((size_t)S.warp_bytes * nw);
+    S.total = o;
+    cudaError_t e = cudaFuncSetAttribute((const void*)k_op_expand, cudaFuncAttributeMaxDynamicSharedMemorySize, limit);
+    if (e != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(counter, 0, sizeof(int), st)) != cudaSuccess) return e;
+    const int grid = std::max(1, std::min(n_sm, (n_blk + nw - 1) / nw));
+    k_op_expand<<<grid, nw * 32, S.total, st>>>(L, S, cell_begin, n_blk, nl.hits, cellbase, hitlist, A, xpos, xc, rowptr, vals, colidx, counter, guard);
+    count_launch();
+    return cudaGetLastError();
 }
 
 // Pattern pass, kernel B: column indices, ascending within each row, from the hit lists.  Thread = output (alpha, m-th
@@ -501,7 +597,7 @@ cudaError_t launch_map_sort(const DevLattice& L, int cell_begin, int n_blk, cons
 cudaError_t launch_scan_rows(const DevLattice& L, int n_blk, const NodeLists& nl, int64_t* cellbase, int64_t* rowptr,
                              int64_t* summary, int64_t capacity, cudaStream_t st)
 {
-    k_scan_cells<<<1, 1024, 0, st>>>(L, n_blk, nl.hits, nl.ntot, cellbase, summary, capacity);
+    k_scan_cells<<<1, 1024, 0, st>>>(L, n_blk, nl.hits, nl.ntot, nl.nchunk, cellbase, summary, capacity);
     ++g_launches;
     const int64_t n = (int64_t)n_blk * L.n_ch + 1;
     k_write_rowptr<<<(unsigned)std::min<int64_t>((n + 255) / 256, 148 * 8), 256, 0, st>>>(L, n_blk, nl.hits, cellbase, rowptr);

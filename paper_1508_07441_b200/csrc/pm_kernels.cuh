@@ -34,17 +34,22 @@ cudaError_t launch_emit_cols(const DevLattice& L, int n_blk, const NodeLists& nl
 cudaError_t launch_count_segments(const DevLattice& L, int n_blk, const NodeLists& nl, unsigned long long* total, cudaStream_t st);
 
 // fill pass (pm_fill.cuh): variant selection and launch
-struct FillLaunch { const void *fn, *fn_cols; int nw, grid; FillSmem smem; const char* name; bool jit; };   // fn_cols also writes colidx;
+struct FillLaunch { const void *fn, *fn_cols, *fn_op; int nw, grid; FillSmem smem; const char* name; bool jit; };   // fn_cols also writes colidx;
                                                       // jit: fn / fn_cols are CUfunction handles of run-time compiled kernels (pm_jit.hpp)
 bool fill_has_spec(unsigned long long tables_hash);
 const char* fill_variant_name(unsigned long long tables_hash);
 cudaError_t fill_plan(const DevLattice& L, unsigned long long tables_hash, int n_sm, FillLaunch* out);
 // run-time compiled kernels for the column-channel groups of one lattice (no build-time kernel): false + message when
 // NVRTC / the driver API fails
-bool fill_plan_jit(const std::vector<DevLattice>& devs, std::vector<KetView> views, int n_sm, bool cols, std::vector<FillLaunch>& out, std::string& err);
+bool fill_plan_jit(const std::vector<DevLattice>& devs, std::vector<KetView> views, int n_sm, int mode, std::vector<FillLaunch>& out, std::string& err);
 cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin, int n_blk, const NodeLists& nl,
-                        const int64_t* rowptr, double* vals, int32_t* colidx, int* counter, const int64_t* guard, cudaStream_t st);
+                        const int64_t* rowptr, double* vals, int32_t* colidx, int* counter, const int64_t* guard, cudaStream_t st,
+                        bool op_mode = false);      // op_mode: the per-pair sums variant (rowptr = scan of the hit counts, vals = the sums)
 
+// CSR rows (values and, if colidx, column indices) from the per-pair sums A of a whole channel set (pm_kernels.cu)
+cudaError_t launch_op_expand(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, const int64_t* cellbase, const int* hitlist,
+                             const double* A, const unsigned short* xpos, const double* xc, const int64_t* rowptr, double* vals,
+                             int32_t* colidx, int* counter, const int64_t* guard, int n_sm, cudaStream_t st);
 cudaError_t launch_hit_list(const DevLattice& L, int n_blk, const NodeLists& nl, const int64_t* cellbase, int* hitlist, cudaStream_t st);
 cudaError_t launch_spmv_implicit(const DevLattice& L, int64_t n_rows, const int64_t* rowptr, const int* hits, const int64_t* cellbase,
                                  const int* hitlist, const double* vals, const double* x, double* y, cudaStream_t st);

@@ -376,6 +376,7 @@ void build_groups(const Tables& T, const pm_channel* ch, int max_slot, int max_f
         OrbFun L = F;
         L.sb0 = slot_local[(size_t)F.sb0];
         G.fun.push_back(L);
+        G.f_global.push_back(f);
     }
     for (int g = 0; g < n_grp; ++g) groups[(size_t)g].ot_off.assign(1, 0);
     for (int a = 0; a < T.n_ch; ++a)

@@ -49,6 +49,7 @@ struct GroupTables {
     std::vector<int32_t> kt_off, kt_ip, kt_iq;        // ket terms per local slot
     std::vector<double> kt_c;
     std::vector<OrbFun> fun;                          // sa0: GLOBAL bra slot, sb0: LOCAL ket slot
+    std::vector<int32_t> f_global;                    // index in Tables::fun of each local function
     std::vector<int32_t> o_alpha, o_m, o_ap;          // outputs: row channel, position in the row's coupled list, column channel;
                                                       // rows ordered by the most terms of their outputs
     int n_out1 = 0, n_out2 = 0, n_out3 = 0;           // outputs in rows with at most one / two / three terms per output
