@@ -92,7 +92,7 @@ int32_t pm_lattice_coupling(const pm_lattice* lat, uint8_t* coupled, int32_t* n_
 /* Pattern pass (the paper's step 2a 'pre-selection') for the rows of source cells
  * [cell_begin, cell_end):
  * The pass bins every quadrature node of the range once and keeps, in library-owned device memory, the node lists
- * sorted by target cell (about 8 bytes per node); pm_fill of the same range reads them.  Calling with d_colidx = NULL
+ * sorted by target cell (about 12 bytes per node: keys and chunk words); pm_fill of the same range reads them.  Calling with d_colidx = NULL
  * (count) and then with d_colidx for the same range maps the nodes only once.
  *   d_rowptr : device, (cell_end-cell_begin)*n_ch + 1 int64, block-local (d_rowptr[0] = 0)
  *   d_colidx : device, nnz int32 GLOBAL column indices — or NULL to count only (d_rowptr is still written)
@@ -214,11 +214,13 @@ int32_t pm_pattern_counts(const pm_lattice* lat, int64_t* nodes_on_grid, int64_t
 int32_t pm_pattern_chunks(const pm_lattice* lat, int64_t* chunks);
 
 /* Name of the fill kernel this lattice's channel set selects: "Spec_<set>" when csrc/build.py generated straight-line
- * ket code for it at build time (the channel sets of BASELINE.json's configs); "jit" when the same kind of code is
- * generated from the lattice's tables and compiled with NVRTC at the first fill (any other channel set; needs
- * libnvrtc and the CUDA driver at run time, about a second once per channel set and process); "generic" for the
- * table-driven kernel used when run-time compilation is switched off or failed.  All three give the same results
- * within the value tolerance and the same pattern.  Host only; library-owned string, never NULL. */
+ * ket code for it at build time (the channel sets of BASELINE.json's configs, in any channel order); "jit" when the same
+ * kind of code is generated from the lattice's tables and compiled with NVRTC at the first fill (any other channel set
+ * of at most 40 ket slots; needs libnvrtc and the CUDA driver at run time, 2-4 s once per channel set, variant and
+ * process); "jit-grouped" for bigger sets (46-62 channels), whose column-channel groups get one such kernel each and
+ * whose CSR rows are assembled from the groups' per-pair sums; "generic" / "generic-grouped" for the
+ * table-driven kernel used when run-time compilation is switched off or failed.  All give the same pattern and the same
+ * results within the value tolerance.  Host only; library-owned string, never NULL. */
 const char* pm_lattice_fill_kernel(const pm_lattice* lat);
 
 /* Switches run-time compilation on (default, unless the environment variable PM_NO_JIT is set) or off for lattices
@@ -226,8 +228,8 @@ const char* pm_lattice_fill_kernel(const pm_lattice* lat);
 int32_t pm_set_jit(int32_t enabled);
 
 /* Diagnostic (host only, no GPU needed): generates this lattice's run-time kernel source and compiles it with NVRTC
- * for sm_100a; *cubin_bytes receives the size of the binary.  PM_ERR_STATE with the compiler log as message on failure
- * (also when libnvrtc cannot be loaded). */
+ * for sm_100a (every column-channel group of a "jit-grouped" set, one after the other); *cubin_bytes receives the total
+ * size of the binaries.  PM_ERR_STATE with the compiler log as message on failure (also when libnvrtc cannot be loaded). */
 int32_t pm_diag_jit_compile(const pm_lattice* lat, int64_t* cubin_bytes);
 
 /* Diagnostic (host only): the smallest double y with sqrt(y) >= edge under IEEE round-to-nearest — the threshold
