@@ -373,6 +373,9 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
             const int cnt = min(32, nck - base);
             double runT[NCH];
             double2 runS[NPC];
+            int fa[NCH], fb[NCH];                       // this lane's function descriptors, for the step's segment ends (the ket
+#pragma unroll                                          // code's accumulators are dead here: registers are free)
+            for (int ch = 0; ch < NCH; ++ch) { fa[ch] = s_fa[ch * 32 + lane]; fb[ch] = s_fb[ch * 32 + lane]; }
             {
                 const int slot = kcur - kdone;
 #pragma unroll
@@ -440,13 +443,13 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
 #pragma unroll
                 for (int ch = 0; ch < NCH; ++ch) {
                     if (kPacked) {
-                        const int ia = s_fa[ch * 32 + lane], ib = s_fb[ch * 32 + lane];
+                        const int ia = fa[ch], ib = fb[ch];
                         double v = bra[ia & 255] * s_sseg[ib & 255];
                         if (Spec::terms(ch) > 1) v = fma(bra[(ia >> 8) & 255], s_sseg[(ib >> 8) & 255], v);
                         if (Spec::terms(ch) > 2) v = fma(bra[ia >> 16], s_sseg[ib >> 16], v);
                         runT[ch] += v;
                     } else {
-                        const int fav = s_fa[ch * 32 + lane], sa = fav & 65535, sb = s_fb[ch * 32 + lane], nM = fav >> 16;
+                        const int fav = fa[ch], sa = fav & 65535, sb = fb[ch], nM = fav >> 16;
                         double v = 0.0;
                         if constexpr (Spec::kStatic && Spec::MAXM <= 12) {
                             // all bra harmonics of the function first (they may come from global memory: one latency, not nM)
