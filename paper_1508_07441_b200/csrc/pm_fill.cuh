@@ -148,7 +148,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
     double* s_bra = (double*)(smem + (S.bra >= 0 ? S.bra : 0));
     int* s_odesc = (int*)(smem + S.odesc);             // per output o: cl_off[alpha] | nc << 12 | m << 19 | alpha' << 25
     int* s_ofi = (int*)(smem + S.ofi);                 // f0 | f1 << 10 | f2 << 20 | (n_terms - 1) << 30, or four f of 8 bits
-    double* s_oc = (double*)(smem + S.oc);             // [o][NOT] coefficients c^L (0 where there is no term)
+    double* s_oc = (double*)(smem + S.oc);             // [NOT][n_out] coefficients c^L, term-major: consecutive lanes read consecutive doubles (0 where there is no term)
     char* wsm = smem + S.warp0 + warp * S.warp_bytes;
     // compile-time offsets for a specialised kernel (the host plan computes the same numbers from the lattice's tables)
     constexpr WarpLayout kW = warp_layout(NP, Spec::NF, kRowBatch);
@@ -184,7 +184,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         s_odesc[o] = off | (nc << 12) | (L.g_m[o] << 19) | (L.g_ap[o] << 25);
         int fi = NOT == 3 ? (nt > 0 ? nt - 1 : 0) << 30 : 0;
         for (int i = 0; i < NOT; ++i) {
-            s_oc[NOT * o + i] = i < nt ? L.ot_c[t0 + i] : 0.0;
+            s_oc[i * L.n_out + o] = i < nt ? L.ot_c[t0 + i] : 0.0;
             fi |= (i < nt ? L.ot_f[t0 + i] : 0) << ((NOT == 3 ? 10 : 8) * i);
         }
         s_ofi[o] = fi;
@@ -247,8 +247,8 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                 for (int o = o_begin + lane; o < o_end; o += 32) {
                     const int od = s_odesc[o], fi = s_ofi[o];
                     const int clo = od & 4095, nc = (od >> 12) & 127, mm = (od >> 19) & 63, ap = (unsigned)od >> 25;
-                    const double c0 = s_oc[NOT * o], c1 = NT > 1 ? s_oc[NOT * o + 1] : 0.0, c2 = NT > 2 ? s_oc[NOT * o + 2] : 0.0,
-                                 c3 = NT > 3 ? s_oc[NOT * o + 3] : 0.0;
+                    const double c0 = s_oc[o], c1 = NT > 1 ? s_oc[L.n_out + o] : 0.0, c2 = NT > 2 ? s_oc[2 * L.n_out + o] : 0.0,
+                                 c3 = NT > 3 ? s_oc[3 * L.n_out + o] : 0.0;
                     constexpr int FB = NOT == 3 ? 10 : 8, FM = (1 << FB) - 1;
                     const int f0 = fi & FM, f1 = (fi >> FB) & FM, f2 = (fi >> (2 * FB)) & FM, f3 = NOT > 3 ? (int)((unsigned)fi >> 24) : 0;
                     // entry of target k0+bb in row alpha: element H*clo + (k0+bb)*nc + m of the cell's block (fits 32 bits)

@@ -389,68 +389,93 @@ __global__ void __launch_bounds__(kThreads) k_count_segments(DevLattice L, int n
 // CSR rows from the per-pair sums (pm_fill.cuh, mode 2), for channel sets whose fill runs group by group: every nonzero
 // of (source cell, k-th hit cell) is a combination of at most four of the pair's sums,
 //   P[(cell, alpha), (cell_k, alpha')] = sum_i xc[4 o + i] * A[(cellbase + k) * stride + xpos[4 o + i]],   o = cl_off[alpha] + m.
-// One warp per source cell; the pair's sums wait in shared memory, lane = output, and a warp store covers consecutive
-// alpha' of one row: every 32-byte sector of vals / colidx is written once, in full (group-by-group fills of the CSR would
-// write a few entries of every sector per group, which DRAM pays with a read-modify-write each time).
-struct ExpandSmem { int odesc, xpos, xc, warp0, warp_bytes, total; };
+// One CTA of 16 warps per source cell (cells from a work counter).  Every thread keeps the terms of its kOPL outputs in
+// REGISTERS for the life of the kernel (output o = (warp * kOPL + j) * 32 + lane: a warp store covers consecutive alpha'
+// of a row); the sums of kExpandTB hit cell pairs at a time arrive in shared memory by cp.async, double buffered.  Every
+// 32-byte sector of vals / colidx is written once, in full (group-by-group fills of the CSR would write a few entries of
+// every sector per group, which DRAM pays with a read-modify-write each time).
+constexpr int kExpandWarps = 16, kExpandTB = 4;
 
-__global__ void __launch_bounds__(512, 1)
-k_op_expand(DevLattice L, ExpandSmem S, int cell_begin, int n_blk, const int* __restrict__ hits, const int64_t* __restrict__ cellbase,
+template <int kOPL>
+__global__ void __launch_bounds__(kExpandWarps * 32, 1)
+k_op_expand(DevLattice L, int cell_begin, int n_blk, const int* __restrict__ hits, const int64_t* __restrict__ cellbase,
             const int* __restrict__ hitlist, const double* __restrict__ A, const unsigned short* __restrict__ g_xpos,
             const double* __restrict__ g_xc, const int64_t* __restrict__ rowptr, double* __restrict__ vals,
             int32_t* __restrict__ colidx, int* __restrict__ counter, const int64_t* __restrict__ guard)
 {
     if (guard != nullptr && guard[4] != 0) return;
     extern __shared__ __align__(16) char smem[];
-    const int T = blockDim.x, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    int* s_odesc = (int*)(smem + S.odesc);                      // cl_off[alpha] | nc << 12 | m << 19 | alpha' << 25
-    uint2* s_xpos = (uint2*)(smem + S.xpos);                    // four positions of 16 bits
-    double* s_xc = (double*)(smem + S.xc);                      // [o][4]
-    double* s_A = (double*)(smem + S.warp0 + warp * S.warp_bytes);      // the sums of two hit cell pairs
-    const int nout = L.totcoup, stride = L.op_stride;
-    for (int o = tid; o < nout; o += T) {
-        const int al = L.o_alpha[o], off = L.cl_off[al], nc = L.cl_off[al + 1] - off;
-        s_odesc[o] = off | (nc << 12) | ((o - off) << 19) | (L.cl[o] << 25);
-        s_xpos[o] = make_uint2((unsigned)g_xpos[4 * o] | ((unsigned)g_xpos[4 * o + 1] << 16), (unsigned)g_xpos[4 * o + 2] | ((unsigned)g_xpos[4 * o + 3] << 16));
-        for (int i = 0; i < 4; ++i) s_xc[4 * o + i] = g_xc[4 * o + i];
+    constexpr int T = kExpandWarps * 32;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int nout = L.totcoup, stride = L.op_stride;           // stride: a multiple of 4 doubles
+    double* s_A = (double*)smem;                                // [2][kExpandTB][stride]
+    int* s_col = (int*)(smem + 2 * kExpandTB * stride * 8);     // [2][kExpandTB] first column of the batch's hit cells
+    __shared__ int s_cb;
+    // this thread's outputs: row offsets, column channel, positions and coefficients of up to four terms
+    int od[kOPL];                                               // cl_off[alpha] | nc << 12 | m << 19 | alpha' << 25; -1: no output
+    unsigned px[kOPL], py[kOPL];
+    double c0[kOPL], c1[kOPL], c2[kOPL], c3[kOPL];
+#pragma unroll
+    for (int j = 0; j < kOPL; ++j) {
+        const int o = (warp * kOPL + j) * 32 + lane;
+        od[j] = -1; px[j] = py[j] = 0u; c0[j] = c1[j] = c2[j] = c3[j] = 0.0;
+        if (o < nout) {
+            const int al = L.o_alpha[o], off = L.cl_off[al], nc = L.cl_off[al + 1] - off;
+            od[j] = off | (nc << 12) | ((o - off) << 19) | (L.cl[o] << 25);
+            px[j] = (unsigned)g_xpos[4 * o] | ((unsigned)g_xpos[4 * o + 1] << 16);
+            py[j] = (unsigned)g_xpos[4 * o + 2] | ((unsigned)g_xpos[4 * o + 3] << 16);
+            c0[j] = g_xc[4 * o]; c1[j] = g_xc[4 * o + 1]; c2[j] = g_xc[4 * o + 2]; c3[j] = g_xc[4 * o + 3];
+        }
     }
-    __syncthreads();
+    const unsigned sA0 = (unsigned)__cvta_generic_to_shared(s_A);
     for (;;) {
-        int cb = 0;
-        if (lane == 0) cb = atomicAdd(counter, 1);
-        cb = __shfl_sync(0xffffffffu, cb, 0);
+        __syncthreads();
+        if (tid == 0) s_cb = atomicAdd(counter, 1);
+        __syncthreads();
+        const int cb = s_cb;
         if (cb >= n_blk) break;
         const int H = hits[cb];
         const int64_t hbase = cellbase[cb], rbase = rowptr[(int64_t)cb * L.n_ch];
         double* __restrict__ row0 = vals + rbase;
         int32_t* __restrict__ col0 = colidx ? colidx + rbase : nullptr;
-        for (int k0 = 0; k0 < H; k0 += 2) {
-            const int nb = min(2, H - k0);
-            const double* __restrict__ Ak = A + (hbase + k0) * (int64_t)stride;
-            for (int i = lane; i < nb * stride; i += 32) s_A[i] = Ak[i];
-            const int t0 = hitlist[hbase + k0] * L.n_ch, t1 = nb > 1 ? hitlist[hbase + k0 + 1] * L.n_ch : 0;
-            __syncwarp();
-#pragma unroll 2
-            for (int o = lane; o < nout; o += 32) {
-                const int od = s_odesc[o];
-                const uint2 xp = s_xpos[o];
-                const double c0 = s_xc[4 * o], c1 = s_xc[4 * o + 1], c2 = s_xc[4 * o + 2], c3 = s_xc[4 * o + 3];
-                const int clo = od & 4095, nc = (od >> 12) & 127, mm = (od >> 19) & 63, ap = (unsigned)od >> 25;
-                const unsigned p0 = xp.x & 65535u, p1 = xp.x >> 16, p2 = xp.y & 65535u, p3 = xp.y >> 16;
-                const unsigned e = (unsigned)(H * clo + k0 * nc + mm);
-                {
-                    const double v = fma(c3, s_A[p3], fma(c2, s_A[p2], fma(c1, s_A[p1], c0 * s_A[p0])));
-                    row0[e] = v;
-                    if (col0) col0[e] = t0 + ap;
-                }
-                if (nb > 1) {
-                    const double* A1 = s_A + stride;
-                    const double v = fma(c3, A1[p3], fma(c2, A1[p2], fma(c1, A1[p1], c0 * A1[p0])));
-                    row0[e + nc] = v;
-                    if (col0) col0[e + nc] = t1 + ap;
+        // batch b of the cell's hit cell pairs -> buffer b & 1 (16-byte cp.async pieces; the pairs' sums are contiguous)
+        auto fetch = [&](int b) {
+            const int k0 = b * kExpandTB, nb = min(kExpandTB, H - k0);
+            if (nb > 0) {
+                const double* src = A + (hbase + k0) * (int64_t)stride;
+                const unsigned dst = sA0 + (unsigned)((b & 1) * kExpandTB * stride * 8);
+                for (int i = tid; i < nb * stride / 2; i += T)
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + 16u * i), "l"(src + 2 * i) : "memory");
+                if (tid < nb) s_col[(b & 1) * kExpandTB + tid] = hitlist[hbase + k0 + tid] * L.n_ch;
+            }
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        };
+        const int nbatch = (H + kExpandTB - 1) / kExpandTB;
+        fetch(0);
+        for (int b = 0; b < nbatch; ++b) {
+            fetch(b + 1);
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+            __syncthreads();
+            const int k0 = b * kExpandTB, nb = min(kExpandTB, H - k0);
+            const double* Ab = s_A + (b & 1) * kExpandTB * stride;
+            const int* colb = s_col + (b & 1) * kExpandTB;
+#pragma unroll
+            for (int j = 0; j < kOPL; ++j) {
+                if (od[j] < 0) continue;
+                const int clo = od[j] & 4095, nc = (od[j] >> 12) & 127, mm = (od[j] >> 19) & 63, ap = (unsigned)od[j] >> 25;
+                const unsigned p0 = px[j] & 65535u, p1 = px[j] >> 16, p2 = py[j] & 65535u, p3 = py[j] >> 16;
+                unsigned e = (unsigned)(H * clo + k0 * nc + mm);
+#pragma unroll
+                for (int t = 0; t < kExpandTB; ++t) {
+                    if (t < nb) {
+                        const double* At = Ab + t * stride;
+                        row0[e] = fma(c3[j], At[p3], fma(c2[j], At[p2], fma(c1[j], At[p1], c0[j] * At[p0])));
+                        if (col0) col0[e] = colb[t] + ap;
+                        e += (unsigned)nc;
+                    }
                 }
             }
-            __syncwarp();
+            __syncthreads();                                    // the buffer is free for batch b + 2
         }
     }
 }
@@ -459,21 +484,20 @@ cudaError_t launch_op_expand(const DevLattice& L, int cell_begin, int n_blk, con
                              const double* A, const unsigned short* xpos, const double* xc, const int64_t* rowptr, double* vals,
                              int32_t* colidx, int* counter, const int64_t* guard, int n_sm, cudaStream_t st)
 {
-    ExpandSmem S{};
-    int o = 0;
-    auto take = [&](size_t bytes) { int r = o; o += (int)al16(bytes); return r; };
-    S.odesc = take(4 * (size_t)L.totcoup); S.xpos = take(8 * (size_t)L.totcoup); S.xc = take(32 * (size_t)L.totcoup);
-    S.warp_bytes = (int)al16(2 * 8 * (size_t)L.op_stride);
-    const int limit = 227 * 1024;
-    int nw = std::min(16, (limit - o) / std::max(S.warp_bytes, 16));
-    if (nw < 1) return cudaErrorInvalidConfiguration;
-    S.warp0 = take((size_t)S.warp_bytes * nw);
-    S.total = o;
-    cudaError_t e = cudaFuncSetAttribute((const void*)k_op_expand, cudaFuncAttributeMaxDynamicSharedMemorySize, limit);
+    using Fn = void (*)(DevLattice, int, int, const int*, const int64_t*, const int*, const double*, const unsigned short*, const double*,
+                        const int64_t*, double*, int32_t*, int*, const int64_t*);
+    const int need = (L.totcoup + kExpandWarps * 32 - 1) / (kExpandWarps * 32);       // outputs per thread
+    Fn fn = need <= 2 ? k_op_expand<2> : need <= 4 ? k_op_expand<4> : need <= 6 ? k_op_expand<6> : need <= 8 ? k_op_expand<8> : nullptr;
+    if (!fn) return cudaErrorInvalidConfiguration;
+    const size_t smem = 2 * (size_t)kExpandTB * (size_t)L.op_stride * 8 + 2 * kExpandTB * sizeof(int);
+    if (smem > 200 * 1024) return cudaErrorInvalidConfiguration;
+    cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(counter, 0, sizeof(int), st)) != cudaSuccess) return e;
-    const int grid = std::max(1, std::min(n_sm, (n_blk + nw - 1) / nw));
-    k_op_expand<<<grid, nw * 32, S.total, st>>>(L, S, cell_begin, n_blk, nl.hits, cellbase, hitlist, A, xpos, xc, rowptr, vals, colidx, counter, guard);
+    int per_sm = 1;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, kExpandWarps * 32, smem)) != cudaSuccess) return e;
+    const int grid = std::max(1, std::min(n_sm * std::max(per_sm, 1), n_blk));
+    fn<<<grid, kExpandWarps * 32, smem, st>>>(L, cell_begin, n_blk, nl.hits, cellbase, hitlist, A, xpos, xc, rowptr, vals, colidx, counter, guard);
     count_launch();
     return cudaGetLastError();
 }
