@@ -431,6 +431,34 @@ def main():
     rot_ms = best_of(lambda: api.pm_rotate_apply(lat.h, rowptr, None, vals, dO, du, yv, work))
     rotation = {"ms": rot_ms, "bound": "hbm", "achieved": 8.0 * nnz / (rot_ms * 1e-3) * 1e-9, "peak": pk["hbm_gbs"], "unit": "GB/s",
                 "frac": 8.0 * nnz / (rot_ms * 1e-3) * 1e-9 / pk["hbm_gbs"], "what": "P x = O P0 O^T x (eq. 20), same synthetic O"}
+    # ---- the operator form of P0 (per-pair sums): build, apply, and the iteration step through it
+    operator = None
+    try:
+        e0, e1 = (torch.cuda.Event(enable_timing=True) for _ in range(2))
+        api.pm_operator_build(lat.h)                                     # untimed: run-time compilation of the sums kernel
+        flush.zero_()
+        e0.record(st)
+        pairs, op_bytes = api.pm_operator_build(lat.h)
+        e1.record(st); torch.cuda.synchronize()
+        op_build_ms = e0.elapsed_time(e1)
+        op_ms = best_of(lambda: api.pm_operator_apply(lat.h, xv, yv))
+        ref = torch.empty_like(yv)
+        api.pm_spmv(lat.h, rowptr, colidx, vals, xv, ref)
+        api.pm_operator_apply(lat.h, xv, yv)
+        op_err = float((yv - ref).abs().max() / ref.abs().max())
+        w1, w2 = work[: wl.M], work[wl.M:]
+
+        def op_iteration():                                             # K u = O (P0 (V~1 (G1 u))), P0 applied from the sums
+            api.pm_block_apply(lat.h, dVt, dg, du, w1)
+            api.pm_operator_apply(lat.h, w1, w2)
+            api.pm_block_apply(lat.h, dO, None, w2, yv)
+        op_it_ms = best_of(op_iteration)
+        operator = {"pairs": pairs, "bytes": op_bytes, "csr_value_bytes": 8 * nnz, "build_ms": op_build_ms, "apply_ms": op_ms,
+                    "apply_gbs": op_bytes / (op_ms * 1e-3) * 1e-9, "apply_frac_of_hbm": op_bytes / (op_ms * 1e-3) * 1e-9 / pk["hbm_gbs"],
+                    "iteration_ms": op_it_ms, "max_rel_diff_vs_spmv": op_err,
+                    "what": "per-pair sums of the orbital functions (pm_operator_build) and y = P0 x straight from them (pm_operator_apply)"}
+    except Exception as ex:                                              # (needs NVRTC on the box)
+        operator = {"error": repr(ex)}
     del xv, yv, work
 
     # ---- the five lattices (north_star): device-timed pm_build of each, same timing rules
@@ -512,7 +540,7 @@ def main():
                         "pattern_median": float(np.median(np.array(step_ms) - np.array(fill_ms))),
                         "fill_median": float(np.median(fill_ms)), "fill_best": float(np.min(fill_ms)),
                         "fill_all": [round(float(x), 3) for x in fill_ms]},
-           "roofline": roof, "spmv": spmv, "iteration": iteration, "rotation": rotation, "lattices": lattices, "sweep": sweep,
+           "roofline": roof, "spmv": spmv, "iteration": iteration, "rotation": rotation, "operator": operator, "lattices": lattices, "sweep": sweep,
            "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks.summary()}
     print(json.dumps(out))
     lat.close()

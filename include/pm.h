@@ -154,6 +154,21 @@ int32_t pm_spmv_implicit(pm_lattice* lat, const int64_t* d_rowptr, const double*
  * events recorded around it on its stream; waits for that kernel.  PM_ERR_STATE before the first fill. */
 int32_t pm_last_fill_ms(pm_lattice* lat, float* ms);
 
+/* ---- The operator form of P0: the per-pair sums -----------------------------------------------
+ * Every nonzero of a hit cell pair (source cell, k-th hit cell) is a combination, with the recoupling coefficients c^L of
+ * eq. (22), of at most four of the pair's sums over quadrature nodes of the orbital functions (140 for 26 channels, 546
+ * for 62): 8 * n_functions bytes per pair instead of 8 bytes per nonzero (580 / 3694 per pair) — 1.7 GB instead of 7.1 GB
+ * on configs[4].  What the paper's iterations need of P0 is its action on a vector.
+ *   pm_operator_build : the sums of the WHOLE lattice into library-owned device memory, from the node lists of the last
+ *                       pm_pattern / pm_build call over [0, n_cells) (PM_ERR_STATE otherwise; PM_ERR_STATE too when NVRTC
+ *                       is unavailable: the sums are written by run-time specialised kernels).  *n_pairs, *bytes (host,
+ *                       may be NULL): hit cell pairs and the size of the sums.  Synchronises the stream once.
+ *   pm_operator_apply : d_y = P0 d_x (M doubles each, distinct buffers) straight from the sums; asynchronous; agrees with
+ *                       pm_spmv on the CSR to rounding (another summation order), bitwise reproducible.
+ * A new pattern pass or pm_lattice_set_normalisation invalidates the sums (PM_ERR_STATE from pm_operator_apply). */
+int32_t pm_operator_build(pm_lattice* lat, int64_t* n_pairs, int64_t* bytes, void* cuda_stream);
+int32_t pm_operator_apply(pm_lattice* lat, const double* d_x, double* d_y, void* cuda_stream);
+
 /* y = A x for a CSR block (convenience check only): n_rows rows, GLOBAL columns. */
 int32_t pm_spmv(pm_lattice* lat, int64_t n_rows, const int64_t* d_rowptr, const int32_t* d_colidx,
                 const double* d_vals, const double* d_x, double* d_y, void* cuda_stream);

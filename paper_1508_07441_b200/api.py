@@ -26,7 +26,7 @@ EXPORTS = ["pm_lattice_create", "pm_lattice_destroy", "pm_lattice_dims", "pm_lat
            "pm_diag_dfma_tflops", "pm_pattern", "pm_fill", "pm_build", "pm_last_fill_ms", "pm_block_apply", "pm_kernel_apply", "pm_spmv_implicit", "pm_spmv", "pm_build_host_count", "pm_build_host",
            "pm_launch_count", "pm_last_error", "pm_lattice_attach", "pm_build_async", "pm_build_wait", "pm_build_reuse",
            "pm_pattern_cell_hits", "pm_partition_cells", "pm_rowptr_offset", "pm_block_apply_t", "pm_rotate_apply",
-           "pm_lattice_set_normalisation"]
+           "pm_lattice_set_normalisation", "pm_operator_build", "pm_operator_apply"]
 
 
 class PmError(RuntimeError):
@@ -58,6 +58,8 @@ def lib():
                                     C.POINTER(_vp)]
     L.pm_lattice_destroy.argtypes = [_vp]
     L.pm_lattice_set_normalisation.argtypes = [_vp, C.c_int32]
+    L.pm_operator_build.argtypes = [_vp, _i64p, _i64p, _vp]
+    L.pm_operator_apply.argtypes = [_vp, _vp, _vp, _vp]
     L.pm_lattice_attach.argtypes = [_vp, C.POINTER(_Channel), C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.POINTER(_vp)]
     L.pm_build_async.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, _vp, C.c_int64, C.c_int32, _vp]
     L.pm_build_wait.argtypes = [_vp, _i64p]
@@ -287,6 +289,18 @@ def pm_rotate_apply(h, d_rowptr, d_colidx, d_vals, d_O, d_x, d_out, d_work, stre
 def pm_spmv_implicit(h, d_rowptr, d_vals, d_x, d_y, stream=None):
     """y = P0 x with the columns implied by the lattice's hit lists (whole lattice, after pm_pattern / pm_build)."""
     _check(lib().pm_spmv_implicit(h, d_rowptr.data_ptr(), d_vals.data_ptr(), d_x.data_ptr(), d_y.data_ptr(), _stream_ptr(stream)))
+
+
+def pm_operator_build(h, stream=None):
+    """Per-pair sums (operator form of P0) of the whole lattice; returns (hit cell pairs, bytes of the sums)."""
+    a, b = C.c_int64(), C.c_int64()
+    _check(lib().pm_operator_build(h, C.byref(a), C.byref(b), _stream_ptr(stream)))
+    return a.value, b.value
+
+
+def pm_operator_apply(h, d_x, d_y, stream=None):
+    """y = P0 x straight from the per-pair sums of pm_operator_build."""
+    _check(lib().pm_operator_apply(h, d_x.data_ptr(), d_y.data_ptr(), _stream_ptr(stream)))
 
 
 def pm_block_apply(h, d_blocks, d_diag, d_in, d_out, stream=None):

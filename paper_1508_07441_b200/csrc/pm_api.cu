@@ -74,6 +74,7 @@ struct pm_geometry {
     bool lists_valid = false;          // nl holds the lists of [pat_begin, pat_end)
     bool pat_count_only = false;       // the last pattern call only counted: an emit call of the same range reuses its lists
     int pat_begin = -1, pat_end = -1;
+    uint64_t pattern_serial = 0;       // counts the pattern passes (pm_operator_apply checks its sums against it)
     int totcoup_of_scan = 0;           // the channel-pair count the last scan multiplied the hit counts with
     int hmax = -1;
     int64_t nnz = 0, nodes_on_grid = 0, hit_cells = 0, segments = -1, overflow = 0, chunks = 0;
@@ -107,6 +108,8 @@ struct pm_lattice {
     const double* d_xc = nullptr;              // [totcoup][4] coefficients
     double* d_opA = nullptr;           // the sums of the last fill, library-owned scratch
     int64_t opA_cap = 0;
+    uint64_t op_serial = 0;            // pattern pass the sums of pm_operator_build belong to (0: none)
+    int op_norm = 0;
     cudaEvent_t ev_fill0 = nullptr, ev_fill1 = nullptr;   // around the last fill kernel, on its stream (pm_last_fill_ms)
     bool fill_timed = false;
     unsigned long long hash = 0;       // pm::tables_hash of T (selects a generated fill kernel)
@@ -280,7 +283,7 @@ int32_t ensure_device(pm_lattice* L)
     // per-pair sums layout of jgroups and the whole set's outputs in terms of it (k_op_expand)
     size_t o_xpos = 0, o_xc = 0;
     L->op_off.clear(); L->op_stride = 0;
-    if (L->jgroups.size() > 1) {
+    if (!L->jgroups.empty()) {
         std::vector<int> pos(T.fun.size(), 0);
         for (const pm::GroupTables& Gt : L->jgroups) {
             L->op_off.push_back(L->op_stride);
@@ -289,7 +292,7 @@ int32_t ensure_device(pm_lattice* L)
         }
         std::vector<uint16_t> xpos(4 * (size_t)T.totcoup, 0);
         std::vector<double> xc(4 * (size_t)T.totcoup, 0.0);
-        bool ok = L->op_stride < 65536;
+        bool ok = L->op_stride < 8192;                 // (k_op_apply packs byte offsets into 16 bits)
         for (int o = 0; o < T.totcoup && ok; ++o) {
             const int t0 = T.ot_off[(size_t)o], nt = T.ot_off[(size_t)o + 1] - t0;
             if (nt > 4) { ok = false; break; }
@@ -674,6 +677,7 @@ int32_t pattern_async(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, int
     if ((e = cudaEventRecord(G->ev_summary, st)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
     G->summary_pending = true;
     G->lists_valid = true; G->pat_begin = cell_begin; G->pat_end = cell_end; G->pat_count_only = count_only;
+    ++G->pattern_serial;
     return PM_OK;
 }
 
@@ -697,6 +701,43 @@ int32_t ensure_hitlist(pm_lattice* lat, cudaStream_t st)
     return PM_OK;
 }
 
+// The per-pair sums of the cells [cell_begin, cell_begin + n_blk) of the last pattern call into lat->d_opA: every group of
+// jgroups through its run-time specialised kernel in mode 2 (compiled on first use).
+int32_t fill_sums(pm_lattice* lat, int32_t cell_begin, int n_blk, const int64_t* guard, cudaStream_t st)
+{
+    pm_geometry* G = lat->G;
+    if (lat->gdev_j.empty() || lat->op_stride <= 0) return fail(PM_ERR_STATE, "this channel set has no per-pair sums form");
+    bool ready = true;
+    for (auto& gd : lat->gdev_j) ready = ready && gd.plan.fn_op != nullptr;
+    if (!ready) {
+        if (!pm::jit_enabled() || lat->jit_failed) return fail(PM_ERR_STATE, "the per-pair sums need run-time compilation (NVRTC): " + lat->jit_error);
+        std::vector<pm::DevLattice> devs;
+        std::vector<pm::KetView> views;
+        for (size_t g = 0; g < lat->gdev_j.size(); ++g) { devs.push_back(lat->gdev_j[g].dev); views.push_back(pm::ket_view(lat->jgroups[g], lat->T.n_slot, true)); }
+        std::vector<pm::FillLaunch> plans;
+        for (auto& gd : lat->gdev_j) plans.push_back(gd.plan);
+        if (!pm::fill_plan_jit(devs, views, G->n_sm, 2, plans, lat->jit_error)) { lat->jit_failed = true; return fail(PM_ERR_STATE, "run-time compilation failed: " + lat->jit_error); }
+        for (size_t g = 0; g < plans.size(); ++g) lat->gdev_j[g].plan = plans[g];
+    }
+    int32_t rc = ensure_hitlist(lat, st);               // (waits for the pattern pass: the number of hit cell pairs sizes the sums)
+    if (rc) return rc;
+    if (G->overflow) return PM_OK;                      // (the caller reports it)
+    cudaError_t e;
+    const int64_t need = std::max<int64_t>(G->hit_cells, 1) * lat->op_stride;
+    if (need > lat->opA_cap) {
+        if (lat->d_opA) cudaFree(lat->d_opA);
+        lat->d_opA = nullptr; lat->opA_cap = 0;
+        if ((e = cudaMalloc(&lat->d_opA, sizeof(double) * (size_t)need)) != cudaSuccess) { cudaGetLastError(); return fail(PM_ERR_NOMEM, "out of device memory for the per-pair sums of this channel set"); }
+        lat->opA_cap = need;
+    }
+    for (auto& gd : lat->gdev_j) {
+        e = pm::launch_fill(gd.dev, gd.plan, cell_begin, n_blk, G->nl, G->d_cellbase, lat->d_opA, nullptr, G->d_counter, guard, st, true);
+        if (e != cudaSuccess) return cuda_fail(e, "k_fill (per-pair sums)");
+    }
+    lat->op_serial = 0;                                 // (pm_operator_build stamps it)
+    return PM_OK;
+}
+
 // values (and, when d_colidx is given, column indices) of the block of the last pattern call; `guard` (device) stops the
 // kernel when the scan found nnz above the caller's capacity
 int32_t fill_block(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const int64_t* d_rowptr, double* d_vals,
@@ -712,10 +753,11 @@ int32_t fill_block(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const 
     const bool has_spec = !grouped && pm::fill_has_spec(lat->hash);
     // several specialised groups: each writes the per-pair sums of its functions, one kernel then writes whole CSR rows
     const bool via_sums = lat->gdev_j.size() > 1 && lat->op_stride > 0;
-    const int mode = via_sums ? 2 : (d_colidx != nullptr ? 1 : 0);
-    auto have_fn = [&](const pm::FillLaunch& F) { return mode == 2 ? F.fn_op != nullptr : mode == 1 ? F.fn_cols != nullptr : F.fn != nullptr; };
-    const bool need_variant = lat->have_plan && lat->use_j && !have_fn(lat->gdev_j[0].plan);
-    if ((!lat->have_plan || need_variant) && !has_spec && !lat->gdev_j.empty() && pm::jit_enabled() && !lat->jit_failed) {
+    const int mode = d_colidx != nullptr ? 1 : 0;
+    auto have_fn = [&](const pm::FillLaunch& F) { return mode == 1 ? F.fn_cols != nullptr : F.fn != nullptr; };
+    const bool need_variant = !via_sums && lat->have_plan && lat->use_j && !have_fn(lat->gdev_j[0].plan);
+    if (via_sums && pm::jit_enabled() && !lat->jit_failed) { lat->have_plan = true; lat->use_j = true; }     // (fill_sums compiles what it needs)
+    if (!via_sums && (!lat->have_plan || need_variant) && !has_spec && !lat->gdev_j.empty() && pm::jit_enabled() && !lat->jit_failed) {
         // no build-time kernel for this channel set: specialise at run time (pm_jit.hpp), one kernel per group of jgroups
         // and only the variant this call launches; else fall back to the table-driven kernel below
         std::vector<pm::DevLattice> devs;
@@ -739,20 +781,9 @@ int32_t fill_block(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const 
     }
     if ((e = cudaEventRecord(lat->ev_fill0, st)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
     if (lat->use_j && via_sums) {
-        int32_t rc = ensure_hitlist(lat, st);           // (waits for the pattern pass: the number of hit cell pairs sizes the sums)
+        int32_t rc = fill_sums(lat, cell_begin, n_blk, guard, st);
         if (rc) return rc;
-        if (G->overflow) return PM_OK;                  // (the caller reports it)
-        const int64_t need = std::max<int64_t>(G->hit_cells, 1) * lat->op_stride;
-        if (need > lat->opA_cap) {
-            if (lat->d_opA) cudaFree(lat->d_opA);
-            lat->d_opA = nullptr; lat->opA_cap = 0;
-            if ((e = cudaMalloc(&lat->d_opA, sizeof(double) * (size_t)need)) != cudaSuccess) { cudaGetLastError(); return fail(PM_ERR_NOMEM, "out of device memory for the per-pair sums of this channel set"); }
-            lat->opA_cap = need;
-        }
-        for (auto& gd : lat->gdev_j) {
-            e = pm::launch_fill(gd.dev, gd.plan, cell_begin, n_blk, G->nl, G->d_cellbase, lat->d_opA, nullptr, G->d_counter, guard, st, true);
-            if (e != cudaSuccess) return cuda_fail(e, "k_fill (per-pair sums)");
-        }
+        if (G->overflow) return PM_OK;
         pm::DevLattice De = lat->dev;
         De.op_stride = lat->op_stride;
         e = pm::launch_op_expand(De, cell_begin, n_blk, G->nl, G->d_cellbase, G->d_hitlist, lat->d_opA, lat->d_xpos, lat->d_xc, d_rowptr, d_vals,
@@ -906,6 +937,39 @@ int32_t pm_spmv_implicit(pm_lattice* lat, const int64_t* d_rowptr, const double*
     if ((rc = ensure_hitlist(lat, st))) return rc;
     cudaError_t e = pm::launch_spmv_implicit(lat->dev, (int64_t)n_cells * lat->n_ch, d_rowptr, G->nl.hits, G->d_cellbase, G->d_hitlist, d_vals, d_x, d_y, st);
     if (e != cudaSuccess) return cuda_fail(e, "k_spmv_implicit");
+    return PM_OK;
+}
+
+int32_t pm_operator_build(pm_lattice* lat, int64_t* n_pairs, int64_t* bytes, void* cuda_stream)
+{
+    if (!lat) return fail(PM_ERR_ARG, "lat is NULL");
+    int32_t rc = ensure_device(lat);
+    if (rc) return rc;
+    pm_geometry* G = lat->G;
+    const int n_cells = G->Np * G->Nq;
+    if (!G->lists_valid || G->pat_begin != 0 || G->pat_end != n_cells)
+        return fail(PM_ERR_STATE, "pm_operator_build needs the node lists of a pm_pattern / pm_build call over the whole lattice");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((rc = fill_sums(lat, 0, n_cells, nullptr, st))) return rc;
+    lat->op_serial = G->pattern_serial; lat->op_norm = lat->norm;
+    if (n_pairs) *n_pairs = G->hit_cells;
+    if (bytes) *bytes = 8 * G->hit_cells * (int64_t)lat->op_stride;
+    return PM_OK;
+}
+
+int32_t pm_operator_apply(pm_lattice* lat, const double* d_x, double* d_y, void* cuda_stream)
+{
+    if (!lat || !d_x || !d_y) return fail(PM_ERR_ARG, "NULL argument");
+    if (d_x == d_y) return fail(PM_ERR_ARG, "pm_operator_apply cannot work in place");
+    pm_geometry* G = lat->G;
+    if (!lat->d_opA || lat->op_serial == 0 || lat->op_serial != G->pattern_serial || lat->op_norm != lat->norm)
+        return fail(PM_ERR_STATE, "pm_operator_apply needs a pm_operator_build after the last pattern pass / change of normalisation");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    pm::DevLattice De = lat->dev;
+    De.op_stride = lat->op_stride;
+    cudaError_t e = pm::launch_op_apply(De, G->Np * G->Nq, G->hmax, G->nl, G->d_cellbase, G->d_hitlist, lat->d_opA, lat->d_xpos, lat->d_xc, d_x, d_y,
+                                        G->d_counter, G->n_sm, st);
+    if (e != cudaSuccess) return cuda_fail(e, "k_op_apply");
     return PM_OK;
 }
 

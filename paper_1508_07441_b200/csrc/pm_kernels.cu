@@ -502,6 +502,142 @@ cudaError_t launch_op_expand(const DevLattice& L, int cell_begin, int n_blk, con
     return cudaGetLastError();
 }
 
+// y = P0 x straight from the per-pair sums (the operator form of P0: 8 * n_functions bytes per hit cell pair instead of
+// 8 bytes per nonzero; PAPER.md:L408-410 — the iterations are what remains the bottleneck once P0 is on the GPU).
+//   y[(cell, alpha)] = sum_k sum_{alpha'} ( sum_i xc[4 o + i] * A[(cellbase + k) * stride + xpos[4 o + i]] ) * x[(cell_k, alpha')]
+// One CTA per source cell; a thread keeps the terms of its kOPL outputs AND their running products with x in registers over
+// all hit cells of the cell, so nothing but the sums (cp.async, double buffered) and the x slices is read and nothing is
+// written until the cell's rows are summed — in a fixed order: bitwise reproducible, no floating-point atomics.
+constexpr int kApplyTB = 8, kApplyStages = 4;       // hit cell pairs per batch; batches in flight
+
+template <int kOPL, int kWarps>
+__global__ void __launch_bounds__(kWarps * 32, (kWarps <= 8 ? 2 : 1))
+k_op_apply(DevLattice L, int n_blk, int hmax, const int* __restrict__ hits, const int64_t* __restrict__ cellbase, const int* __restrict__ hitlist,
+           const double* __restrict__ A, const unsigned short* __restrict__ g_xpos, const double* __restrict__ g_xc,
+           const double* __restrict__ x, double* __restrict__ y, int* __restrict__ counter)
+{
+    extern __shared__ __align__(16) char smem[];
+    constexpr int T = kWarps * 32;
+    const int tid = threadIdx.x;
+    const int nout = L.totcoup, stride = L.op_stride, nch = L.n_ch;
+    const int nchp = (nch + 1) & ~1;                                     // x slices padded to 16 bytes
+    double* s_A = (double*)smem;                                        // [kApplyStages][kApplyTB][stride]
+    double* s_x = s_A + kApplyStages * kApplyTB * stride;               // [kApplyStages][kApplyTB][nchp]
+    double* s_y = s_x + kApplyStages * kApplyTB * nchp;                 // [totcoup] per-output sums of the cell
+    int* s_hit = (int*)(s_y + nout);                                    // [hmax] the cell's hit cells
+    __shared__ int s_cb;
+    int ap[kOPL];                                                       // column channel of the output
+    unsigned px[kOPL], py[kOPL];
+    double c0[kOPL], c1[kOPL], c2[kOPL], c3[kOPL];
+#pragma unroll
+    for (int j = 0; j < kOPL; ++j) {
+        const int o = j * T + tid;
+        ap[j] = 0; px[j] = py[j] = 0u; c0[j] = c1[j] = c2[j] = c3[j] = 0.0;      // (no output: zero coefficients)
+        if (o < nout) {
+            ap[j] = L.cl[o];
+            px[j] = 8u * g_xpos[4 * o] | (8u * g_xpos[4 * o + 1] << 16);         // byte offsets (8 * stride < 65536)
+            py[j] = 8u * g_xpos[4 * o + 2] | (8u * g_xpos[4 * o + 3] << 16);
+            c0[j] = g_xc[4 * o]; c1[j] = g_xc[4 * o + 1]; c2[j] = g_xc[4 * o + 2]; c3[j] = g_xc[4 * o + 3];
+        }
+    }
+    const unsigned sA0 = (unsigned)__cvta_generic_to_shared(s_A), sX0 = (unsigned)__cvta_generic_to_shared(s_x);
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) s_cb = atomicAdd(counter, 1);
+        __syncthreads();
+        const int cb = s_cb;
+        if (cb >= n_blk) break;
+        const int H = min(hits[cb], hmax);
+        const int64_t hbase = cellbase[cb];
+        for (int k = tid; k < H; k += T) s_hit[k] = hitlist[hbase + k];
+        __syncthreads();
+        double acc[kOPL];
+#pragma unroll
+        for (int j = 0; j < kOPL; ++j) acc[j] = 0.0;
+        // batch b of the cell's pairs -> ring slot b % kApplyStages: the pairs' sums (contiguous, 16-byte pieces) and the x
+        // slices of their hit cells (8-byte pieces), all by cp.async
+        auto fetch = [&](int b) {
+            const int k0 = b * kApplyTB, nb = min(kApplyTB, H - k0), slot = b % kApplyStages;
+            if (nb > 0) {
+                const double* src = A + (hbase + k0) * (int64_t)stride;
+                const unsigned dst = sA0 + (unsigned)(slot * kApplyTB * stride * 8);
+                for (int i = tid; i < nb * stride / 2; i += T)
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + 16u * i), "l"(src + 2 * i) : "memory");
+                const unsigned dx = sX0 + (unsigned)(slot * kApplyTB * nchp * 8);
+                for (int i = tid; i < nb * nch; i += T) {
+                    const int t = i / nch, a = i - t * nch;
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dx + 8u * (t * nchp + a)), "l"(x + (int64_t)s_hit[k0 + t] * nch + a) : "memory");
+                }
+            }
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        };
+        const int nbatch = (H + kApplyTB - 1) / kApplyTB;
+#pragma unroll
+        for (int b = 0; b < kApplyStages - 1; ++b) fetch(b);
+        for (int b = 0; b < nbatch; ++b) {
+            fetch(b + kApplyStages - 1);
+            asm volatile("cp.async.wait_group %0;" ::"n"(kApplyStages - 1) : "memory");
+            __syncthreads();
+            const int nb = min(kApplyTB, H - b * kApplyTB), slot = b % kApplyStages;
+            const double* Ab = s_A + slot * kApplyTB * stride;
+            const double* xb = s_x + slot * kApplyTB * nchp;
+            // pair by pair (the pair's base address is the same for all threads), output by output: byte offsets of the four sums
+            // come unpacked from registers, so a term is one add, one shared-memory load and one FMA
+#pragma unroll
+            for (int t = 0; t < kApplyTB; ++t) {
+                if (t < nb) {
+                    const char* At = (const char*)(Ab + t * stride);
+                    const double* xt = xb + t * nchp;
+#pragma unroll
+                    for (int j = 0; j < kOPL; ++j) {
+                        const double v = fma(c3[j], *(const double*)(At + (py[j] >> 16)),
+                                         fma(c2[j], *(const double*)(At + (py[j] & 65535u)),
+                                         fma(c1[j], *(const double*)(At + (px[j] >> 16)), c0[j] * *(const double*)(At + (px[j] & 65535u)))));
+                        acc[j] = fma(v, xt[ap[j]], acc[j]);
+                    }
+                }
+            }
+            __syncthreads();                                            // the slot is free for batch b + kApplyStages
+        }
+#pragma unroll
+        for (int j = 0; j < kOPL; ++j) { const int o = j * T + tid; if (o < nout) s_y[o] = acc[j]; }
+        __syncthreads();
+        if (tid < nch) {                                                // row alpha = the outputs cl_off[alpha] .. cl_off[alpha + 1], in order
+            double r = 0.0;
+            for (int o = L.cl_off[tid]; o < L.cl_off[tid + 1]; ++o) r += s_y[o];
+            y[(int64_t)cb * nch + tid] = r;
+        }
+    }
+}
+
+cudaError_t launch_op_apply(const DevLattice& L, int n_blk, int hmax, const NodeLists& nl, const int64_t* cellbase, const int* hitlist, const double* A,
+                            const unsigned short* xpos, const double* xc, const double* x, double* y, int* counter, int n_sm, cudaStream_t st)
+{
+    using Fn = void (*)(DevLattice, int, int, const int*, const int64_t*, const int*, const double*, const unsigned short*, const double*,
+                        const double*, double*, int*);
+    Fn fn = nullptr;
+    int warps = 8;
+    const int n = L.totcoup;
+    if (n <= 256) fn = k_op_apply<1, 8>;
+    else if (n <= 512) fn = k_op_apply<2, 8>;
+    else if (n <= 768) fn = k_op_apply<3, 8>;
+    else if (n <= 1024) fn = k_op_apply<4, 8>;
+    else { warps = 16; fn = n <= 2048 ? k_op_apply<4, 16> : n <= 3072 ? k_op_apply<6, 16> : n <= 4096 ? k_op_apply<8, 16> : nullptr; }
+    if (!fn) return cudaErrorInvalidConfiguration;
+    const size_t nchp = ((size_t)L.n_ch + 1) & ~(size_t)1;
+    const size_t smem = 8 * ((size_t)kApplyStages * kApplyTB * ((size_t)L.op_stride + nchp) + (size_t)L.totcoup) + 4 * (size_t)std::max(hmax, 1);
+    if (smem > 200 * 1024) return cudaErrorInvalidConfiguration;
+    cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(counter, 0, sizeof(int), st)) != cudaSuccess) return e;
+    int per_sm = 1;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, warps * 32, smem)) != cudaSuccess) return e;
+    const int grid = std::max(1, std::min(n_sm * std::max(per_sm, 1), n_blk));
+    fn<<<grid, warps * 32, smem, st>>>(L, n_blk, hmax, nl.hits, cellbase, hitlist, A, xpos, xc, x, y, counter);
+    count_launch();
+    return cudaGetLastError();
+}
+
 // Pattern pass, kernel B: column indices, ascending within each row, from the hit lists.  Thread = output (alpha, m-th
 // coupled alpha'), looping over the hit cells k: entry k of row alpha sits at row_start + k*nc + m, so the threads
 // of a warp write runs of consecutive m and consecutive k fill the gaps (the same store pattern as the fill's rows).

@@ -50,6 +50,9 @@ cudaError_t launch_fill(const DevLattice& L, const FillLaunch& F, int cell_begin
 cudaError_t launch_op_expand(const DevLattice& L, int cell_begin, int n_blk, const NodeLists& nl, const int64_t* cellbase, const int* hitlist,
                              const double* A, const unsigned short* xpos, const double* xc, const int64_t* rowptr, double* vals,
                              int32_t* colidx, int* counter, const int64_t* guard, int n_sm, cudaStream_t st);
+// y = P0 x from the per-pair sums A of the whole lattice (pm_kernels.cu)
+cudaError_t launch_op_apply(const DevLattice& L, int n_blk, int hmax, const NodeLists& nl, const int64_t* cellbase, const int* hitlist, const double* A,
+                            const unsigned short* xpos, const double* xc, const double* x, double* y, int* counter, int n_sm, cudaStream_t st);
 cudaError_t launch_hit_list(const DevLattice& L, int n_blk, const NodeLists& nl, const int64_t* cellbase, int* hitlist, cudaStream_t st);
 cudaError_t launch_spmv_implicit(const DevLattice& L, int64_t n_rows, const int64_t* rowptr, const int* hits, const int64_t* cellbase,
                                  const int* hitlist, const double* vals, const double* x, double* y, cudaStream_t st);

@@ -540,3 +540,46 @@ def test_reading_B_normalisation(api, oracle, wl):
     with pytest.raises(api.PmError):
         api.pm_lattice_set_normalisation(lat.h, 7)
     lat.close()
+
+
+@pytest.mark.parametrize("wl", [I.config(1), I.small_coupled(N=6, jmax=3, orders=(3, 4, 6), Nq=9),
+                                I.boson_lattice(9, 5, waves=((0, 0), (2, 2)), orders=(4, 3, 6), cp=0.7, cq=1.3),
+                                I.small_coupled(N=4, jmax=3, orders=(3, 2, 5), Nq=5, J2=3, parity=-1),
+                                I.small_coupled(N=4, jmax=3, orders=(3, 2, 5), Nq=5, J2=17, parity=+1)], ids=lambda w: w.name)
+def test_operator_form_applies_P0(api, oracle, wl):
+    """The per-pair sums (operator form of P0): pm_operator_apply against y = P0 x with the ORACLE's
+    CSR (scipy), for one kernel per set (2, 26 channels, bosons) and for sets built group by group (46 and 62 channels),
+    both normalisations; bitwise reproducible; stale sums are refused (PM_ERR_STATE)."""
+    import scipy.sparse as sp
+    import torch
+    lat = api.Lattice(wl)
+    x = np.random.default_rng(77).uniform(-1, 1, wl.M)
+    dx = torch.from_numpy(x).cuda()
+    y = torch.empty(wl.M, dtype=torch.float64, device="cuda")
+    with pytest.raises(api.PmError) as e:
+        api.pm_operator_build(lat.h)                                    # no node lists yet
+    assert e.value.code == -7
+    lat.build_fused()
+    with pytest.raises(api.PmError) as e:
+        api.pm_operator_apply(lat.h, dx, y)                             # no sums yet
+    assert e.value.code == -7
+    for norm in (0, 1):
+        api.pm_lattice_set_normalisation(lat.h, norm)
+        if norm:
+            with pytest.raises(api.PmError):
+                api.pm_operator_apply(lat.h, dx, y)                     # the sums belong to the other normalisation
+        pairs, nbytes = api.pm_operator_build(lat.h)
+        rpo, cio, vo = oracle.build_csr(wl, norm=norm)
+        assert pairs * int(api.pm_lattice_coupling(lat.h, wl.n_ch)[0].sum()) == len(vo) and nbytes >= 8 * pairs
+        ref = sp.csr_matrix((vo, cio, rpo), shape=(wl.M, wl.M)) @ x
+        api.pm_operator_apply(lat.h, dx, y)
+        assert np.max(np.abs(y.cpu().numpy() - ref)) <= 1e-11 * np.max(np.abs(ref))
+        y2 = torch.empty_like(y)
+        api.pm_operator_apply(lat.h, dx, y2)
+        assert torch.equal(y, y2)
+    api.pm_lattice_set_normalisation(lat.h, 0)
+    lat.build_fused()                                                   # a new pattern pass: the sums are stale
+    with pytest.raises(api.PmError) as e:
+        api.pm_operator_apply(lat.h, dx, y)
+    assert e.value.code == -7
+    lat.close()
