@@ -583,3 +583,31 @@ def test_operator_form_applies_P0(api, oracle, wl):
         api.pm_operator_apply(lat.h, dx, y)
     assert e.value.code == -7
     lat.close()
+
+
+def test_grouped_set_in_blocks_and_streamed(api, oracle):
+    """A channel set filled group by group through the per-pair sums (46 channels, J = 3/2-): block ranges of source cells
+    (pm_pattern + pm_fill without columns, pm_build with columns) and the streaming build with several blocks, all against
+    the oracle and bit-identical to the whole build."""
+    wl = I.small_coupled(N=5, jmax=3, orders=(3, 2, 5), Nq=6, J2=3, parity=-1)
+    lat = api.Lattice(wl)
+    rpo, cio, vo = oracle.build_csr(wl)
+    rp, ci, v = lat.build_fused()
+    assert api.pm_lattice_fill_kernel(lat.h) == "jit-grouped"
+    assert np.array_equal(rp.cpu().numpy(), rpo) and np.array_equal(ci.cpu().numpy(), cio)
+    _assert_values(v.cpu().numpy(), vo)
+    whole = v.cpu().numpy()
+    n = wl.n_cells
+    for cb, ce in ((0, 7), (7, n), (n // 2, n // 2 + 1)):
+        for build in (lat.build, lat.build_fused):
+            rpb, cib, vb = build(cb, ce)
+            rb, cb_, vb_ = oracle.build_csr(wl, cb, ce)
+            assert np.array_equal(rpb.cpu().numpy(), rb) and np.array_equal(cib.cpu().numpy(), cb_)
+            lo = int(rpo[cb * wl.n_ch])
+            assert np.array_equal(vb.cpu().numpy(), whole[lo:lo + len(vb_)])
+    for blocks in (1, 4):
+        budget = (1 << 40) if blocks == 1 else int((12 * len(vo) + 12 * wl.nodes_per_cell * wl.n_cells) / blocks) + 1
+        h_rp, h_ci, h_v, nnz, nb = lat.build_host(budget)
+        assert nnz == len(vo) and nb >= blocks
+        assert np.array_equal(h_rp.numpy(), rpo) and np.array_equal(h_ci.numpy(), cio) and np.array_equal(h_v.numpy(), whole)
+    lat.close()
