@@ -292,7 +292,7 @@ int32_t ensure_device(pm_lattice* L)
         }
         std::vector<uint16_t> xpos(4 * (size_t)T.totcoup, 0);
         std::vector<double> xc(4 * (size_t)T.totcoup, 0.0);
-        bool ok = L->op_stride < 8192;                 // (k_op_apply packs byte offsets into 16 bits)
+        bool ok = L->op_stride <= 2048;                // (k_op_apply packs byte offsets into 16 bits; k_op_expand keeps 8 pairs' sums in shared memory)
         for (int o = 0; o < T.totcoup && ok; ++o) {
             const int t0 = T.ot_off[(size_t)o], nt = T.ot_off[(size_t)o + 1] - t0;
             if (nt > 4) { ok = false; break; }
@@ -701,24 +701,31 @@ int32_t ensure_hitlist(pm_lattice* lat, cudaStream_t st)
     return PM_OK;
 }
 
+// run-time specialised kernels (mode 2: per-pair sums) for every group of jgroups; false when NVRTC is off, missing or fails
+bool ensure_sums_plans(pm_lattice* lat)
+{
+    if (lat->gdev_j.empty() || lat->op_stride <= 0) return false;
+    bool ready = true;
+    for (auto& gd : lat->gdev_j) ready = ready && gd.plan.fn_op != nullptr;
+    if (ready) return true;
+    if (!pm::jit_enabled() || lat->jit_failed) { if (lat->jit_error.empty()) lat->jit_error = "run-time compilation is switched off"; return false; }
+    std::vector<pm::DevLattice> devs;
+    std::vector<pm::KetView> views;
+    for (size_t g = 0; g < lat->gdev_j.size(); ++g) { devs.push_back(lat->gdev_j[g].dev); views.push_back(pm::ket_view(lat->jgroups[g], lat->T.n_slot, true)); }
+    std::vector<pm::FillLaunch> plans;
+    for (auto& gd : lat->gdev_j) plans.push_back(gd.plan);
+    if (!pm::fill_plan_jit(devs, views, lat->G->n_sm, 2, plans, lat->jit_error)) { lat->jit_failed = true; return false; }
+    for (size_t g = 0; g < plans.size(); ++g) lat->gdev_j[g].plan = plans[g];
+    return true;
+}
+
 // The per-pair sums of the cells [cell_begin, cell_begin + n_blk) of the last pattern call into lat->d_opA: every group of
 // jgroups through its run-time specialised kernel in mode 2 (compiled on first use).
 int32_t fill_sums(pm_lattice* lat, int32_t cell_begin, int n_blk, const int64_t* guard, cudaStream_t st)
 {
     pm_geometry* G = lat->G;
     if (lat->gdev_j.empty() || lat->op_stride <= 0) return fail(PM_ERR_STATE, "this channel set has no per-pair sums form");
-    bool ready = true;
-    for (auto& gd : lat->gdev_j) ready = ready && gd.plan.fn_op != nullptr;
-    if (!ready) {
-        if (!pm::jit_enabled() || lat->jit_failed) return fail(PM_ERR_STATE, "the per-pair sums need run-time compilation (NVRTC): " + lat->jit_error);
-        std::vector<pm::DevLattice> devs;
-        std::vector<pm::KetView> views;
-        for (size_t g = 0; g < lat->gdev_j.size(); ++g) { devs.push_back(lat->gdev_j[g].dev); views.push_back(pm::ket_view(lat->jgroups[g], lat->T.n_slot, true)); }
-        std::vector<pm::FillLaunch> plans;
-        for (auto& gd : lat->gdev_j) plans.push_back(gd.plan);
-        if (!pm::fill_plan_jit(devs, views, G->n_sm, 2, plans, lat->jit_error)) { lat->jit_failed = true; return fail(PM_ERR_STATE, "run-time compilation failed: " + lat->jit_error); }
-        for (size_t g = 0; g < plans.size(); ++g) lat->gdev_j[g].plan = plans[g];
-    }
+    if (!ensure_sums_plans(lat)) return fail(PM_ERR_STATE, "the per-pair sums need run-time compilation (NVRTC): " + lat->jit_error);
     int32_t rc = ensure_hitlist(lat, st);               // (waits for the pattern pass: the number of hit cell pairs sizes the sums)
     if (rc) return rc;
     if (G->overflow) return PM_OK;                      // (the caller reports it)
@@ -752,11 +759,12 @@ int32_t fill_block(pm_lattice* lat, int32_t cell_begin, int32_t cell_end, const 
     const bool grouped = lat->gdev.size() > 1;         // big channel sets: one launch per column-channel group
     const bool has_spec = !grouped && pm::fill_has_spec(lat->hash);
     // several specialised groups: each writes the per-pair sums of its functions, one kernel then writes whole CSR rows
-    const bool via_sums = lat->gdev_j.size() > 1 && lat->op_stride > 0;
+    const bool via_sums = lat->gdev_j.size() > 1 && lat->op_stride > 0 && ensure_sums_plans(lat);       // (else the table-driven groups below)
     const int mode = d_colidx != nullptr ? 1 : 0;
     auto have_fn = [&](const pm::FillLaunch& F) { return mode == 1 ? F.fn_cols != nullptr : F.fn != nullptr; };
     const bool need_variant = !via_sums && lat->have_plan && lat->use_j && !have_fn(lat->gdev_j[0].plan);
-    if (via_sums && pm::jit_enabled() && !lat->jit_failed) { lat->have_plan = true; lat->use_j = true; }     // (fill_sums compiles what it needs)
+    if (via_sums) { lat->have_plan = true; lat->use_j = true; }
+    else if (lat->use_j && lat->gdev_j.size() > 1) { lat->have_plan = false; lat->use_j = false; }              // (run-time compilation went away)
     if (!via_sums && (!lat->have_plan || need_variant) && !has_spec && !lat->gdev_j.empty() && pm::jit_enabled() && !lat->jit_failed) {
         // no build-time kernel for this channel set: specialise at run time (pm_jit.hpp), one kernel per group of jgroups
         // and only the variant this call launches; else fall back to the table-driven kernel below
