@@ -876,15 +876,30 @@ __global__ void __launch_bounds__(256) k_block_apply(int Np, int Nq, int n_ch, c
     const int a = blockIdx.x / (ti * tj), rem = blockIdx.x - a * ti * tj, i0 = (rem / tj) * kBlkT, j0 = (rem % tj) * kBlkT;
     const int64_t stride = (int64_t)Nq * n_ch;
     const double* Ba = B + (size_t)a * Np * Np;
+    // staging by cp.async: all of a thread's loads are in flight at once (the strided 8-byte reads of the vector are what the
+    // kernel waits for); out-of-range entries are zeroed with plain stores
+    const unsigned sB0 = (unsigned)__cvta_generic_to_shared(sB), sX0 = (unsigned)__cvta_generic_to_shared(sX);
     for (int k = threadIdx.x; k < kBlkT * Np; k += blockDim.x) {
         const int r = k / Np, c = k - r * Np;
-        sB[r * ld + c] = (i0 + r < Np) ? (transpose ? Ba[(size_t)c * Np + (i0 + r)] : Ba[(size_t)(i0 + r) * Np + c]) : 0.0;   // B_a or its transpose
+        if (i0 + r < Np) {
+            const double* src = transpose ? Ba + (size_t)c * Np + (i0 + r) : Ba + (size_t)(i0 + r) * Np + c;     // B_a or its transpose
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sB0 + 8u * (unsigned)(r * ld + c)), "l"(src) : "memory");
+        } else sB[r * ld + c] = 0.0;
     }
     for (int k = threadIdx.x; k < Np * kBlkT; k += blockDim.x) {
         const int ip = k / kBlkT, jj = k - ip * kBlkT;
-        double x = 0.0;
-        if (j0 + jj < Nq) { const int64_t c = (int64_t)ip * stride + (int64_t)(j0 + jj) * n_ch + a; x = diag ? diag[c] * in[c] : in[c]; }
-        sX[k] = x;
+        if (j0 + jj < Nq) {
+            const int64_t c = (int64_t)ip * stride + (int64_t)(j0 + jj) * n_ch + a;
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sX0 + 8u * (unsigned)k), "l"(in + c) : "memory");
+        } else sX[k] = 0.0;
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    if (diag) {                                                 // the diagonal factor: every thread scales the entries it copied
+        for (int k = threadIdx.x; k < Np * kBlkT; k += blockDim.x) {
+            const int ip = k / kBlkT, jj = k - ip * kBlkT;
+            if (j0 + jj < Nq) sX[k] *= diag[(int64_t)ip * stride + (int64_t)(j0 + jj) * n_ch + a];
+        }
     }
     __syncthreads();
     const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;     // outputs (i0 + ty, +16) x (j0 + tx, +16)
