@@ -227,9 +227,10 @@ k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl,
         // the previous step when the chunk began there).
         __syncwarp();
         int nck = 0;
-        {
+        auto emit_chunks = [&](auto r_tag) {                    // r_tag: the chunk length at compile time (4: every config of BASELINE.json), 0: run time
+            constexpr unsigned kR = decltype(r_tag)::value;
             uint2* g_chunk = nl.chunk + (size_t)cb * L.nnode;
-            const unsigned R = (unsigned)nl.chunk_len, bits = (unsigned)nl.ab_bits;      // R: a power of two, R * bits <= 32
+            const unsigned R = kR ? kR : (unsigned)nl.chunk_len, bits = (unsigned)nl.ab_bits;      // R: a power of two, R * bits <= 32
             const unsigned npq = (unsigned)(L.n_p * L.n_q);
             int seg_start = 0;                                  // first position of the segment that is open at the start of a step
             unsigned carry = 1u;                                // the step's first position starts a segment
@@ -267,7 +268,7 @@ k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl,
 #pragma unroll
                 for (int lv = 0; lv < 4; ++lv) {
                     const unsigned d = 1u << lv;
-                    if (d < R) {
+                    if (kR ? d < kR : d < R) {
                         const unsigned src = (unsigned)(lane - (int)d) & 31u;
                         const unsigned va = __shfl_sync(0xffffffffu, v, src), vb = __shfl_sync(0xffffffffu, prev[lv], src);
                         prev[lv] = v;
@@ -282,7 +283,8 @@ k_map_sort(DevLattice L, MapSortSmem S, int cell_begin, int n_blk, NodeLists nl,
                 carry = smask >> 31;
                 k = kn; kn = knn;
             }
-        }
+        };
+        if (nl.chunk_len == 4) emit_chunks(std::integral_constant<unsigned, 4>{}); else emit_chunks(std::integral_constant<unsigned, 0>{});
         if (lane == 0) { nl.hits[cb] = H; nl.ntot[cb] = placed; nl.nchunk[cb] = nck; }
     }
 }
