@@ -293,10 +293,30 @@ int32_t ensure_device(pm_lattice* L)
         std::vector<uint16_t> xpos(4 * (size_t)T.totcoup, 0);
         std::vector<double> xc(4 * (size_t)T.totcoup, 0.0);
         bool ok = L->op_stride <= 2048;                // (k_op_apply packs byte offsets into 16 bits; k_op_expand keeps 8 pairs' sums in shared memory)
-        for (int o = 0; o < T.totcoup && ok; ++o) {
-            const int t0 = T.ot_off[(size_t)o], nt = T.ot_off[(size_t)o + 1] - t0;
-            if (nt > 4) { ok = false; break; }
-            for (int i = 0; i < nt; ++i) { xpos[4 * (size_t)o + i] = (uint16_t)pos[(size_t)T.ot_f[(size_t)(t0 + i)]]; xc[4 * (size_t)o + i] = T.ot_c[(size_t)(t0 + i)]; }
+        // Term slot i of every output of a row belongs to the row's i-th L value (coefficient 0 where the output has no term
+        // with that L): neighbouring outputs of a row then read, slot by slot, sums of one bra triple and neighbouring ket
+        // triples — neighbouring or equal positions, few shared-memory bank conflicts in k_op_expand / k_op_apply.
+        for (int a = 0; a < L->n_ch && ok; ++a) {
+            std::vector<int> Ls;                        // distinct L of the row's terms, ascending
+            for (int o = T.cl_off[(size_t)a]; o < T.cl_off[(size_t)a + 1]; ++o)
+                for (int t = T.ot_off[(size_t)o]; t < T.ot_off[(size_t)o + 1]; ++t) {
+                    const int Lt = T.fun[(size_t)T.ot_f[(size_t)t]].L;
+                    if (std::find(Ls.begin(), Ls.end(), Lt) == Ls.end()) Ls.push_back(Lt);
+                }
+            std::sort(Ls.begin(), Ls.end());
+            if (Ls.size() > 4) { ok = false; break; }
+            int last_pos[4] = {0, 0, 0, 0};             // an output without the slot's L repeats its neighbour's position
+            for (size_t i = 0; i < Ls.size(); ++i)
+                for (int o = T.cl_off[(size_t)a]; o < T.cl_off[(size_t)a + 1] && last_pos[i] == 0; ++o)
+                    for (int t = T.ot_off[(size_t)o]; t < T.ot_off[(size_t)o + 1]; ++t)
+                        if (T.fun[(size_t)T.ot_f[(size_t)t]].L == Ls[i]) { last_pos[i] = pos[(size_t)T.ot_f[(size_t)t]]; break; }
+            for (int o = T.cl_off[(size_t)a]; o < T.cl_off[(size_t)a + 1]; ++o) {
+                for (size_t i = 0; i < Ls.size(); ++i) {
+                    for (int t = T.ot_off[(size_t)o]; t < T.ot_off[(size_t)o + 1]; ++t)
+                        if (T.fun[(size_t)T.ot_f[(size_t)t]].L == Ls[i]) { last_pos[i] = pos[(size_t)T.ot_f[(size_t)t]]; xc[4 * (size_t)o + i] = T.ot_c[(size_t)t]; }
+                    xpos[4 * (size_t)o + i] = (uint16_t)last_pos[i];
+                }
+            }
         }
         if (ok) { o_xpos = B.put(xpos.data(), 2 * xpos.size()); o_xc = B.put(xc.data(), 8 * xc.size()); }
         else { L->op_stride = 0; L->op_off.clear(); }          // (more than four terms per output: group by group into the CSR)
