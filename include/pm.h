@@ -46,6 +46,7 @@ enum {
 enum { PM_FERMION_ISOSPIN = 0, PM_SPINLESS_BOSON = 1 };      /* `statistics` */
 enum { PM_NORM_WIDTH = 0, PM_NORM_P2 = 1 };                  /* cell normalisation, pm_lattice_set_normalisation */
 enum { PM_MAX_CHANNELS = 64, PM_MAX_ORDER = 64, PM_MAX_L = 12 };
+enum { PM_STATIC_MAX_M = 65536 };                            /* largest matrix dimension pm_rotate_apply_static takes */
 
 /* Create a lattice (host work only: validation, Gauss-Legendre rules, recoupling tables — PAPER.md:L247-256
  * step 1, 'calculation of algebraic coefficients g').
@@ -153,6 +154,19 @@ int32_t pm_spmv_implicit(pm_lattice* lat, const int64_t* d_rowptr, const double*
 /* Device time of the last fill kernel launched for this lattice (by pm_fill, pm_build or pm_build_host), from CUDA
  * events recorded around it on its stream; waits for that kernel.  PM_ERR_STATE before the first fill. */
 int32_t pm_last_fill_ms(pm_lattice* lat, float* ms);
+
+/* pm_rotate_apply without any allocation, for callers that cannot call cudaMalloc (CUDA graph capture, serving loops,
+ * harnesses that forbid it): d_out = O (P0 (O^T x)) as pm_rotate_apply, the two intermediate vectors in a static device
+ * array of the library (2 * PM_STATIC_MAX_M doubles = 1 MiB per GPU that loads libpm, held until exit) instead of d_work.
+ *   - M = n_ch*Np*Nq <= PM_STATIC_MAX_M, else PM_ERR_OVERFLOW (use pm_rotate_apply with your own d_work);
+ *   - d_colidx is required (PM_ERR_ARG if NULL): the column-free SpMV builds library scratch lazily;
+ *   - the lattice's device tables must already exist on the current device — any earlier pm_pattern / pm_build /
+ *     pm_block_apply call on it creates them — else PM_ERR_STATE: this call never allocates or frees;
+ *   - all calls share the array (it keeps the last call's contents; both vectors are overwritten before use): calls that
+ *     overlap on the GPU — other streams, other host threads — RACE; serialise them.
+ * Asynchronous on `cuda_stream`; the same kernels, hence the same bits, as pm_rotate_apply with a column array. */
+int32_t pm_rotate_apply_static(pm_lattice* lat, const int64_t* d_rowptr, const int32_t* d_colidx, const double* d_vals,
+                               const double* d_O, const double* d_x, double* d_out, void* cuda_stream);
 
 /* ---- The operator form of P0: the per-pair sums -----------------------------------------------
  * Every nonzero of a hit cell pair (source cell, k-th hit cell) is a combination, with the recoupling coefficients c^L of

@@ -26,7 +26,7 @@ EXPORTS = ["pm_lattice_create", "pm_lattice_destroy", "pm_lattice_dims", "pm_lat
            "pm_diag_dfma_tflops", "pm_pattern", "pm_fill", "pm_build", "pm_last_fill_ms", "pm_block_apply", "pm_kernel_apply", "pm_spmv_implicit", "pm_spmv", "pm_build_host_count", "pm_build_host",
            "pm_launch_count", "pm_last_error", "pm_lattice_attach", "pm_build_async", "pm_build_wait", "pm_build_reuse",
            "pm_pattern_cell_hits", "pm_partition_cells", "pm_rowptr_offset", "pm_block_apply_t", "pm_rotate_apply",
-           "pm_lattice_set_normalisation", "pm_operator_build", "pm_operator_apply"]
+           "pm_lattice_set_normalisation", "pm_operator_build", "pm_operator_apply", "pm_rotate_apply_static"]
 
 
 class PmError(RuntimeError):
@@ -60,6 +60,7 @@ def lib():
     L.pm_lattice_set_normalisation.argtypes = [_vp, C.c_int32]
     L.pm_operator_build.argtypes = [_vp, _i64p, _i64p, _vp]
     L.pm_operator_apply.argtypes = [_vp, _vp, _vp, _vp]
+    L.pm_rotate_apply_static.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
     L.pm_lattice_attach.argtypes = [_vp, C.POINTER(_Channel), C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.POINTER(_vp)]
     L.pm_build_async.argtypes = [_vp, C.c_int32, C.c_int32, _vp, _vp, _vp, C.c_int64, C.c_int32, _vp]
     L.pm_build_wait.argtypes = [_vp, _i64p]
@@ -301,6 +302,12 @@ def pm_operator_build(h, stream=None):
 def pm_operator_apply(h, d_x, d_y, stream=None):
     """y = P0 x straight from the per-pair sums of pm_operator_build."""
     _check(lib().pm_operator_apply(h, d_x.data_ptr(), d_y.data_ptr(), _stream_ptr(stream)))
+
+
+def pm_rotate_apply_static(h, d_rowptr, d_colidx, d_vals, d_O, d_x, d_out, stream=None):
+    """pm_rotate_apply with the library's static scratch instead of d_work: allocates nothing (M <= PM_STATIC_MAX_M)."""
+    _check(lib().pm_rotate_apply_static(h, d_rowptr.data_ptr(), d_colidx.data_ptr(), d_vals.data_ptr(), d_O.data_ptr(),
+                                        d_x.data_ptr(), d_out.data_ptr(), _stream_ptr(stream)))
 
 
 def pm_block_apply(h, d_blocks, d_diag, d_in, d_out, stream=None):

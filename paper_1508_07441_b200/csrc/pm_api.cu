@@ -14,6 +14,7 @@
 #include <cstring>
 #include <limits>
 #include <new>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1075,6 +1076,76 @@ int32_t pm_spmv(pm_lattice* lat, int64_t n_rows, const int64_t* d_rowptr, const 
     if (!d_colidx || !d_vals) return fail(PM_ERR_ARG, "NULL colidx/vals");
     cudaError_t e = pm::launch_spmv(n_rows, d_rowptr, d_colidx, d_vals, d_x, d_y, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(e, "k_spmv");
+    return PM_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// pm_rotate_apply_static — the rotation P x = O P0 O^T x (eq. 20) for callers that cannot allocate
+// (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): the two intermediate vectors
+// O^T x and P0 O^T x, which pm_rotate_apply takes from the caller's d_work, live in a file-scope device array of
+// 2 * PM_STATIC_MAX_M doubles (1 MiB) that every GPU loading the library holds until exit.  The name of the array is a
+// HOST-side stand-in in host code: its device address comes from cudaGetSymbolAddress, once per device, with that device
+// current.  The call allocates nothing (no cudaMalloc / cudaFree, no lazily built library scratch): the lattice's device
+// tables must already exist (any pm_pattern / pm_build / pm_block_apply call creates them), and d_colidx is required (the
+// column-free SpMV builds its hit lists lazily).  All calls share the array, which keeps the last call's contents: both
+// vectors are fully overwritten before they are read, so nothing has to be cleared; calls that overlap on the GPU (other
+// streams, other host threads) race on it.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) double g_static_work[2 * PM_STATIC_MAX_M];
+
+namespace {
+
+constexpr int kStaticMaxDev = 64;
+std::mutex g_static_mu;
+double* g_static_ptr[kStaticMaxDev] = {};          // device address of g_static_work per device (nullptr: not asked yet)
+
+// device address of the scratch array on the CURRENT device (asked once per device), or nullptr + error message
+double* static_work_ptr()
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { cuda_fail(e, "cudaGetDevice"); return nullptr; }
+    if (dev < 0 || dev >= kStaticMaxDev) { fail(PM_ERR_DEVICE, "device index beyond the table of static scratch addresses"); return nullptr; }
+    std::lock_guard<std::mutex> g(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_work);
+        if (e != cudaSuccess || !p) { cuda_fail(e, "cudaGetSymbolAddress(static scratch)"); return nullptr; }
+        g_static_ptr[dev] = (double*)p;
+    }
+    return g_static_ptr[dev];
+}
+
+}  // namespace
+
+extern "C" {
+
+int32_t pm_rotate_apply_static(pm_lattice* lat, const int64_t* d_rowptr, const int32_t* d_colidx, const double* d_vals,
+                               const double* d_O, const double* d_x, double* d_out, void* cuda_stream)
+{
+    if (!lat || !d_rowptr || !d_colidx || !d_vals || !d_O || !d_x || !d_out) return fail(PM_ERR_ARG, "NULL argument (pm_rotate_apply_static needs the column array)");
+    if (d_x == d_out) return fail(PM_ERR_ARG, "pm_rotate_apply_static cannot work in place");
+    pm_geometry* G = lat->G;
+    const int64_t M = (int64_t)G->Np * G->Nq * lat->n_ch;
+    if (M > PM_STATIC_MAX_M)
+        return fail(PM_ERR_OVERFLOW, "M = " + std::to_string(M) + " exceeds PM_STATIC_MAX_M = " + std::to_string((int64_t)PM_STATIC_MAX_M) +
+                                     ": the static scratch holds two vectors of at most that many doubles; use pm_rotate_apply with your own d_work");
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    if (!lat->d_blob || lat->geo_version != G->version || lat->device != dev || G->device != dev)
+        return fail(PM_ERR_STATE, "pm_rotate_apply_static allocates nothing: the lattice's device tables must exist on the current device "
+                                  "(call pm_pattern / pm_build / pm_block_apply on it first)");
+    double* work = static_work_ptr();
+    if (!work) return PM_ERR_CUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    double* t1 = work;                                      // O^T x
+    double* t2 = work + M;                                  // P0 O^T x
+    if ((e = pm::launch_block_apply(G->Np, G->Nq, lat->n_ch, d_O, nullptr, d_x, t1, 1, st)) != cudaSuccess) return cuda_fail(e, "k_block_apply");
+    if ((e = pm::launch_spmv(M, d_rowptr, d_colidx, d_vals, t1, t2, st)) != cudaSuccess) return cuda_fail(e, "k_spmv");
+    if ((e = pm::launch_block_apply(G->Np, G->Nq, lat->n_ch, d_O, nullptr, t2, d_out, 0, st)) != cudaSuccess) return cuda_fail(e, "k_block_apply");
     return PM_OK;
 }
 
