@@ -336,9 +336,8 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                     const double x = s_tx[c], sx = s_sx[c];
                     const double2 pw = s_p2[a], qw = s_p2[L.n_p + b];
                     const double p = pw.x, q = qw.x;                        // cp + hp t_a, cq + hq t_b: the node of DESIGN.md sec. 3.1
-                    double P2, Q2;
-                    map_pq_sq(p, q, x, P2, Q2);
-                    // omega = w * p q / (p' q'),  w = ((hp wp_a)(hq wq_b)) wx_c
+                    // omega = w * p q / (p' q'),  w = ((hp wp_a)(hq wq_b)) wx_c; |p'| and |q'| are the lengths
+                    // of the rotated vectors below (1/(p'q') = ra * rb: no third reciprocal square root, no second node map)
                     const double w = __dmul_rn(__dmul_rn(pw.y, qw.y), s_wx[c]);
                     // rotated directions from vector components (frame: q^ = z, p^ = (sx, 0, x)):
                     //   p' = -p/2 - 3q/4 ,  q' = p - q/2
@@ -347,7 +346,7 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
                     const double bx = psx, bz = fma(-0.5, q, px);
                     const double ra = rsqrt(fma(ax, ax, az * az)), rb = rsqrt(fma(bx, bx, bz * bz));
                     // (reading B: omega = w * p^2 q^2, no Jacobian of the delta functions)
-                    const double om = L.norm ? w * ((p * q) * (p * q)) : w * (p * q) * rsqrt(P2 * Q2);
+                    const double om = L.norm ? w * ((p * q) * (p * q)) : w * (p * q) * (ra * rb);
                     return NodeIn{valid ? om : 0.0, ax * ra, az * ra, bx * rb, bz * rb};
                 };
                 unsigned abs_ = dC.y;
