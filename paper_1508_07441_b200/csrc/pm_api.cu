@@ -552,9 +552,10 @@ int32_t pm_lattice_work(const pm_lattice* lat, double* flop_per_node, double* fl
 {
     if (!lat) return fail(PM_ERR_ARG, "lat is NULL");
     const pm::Tables& T = lat->T;
-    // per node on the grid (pm_fill.cuh, phase C): node map 16, weight and omega 7 (one rsqrt), rotated directions 20
-    // (two rsqrt), the generated ket code, and one add per slot in the segment sum (phase D)
-    if (flop_per_node) *flop_per_node = 16.0 + 7.0 + 20.0 + pm::ket_flops(T) + (double)T.n_slot;
+    // per node on the grid (pm_fill.cuh, phase C): weight and omega 5 (w = two products, p q, ra rb, two more products),
+    // rotated directions 20 (two rsqrt), the generated ket code, and one add per slot into the chunk sum.  (The node map is
+    // the pattern pass's work: the fill reads the nodes' (a, b, c) from the chunk words.)
+    if (flop_per_node) *flop_per_node = 5.0 + 20.0 + pm::ket_flops(T) + (double)T.n_slot;
     // per (target, x-node) segment: sum_M bra*S per orbital function (nM multiply-adds) and one add into the target sum
     double seg = 0.0;
     for (const pm::OrbFun& f : T.fun) seg += 2.0 * f.nM;
