@@ -85,7 +85,7 @@ __host__ __device__ constexpr WarpLayout warp_layout(int np, int nf, int row_bat
 }
 
 struct FillSmem {           // byte offsets into dynamic shared memory, computed on the host
-    int dp, dq, tx, sx, wx, bra, odesc, ofi, oc, fa, fb, warp0, warp_bytes, total;
+    int dp, dq, tx, sx, wx, bra, odesc, ofi, oc, fa, fb, fc, warp0, warp_bytes, total;
     WarpLayout w;
 };
 
@@ -104,7 +104,7 @@ inline FillSmem fill_smem_plan(const DevLattice& L, int nw, int row_batch, int n
     s.tx = take(8 * L.n_x); s.sx = take(8 * L.n_x); s.wx = take(8 * L.n_x);
     s.bra = bra_in_smem ? take(8 * L.n_x * (L.n_bra + 1)) : -1;      // rows end with one zero slot; -1: read from global memory
     s.odesc = take(4 * L.n_out); s.ofi = take(4 * L.n_out); s.oc = take(8 * n_oterm * L.n_out);
-    s.fa = take(4 * nfun_pad); s.fb = take(4 * nfun_pad);             // (every function chunk of the stage reads its entry)
+    s.fa = take(4 * nfun_pad); s.fb = take(4 * nfun_pad); s.fc = take(4 * nfun_pad);             // (every function chunk of the stage reads its entry)
     const int np = (L.n_slot + 1) / 2;              // slot pairs
     s.w = warp_layout(np, L.n_fun, row_batch);
     const int w = s.w.fixed_bytes + 16 * (L.n_p + L.n_q);
@@ -190,24 +190,27 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
         s_ofi[o] = fi;
     }
     // descriptors of function f (lane = f & 31 in the stage), kept in shared memory (registers are what limits the
-    // warps per SM here).  kPacked (at most 3 M-terms per function): byte i of fa / fb = bra / ket slot of term i,
-    // unused terms point at the zero bra slot; else fa = sa | nM << 16, fb = sb.
+    // warps per SM here).  kPacked (at most 3 M-terms per function): byte i of fa = bra slot of term i, unused terms point
+    // at the zero bra slot; else fa = sa | nM << 16, fb = sb.
     constexpr bool kPacked = Spec::MAXM <= 3;
     int* s_fa = (int*)(smem + S.fa);
     int* s_fb = (int*)(smem + S.fb);
+    int* s_fc = (int*)(smem + S.fc);
+    // (the ket side is read from the K tile, where the walk leaves a segment's sums in the column of the segment's last
+    // chunk: kPacked keeps the byte offset of each term's slot in column 0, 16 bits each, in fb (terms 0, 1) and fc (term 2))
+    auto tile_byte = [](int slot) { return (slot >> 1) * (kTileStride * 16) + (slot & 1) * 8; };
     for (int f = tid; f < NCH * 32; f += T) {
-        int va = kPacked ? (nb_ | (nb_ << 8) | (nb_ << 16)) : 0, vb = 0;
+        int va = kPacked ? (nb_ | (nb_ << 8) | (nb_ << 16)) : 0, vb = 0, vc = 0;
         if (f < nf) {
             const int4 fn = L.fun[f];
             if (kPacked) {
                 va = 0;
-                for (int i = 0; i < 3; ++i) {
-                    va |= (i < fn.z ? fn.x + i : nb_) << (8 * i);
-                    vb |= (i < fn.z ? fn.y + i : 0) << (8 * i);
-                }
+                for (int i = 0; i < 3; ++i) va |= (i < fn.z ? fn.x + i : nb_) << (8 * i);
+                vb = tile_byte(0 < fn.z ? fn.y : 0) | (tile_byte(1 < fn.z ? fn.y + 1 : 0) << 16);
+                vc = tile_byte(2 < fn.z ? fn.y + 2 : 0);
             } else { va = fn.x | (fn.z << 16); vb = fn.y; }
         }
-        s_fa[f] = va; s_fb[f] = vb;
+        s_fa[f] = va; s_fb[f] = vb; s_fc[f] = vc;
     }
     __syncthreads();                                    // the only block-level barrier
 
@@ -372,9 +375,9 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
             const int cnt = min(32, nck - base);
             double runT[NCH];
             double2 runS[NPC];
-            int fa[NCH], fb[NCH];                       // this lane's function descriptors, for the step's segment ends (the ket
+            int fa[NCH], fb[NCH], fc[NCH];              // this lane's function descriptors, for the step's segment ends (the ket
 #pragma unroll                                          // code's accumulators are dead here: registers are free)
-            for (int ch = 0; ch < NCH; ++ch) { fa[ch] = s_fa[ch * 32 + lane]; fb[ch] = s_fb[ch * 32 + lane]; }
+            for (int ch = 0; ch < NCH; ++ch) { fa[ch] = s_fa[ch * 32 + lane]; fb[ch] = s_fb[ch * 32 + lane]; fc[ch] = kPacked ? s_fc[ch * 32 + lane] : 0; }
             {
                 const int slot = kcur - kdone;
 #pragma unroll
@@ -382,70 +385,43 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
 #pragma unroll
                 for (int i = 0; i < NPC; ++i) { const int sp = i * 32 + lane; runS[i] = sp < np ? s_sseg2[sp] : make_double2(0.0, 0.0); }
             }
-            // lane = slot pair: walks the tile's nodes, up to 16 per step, stopping at every segment end (and at the tile end)
-            const unsigned stops = smask | (1u << (cnt - 1));
-            for (int j = 0; j < cnt;) {
-                const int n = min(__ffs(stops >> j), 16);                // nodes up to and including the next stop, at most 16
+            // D1, lane = slot pair: ONE pass over the step's chunk columns (loads in bursts of 16, every branch uniform); at a
+            // segment end the segment's sum replaces the column of its last chunk, where the stage below reads it
 #pragma unroll
-                for (int i = 0; i < NPC; ++i) {
-                    const int sp = i * 32 + lane;
-                    if (sp < np) {
-                        const double2* row = s_tile + sp * kTileStride + j;
-                        double2 r = runS[i];
-                        if (n & 16) {
-                            double2 d[16];
+            for (int i = 0; i < NPC; ++i) {
+                const int sp = i * 32 + lane;
+                if (sp < np) {
+                    double2* row = s_tile + sp * kTileStride;
+                    double2 r = runS[i];
+                    for (int c0 = 0; c0 < cnt; c0 += 16) {
+                        double2 d[16];
 #pragma unroll
-                            for (int k = 0; k < 16; ++k) d[k] = row[k];
+                        for (int k = 0; k < 16; ++k) d[k] = c0 + k < cnt ? row[c0 + k] : make_double2(0.0, 0.0);
 #pragma unroll
-                            for (int w = 8; w > 0; w >>= 1)
-#pragma unroll
-                                for (int k = 0; k < w; ++k) { d[k].x += d[k + w].x; d[k].y += d[k + w].y; }
-                            r.x += d[0].x; r.y += d[0].y;
-                        } else {
-                            if (n & 8) {
-                                const double2 d0 = row[0], d1 = row[1], d2 = row[2], d3 = row[3], d4 = row[4], d5 = row[5], d6 = row[6], d7 = row[7];
-                                r.x += ((d0.x + d1.x) + (d2.x + d3.x)) + ((d4.x + d5.x) + (d6.x + d7.x));
-                                r.y += ((d0.y + d1.y) + (d2.y + d3.y)) + ((d4.y + d5.y) + (d6.y + d7.y));
-                                row += 8;
-                            }
-                            if (n & 4) {
-                                const double2 d0 = row[0], d1 = row[1], d2 = row[2], d3 = row[3];
-                                r.x += (d0.x + d1.x) + (d2.x + d3.x);
-                                r.y += (d0.y + d1.y) + (d2.y + d3.y);
-                                row += 4;
-                            }
-                            if (n & 2) {
-                                const double2 d0 = row[0], d1 = row[1];
-                                r.x += d0.x + d1.x;
-                                r.y += d0.y + d1.y;
-                                row += 2;
-                            }
-                            if (n & 1) { const double2 d = row[0]; r.x += d.x; r.y += d.y; }
+                        for (int k = 0; k < 16; ++k) {
+                            r.x += d[k].x; r.y += d[k].y;
+                            if ((smask >> (c0 + k)) & 1u) { row[c0 + k] = r; r = make_double2(0.0, 0.0); }
                         }
-                        runS[i] = r;
                     }
+                    runS[i] = r;                                         // the segment that is still open behind the step
                 }
-                j += n;
-                if (!((smask >> (j - 1)) & 1u)) continue;
-                const int jb = j - 1;                                    // node jb ends a (t, c) segment
-#pragma unroll
-                for (int i = 0; i < NPC; ++i) {
-                    const int sp = i * 32 + lane;
-                    if (sp < np) s_sseg2[sp] = runS[i];
-                    runS[i] = make_double2(0.0, 0.0);
-                }
-                __syncwarp();
+            }
+            __syncwarp();
+            // D2, lane = orbital function, segment end by segment end
+            for (unsigned rem = smask; rem; rem &= rem - 1u) {
+                const int jb = __ffs(rem) - 1;                           // chunk jb ends a (t, c) segment
                 const int cseg = (int)(s_step[jb].x >> 24);
                 const double* bra;                                     // (shared-memory loads for the specialised kernels)
                 if constexpr (Spec::kStatic) { if (Spec::kBraSmem) bra = s_bra + cseg * nsb; else bra = L.bra + cseg * nsb; }
                 else bra = bra_tab + cseg * bra_stride;
+                const char* Sb = (const char*)(s_tile + jb);             // column jb of the tile: the segment's sums
 #pragma unroll
                 for (int ch = 0; ch < NCH; ++ch) {
                     if (kPacked) {
                         const int ia = fa[ch], ib = fb[ch];
-                        double v = bra[ia & 255] * s_sseg[ib & 255];
-                        if (Spec::terms(ch) > 1) v = fma(bra[(ia >> 8) & 255], s_sseg[(ib >> 8) & 255], v);
-                        if (Spec::terms(ch) > 2) v = fma(bra[ia >> 16], s_sseg[ib >> 16], v);
+                        double v = bra[ia & 255] * *(const double*)(Sb + (ib & 65535));
+                        if (Spec::terms(ch) > 1) v = fma(bra[(ia >> 8) & 255], *(const double*)(Sb + ((unsigned)ib >> 16)), v);
+                        if (Spec::terms(ch) > 2) v = fma(bra[ia >> 16], *(const double*)(Sb + fc[ch]), v);
                         runT[ch] += v;
                     } else {
                         const int fav = fa[ch], sa = fav & 65535, sb = fb[ch], nM = fav >> 16;
@@ -456,14 +432,13 @@ k_fill_warp(DevLattice L, FillSmem S, NodeLists nl, int cell_begin, int n_blk, c
 #pragma unroll
                             for (int i = 0; i < Spec::MAXM; ++i) bv[i] = i < nM ? bra[sa + i] : 0.0;
 #pragma unroll
-                            for (int i = 0; i < Spec::MAXM; ++i) if (i < nM) v = fma(bv[i], s_sseg[sb + i], v);
+                            for (int i = 0; i < Spec::MAXM; ++i) if (i < nM) v = fma(bv[i], *(const double*)(Sb + tile_byte(sb + i)), v);
                         } else {
-                            for (int i = 0; i < nM; ++i) v = fma(bra[sa + i], s_sseg[sb + i], v);
+                            for (int i = 0; i < nM; ++i) v = fma(bra[sa + i], *(const double*)(Sb + tile_byte(sb + i)), v);
                         }
                         runT[ch] += v;
                     }
                 }
-                __syncwarp();
                 if (!((tmask >> jb) & 1u)) continue;
                 // node jb also ends target t: its sums are complete; kRowBatch finished targets are written together
                 {
