@@ -33,7 +33,7 @@ UNIT = "nnz/s"
 FP64_LANES_PER_SM = 64
 # dram__bytes_read.sum + dram__bytes_write.sum of one fill launch, QUOTED from the committed `ncu --set full` capture
 # named beside it (bench.py cannot run under the profiler); None where no capture exists.
-FILL_DRAM_TRAFFIC = {"cfg4_3N_Jhalf+_jle3_26ch_150x150": (10.78e9 + 0.313e9, "profiles/r2_final.md (ncu --set full of this kernel, round 2; quoted, not measured in this run)")}
+FILL_DRAM_TRAFFIC = {"cfg4_3N_Jhalf+_jle3_26ch_150x150": (10.777e9 + 0.318e9, "profiles/r2_final.md (ncu --set full of this kernel, round 2; quoted, not measured in this run)")}
 
 
 def _peaks():
